@@ -1,0 +1,155 @@
+/* hb.h -- C ABI of the B200 Metropolis colour-sweep library (libhb.so).
+ *
+ * What it computes: the single-spin-update Metropolis sweep of the classical
+ * anisotropic Heisenberg model of arXiv 2106.11286,
+ *     H = -J sum_<ij> S_i.S_j - sum_i K_i (S_i.e_i)^2          (eq. 1)
+ * with |S_i| = 1 (line 40), update rule (i)-(iii) of line 20 (propose a uniformly
+ * random orientation, accept if dH <= 0 or P <= exp(-dH/T)), and the
+ * magnetisation M = (1/N) sum_i S_i of eq. 2 (line 22) plus the total energy,
+ * both reduced on the device.  The random site choice of step (i) is replaced
+ * by conflict-free colour-ordered sweeps (reading A3): every site
+ * attempts exactly once per sweep, colour by colour, one CUDA kernel per colour.
+ *
+ * Conventions
+ *  - every function returns HB_OK (0) or a negative hb_status; nothing throws,
+ *    aborts or prints.  hb_strerror() names a status, hb_error_detail() gives
+ *    the last message (CUDA error string included) of a context.
+ *  - "host" pointers are ordinary CPU memory, "device" pointers are CUDA device
+ *    memory of the current device.  The library never frees caller memory.
+ *  - spins are three fp32 planes (x, y, z), as in the paper (line 30: "three
+ *    one-dimensional arrays").  Host-side spin arrays use the CANONICAL site
+ *    order: sc id = (z*Ly + y)*Lx + x; bcc/fcc id = b*Ncell + (z*Ly + y)*Lx + x
+ *    with b the basis index; CSR id = the caller's row index.  The device
+ *    layout is private to the library.
+ *  - a context is not thread-safe; distinct contexts are independent.
+ *  - all work is enqueued on the context's CUDA stream; hb_sweep is
+ *    asynchronous, every call that returns data to the host synchronises.
+ */
+#ifndef HB_H_
+#define HB_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hb_ctx hb_ctx;
+
+typedef enum {
+  HB_OK = 0,
+  HB_EINVAL = -1,  /* bad argument: odd L for sc, T <= 0 or NaN, non-unit axis, asymmetric CSR, improper colouring ... */
+  HB_ENOMEM = -2,  /* host or device allocation failed, or a caller buffer is too small */
+  HB_ECUDA = -3,   /* a CUDA call failed; sticky for the context */
+  HB_ESTATE = -4   /* call order: sweep or measure before the spins were initialised */
+} hb_status;
+
+typedef enum {
+  HB_SC = 0,   /* simple cubic, periodic, z = 6, 2 colours (x+y+z) mod 2; Lx, Ly, Lz even            */
+  HB_BCC = 1,  /* bcc, periodic, 2 sites per conventional cell, z = 8, colour = basis index          */
+  HB_FCC = 2,  /* fcc, periodic, 4 sites per conventional cell, z = 12, colour = basis index         */
+  HB_CSR = 3   /* arbitrary neighbour table (free-boundary nanostructures), any proper colouring     */
+} hb_kind;
+
+/* Lattice description (host memory, read during hb_create only; the caller keeps ownership).
+ * Neighbour summation order is part of the arithmetic (fp32 adds do not commute bitwise):
+ *   sc : -x,+x,-y,+y,-z,+z
+ *   bcc: corner (b=0) of cell (x,y,z): centres of cells (x-1|x, y-1|y, z-1|z), x fastest;
+ *        centre (b=1): corners of cells (x|x+1, y|y+1, z|z+1), x fastest
+ *   fcc: basis b0 (0,0,0), b1 (0,1/2,1/2), b2 (1/2,0,1/2), b3 (1/2,1/2,0); offsets in doubled
+ *        coordinates (+1,+1,0),(+1,-1,0),(-1,+1,0),(-1,-1,0),(+1,0,+1),(+1,0,-1),(-1,0,+1),
+ *        (-1,0,-1),(0,+1,+1),(0,+1,-1),(0,-1,+1),(0,-1,-1)
+ *   CSR: the order of col_idx within the row.                                                   */
+typedef struct {
+  int32_t kind;            /* hb_kind */
+  int32_t Lx, Ly, Lz;      /* conventional cells per direction (Bravais kinds) */
+  /* HB_CSR only: */
+  int64_t n_sites;
+  const int64_t* row_ptr;  /* n_sites + 1 entries, row_ptr[0] = 0 */
+  const int32_t* col_idx;  /* row_ptr[n_sites] entries; symmetric (with multiplicity), no self loops */
+  int32_t n_colours;       /* with colour != NULL: number of colours, values 0..n_colours-1 */
+  const int32_t* colour;   /* NULL => the library runs greedy first-fit in site order */
+  /* any kind, optional per-site anisotropy (canonical order); NULL => the uniform (K, e) of hb_create */
+  const float* K_site;     /* n entries */
+  const float* e_site;     /* 3n entries, (ex,ey,ez) per site, unit vectors */
+} hb_lattice;
+
+/* Caller-owned device memory (e.g. torch tensors).  Sizes from hb_sizes().  Both
+ * pointers must be 256-byte aligned.  NULL hb_buffers* in hb_create => the library
+ * allocates with cudaMalloc and frees in hb_destroy. */
+typedef struct {
+  void* spins;            /* device, spins_bytes */
+  size_t spins_bytes;
+  void* workspace;        /* device, workspace_bytes (lattice tables, staging, reduction scratch) */
+  size_t workspace_bytes;
+  void* cuda_stream;      /* cudaStream_t; NULL => the legacy default stream */
+} hb_buffers;
+
+/* Number of sites and the device bytes a context for this lattice needs. */
+int hb_sizes(const hb_lattice* lat, int64_t* n_sites, size_t* spins_bytes, size_t* workspace_bytes);
+
+/* Build a context: validates the lattice, colours it, uploads its tables.
+ * J: exchange; (K, e): uniform uniaxial anisotropy, e a unit vector (|e|^2 within 1e-5 of 1);
+ * seed: key of the counter-based Philox4x32-10 stream.  The random numbers of the attempt
+ * at site i in sweep s are Philox(counter = (i, 0, s_lo, s_hi), key = (seed_lo, seed_hi)),
+ * identical on any device and in the CPU oracle. */
+int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float e[3], uint64_t seed,
+              const hb_buffers* bufs);
+int hb_destroy(hb_ctx* ctx);
+
+/* Initial state.  random: S_i = sphere(Philox(counter = (i, 1, 0, 0))): uniform unit vectors.
+ * aligned: S_i = dir (a unit vector).  set/get: host arrays of n floats each, canonical order. */
+int hb_init_random(hb_ctx* ctx);
+int hb_init_aligned(hb_ctx* ctx, const float dir[3]);
+int hb_set_spins(hb_ctx* ctx, const float* sx, const float* sy, const float* sz);
+int hb_get_spins(hb_ctx* ctx, float* sx, float* sy, float* sz);
+
+/* n_sweeps Metropolis sweeps at temperature T (units of J/k_B, T > 0, +inf allowed).
+ * One sweep = one attempt at every site, colours in ascending order.  Asynchronous.
+ * The sweep counter (the Philox counter words 2,3) advances by n_sweeps and is never reset. */
+int hb_sweep(hb_ctx* ctx, float T, int64_t n_sweeps);
+
+/* M[3] = (1/N) sum_i S_i (eq. 2) and E = total energy of eq. 1 (each bond once), accumulated
+ * in fp64 from fp32 per-site terms -0.5 J (S_i.h_i) - K_i (S_i.e_i)^2.  Synchronises. */
+int hb_measure(hb_ctx* ctx, double M[3], double* E);
+
+/* n_sweeps sweeps with a measurement after each, results kept on the device until the end:
+ * M_series[3*s .. 3*s+2], E_series[s] (host, n_sweeps entries).  One synchronisation. */
+int hb_sweep_series(hb_ctx* ctx, float T, int64_t n_sweeps, double* M_series, double* E_series);
+
+/* Diagnostic: ONE sweep that also records every decision; accept[i] = 1 if the attempt at
+ * canonical site i was accepted (host, n bytes).  Same arithmetic as hb_sweep.  Synchronises. */
+int hb_sweep_record(hb_ctx* ctx, float T, uint8_t* accept);
+
+/* Checkpoint: (spins, sweep counter, seed, parameters) reproduce the trajectory bit for bit. */
+int hb_sweep_count(hb_ctx* ctx, uint64_t* out);
+int hb_set_sweep_count(hb_ctx* ctx, uint64_t value);
+
+/* The colouring in use (host, n entries) and the number of colours.  colour may be NULL. */
+int hb_get_colouring(hb_ctx* ctx, int32_t* colour, int32_t* n_colours);
+
+/* Counters since hb_create: kernels launched by this context, sites attempted. */
+int hb_counters(hb_ctx* ctx, uint64_t* kernel_launches, uint64_t* attempts);
+
+/* Tuning knobs, by name (DESIGN.md section 6 lists them); unknown names give HB_EINVAL. */
+int hb_set_option(hb_ctx* ctx, const char* name, int64_t value);
+int hb_get_option(hb_ctx* ctx, const char* name, int64_t* value);
+
+/* Host-side lattice builder for a sphere cut from fcc with a free surface (A10-A12):
+ * doubled integer coordinates X+Y+Z even, X^2+Y^2+Z^2 <= (2R)^2, site order ascending (Z,Y,X).
+ * Core sites (12 neighbours): K_core along e_core; surface sites: K_surf along the radial direction.
+ * colouring: 0 = greedy first-fit in site order, 1 = the four parity classes (X mod 2, Y mod 2).
+ * Fills *out with malloc'ed tables; release with hb_lattice_free.  xyz (optional, may be NULL):
+ * receives a malloc'ed 3n array of the doubled coordinates, to be free()d by the caller. */
+int hb_lattice_fcc_sphere(int32_t R, float K_core, const float e_core[3], float K_surf, int32_t colouring,
+                          hb_lattice* out, int32_t** xyz);
+int hb_lattice_free(hb_lattice* lat);
+
+const char* hb_strerror(int status);
+const char* hb_error_detail(hb_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HB_H_ */

@@ -1,0 +1,275 @@
+"""Thin ctypes binding of libhb.so (include/hb.h): argument marshalling only.
+
+Every step of the hot path runs inside the CUDA library.  PyTorch supplies device
+memory and the stream.  There is no CPU fallback: if the library is missing or no
+CUDA device is present, construction raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+HB_SC, HB_BCC, HB_FCC, HB_CSR = 0, 1, 2, 3
+_KINDS = {"sc": HB_SC, "bcc": HB_BCC, "fcc": HB_FCC, "csr": HB_CSR}
+
+EXPORTS = [
+    "hb_sizes", "hb_create", "hb_destroy", "hb_init_random", "hb_init_aligned", "hb_set_spins", "hb_get_spins",
+    "hb_sweep", "hb_measure", "hb_sweep_series", "hb_sweep_record", "hb_sweep_count", "hb_set_sweep_count",
+    "hb_get_colouring", "hb_counters", "hb_set_option", "hb_get_option", "hb_lattice_fcc_sphere", "hb_lattice_free",
+    "hb_strerror", "hb_error_detail",
+]
+
+
+class hb_lattice(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("Lx", C.c_int32), ("Ly", C.c_int32), ("Lz", C.c_int32),
+                ("n_sites", C.c_int64), ("row_ptr", C.c_void_p), ("col_idx", C.c_void_p),
+                ("n_colours", C.c_int32), ("colour", C.c_void_p), ("K_site", C.c_void_p), ("e_site", C.c_void_p)]
+
+
+class hb_buffers(C.Structure):
+    _fields_ = [("spins", C.c_void_p), ("spins_bytes", C.c_size_t), ("workspace", C.c_void_p),
+                ("workspace_bytes", C.c_size_t), ("cuda_stream", C.c_void_p)]
+
+
+class HbError(RuntimeError):
+    def __init__(self, status, what, detail=""):
+        super().__init__("%s: %s%s" % (what, status, (" (" + detail + ")") if detail else ""))
+        self.status = status
+
+
+_lib = None
+
+
+def library_path():
+    return os.path.join(os.path.dirname(os.path.abspath(__file__)), "libhb.so")
+
+
+def load_library():
+    """dlopen libhb.so and declare the prototypes of include/hb.h.  Fails loudly if it is not built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = library_path()
+    if not os.path.exists(path):
+        raise ImportError("libhb.so is not built: run `python -m paper_2106_11286_b200.build` (needs nvcc)")
+    L = C.CDLL(path)
+    vp, i32, i64, u64, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint64, C.c_float
+    P = C.POINTER
+    protos = {
+        "hb_sizes": [P(hb_lattice), P(i64), P(C.c_size_t), P(C.c_size_t)],
+        "hb_create": [P(vp), P(hb_lattice), f32, f32, P(f32), u64, P(hb_buffers)],
+        "hb_destroy": [vp],
+        "hb_init_random": [vp],
+        "hb_init_aligned": [vp, P(f32)],
+        "hb_set_spins": [vp, vp, vp, vp],
+        "hb_get_spins": [vp, vp, vp, vp],
+        "hb_sweep": [vp, f32, i64],
+        "hb_measure": [vp, P(C.c_double), P(C.c_double)],
+        "hb_sweep_series": [vp, f32, i64, vp, vp],
+        "hb_sweep_record": [vp, f32, vp],
+        "hb_sweep_count": [vp, P(u64)],
+        "hb_set_sweep_count": [vp, u64],
+        "hb_get_colouring": [vp, vp, P(i32)],
+        "hb_counters": [vp, P(u64), P(u64)],
+        "hb_set_option": [vp, C.c_char_p, i64],
+        "hb_get_option": [vp, C.c_char_p, P(i64)],
+        "hb_lattice_fcc_sphere": [i32, f32, P(f32), f32, i32, P(hb_lattice), P(vp)],
+        "hb_lattice_free": [P(hb_lattice)],
+    }
+    for name, args in protos.items():
+        fn = getattr(L, name)
+        fn.restype, fn.argtypes = C.c_int, args
+    L.hb_strerror.restype, L.hb_strerror.argtypes = C.c_char_p, [C.c_int]
+    L.hb_error_detail.restype, L.hb_error_detail.argtypes = C.c_char_p, [vp]
+    _lib = L
+    return L
+
+
+def _vec3(v):
+    return (C.c_float * 3)(*[float(x) for x in v])
+
+
+def _np(a, dt):
+    return np.ascontiguousarray(a, dtype=dt)
+
+
+def _ptr(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+class Lattice:
+    """Host description of a lattice (the hb_lattice struct plus the arrays it points to)."""
+
+    def __init__(self, kind, Lx=0, Ly=0, Lz=0, row_ptr=None, col_idx=None, colour=None, n_colours=0,
+                 K_site=None, e_site=None, xyz=None):
+        self.kind = _KINDS[kind] if isinstance(kind, str) else int(kind)
+        self.Lx, self.Ly, self.Lz = int(Lx), int(Ly or Lx), int(Lz or Lx)
+        self.row_ptr = _np(row_ptr, np.int64) if row_ptr is not None else None
+        self.col_idx = _np(col_idx, np.int32) if col_idx is not None else None
+        self.colour = _np(colour, np.int32) if colour is not None else None
+        self.n_colours = int(n_colours)
+        self.K_site = _np(K_site, np.float32) if K_site is not None else None
+        self.e_site = _np(e_site, np.float32) if e_site is not None else None
+        self.xyz = xyz
+
+    @classmethod
+    def fcc_sphere(cls, R, K_core=0.0, e_core=(0, 0, 1), K_surf=0.0, colouring="greedy"):
+        """hb_lattice_fcc_sphere: the library's own builder (A10-A12)."""
+        L = load_library()
+        out, xyz = hb_lattice(), C.c_void_p()
+        rc = L.hb_lattice_fcc_sphere(R, K_core, _vec3(e_core), K_surf, {"greedy": 0, "parity": 1}[colouring],
+                                     C.byref(out), C.byref(xyz))
+        if rc != 0:
+            raise HbError(rc, "hb_lattice_fcc_sphere", L.hb_strerror(rc).decode())
+        n = out.n_sites
+
+        def take(ptr, count, ctype, dt):
+            return np.ctypeslib.as_array(C.cast(ptr, C.POINTER(ctype)), shape=(count,)).astype(dt, copy=True)
+
+        rp = take(out.row_ptr, n + 1, C.c_int64, np.int64)
+        lat = cls("csr", row_ptr=rp, col_idx=take(out.col_idx, max(int(rp[-1]), 1), C.c_int32, np.int32)[:int(rp[-1])],
+                  colour=take(out.colour, n, C.c_int32, np.int32), n_colours=out.n_colours,
+                  K_site=take(out.K_site, n, C.c_float, np.float32),
+                  e_site=take(out.e_site, 3 * n, C.c_float, np.float32).reshape(n, 3),
+                  xyz=take(xyz, 3 * n, C.c_int32, np.int32).reshape(n, 3))
+        L.hb_lattice_free(C.byref(out))
+        C.CDLL(None).free(xyz)
+        return lat
+
+    def struct(self):
+        s = hb_lattice()
+        s.kind, s.Lx, s.Ly, s.Lz = self.kind, self.Lx, self.Ly, self.Lz
+        if self.row_ptr is not None:
+            s.n_sites = self.row_ptr.size - 1
+            s.row_ptr = _ptr(self.row_ptr)
+            s.col_idx = _ptr(self.col_idx) if self.col_idx is not None and self.col_idx.size else None
+        if self.colour is not None:
+            s.colour, s.n_colours = _ptr(self.colour), self.n_colours
+        if self.K_site is not None:
+            s.K_site, s.e_site = _ptr(self.K_site), _ptr(self.e_site)
+        return s
+
+
+def sizes(lat):
+    """hb_sizes -> (n_sites, spins_bytes, workspace_bytes)."""
+    L = load_library()
+    n, a, b = C.c_int64(), C.c_size_t(), C.c_size_t()
+    s = lat.struct()
+    rc = L.hb_sizes(C.byref(s), C.byref(n), C.byref(a), C.byref(b))
+    if rc != 0:
+        raise HbError(rc, "hb_sizes", L.hb_strerror(rc).decode())
+    return n.value, a.value, b.value
+
+
+class Context:
+    """hb_ctx with torch-owned device memory.  Method names follow include/hb.h."""
+
+    def __init__(self, lat, J=1.0, K=0.0, e=(0.0, 0.0, 1.0), seed=1, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2106_11286_b200 needs a CUDA device; there is no CPU path")
+        self._L = load_library()
+        self.lat = lat
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.n, spins_bytes, ws_bytes = sizes(lat)
+        self._spins = torch.empty(spins_bytes, dtype=torch.uint8, device=self.device)
+        self._ws = torch.empty(ws_bytes, dtype=torch.uint8, device=self.device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        bufs = hb_buffers(self._spins.data_ptr(), spins_bytes, self._ws.data_ptr(), ws_bytes, self.stream.cuda_stream)
+        s = lat.struct()
+        h = C.c_void_p()
+        rc = self._L.hb_create(C.byref(h), C.byref(s), J, K, _vec3(e), seed, C.byref(bufs))
+        self._h = h
+        if rc != 0:
+            detail = self._L.hb_error_detail(h).decode() if h else ""
+            self._L.hb_destroy(h)
+            self._h = None
+            raise HbError(rc, "hb_create", detail or self._L.hb_strerror(rc).decode())
+
+    def _check(self, rc, what):
+        if rc != 0:
+            raise HbError(rc, what, self._L.hb_error_detail(self._h).decode() or self._L.hb_strerror(rc).decode())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.hb_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def init_random(self):
+        self._check(self._L.hb_init_random(self._h), "hb_init_random")
+
+    def init_aligned(self, direction):
+        self._check(self._L.hb_init_aligned(self._h, _vec3(direction)), "hb_init_aligned")
+
+    def set_spins(self, sx, sy, sz):
+        """Host arrays (numpy, or pinned torch CPU tensors) of n floats, canonical order."""
+        p = [self._host_ptr(a) for a in (sx, sy, sz)]
+        self._check(self._L.hb_set_spins(self._h, p[0][0], p[1][0], p[2][0]), "hb_set_spins")
+
+    def _host_ptr(self, a):
+        if isinstance(a, np.ndarray):
+            b = _np(a, np.float32)
+            assert b.size == self.n
+            return C.c_void_p(b.ctypes.data), b
+        assert a.device.type == "cpu" and a.is_contiguous() and a.numel() == self.n and a.element_size() == 4
+        return C.c_void_p(a.data_ptr()), a
+
+    def get_spins(self, out=None):
+        if out is None:
+            out = [np.empty(self.n, np.float32) for _ in range(3)]
+        p = [self._host_ptr(a) for a in out]
+        self._check(self._L.hb_get_spins(self._h, p[0][0], p[1][0], p[2][0]), "hb_get_spins")
+        return out
+
+    def sweep(self, T, n_sweeps=1):
+        self._check(self._L.hb_sweep(self._h, T, n_sweeps), "hb_sweep")
+
+    def measure(self):
+        M, E = (C.c_double * 3)(), C.c_double()
+        self._check(self._L.hb_measure(self._h, M, C.byref(E)), "hb_measure")
+        return np.array(M[:]), E.value
+
+    def sweep_series(self, T, n_sweeps):
+        M, E = np.zeros((n_sweeps, 3)), np.zeros(n_sweeps)
+        self._check(self._L.hb_sweep_series(self._h, T, n_sweeps, _ptr(M), _ptr(E)), "hb_sweep_series")
+        return M, E
+
+    def sweep_record(self, T):
+        acc = np.zeros(self.n, np.uint8)
+        self._check(self._L.hb_sweep_record(self._h, T, _ptr(acc)), "hb_sweep_record")
+        return acc
+
+    @property
+    def sweep_count(self):
+        v = C.c_uint64()
+        self._check(self._L.hb_sweep_count(self._h, C.byref(v)), "hb_sweep_count")
+        return v.value
+
+    @sweep_count.setter
+    def sweep_count(self, value):
+        self._check(self._L.hb_set_sweep_count(self._h, value), "hb_set_sweep_count")
+
+    def colouring(self):
+        col, nc = np.zeros(self.n, np.int32), C.c_int32()
+        self._check(self._L.hb_get_colouring(self._h, _ptr(col), C.byref(nc)), "hb_get_colouring")
+        return col, nc.value
+
+    def counters(self):
+        a, b = C.c_uint64(), C.c_uint64()
+        self._check(self._L.hb_counters(self._h, C.byref(a), C.byref(b)), "hb_counters")
+        return a.value, b.value
+
+    def set_option(self, name, value):
+        self._check(self._L.hb_set_option(self._h, name.encode(), int(value)), "hb_set_option(%s)" % name)
+
+    def get_option(self, name):
+        v = C.c_int64()
+        self._check(self._L.hb_get_option(self._h, name.encode(), C.byref(v)), "hb_get_option(%s)" % name)
+        return v.value

@@ -1,0 +1,640 @@
+// hb_api.cpp -- the C ABI of include/hb.h: context, validation, sweep driver.
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/hb.h"
+#include "hb_internal.h"
+
+using namespace hb;
+
+namespace {
+
+constexpr size_t kAlign = 256;
+constexpr int kSeriesChunk = 1024;
+
+inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+enum Engine { ENGINE_SC = 0, ENGINE_CSR = 1 };
+
+struct Plan {                 // device memory plan of a lattice
+  int64_t n = 0, nnz = 0;
+  int engine = ENGINE_CSR;
+  bool per_site = false;
+  size_t spins_bytes = 0, ws_bytes = 0;
+  size_t off_partials = 0, off_series = 0, off_counters = 0, off_staging = 0;
+  size_t off_row_ptr = 0, off_col = 0, off_list = 0, off_K = 0, off_e = 0;
+};
+
+int make_plan(const hb_lattice* lat, Plan& p, std::string& why) {
+  if (!lat) { why = "lattice is NULL"; return HB_EINVAL; }
+  const int k = lat->kind;
+  if (k == HB_SC || k == HB_BCC || k == HB_FCC) {
+    if (lat->Lx < 1 || lat->Ly < 1 || lat->Lz < 1) { why = "Lx, Ly, Lz must be >= 1"; return HB_EINVAL; }
+    const int64_t cells = (int64_t)lat->Lx * lat->Ly * lat->Lz;
+    const int basis = k == HB_SC ? 1 : (k == HB_BCC ? 2 : 4);
+    const int z = k == HB_SC ? 6 : (k == HB_BCC ? 8 : 12);
+    p.n = cells * basis;
+    p.nnz = p.n * z;
+    if (k == HB_SC && ((lat->Lx | lat->Ly | lat->Lz) & 1)) {
+      why = "simple cubic needs even Lx, Ly, Lz (two-colour checkerboard with periodic wrap)";
+      return HB_EINVAL;
+    }
+  } else if (k == HB_CSR) {
+    if (lat->n_sites < 0 || !lat->row_ptr) { why = "CSR lattice needs n_sites >= 0 and row_ptr"; return HB_EINVAL; }
+    p.n = lat->n_sites;
+    p.nnz = lat->row_ptr[lat->n_sites];
+  } else {
+    why = "unknown lattice kind";
+    return HB_EINVAL;
+  }
+  if (p.n < 1) { why = "lattice has no sites"; return HB_EINVAL; }
+  if (p.n > 0xFFFFFFFFll) { why = "more than 2^32-1 sites (site ids are 32-bit Philox counter words)"; return HB_EINVAL; }
+  if (p.nnz >= 0x7FFFFFFFll) { why = "more than 2^31-2 neighbour entries"; return HB_EINVAL; }
+  if ((lat->K_site == nullptr) != (lat->e_site == nullptr)) { why = "K_site and e_site go together"; return HB_EINVAL; }
+  p.per_site = lat->K_site != nullptr;
+  p.engine = (k == HB_SC && !p.per_site) ? ENGINE_SC : ENGINE_CSR;
+  p.spins_bytes = align_up(3 * (size_t)p.n * sizeof(float));
+  size_t o = 0;
+  p.off_partials = o; o += align_up((size_t)kMeasureBlocks * 4 * sizeof(double));
+  p.off_series = o;   o += align_up((size_t)kSeriesChunk * 4 * sizeof(double));
+  p.off_counters = o; o += kAlign;
+  p.off_staging = o;  o += align_up((size_t)p.n * sizeof(float));
+  if (p.engine == ENGINE_CSR) {
+    p.off_row_ptr = o; o += align_up(((size_t)p.n + 1) * sizeof(int32_t));
+    p.off_col = o;     o += align_up((size_t)p.nnz * sizeof(int32_t));
+    p.off_list = o;    o += align_up((size_t)p.n * sizeof(int32_t));
+    if (p.per_site) {
+      p.off_K = o; o += align_up((size_t)p.n * sizeof(float));
+      p.off_e = o; o += align_up(3 * (size_t)p.n * sizeof(float));
+    }
+  }
+  p.ws_bytes = o;
+  return HB_OK;
+}
+
+}  // namespace
+
+struct hb_ctx {
+  Plan plan;
+  int32_t kind = 0, Lx = 0, Ly = 0, Lz = 0;
+  ScLayout sc{};
+  ScTile tile{};
+  CsrDev csr{};
+  int csr_block = 128;
+  std::vector<uint32_t> colour_begin;     // CSR engine: offsets into the colour-sorted list
+  std::vector<int32_t> colour_host;       // CSR engine: colour of every site
+  int32_t n_colours = 0;
+  float J = 0, K = 0, e[3] = {0, 0, 1};
+  uint64_t seed = 0, sweep = 0;
+  bool initialised = false;
+  cudaStream_t stream = nullptr;
+  float* spins = nullptr;
+  char* ws = nullptr;
+  bool own_spins = false, own_ws = false;
+  uint64_t launches = 0, attempts = 0;
+  int sticky = HB_OK;
+  std::string detail;
+
+  double* partials() const { return reinterpret_cast<double*>(ws + plan.off_partials); }
+  double* series() const { return reinterpret_cast<double*>(ws + plan.off_series); }
+  unsigned long long* counters() const { return reinterpret_cast<unsigned long long*>(ws + plan.off_counters); }
+  float* staging() const { return reinterpret_cast<float*>(ws + plan.off_staging); }
+};
+
+namespace {
+
+int fail(hb_ctx* c, int status, const std::string& msg) {
+  if (c) {
+    c->detail = msg;
+    if (status == HB_ECUDA) c->sticky = HB_ECUDA;
+  }
+  return status;
+}
+
+#define HB_CUDA(ctx, call)                                                                      \
+  do {                                                                                          \
+    const cudaError_t err__ = (call);                                                           \
+    if (err__ != cudaSuccess)                                                                   \
+      return fail(ctx, HB_ECUDA, std::string(#call) + ": " + cudaGetErrorString(err__));        \
+  } while (0)
+
+#define HB_CHECK_CTX(ctx)                                   \
+  do {                                                      \
+    if (!(ctx)) return HB_EINVAL;                           \
+    if ((ctx)->sticky != HB_OK) return (ctx)->sticky;       \
+  } while (0)
+
+SweepParams params(const hb_ctx* c, float beta) {
+  SweepParams p;
+  p.J = c->J; p.K = c->K; p.ex = c->e[0]; p.ey = c->e[1]; p.ez = c->e[2]; p.beta = beta;
+  p.seed_lo = (uint32_t)c->seed; p.seed_hi = (uint32_t)(c->seed >> 32);
+  p.sweep_lo = (uint32_t)c->sweep; p.sweep_hi = (uint32_t)(c->sweep >> 32);
+  return p;
+}
+
+bool unit_vector(const float* v) {
+  const double n2 = (double)v[0] * v[0] + (double)v[1] * v[1] + (double)v[2] * v[2];
+  return std::isfinite(n2) && std::fabs(n2 - 1.0) <= 1e-5;
+}
+
+// default launch shape of the sc kernels for a lattice
+ScTile default_tile(const ScLayout& L) {
+  ScTile t;
+  t.V = (L.H % 4 == 0) ? 4 : ((L.H % 2 == 0) ? 2 : 1);
+  const int HV = L.H / t.V;
+  int best = HV <= 64 ? HV : 64, best_waste = 1 << 30;
+  if (HV > 64) {
+    for (int jx = 64; jx >= 24; --jx) {
+      const int waste = (HV + jx - 1) / jx * jx - HV;
+      if (waste < best_waste) { best_waste = waste; best = jx; }
+    }
+  }
+  t.JX = best;
+  t.TY = 256 / t.JX;
+  if (t.TY > L.Ly) t.TY = L.Ly;
+  if (t.TY < 1) t.TY = 1;
+  // enough blocks to fill 148 SMs several times over, else shorter z-marches
+  const int64_t cols = (int64_t)((HV + t.JX - 1) / t.JX) * ((L.Ly + t.TY - 1) / t.TY);
+  t.ZT = 8;
+  while (t.ZT > 1 && cols * ((L.Lz + t.ZT - 1) / t.ZT) < 148 * 16) t.ZT /= 2;
+  return t;
+}
+
+int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d) {
+  if (c->plan.engine == ENGINE_SC) {
+    HB_CUDA(c, launch_sweep_sc(c->stream, c->spins, c->sc, c->tile, p, colour, d));
+  } else {
+    const uint32_t b = c->colour_begin[colour], e = c->colour_begin[colour + 1];
+    if (e == b) return HB_OK;
+    HB_CUDA(c, launch_sweep_csr(c->stream, c->spins, c->csr, b, e - b, p, c->csr_block, d));
+  }
+  c->launches += 1;
+  return HB_OK;
+}
+
+int one_sweep(hb_ctx* c, float beta, Diag d) {
+  const SweepParams p = params(c, beta);
+  for (int colour = 0; colour < c->n_colours; ++colour) {
+    const int rc = one_colour(c, colour, p, d);
+    if (rc != HB_OK) return rc;
+  }
+  c->sweep += 1;
+  c->attempts += (uint64_t)c->plan.n;
+  return HB_OK;
+}
+
+int measure_into(hb_ctx* c, double* dev_out) {
+  const SweepParams p = params(c, 0.0f);
+  if (c->plan.engine == ENGINE_SC)
+    HB_CUDA(c, launch_measure_sc(c->stream, c->spins, c->sc, c->tile.V, p, c->partials(), dev_out));
+  else
+    HB_CUDA(c, launch_measure_csr(c->stream, c->spins, c->csr, p, c->partials(), dev_out));
+  c->launches += 2;
+  return HB_OK;
+}
+
+int check_T(hb_ctx* c, float T, float* beta) {
+  if (!(T > 0.0f)) return fail(c, HB_EINVAL, "temperature must be > 0 (NaN and T <= 0 are rejected)");
+  *beta = 1.0f / T;   // computed once on the host, passed to every kernel
+  return HB_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int hb_sizes(const hb_lattice* lat, int64_t* n_sites, size_t* spins_bytes, size_t* workspace_bytes) {
+  Plan p;
+  std::string why;
+  const int rc = make_plan(lat, p, why);
+  if (rc != HB_OK) return rc;
+  if (n_sites) *n_sites = p.n;
+  if (spins_bytes) *spins_bytes = p.spins_bytes;
+  if (workspace_bytes) *workspace_bytes = p.ws_bytes;
+  return HB_OK;
+}
+
+int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float e[3], uint64_t seed,
+              const hb_buffers* bufs) {
+  if (!out) return HB_EINVAL;
+  *out = nullptr;
+  hb_ctx* c = new (std::nothrow) hb_ctx;
+  if (!c) return HB_ENOMEM;
+  // the context is handed back even on failure so that hb_error_detail can say why
+  *out = c;
+  std::string why;
+  int rc = make_plan(lat, c->plan, why);
+  if (rc != HB_OK) { c->sticky = rc; return fail(c, rc, why); }
+  if (!e || !unit_vector(e) || !std::isfinite(J) || !std::isfinite(K)) {
+    c->sticky = HB_EINVAL;
+    return fail(c, HB_EINVAL, "J, K must be finite and e a unit vector");
+  }
+  c->kind = lat->kind; c->Lx = lat->Lx; c->Ly = lat->Ly; c->Lz = lat->Lz;
+  c->J = J; c->K = K; c->e[0] = e[0]; c->e[1] = e[1]; c->e[2] = e[2];
+  c->seed = seed;
+  const Plan& P = c->plan;
+  if (P.per_site)
+    for (int64_t i = 0; i < P.n; ++i)
+      if (!unit_vector(lat->e_site + 3 * i) || !std::isfinite(lat->K_site[i])) {
+        c->sticky = HB_EINVAL;
+        return fail(c, HB_EINVAL, "e_site must hold unit vectors and K_site finite values");
+      }
+
+  // ---- host tables -------------------------------------------------------------------------
+  HostCsr g;
+  const int64_t* row_ptr = nullptr;
+  const int32_t* col = nullptr;
+  if (P.engine == ENGINE_CSR) {
+    if (lat->kind == HB_CSR) {
+      why = validate_csr(P.n, lat->row_ptr, lat->col_idx);
+      if (!why.empty()) { c->sticky = HB_EINVAL; return fail(c, HB_EINVAL, why); }
+      row_ptr = lat->row_ptr; col = lat->col_idx;
+      if (lat->colour) {
+        why = validate_colouring(P.n, row_ptr, col, lat->colour, lat->n_colours);
+        if (!why.empty()) { c->sticky = HB_EINVAL; return fail(c, HB_EINVAL, why); }
+        c->colour_host.assign(lat->colour, lat->colour + P.n);
+        c->n_colours = lat->n_colours;
+      } else {
+        g.n = P.n;
+        g.row_ptr.assign(row_ptr, row_ptr + P.n + 1);
+        g.col.assign(col, col + P.nnz);
+        greedy_first_fit(g);
+        c->colour_host = g.colour;
+        c->n_colours = g.n_colours;
+      }
+    } else {
+      if (lat->kind == HB_BCC) build_bcc_csr(lat->Lx, lat->Ly, lat->Lz, g);
+      else if (lat->kind == HB_FCC) build_fcc_csr(lat->Lx, lat->Ly, lat->Lz, g);
+      else {  // sc with per-site anisotropy: explicit table, same order -x,+x,-y,+y,-z,+z
+        const int32_t Lx = lat->Lx, Ly = lat->Ly, Lz = lat->Lz;
+        g.n = P.n; g.n_colours = 2;
+        g.row_ptr.resize(P.n + 1); g.col.resize(6 * P.n); g.colour.resize(P.n);
+        for (int64_t i = 0; i <= P.n; ++i) g.row_ptr[i] = 6 * i;
+        for (int32_t z = 0; z < Lz; ++z)
+          for (int32_t y = 0; y < Ly; ++y)
+            for (int32_t x = 0; x < Lx; ++x) {
+              const int64_t plane = (int64_t)z * Ly, i = (plane + y) * Lx + x;
+              int32_t* o = &g.col[6 * i];
+              o[0] = (int32_t)((plane + y) * Lx + (x ? x - 1 : Lx - 1));
+              o[1] = (int32_t)((plane + y) * Lx + (x + 1 < Lx ? x + 1 : 0));
+              o[2] = (int32_t)((plane + (y ? y - 1 : Ly - 1)) * Lx + x);
+              o[3] = (int32_t)((plane + (y + 1 < Ly ? y + 1 : 0)) * Lx + x);
+              o[4] = (int32_t)(((int64_t)(z ? z - 1 : Lz - 1) * Ly + y) * Lx + x);
+              o[5] = (int32_t)(((int64_t)(z + 1 < Lz ? z + 1 : 0) * Ly + y) * Lx + x);
+              g.colour[i] = (x + y + z) & 1;
+            }
+      }
+      row_ptr = g.row_ptr.data(); col = g.col.data();
+      c->colour_host = g.colour;
+      c->n_colours = g.n_colours;
+    }
+  } else {
+    c->n_colours = 2;
+    c->sc.Lx = lat->Lx; c->sc.Ly = lat->Ly; c->sc.Lz = lat->Lz;
+    c->sc.H = lat->Lx / 2; c->sc.n = (uint32_t)P.n; c->sc.half = (uint32_t)(P.n / 2);
+    c->tile = default_tile(c->sc);
+  }
+
+  // ---- device memory --------------------------------------------------------------------------
+  if (bufs) {
+    if (!bufs->spins || !bufs->workspace || bufs->spins_bytes < P.spins_bytes || bufs->workspace_bytes < P.ws_bytes ||
+        ((uintptr_t)bufs->spins % kAlign) || ((uintptr_t)bufs->workspace % kAlign)) {
+      c->sticky = HB_ENOMEM;
+      return fail(c, HB_ENOMEM, "caller buffers are NULL, too small (see hb_sizes) or not 256-byte aligned");
+    }
+    c->spins = static_cast<float*>(bufs->spins);
+    c->ws = static_cast<char*>(bufs->workspace);
+    c->stream = static_cast<cudaStream_t>(bufs->cuda_stream);
+  } else {
+    void* a = nullptr; void* b = nullptr;
+    if (cudaMalloc(&a, P.spins_bytes) != cudaSuccess || cudaMalloc(&b, P.ws_bytes) != cudaSuccess) {
+      if (a) cudaFree(a);
+      cudaGetLastError();
+      c->sticky = HB_ENOMEM;
+      return fail(c, HB_ENOMEM, "cudaMalloc failed");
+    }
+    c->spins = static_cast<float*>(a); c->ws = static_cast<char*>(b);
+    c->own_spins = c->own_ws = true;
+  }
+  HB_CUDA(c, cudaMemsetAsync(c->ws + P.off_counters, 0, kAlign, c->stream));
+
+  if (P.engine == ENGINE_CSR) {
+    // sites sorted by (colour, id): one contiguous list segment per colour
+    std::vector<uint32_t> count((size_t)c->n_colours + 1, 0);
+    for (int64_t i = 0; i < P.n; ++i) count[c->colour_host[i] + 1] += 1;
+    for (int k = 0; k < c->n_colours; ++k) count[k + 1] += count[k];
+    c->colour_begin = count;
+    std::vector<int32_t> list((size_t)P.n);
+    {
+      std::vector<uint32_t> cur(count.begin(), count.end() - 1);
+      for (int64_t i = 0; i < P.n; ++i) list[cur[c->colour_host[i]]++] = (int32_t)i;
+    }
+    std::vector<int32_t> rp32((size_t)P.n + 1);
+    for (int64_t i = 0; i <= P.n; ++i) rp32[i] = (int32_t)row_ptr[i];
+    int32_t* d_rp = reinterpret_cast<int32_t*>(c->ws + P.off_row_ptr);
+    int32_t* d_col = reinterpret_cast<int32_t*>(c->ws + P.off_col);
+    int32_t* d_list = reinterpret_cast<int32_t*>(c->ws + P.off_list);
+    HB_CUDA(c, cudaMemcpyAsync(d_rp, rp32.data(), rp32.size() * 4, cudaMemcpyHostToDevice, c->stream));
+    if (P.nnz) HB_CUDA(c, cudaMemcpyAsync(d_col, col, (size_t)P.nnz * 4, cudaMemcpyHostToDevice, c->stream));
+    HB_CUDA(c, cudaMemcpyAsync(d_list, list.data(), list.size() * 4, cudaMemcpyHostToDevice, c->stream));
+    c->csr.n = (uint32_t)P.n; c->csr.row_ptr = d_rp; c->csr.col = d_col; c->csr.list = d_list;
+    c->csr.K_site = nullptr; c->csr.e_site = nullptr;
+    if (P.per_site) {
+      float* d_K = reinterpret_cast<float*>(c->ws + P.off_K);
+      float* d_e = reinterpret_cast<float*>(c->ws + P.off_e);
+      HB_CUDA(c, cudaMemcpyAsync(d_K, lat->K_site, (size_t)P.n * 4, cudaMemcpyHostToDevice, c->stream));
+      HB_CUDA(c, cudaMemcpyAsync(d_e, lat->e_site, (size_t)P.n * 12, cudaMemcpyHostToDevice, c->stream));
+      c->csr.K_site = d_K; c->csr.e_site = d_e;
+    }
+    HB_CUDA(c, cudaStreamSynchronize(c->stream));   // the host vectors die at return
+  }
+  return HB_OK;
+}
+
+int hb_destroy(hb_ctx* c) {
+  if (!c) return HB_OK;
+  if (c->own_spins && c->spins) cudaFree(c->spins);
+  if (c->own_ws && c->ws) cudaFree(c->ws);
+  delete c;
+  return HB_OK;
+}
+
+int hb_init_random(hb_ctx* c) {
+  HB_CHECK_CTX(c);
+  if (c->plan.engine == ENGINE_SC)
+    HB_CUDA(c, launch_init_random_sc(c->stream, c->spins, c->sc, (uint32_t)c->seed, (uint32_t)(c->seed >> 32)));
+  else
+    HB_CUDA(c, launch_init_random_flat(c->stream, c->spins, (uint32_t)c->plan.n, (uint32_t)c->seed, (uint32_t)(c->seed >> 32)));
+  c->launches += 1;
+  c->initialised = true;
+  return HB_OK;
+}
+
+int hb_init_aligned(hb_ctx* c, const float dir[3]) {
+  HB_CHECK_CTX(c);
+  if (!dir || !unit_vector(dir)) return fail(c, HB_EINVAL, "dir must be a unit vector");
+  HB_CUDA(c, launch_fill(c->stream, c->spins, (uint32_t)c->plan.n, dir[0], dir[1], dir[2]));
+  c->launches += 1;
+  c->initialised = true;
+  return HB_OK;
+}
+
+int hb_set_spins(hb_ctx* c, const float* sx, const float* sy, const float* sz) {
+  HB_CHECK_CTX(c);
+  if (!sx || !sy || !sz) return fail(c, HB_EINVAL, "NULL spin array");
+  const size_t n = (size_t)c->plan.n;
+  const float* src[3] = {sx, sy, sz};
+  for (int k = 0; k < 3; ++k) {
+    if (c->plan.engine == ENGINE_SC) {
+      HB_CUDA(c, cudaMemcpyAsync(c->staging(), src[k], n * 4, cudaMemcpyHostToDevice, c->stream));
+      HB_CUDA(c, launch_sc_permute(c->stream, c->spins + k * n, c->staging(), c->sc, true));
+      c->launches += 1;
+    } else {
+      HB_CUDA(c, cudaMemcpyAsync(c->spins + k * n, src[k], n * 4, cudaMemcpyHostToDevice, c->stream));
+    }
+  }
+  HB_CUDA(c, cudaStreamSynchronize(c->stream));   // the caller may reuse its arrays
+  c->initialised = true;
+  return HB_OK;
+}
+
+int hb_get_spins(hb_ctx* c, float* sx, float* sy, float* sz) {
+  HB_CHECK_CTX(c);
+  if (!sx || !sy || !sz) return fail(c, HB_EINVAL, "NULL spin array");
+  if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
+  const size_t n = (size_t)c->plan.n;
+  float* dst[3] = {sx, sy, sz};
+  for (int k = 0; k < 3; ++k) {
+    if (c->plan.engine == ENGINE_SC) {
+      HB_CUDA(c, launch_sc_permute(c->stream, c->staging(), c->spins + k * n, c->sc, false));
+      c->launches += 1;
+      HB_CUDA(c, cudaMemcpyAsync(dst[k], c->staging(), n * 4, cudaMemcpyDeviceToHost, c->stream));
+    } else {
+      HB_CUDA(c, cudaMemcpyAsync(dst[k], c->spins + k * n, n * 4, cudaMemcpyDeviceToHost, c->stream));
+    }
+  }
+  HB_CUDA(c, cudaStreamSynchronize(c->stream));
+  return HB_OK;
+}
+
+int hb_sweep(hb_ctx* c, float T, int64_t n_sweeps) {
+  HB_CHECK_CTX(c);
+  if (n_sweeps < 0) return fail(c, HB_EINVAL, "n_sweeps < 0");
+  if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
+  float beta;
+  int rc = check_T(c, T, &beta);
+  if (rc != HB_OK) return rc;
+  for (int64_t s = 0; s < n_sweeps; ++s) {
+    rc = one_sweep(c, beta, Diag{nullptr, nullptr});
+    if (rc != HB_OK) return rc;
+  }
+  return HB_OK;
+}
+
+int hb_measure(hb_ctx* c, double M[3], double* E) {
+  HB_CHECK_CTX(c);
+  if (!M || !E) return fail(c, HB_EINVAL, "NULL output");
+  if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
+  int rc = measure_into(c, c->series());
+  if (rc != HB_OK) return rc;
+  double h[4];
+  HB_CUDA(c, cudaMemcpyAsync(h, c->series(), sizeof h, cudaMemcpyDeviceToHost, c->stream));
+  HB_CUDA(c, cudaStreamSynchronize(c->stream));
+  const double inv = 1.0 / (double)c->plan.n;
+  M[0] = h[0] * inv; M[1] = h[1] * inv; M[2] = h[2] * inv;
+  *E = h[3];
+  return HB_OK;
+}
+
+int hb_sweep_series(hb_ctx* c, float T, int64_t n_sweeps, double* M_series, double* E_series) {
+  HB_CHECK_CTX(c);
+  if (n_sweeps < 0 || !M_series || !E_series) return fail(c, HB_EINVAL, "bad series arguments");
+  if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
+  float beta;
+  int rc = check_T(c, T, &beta);
+  if (rc != HB_OK) return rc;
+  std::vector<double> h((size_t)kSeriesChunk * 4);
+  const double inv = 1.0 / (double)c->plan.n;
+  for (int64_t s0 = 0; s0 < n_sweeps; s0 += kSeriesChunk) {
+    const int64_t m = n_sweeps - s0 < kSeriesChunk ? n_sweeps - s0 : kSeriesChunk;
+    for (int64_t s = 0; s < m; ++s) {
+      rc = one_sweep(c, beta, Diag{nullptr, nullptr});
+      if (rc != HB_OK) return rc;
+      rc = measure_into(c, c->series() + 4 * s);
+      if (rc != HB_OK) return rc;
+    }
+    HB_CUDA(c, cudaMemcpyAsync(h.data(), c->series(), (size_t)m * 32, cudaMemcpyDeviceToHost, c->stream));
+    HB_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (int64_t s = 0; s < m; ++s) {
+      M_series[3 * (s0 + s) + 0] = h[4 * s + 0] * inv;
+      M_series[3 * (s0 + s) + 1] = h[4 * s + 1] * inv;
+      M_series[3 * (s0 + s) + 2] = h[4 * s + 2] * inv;
+      E_series[s0 + s] = h[4 * s + 3];
+    }
+  }
+  return HB_OK;
+}
+
+int hb_sweep_record(hb_ctx* c, float T, uint8_t* accept) {
+  HB_CHECK_CTX(c);
+  if (!accept) return fail(c, HB_EINVAL, "NULL accept array");
+  if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
+  float beta;
+  int rc = check_T(c, T, &beta);
+  if (rc != HB_OK) return rc;
+  uint8_t* d_acc = reinterpret_cast<uint8_t*>(c->staging());
+  HB_CUDA(c, cudaMemsetAsync(d_acc, 0xFF, (size_t)c->plan.n, c->stream));   // every site must be overwritten
+  rc = one_sweep(c, beta, Diag{d_acc, c->counters()});
+  if (rc != HB_OK) return rc;
+  HB_CUDA(c, cudaMemcpyAsync(accept, d_acc, (size_t)c->plan.n, cudaMemcpyDeviceToHost, c->stream));
+  HB_CUDA(c, cudaStreamSynchronize(c->stream));
+  return HB_OK;
+}
+
+int hb_sweep_count(hb_ctx* c, uint64_t* out) {
+  if (!c || !out) return HB_EINVAL;
+  *out = c->sweep;
+  return HB_OK;
+}
+
+int hb_set_sweep_count(hb_ctx* c, uint64_t value) {
+  if (!c) return HB_EINVAL;
+  c->sweep = value;
+  return HB_OK;
+}
+
+int hb_get_colouring(hb_ctx* c, int32_t* colour, int32_t* n_colours) {
+  HB_CHECK_CTX(c);
+  if (n_colours) *n_colours = c->n_colours;
+  if (!colour) return HB_OK;
+  if (c->plan.engine == ENGINE_SC) {
+    for (int32_t z = 0; z < c->Lz; ++z)
+      for (int32_t y = 0; y < c->Ly; ++y)
+        for (int32_t x = 0; x < c->Lx; ++x) colour[((int64_t)z * c->Ly + y) * c->Lx + x] = (x + y + z) & 1;
+  } else {
+    std::memcpy(colour, c->colour_host.data(), c->colour_host.size() * sizeof(int32_t));
+  }
+  return HB_OK;
+}
+
+int hb_counters(hb_ctx* c, uint64_t* kernel_launches, uint64_t* attempts) {
+  if (!c) return HB_EINVAL;
+  if (kernel_launches) *kernel_launches = c->launches;
+  if (attempts) *attempts = c->attempts;
+  return HB_OK;
+}
+
+int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
+  HB_CHECK_CTX(c);
+  if (!name) return HB_EINVAL;
+  const std::string s(name);
+  if (s == "csr_block") {
+    if (value < 32 || value > 256 || value % 32) return fail(c, HB_EINVAL, "csr_block: multiple of 32 in [32,256]");
+    c->csr_block = (int)value;
+    return HB_OK;
+  }
+  if (c->plan.engine != ENGINE_SC) return fail(c, HB_EINVAL, "option not valid for this lattice");
+  ScTile t = c->tile;
+  if (s == "sc_v") {
+    if (!(value == 1 || value == 2 || value == 4) || c->sc.H % value) return fail(c, HB_EINVAL, "sc_v: 1, 2 or 4 dividing Lx/2");
+    t.V = (int)value;
+    if (t.JX > c->sc.H / t.V) t.JX = c->sc.H / t.V;
+  } else if (s == "sc_jx") t.JX = (int)value;
+  else if (s == "sc_ty") t.TY = (int)value;
+  else if (s == "sc_zt") t.ZT = (int)value;
+  else return fail(c, HB_EINVAL, "unknown option");
+  if (t.JX < 1 || t.TY < 1 || t.ZT < 1 || (int64_t)t.JX * t.TY > 256 || t.ZT > c->sc.Lz)
+    return fail(c, HB_EINVAL, "sc tile: JX, TY, ZT >= 1, JX*TY <= 256, ZT <= Lz");
+  c->tile = t;
+  return HB_OK;
+}
+
+int hb_get_option(hb_ctx* c, const char* name, int64_t* value) {
+  if (!c || !name || !value) return HB_EINVAL;
+  const std::string s(name);
+  if (s == "csr_block") *value = c->csr_block;
+  else if (s == "sc_v") *value = c->tile.V;
+  else if (s == "sc_jx") *value = c->tile.JX;
+  else if (s == "sc_ty") *value = c->tile.TY;
+  else if (s == "sc_zt") *value = c->tile.ZT;
+  else if (s == "engine") *value = c->plan.engine;
+  else return HB_EINVAL;
+  return HB_OK;
+}
+
+int hb_lattice_fcc_sphere(int32_t R, float K_core, const float e_core[3], float K_surf, int32_t colouring,
+                          hb_lattice* out, int32_t** xyz_out) {
+  if (!out || !e_core || R < 0 || R > 200 || (colouring != 0 && colouring != 1)) return HB_EINVAL;
+  HostCsr g;
+  std::vector<int32_t> xyz;
+  build_fcc_sphere_csr(R, g, xyz);
+  if (colouring == 0) {
+    greedy_first_fit(g);
+  } else {
+    for (int64_t i = 0; i < g.n; ++i) g.colour[i] = (xyz[3 * i] & 1) * 2 + (xyz[3 * i + 1] & 1);
+    g.n_colours = 4;
+    if (g.n == 1) g.n_colours = 1;
+  }
+  std::memset(out, 0, sizeof *out);
+  const size_t n = (size_t)g.n, nnz = g.col.size();
+  int64_t* rp = static_cast<int64_t*>(std::malloc((n + 1) * sizeof(int64_t)));
+  int32_t* ci = static_cast<int32_t*>(std::malloc((nnz ? nnz : 1) * sizeof(int32_t)));
+  int32_t* cc = static_cast<int32_t*>(std::malloc(n * sizeof(int32_t)));
+  float* Ks = static_cast<float*>(std::malloc(n * sizeof(float)));
+  float* es = static_cast<float*>(std::malloc(3 * n * sizeof(float)));
+  int32_t* xo = xyz_out ? static_cast<int32_t*>(std::malloc(3 * n * sizeof(int32_t))) : nullptr;
+  if (!rp || !ci || !cc || !Ks || !es || (xyz_out && !xo)) {
+    std::free(rp); std::free(ci); std::free(cc); std::free(Ks); std::free(es); std::free(xo);
+    return HB_ENOMEM;
+  }
+  std::memcpy(rp, g.row_ptr.data(), (n + 1) * sizeof(int64_t));
+  if (nnz) std::memcpy(ci, g.col.data(), nnz * sizeof(int32_t));
+  std::memcpy(cc, g.colour.data(), n * sizeof(int32_t));
+  for (size_t i = 0; i < n; ++i) {
+    const bool core = (rp[i + 1] - rp[i]) == 12;
+    if (core) {
+      Ks[i] = K_core; es[3 * i] = e_core[0]; es[3 * i + 1] = e_core[1]; es[3 * i + 2] = e_core[2];
+    } else {
+      const double X = xyz[3 * i], Y = xyz[3 * i + 1], Z = xyz[3 * i + 2];
+      const double rr = std::sqrt(X * X + Y * Y + Z * Z);
+      Ks[i] = K_surf;
+      es[3 * i] = rr > 0 ? (float)(X / rr) : 0.0f;
+      es[3 * i + 1] = rr > 0 ? (float)(Y / rr) : 0.0f;
+      es[3 * i + 2] = rr > 0 ? (float)(Z / rr) : 1.0f;
+    }
+  }
+  if (xo) { std::memcpy(xo, xyz.data(), 3 * n * sizeof(int32_t)); *xyz_out = xo; }
+  out->kind = HB_CSR; out->n_sites = g.n; out->row_ptr = rp; out->col_idx = ci;
+  out->n_colours = g.n_colours; out->colour = cc; out->K_site = Ks; out->e_site = es;
+  return HB_OK;
+}
+
+int hb_lattice_free(hb_lattice* lat) {
+  if (!lat) return HB_OK;
+  std::free(const_cast<int64_t*>(lat->row_ptr));
+  std::free(const_cast<int32_t*>(lat->col_idx));
+  std::free(const_cast<int32_t*>(lat->colour));
+  std::free(const_cast<float*>(lat->K_site));
+  std::free(const_cast<float*>(lat->e_site));
+  std::memset(lat, 0, sizeof *lat);
+  return HB_OK;
+}
+
+const char* hb_strerror(int status) {
+  switch (status) {
+    case HB_OK: return "ok";
+    case HB_EINVAL: return "invalid argument";
+    case HB_ENOMEM: return "out of memory or buffer too small";
+    case HB_ECUDA: return "CUDA error";
+    case HB_ESTATE: return "call out of order";
+    default: return "unknown status";
+  }
+}
+
+const char* hb_error_detail(hb_ctx* c) { return c ? c->detail.c_str() : ""; }
+
+}  // extern "C"

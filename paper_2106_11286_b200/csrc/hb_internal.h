@@ -1,0 +1,78 @@
+// hb_internal.h -- host-side declarations shared by hb_api.cpp, hb_lattice.cpp and hb_kernels.cu.
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+namespace hb {
+
+// parameters of one colour pass (passed by value to the kernels)
+struct SweepParams {
+  float J, K, ex, ey, ez, beta;
+  uint32_t seed_lo, seed_hi, sweep_lo, sweep_hi;
+};
+
+// simple cubic, colour-split storage
+struct ScLayout {
+  int32_t Lx, Ly, Lz;
+  int32_t H;        // Lx/2: sites of one colour per x-row
+  uint32_t half;    // N/2: sites per colour
+  uint32_t n;       // N
+};
+
+// launch shape of the sc kernels: a block is JX x TY threads, each thread owns V
+// consecutive same-colour sites of one x-row and marches ZT planes in z
+struct ScTile {
+  int32_t V, JX, TY, ZT;
+};
+
+// CSR tables on the device
+struct CsrDev {
+  uint32_t n;
+  const int32_t* row_ptr;   // n+1
+  const int32_t* col;       // nnz
+  const int32_t* list;      // sites sorted by (colour, id)
+  const float* K_site;      // n or nullptr
+  const float* e_site;      // 3n or nullptr
+};
+
+// diagnostics of one sweep
+struct Diag {
+  uint8_t* accept;                  // n bytes (canonical id) or nullptr
+  unsigned long long* n_accept;     // or nullptr
+};
+
+// ---- kernels (hb_kernels.cu); every launcher returns the launch status -----------------
+cudaError_t launch_init_random_sc(cudaStream_t st, float* spins, ScLayout L, uint32_t seed_lo, uint32_t seed_hi);
+cudaError_t launch_init_random_flat(cudaStream_t st, float* spins, uint32_t n, uint32_t seed_lo, uint32_t seed_hi);
+cudaError_t launch_fill(cudaStream_t st, float* spins, uint32_t n, float x, float y, float z);
+cudaError_t launch_sc_permute(cudaStream_t st, float* dst, const float* src, ScLayout L, bool to_internal);
+cudaError_t launch_sweep_sc(cudaStream_t st, float* spins, ScLayout L, ScTile t, SweepParams p, int colour, Diag d);
+cudaError_t launch_sweep_csr(cudaStream_t st, float* spins, CsrDev g, uint32_t list_begin, uint32_t list_count,
+                             SweepParams p, int block, Diag d);
+// measurement: partials must hold kMeasureBlocks*4 doubles; out receives (Mx*N, My*N, Mz*N, E)
+constexpr int kMeasureBlocks = 1184;
+cudaError_t launch_measure_sc(cudaStream_t st, const float* spins, ScLayout L, int V, SweepParams p, double* partials, double* out);
+cudaError_t launch_measure_csr(cudaStream_t st, const float* spins, CsrDev g, SweepParams p, double* partials, double* out);
+
+// ---- host lattice tables (hb_lattice.cpp) -------------------------------------------------
+struct HostCsr {
+  int64_t n = 0;
+  std::vector<int64_t> row_ptr;
+  std::vector<int32_t> col;
+  std::vector<int32_t> colour;
+  int32_t n_colours = 0;
+};
+void build_bcc_csr(int32_t Lx, int32_t Ly, int32_t Lz, HostCsr& out);
+void build_fcc_csr(int32_t Lx, int32_t Ly, int32_t Lz, HostCsr& out);
+void build_fcc_sphere_csr(int32_t R, HostCsr& out, std::vector<int32_t>& xyz);
+void greedy_first_fit(HostCsr& g);
+// empty string = valid; otherwise what is wrong
+std::string validate_csr(int64_t n, const int64_t* row_ptr, const int32_t* col);
+std::string validate_colouring(int64_t n, const int64_t* row_ptr, const int32_t* col, const int32_t* colour,
+                               int32_t n_colours);
+
+}  // namespace hb

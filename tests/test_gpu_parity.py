@@ -1,0 +1,212 @@
+"""GPU-vs-oracle parity through the C ABI.
+
+Bar (BASELINE.json north_star): identical accept/reject decisions on >= 99.9999 % of the
+attempts of the first 10 sweeps, max |dS_component| <= 1e-5 on agreeing sites.  With the
+arithmetic contract of DESIGN.md section 4 the expected result is 100 % and 0.0; the
+small cases assert exactly that, the full-size cases assert the bar and print the counts.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_2106_11286_b200 as hb
+from paper_2106_11286_b200 import workloads as W
+
+from hbtest import compare_trajectory, make_gpu, make_oracle, spins_equal, start
+
+pytestmark = pytest.mark.gpu
+
+
+def _bar(attempts, mism, max_ds):
+    assert mism <= 1e-6 * attempts, (attempts, mism)
+    assert max_ds <= 1e-5, max_ds
+
+
+def _measure_close(ctx, st, n):
+    Mg, Eg = ctx.measure()
+    Mo, Eo32, Eo64 = st.measure()
+    assert np.max(np.abs(Mg - Mo)) <= 1e-7                      # P2
+    assert abs(Eg - Eo32) <= 1e-6 * n and abs(Eg - Eo64) <= 1e-6 * n
+
+
+SMALL_CASES = {
+    "sc16_c1": W.SMALL["c1"],
+    "sc24_K": W.SMALL["c4"],
+    "sc_v2_ragged": dict(W.SMALL["c4"], L=(12, 10, 6), K=0.3, e=(0.6, 0.0, 0.8)),
+    "sc_v1": dict(W.SMALL["c4"], L=(6, 4, 2), K=-0.2, e=(0.0, 1.0, 0.0)),
+    "sc_L2": dict(W.SMALL["c4"], L=2, K=0.2),
+    "sc_wide": dict(W.SMALL["c4"], L=(528, 6, 4)),
+    "bcc8": W.SMALL["c2"],
+    "bcc_ragged": dict(W.SMALL["c2"], L=(3, 4, 5)),
+    "fcc6": W.SMALL["c3"],
+    "fcc_ragged": dict(W.SMALL["c3"], L=(5, 3, 4), start="random"),
+    "sphere5": W.SMALL["c5"],
+    "sphere5_parity": dict(W.SMALL["c5"], colouring="parity"),
+}
+
+
+@pytest.mark.parametrize("name", sorted(SMALL_CASES))
+def test_small_trajectories_bit_exact(name):
+    cfg = SMALL_CASES[name]
+    ctx = make_gpu(cfg)
+    lat, st = make_oracle(cfg)
+    assert ctx.n == lat.n
+    col, nc = ctx.colouring()
+    assert nc == lat.n_colours and np.array_equal(col, lat.colour)
+    start(cfg, ctx, st)
+    assert spins_equal(ctx.get_spins(), st.get_spins())          # a3: same initial state
+    for T in (cfg["T"][0], 0.3):
+        attempts, mism, max_ds, differ = compare_trajectory(cfg, ctx, st, T, 5)
+        assert attempts == 5 * lat.n and mism == 0 and max_ds == 0.0 and differ == 0
+        _measure_close(ctx, st, lat.n)
+    assert ctx.sweep_count == st.sweep_count == 10
+    # the production kernels (no recording) walk the same trajectory
+    ctx.sweep(1.0, 7)
+    st.sweep(1.0, 7)
+    assert spins_equal(ctx.get_spins(), st.get_spins())
+    ctx.close()
+
+
+def test_sc_tile_shapes_do_not_change_the_result():
+    cfg = dict(W.SMALL["c4"], L=(40, 12, 10))
+    lat, st = make_oracle(cfg)
+    st.init_random()
+    st.sweep(1.44, 3)
+    want = st.get_spins()
+    for v, jx, ty, zt in [(4, 5, 12, 10), (4, 3, 5, 3), (4, 1, 1, 1), (2, 10, 7, 4), (1, 20, 12, 2), (4, 5, 51, 10)]:
+        ctx = make_gpu(cfg)
+        ctx.set_option("sc_v", v)
+        ctx.set_option("sc_jx", jx)
+        ctx.set_option("sc_ty", ty)
+        ctx.set_option("sc_zt", zt)
+        ctx.init_random()
+        ctx.sweep(1.44, 3)
+        assert spins_equal(ctx.get_spins(), want), (v, jx, ty, zt)
+        ctx.close()
+
+
+def test_random_graph_greedy_colouring_and_per_site_anisotropy():
+    n = 5000
+    rp, ci = W.random_csr_graph(n, 7.0, seed=3)
+    rng = np.random.default_rng(4)
+    cfg = dict(kind="csr", row_ptr=rp, col_idx=ci, J=0.8, K=0.0, e=(0, 0, 1), seed=77, start="random",
+               K_site=rng.uniform(-0.5, 0.5, n).astype(np.float32), e_site=W.random_unit_vectors(n, 5))
+    ctx = make_gpu(cfg)
+    lat, st = make_oracle(cfg)
+    col, nc = ctx.colouring()                                    # both sides ran first-fit on their own
+    assert nc == lat.n_colours and np.array_equal(col, lat.colour)
+    start(cfg, ctx, st)
+    attempts, mism, max_ds, differ = compare_trajectory(cfg, ctx, st, 0.9, 6)
+    assert mism == 0 and max_ds == 0.0 and differ == 0
+    _measure_close(ctx, st, n)
+    # isolated sites and an empty colour are legal
+    rp2 = np.zeros(11, np.int64)
+    cfg2 = dict(kind="csr", row_ptr=rp2, col_idx=np.zeros(0, np.int32), colour=np.full(10, 2, np.int32), n_colours=4,
+                J=1.0, K=0.7, e=(0, 0, 1), seed=5, start="random")
+    c2 = make_gpu(cfg2)
+    l2, s2 = make_oracle(cfg2)
+    start(cfg2, c2, s2)
+    assert compare_trajectory(cfg2, c2, s2, 0.5, 4)[1:] == (0, 0.0, 0)
+
+
+def test_set_get_spins_and_checkpoint_identity():
+    cfg = W.SMALL["c4"]
+    lat, st = make_oracle(cfg)
+    S = W.random_unit_vectors(lat.n, 9)
+    a = make_gpu(cfg)
+    a.set_spins(S[:, 0], S[:, 1], S[:, 2])
+    back = a.get_spins()
+    assert all(np.array_equal(back[k], S[:, k]) for k in range(3))     # layout round trip
+    st.set_spins(S[:, 0], S[:, 1], S[:, 2])
+    _measure_close(a, st, lat.n)
+    a.sweep(1.44, 6)
+    b = make_gpu(cfg)
+    b.set_spins(S[:, 0], S[:, 1], S[:, 2])
+    b.sweep(1.44, 3)
+    c = make_gpu(cfg)                                                   # K12: resume from (spins, counter)
+    c.set_spins(*b.get_spins())
+    c.sweep_count = b.sweep_count
+    c.sweep(1.44, 3)
+    assert spins_equal(a.get_spins(), c.get_spins())
+    st.sweep(1.44, 6)
+    assert spins_equal(a.get_spins(), st.get_spins())
+
+
+def test_c1_full_series():
+    # config 1 as specified: sc 16^3, K=0, T=1.2, 1000 sweeps, M and E every sweep
+    cfg = W.CONFIGS["c1"]
+    ctx = make_gpu(cfg)
+    lat, st = make_oracle(cfg)
+    start(cfg, ctx, st)
+    Mg, Eg = ctx.sweep_series(1.2, 1000)
+    Mo, Eo = st.series(1.2, 1000)
+    assert spins_equal(ctx.get_spins(), st.get_spins())
+    assert np.max(np.abs(Mg - Mo)) <= 1e-7
+    assert np.max(np.abs(Eg - Eo)) <= 1e-6 * lat.n
+    nrm = sum(x.astype(np.float64) ** 2 for x in ctx.get_spins())
+    assert np.max(np.abs(nrm - 1.0)) <= 5e-7                            # K3
+    launches, attempts = ctx.counters()
+    assert attempts == 1000 * lat.n and launches >= 2000
+
+
+def test_limits_on_device():
+    cfg = dict(W.SMALL["c4"], L=16)
+    ctx = make_gpu(cfg)
+    ctx.init_aligned((0, 0, 1))
+    acc = ctx.sweep_record(float("inf"))                                # K8: T = inf accepts everything
+    assert acc.min() == 1 and acc.max() == 1
+    M, _ = ctx.sweep_series(float("inf"), 100)
+    absM = np.linalg.norm(M, axis=1)
+    assert abs(absM.mean() - math.sqrt(8 / (3 * math.pi * ctx.n))) < 4 * absM.std(ddof=1) / 10
+    ctx.init_aligned((0, 0, 1))
+    ctx.sweep(0.01, 20)                                                 # K9: T -> 0 stays ordered
+    M, E = ctx.measure()
+    assert np.linalg.norm(M) > 0.99 and E / ctx.n < -2.98
+
+
+def test_error_paths():
+    with pytest.raises(hb.HbError):
+        hb.Context(hb.Lattice("sc", 15))                                # odd L
+    with pytest.raises(hb.HbError):
+        hb.Context(hb.Lattice("sc", 8), e=(0, 0, 2))                    # non-unit axis
+    rp = np.array([0, 1, 1], np.int64)
+    with pytest.raises(hb.HbError):
+        hb.Context(hb.Lattice("csr", row_ptr=rp, col_idx=np.array([1], np.int32)))   # asymmetric
+    rp = np.array([0, 1, 2], np.int64)
+    with pytest.raises(hb.HbError):
+        hb.Context(hb.Lattice("csr", row_ptr=rp, col_idx=np.array([1, 0], np.int32),
+                              colour=np.zeros(2, np.int32), n_colours=1))             # improper colouring
+    ctx = hb.Context(hb.Lattice("sc", 8))
+    with pytest.raises(hb.HbError):
+        ctx.sweep(1.0, 1)                                               # before init
+    ctx.init_random()
+    for T in (0.0, -1.0, float("nan")):
+        with pytest.raises(hb.HbError):
+            ctx.sweep(T, 1)
+    ctx.sweep(1.0, 0)                                                   # no-op
+    assert ctx.sweep_count == 0
+
+
+# ---- full-size configs: first 10 sweeps, every attempt ------------------------------------------
+@pytest.mark.parametrize("name", ["c2", "c3", "c5", "c4"])
+def test_full_size_first_10_sweeps(name):
+    cfg = W.CONFIGS[name]
+    ctx = make_gpu(cfg)
+    lat, st = make_oracle(cfg)
+    start(cfg, ctx, st)
+    T = cfg["T"][0]
+    attempts, mism, max_ds, differ = compare_trajectory(cfg, ctx, st, T, 10)
+    print("%s: N=%d attempts=%d decision mismatches=%d max|dS|=%g differing sites=%d"
+          % (name, lat.n, attempts, mism, max_ds, differ))
+    assert attempts == 10 * lat.n
+    _bar(attempts, mism, max_ds)
+    if mism == 0:
+        assert differ == 0
+    _measure_close(ctx, st, lat.n)
+    # the timed launch configuration (hb_sweep, no recording) continues the same trajectory
+    ctx.sweep(T, 2)
+    st.sweep(T, 2)
+    if mism == 0:
+        assert spins_equal(ctx.get_spins(), st.get_spins())
