@@ -1,0 +1,341 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the Metropolis colour sweep on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c4]
+
+One "step" is one pass of the whole hot path over the resident lattice: SWEEPS_PER_STEP
+Metropolis sweeps (one kernel per colour per sweep: SURVEY 8(a) rows a4, a6) followed by
+one M/E measurement (row a5).  Lattice build, colouring and the initial state (rows a1-a3)
+are set-up, done once before the warm-up.
+
+Workload at N = 1: config 4 of BASELINE.json, simple cubic L = 464 (99,897,344 spins, 1.2 GB
+of fp32 SoA state, far larger than the 126 MB L2, so no flush between iterations), J = 1,
+K = 0.01 along z, random start from seed 1, T = 1.44.  With N > 1 every rank runs an
+independent replica of that workload (seed + rank): the path has no multi-GPU exchange in
+scope ("replicas only"), so scaling is weak and there is no collective
+on the data path.
+
+Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle instead (the tier's
+reference arm): single-threaded, on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+SWEEPS_PER_STEP = 10
+METRIC = "attempted spin updates/sec (Gupd/s) and % of HBM roofline, 1 B200"
+UNIT = "Gupd/s"
+
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant kernel,
+# from the `ncu --set full` capture summarised in profiles/ (file named beside each value).
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {}
+try:
+    with open(os.path.join(ROOT, "profiles", "traffic.csv")) as _f:
+        for _ln in _f:
+            if _ln.strip() and not _ln.startswith("#"):
+                _k, _v = _ln.split(",")[:2]
+                NCU_TRAFFIC_BYTES_PER_LAUNCH[_k.strip()] = float(_v)
+except OSError:
+    pass
+
+
+def algorithmic_bytes_per_update(cfg, n_colours):
+    """SURVEY 8(d) / DESIGN.md section 7: what one colour pass must move, per attempted update."""
+    if cfg["kind"] in ("sc", "bcc"):
+        return 36.0      # read own 12 B + the other colour once 12 B + write own 12 B
+    if cfg["kind"] == "fcc":
+        return 60.0      # own 12 + three other sublattices 36 + write 12
+    return 12.0 * (n_colours + 1) + 48.0 + 8.0 + 16.0   # CSR z~12: spins, col_idx, row_ptr, (K_i, e_i)
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.FIELDS,
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.f:
+            c = [x.strip() for x in ln.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1]))
+            except ValueError:
+                continue
+            for name, v in zip(names, c[3:7]):
+                if v == "Active":
+                    reasons.add(name)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def make_context(cfg, seed_offset, device):
+    import paper_2106_11286_b200 as hb
+    if cfg["kind"] == "sphere":
+        lat = hb.Lattice.fcc_sphere(cfg["R"], cfg["K"], cfg["e"], cfg["K_surf"], cfg.get("colouring", "greedy"))
+    else:
+        lat = hb.Lattice(cfg["kind"], cfg["L"])
+    ctx = hb.Context(lat, cfg["J"], cfg["K"], cfg["e"], cfg["seed"] + seed_offset, device=device)
+    if cfg["start"] == "random":
+        ctx.init_random()
+    else:
+        ctx.init_aligned(cfg["e"])
+    return ctx
+
+
+def cpu_sample_cfg(cfg):
+    """A bounded sample of the workload for the single-threaded oracle (about 10-30 s of CPU work)."""
+    if cfg["kind"] == "sc" and cfg["L"] > 232:
+        return dict(cfg, L=232), "sc L=232 (1/8 of the L=464 volume), same J, K, e, T, random start"
+    if cfg["kind"] == "fcc" and cfg["L"] > 64:
+        return dict(cfg, L=64), "fcc L=64 (1/8 of the volume), same parameters"
+    if cfg["kind"] == "sphere" and cfg["R"] > 30:
+        return dict(cfg, R=30), "fcc sphere R=30 (1/8 of the volume), same parameters"
+    return dict(cfg), "the full workload"
+
+
+def make_oracle_state(cfg):
+    import oracle
+    if cfg["kind"] == "sphere":
+        lat = oracle.Lattice.fcc_sphere(cfg["R"], cfg["K"], cfg["e"], cfg["K_surf"], cfg.get("colouring", "greedy"))
+    else:
+        lat = getattr(oracle.Lattice, cfg["kind"])(cfg["L"])
+        lat.set_uniform_anisotropy(cfg["K"], cfg["e"])
+    st = oracle.State32(lat, cfg["J"], cfg["seed"])
+    if cfg["start"] == "random":
+        st.init_random()
+    else:
+        st.init_aligned(cfg["e"])
+    return lat, st
+
+
+def run_cpu_baseline(cfg, budget_attempts=1.0e8):
+    scfg, what = cpu_sample_cfg(cfg)
+    lat, st = make_oracle_state(scfg)
+    T = scfg["T"][0]
+    n = lat.n
+    sweeps = max(1, int(round(budget_attempts / n)))
+    st.sweep(T, 1)
+    t0 = time.perf_counter()
+    st.sweep(T, sweeps)
+    st.measure()
+    dt = time.perf_counter() - t0
+    return {"value": n * sweeps / dt / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": "%s; %d sweeps + 1 measurement (%d attempts), O32 single thread" % (what, sweeps, n * sweeps),
+            "ns_per_update": dt / (n * sweeps) * 1e9}
+
+
+def run_reference(args, cfg, name):
+    """--impl reference: the CPU oracle as it stands, one sweep of the bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    scfg, what = cpu_sample_cfg(cfg)
+    lat, st = make_oracle_state(scfg)
+    T = scfg["T"][0]
+    for _ in range(args.warmup):
+        st.sweep(T, 1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        st.sweep(T, 1)
+        st.measure()
+    dt = time.perf_counter() - t0
+    value = lat.n * args.steps / dt / 1e9
+    sample = "%s; each step = 1 sweep + 1 measurement of the sample, O32 single thread" % what
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": name, "lattice": "%s %s" % (cfg["kind"], cfg.get("L", cfg.get("R"))),
+                   "T": T, "J": cfg["J"], "K": cfg["K"]},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c4", help="c1..c5 (BASELINE.json configs); the headline is c4")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    from paper_2106_11286_b200 import workloads
+    cfg = workloads.CONFIGS[args.workload]
+    if args.impl == "reference":
+        return run_reference(args, cfg, args.workload)
+
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU path")
+    device = "cuda:%d" % local
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(device))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    ctx = make_context(cfg, rank, device)
+    T = cfg["T"][0]
+    n = ctx.n
+    _, n_colours = ctx.colouring()
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def timed_run(steps):
+        """K steps; returns (region ms by CUDA events, ms inside hb_sweep only, kernel launches)."""
+        l0, _ = ctx.counters()
+        e0, e1 = ev(), ev()
+        marks = []
+        barrier()
+        e0.record()
+        for _ in range(steps):
+            a, b = ev(), ev()
+            a.record()
+            ctx.sweep(T, SWEEPS_PER_STEP)
+            b.record()
+            ctx.measure()
+            marks.append((a, b))
+        e1.record()
+        barrier()
+        l1, _ = ctx.counters()
+        return e0.elapsed_time(e1), sum(a.elapsed_time(b) for a, b in marks), l1 - l0
+
+    for _ in range(args.warmup):
+        ctx.sweep(T, SWEEPS_PER_STEP)
+        ctx.measure()
+    clocks = None
+    for attempt in range(2):
+        sampler = ClockSampler(local) if rank == 0 else None
+        ms, ms_sweeps, launches = timed_run(args.steps)
+        clocks = sampler.stop() if sampler else None
+        bad = clocks and any(r in clocks["reasons"] for r in ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"))
+        if not bad:
+            break
+    if world > 1:
+        t = torch.tensor([ms, ms_sweeps], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, ms_sweeps = float(t[0]), float(t[1])
+        lt = torch.tensor([launches], device=device, dtype=torch.int64)
+        dist.all_reduce(lt, op=dist.ReduceOp.SUM)
+        launches = int(lt[0])
+    updates = float(n) * SWEEPS_PER_STEP * args.steps * world
+    value = updates / (ms * 1e-3) / 1e9
+
+    # ---- end to end through the public API with HOST buffers ------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        host = [torch.empty(n, dtype=torch.float32).pin_memory() for _ in range(3)]
+        ctx.get_spins(out=host)
+        e2e_steps = max(1, min(args.steps, 10))
+        for _ in range(2):
+            ctx.set_spins(*host); ctx.sweep(T, SWEEPS_PER_STEP); ctx.measure()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            ctx.set_spins(*host)                     # H2D of the step's input state (pinned host memory)
+            ctx.sweep(T, SWEEPS_PER_STEP)
+            ctx.measure()                            # D2H of the step's result (M, E)
+        barrier()
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], device=device, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t[0])
+        e2e = {"value": float(n) * SWEEPS_PER_STEP * e2e_steps * world / dt / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": 3 * n * 4, "d2h_bytes_per_step": 32, "steps": e2e_steps}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (one colour pass) -----------------------------------------
+    peak, peak_src = measured_peaks()
+    bytes_per_update = algorithmic_bytes_per_update(cfg, n_colours)
+    launches_sweep = n_colours * SWEEPS_PER_STEP * args.steps
+    avg_launch_s = ms_sweeps * 1e-3 / launches_sweep
+    bytes_per_launch = bytes_per_update * n / n_colours
+    achieved = bytes_per_launch / avg_launch_s / 1e9
+    kernel = {"sc": "k_sweep_sc", "bcc": "k_sweep_csr", "fcc": "k_sweep_csr", "sphere": "k_sweep_csr"}[cfg["kind"]]
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.workload), "kernel": kernel, "peak_source": peak_src,
+                "algorithmic_bytes_per_update": bytes_per_update, "bytes_per_launch": bytes_per_launch,
+                "avg_launch_ms": avg_launch_s * 1e3, "frac_of_8TBs_nominal": achieved / 8000.0}
+
+    cpu = None if args.no_cpu_baseline else run_cpu_baseline(cfg)
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": args.workload,
+                   "lattice": "%s %s" % (cfg["kind"], cfg.get("L", cfg.get("R"))), "n_spins": n, "colours": n_colours,
+                   "J": cfg["J"], "K": cfg["K"], "T": T, "start": cfg["start"], "seed": cfg["seed"],
+                   "sweeps_per_step": SWEEPS_PER_STEP, "measurements_per_step": 1,
+                   "l2": "state %.0f MB >> 126 MB L2: no flush between iterations" % (12.0 * n / 1e6)
+                   if 12.0 * n > 4 * 126e6 else "state fits in L2: HBM roofline not meaningful",
+                   "multi_gpu": "replicas only (seed + rank)"},
+        "ns_per_update": 1.0 / value, "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
+        "roofline": roofline, "cpu_baseline": cpu,
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
