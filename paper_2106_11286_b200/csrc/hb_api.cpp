@@ -85,6 +85,8 @@ struct hb_ctx {
   ScTile tile{};
   CsrDev csr{};
   int csr_block = 128;
+  int sc_kernel = 0;      // 0: direct loads through L1, 1: neighbour planes staged in shared memory
+  int staged_zt = 16;
   std::vector<uint32_t> colour_begin;     // CSR engine: offsets into the colour-sorted list
   std::vector<int32_t> colour_host;       // CSR engine: colour of every site
   int32_t n_colours = 0;
@@ -144,6 +146,7 @@ bool unit_vector(const float* v) {
 // default launch shape of the sc kernels for a lattice
 ScTile default_tile(const ScLayout& L) {
   ScTile t;
+  t.PF = 1;
   t.V = (L.H % 4 == 0) ? 4 : ((L.H % 2 == 0) ? 2 : 1);
   const int HV = L.H / t.V;
   int best = HV <= 64 ? HV : 64, best_waste = 1 << 30;
@@ -166,7 +169,10 @@ ScTile default_tile(const ScLayout& L) {
 
 int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d) {
   if (c->plan.engine == ENGINE_SC) {
-    HB_CUDA(c, launch_sweep_sc(c->stream, c->spins, c->sc, c->tile, p, colour, d));
+    if (c->sc_kernel == 1)
+      HB_CUDA(c, launch_sweep_sc_staged(c->stream, c->spins, c->sc, c->staged_zt, p, colour, d));
+    else
+      HB_CUDA(c, launch_sweep_sc(c->stream, c->spins, c->sc, c->tile, p, colour, d));
   } else {
     const uint32_t b = c->colour_begin[colour], e = c->colour_begin[colour + 1];
     if (e == b) return HB_OK;
@@ -297,6 +303,8 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
     c->sc.Lx = lat->Lx; c->sc.Ly = lat->Ly; c->sc.Lz = lat->Lz;
     c->sc.H = lat->Lx / 2; c->sc.n = (uint32_t)P.n; c->sc.half = (uint32_t)(P.n / 2);
     c->tile = default_tile(c->sc);
+    c->sc_kernel = 0;   // measured on B200: direct + L2 prefetch 141 Gupd/s, staged 135
+    c->staged_zt = c->sc.Lz < 16 ? c->sc.Lz : 16;
   }
 
   // ---- device memory --------------------------------------------------------------------------
@@ -538,6 +546,17 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
     return HB_OK;
   }
   if (c->plan.engine != ENGINE_SC) return fail(c, HB_EINVAL, "option not valid for this lattice");
+  if (s == "sc_kernel") {
+    if (value != 0 && !(value == 1 && sc_staged_supported(c->sc)))
+      return fail(c, HB_EINVAL, "sc_kernel: 0 (direct) or 1 (staged; needs Lx % 8 == 0 and Lx <= 512)");
+    c->sc_kernel = (int)value;
+    return HB_OK;
+  }
+  if (s == "sc_staged_zt") {
+    if (value < 1 || value > c->sc.Lz) return fail(c, HB_EINVAL, "sc_staged_zt: 1..Lz");
+    c->staged_zt = (int)value;
+    return HB_OK;
+  }
   ScTile t = c->tile;
   if (s == "sc_v") {
     if (!(value == 1 || value == 2 || value == 4) || c->sc.H % value) return fail(c, HB_EINVAL, "sc_v: 1, 2 or 4 dividing Lx/2");
@@ -546,6 +565,7 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
   } else if (s == "sc_jx") t.JX = (int)value;
   else if (s == "sc_ty") t.TY = (int)value;
   else if (s == "sc_zt") t.ZT = (int)value;
+  else if (s == "sc_prefetch") { if (value < 0 || value > 3) return fail(c, HB_EINVAL, "sc_prefetch: 0..3"); t.PF = (int)value; }
   else return fail(c, HB_EINVAL, "unknown option");
   if (t.JX < 1 || t.TY < 1 || t.ZT < 1 || (int64_t)t.JX * t.TY > 256 || t.ZT > c->sc.Lz)
     return fail(c, HB_EINVAL, "sc tile: JX, TY, ZT >= 1, JX*TY <= 256, ZT <= Lz");
@@ -561,7 +581,10 @@ int hb_get_option(hb_ctx* c, const char* name, int64_t* value) {
   else if (s == "sc_jx") *value = c->tile.JX;
   else if (s == "sc_ty") *value = c->tile.TY;
   else if (s == "sc_zt") *value = c->tile.ZT;
+  else if (s == "sc_prefetch") *value = c->tile.PF;
   else if (s == "engine") *value = c->plan.engine;
+  else if (s == "sc_kernel") *value = c->sc_kernel;
+  else if (s == "sc_staged_zt") *value = c->staged_zt;
   else return HB_EINVAL;
   return HB_OK;
 }

@@ -27,6 +27,7 @@ struct ScLayout {
 // consecutive same-colour sites of one x-row and marches ZT planes in z
 struct ScTile {
   int32_t V, JX, TY, ZT;
+  int32_t PF;   // software prefetch of the next z-plane: 0 none, 1 L2, 2 L1, 3 touch
 };
 
 // CSR tables on the device
@@ -51,6 +52,8 @@ cudaError_t launch_init_random_flat(cudaStream_t st, float* spins, uint32_t n, u
 cudaError_t launch_fill(cudaStream_t st, float* spins, uint32_t n, float x, float y, float z);
 cudaError_t launch_sc_permute(cudaStream_t st, float* dst, const float* src, ScLayout L, bool to_internal);
 cudaError_t launch_sweep_sc(cudaStream_t st, float* spins, ScLayout L, ScTile t, SweepParams p, int colour, Diag d);
+bool sc_staged_supported(const ScLayout& L);
+cudaError_t launch_sweep_sc_staged(cudaStream_t st, float* spins, ScLayout L, int ZT, SweepParams p, int colour, Diag d);
 cudaError_t launch_sweep_csr(cudaStream_t st, float* spins, CsrDev g, uint32_t list_begin, uint32_t list_count,
                              SweepParams p, int block, Diag d);
 // measurement: partials must hold kMeasureBlocks*4 doubles; out receives (Mx*N, My*N, Mz*N, E)

@@ -86,12 +86,13 @@ __device__ __forceinline__ Vec<V> sc_field(const float* __restrict__ b, const Sc
 }
 
 // one Metropolis attempt (steps ii-iii of the paper) on registers; returns the decision
+template <int ANISO = ANISO_GENERAL>
 __device__ __forceinline__ bool attempt(uint32_t site, const SweepParams& P, float K, float ex, float ey, float ez,
                                         float hx, float hy, float hz, float& sx, float& sy, float& sz) {
   const Rand4 r = philox4x32_10(site, 0u, P.sweep_lo, P.sweep_hi, P.seed_lo, P.seed_hi);
   float nx, ny, nz;
   sphere(r.r0, r.r1, nx, ny, nz);
-  const float dH = delta_h(sx, sy, sz, nx, ny, nz, hx, hy, hz, P.J, K, ex, ey, ez);
+  const float dH = delta_h_t<ANISO>(sx, sy, sz, nx, ny, nz, hx, hy, hz, P.J, K, ex, ey, ez);
   const bool acc = metropolis_accept(dH, P.beta, r.r2);
   sx = acc ? nx : sx;
   sy = acc ? ny : sy;
@@ -99,8 +100,54 @@ __device__ __forceinline__ bool attempt(uint32_t site, const SweepParams& P, flo
   return acc;
 }
 
-template <int V, bool DIAG>
-__global__ void __launch_bounds__(256)
+#ifndef HB_SC_MINBLOCKS
+#define HB_SC_MINBLOCKS 4
+#endif
+// Software prefetch of the lines the NEXT z-plane of the march touches for the first time:
+// PF 0 none, 1 prefetch.global.L2, 2 prefetch.global.L1, 3 a real load into a register nobody reads.
+template <int PF>
+__device__ __forceinline__ void prefetch_line(const float* p) {
+  if (PF == 1) asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+  if (PF == 2) asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
+  if (PF == 3) { float t; asm volatile("ld.global.ca.f32 %0, [%1];" : "=f"(t) : "l"(p)); }
+}
+
+// Neighbour field from 32-bit element offsets into one component plane of the other colour.
+template <int V>
+__device__ __forceinline__ Vec<V> sc_field_off(const float* __restrict__ b, uint32_t oc, uint32_t oh, uint32_t oym,
+                                               uint32_t oyp, uint32_t ozm, uint32_t ozp, int32_t p) {
+  const Vec<V> c = load_ro<V>(b + oc);
+  const float halo = __ldg(b + oh);
+  const Vec<V> ym = load_ro<V>(b + oym);
+  const Vec<V> yp = load_ro<V>(b + oyp);
+  const Vec<V> zm = load_ro<V>(b + ozm);
+  const Vec<V> zp = load_ro<V>(b + ozp);
+  Vec<V> h;
+  if (V >= 2) {           // packed fp32x2 adds: same rounding per element, half the instructions
+#pragma unroll
+    for (int k = 0; k + 1 < V; k += 2) {
+      const float lo0 = (k == 0) ? halo : c.v[k > 0 ? k - 1 : 0], lo1 = c.v[k];
+      const float hi0 = c.v[k + 1], hi1 = (k + 1 == V - 1) ? halo : c.v[k + 2 < V ? k + 2 : 0];
+      f2 s2 = add2(make_float2(c.v[k], c.v[k + 1]), make_float2(p ? hi0 : lo0, p ? hi1 : lo1));
+      s2 = add2(s2, make_float2(ym.v[k], ym.v[k + 1]));
+      s2 = add2(s2, make_float2(yp.v[k], yp.v[k + 1]));
+      s2 = add2(s2, make_float2(zm.v[k], zm.v[k + 1]));
+      s2 = add2(s2, make_float2(zp.v[k], zp.v[k + 1]));
+      h.v[k] = s2.x; h.v[k + 1] = s2.y;
+    }
+  } else {
+    float s = __fadd_rn(c.v[0], halo);
+    s = __fadd_rn(s, ym.v[0]);
+    s = __fadd_rn(s, yp.v[0]);
+    s = __fadd_rn(s, zm.v[0]);
+    s = __fadd_rn(s, zp.v[0]);
+    h.v[0] = s;
+  }
+  return h;
+}
+
+template <int V, int ANISO, bool DIAG, int PF>
+__global__ void __launch_bounds__(256, HB_SC_MINBLOCKS)
 k_sweep_sc(float* __restrict__ ax, float* __restrict__ ay, float* __restrict__ az,
            const float* __restrict__ bx, const float* __restrict__ by, const float* __restrict__ bz,
            ScLayout L, ScTile t, SweepParams P, int colour, Diag d) {
@@ -109,39 +156,211 @@ k_sweep_sc(float* __restrict__ ax, float* __restrict__ ay, float* __restrict__ a
   const int32_t y = blockIdx.y * t.TY + ty;
   const int32_t i0 = j * V;
   if (i0 >= L.H || y >= L.Ly) return;
-  const int32_t ym = (y == 0) ? L.Ly - 1 : y - 1;
-  const int32_t yp = (y == L.Ly - 1) ? 0 : y + 1;
+  const uint32_t H = (uint32_t)L.H, plane = (uint32_t)L.Ly * H;
+  const uint32_t ym = (uint32_t)((y == 0) ? L.Ly - 1 : y - 1) * H + (uint32_t)i0;
+  const uint32_t yp = (uint32_t)((y == L.Ly - 1) ? 0 : y + 1) * H + (uint32_t)i0;
+  const uint32_t yc = (uint32_t)y * H + (uint32_t)i0;
   const int32_t z0 = blockIdx.z * t.ZT;
   const int32_t z1 = min(z0 + t.ZT, L.Lz);
   unsigned n_acc = 0;
   for (int32_t z = z0; z < z1; ++z) {
-    const int32_t zm = (z == 0) ? L.Lz - 1 : z - 1;
-    const int32_t zp = (z == L.Lz - 1) ? 0 : z + 1;
+    const uint32_t pz = (uint32_t)z * plane;
+    const uint32_t pzm = (uint32_t)((z == 0) ? L.Lz - 1 : z - 1) * plane;
+    const uint32_t pzp = (uint32_t)((z == L.Lz - 1) ? 0 : z + 1) * plane;
     const int32_t p = (colour + y + z) & 1;
-    const uint32_t row_c = (uint32_t)(z * L.Ly + y) * L.H;
-    const uint32_t row_ym = (uint32_t)(z * L.Ly + ym) * L.H, row_yp = (uint32_t)(z * L.Ly + yp) * L.H;
-    const uint32_t row_zm = (uint32_t)(zm * L.Ly + y) * L.H, row_zp = (uint32_t)(zp * L.Ly + y) * L.H;
-    const Vec<V> hx = sc_field<V>(bx, L, row_c, row_ym, row_yp, row_zm, row_zp, i0, p);
-    const Vec<V> hy = sc_field<V>(by, L, row_c, row_ym, row_yp, row_zm, row_zp, i0, p);
-    const Vec<V> hz = sc_field<V>(bz, L, row_c, row_ym, row_yp, row_zm, row_zp, i0, p);
-    Vec<V> sx = load_rw<V>(ax + row_c + i0), sy = load_rw<V>(ay + row_c + i0), sz = load_rw<V>(az + row_c + i0);
+    int32_t ih = p ? V : -1;                          // the one element outside [i0, i0+V), periodic in x
+    ih = (i0 + ih < 0) ? ih + L.H : ((i0 + ih >= L.H) ? ih - L.H : ih);
+    const uint32_t oc = pz + yc, oh = oc + (uint32_t)ih, oym = pz + ym, oyp = pz + yp, ozm = pzm + yc, ozp = pzp + yc;
+    Vec<V> sx = load_rw<V>(ax + oc), sy = load_rw<V>(ay + oc), sz = load_rw<V>(az + oc);
+    const Vec<V> hx = sc_field_off<V>(bx, oc, oh, oym, oyp, ozm, ozp, p);
+    const Vec<V> hy = sc_field_off<V>(by, oc, oh, oym, oyp, ozm, ozp, p);
+    const Vec<V> hz = sc_field_off<V>(bz, oc, oh, oym, oyp, ozm, ozp, p);
+    if (PF != 0 && z + 1 < z1) {
+      const uint32_t zpp = (uint32_t)((z + 2 >= L.Lz) ? z + 2 - L.Lz : z + 2) * plane + yc;
+      prefetch_line<PF>(ax + pzp + yc); prefetch_line<PF>(ay + pzp + yc); prefetch_line<PF>(az + pzp + yc);
+      prefetch_line<PF>(bx + pzp + ym); prefetch_line<PF>(by + pzp + ym); prefetch_line<PF>(bz + pzp + ym);
+      prefetch_line<PF>(bx + pzp + yp); prefetch_line<PF>(by + pzp + yp); prefetch_line<PF>(bz + pzp + yp);
+      prefetch_line<PF>(bx + zpp); prefetch_line<PF>(by + zpp); prefetch_line<PF>(bz + zpp);
+    }
     const uint32_t site0 = (uint32_t)(z * L.Ly + y) * (uint32_t)L.Lx + 2u * (uint32_t)i0 + (uint32_t)p;
     bool any = false;
+    if (V >= 2) {
 #pragma unroll
-    for (int k = 0; k < V; ++k) {
-      const bool acc = attempt(site0 + 2u * k, P, P.K, P.ex, P.ey, P.ez, hx.v[k], hy.v[k], hz.v[k],
-                               sx.v[k], sy.v[k], sz.v[k]);
+      for (int k = 0; k + 1 < V; k += 2) {
+        const Rand4 ra = philox4x32_10(site0 + 2u * k, 0u, P.sweep_lo, P.sweep_hi, P.seed_lo, P.seed_hi);
+        const Rand4 rb = philox4x32_10(site0 + 2u * k + 2u, 0u, P.sweep_lo, P.sweep_hi, P.seed_lo, P.seed_hi);
+        f2 px = make_float2(sx.v[k], sx.v[k + 1]), py = make_float2(sy.v[k], sy.v[k + 1]), pz = make_float2(sz.v[k], sz.v[k + 1]);
+        bool acc_a, acc_b;
+        attempt2<ANISO>(ra, rb, P.J, P.K, P.beta, P.ex, P.ey, P.ez, make_float2(hx.v[k], hx.v[k + 1]),
+                        make_float2(hy.v[k], hy.v[k + 1]), make_float2(hz.v[k], hz.v[k + 1]), px, py, pz, acc_a, acc_b);
+        sx.v[k] = px.x; sx.v[k + 1] = px.y; sy.v[k] = py.x; sy.v[k + 1] = py.y; sz.v[k] = pz.x; sz.v[k + 1] = pz.y;
+        any |= acc_a | acc_b;
+        if (DIAG) {
+          n_acc += (unsigned)acc_a + (unsigned)acc_b;
+          if (d.accept) { d.accept[site0 + 2u * k] = acc_a; d.accept[site0 + 2u * k + 2u] = acc_b; }
+        }
+      }
+    } else {
+      const bool acc = attempt<ANISO>(site0, P, P.K, P.ex, P.ey, P.ez, hx.v[0], hy.v[0], hz.v[0], sx.v[0], sy.v[0], sz.v[0]);
       any |= acc;
       if (DIAG) {
         n_acc += acc;
-        if (d.accept) d.accept[site0 + 2u * k] = acc;
+        if (d.accept) d.accept[site0] = acc;
       }
     }
     if (any) {
-      store<V>(ax + row_c + i0, sx);
-      store<V>(ay + row_c + i0, sy);
-      store<V>(az + row_c + i0, sz);
+      store<V>(ax + oc, sx);
+      store<V>(ay + oc, sy);
+      store<V>(az + oc, sz);
     }
+  }
+  if (DIAG && d.n_accept && n_acc) atomicAdd(d.n_accept, (unsigned long long)n_acc);
+}
+
+// ---- simple cubic, neighbour planes staged in shared memory by bulk async copies (TMA 1-D) --------
+// A block owns TY consecutive x-rows (all of x) and marches ZT planes in z.  Three plane slots of
+// the OTHER colour (z-1, z, z+1; rows y0-1 .. y0+TY) live in shared memory; while the block works on
+// plane z, lanes of warp 0 have already issued cp.async.bulk copies (one per row and component,
+// completion counted on an mbarrier) for plane z+2.  Every neighbour read is then an LDS with a
+// compile-time offset, the periodic wrap in x is an index inside the staged row, and no load of the
+// neighbour field ever waits on DRAM.  Own spins stay in registers (one LDG.128/STG.128 per component).
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "HB_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra HB_DONE;\n"
+      "bra HB_WAIT;\n"
+      "HB_DONE:\n"
+      "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+template <int TY, int ROWB, int ANISO, bool DIAG>
+__global__ void __launch_bounds__(ROWB / 16 * TY, (ROWB / 16 * TY) >= 256 ? 4 : 1)
+k_sweep_sc_staged(float* __restrict__ ax, float* __restrict__ ay, float* __restrict__ az,
+                  const float* __restrict__ bx, const float* __restrict__ by, const float* __restrict__ bz,
+                  ScLayout L, SweepParams P, int colour, int ZT, Diag d) {
+  constexpr int ROWS = TY + 2;
+  constexpr uint32_t COMP_B = ROWS * ROWB;       // one component of one plane slot
+  constexpr uint32_t SLOT_B = 3 * COMP_B;        // one plane slot
+  extern __shared__ __align__(128) unsigned char smem[];
+  const uint32_t sbase = smem_u32(smem), bar0 = sbase + 3 * SLOT_B;
+  const int HV = L.H >> 2;
+  const int tj = threadIdx.x % HV, ty = threadIdx.x / HV;
+  const int y0 = blockIdx.x * TY;
+  const int ny = min(TY, L.Ly - y0);
+  const int z0 = blockIdx.y * ZT;
+  const int nz = min(ZT, L.Lz - z0);
+  const uint32_t row_bytes = (uint32_t)L.H * 4u;
+  const uint32_t n_rows = 3u * (uint32_t)(ny + 2);
+  const bool issuer = threadIdx.x < 32;
+  const uint32_t n_issuers = blockDim.x < 32 ? blockDim.x : 32;
+
+  // plane k of the march = lattice plane z0-1+k (periodic), slot k % 3
+  auto issue_plane = [&](int k) {
+    int zz = z0 - 1 + k;
+    zz = zz < 0 ? zz + L.Lz : (zz >= L.Lz ? zz - L.Lz : zz);
+    const uint32_t slot = (uint32_t)k % 3u, bar = bar0 + 8u * slot;
+    if (threadIdx.x == 0) mbar_expect_tx(bar, n_rows * row_bytes);
+    __syncwarp();
+    for (uint32_t q = threadIdx.x; q < n_rows; q += n_issuers) {
+      const uint32_t comp = q / (uint32_t)(ny + 2), r = q - comp * (uint32_t)(ny + 2);
+      int yy = y0 - 1 + (int)r;
+      yy = yy < 0 ? yy + L.Ly : (yy >= L.Ly ? yy - L.Ly : yy);
+      const float* src = (comp == 0 ? bx : (comp == 1 ? by : bz)) + ((size_t)zz * L.Ly + yy) * L.H;
+      bulk_g2s(sbase + slot * SLOT_B + comp * COMP_B + r * ROWB, src, row_bytes, bar);
+    }
+  };
+
+  if (threadIdx.x == 0) {
+    mbar_init(bar0, 1); mbar_init(bar0 + 8, 1); mbar_init(bar0 + 16, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (issuer) { issue_plane(0); issue_plane(1); issue_plane(2); }
+
+  const bool active = ty < ny;
+  const int y = y0 + ty;
+  const int i0 = tj * 4;
+  // byte offset of this thread's float4 inside a component slab (row ty+1), and of its row start
+  const uint32_t t_row = (uint32_t)(ty + 1) * ROWB;
+  const uint32_t t_off = t_row + (uint32_t)tj * 16u;
+  uint32_t o_m = 0, o_c = SLOT_B, o_p = 2 * SLOT_B;
+  unsigned n_acc = 0;
+
+  for (int s = 0; s < nz; ++s) {
+    const int z = z0 + s;
+    const int p = (colour + y + z) & 1;
+    const uint32_t grow = (uint32_t)(z * L.Ly + y) * (uint32_t)L.H + (uint32_t)i0;   // element offset in the colour plane
+    Vec<4> sx, sy, sz;
+    if (active) { sx = load_rw<4>(ax + grow); sy = load_rw<4>(ay + grow); sz = load_rw<4>(az + grow); }
+    if (s == 0) { mbar_wait(bar0, 0); mbar_wait(bar0 + 8, 0); }
+    mbar_wait(bar0 + 8u * ((uint32_t)(s + 2) % 3u), ((uint32_t)(s + 2) / 3u) & 1u);
+
+    Vec<4> h[3];
+    if (active) {
+      int ih = p ? i0 + 4 : i0 - 1;
+      ih = ih < 0 ? ih + L.H : (ih >= L.H ? ih - L.H : ih);
+      const uint32_t a_halo = t_row + (uint32_t)ih * 4u + o_c;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        const unsigned char* base = smem + c * COMP_B;
+        const float4 cc = *reinterpret_cast<const float4*>(base + o_c + t_off);
+        const float halo = *reinterpret_cast<const float*>(base + a_halo);
+        const float4 ym = *reinterpret_cast<const float4*>(base + o_c + t_off - ROWB);
+        const float4 yp = *reinterpret_cast<const float4*>(base + o_c + t_off + ROWB);
+        const float4 zm = *reinterpret_cast<const float4*>(base + o_m + t_off);
+        const float4 zp = *reinterpret_cast<const float4*>(base + o_p + t_off);
+        const f2 sel_lo = make_float2(p ? cc.y : halo, p ? cc.z : cc.x);
+        const f2 sel_hi = make_float2(p ? cc.w : cc.y, p ? halo : cc.z);
+        f2 a = add2(make_float2(cc.x, cc.y), sel_lo), b = add2(make_float2(cc.z, cc.w), sel_hi);
+        a = add2(a, make_float2(ym.x, ym.y)); b = add2(b, make_float2(ym.z, ym.w));
+        a = add2(a, make_float2(yp.x, yp.y)); b = add2(b, make_float2(yp.z, yp.w));
+        a = add2(a, make_float2(zm.x, zm.y)); b = add2(b, make_float2(zm.z, zm.w));
+        a = add2(a, make_float2(zp.x, zp.y)); b = add2(b, make_float2(zp.z, zp.w));
+        h[c].v[0] = a.x; h[c].v[1] = a.y; h[c].v[2] = b.x; h[c].v[3] = b.y;
+      }
+    }
+    __syncthreads();                                   // slot o_m has been read by everyone
+    if (issuer && s + 1 < nz) issue_plane(s + 3);      // refill it with the plane needed next step
+
+    if (active) {
+      const uint32_t site0 = (uint32_t)(z * L.Ly + y) * (uint32_t)L.Lx + 2u * (uint32_t)i0 + (uint32_t)p;
+      bool any = false;
+#pragma unroll
+      for (int k = 0; k < 4; k += 2) {
+        const Rand4 ra = philox4x32_10(site0 + 2u * k, 0u, P.sweep_lo, P.sweep_hi, P.seed_lo, P.seed_hi);
+        const Rand4 rb = philox4x32_10(site0 + 2u * k + 2u, 0u, P.sweep_lo, P.sweep_hi, P.seed_lo, P.seed_hi);
+        f2 px = make_float2(sx.v[k], sx.v[k + 1]), py = make_float2(sy.v[k], sy.v[k + 1]), pz = make_float2(sz.v[k], sz.v[k + 1]);
+        bool acc_a, acc_b;
+        attempt2<ANISO>(ra, rb, P.J, P.K, P.beta, P.ex, P.ey, P.ez, make_float2(h[0].v[k], h[0].v[k + 1]),
+                        make_float2(h[1].v[k], h[1].v[k + 1]), make_float2(h[2].v[k], h[2].v[k + 1]), px, py, pz, acc_a, acc_b);
+        sx.v[k] = px.x; sx.v[k + 1] = px.y; sy.v[k] = py.x; sy.v[k + 1] = py.y; sz.v[k] = pz.x; sz.v[k + 1] = pz.y;
+        any |= acc_a | acc_b;
+        if (DIAG) {
+          n_acc += (unsigned)acc_a + (unsigned)acc_b;
+          if (d.accept) { d.accept[site0 + 2u * k] = acc_a; d.accept[site0 + 2u * k + 2u] = acc_b; }
+        }
+      }
+      if (any) {
+        store<4>(ax + grow, sx);
+        store<4>(ay + grow, sy);
+        store<4>(az + grow, sz);
+      }
+    }
+    const uint32_t t = o_m; o_m = o_c; o_c = o_p; o_p = t;
   }
   if (DIAG && d.n_accept && n_acc) atomicAdd(d.n_accept, (unsigned long long)n_acc);
 }
@@ -355,24 +574,90 @@ cudaError_t launch_sc_permute(cudaStream_t st, float* dst, const float* src, ScL
   return cudaGetLastError();
 }
 
-template <int V, bool DIAG>
+inline int aniso_case(const SweepParams& p) {
+  return (p.K == 0.0f) ? ANISO_NONE : ((p.ex == 0.0f && p.ey == 0.0f && p.ez == 1.0f) ? ANISO_Z : ANISO_GENERAL);
+}
+
+template <int V, int ANISO, bool DIAG>
 static cudaError_t sweep_sc_impl(cudaStream_t st, float* s, ScLayout L, ScTile t, SweepParams p, int colour, Diag d) {
+  auto kern = k_sweep_sc<V, ANISO, DIAG, 0>;
+  if (!DIAG && V == 4) {   // the tuned configuration carries the prefetch variants
+    switch (t.PF) {
+      case 1: kern = k_sweep_sc<V, ANISO, DIAG, (!DIAG && V == 4) ? 1 : 0>; break;
+      case 2: kern = k_sweep_sc<V, ANISO, DIAG, (!DIAG && V == 4) ? 2 : 0>; break;
+      case 3: kern = k_sweep_sc<V, ANISO, DIAG, (!DIAG && V == 4) ? 3 : 0>; break;
+      default: break;
+    }
+  }
   const size_t n = L.n;
   float* a = s + (size_t)colour * L.half;
   const float* b = s + (size_t)(1 - colour) * L.half;
   const int HV = L.H / V;
   dim3 grid((HV + t.JX - 1) / t.JX, (L.Ly + t.TY - 1) / t.TY, (L.Lz + t.ZT - 1) / t.ZT);
-  k_sweep_sc<V, DIAG><<<grid, t.JX * t.TY, 0, st>>>(a, a + n, a + 2 * n, b, b + n, b + 2 * n, L, t, p, colour, d);
+  kern<<<grid, t.JX * t.TY, 0, st>>>(a, a + n, a + 2 * n, b, b + n, b + 2 * n, L, t, p, colour, d);
   return cudaGetLastError();
+}
+
+template <int V, bool DIAG>
+static cudaError_t sweep_sc_aniso(cudaStream_t st, float* s, ScLayout L, ScTile t, SweepParams p, int colour, Diag d) {
+  switch (aniso_case(p)) {
+    case ANISO_NONE: return sweep_sc_impl<V, ANISO_NONE, DIAG>(st, s, L, t, p, colour, d);
+    case ANISO_Z: return sweep_sc_impl<V, ANISO_Z, DIAG>(st, s, L, t, p, colour, d);
+    default: return sweep_sc_impl<V, ANISO_GENERAL, DIAG>(st, s, L, t, p, colour, d);
+  }
 }
 
 cudaError_t launch_sweep_sc(cudaStream_t st, float* s, ScLayout L, ScTile t, SweepParams p, int colour, Diag d) {
   const bool diag = d.accept || d.n_accept;
   switch (t.V) {
-    case 4: return diag ? sweep_sc_impl<4, true>(st, s, L, t, p, colour, d) : sweep_sc_impl<4, false>(st, s, L, t, p, colour, d);
-    case 2: return diag ? sweep_sc_impl<2, true>(st, s, L, t, p, colour, d) : sweep_sc_impl<2, false>(st, s, L, t, p, colour, d);
-    default: return diag ? sweep_sc_impl<1, true>(st, s, L, t, p, colour, d) : sweep_sc_impl<1, false>(st, s, L, t, p, colour, d);
+    case 4: return diag ? sweep_sc_aniso<4, true>(st, s, L, t, p, colour, d) : sweep_sc_aniso<4, false>(st, s, L, t, p, colour, d);
+    case 2: return diag ? sweep_sc_aniso<2, true>(st, s, L, t, p, colour, d) : sweep_sc_aniso<2, false>(st, s, L, t, p, colour, d);
+    default: return diag ? sweep_sc_aniso<1, true>(st, s, L, t, p, colour, d) : sweep_sc_aniso<1, false>(st, s, L, t, p, colour, d);
   }
+}
+
+template <int TY, int ROWB, int ANISO, bool DIAG>
+static cudaError_t sweep_sc_staged_impl(cudaStream_t st, float* s, ScLayout L, int ZT, SweepParams p, int colour, Diag d) {
+  constexpr size_t smem_bytes = 3 * 3 * (TY + 2) * (size_t)ROWB + 64;
+  static bool configured = false;
+  auto kern = k_sweep_sc_staged<TY, ROWB, ANISO, DIAG>;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  const size_t n = L.n;
+  float* a = s + (size_t)colour * L.half;
+  const float* b = s + (size_t)(1 - colour) * L.half;
+  dim3 grid((L.Ly + TY - 1) / TY, (L.Lz + ZT - 1) / ZT);
+  kern<<<grid, (L.H / 4) * TY, smem_bytes, st>>>(a, a + n, a + 2 * n, b, b + n, b + 2 * n, L, p, colour, ZT, d);
+  return cudaGetLastError();
+}
+
+template <int TY, int ROWB>
+static cudaError_t sweep_sc_staged_pick(cudaStream_t st, float* s, ScLayout L, int ZT, SweepParams p, int colour, Diag d) {
+  const bool diag = d.accept || d.n_accept;
+  const int aniso = aniso_case(p);
+  if (diag) {
+    switch (aniso) {
+      case ANISO_NONE: return sweep_sc_staged_impl<TY, ROWB, ANISO_NONE, true>(st, s, L, ZT, p, colour, d);
+      case ANISO_Z: return sweep_sc_staged_impl<TY, ROWB, ANISO_Z, true>(st, s, L, ZT, p, colour, d);
+      default: return sweep_sc_staged_impl<TY, ROWB, ANISO_GENERAL, true>(st, s, L, ZT, p, colour, d);
+    }
+  }
+  switch (aniso) {
+    case ANISO_NONE: return sweep_sc_staged_impl<TY, ROWB, ANISO_NONE, false>(st, s, L, ZT, p, colour, d);
+    case ANISO_Z: return sweep_sc_staged_impl<TY, ROWB, ANISO_Z, false>(st, s, L, ZT, p, colour, d);
+    default: return sweep_sc_staged_impl<TY, ROWB, ANISO_GENERAL, false>(st, s, L, ZT, p, colour, d);
+  }
+}
+
+bool sc_staged_supported(const ScLayout& L) { return L.H % 4 == 0 && L.H <= 256; }
+
+cudaError_t launch_sweep_sc_staged(cudaStream_t st, float* s, ScLayout L, int ZT, SweepParams p, int colour, Diag d) {
+  if (L.H > 128) return sweep_sc_staged_pick<4, 1024>(st, s, L, ZT, p, colour, d);
+  if (L.H > 64) return sweep_sc_staged_pick<8, 512>(st, s, L, ZT, p, colour, d);
+  return sweep_sc_staged_pick<16, 256>(st, s, L, ZT, p, colour, d);
 }
 
 cudaError_t launch_sweep_csr(cudaStream_t st, float* s, CsrDev g, uint32_t list_begin, uint32_t list_count,
