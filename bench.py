@@ -110,13 +110,33 @@ class ClockSampler:
         return out
 
 
+def reduce_over_ranks(maxima, sums, device):
+    """The only cross-rank step of the bench (replicas only: no data-path collective): every timing
+    is the MAX over ranks, every count the SUM.  `device` is where the tensors live ("cuda:k" under
+    NCCL, "cpu" under gloo in the CPU tests).  World size 1 (no process group) returns the inputs."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return [float(x) for x in maxima], [int(x) for x in sums]
+    t = torch.tensor([float(x) for x in maxima], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor([int(x) for x in sums] + [0], device=device, dtype=torch.int64)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return [float(x) for x in t.tolist()], [int(x) for x in c.tolist()[:-1]]
+
+
+def replica_seed(cfg, rank):
+    """Rank r runs an independent replica of the workload: same lattice and parameters, seed + r."""
+    return int(cfg["seed"]) + int(rank)
+
+
 def make_context(cfg, seed_offset, device):
     import paper_2106_11286_b200 as hb
     if cfg["kind"] == "sphere":
         lat = hb.Lattice.fcc_sphere(cfg["R"], cfg["K"], cfg["e"], cfg["K_surf"], cfg.get("colouring", "greedy"))
     else:
         lat = hb.Lattice(cfg["kind"], cfg["L"])
-    ctx = hb.Context(lat, cfg["J"], cfg["K"], cfg["e"], cfg["seed"] + seed_offset, device=device)
+    ctx = hb.Context(lat, cfg["J"], cfg["K"], cfg["e"], replica_seed(cfg, seed_offset), device=device)
     if cfg["start"] == "random":
         ctx.init_random()
     else:
@@ -265,13 +285,7 @@ def main():
         bad = clocks and any(r in clocks["reasons"] for r in ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"))
         if not bad:
             break
-    if world > 1:
-        t = torch.tensor([ms, ms_sweeps], device=device, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, ms_sweeps = float(t[0]), float(t[1])
-        lt = torch.tensor([launches], device=device, dtype=torch.int64)
-        dist.all_reduce(lt, op=dist.ReduceOp.SUM)
-        launches = int(lt[0])
+    (ms, ms_sweeps), (launches,) = reduce_over_ranks([ms, ms_sweeps], [launches], device)
     updates = float(n) * SWEEPS_PER_STEP * args.steps * world
     value = updates / (ms * 1e-3) / 1e9
 
@@ -291,10 +305,7 @@ def main():
             ctx.measure()                            # D2H of the step's result (M, E)
         barrier()
         dt = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt], device=device, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t[0])
+        (dt,), _ = reduce_over_ranks([dt], [], device)
         e2e = {"value": float(n) * SWEEPS_PER_STEP * e2e_steps * world / dt / 1e9, "unit": UNIT,
                "h2d_bytes_per_step": 3 * n * 4, "d2h_bytes_per_step": 32, "steps": e2e_steps}
 
@@ -310,7 +321,7 @@ def main():
     avg_launch_s = ms_sweeps * 1e-3 / launches_sweep
     bytes_per_launch = bytes_per_update * n / n_colours
     achieved = bytes_per_launch / avg_launch_s / 1e9
-    kernel = {"sc": "k_sweep_sc", "bcc": "k_sweep_csr", "fcc": "k_sweep_csr", "sphere": "k_sweep_csr"}[cfg["kind"]]
+    kernel = {"sc": "k_sweep_sc", "bcc": "k_sweep_bravais", "fcc": "k_sweep_bravais", "sphere": "k_sweep_csr"}[cfg["kind"]]
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.workload), "kernel": kernel, "peak_source": peak_src,
                 "algorithmic_bytes_per_update": bytes_per_update, "bytes_per_launch": bytes_per_launch,

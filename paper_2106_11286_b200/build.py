@@ -13,13 +13,13 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libhb.so")
-SOURCES = ["hb_api.cpp", "hb_lattice.cpp", "hb_kernels.cu"]
+SOURCES = ["hb_api.cpp", "hb_lattice.cpp", "hb_kernels.cu", "hb_bravais.cu"]
 HEADERS = ["hb_internal.h", "hb_device.cuh", os.path.join("..", "..", "include", "hb.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-fmad=false",           # the arithmetic contract spells out every fused multiply-add
-    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
+    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "--threads", "0",
 ]
 
 

@@ -18,7 +18,7 @@ constexpr int kSeriesChunk = 1024;
 
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
-enum Engine { ENGINE_SC = 0, ENGINE_CSR = 1 };
+enum Engine { ENGINE_SC = 0, ENGINE_CSR = 1, ENGINE_BRAVAIS = 2 };
 
 struct Plan {                 // device memory plan of a lattice
   int64_t n = 0, nnz = 0;
@@ -56,7 +56,8 @@ int make_plan(const hb_lattice* lat, Plan& p, std::string& why) {
   if (p.nnz >= 0x7FFFFFFFll) { why = "more than 2^31-2 neighbour entries"; return HB_EINVAL; }
   if ((lat->K_site == nullptr) != (lat->e_site == nullptr)) { why = "K_site and e_site go together"; return HB_EINVAL; }
   p.per_site = lat->K_site != nullptr;
-  p.engine = (k == HB_SC && !p.per_site) ? ENGINE_SC : ENGINE_CSR;
+  // implicit indexing for the periodic kinds; the table engine for CSR input and per-site anisotropy
+  p.engine = p.per_site || k == HB_CSR ? ENGINE_CSR : (k == HB_SC ? ENGINE_SC : ENGINE_BRAVAIS);
   p.spins_bytes = align_up(3 * (size_t)p.n * sizeof(float));
   size_t o = 0;
   p.off_partials = o; o += align_up((size_t)kMeasureBlocks * 4 * sizeof(double));
@@ -82,6 +83,7 @@ struct hb_ctx {
   Plan plan;
   int32_t kind = 0, Lx = 0, Ly = 0, Lz = 0;
   ScLayout sc{};
+  BrLayout br{};
   ScTile tile{};
   CsrDev csr{};
   int csr_block = 128;
@@ -143,8 +145,9 @@ bool unit_vector(const float* v) {
   return std::isfinite(n2) && std::fabs(n2 - 1.0) <= 1e-5;
 }
 
-// default launch shape of the sc kernels for a lattice
-ScTile default_tile(const ScLayout& L) {
+// default launch shape of the structured kernels for rows of H floats
+ScTile default_tile(int32_t H, int32_t Ly, int32_t Lz) {
+  struct { int32_t H, Ly, Lz; } L{H, Ly, Lz};
   ScTile t;
   t.PF = 1;
   t.V = (L.H % 4 == 0) ? 4 : ((L.H % 2 == 0) ? 2 : 1);
@@ -173,6 +176,8 @@ int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d) {
       HB_CUDA(c, launch_sweep_sc_staged(c->stream, c->spins, c->sc, c->staged_zt, p, colour, d));
     else
       HB_CUDA(c, launch_sweep_sc(c->stream, c->spins, c->sc, c->tile, p, colour, d));
+  } else if (c->plan.engine == ENGINE_BRAVAIS) {
+    HB_CUDA(c, launch_sweep_bravais(c->stream, c->spins, c->br, c->tile, p, colour, d));
   } else {
     const uint32_t b = c->colour_begin[colour], e = c->colour_begin[colour + 1];
     if (e == b) return HB_OK;
@@ -197,6 +202,8 @@ int measure_into(hb_ctx* c, double* dev_out) {
   const SweepParams p = params(c, 0.0f);
   if (c->plan.engine == ENGINE_SC)
     HB_CUDA(c, launch_measure_sc(c->stream, c->spins, c->sc, c->tile.V, p, c->partials(), dev_out));
+  else if (c->plan.engine == ENGINE_BRAVAIS)
+    HB_CUDA(c, launch_measure_bravais(c->stream, c->spins, c->br, c->tile.V, p, c->partials(), dev_out));
   else
     HB_CUDA(c, launch_measure_csr(c->stream, c->spins, c->csr, p, c->partials(), dev_out));
   c->launches += 2;
@@ -298,11 +305,16 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
       c->colour_host = g.colour;
       c->n_colours = g.n_colours;
     }
+  } else if (P.engine == ENGINE_BRAVAIS) {
+    c->n_colours = lat->kind == HB_BCC ? 2 : 4;       // colour = basis index
+    c->br.kind = lat->kind; c->br.Lx = lat->Lx; c->br.Ly = lat->Ly; c->br.Lz = lat->Lz;
+    c->br.n = (uint32_t)P.n; c->br.nc = (uint32_t)(P.n / c->n_colours);
+    c->tile = default_tile(lat->Lx, lat->Ly, lat->Lz);
   } else {
     c->n_colours = 2;
     c->sc.Lx = lat->Lx; c->sc.Ly = lat->Ly; c->sc.Lz = lat->Lz;
     c->sc.H = lat->Lx / 2; c->sc.n = (uint32_t)P.n; c->sc.half = (uint32_t)(P.n / 2);
-    c->tile = default_tile(c->sc);
+    c->tile = default_tile(c->sc.H, c->sc.Ly, c->sc.Lz);
     c->sc_kernel = 0;   // measured on B200: direct + L2 prefetch 141 Gupd/s, staged 135
     c->staged_zt = c->sc.Lz < 16 ? c->sc.Lz : 16;
   }
@@ -523,6 +535,8 @@ int hb_get_colouring(hb_ctx* c, int32_t* colour, int32_t* n_colours) {
     for (int32_t z = 0; z < c->Lz; ++z)
       for (int32_t y = 0; y < c->Ly; ++y)
         for (int32_t x = 0; x < c->Lx; ++x) colour[((int64_t)z * c->Ly + y) * c->Lx + x] = (x + y + z) & 1;
+  } else if (c->plan.engine == ENGINE_BRAVAIS) {
+    for (int64_t i = 0; i < c->plan.n; ++i) colour[i] = (int32_t)(i / c->br.nc);
   } else {
     std::memcpy(colour, c->colour_host.data(), c->colour_host.size() * sizeof(int32_t));
   }
@@ -545,7 +559,11 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
     c->csr_block = (int)value;
     return HB_OK;
   }
-  if (c->plan.engine != ENGINE_SC) return fail(c, HB_EINVAL, "option not valid for this lattice");
+  if (c->plan.engine == ENGINE_CSR) return fail(c, HB_EINVAL, "option not valid for this lattice");
+  const bool is_sc = c->plan.engine == ENGINE_SC;
+  if (!is_sc && (s == "sc_kernel" || s == "sc_staged_zt" || s == "sc_prefetch"))
+    return fail(c, HB_EINVAL, "option valid for the simple cubic lattice only");
+  const int32_t rowH = is_sc ? c->sc.H : c->br.Lx, rowLz = is_sc ? c->sc.Lz : c->br.Lz;
   if (s == "sc_kernel") {
     if (value != 0 && !(value == 1 && sc_staged_supported(c->sc)))
       return fail(c, HB_EINVAL, "sc_kernel: 0 (direct) or 1 (staged; needs Lx % 8 == 0 and Lx <= 512)");
@@ -559,15 +577,16 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
   }
   ScTile t = c->tile;
   if (s == "sc_v") {
-    if (!(value == 1 || value == 2 || value == 4) || c->sc.H % value) return fail(c, HB_EINVAL, "sc_v: 1, 2 or 4 dividing Lx/2");
+    if (!(value == 1 || value == 2 || value == 4) || rowH % value)
+      return fail(c, HB_EINVAL, "sc_v: 1, 2 or 4 dividing the row length (Lx/2 for sc, Lx for bcc/fcc)");
     t.V = (int)value;
-    if (t.JX > c->sc.H / t.V) t.JX = c->sc.H / t.V;
+    if (t.JX > rowH / t.V) t.JX = rowH / t.V;
   } else if (s == "sc_jx") t.JX = (int)value;
   else if (s == "sc_ty") t.TY = (int)value;
   else if (s == "sc_zt") t.ZT = (int)value;
   else if (s == "sc_prefetch") { if (value < 0 || value > 3) return fail(c, HB_EINVAL, "sc_prefetch: 0..3"); t.PF = (int)value; }
   else return fail(c, HB_EINVAL, "unknown option");
-  if (t.JX < 1 || t.TY < 1 || t.ZT < 1 || (int64_t)t.JX * t.TY > 256 || t.ZT > c->sc.Lz)
+  if (t.JX < 1 || t.TY < 1 || t.ZT < 1 || (int64_t)t.JX * t.TY > 256 || t.ZT > rowLz)
     return fail(c, HB_EINVAL, "sc tile: JX, TY, ZT >= 1, JX*TY <= 256, ZT <= Lz");
   c->tile = t;
   return HB_OK;

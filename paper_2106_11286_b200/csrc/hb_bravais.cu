@@ -1,0 +1,284 @@
+// hb_bravais.cu -- colour kernels for periodic Bravais lattices with a basis (bcc, fcc), implicit
+// neighbour indexing: no neighbour table is read, the geometry is a compile-time descriptor.
+//
+// Storage is the canonical order: sublattice b is a plain Lx x Ly x Lz array at
+// offset b*Nc of each component plane, and colour = b.  A thread owns V consecutive cells of one
+// x-row of its sublattice and marches ZT planes in z, exactly like the sc kernel; a neighbour of
+// the V cells [i0, i0+V) of row (y,z) is the same V-vector of another sublattice's row
+// (y+dy, z+dz), shifted by dx in {-1,0,+1}: one aligned vector load plus, for dx != 0, one halo
+// element.  Neighbours that share a row share the loads (the compiler merges them; ptxas output
+// is checked in profiles/).  Neighbour order is the arithmetic contract of include/hb.h.
+//
+// HBM traffic per attempted update: bcc 36 B (own 12 + other sublattice once 12 + write 12),
+// fcc 60 B (own 12 + three other sublattices 36 + write 12); DESIGN.md section 7.
+#include "hb_device.cuh"
+#include "hb_internal.h"
+
+namespace hb {
+
+namespace {
+
+struct Nbr { int nb, dx, dy, dz; };
+
+// floor(t / 2) for t in {-1, 0, 1, 2}
+__host__ __device__ constexpr int half_floor(int t) { return t < 0 ? -1 : t / 2; }
+
+template <int KIND> struct Geo;
+
+// bcc: a corner (b = 0) of cell (x,y,z) touches the centres of cells (x-1|x, y-1|y, z-1|z), a
+// centre (b = 1) the corners of (x|x+1, y|y+1, z|z+1); k = 4 sz + 2 sy + sx, x fastest.
+template <> struct Geo<BR_BCC> {
+  static constexpr int NB = 2, Z = 8;
+  __host__ __device__ static constexpr Nbr nbr(int b, int k) {
+    const int lo = b ? 0 : -1;
+    return Nbr{1 - b, lo + (k & 1), lo + ((k >> 1) & 1), lo + ((k >> 2) & 1)};
+  }
+};
+
+// fcc: four sc sublattices; in doubled coordinates a site is 2(x,y,z) + d_b with d_0 = (0,0,0),
+// d_1 = (0,1,1), d_2 = (1,0,1), d_3 = (1,1,0); the twelve neighbour offsets in the order of
+// include/hb.h.  The parity pattern of the doubled neighbour coordinate names its sublattice.
+template <> struct Geo<BR_FCC> {
+  static constexpr int NB = 4, Z = 12;
+  __host__ __device__ static constexpr Nbr nbr(int b, int k) {
+    const int off[12][3] = {{1, 1, 0}, {1, -1, 0}, {-1, 1, 0}, {-1, -1, 0}, {1, 0, 1}, {1, 0, -1},
+                            {-1, 0, 1}, {-1, 0, -1}, {0, 1, 1}, {0, 1, -1}, {0, -1, 1}, {0, -1, -1}};
+    const int dbl[4][3] = {{0, 0, 0}, {0, 1, 1}, {1, 0, 1}, {1, 1, 0}};
+    const int tx = dbl[b][0] + off[k][0], ty = dbl[b][1] + off[k][1], tz = dbl[b][2] + off[k][2];
+    const bool ox = (tx & 1) != 0, oy = (ty & 1) != 0;
+    return Nbr{ox ? (oy ? 3 : 2) : (oy ? 1 : 0), half_floor(tx), half_floor(ty), half_floor(tz)};
+  }
+};
+
+// what a thread knows about its V cells in row (y,z): element offsets inside one sublattice array
+struct Where {
+  uint32_t yo[3];   // (y-1, y, y+1 periodic) * Lx
+  uint32_t zo[3];   // (z-1, z, z+1 periodic) * Ly * Lx
+  uint32_t i0, il, ir;   // first cell, the cell left of it and the cell right of the last one (periodic)
+};
+
+template <int V>
+__device__ __forceinline__ Vec<V> shifted(const float* __restrict__ row, const Where& w, int dx) {
+  const Vec<V> c = load_ro<V>(row + w.i0);
+  if (dx == 0) return c;
+  Vec<V> t;
+  if (dx < 0) {
+    t.v[0] = __ldg(row + w.il);
+#pragma unroll
+    for (int k = 1; k < V; ++k) t.v[k] = c.v[k - 1];
+  } else {
+#pragma unroll
+    for (int k = 0; k + 1 < V; ++k) t.v[k] = c.v[k + 1];
+    t.v[V - 1] = __ldg(row + w.ir);
+  }
+  return t;
+}
+
+template <int V>
+__device__ __forceinline__ Vec<V> vadd(const Vec<V>& a, const Vec<V>& b) {
+  Vec<V> r;
+  if (V >= 2) {
+#pragma unroll
+    for (int k = 0; k + 1 < V; k += 2) {
+      const f2 s = add2(make_float2(a.v[k], a.v[k + 1]), make_float2(b.v[k], b.v[k + 1]));
+      r.v[k] = s.x; r.v[k + 1] = s.y;
+    }
+  } else {
+    r.v[0] = __fadd_rn(a.v[0], b.v[0]);
+  }
+  return r;
+}
+
+// h = sum over the Z neighbours in contract order, starting from the first one (0 + a = a exactly)
+template <int KIND, int B, int V, int K = 0>
+__device__ __forceinline__ void field(const float* __restrict__ s, uint32_t nc, uint32_t n, const Where& w,
+                                      Vec<V>& hx, Vec<V>& hy, Vec<V>& hz) {
+  if constexpr (K < Geo<KIND>::Z) {
+    constexpr Nbr g = Geo<KIND>::nbr(B, K);
+    const float* row = s + (size_t)g.nb * nc + (w.zo[g.dz + 1] + w.yo[g.dy + 1]);
+    const Vec<V> tx = shifted<V>(row, w, g.dx);
+    const Vec<V> ty = shifted<V>(row + n, w, g.dx);
+    const Vec<V> tz = shifted<V>(row + 2 * (size_t)n, w, g.dx);
+    if constexpr (K == 0) { hx = tx; hy = ty; hz = tz; }
+    else { hx = vadd<V>(hx, tx); hy = vadd<V>(hy, ty); hz = vadd<V>(hz, tz); }
+    field<KIND, B, V, K + 1>(s, nc, n, w, hx, hy, hz);
+  }
+}
+
+__device__ __forceinline__ void where_y(Where& w, const BrLayout& L, int32_t y, int32_t i0, int V) {
+  w.yo[0] = (uint32_t)((y == 0) ? L.Ly - 1 : y - 1) * (uint32_t)L.Lx;
+  w.yo[1] = (uint32_t)y * (uint32_t)L.Lx;
+  w.yo[2] = (uint32_t)((y == L.Ly - 1) ? 0 : y + 1) * (uint32_t)L.Lx;
+  w.i0 = (uint32_t)i0;
+  w.il = (uint32_t)((i0 == 0) ? L.Lx - 1 : i0 - 1);
+  w.ir = (uint32_t)((i0 + V >= L.Lx) ? i0 + V - L.Lx : i0 + V);
+}
+__device__ __forceinline__ void where_z(Where& w, const BrLayout& L, int32_t z) {
+  const uint32_t plane = (uint32_t)L.Ly * (uint32_t)L.Lx;
+  w.zo[0] = (uint32_t)((z == 0) ? L.Lz - 1 : z - 1) * plane;
+  w.zo[1] = (uint32_t)z * plane;
+  w.zo[2] = (uint32_t)((z == L.Lz - 1) ? 0 : z + 1) * plane;
+}
+
+template <int KIND, int B, int V, int ANISO, bool DIAG>
+__global__ void __launch_bounds__(256, 3)
+k_sweep_bravais(float* __restrict__ own, const float* __restrict__ all, BrLayout L, ScTile t, SweepParams P, Diag d) {
+  const int32_t tj = threadIdx.x % t.JX, ty = threadIdx.x / t.JX;
+  const int32_t i0 = (blockIdx.x * t.JX + tj) * V;
+  const int32_t y = blockIdx.y * t.TY + ty;
+  if (i0 >= L.Lx || y >= L.Ly) return;
+  Where w;
+  where_y(w, L, y, i0, V);
+  const int32_t z0 = blockIdx.z * t.ZT, z1 = min(z0 + t.ZT, L.Lz);
+  const size_t n = L.n;
+  unsigned n_acc = 0;
+  for (int32_t z = z0; z < z1; ++z) {
+    where_z(w, L, z);
+    const uint32_t o = w.zo[1] + w.yo[1] + w.i0;             // offset inside the own sublattice
+    Vec<V> sx = load_rw<V>(own + o), sy = load_rw<V>(own + n + o), sz = load_rw<V>(own + 2 * n + o);
+    Vec<V> hx, hy, hz;
+    field<KIND, B, V>(all, L.nc, L.n, w, hx, hy, hz);
+    const uint32_t site0 = (uint32_t)B * L.nc + o;          // canonical id = b*Nc + cell
+    bool any = false;
+    if constexpr (V >= 2) {
+#pragma unroll
+      for (int k = 0; k + 1 < V; k += 2) {
+        const Rand4 ra = philox4x32_10(site0 + k, 0u, P.sweep_lo, P.sweep_hi, P.seed_lo, P.seed_hi);
+        const Rand4 rb = philox4x32_10(site0 + k + 1, 0u, P.sweep_lo, P.sweep_hi, P.seed_lo, P.seed_hi);
+        f2 px = make_float2(sx.v[k], sx.v[k + 1]), py = make_float2(sy.v[k], sy.v[k + 1]), pz = make_float2(sz.v[k], sz.v[k + 1]);
+        bool acc_a, acc_b;
+        attempt2<ANISO>(ra, rb, P.J, P.K, P.beta, P.ex, P.ey, P.ez, make_float2(hx.v[k], hx.v[k + 1]),
+                        make_float2(hy.v[k], hy.v[k + 1]), make_float2(hz.v[k], hz.v[k + 1]), px, py, pz, acc_a, acc_b);
+        sx.v[k] = px.x; sx.v[k + 1] = px.y; sy.v[k] = py.x; sy.v[k + 1] = py.y; sz.v[k] = pz.x; sz.v[k + 1] = pz.y;
+        any |= acc_a | acc_b;
+        if (DIAG) {
+          n_acc += (unsigned)acc_a + (unsigned)acc_b;
+          if (d.accept) { d.accept[site0 + k] = acc_a; d.accept[site0 + k + 1] = acc_b; }
+        }
+      }
+    } else {
+      const Rand4 r = philox4x32_10(site0, 0u, P.sweep_lo, P.sweep_hi, P.seed_lo, P.seed_hi);
+      float nx, ny, nz;
+      sphere(r.r0, r.r1, nx, ny, nz);
+      const float dH = delta_h_t<ANISO>(sx.v[0], sy.v[0], sz.v[0], nx, ny, nz, hx.v[0], hy.v[0], hz.v[0], P.J, P.K, P.ex, P.ey, P.ez);
+      const bool acc = metropolis_accept(dH, P.beta, r.r2);
+      if (acc) { sx.v[0] = nx; sy.v[0] = ny; sz.v[0] = nz; }
+      any = acc;
+      if (DIAG) {
+        n_acc += acc;
+        if (d.accept) d.accept[site0] = acc;
+      }
+    }
+    if (any) {
+      store<V>(own + o, sx);
+      store<V>(own + n + o, sy);
+      store<V>(own + 2 * n + o, sz);
+    }
+  }
+  if (DIAG && d.n_accept && n_acc) atomicAdd(d.n_accept, (unsigned long long)n_acc);
+}
+
+// ---- measurement: M and E over all sublattices, fp64 accumulation ---------------------------------
+template <int KIND, int B, int V>
+__device__ __forceinline__ void measure_sub(const float* __restrict__ s, const BrLayout& L, const SweepParams& P,
+                                            double& mx, double& my, double& mz, double& en) {
+  if constexpr (B < Geo<KIND>::NB) {
+    const uint32_t HV = (uint32_t)L.Lx / V, chunks = (uint32_t)L.Lz * (uint32_t)L.Ly * HV;
+    const size_t n = L.n;
+    for (uint32_t q = blockIdx.x * blockDim.x + threadIdx.x; q < chunks; q += gridDim.x * blockDim.x) {
+      const uint32_t row = q / HV, j = q - row * HV;
+      const int32_t z = (int32_t)(row / (uint32_t)L.Ly), y = (int32_t)(row - (uint32_t)z * (uint32_t)L.Ly);
+      Where w;
+      where_y(w, L, y, (int32_t)(j * V), V);
+      where_z(w, L, z);
+      Vec<V> hx, hy, hz;
+      field<KIND, B, V>(s, L.nc, L.n, w, hx, hy, hz);
+      const float* own = s + (size_t)B * L.nc + (w.zo[1] + w.yo[1] + w.i0);
+      const Vec<V> ox = load_ro<V>(own), oy = load_ro<V>(own + n), oz = load_ro<V>(own + 2 * n);
+#pragma unroll
+      for (int k = 0; k < V; ++k) {
+        mx += (double)ox.v[k]; my += (double)oy.v[k]; mz += (double)oz.v[k];
+        en += (double)site_energy(ox.v[k], oy.v[k], oz.v[k], hx.v[k], hy.v[k], hz.v[k], P.J, P.K, P.ex, P.ey, P.ez);
+      }
+    }
+    measure_sub<KIND, B + 1, V>(s, L, P, mx, my, mz, en);
+  }
+}
+
+template <int KIND, int V>
+__global__ void __launch_bounds__(256)
+k_measure_bravais(const float* __restrict__ s, BrLayout L, SweepParams P, double* partials) {
+  double mx = 0, my = 0, mz = 0, en = 0;
+  measure_sub<KIND, 0, V>(s, L, P, mx, my, mz, en);
+  block_reduce4(mx, my, mz, en, partials);
+}
+
+inline int aniso_of(const SweepParams& p) {
+  return (p.K == 0.0f) ? ANISO_NONE : ((p.ex == 0.0f && p.ey == 0.0f && p.ez == 1.0f) ? ANISO_Z : ANISO_GENERAL);
+}
+
+template <int KIND, int B, int V, int ANISO, bool DIAG>
+cudaError_t go(cudaStream_t st, float* s, const BrLayout& L, const ScTile& t, const SweepParams& p, const Diag& d) {
+  const int HV = L.Lx / V;
+  dim3 grid((HV + t.JX - 1) / t.JX, (L.Ly + t.TY - 1) / t.TY, (L.Lz + t.ZT - 1) / t.ZT);
+  k_sweep_bravais<KIND, B, V, ANISO, DIAG><<<grid, t.JX * t.TY, 0, st>>>(s + (size_t)B * L.nc, s, L, t, p, d);
+  return cudaGetLastError();
+}
+
+// The tuned shape (V = 4, no diagnostics) carries the three anisotropy specialisations; the
+// narrow vectors and the recording variant use the general formula, which gives the same bits.
+template <int KIND, int B>
+cudaError_t pick(cudaStream_t st, float* s, const BrLayout& L, const ScTile& t, const SweepParams& p, const Diag& d) {
+  const bool diag = d.accept || d.n_accept;
+  if (t.V == 4) {
+    if (diag) return go<KIND, B, 4, ANISO_GENERAL, true>(st, s, L, t, p, d);
+    switch (aniso_of(p)) {
+      case ANISO_NONE: return go<KIND, B, 4, ANISO_NONE, false>(st, s, L, t, p, d);
+      case ANISO_Z: return go<KIND, B, 4, ANISO_Z, false>(st, s, L, t, p, d);
+      default: return go<KIND, B, 4, ANISO_GENERAL, false>(st, s, L, t, p, d);
+    }
+  }
+  if (t.V == 2)
+    return diag ? go<KIND, B, 2, ANISO_GENERAL, true>(st, s, L, t, p, d) : go<KIND, B, 2, ANISO_GENERAL, false>(st, s, L, t, p, d);
+  return diag ? go<KIND, B, 1, ANISO_GENERAL, true>(st, s, L, t, p, d) : go<KIND, B, 1, ANISO_GENERAL, false>(st, s, L, t, p, d);
+}
+
+template <int KIND>
+cudaError_t measure(cudaStream_t st, const float* s, const BrLayout& L, int V, const SweepParams& p, double* partials, int grid) {
+  switch (V) {
+    case 4: k_measure_bravais<KIND, 4><<<grid, 256, 0, st>>>(s, L, p, partials); break;
+    case 2: k_measure_bravais<KIND, 2><<<grid, 256, 0, st>>>(s, L, p, partials); break;
+    default: k_measure_bravais<KIND, 1><<<grid, 256, 0, st>>>(s, L, p, partials); break;
+  }
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t launch_sweep_bravais(cudaStream_t st, float* s, BrLayout L, ScTile t, SweepParams p, int colour, Diag d) {
+  if (L.kind == BR_BCC) {
+    switch (colour) {
+      case 0: return pick<BR_BCC, 0>(st, s, L, t, p, d);
+      case 1: return pick<BR_BCC, 1>(st, s, L, t, p, d);
+    }
+  } else if (L.kind == BR_FCC) {
+    switch (colour) {
+      case 0: return pick<BR_FCC, 0>(st, s, L, t, p, d);
+      case 1: return pick<BR_FCC, 1>(st, s, L, t, p, d);
+      case 2: return pick<BR_FCC, 2>(st, s, L, t, p, d);
+      case 3: return pick<BR_FCC, 3>(st, s, L, t, p, d);
+    }
+  }
+  return cudaErrorInvalidValue;
+}
+
+cudaError_t launch_measure_bravais(cudaStream_t st, const float* s, BrLayout L, int V, SweepParams p, double* partials, double* out) {
+  const long long chunks = (long long)L.nc / V;
+  const long long want = (chunks + 255) / 256;
+  const int grid = (int)(want < 1 ? 1 : (want > kMeasureBlocks ? kMeasureBlocks : want));
+  cudaError_t e = L.kind == BR_BCC ? measure<BR_BCC>(st, s, L, V, p, partials, grid) : measure<BR_FCC>(st, s, L, V, p, partials, grid);
+  if (e != cudaSuccess) return e;
+  return launch_reduce_final(st, partials, grid, out);
+}
+
+}  // namespace hb

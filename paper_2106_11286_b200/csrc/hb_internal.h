@@ -30,6 +30,16 @@ struct ScTile {
   int32_t PF;   // software prefetch of the next z-plane: 0 none, 1 L2, 2 L1, 3 touch
 };
 
+// periodic Bravais lattice with a basis (bcc: 2 sublattices, fcc: 4), canonical storage:
+// sublattice b is an Lx x Ly x Lz array at offset b*nc of each component plane
+enum { BR_BCC = 1, BR_FCC = 2 };   // values of hb_kind
+struct BrLayout {
+  int32_t kind;
+  int32_t Lx, Ly, Lz;
+  uint32_t nc;      // cells = sites per sublattice
+  uint32_t n;       // N
+};
+
 // CSR tables on the device
 struct CsrDev {
   uint32_t n;
@@ -56,10 +66,13 @@ bool sc_staged_supported(const ScLayout& L);
 cudaError_t launch_sweep_sc_staged(cudaStream_t st, float* spins, ScLayout L, int ZT, SweepParams p, int colour, Diag d);
 cudaError_t launch_sweep_csr(cudaStream_t st, float* spins, CsrDev g, uint32_t list_begin, uint32_t list_count,
                              SweepParams p, int block, Diag d);
+cudaError_t launch_sweep_bravais(cudaStream_t st, float* spins, BrLayout L, ScTile t, SweepParams p, int colour, Diag d);
 // measurement: partials must hold kMeasureBlocks*4 doubles; out receives (Mx*N, My*N, Mz*N, E)
 constexpr int kMeasureBlocks = 1184;
 cudaError_t launch_measure_sc(cudaStream_t st, const float* spins, ScLayout L, int V, SweepParams p, double* partials, double* out);
 cudaError_t launch_measure_csr(cudaStream_t st, const float* spins, CsrDev g, SweepParams p, double* partials, double* out);
+cudaError_t launch_measure_bravais(cudaStream_t st, const float* spins, BrLayout L, int V, SweepParams p, double* partials, double* out);
+cudaError_t launch_reduce_final(cudaStream_t st, const double* partials, int n_blocks, double* out);
 
 // ---- host lattice tables (hb_lattice.cpp) -------------------------------------------------
 struct HostCsr {

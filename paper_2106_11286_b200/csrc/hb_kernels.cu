@@ -15,40 +15,6 @@ namespace hb {
 
 namespace {
 
-// ---- small vector helpers: V consecutive floats ------------------------------------------
-template <int V> struct Vec { float v[V]; };
-
-template <int V> __device__ __forceinline__ Vec<V> load_ro(const float* p);   // read-only path
-template <> __device__ __forceinline__ Vec<4> load_ro<4>(const float* p) {
-  const float4 t = __ldg(reinterpret_cast<const float4*>(p));
-  return Vec<4>{{t.x, t.y, t.z, t.w}};
-}
-template <> __device__ __forceinline__ Vec<2> load_ro<2>(const float* p) {
-  const float2 t = __ldg(reinterpret_cast<const float2*>(p));
-  return Vec<2>{{t.x, t.y}};
-}
-template <> __device__ __forceinline__ Vec<1> load_ro<1>(const float* p) { return Vec<1>{{__ldg(p)}}; }
-
-template <int V> __device__ __forceinline__ Vec<V> load_rw(const float* p);
-template <> __device__ __forceinline__ Vec<4> load_rw<4>(const float* p) {
-  const float4 t = *reinterpret_cast<const float4*>(p);
-  return Vec<4>{{t.x, t.y, t.z, t.w}};
-}
-template <> __device__ __forceinline__ Vec<2> load_rw<2>(const float* p) {
-  const float2 t = *reinterpret_cast<const float2*>(p);
-  return Vec<2>{{t.x, t.y}};
-}
-template <> __device__ __forceinline__ Vec<1> load_rw<1>(const float* p) { return Vec<1>{{*p}}; }
-
-template <int V> __device__ __forceinline__ void store(float* p, const Vec<V>& a);
-template <> __device__ __forceinline__ void store<4>(float* p, const Vec<4>& a) {
-  *reinterpret_cast<float4*>(p) = make_float4(a.v[0], a.v[1], a.v[2], a.v[3]);
-}
-template <> __device__ __forceinline__ void store<2>(float* p, const Vec<2>& a) {
-  *reinterpret_cast<float2*>(p) = make_float2(a.v[0], a.v[1]);
-}
-template <> __device__ __forceinline__ void store<1>(float* p, const Vec<1>& a) { *p = a.v[0]; }
-
 // ---- simple cubic, colour-split layout -----------------------------------------------------
 // Plane c of a component holds the sites with (x+y+z) mod 2 == c, row (y,z) of H = Lx/2 floats:
 // element i of that row is x = 2 i + ((c+y+z) & 1).  For a site of colour c in row (y,z), with
@@ -440,36 +406,6 @@ __global__ void k_sc_permute(float* dst, const float* src, ScLayout L, bool to_i
 }
 
 // ---- measurement --------------------------------------------------------------------------------
-// block partial of (sum Sx, sum Sy, sum Sz, sum e_i) in double; partials[block*4 + q]
-__device__ __forceinline__ void block_reduce4(double a0, double a1, double a2, double a3, double* partials) {
-  __shared__ double sh[4][32];
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    a0 += __shfl_xor_sync(0xffffffffu, a0, o);
-    a1 += __shfl_xor_sync(0xffffffffu, a1, o);
-    a2 += __shfl_xor_sync(0xffffffffu, a2, o);
-    a3 += __shfl_xor_sync(0xffffffffu, a3, o);
-  }
-  const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
-  if (l == 0) { sh[0][w] = a0; sh[1][w] = a1; sh[2][w] = a2; sh[3][w] = a3; }
-  __syncthreads();
-  if (w == 0) {
-    a0 = l < nw ? sh[0][l] : 0.0; a1 = l < nw ? sh[1][l] : 0.0;
-    a2 = l < nw ? sh[2][l] : 0.0; a3 = l < nw ? sh[3][l] : 0.0;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      a0 += __shfl_xor_sync(0xffffffffu, a0, o);
-      a1 += __shfl_xor_sync(0xffffffffu, a1, o);
-      a2 += __shfl_xor_sync(0xffffffffu, a2, o);
-      a3 += __shfl_xor_sync(0xffffffffu, a3, o);
-    }
-    if (l == 0) {
-      partials[blockIdx.x * 4 + 0] = a0; partials[blockIdx.x * 4 + 1] = a1;
-      partials[blockIdx.x * 4 + 2] = a2; partials[blockIdx.x * 4 + 3] = a3;
-    }
-  }
-}
-
 // fixed-order final sum of the block partials: one block of 256 threads
 __global__ void k_reduce_final(const double* partials, int n_blocks, double* out) {
   double a[4] = {0, 0, 0, 0};
@@ -669,6 +605,11 @@ cudaError_t launch_sweep_csr(cudaStream_t st, float* s, CsrDev g, uint32_t list_
     k_sweep_csr<true><<<grid, block, 0, st>>>(s, s + n, s + 2 * n, g, list_begin, list_count, p, d);
   else
     k_sweep_csr<false><<<grid, block, 0, st>>>(s, s + n, s + 2 * n, g, list_begin, list_count, p, d);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_reduce_final(cudaStream_t st, const double* partials, int n_blocks, double* out) {
+  k_reduce_final<<<1, 256, 0, st>>>(partials, n_blocks, out);
   return cudaGetLastError();
 }
 

@@ -1,0 +1,130 @@
+"""The C-ABI boundary without a GPU: libhb.so loads, exports every symbol include/hb.h declares,
+the binding names the same set, and the host-only entry points (sizes, validation, the sphere
+builder, error strings) behave as the header says.  No compute call is made here."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2106_11286_b200 as hb
+from paper_2106_11286_b200 import binding
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_functions():
+    """Every function declared in include/*.h (comments stripped)."""
+    names = []
+    inc = os.path.join(ROOT, "include")
+    for fn in sorted(os.listdir(inc)):
+        if not fn.endswith(".h"):
+            continue
+        text = open(os.path.join(inc, fn)).read()
+        text = re.sub(r"/\*.*?\*/", " ", text, flags=re.S)
+        text = re.sub(r"//[^\n]*", " ", text)
+        names += re.findall(r"\b(hb_[a-z0-9_]+)\s*\(", text)
+    return sorted(set(names))
+
+
+def test_header_declares_the_three_north_star_calls():
+    names = declared_functions()
+    for must in ("hb_create", "hb_sweep", "hb_measure"):
+        assert must in names
+
+
+def test_library_exports_every_declared_symbol():
+    lib = hb.load_library()
+    names = declared_functions()
+    assert len(names) >= 20
+    for name in names:
+        assert hasattr(lib, name), "libhb.so does not export %s" % name
+    # the binding marshals exactly the declared set
+    assert sorted(binding.EXPORTS) == names
+
+
+def test_library_has_sm100a_code_only():
+    """The kernels are built for sm_100a (no PTX-only or multi-arch fallback)."""
+    import shutil
+    import subprocess
+    exe = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(exe):
+        pytest.skip("cuobjdump not available")
+    out = subprocess.run([exe, "-lelf", binding.library_path()], capture_output=True, text=True).stdout
+    archs = set(re.findall(r"sm_(\d+a?)", out))
+    assert archs == {"100a"}, archs
+
+
+def test_strerror_and_null_arguments():
+    lib = hb.load_library()
+    assert lib.hb_strerror(0) == b"ok"
+    for code in (-1, -2, -3, -4):
+        assert lib.hb_strerror(code) not in (b"", b"ok", b"unknown status")
+    assert lib.hb_strerror(-99) == b"unknown status"
+    assert lib.hb_sizes(None, None, None, None) == -1            # HB_EINVAL
+    assert lib.hb_create(None, None, 1.0, 0.0, None, 0, None) == -1
+    assert lib.hb_destroy(None) == 0
+    assert lib.hb_lattice_free(None) == 0
+    assert lib.hb_error_detail(None) == b""
+
+
+@pytest.mark.parametrize("kind,L,n", [("sc", 16, 4096), ("bcc", 64, 524288), ("fcc", 128, 8388608), ("sc", 464, 99897344)])
+def test_sizes_of_the_baseline_configs(kind, L, n):
+    got, spins_bytes, ws_bytes = hb.sizes(hb.Lattice(kind, L))
+    assert got == n
+    assert spins_bytes >= 12 * n and spins_bytes % 256 == 0
+    assert ws_bytes > 0 and ws_bytes % 256 == 0
+
+
+def test_sizes_rejects_bad_lattices():
+    for lat in (hb.Lattice("sc", 15), hb.Lattice("sc", 16, 16, 7), hb.Lattice("bcc", 0), hb.Lattice(7, 4)):
+        with pytest.raises(hb.HbError) as e:
+            hb.sizes(lat)
+        assert e.value.status == -1
+    # more than 2^32-1 sites cannot be keyed by a 32-bit Philox counter word
+    with pytest.raises(hb.HbError):
+        hb.sizes(hb.Lattice("fcc", 1100))
+
+
+def test_sphere_builder_matches_the_oracles_independent_builder():
+    """Host logic of rows a1/a2: the library's fcc-sphere table, anisotropy classes and greedy
+    colouring against the oracle's own construction (the two share no code)."""
+    import oracle
+    for R, colouring in ((2, "greedy"), (5, "greedy"), (5, "parity"), (0, "greedy")):
+        g = hb.Lattice.fcc_sphere(R, 0.05, (0, 0, 1), 0.5, colouring)
+        o = oracle.Lattice.fcc_sphere(R, 0.05, (0, 0, 1), 0.5, colouring)
+        assert g.row_ptr.size - 1 == o.n
+        assert np.array_equal(g.row_ptr, o.row_ptr)
+        assert np.array_equal(g.col_idx, o.col)
+        assert g.n_colours == o.n_colours
+        assert np.array_equal(g.colour, o.colour)
+        assert np.array_equal(g.K_site.view(np.uint32), o.K.view(np.uint32))
+        assert np.array_equal(g.e_site.view(np.uint32).ravel(), o.e.view(np.uint32).ravel())
+        assert np.array_equal(g.xyz, o.xyz)
+
+
+def test_no_cpu_path():
+    """Without a CUDA device the product refuses to construct a context (no fallback)."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    with pytest.raises(RuntimeError):
+        hb.Context(hb.Lattice("sc", 4))
+
+
+def test_product_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2106_11286_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for fn in files:
+            if fn.endswith((".py", ".cpp", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, fn)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", text, flags=re.M), fn
+                assert "hb_oracle" not in text, fn
+    for dirpath, _, files in os.walk(os.path.join(ROOT, "oracle")):
+        for fn in files:
+            if fn.endswith((".py", ".cpp", ".h")):
+                text = open(os.path.join(dirpath, fn)).read()
+                assert not re.search(r"^\s*(import|from)\s+paper_2106_11286_b200\b", text, flags=re.M), fn
+                assert not re.search(r"#\s*include\s*[\"<][^\">]*(hb\.h|hb_internal\.h|hb_device\.cuh)", text), fn
+                assert "libhb.so" not in text, fn
