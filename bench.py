@@ -218,7 +218,7 @@ def run_reference(args, cfg, name):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c4", help="c1..c5 (BASELINE.json configs); the headline is c4")
@@ -280,6 +280,10 @@ def main():
     clocks = None
     for attempt in range(2):
         sampler = ClockSampler(local) if rank == 0 else None
+        if sampler:
+            time.sleep(0.5)          # nvidia-smi needs a moment before its first sample
+            for _ in range(2):       # keep the device under load while it starts
+                ctx.sweep(T, SWEEPS_PER_STEP)
         ms, ms_sweeps, launches = timed_run(args.steps)
         clocks = sampler.stop() if sampler else None
         bad = clocks and any(r in clocks["reasons"] for r in ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"))

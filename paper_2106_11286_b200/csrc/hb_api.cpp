@@ -60,7 +60,8 @@ int make_plan(const hb_lattice* lat, Plan& p, std::string& why) {
   p.engine = p.per_site || k == HB_CSR ? ENGINE_CSR : (k == HB_SC ? ENGINE_SC : ENGINE_BRAVAIS);
   p.spins_bytes = align_up(3 * (size_t)p.n * sizeof(float));
   size_t o = 0;
-  p.off_partials = o; o += align_up((size_t)kMeasureBlocks * 4 * sizeof(double));
+  const size_t n_partials = kMeasureBlocks > 2 * kFusedBlocksMax ? kMeasureBlocks : 2 * kFusedBlocksMax;
+  p.off_partials = o; o += align_up(n_partials * 4 * sizeof(double));
   p.off_series = o;   o += align_up((size_t)kSeriesChunk * 4 * sizeof(double));
   p.off_counters = o; o += kAlign;
   p.off_staging = o;  o += align_up((size_t)p.n * sizeof(float));
@@ -89,6 +90,8 @@ struct hb_ctx {
   int csr_block = 128;
   int sc_kernel = 0;      // 0: direct loads through L1, 1: neighbour planes staged in shared memory
   int staged_zt = 16;
+  bool fused_measure = true;   // sc: the last sweep of hb_sweep also reduces M and E
+  bool cache_valid = false;    // cached() holds the measurement of the current spins
   std::vector<uint32_t> colour_begin;     // CSR engine: offsets into the colour-sorted list
   std::vector<int32_t> colour_host;       // CSR engine: colour of every site
   int32_t n_colours = 0;
@@ -107,6 +110,7 @@ struct hb_ctx {
   double* series() const { return reinterpret_cast<double*>(ws + plan.off_series); }
   unsigned long long* counters() const { return reinterpret_cast<unsigned long long*>(ws + plan.off_counters); }
   float* staging() const { return reinterpret_cast<float*>(ws + plan.off_staging); }
+  double* cached() const { return reinterpret_cast<double*>(ws + plan.off_counters + 64); }
 };
 
 namespace {
@@ -150,6 +154,7 @@ ScTile default_tile(int32_t H, int32_t Ly, int32_t Lz) {
   struct { int32_t H, Ly, Lz; } L{H, Ly, Lz};
   ScTile t;
   t.PF = 1;
+  t.LIN = 0;
   t.V = (L.H % 4 == 0) ? 4 : ((L.H % 2 == 0) ? 2 : 1);
   const int HV = L.H / t.V;
   int best = HV <= 64 ? HV : 64, best_waste = 1 << 30;
@@ -170,12 +175,12 @@ ScTile default_tile(int32_t H, int32_t Ly, int32_t Lz) {
   return t;
 }
 
-int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d) {
+int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d, Meas m = Meas{nullptr, 0}) {
   if (c->plan.engine == ENGINE_SC) {
     if (c->sc_kernel == 1)
       HB_CUDA(c, launch_sweep_sc_staged(c->stream, c->spins, c->sc, c->staged_zt, p, colour, d));
     else
-      HB_CUDA(c, launch_sweep_sc(c->stream, c->spins, c->sc, c->tile, p, colour, d));
+      HB_CUDA(c, launch_sweep_sc(c->stream, c->spins, c->sc, c->tile, p, colour, d, m));
   } else if (c->plan.engine == ENGINE_BRAVAIS) {
     HB_CUDA(c, launch_sweep_bravais(c->stream, c->spins, c->br, c->tile, p, colour, d));
   } else {
@@ -187,11 +192,26 @@ int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d) {
   return HB_OK;
 }
 
-int one_sweep(hb_ctx* c, float beta, Diag d) {
+// blocks per colour launch if this context can fuse the measurement into its colour passes, else 0
+int fused_blocks(const hb_ctx* c) {
+  if (!c->fused_measure || c->plan.engine != ENGINE_SC || c->sc_kernel != 0) return 0;
+  return sc_fused_blocks(c->sc, c->tile);
+}
+
+// one sweep; with dev_out != nullptr (and fused_blocks() > 0) the colour passes also reduce M and E of
+// the state they leave behind, and dev_out receives (sum Sx, sum Sy, sum Sz, E)
+int one_sweep(hb_ctx* c, float beta, Diag d, double* dev_out = nullptr) {
   const SweepParams p = params(c, beta);
+  const int fb = dev_out ? fused_blocks(c) : 0;
   for (int colour = 0; colour < c->n_colours; ++colour) {
-    const int rc = one_colour(c, colour, p, d);
+    Meas m{nullptr, 0};
+    if (fb) m = Meas{c->partials() + (size_t)colour * fb * 4, colour == c->n_colours - 1 ? 2 : 1};
+    const int rc = one_colour(c, colour, p, d, m);
     if (rc != HB_OK) return rc;
+  }
+  if (fb) {
+    HB_CUDA(c, launch_reduce_final(c->stream, c->partials(), c->n_colours * fb, dev_out));
+    c->launches += 1;
   }
   c->sweep += 1;
   c->attempts += (uint64_t)c->plan.n;
@@ -385,6 +405,7 @@ int hb_destroy(hb_ctx* c) {
 
 int hb_init_random(hb_ctx* c) {
   HB_CHECK_CTX(c);
+  c->cache_valid = false;
   if (c->plan.engine == ENGINE_SC)
     HB_CUDA(c, launch_init_random_sc(c->stream, c->spins, c->sc, (uint32_t)c->seed, (uint32_t)(c->seed >> 32)));
   else
@@ -397,6 +418,7 @@ int hb_init_random(hb_ctx* c) {
 int hb_init_aligned(hb_ctx* c, const float dir[3]) {
   HB_CHECK_CTX(c);
   if (!dir || !unit_vector(dir)) return fail(c, HB_EINVAL, "dir must be a unit vector");
+  c->cache_valid = false;
   HB_CUDA(c, launch_fill(c->stream, c->spins, (uint32_t)c->plan.n, dir[0], dir[1], dir[2]));
   c->launches += 1;
   c->initialised = true;
@@ -405,6 +427,7 @@ int hb_init_aligned(hb_ctx* c, const float dir[3]) {
 
 int hb_set_spins(hb_ctx* c, const float* sx, const float* sy, const float* sz) {
   HB_CHECK_CTX(c);
+  c->cache_valid = false;
   if (!sx || !sy || !sz) return fail(c, HB_EINVAL, "NULL spin array");
   const size_t n = (size_t)c->plan.n;
   const float* src[3] = {sx, sy, sz};
@@ -448,10 +471,13 @@ int hb_sweep(hb_ctx* c, float T, int64_t n_sweeps) {
   float beta;
   int rc = check_T(c, T, &beta);
   if (rc != HB_OK) return rc;
+  if (n_sweeps > 0) c->cache_valid = false;
+  const bool fuse = fused_blocks(c) > 0;
   for (int64_t s = 0; s < n_sweeps; ++s) {
-    rc = one_sweep(c, beta, Diag{nullptr, nullptr});
+    rc = one_sweep(c, beta, Diag{nullptr, nullptr}, (fuse && s == n_sweeps - 1) ? c->cached() : nullptr);
     if (rc != HB_OK) return rc;
   }
+  if (fuse && n_sweeps > 0) c->cache_valid = true;
   return HB_OK;
 }
 
@@ -459,10 +485,13 @@ int hb_measure(hb_ctx* c, double M[3], double* E) {
   HB_CHECK_CTX(c);
   if (!M || !E) return fail(c, HB_EINVAL, "NULL output");
   if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
-  int rc = measure_into(c, c->series());
-  if (rc != HB_OK) return rc;
+  if (!c->cache_valid) {
+    const int rc = measure_into(c, c->cached());
+    if (rc != HB_OK) return rc;
+    c->cache_valid = true;
+  }
   double h[4];
-  HB_CUDA(c, cudaMemcpyAsync(h, c->series(), sizeof h, cudaMemcpyDeviceToHost, c->stream));
+  HB_CUDA(c, cudaMemcpyAsync(h, c->cached(), sizeof h, cudaMemcpyDeviceToHost, c->stream));
   HB_CUDA(c, cudaStreamSynchronize(c->stream));
   const double inv = 1.0 / (double)c->plan.n;
   M[0] = h[0] * inv; M[1] = h[1] * inv; M[2] = h[2] * inv;
@@ -479,13 +508,17 @@ int hb_sweep_series(hb_ctx* c, float T, int64_t n_sweeps, double* M_series, doub
   if (rc != HB_OK) return rc;
   std::vector<double> h((size_t)kSeriesChunk * 4);
   const double inv = 1.0 / (double)c->plan.n;
+  const bool fuse = fused_blocks(c) > 0;
+  if (n_sweeps > 0) c->cache_valid = false;
   for (int64_t s0 = 0; s0 < n_sweeps; s0 += kSeriesChunk) {
     const int64_t m = n_sweeps - s0 < kSeriesChunk ? n_sweeps - s0 : kSeriesChunk;
     for (int64_t s = 0; s < m; ++s) {
-      rc = one_sweep(c, beta, Diag{nullptr, nullptr});
+      rc = one_sweep(c, beta, Diag{nullptr, nullptr}, fuse ? c->series() + 4 * s : nullptr);
       if (rc != HB_OK) return rc;
-      rc = measure_into(c, c->series() + 4 * s);
-      if (rc != HB_OK) return rc;
+      if (!fuse) {
+        rc = measure_into(c, c->series() + 4 * s);
+        if (rc != HB_OK) return rc;
+      }
     }
     HB_CUDA(c, cudaMemcpyAsync(h.data(), c->series(), (size_t)m * 32, cudaMemcpyDeviceToHost, c->stream));
     HB_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -508,6 +541,7 @@ int hb_sweep_record(hb_ctx* c, float T, uint8_t* accept) {
   if (rc != HB_OK) return rc;
   uint8_t* d_acc = reinterpret_cast<uint8_t*>(c->staging());
   HB_CUDA(c, cudaMemsetAsync(d_acc, 0xFF, (size_t)c->plan.n, c->stream));   // every site must be overwritten
+  c->cache_valid = false;
   rc = one_sweep(c, beta, Diag{d_acc, c->counters()});
   if (rc != HB_OK) return rc;
   HB_CUDA(c, cudaMemcpyAsync(accept, d_acc, (size_t)c->plan.n, cudaMemcpyDeviceToHost, c->stream));
@@ -554,6 +588,11 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
   HB_CHECK_CTX(c);
   if (!name) return HB_EINVAL;
   const std::string s(name);
+  if (s == "fused_measure") {
+    if (value != 0 && value != 1) return fail(c, HB_EINVAL, "fused_measure: 0 or 1");
+    c->fused_measure = value != 0;
+    return HB_OK;
+  }
   if (s == "csr_block") {
     if (value < 32 || value > 256 || value % 32) return fail(c, HB_EINVAL, "csr_block: multiple of 32 in [32,256]");
     c->csr_block = (int)value;
@@ -561,7 +600,7 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
   }
   if (c->plan.engine == ENGINE_CSR) return fail(c, HB_EINVAL, "option not valid for this lattice");
   const bool is_sc = c->plan.engine == ENGINE_SC;
-  if (!is_sc && (s == "sc_kernel" || s == "sc_staged_zt" || s == "sc_prefetch"))
+  if (!is_sc && (s == "sc_kernel" || s == "sc_staged_zt" || s == "sc_prefetch" || s == "sc_linear"))
     return fail(c, HB_EINVAL, "option valid for the simple cubic lattice only");
   const int32_t rowH = is_sc ? c->sc.H : c->br.Lx, rowLz = is_sc ? c->sc.Lz : c->br.Lz;
   if (s == "sc_kernel") {
@@ -585,9 +624,14 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
   else if (s == "sc_ty") t.TY = (int)value;
   else if (s == "sc_zt") t.ZT = (int)value;
   else if (s == "sc_prefetch") { if (value < 0 || value > 3) return fail(c, HB_EINVAL, "sc_prefetch: 0..3"); t.PF = (int)value; }
+  else if (s == "sc_linear") {
+    if (value != 0 && (value < 32 || value > 256 || value % 32)) return fail(c, HB_EINVAL, "sc_linear: 0 or a multiple of 32 up to 256");
+    t.LIN = (int)value;
+  }
   else return fail(c, HB_EINVAL, "unknown option");
-  if (t.JX < 1 || t.TY < 1 || t.ZT < 1 || (int64_t)t.JX * t.TY > 256 || t.ZT > rowLz)
-    return fail(c, HB_EINVAL, "sc tile: JX, TY, ZT >= 1, JX*TY <= 256, ZT <= Lz");
+  const int64_t max_threads = (is_sc && t.V == 4) ? 1024 : 256;   // the big-block variants exist for sc, V = 4
+  if (t.JX < 1 || t.TY < 1 || t.ZT < 1 || (int64_t)t.JX * t.TY > max_threads || t.ZT > rowLz)
+    return fail(c, HB_EINVAL, "sc tile: JX, TY, ZT >= 1, JX*TY <= 256 (1024 for sc with V = 4), ZT <= Lz");
   c->tile = t;
   return HB_OK;
 }
@@ -596,11 +640,13 @@ int hb_get_option(hb_ctx* c, const char* name, int64_t* value) {
   if (!c || !name || !value) return HB_EINVAL;
   const std::string s(name);
   if (s == "csr_block") *value = c->csr_block;
+  else if (s == "fused_measure") *value = c->fused_measure ? 1 : 0;
   else if (s == "sc_v") *value = c->tile.V;
   else if (s == "sc_jx") *value = c->tile.JX;
   else if (s == "sc_ty") *value = c->tile.TY;
   else if (s == "sc_zt") *value = c->tile.ZT;
   else if (s == "sc_prefetch") *value = c->tile.PF;
+  else if (s == "sc_linear") *value = c->tile.LIN;
   else if (s == "engine") *value = c->plan.engine;
   else if (s == "sc_kernel") *value = c->sc_kernel;
   else if (s == "sc_staged_zt") *value = c->staged_zt;

@@ -210,7 +210,7 @@ __global__ void __launch_bounds__(256)
 k_measure_bravais(const float* __restrict__ s, BrLayout L, SweepParams P, double* partials) {
   double mx = 0, my = 0, mz = 0, en = 0;
   measure_sub<KIND, 0, V>(s, L, P, mx, my, mz, en);
-  block_reduce4(mx, my, mz, en, partials);
+  block_reduce4(mx, my, mz, en, partials + (size_t)blockIdx.x * 4);
 }
 
 inline int aniso_of(const SweepParams& p) {

@@ -28,6 +28,7 @@ struct ScLayout {
 struct ScTile {
   int32_t V, JX, TY, ZT;
   int32_t PF;   // software prefetch of the next z-plane: 0 none, 1 L2, 2 L1, 3 touch
+  int32_t LIN;  // 0: JX x TY tile; else threads per block of the linear (y, j) mapping (full warps)
 };
 
 // periodic Bravais lattice with a basis (bcc: 2 sublattices, fcc: 4), canonical storage:
@@ -56,12 +57,21 @@ struct Diag {
   unsigned long long* n_accept;     // or nullptr
 };
 
+// measurement fused into a colour pass (sc, two colours): block partials of (sum S, energy terms)
+struct Meas {
+  double* partials;   // 4 doubles per block of the launch, or nullptr
+  int mode;           // 0 off, 1 own spins + anisotropy energy, 2 also the exchange energy (last colour)
+};
+constexpr int kFusedBlocksMax = 16384;   // per colour: larger grids use the separate measurement pass
+
 // ---- kernels (hb_kernels.cu); every launcher returns the launch status -----------------
 cudaError_t launch_init_random_sc(cudaStream_t st, float* spins, ScLayout L, uint32_t seed_lo, uint32_t seed_hi);
 cudaError_t launch_init_random_flat(cudaStream_t st, float* spins, uint32_t n, uint32_t seed_lo, uint32_t seed_hi);
 cudaError_t launch_fill(cudaStream_t st, float* spins, uint32_t n, float x, float y, float z);
 cudaError_t launch_sc_permute(cudaStream_t st, float* dst, const float* src, ScLayout L, bool to_internal);
-cudaError_t launch_sweep_sc(cudaStream_t st, float* spins, ScLayout L, ScTile t, SweepParams p, int colour, Diag d);
+cudaError_t launch_sweep_sc(cudaStream_t st, float* spins, ScLayout L, ScTile t, SweepParams p, int colour, Diag d, Meas m);
+// blocks one launch_sweep_sc launch uses with this tile if it can carry the fused measurement, else 0
+int sc_fused_blocks(const ScLayout& L, const ScTile& t);
 bool sc_staged_supported(const ScLayout& L);
 cudaError_t launch_sweep_sc_staged(cudaStream_t st, float* spins, ScLayout L, int ZT, SweepParams p, int colour, Diag d);
 cudaError_t launch_sweep_csr(cudaStream_t st, float* spins, CsrDev g, uint32_t list_begin, uint32_t list_count,

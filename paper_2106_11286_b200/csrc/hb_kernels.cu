@@ -112,23 +112,39 @@ __device__ __forceinline__ Vec<V> sc_field_off(const float* __restrict__ b, uint
   return h;
 }
 
-template <int V, int ANISO, bool DIAG, int PF>
-__global__ void __launch_bounds__(256, HB_SC_MINBLOCKS)
+// MEAS: the pass also reduces what a measurement needs from the spins it has just decided (SURVEY 8(a)
+// note on fusing a5 into a4): every colour adds its own final spins to M and its anisotropy energy;
+// the LAST colour (m.mode == 2) sees only final neighbours, and since every bond of a 2-colour lattice
+// has exactly one end in it, -J sum_{i in last colour} S_i.h_i is the whole exchange energy.
+template <int V, int ANISO, bool DIAG, int PF, int BLK = 256, bool MEAS = false>
+__global__ void __launch_bounds__(BLK, (MEAS ? 3 : HB_SC_MINBLOCKS) * 256 / BLK)   // MEAS needs ~80 registers
 k_sweep_sc(float* __restrict__ ax, float* __restrict__ ay, float* __restrict__ az,
            const float* __restrict__ bx, const float* __restrict__ by, const float* __restrict__ bz,
-           ScLayout L, ScTile t, SweepParams P, int colour, Diag d) {
-  const int32_t tj = threadIdx.x % t.JX, ty = threadIdx.x / t.JX;
-  const int32_t j = blockIdx.x * t.JX + tj;
-  const int32_t y = blockIdx.y * t.TY + ty;
+           ScLayout L, ScTile t, SweepParams P, int colour, Diag d, Meas m) {
+  int32_t j, y;
+  if (t.LIN) {
+    // linear mapping: the block owns blockDim.x consecutive (y, j) slots, so every warp is full
+    // even when a row does not hold a multiple of 32 vectors (L = 464: 116 vectors per row)
+    const int32_t HV = L.H / V;
+    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    y = (int32_t)(s / (uint32_t)HV);
+    j = (int32_t)(s - (uint32_t)y * (uint32_t)HV);
+  } else {
+    const int32_t tj = threadIdx.x % t.JX, ty = threadIdx.x / t.JX;
+    j = blockIdx.x * t.JX + tj;
+    y = blockIdx.y * t.TY + ty;
+  }
   const int32_t i0 = j * V;
-  if (i0 >= L.H || y >= L.Ly) return;
+  const bool outside = i0 >= L.H || y >= L.Ly;
+  if (!MEAS && outside) return;
   const uint32_t H = (uint32_t)L.H, plane = (uint32_t)L.Ly * H;
   const uint32_t ym = (uint32_t)((y == 0) ? L.Ly - 1 : y - 1) * H + (uint32_t)i0;
   const uint32_t yp = (uint32_t)((y == L.Ly - 1) ? 0 : y + 1) * H + (uint32_t)i0;
   const uint32_t yc = (uint32_t)y * H + (uint32_t)i0;
   const int32_t z0 = blockIdx.z * t.ZT;
-  const int32_t z1 = min(z0 + t.ZT, L.Lz);
+  const int32_t z1 = (MEAS && outside) ? z0 : min(z0 + t.ZT, L.Lz);   // MEAS: every thread reaches the block reduction
   unsigned n_acc = 0;
+  double acc_mx = 0.0, acc_my = 0.0, acc_mz = 0.0, acc_en = 0.0;
   for (int32_t z = z0; z < z1; ++z) {
     const uint32_t pz = (uint32_t)z * plane;
     const uint32_t pzm = (uint32_t)((z == 0) ? L.Lz - 1 : z - 1) * plane;
@@ -179,8 +195,25 @@ k_sweep_sc(float* __restrict__ ax, float* __restrict__ ay, float* __restrict__ a
       store<V>(ay + oc, sy);
       store<V>(az + oc, sz);
     }
+    if (MEAS) {
+      // fp32 per-site terms, summed over the thread's V sites in fp32, accumulated in fp64
+      float gx = 0.0f, gy = 0.0f, gz = 0.0f, ge = 0.0f;
+      const float Jx = (m.mode == 2) ? -P.J : 0.0f;
+#pragma unroll
+      for (int k = 0; k < V; ++k) {
+        gx = __fadd_rn(gx, sx.v[k]); gy = __fadd_rn(gy, sy.v[k]); gz = __fadd_rn(gz, sz.v[k]);
+        const float sh = __fmaf_rn(sz.v[k], hz.v[k], __fmaf_rn(sy.v[k], hy.v[k], __fmul_rn(sx.v[k], hx.v[k])));
+        const float a = __fmaf_rn(sz.v[k], P.ez, __fmaf_rn(sy.v[k], P.ey, __fmul_rn(sx.v[k], P.ex)));
+        ge = __fadd_rn(ge, __fmaf_rn(Jx, sh, __fmul_rn(-P.K, __fmul_rn(a, a))));
+      }
+      acc_mx += (double)gx; acc_my += (double)gy; acc_mz += (double)gz; acc_en += (double)ge;
+    }
   }
   if (DIAG && d.n_accept && n_acc) atomicAdd(d.n_accept, (unsigned long long)n_acc);
+  if (MEAS) {
+    const uint32_t blk = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+    block_reduce4(acc_mx, acc_my, acc_mz, acc_en, m.partials + (size_t)blk * 4);
+  }
 }
 
 // ---- simple cubic, neighbour planes staged in shared memory by bulk async copies (TMA 1-D) --------
@@ -452,7 +485,7 @@ k_measure_sc(const float* __restrict__ sx, const float* __restrict__ sy, const f
       en += (double)site_energy(ox.v[k], oy.v[k], oz.v[k], hx.v[k], hy.v[k], hz.v[k], P.J, P.K, P.ex, P.ey, P.ez);
     }
   }
-  block_reduce4(mx, my, mz, en, partials);
+  block_reduce4(mx, my, mz, en, partials + (size_t)blockIdx.x * 4);
 }
 
 __global__ void __launch_bounds__(256)
@@ -479,7 +512,7 @@ k_measure_csr(const float* __restrict__ sx, const float* __restrict__ sy, const 
     mx += (double)ox; my += (double)oy; mz += (double)oz;
     en += (double)site_energy(ox, oy, oz, hx, hy, hz, P.J, K, ex, ey, ez);
   }
-  block_reduce4(mx, my, mz, en, partials);
+  block_reduce4(mx, my, mz, en, partials + (size_t)blockIdx.x * 4);
 }
 
 inline int grid_for(uint32_t n, int block, int cap) {
@@ -514,41 +547,70 @@ inline int aniso_case(const SweepParams& p) {
   return (p.K == 0.0f) ? ANISO_NONE : ((p.ex == 0.0f && p.ey == 0.0f && p.ez == 1.0f) ? ANISO_Z : ANISO_GENERAL);
 }
 
+// launch shape of k_sweep_sc for a tile
+static void sc_launch_shape(const ScLayout& L, const ScTile& t, int V, dim3& grid, int& threads) {
+  const int HV = L.H / V;
+  threads = t.LIN ? t.LIN : t.JX * t.TY;
+  grid = dim3((HV + t.JX - 1) / t.JX, (L.Ly + t.TY - 1) / t.TY, (L.Lz + t.ZT - 1) / t.ZT);
+  if (t.LIN) grid = dim3((unsigned)(((long long)HV * L.Ly + threads - 1) / threads), 1, (L.Lz + t.ZT - 1) / t.ZT);
+}
+
+int sc_fused_blocks(const ScLayout& L, const ScTile& t) {
+  if (t.V != 4) return 0;                    // the fused measurement is built for the tuned vector width
+  dim3 grid; int threads;
+  sc_launch_shape(L, t, 4, grid, threads);
+  const long long blocks = (long long)grid.x * grid.y * grid.z;
+  return blocks <= kFusedBlocksMax ? (int)blocks : 0;
+}
+
 template <int V, int ANISO, bool DIAG>
-static cudaError_t sweep_sc_impl(cudaStream_t st, float* s, ScLayout L, ScTile t, SweepParams p, int colour, Diag d) {
+static cudaError_t sweep_sc_impl(cudaStream_t st, float* s, ScLayout L, ScTile t, SweepParams p, int colour, Diag d, Meas m) {
+  int threads = t.LIN ? t.LIN : t.JX * t.TY;
   auto kern = k_sweep_sc<V, ANISO, DIAG, 0>;
-  if (!DIAG && V == 4) {   // the tuned configuration carries the prefetch variants
-    switch (t.PF) {
-      case 1: kern = k_sweep_sc<V, ANISO, DIAG, (!DIAG && V == 4) ? 1 : 0>; break;
-      case 2: kern = k_sweep_sc<V, ANISO, DIAG, (!DIAG && V == 4) ? 2 : 0>; break;
-      case 3: kern = k_sweep_sc<V, ANISO, DIAG, (!DIAG && V == 4) ? 3 : 0>; break;
+  constexpr bool TUNED = !DIAG && V == 4;   // the tuned configuration carries the prefetch, big-block and fused-measurement variants
+  constexpr int P1 = TUNED ? 1 : 0, B512 = TUNED ? 512 : 256, B1024 = TUNED ? 1024 : 256;
+  if (m.mode != 0 && !TUNED) return cudaErrorInvalidValue;
+  if (TUNED) {
+    if (m.mode != 0) {
+      if (threads > 512) kern = k_sweep_sc<V, ANISO, DIAG, P1, B1024, TUNED>;
+      else if (threads > 256) kern = k_sweep_sc<V, ANISO, DIAG, P1, B512, TUNED>;
+      else kern = k_sweep_sc<V, ANISO, DIAG, P1, 256, TUNED>;
+    } else if (threads > 512) kern = t.PF ? k_sweep_sc<V, ANISO, DIAG, P1, B1024> : k_sweep_sc<V, ANISO, DIAG, 0, B1024>;
+    else if (threads > 256) kern = t.PF ? k_sweep_sc<V, ANISO, DIAG, P1, B512> : k_sweep_sc<V, ANISO, DIAG, 0, B512>;
+    else switch (t.PF) {
+      case 1: kern = k_sweep_sc<V, ANISO, DIAG, P1>; break;
+      case 2: kern = k_sweep_sc<V, ANISO, DIAG, TUNED ? 2 : 0>; break;
+      case 3: kern = k_sweep_sc<V, ANISO, DIAG, TUNED ? 3 : 0>; break;
       default: break;
     }
+  } else if (threads > 256) {   // the other variants are built for blocks of up to 256 threads: shrink the tile
+    if (t.JX > 256) t.JX = 256;
+    t.TY = 256 / t.JX;
   }
   const size_t n = L.n;
   float* a = s + (size_t)colour * L.half;
   const float* b = s + (size_t)(1 - colour) * L.half;
-  const int HV = L.H / V;
-  dim3 grid((HV + t.JX - 1) / t.JX, (L.Ly + t.TY - 1) / t.TY, (L.Lz + t.ZT - 1) / t.ZT);
-  kern<<<grid, t.JX * t.TY, 0, st>>>(a, a + n, a + 2 * n, b, b + n, b + 2 * n, L, t, p, colour, d);
+  dim3 grid;
+  sc_launch_shape(L, t, V, grid, threads);
+  kern<<<grid, threads, 0, st>>>(a, a + n, a + 2 * n, b, b + n, b + 2 * n, L, t, p, colour, d, m);
   return cudaGetLastError();
 }
 
 template <int V, bool DIAG>
-static cudaError_t sweep_sc_aniso(cudaStream_t st, float* s, ScLayout L, ScTile t, SweepParams p, int colour, Diag d) {
+static cudaError_t sweep_sc_aniso(cudaStream_t st, float* s, ScLayout L, ScTile t, SweepParams p, int colour, Diag d, Meas m) {
   switch (aniso_case(p)) {
-    case ANISO_NONE: return sweep_sc_impl<V, ANISO_NONE, DIAG>(st, s, L, t, p, colour, d);
-    case ANISO_Z: return sweep_sc_impl<V, ANISO_Z, DIAG>(st, s, L, t, p, colour, d);
-    default: return sweep_sc_impl<V, ANISO_GENERAL, DIAG>(st, s, L, t, p, colour, d);
+    case ANISO_NONE: return sweep_sc_impl<V, ANISO_NONE, DIAG>(st, s, L, t, p, colour, d, m);
+    case ANISO_Z: return sweep_sc_impl<V, ANISO_Z, DIAG>(st, s, L, t, p, colour, d, m);
+    default: return sweep_sc_impl<V, ANISO_GENERAL, DIAG>(st, s, L, t, p, colour, d, m);
   }
 }
 
-cudaError_t launch_sweep_sc(cudaStream_t st, float* s, ScLayout L, ScTile t, SweepParams p, int colour, Diag d) {
+cudaError_t launch_sweep_sc(cudaStream_t st, float* s, ScLayout L, ScTile t, SweepParams p, int colour, Diag d, Meas m) {
   const bool diag = d.accept || d.n_accept;
   switch (t.V) {
-    case 4: return diag ? sweep_sc_aniso<4, true>(st, s, L, t, p, colour, d) : sweep_sc_aniso<4, false>(st, s, L, t, p, colour, d);
-    case 2: return diag ? sweep_sc_aniso<2, true>(st, s, L, t, p, colour, d) : sweep_sc_aniso<2, false>(st, s, L, t, p, colour, d);
-    default: return diag ? sweep_sc_aniso<1, true>(st, s, L, t, p, colour, d) : sweep_sc_aniso<1, false>(st, s, L, t, p, colour, d);
+    case 4: return diag ? sweep_sc_aniso<4, true>(st, s, L, t, p, colour, d, m) : sweep_sc_aniso<4, false>(st, s, L, t, p, colour, d, m);
+    case 2: return diag ? sweep_sc_aniso<2, true>(st, s, L, t, p, colour, d, m) : sweep_sc_aniso<2, false>(st, s, L, t, p, colour, d, m);
+    default: return diag ? sweep_sc_aniso<1, true>(st, s, L, t, p, colour, d, m) : sweep_sc_aniso<1, false>(st, s, L, t, p, colour, d, m);
   }
 }
 

@@ -210,3 +210,76 @@ def test_full_size_first_10_sweeps(name):
     st.sweep(T, 2)
     if mism == 0:
         assert spins_equal(ctx.get_spins(), st.get_spins())
+
+
+# ---- P3: long-run statistics against the fp64 random-site oracle (BASELINE.json north_star) ----------
+# <|M|> and <E>/N of the CUDA path must lie within 3 standard errors of O64.  Standard errors come from
+# R independent replicas on each side (replica means, Welch), not from one autocorrelated series
+# (SURVEY.md 8(c) P3).  c1 runs at full size; the other kinds at the reduced shapes the oracle finishes
+# in seconds, one temperature of their scan each.
+P3_CASES = {
+    "c1": (W.CONFIGS["c1"], 1.2, 500, 500),
+    "bcc8": (W.SMALL["c2"], 1.6, 300, 500),
+    "fcc6": (dict(W.SMALL["c3"], start="random"), 2.6, 300, 500),
+    "sphere5": (W.SMALL["c5"], 1.5, 300, 500),
+}
+
+
+@pytest.mark.parametrize("name", sorted(P3_CASES))
+def test_long_run_statistics_within_3_standard_errors_of_o64(name):
+    cfg, T, equil, meas = P3_CASES[name]
+    reps = 16
+    lat, _ = make_oracle(cfg)
+    g_m, g_e, o_m, o_e = [], [], [], []
+    for r in range(reps):
+        ctx = make_gpu(dict(cfg, seed=1000 + r))
+        ctx.init_random()
+        ctx.sweep(T, equil)
+        M, E = ctx.sweep_series(T, meas)
+        g_m.append(np.linalg.norm(M, axis=1).mean())
+        g_e.append(E.mean() / lat.n)
+        ctx.close()
+        st = oracle.State64(lat, cfg["J"], 2000 + r)
+        st.init_random()
+        st.sweep(T, equil)
+        m, e, _ = st.series(T, meas)
+        o_m.append(m.mean())
+        o_e.append(e.mean() / lat.n)
+    for what, x, y in (("|M|", g_m, o_m), ("E/N", g_e, o_e)):
+        x, y = np.array(x), np.array(y)
+        se = math.sqrt(x.var(ddof=1) / reps + y.var(ddof=1) / reps)
+        print("%s %s: gpu %.6f  o64 %.6f  diff %.2e  se %.2e" % (name, what, x.mean(), y.mean(), x.mean() - y.mean(), se))
+        assert abs(x.mean() - y.mean()) < 3 * se, (name, what, x.mean(), y.mean(), se)
+
+
+def test_fused_measurement_equals_the_separate_pass():
+    # hb_sweep's last sweep also reduces M and E (SURVEY 8(a) note on fusing a5 into a4); hb_measure then
+    # returns those.  Same P2 tolerances against the oracle, and against the separate pass on the same state.
+    for cfg, opts in ((W.SMALL["c4"], {}), (W.SMALL["c1"], {}),
+                      (dict(W.SMALL["c4"], L=(40, 12, 10), K=0.3, e=(0.6, 0.0, 0.8)), {"sc_jx": 3, "sc_ty": 5, "sc_zt": 3}),
+                      (dict(W.SMALL["c4"], L=(64, 8, 6)), {"sc_linear": 96})):
+        lat, st = make_oracle(cfg)
+        fused, plain = make_gpu(cfg), make_gpu(cfg)
+        plain.set_option("fused_measure", 0)
+        for k, v in opts.items():
+            fused.set_option(k, v)
+        start(cfg, fused, st)
+        plain.init_random() if cfg["start"] == "random" else plain.init_aligned(cfg["e"])
+        for T, k in ((1.44, 3), (0.4, 2)):
+            fused.sweep(T, k)
+            plain.sweep(T, k)
+            st.sweep(T, k)
+            l0, _ = fused.counters()
+            Mf, Ef = fused.measure()
+            l1, _ = fused.counters()
+            assert l1 == l0                                           # no extra pass was launched
+            Mp, Ep = plain.measure()
+            Mo, Eo32, Eo64 = st.measure()
+            assert np.max(np.abs(Mf - Mo)) <= 1e-7 and np.max(np.abs(Mf - Mp)) <= 1e-7
+            assert abs(Ef - Eo32) <= 1e-6 * lat.n and abs(Ef - Eo64) <= 1e-6 * lat.n and abs(Ef - Ep) <= 1e-6 * lat.n
+        assert spins_equal(fused.get_spins(), st.get_spins())
+        # a state change invalidates the cached measurement
+        S = W.random_unit_vectors(lat.n, 11)
+        fused.set_spins(S[:, 0], S[:, 1], S[:, 2])
+        st.set_spins(S[:, 0], S[:, 1], S[:, 2])
+        _measure_close(fused, st, lat.n)
