@@ -15,6 +15,7 @@ namespace {
 
 constexpr size_t kAlign = 256;
 constexpr int kSeriesChunk = 1024;
+constexpr int64_t kMaxColours = 65536;   // bound on the colour count the ELL workspace is sized for
 
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
@@ -24,6 +25,9 @@ struct Plan {                 // device memory plan of a lattice
   int64_t n = 0, nnz = 0;
   int engine = ENGINE_CSR;
   bool per_site = false;
+  bool ell = false;           // table engine: colour-major ELL layout (else plain CSR in canonical order)
+  int32_t maxdeg = 0;
+  size_t off_ell = 0, off_cbegin = 0;
   size_t spins_bytes = 0, ws_bytes = 0;
   size_t off_partials = 0, off_series = 0, off_counters = 0, off_staging = 0;
   size_t off_row_ptr = 0, off_col = 0, off_list = 0, off_K = 0, off_e = 0;
@@ -39,6 +43,7 @@ int make_plan(const hb_lattice* lat, Plan& p, std::string& why) {
     const int z = k == HB_SC ? 6 : (k == HB_BCC ? 8 : 12);
     p.n = cells * basis;
     p.nnz = p.n * z;
+    p.maxdeg = z;
     if (k == HB_SC && ((lat->Lx | lat->Ly | lat->Lz) & 1)) {
       why = "simple cubic needs even Lx, Ly, Lz (two-colour checkerboard with periodic wrap)";
       return HB_EINVAL;
@@ -47,6 +52,12 @@ int make_plan(const hb_lattice* lat, Plan& p, std::string& why) {
     if (lat->n_sites < 0 || !lat->row_ptr) { why = "CSR lattice needs n_sites >= 0 and row_ptr"; return HB_EINVAL; }
     p.n = lat->n_sites;
     p.nnz = lat->row_ptr[lat->n_sites];
+    int64_t md = 0;
+    for (int64_t i = 0; i < p.n; ++i) {
+      const int64_t deg = lat->row_ptr[i + 1] - lat->row_ptr[i];
+      if (deg > md) md = deg;
+    }
+    p.maxdeg = (int32_t)(md > 0x7FFFFFFF ? 0x7FFFFFFF : md);
   } else {
     why = "unknown lattice kind";
     return HB_EINVAL;
@@ -58,7 +69,6 @@ int make_plan(const hb_lattice* lat, Plan& p, std::string& why) {
   p.per_site = lat->K_site != nullptr;
   // implicit indexing for the periodic kinds; the table engine for CSR input and per-site anisotropy
   p.engine = p.per_site || k == HB_CSR ? ENGINE_CSR : (k == HB_SC ? ENGINE_SC : ENGINE_BRAVAIS);
-  p.spins_bytes = align_up(3 * (size_t)p.n * sizeof(float));
   size_t o = 0;
   const size_t n_partials = kMeasureBlocks > 2 * kFusedBlocksMax ? kMeasureBlocks : 2 * kFusedBlocksMax;
   p.off_partials = o; o += align_up(n_partials * 4 * sizeof(double));
@@ -66,8 +76,16 @@ int make_plan(const hb_lattice* lat, Plan& p, std::string& why) {
   p.off_counters = o; o += kAlign;
   p.off_staging = o;  o += align_up((size_t)p.n * sizeof(float));
   if (p.engine == ENGINE_CSR) {
-    p.off_row_ptr = o; o += align_up(((size_t)p.n + 1) * sizeof(int32_t));
-    p.off_col = o;     o += align_up((size_t)p.nnz * sizeof(int32_t));
+    // ELL when padding every row to the maximum degree costs little (regular lattices, cut-outs of them);
+    // graphs with a few high-degree sites keep the plain CSR kernel
+    p.ell = p.maxdeg >= 1 && p.maxdeg <= 64 && (int64_t)p.maxdeg * p.n <= 2 * p.nnz + 1024;
+    if (p.ell) {
+      p.off_ell = o;    o += align_up((size_t)p.maxdeg * (size_t)p.n * sizeof(int32_t));
+      p.off_cbegin = o; o += align_up(((size_t)(p.n < kMaxColours ? p.n : kMaxColours) + 2) * sizeof(uint32_t));
+    } else {
+      p.off_row_ptr = o; o += align_up(((size_t)p.n + 1) * sizeof(int32_t));
+      p.off_col = o;     o += align_up((size_t)p.nnz * sizeof(int32_t));
+    }
     p.off_list = o;    o += align_up((size_t)p.n * sizeof(int32_t));
     if (p.per_site) {
       p.off_K = o; o += align_up((size_t)p.n * sizeof(float));
@@ -75,6 +93,7 @@ int make_plan(const hb_lattice* lat, Plan& p, std::string& why) {
     }
   }
   p.ws_bytes = o;
+  p.spins_bytes = align_up((p.ell ? 4 : 3) * (size_t)p.n * sizeof(float));   // ELL engine: AoS float4
   return HB_OK;
 }
 
@@ -87,6 +106,7 @@ struct hb_ctx {
   BrLayout br{};
   ScTile tile{};
   CsrDev csr{};
+  EllDev ell{};
   int csr_block = 128;
   int sc_kernel = 0;      // 0: direct loads through L1, 1: neighbour planes staged in shared memory
   int staged_zt = 16;
@@ -186,7 +206,8 @@ int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d, Meas m = Mea
   } else {
     const uint32_t b = c->colour_begin[colour], e = c->colour_begin[colour + 1];
     if (e == b) return HB_OK;
-    HB_CUDA(c, launch_sweep_csr(c->stream, c->spins, c->csr, b, e - b, p, c->csr_block, d));
+    if (c->plan.ell) HB_CUDA(c, launch_sweep_ell(c->stream, c->spins, c->ell, b, e - b, p, c->csr_block, d));
+    else HB_CUDA(c, launch_sweep_csr(c->stream, c->spins, c->csr, b, e - b, p, c->csr_block, d));
   }
   c->launches += 1;
   return HB_OK;
@@ -224,6 +245,8 @@ int measure_into(hb_ctx* c, double* dev_out) {
     HB_CUDA(c, launch_measure_sc(c->stream, c->spins, c->sc, c->tile.V, p, c->partials(), dev_out));
   else if (c->plan.engine == ENGINE_BRAVAIS)
     HB_CUDA(c, launch_measure_bravais(c->stream, c->spins, c->br, c->tile.V, p, c->partials(), dev_out));
+  else if (c->plan.ell)
+    HB_CUDA(c, launch_measure_ell(c->stream, c->spins, c->ell, p, c->partials(), dev_out));
   else
     HB_CUDA(c, launch_measure_csr(c->stream, c->spins, c->csr, p, c->partials(), dev_out));
   c->launches += 2;
@@ -368,27 +391,67 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
     for (int64_t i = 0; i < P.n; ++i) count[c->colour_host[i] + 1] += 1;
     for (int k = 0; k < c->n_colours; ++k) count[k + 1] += count[k];
     c->colour_begin = count;
+    if (c->n_colours > kMaxColours) { c->sticky = HB_EINVAL; return fail(c, HB_EINVAL, "more than 65536 colours"); }
     std::vector<int32_t> list((size_t)P.n);
     {
       std::vector<uint32_t> cur(count.begin(), count.end() - 1);
       for (int64_t i = 0; i < P.n; ++i) list[cur[c->colour_host[i]]++] = (int32_t)i;
     }
-    std::vector<int32_t> rp32((size_t)P.n + 1);
-    for (int64_t i = 0; i <= P.n; ++i) rp32[i] = (int32_t)row_ptr[i];
-    int32_t* d_rp = reinterpret_cast<int32_t*>(c->ws + P.off_row_ptr);
-    int32_t* d_col = reinterpret_cast<int32_t*>(c->ws + P.off_col);
     int32_t* d_list = reinterpret_cast<int32_t*>(c->ws + P.off_list);
-    HB_CUDA(c, cudaMemcpyAsync(d_rp, rp32.data(), rp32.size() * 4, cudaMemcpyHostToDevice, c->stream));
-    if (P.nnz) HB_CUDA(c, cudaMemcpyAsync(d_col, col, (size_t)P.nnz * 4, cudaMemcpyHostToDevice, c->stream));
     HB_CUDA(c, cudaMemcpyAsync(d_list, list.data(), list.size() * 4, cudaMemcpyHostToDevice, c->stream));
-    c->csr.n = (uint32_t)P.n; c->csr.row_ptr = d_rp; c->csr.col = d_col; c->csr.list = d_list;
-    c->csr.K_site = nullptr; c->csr.e_site = nullptr;
-    if (P.per_site) {
-      float* d_K = reinterpret_cast<float*>(c->ws + P.off_K);
-      float* d_e = reinterpret_cast<float*>(c->ws + P.off_e);
-      HB_CUDA(c, cudaMemcpyAsync(d_K, lat->K_site, (size_t)P.n * 4, cudaMemcpyHostToDevice, c->stream));
-      HB_CUDA(c, cudaMemcpyAsync(d_e, lat->e_site, (size_t)P.n * 12, cudaMemcpyHostToDevice, c->stream));
-      c->csr.K_site = d_K; c->csr.e_site = d_e;
+    std::vector<int32_t> rp32, ell;
+    std::vector<float> soa;
+    if (P.ell) {
+      // internal order m = position in the colour-sorted list; table entries are internal indices
+      std::vector<int32_t> inv((size_t)P.n);
+      for (int64_t m = 0; m < P.n; ++m) inv[list[m]] = (int32_t)m;
+      ell.assign((size_t)P.maxdeg * (size_t)P.n, -1);
+      for (int k = 0; k < c->n_colours; ++k) {
+        const size_t begin = count[k], nc = count[k + 1] - count[k];
+        for (size_t t = 0; t < nc; ++t) {
+          const int64_t id = list[begin + t];
+          int32_t* e0 = ell.data() + (size_t)P.maxdeg * begin + t;
+          for (int64_t q = row_ptr[id]; q < row_ptr[id + 1]; ++q) e0[(size_t)(q - row_ptr[id]) * nc] = inv[col[q]];
+        }
+      }
+      int32_t* d_ell = reinterpret_cast<int32_t*>(c->ws + P.off_ell);
+      uint32_t* d_cb = reinterpret_cast<uint32_t*>(c->ws + P.off_cbegin);
+      HB_CUDA(c, cudaMemcpyAsync(d_ell, ell.data(), ell.size() * 4, cudaMemcpyHostToDevice, c->stream));
+      HB_CUDA(c, cudaMemcpyAsync(d_cb, count.data(), count.size() * 4, cudaMemcpyHostToDevice, c->stream));
+      c->ell.n = (uint32_t)P.n; c->ell.maxdeg = (uint32_t)P.maxdeg; c->ell.ell = d_ell; c->ell.perm = d_list;
+      c->ell.colour_begin = d_cb; c->ell.n_colours = c->n_colours;
+      c->ell.K = c->ell.ex = c->ell.ey = c->ell.ez = nullptr;
+      if (P.per_site) {   // (K, e) in internal order, one plane each: K at off_K, ex|ey|ez at off_e
+        soa.resize(4 * (size_t)P.n);
+        for (int64_t m = 0; m < P.n; ++m) {
+          const int64_t id = list[m];
+          soa[m] = lat->K_site[id];
+          soa[(size_t)P.n + m] = lat->e_site[3 * id];
+          soa[2 * (size_t)P.n + m] = lat->e_site[3 * id + 1];
+          soa[3 * (size_t)P.n + m] = lat->e_site[3 * id + 2];
+        }
+        float* d_K = reinterpret_cast<float*>(c->ws + P.off_K);
+        float* d_e = reinterpret_cast<float*>(c->ws + P.off_e);
+        HB_CUDA(c, cudaMemcpyAsync(d_K, soa.data(), (size_t)P.n * 4, cudaMemcpyHostToDevice, c->stream));
+        HB_CUDA(c, cudaMemcpyAsync(d_e, soa.data() + P.n, (size_t)P.n * 12, cudaMemcpyHostToDevice, c->stream));
+        c->ell.K = d_K; c->ell.ex = d_e; c->ell.ey = d_e + P.n; c->ell.ez = d_e + 2 * (size_t)P.n;
+      }
+    } else {
+      rp32.resize((size_t)P.n + 1);
+      for (int64_t i = 0; i <= P.n; ++i) rp32[i] = (int32_t)row_ptr[i];
+      int32_t* d_rp = reinterpret_cast<int32_t*>(c->ws + P.off_row_ptr);
+      int32_t* d_col = reinterpret_cast<int32_t*>(c->ws + P.off_col);
+      HB_CUDA(c, cudaMemcpyAsync(d_rp, rp32.data(), rp32.size() * 4, cudaMemcpyHostToDevice, c->stream));
+      if (P.nnz) HB_CUDA(c, cudaMemcpyAsync(d_col, col, (size_t)P.nnz * 4, cudaMemcpyHostToDevice, c->stream));
+      c->csr.n = (uint32_t)P.n; c->csr.row_ptr = d_rp; c->csr.col = d_col; c->csr.list = d_list;
+      c->csr.K_site = nullptr; c->csr.e_site = nullptr;
+      if (P.per_site) {
+        float* d_K = reinterpret_cast<float*>(c->ws + P.off_K);
+        float* d_e = reinterpret_cast<float*>(c->ws + P.off_e);
+        HB_CUDA(c, cudaMemcpyAsync(d_K, lat->K_site, (size_t)P.n * 4, cudaMemcpyHostToDevice, c->stream));
+        HB_CUDA(c, cudaMemcpyAsync(d_e, lat->e_site, (size_t)P.n * 12, cudaMemcpyHostToDevice, c->stream));
+        c->csr.K_site = d_K; c->csr.e_site = d_e;
+      }
     }
     HB_CUDA(c, cudaStreamSynchronize(c->stream));   // the host vectors die at return
   }
@@ -408,6 +471,8 @@ int hb_init_random(hb_ctx* c) {
   c->cache_valid = false;
   if (c->plan.engine == ENGINE_SC)
     HB_CUDA(c, launch_init_random_sc(c->stream, c->spins, c->sc, (uint32_t)c->seed, (uint32_t)(c->seed >> 32)));
+  else if (c->plan.ell)
+    HB_CUDA(c, launch_init_random_perm(c->stream, c->spins, c->ell.perm, (uint32_t)c->plan.n, (uint32_t)c->seed, (uint32_t)(c->seed >> 32)));
   else
     HB_CUDA(c, launch_init_random_flat(c->stream, c->spins, (uint32_t)c->plan.n, (uint32_t)c->seed, (uint32_t)(c->seed >> 32)));
   c->launches += 1;
@@ -419,7 +484,8 @@ int hb_init_aligned(hb_ctx* c, const float dir[3]) {
   HB_CHECK_CTX(c);
   if (!dir || !unit_vector(dir)) return fail(c, HB_EINVAL, "dir must be a unit vector");
   c->cache_valid = false;
-  HB_CUDA(c, launch_fill(c->stream, c->spins, (uint32_t)c->plan.n, dir[0], dir[1], dir[2]));
+  if (c->plan.ell) HB_CUDA(c, launch_fill_ell(c->stream, c->spins, (uint32_t)c->plan.n, dir[0], dir[1], dir[2]));
+  else HB_CUDA(c, launch_fill(c->stream, c->spins, (uint32_t)c->plan.n, dir[0], dir[1], dir[2]));
   c->launches += 1;
   c->initialised = true;
   return HB_OK;
@@ -435,6 +501,10 @@ int hb_set_spins(hb_ctx* c, const float* sx, const float* sy, const float* sz) {
     if (c->plan.engine == ENGINE_SC) {
       HB_CUDA(c, cudaMemcpyAsync(c->staging(), src[k], n * 4, cudaMemcpyHostToDevice, c->stream));
       HB_CUDA(c, launch_sc_permute(c->stream, c->spins + k * n, c->staging(), c->sc, true));
+      c->launches += 1;
+    } else if (c->plan.ell) {
+      HB_CUDA(c, cudaMemcpyAsync(c->staging(), src[k], n * 4, cudaMemcpyHostToDevice, c->stream));
+      HB_CUDA(c, launch_permute_ell(c->stream, c->spins, c->staging(), c->ell.perm, (uint32_t)n, k, true));
       c->launches += 1;
     } else {
       HB_CUDA(c, cudaMemcpyAsync(c->spins + k * n, src[k], n * 4, cudaMemcpyHostToDevice, c->stream));
@@ -454,6 +524,10 @@ int hb_get_spins(hb_ctx* c, float* sx, float* sy, float* sz) {
   for (int k = 0; k < 3; ++k) {
     if (c->plan.engine == ENGINE_SC) {
       HB_CUDA(c, launch_sc_permute(c->stream, c->staging(), c->spins + k * n, c->sc, false));
+      c->launches += 1;
+      HB_CUDA(c, cudaMemcpyAsync(dst[k], c->staging(), n * 4, cudaMemcpyDeviceToHost, c->stream));
+    } else if (c->plan.ell) {
+      HB_CUDA(c, launch_permute_ell(c->stream, c->spins, c->staging(), c->ell.perm, (uint32_t)n, k, false));
       c->launches += 1;
       HB_CUDA(c, cudaMemcpyAsync(dst[k], c->staging(), n * 4, cudaMemcpyDeviceToHost, c->stream));
     } else {
@@ -648,6 +722,7 @@ int hb_get_option(hb_ctx* c, const char* name, int64_t* value) {
   else if (s == "sc_prefetch") *value = c->tile.PF;
   else if (s == "sc_linear") *value = c->tile.LIN;
   else if (s == "engine") *value = c->plan.engine;
+  else if (s == "ell") *value = c->plan.ell ? 1 : 0;
   else if (s == "sc_kernel") *value = c->sc_kernel;
   else if (s == "sc_staged_zt") *value = c->staged_zt;
   else return HB_EINVAL;

@@ -51,6 +51,20 @@ struct CsrDev {
   const float* e_site;      // 3n or nullptr
 };
 
+// Neighbour table in colour-major ELL form.  Spins are AoS float4 (x, y, z, 0) in INTERNAL order m
+// (sorted by colour, then canonical id); colour c owns m in [begin_c, begin_c + n_c).  Entry k of the
+// t-th site of colour c sits at ell[maxdeg*begin_c + k*n_c + t] (consecutive threads read consecutive
+// words), holds the internal index of the k-th neighbour in the caller's order, or -1 past the degree.
+struct EllDev {
+  uint32_t n, maxdeg;
+  const int32_t* ell;
+  const int32_t* perm;          // internal index -> canonical id (the Philox counter word)
+  const uint32_t* colour_begin; // n_colours + 1 entries (device copy, for the measurement pass)
+  int32_t n_colours;
+  const float* K;               // per-site anisotropy in internal order, SoA; or nullptr
+  const float* ex; const float* ey; const float* ez;
+};
+
 // diagnostics of one sweep
 struct Diag {
   uint8_t* accept;                  // n bytes (canonical id) or nullptr
@@ -76,6 +90,13 @@ bool sc_staged_supported(const ScLayout& L);
 cudaError_t launch_sweep_sc_staged(cudaStream_t st, float* spins, ScLayout L, int ZT, SweepParams p, int colour, Diag d);
 cudaError_t launch_sweep_csr(cudaStream_t st, float* spins, CsrDev g, uint32_t list_begin, uint32_t list_count,
                              SweepParams p, int block, Diag d);
+cudaError_t launch_sweep_ell(cudaStream_t st, float* spins, EllDev g, uint32_t begin, uint32_t count, SweepParams p,
+                             int block, Diag d);
+cudaError_t launch_measure_ell(cudaStream_t st, const float* spins, EllDev g, SweepParams p, double* partials, double* out);
+cudaError_t launch_init_random_perm(cudaStream_t st, float* spins, const int32_t* perm, uint32_t n, uint32_t seed_lo, uint32_t seed_hi);
+cudaError_t launch_fill_ell(cudaStream_t st, float* spins, uint32_t n, float x, float y, float z);
+// component comp of the internal float4 state <- plane[perm[m]] (to_internal) or plane[perm[m]] <- component
+cudaError_t launch_permute_ell(cudaStream_t st, float* spins, float* plane, const int32_t* perm, uint32_t n, int comp, bool to_internal);
 cudaError_t launch_sweep_bravais(cudaStream_t st, float* spins, BrLayout L, ScTile t, SweepParams p, int colour, Diag d);
 // measurement: partials must hold kMeasureBlocks*4 doubles; out receives (Mx*N, My*N, Mz*N, E)
 constexpr int kMeasureBlocks = 1184;

@@ -44,6 +44,14 @@ SMALL_CASES = {
     "fcc_ragged": dict(W.SMALL["c3"], L=(5, 3, 4), start="random"),
     "sphere5": W.SMALL["c5"],
     "sphere5_parity": dict(W.SMALL["c5"], colouring="parity"),
+    "sphere2": dict(W.SMALL["c5"], R=2),
+    # per-site anisotropy on the periodic kinds runs on the table engine (ELL, maxdeg 6 / 8 / 12)
+    "sc_persite": dict(W.SMALL["c4"], L=(6, 4, 8), K_site=np.linspace(-0.4, 0.6, 192).astype(np.float32),
+                       e_site=W.random_unit_vectors(192, 21)),
+    "bcc_persite": dict(W.SMALL["c2"], L=(4, 3, 5), K_site=np.linspace(0.5, -0.3, 120).astype(np.float32),
+                        e_site=W.random_unit_vectors(120, 22)),
+    "fcc_persite": dict(W.SMALL["c3"], L=(3, 4, 2), start="random", K_site=np.linspace(0.0, 0.8, 96).astype(np.float32),
+                        e_site=W.random_unit_vectors(96, 23)),
 }
 
 
@@ -97,6 +105,10 @@ def test_random_graph_greedy_colouring_and_per_site_anisotropy():
     lat, st = make_oracle(cfg)
     col, nc = ctx.colouring()                                    # both sides ran first-fit on their own
     assert nc == lat.n_colours and np.array_equal(col, lat.colour)
+    assert ctx.get_option("ell") == 0                            # irregular degrees: the plain CSR kernel
+    sph = make_gpu(W.SMALL["c5"])
+    assert sph.get_option("ell") == 1                            # a cut-out of a regular lattice: the ELL kernel
+    sph.close()
     start(cfg, ctx, st)
     attempts, mism, max_ds, differ = compare_trajectory(cfg, ctx, st, 0.9, 6)
     assert mism == 0 and max_ds == 0.0 and differ == 0
