@@ -110,6 +110,7 @@ struct hb_ctx {
   int csr_block = 128;
   int sc_kernel = 0;      // 0: direct loads through L1, 1: neighbour planes staged in shared memory
   int staged_zt = 16;
+  int sc_coop = -1;            // persistent multi-sweep kernel: -1 auto, 0 off, 1 / 2 forced (see hb_set_option)
   bool fused_measure = true;   // sc: the last sweep of hb_sweep also reduces M and E
   bool cache_valid = false;    // cached() holds the measurement of the current spins
   std::vector<uint32_t> colour_begin;     // CSR engine: offsets into the colour-sorted list
@@ -217,6 +218,30 @@ int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d, Meas m = Mea
 int fused_blocks(const hb_ctx* c) {
   if (!c->fused_measure || c->plan.engine != ENGINE_SC || c->sc_kernel != 0) return 0;
   return sc_fused_blocks(c->sc, c->tile);
+}
+
+// persistent path of hb_sweep: 1 = one block (auto for lattices whose colour pass fits 1024 threads), 2 = cooperative
+// grid (only when forced with sc_coop = 1 or 2: measured slower than one launch per colour at every size), 0 = none
+int coop_mode(const hb_ctx* c) {
+  if (c->plan.engine != ENGINE_SC || c->sc_kernel != 0 || !c->fused_measure || c->sc_coop == 0) return 0;
+  if (c->sc_coop != 2 && sc_one_block_threads(c->sc) > 0) return 1;
+  return (c->sc_coop >= 1 && sc_coop_blocks(c->sc, c->tile) > 0) ? 2 : 0;
+}
+
+// n sweeps in cooperative launches; series (device, 4 doubles per sweep) or final_out (device, 4 doubles) or neither
+int coop_sweeps(hb_ctx* c, float beta, int64_t n_sweeps, double* series, double* final_out) {
+  const SweepParams p = params(c, beta);
+  const int64_t chunk = int64_t(1) << 20;
+  for (int64_t s0 = 0; s0 < n_sweeps; s0 += chunk) {
+    const int m = (int)(n_sweeps - s0 < chunk ? n_sweeps - s0 : chunk);
+    const bool last = s0 + m == n_sweeps;
+    HB_CUDA(c, launch_sweeps_sc_coop(c->stream, c->spins, c->sc, c->tile, p, c->sweep, m, coop_mode(c) == 1, c->partials(),
+                                     series ? series + 4 * s0 : nullptr, last ? final_out : nullptr));
+    c->launches += 1;
+    c->sweep += (uint64_t)m;
+    c->attempts += (uint64_t)m * (uint64_t)c->plan.n;
+  }
+  return HB_OK;
 }
 
 // one sweep; with dev_out != nullptr (and fused_blocks() > 0) the colour passes also reduce M and E of
@@ -546,6 +571,11 @@ int hb_sweep(hb_ctx* c, float T, int64_t n_sweeps) {
   int rc = check_T(c, T, &beta);
   if (rc != HB_OK) return rc;
   if (n_sweeps > 0) c->cache_valid = false;
+  if (n_sweeps > 0 && coop_mode(c) != 0) {
+    rc = coop_sweeps(c, beta, n_sweeps, nullptr, c->cached());
+    if (rc == HB_OK) c->cache_valid = true;
+    return rc;
+  }
   const bool fuse = fused_blocks(c) > 0;
   for (int64_t s = 0; s < n_sweeps; ++s) {
     rc = one_sweep(c, beta, Diag{nullptr, nullptr}, (fuse && s == n_sweeps - 1) ? c->cached() : nullptr);
@@ -586,6 +616,10 @@ int hb_sweep_series(hb_ctx* c, float T, int64_t n_sweeps, double* M_series, doub
   if (n_sweeps > 0) c->cache_valid = false;
   for (int64_t s0 = 0; s0 < n_sweeps; s0 += kSeriesChunk) {
     const int64_t m = n_sweeps - s0 < kSeriesChunk ? n_sweeps - s0 : kSeriesChunk;
+    if (coop_mode(c) != 0) {
+      rc = coop_sweeps(c, beta, m, c->series(), nullptr);
+      if (rc != HB_OK) return rc;
+    } else
     for (int64_t s = 0; s < m; ++s) {
       rc = one_sweep(c, beta, Diag{nullptr, nullptr}, fuse ? c->series() + 4 * s : nullptr);
       if (rc != HB_OK) return rc;
@@ -662,6 +696,12 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
   HB_CHECK_CTX(c);
   if (!name) return HB_EINVAL;
   const std::string s(name);
+  if (s == "sc_coop") {
+    if (value < -1 || value > 2)
+      return fail(c, HB_EINVAL, "sc_coop: -1 auto (one block when it fits), 0 off, 1 one block else cooperative grid, 2 cooperative grid");
+    c->sc_coop = (int)value;
+    return HB_OK;
+  }
   if (s == "fused_measure") {
     if (value != 0 && value != 1) return fail(c, HB_EINVAL, "fused_measure: 0 or 1");
     c->fused_measure = value != 0;
@@ -715,6 +755,8 @@ int hb_get_option(hb_ctx* c, const char* name, int64_t* value) {
   const std::string s(name);
   if (s == "csr_block") *value = c->csr_block;
   else if (s == "fused_measure") *value = c->fused_measure ? 1 : 0;
+  else if (s == "sc_coop") *value = c->sc_coop;
+  else if (s == "coop_active") *value = coop_mode(c) != 0 ? 1 : 0;
   else if (s == "sc_v") *value = c->tile.V;
   else if (s == "sc_jx") *value = c->tile.JX;
   else if (s == "sc_ty") *value = c->tile.TY;

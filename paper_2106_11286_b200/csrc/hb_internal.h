@@ -28,7 +28,7 @@ struct ScLayout {
 struct ScTile {
   int32_t V, JX, TY, ZT;
   int32_t PF;   // software prefetch of the next z-plane: 0 none, 1 L2, 2 L1, 3 touch
-  int32_t LIN;  // 0: JX x TY tile; else threads per block of the linear (y, j) mapping (full warps)
+  int32_t LIN;  // 0: JX x TY tile; > 0: threads per block of the linear (y, j) mapping (full warps); < 0: one block, (z, y, j)
 };
 
 // periodic Bravais lattice with a basis (bcc: 2 sublattices, fcc: 4), canonical storage:
@@ -86,6 +86,13 @@ cudaError_t launch_sc_permute(cudaStream_t st, float* dst, const float* src, ScL
 cudaError_t launch_sweep_sc(cudaStream_t st, float* spins, ScLayout L, ScTile t, SweepParams p, int colour, Diag d, Meas m);
 // blocks one launch_sweep_sc launch uses with this tile if it can carry the fused measurement, else 0
 int sc_fused_blocks(const ScLayout& L, const ScTile& t);
+// persistent multi-sweep paths of the sc engine: ONE block when a colour pass fits 1024 threads (N <= 8192), or a
+// cooperative grid with a grid-wide barrier per colour.  sc_coop_blocks: virtual blocks of a pass, 0 = unavailable.
+// partials must hold 2 x 2 x blocks x 4 doubles; series (4 doubles per sweep) or final_out (4 doubles) may be null
+int sc_one_block_threads(const ScLayout& L);
+int sc_coop_blocks(const ScLayout& L, const ScTile& t);
+cudaError_t launch_sweeps_sc_coop(cudaStream_t st, float* spins, ScLayout L, ScTile t, SweepParams p, uint64_t sweep0, int n_sweeps,
+                                  bool one_block, double* partials, double* series, double* final_out);
 bool sc_staged_supported(const ScLayout& L);
 cudaError_t launch_sweep_sc_staged(cudaStream_t st, float* spins, ScLayout L, int ZT, SweepParams p, int colour, Diag d);
 cudaError_t launch_sweep_csr(cudaStream_t st, float* spins, CsrDev g, uint32_t list_begin, uint32_t list_count,

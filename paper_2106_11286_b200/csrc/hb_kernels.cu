@@ -8,6 +8,8 @@
 //
 // No tensor cores: the path is not a contraction.  HBM traffic per attempted update is
 // the roofline quantity (36 B for two colours); see DESIGN.md section 7.
+#include <cooperative_groups.h>
+
 #include "hb_device.cuh"
 #include "hb_internal.h"
 
@@ -79,15 +81,15 @@ __device__ __forceinline__ void prefetch_line(const float* p) {
 }
 
 // Neighbour field from 32-bit element offsets into one component plane of the other colour.
-template <int V>
-__device__ __forceinline__ Vec<V> sc_field_off(const float* __restrict__ b, uint32_t oc, uint32_t oh, uint32_t oym,
+template <int V, bool CO = false>
+__device__ __forceinline__ Vec<V> sc_field_off(const float* b, uint32_t oc, uint32_t oh, uint32_t oym,
                                                uint32_t oyp, uint32_t ozm, uint32_t ozp, int32_t p) {
-  const Vec<V> c = load_ro<V>(b + oc);
-  const float halo = __ldg(b + oh);
-  const Vec<V> ym = load_ro<V>(b + oym);
-  const Vec<V> yp = load_ro<V>(b + oyp);
-  const Vec<V> zm = load_ro<V>(b + ozm);
-  const Vec<V> zp = load_ro<V>(b + ozp);
+  const Vec<V> c = CO ? load_co<V>(b + oc) : load_ro<V>(b + oc);
+  const float halo = CO ? __ldca(b + oh) : __ldg(b + oh);
+  const Vec<V> ym = CO ? load_co<V>(b + oym) : load_ro<V>(b + oym);
+  const Vec<V> yp = CO ? load_co<V>(b + oyp) : load_ro<V>(b + oyp);
+  const Vec<V> zm = CO ? load_co<V>(b + ozm) : load_ro<V>(b + ozm);
+  const Vec<V> zp = CO ? load_co<V>(b + ozp) : load_ro<V>(b + ozp);
   Vec<V> h;
   if (V >= 2) {           // packed fp32x2 adds: same rounding per element, half the instructions
 #pragma unroll
@@ -116,33 +118,41 @@ __device__ __forceinline__ Vec<V> sc_field_off(const float* __restrict__ b, uint
 // note on fusing a5 into a4): every colour adds its own final spins to M and its anisotropy energy;
 // the LAST colour (m.mode == 2) sees only final neighbours, and since every bond of a 2-colour lattice
 // has exactly one end in it, -J sum_{i in last colour} S_i.h_i is the whole exchange energy.
-template <int V, int ANISO, bool DIAG, int PF, int BLK = 256, bool MEAS = false>
-__global__ void __launch_bounds__(BLK, (MEAS ? 3 : HB_SC_MINBLOCKS) * 256 / BLK)   // MEAS needs ~80 registers
-k_sweep_sc(float* __restrict__ ax, float* __restrict__ ay, float* __restrict__ az,
-           const float* __restrict__ bx, const float* __restrict__ by, const float* __restrict__ bz,
-           ScLayout L, ScTile t, SweepParams P, int colour, Diag d, Meas m) {
-  int32_t j, y;
-  if (t.LIN) {
+// The pass of one block (bid of nblk): the body of k_sweep_sc, and of the persistent multi-sweep kernel below,
+// which walks virtual blocks and needs coherent loads (CO) because other blocks of the same launch wrote b.
+template <int V, int ANISO, bool DIAG, int PF, bool MEAS, bool CO>
+__device__ __forceinline__ void sc_pass(float* ax, float* ay, float* az, const float* bx, const float* by, const float* bz,
+                                        const ScLayout& L, const ScTile& t, const SweepParams& P, int colour, const Diag& d,
+                                        const Meas& m, const uint3 bid, const uint3 nblk) {
+  int32_t j, y, zl = -1;
+  if (t.LIN < 0) {
+    // whole colour pass in ONE block (tiny lattices): thread = one (z, y, x-vector) slot
+    const int32_t HV = L.H / V;
+    const uint32_t s = threadIdx.x;
+    j = (int32_t)(s % (uint32_t)HV);
+    y = (int32_t)((s / (uint32_t)HV) % (uint32_t)L.Ly);
+    zl = (int32_t)(s / (uint32_t)(HV * L.Ly));
+  } else if (t.LIN) {
     // linear mapping: the block owns blockDim.x consecutive (y, j) slots, so every warp is full
     // even when a row does not hold a multiple of 32 vectors (L = 464: 116 vectors per row)
     const int32_t HV = L.H / V;
-    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t s = bid.x * blockDim.x + threadIdx.x;
     y = (int32_t)(s / (uint32_t)HV);
     j = (int32_t)(s - (uint32_t)y * (uint32_t)HV);
   } else {
     const int32_t tj = threadIdx.x % t.JX, ty = threadIdx.x / t.JX;
-    j = blockIdx.x * t.JX + tj;
-    y = blockIdx.y * t.TY + ty;
+    j = (int32_t)bid.x * t.JX + tj;
+    y = (int32_t)bid.y * t.TY + ty;
   }
   const int32_t i0 = j * V;
-  const bool outside = i0 >= L.H || y >= L.Ly;
+  const bool outside = i0 >= L.H || y >= L.Ly || zl >= L.Lz;
   if (!MEAS && outside) return;
   const uint32_t H = (uint32_t)L.H, plane = (uint32_t)L.Ly * H;
   const uint32_t ym = (uint32_t)((y == 0) ? L.Ly - 1 : y - 1) * H + (uint32_t)i0;
   const uint32_t yp = (uint32_t)((y == L.Ly - 1) ? 0 : y + 1) * H + (uint32_t)i0;
   const uint32_t yc = (uint32_t)y * H + (uint32_t)i0;
-  const int32_t z0 = blockIdx.z * t.ZT;
-  const int32_t z1 = (MEAS && outside) ? z0 : min(z0 + t.ZT, L.Lz);   // MEAS: every thread reaches the block reduction
+  const int32_t z0 = zl >= 0 ? zl : (int32_t)bid.z * t.ZT;
+  const int32_t z1 = (MEAS && outside) ? z0 : (zl >= 0 ? zl + 1 : min(z0 + t.ZT, L.Lz));   // MEAS: every thread reaches the block reduction
   unsigned n_acc = 0;
   double acc_mx = 0.0, acc_my = 0.0, acc_mz = 0.0, acc_en = 0.0;
   for (int32_t z = z0; z < z1; ++z) {
@@ -154,9 +164,9 @@ k_sweep_sc(float* __restrict__ ax, float* __restrict__ ay, float* __restrict__ a
     ih = (i0 + ih < 0) ? ih + L.H : ((i0 + ih >= L.H) ? ih - L.H : ih);
     const uint32_t oc = pz + yc, oh = oc + (uint32_t)ih, oym = pz + ym, oyp = pz + yp, ozm = pzm + yc, ozp = pzp + yc;
     Vec<V> sx = load_rw<V>(ax + oc), sy = load_rw<V>(ay + oc), sz = load_rw<V>(az + oc);
-    const Vec<V> hx = sc_field_off<V>(bx, oc, oh, oym, oyp, ozm, ozp, p);
-    const Vec<V> hy = sc_field_off<V>(by, oc, oh, oym, oyp, ozm, ozp, p);
-    const Vec<V> hz = sc_field_off<V>(bz, oc, oh, oym, oyp, ozm, ozp, p);
+    const Vec<V> hx = sc_field_off<V, CO>(bx, oc, oh, oym, oyp, ozm, ozp, p);
+    const Vec<V> hy = sc_field_off<V, CO>(by, oc, oh, oym, oyp, ozm, ozp, p);
+    const Vec<V> hz = sc_field_off<V, CO>(bz, oc, oh, oym, oyp, ozm, ozp, p);
     if (PF != 0 && z + 1 < z1) {
       const uint32_t zpp = (uint32_t)((z + 2 >= L.Lz) ? z + 2 - L.Lz : z + 2) * plane + yc;
       prefetch_line<PF>(ax + pzp + yc); prefetch_line<PF>(ay + pzp + yc); prefetch_line<PF>(az + pzp + yc);
@@ -211,9 +221,17 @@ k_sweep_sc(float* __restrict__ ax, float* __restrict__ ay, float* __restrict__ a
   }
   if (DIAG && d.n_accept && n_acc) atomicAdd(d.n_accept, (unsigned long long)n_acc);
   if (MEAS) {
-    const uint32_t blk = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+    const uint32_t blk = (bid.z * nblk.y + bid.y) * nblk.x + bid.x;
     block_reduce4(acc_mx, acc_my, acc_mz, acc_en, m.partials + (size_t)blk * 4);
   }
+}
+
+template <int V, int ANISO, bool DIAG, int PF, int BLK = 256, bool MEAS = false>
+__global__ void __launch_bounds__(BLK, (MEAS ? 3 : HB_SC_MINBLOCKS) * 256 / BLK)   // MEAS needs ~80 registers
+k_sweep_sc(float* __restrict__ ax, float* __restrict__ ay, float* __restrict__ az,
+           const float* __restrict__ bx, const float* __restrict__ by, const float* __restrict__ bz,
+           ScLayout L, ScTile t, SweepParams P, int colour, Diag d, Meas m) {
+  sc_pass<V, ANISO, DIAG, PF, MEAS, false>(ax, ay, az, bx, by, bz, L, t, P, colour, d, m, blockIdx, gridDim);
 }
 
 // ---- simple cubic, neighbour planes staged in shared memory by bulk async copies (TMA 1-D) --------
@@ -439,13 +457,21 @@ __global__ void k_sc_permute(float* dst, const float* src, ScLayout L, bool to_i
 }
 
 // ---- measurement --------------------------------------------------------------------------------
-// fixed-order final sum of the block partials: one block of 256 threads
-__global__ void k_reduce_final(const double* partials, int n_blocks, double* out) {
+// fixed-order final sum of the block partials by one block (fixed for a given block size)
+__device__ __forceinline__ void reduce_final_block(const double* partials, int n_blocks, double* out) {
+  // any block size: threads beyond 256 stay out, missing ones leave zeros
   double a[4] = {0, 0, 0, 0};
-  for (int b = threadIdx.x; b < n_blocks; b += blockDim.x)
-    for (int q = 0; q < 4; ++q) a[q] += partials[b * 4 + q];
+  const int nt = blockDim.x < 256 ? blockDim.x : 256;
+  if ((int)threadIdx.x < nt)
+    for (int b = threadIdx.x; b < n_blocks; b += nt)
+      for (int q = 0; q < 4; ++q) a[q] += partials[b * 4 + q];
   __shared__ double sh[4][256];
-  for (int q = 0; q < 4; ++q) sh[q][threadIdx.x] = a[q];
+  __syncthreads();
+  for (int k = threadIdx.x; k < 256; k += blockDim.x)
+    for (int q = 0; q < 4; ++q) sh[q][k] = 0.0;
+  __syncthreads();
+  if ((int)threadIdx.x < nt)
+    for (int q = 0; q < 4; ++q) sh[q][threadIdx.x] = a[q];
   __syncthreads();
   for (int s = 128; s > 0; s >>= 1) {
     if ((int)threadIdx.x < s)
@@ -453,6 +479,53 @@ __global__ void k_reduce_final(const double* partials, int n_blocks, double* out
     __syncthreads();
   }
   if (threadIdx.x < 4) out[threadIdx.x] = sh[threadIdx.x][0];
+}
+
+__global__ void __launch_bounds__(256) k_reduce_final(const double* partials, int n_blocks, double* out) {
+  reduce_final_block(partials, n_blocks, out);
+}
+
+// ---- persistent multi-sweep kernel for lattices whose colour pass is shorter than a kernel launch ----------
+// One cooperative launch runs n_sweeps sweeps: every block walks the virtual blocks of a colour pass, then the
+// whole grid meets at a barrier (cooperative groups) before the next colour.  Same arithmetic, same tiles, same
+// bits as the one-launch-per-colour path; what it removes is the launch gap (5-6 us per colour on B200, against
+// 1-2 us of work for L <= 128).  Measurement (fused, section 6.5): with series != nullptr EVERY sweep is measured
+// and (sum S, E) of sweep s goes to series[4 s ..]; else with final_out != nullptr only the last sweep is.
+// Block 0 sums the block partials of sweep s while the grid already runs colour 0 of sweep s+1, so the partials
+// are double-buffered by sweep parity (2 x 2 x total x 4 doubles).
+// ONE: the whole colour pass fits one block of up to 1024 threads (N <= 8192): a single block on a single SM, the
+// barrier is __syncthreads and the 12 N bytes of state stay in that SM's L1.
+template <int ANISO, bool ONE>
+__global__ void __launch_bounds__(ONE ? 1024 : 256, ONE ? 1 : 3)
+k_sweeps_sc_coop(float* s, ScLayout L, ScTile t, SweepParams P, unsigned long long sweep0, int n_sweeps, uint3 nblk,
+                 double* partials, double* series, double* final_out) {
+  cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+  const size_t n = L.n;
+  const uint32_t total = nblk.x * nblk.y * nblk.z;
+  const Diag d{nullptr, nullptr};
+  if (ONE) t.LIN = -1;
+  for (int sw = 0; sw < n_sweeps; ++sw) {
+    const unsigned long long sc = sweep0 + (unsigned long long)sw;
+    P.sweep_lo = (uint32_t)sc; P.sweep_hi = (uint32_t)(sc >> 32);
+    const bool meas = series != nullptr || (final_out != nullptr && sw == n_sweeps - 1);
+    double* part = partials + (size_t)(sw & 1) * 2 * total * 4;
+    for (int colour = 0; colour < 2; ++colour) {
+      float* a = s + (size_t)colour * L.half;
+      const float* b = s + (size_t)(1 - colour) * L.half;
+      for (uint32_t v = blockIdx.x; v < total; v += gridDim.x) {
+        const uint3 bid = make_uint3(v % nblk.x, (v / nblk.x) % nblk.y, v / (nblk.x * nblk.y));
+        if (meas) {
+          const Meas mc{part + (size_t)colour * total * 4, colour == 1 ? 2 : 1};
+          sc_pass<4, ANISO, false, 0, true, true>(a, a + n, a + 2 * n, b, b + n, b + 2 * n, L, t, P, colour, d, mc, bid, nblk);
+        } else {
+          sc_pass<4, ANISO, false, 0, false, true>(a, a + n, a + 2 * n, b, b + n, b + 2 * n, L, t, P, colour, d, Meas{nullptr, 0}, bid, nblk);
+        }
+      }
+      if (ONE) __syncthreads(); else grid.sync();
+    }
+    if (meas && blockIdx.x == 0)
+      reduce_final_block(part, 2 * (int)total, series ? series + 4 * (size_t)sw : final_out);
+  }
 }
 
 template <int V>
@@ -612,6 +685,59 @@ cudaError_t launch_sweep_sc(cudaStream_t st, float* s, ScLayout L, ScTile t, Swe
     case 2: return diag ? sweep_sc_aniso<2, true>(st, s, L, t, p, colour, d, m) : sweep_sc_aniso<2, false>(st, s, L, t, p, colour, d, m);
     default: return diag ? sweep_sc_aniso<1, true>(st, s, L, t, p, colour, d, m) : sweep_sc_aniso<1, false>(st, s, L, t, p, colour, d, m);
   }
+}
+
+// threads of the one-block path if a whole colour pass fits one block (V = 4, N/8 <= 1024 threads), else 0
+int sc_one_block_threads(const ScLayout& L) {
+  if (L.H % 4 != 0) return 0;
+  const long long slots = (long long)(L.H / 4) * L.Ly * L.Lz;
+  return slots <= 1024 ? (int)((slots + 31) / 32 * 32) : 0;
+}
+
+// persistent cooperative path: virtual blocks of a colour pass (0 = not available for this tile)
+int sc_coop_blocks(const ScLayout& L, const ScTile& t) {
+  if (t.V != 4 || (t.LIN ? t.LIN : t.JX * t.TY) > 256) return 0;
+  dim3 grid; int threads;
+  sc_launch_shape(L, t, 4, grid, threads);
+  const long long blocks = (long long)grid.x * grid.y * grid.z;
+  return blocks <= kFusedBlocksMax / 2 ? (int)blocks : 0;
+}
+
+cudaError_t launch_sweeps_sc_coop(cudaStream_t st, float* s, ScLayout L, ScTile t, SweepParams p, uint64_t sweep0, int n_sweeps,
+                                  bool one_block, double* partials, double* series, double* final_out) {
+  const int aniso = aniso_case(p);
+  if (one_block) {
+    const int threads = sc_one_block_threads(L);
+    if (!threads) return cudaErrorInvalidValue;
+    const uint3 nblk = make_uint3(1, 1, 1);
+    switch (aniso) {
+      case ANISO_NONE: k_sweeps_sc_coop<ANISO_NONE, true><<<1, threads, 0, st>>>(s, L, t, p, sweep0, n_sweeps, nblk, partials, series, final_out); break;
+      case ANISO_Z: k_sweeps_sc_coop<ANISO_Z, true><<<1, threads, 0, st>>>(s, L, t, p, sweep0, n_sweeps, nblk, partials, series, final_out); break;
+      default: k_sweeps_sc_coop<ANISO_GENERAL, true><<<1, threads, 0, st>>>(s, L, t, p, sweep0, n_sweeps, nblk, partials, series, final_out); break;
+    }
+    return cudaGetLastError();
+  }
+  dim3 vgrid; int threads;
+  sc_launch_shape(L, t, 4, vgrid, threads);
+  void (*kern)(float*, ScLayout, ScTile, SweepParams, unsigned long long, int, uint3, double*, double*, double*);
+  switch (aniso) {
+    case ANISO_NONE: kern = k_sweeps_sc_coop<ANISO_NONE, false>; break;
+    case ANISO_Z: kern = k_sweeps_sc_coop<ANISO_Z, false>; break;
+    default: kern = k_sweeps_sc_coop<ANISO_GENERAL, false>; break;
+  }
+  int dev = 0, sms = 0, per_sm = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, 0);
+  if (e != cudaSuccess) return e;
+  if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+  const long long total = (long long)vgrid.x * vgrid.y * vgrid.z;
+  const long long resident = (long long)per_sm * sms;
+  const unsigned grid = (unsigned)(total < resident ? total : resident);
+  uint3 nblk = make_uint3(vgrid.x, vgrid.y, vgrid.z);
+  unsigned long long s0 = sweep0;
+  void* args[] = {&s, &L, &t, &p, &s0, &n_sweeps, &nblk, &partials, &series, &final_out};
+  return cudaLaunchCooperativeKernel((const void*)kern, dim3(grid), dim3(threads), args, 0, st);
 }
 
 template <int TY, int ROWB, int ANISO, bool DIAG>

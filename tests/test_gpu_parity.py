@@ -70,10 +70,18 @@ def test_small_trajectories_bit_exact(name):
         assert attempts == 5 * lat.n and mism == 0 and max_ds == 0.0 and differ == 0
         _measure_close(ctx, st, lat.n)
     assert ctx.sweep_count == st.sweep_count == 10
-    # the production kernels (no recording) walk the same trajectory
-    ctx.sweep(1.0, 7)
+    # the production kernels (no recording) walk the same trajectory: one launch per colour, and for the sc
+    # engine the persistent cooperative multi-sweep kernel that small lattices use by default
+    sc_engine = cfg["kind"] == "sc" and cfg.get("K_site") is None
+    if sc_engine:
+        ctx.set_option("sc_coop", 0)
+    ctx.sweep(1.0, 3)
+    if sc_engine:
+        ctx.set_option("sc_coop", 1)
+    ctx.sweep(1.0, 4)
     st.sweep(1.0, 7)
     assert spins_equal(ctx.get_spins(), st.get_spins())
+    _measure_close(ctx, st, lat.n)
     ctx.close()
 
 
@@ -83,15 +91,18 @@ def test_sc_tile_shapes_do_not_change_the_result():
     st.init_random()
     st.sweep(1.44, 3)
     want = st.get_spins()
-    for v, jx, ty, zt in [(4, 5, 12, 10), (4, 3, 5, 3), (4, 1, 1, 1), (2, 10, 7, 4), (1, 20, 12, 2), (4, 5, 51, 10)]:
+    for v, jx, ty, zt, coop in [(4, 5, 12, 10, 0), (4, 3, 5, 3, 0), (4, 1, 1, 1, 0), (2, 10, 7, 4, 0), (1, 20, 12, 2, 0),
+                                (4, 5, 51, 10, 0), (4, 5, 12, 10, 2), (4, 3, 5, 3, 2), (4, 2, 7, 4, 2), (4, 5, 51, 10, 2),
+                                (4, 5, 12, 10, 1)]:
         ctx = make_gpu(cfg)
+        ctx.set_option("sc_coop", coop)
         ctx.set_option("sc_v", v)
         ctx.set_option("sc_jx", jx)
         ctx.set_option("sc_ty", ty)
         ctx.set_option("sc_zt", zt)
         ctx.init_random()
         ctx.sweep(1.44, 3)
-        assert spins_equal(ctx.get_spins(), want), (v, jx, ty, zt)
+        assert spins_equal(ctx.get_spins(), want), (v, jx, ty, zt, coop)
         ctx.close()
 
 
@@ -160,7 +171,15 @@ def test_c1_full_series():
     nrm = sum(x.astype(np.float64) ** 2 for x in ctx.get_spins())
     assert np.max(np.abs(nrm - 1.0)) <= 5e-7                            # K3
     launches, attempts = ctx.counters()
-    assert attempts == 1000 * lat.n and launches >= 2000
+    assert attempts == 1000 * lat.n and launches >= 1
+    # the same series from one launch per colour (the persistent kernel off)
+    ctx2 = make_gpu(cfg)
+    ctx2.set_option("sc_coop", 0)
+    ctx2.init_random()
+    M2, E2 = ctx2.sweep_series(1.2, 1000)
+    assert spins_equal(ctx2.get_spins(), st.get_spins())
+    assert np.max(np.abs(M2 - Mo)) <= 1e-7 and np.max(np.abs(E2 - Eo)) <= 1e-6 * lat.n
+    assert ctx2.counters()[0] >= 2000
 
 
 def test_limits_on_device():
@@ -273,6 +292,7 @@ def test_fused_measurement_equals_the_separate_pass():
         lat, st = make_oracle(cfg)
         fused, plain = make_gpu(cfg), make_gpu(cfg)
         plain.set_option("fused_measure", 0)
+        fused.set_option("sc_coop", 0)                                # this test is about the per-colour launches
         for k, v in opts.items():
             fused.set_option(k, v)
         start(cfg, fused, st)
@@ -295,3 +315,36 @@ def test_fused_measurement_equals_the_separate_pass():
         fused.set_spins(S[:, 0], S[:, 1], S[:, 2])
         st.set_spins(S[:, 0], S[:, 1], S[:, 2])
         _measure_close(fused, st, lat.n)
+
+
+def test_persistent_kernels_match_the_oracle():
+    # hb_sweep on a small sc lattice runs all its sweeps in ONE launch: a single block when a colour pass fits 1024
+    # threads (the default for N <= 8192, barrier = __syncthreads), or, when forced, a cooperative grid with a
+    # grid-wide barrier between colours.  The measurement of the last sweep (or of every sweep, for the series) is
+    # reduced inside the launch.
+    cases = [(W.SMALL["c1"], -1, 1), (dict(W.SMALL["c4"], L=(8, 6, 4), K=0.3, e=(0.6, 0.0, 0.8)), -1, 1),
+             (dict(W.SMALL["c4"], L=(16, 16, 32)), -1, 1), (W.SMALL["c4"], 1, 1), (W.SMALL["c1"], 2, 1),
+             (dict(W.SMALL["c4"], L=(40, 12, 10), K=0.3, e=(0.6, 0.0, 0.8)), 2, 1), (dict(W.SMALL["c4"], L=64), 1, 1),
+             (W.SMALL["c4"], -1, 0)]
+    for cfg, coop, active in cases:
+        lat, st = make_oracle(cfg)
+        ctx = make_gpu(cfg)
+        ctx.set_option("sc_coop", coop)
+        assert ctx.get_option("coop_active") == active, (cfg["L"], coop)
+        if not active:
+            continue
+        start(cfg, ctx, st)
+        for T, k in ((1.44, 1), (1.44, 6), (0.5, 3)):
+            l0, _ = ctx.counters()
+            ctx.sweep(T, k)
+            l1, _ = ctx.counters()
+            assert l1 - l0 == 1                                       # one launch, whatever k
+            st.sweep(T, k)
+            _measure_close(ctx, st, lat.n)                            # the fused measurement of the last sweep
+        assert spins_equal(ctx.get_spins(), st.get_spins())
+        Mg, Eg = ctx.sweep_series(1.2, 37)
+        Mo, Eo = st.series(1.2, 37)
+        assert spins_equal(ctx.get_spins(), st.get_spins())
+        assert np.max(np.abs(Mg - Mo)) <= 1e-7 and np.max(np.abs(Eg - Eo)) <= 1e-6 * lat.n
+        assert ctx.sweep_count == st.sweep_count
+        ctx.close()
