@@ -227,6 +227,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c4", help="c1..c5 (BASELINE.json configs); the headline is c4")
+    ap.add_argument("--option", action="append", default=[], metavar="NAME=VALUE",
+                    help="hb_set_option on the context (tuning knobs of DESIGN.md section 6), repeatable")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -257,6 +259,11 @@ def main():
         torch.cuda.synchronize()
 
     ctx = make_context(cfg, rank, device)
+    options = {}
+    for kv in args.option:
+        k, v = kv.split("=", 1)
+        ctx.set_option(k, int(v))
+        options[k] = int(v)
     T = cfg["T"][0]
     n = ctx.n
     _, n_colours = ctx.colouring()
@@ -345,7 +352,7 @@ def main():
         "config": {"workload": args.workload,
                    "lattice": "%s %s" % (cfg["kind"], cfg.get("L", cfg.get("R"))), "n_spins": n, "colours": n_colours,
                    "J": cfg["J"], "K": cfg["K"], "T": T, "start": cfg["start"], "seed": cfg["seed"],
-                   "sweeps_per_step": SWEEPS_PER_STEP, "measurements_per_step": 1,
+                   "sweeps_per_step": SWEEPS_PER_STEP, "measurements_per_step": 1, "options": options,
                    "l2": "state %.0f MB >> 126 MB L2: no flush between iterations" % (12.0 * n / 1e6)
                    if 12.0 * n > 4 * 126e6 else "state fits in L2: HBM roofline not meaningful",
                    "multi_gpu": "replicas only (seed + rank)"},

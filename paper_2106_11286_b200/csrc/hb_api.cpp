@@ -108,8 +108,8 @@ struct hb_ctx {
   CsrDev csr{};
   EllDev ell{};
   int csr_block = 128;
-  int sc_kernel = 0;      // 0: direct loads through L1, 1: neighbour planes staged in shared memory
-  int staged_zt = 16;
+  int sc_kernel = 0;      // 0: direct loads through L1, 1: warp-specialised persistent kernel (TMA-staged neighbour planes)
+  int ws_zt = 32, n_sms = 148, ws_variant = 0;   // warp-specialised kernel: planes per tile, CTAs = n_sms x CTAs/SM
   int sc_coop = -1;            // persistent multi-sweep kernel: -1 auto, 0 off, 1 / 2 forced (see hb_set_option)
   bool fused_measure = true;   // sc: the last sweep of hb_sweep also reduces M and E
   bool cache_valid = false;    // cached() holds the measurement of the current spins
@@ -198,8 +198,9 @@ ScTile default_tile(int32_t H, int32_t Ly, int32_t Lz) {
 
 int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d, Meas m = Meas{nullptr, 0}) {
   if (c->plan.engine == ENGINE_SC) {
-    if (c->sc_kernel == 1)
-      HB_CUDA(c, launch_sweep_sc_staged(c->stream, c->spins, c->sc, c->staged_zt, p, colour, d));
+    const bool diag = d.accept || d.n_accept;
+    if (c->sc_kernel == 1 && !diag)
+      HB_CUDA(c, launch_sweep_sc_ws(c->stream, c->spins, c->sc, c->ws_zt, c->n_sms, c->ws_variant, p, colour, m));
     else
       HB_CUDA(c, launch_sweep_sc(c->stream, c->spins, c->sc, c->tile, p, colour, d, m));
   } else if (c->plan.engine == ENGINE_BRAVAIS) {
@@ -216,7 +217,8 @@ int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d, Meas m = Mea
 
 // blocks per colour launch if this context can fuse the measurement into its colour passes, else 0
 int fused_blocks(const hb_ctx* c) {
-  if (!c->fused_measure || c->plan.engine != ENGINE_SC || c->sc_kernel != 0) return 0;
+  if (!c->fused_measure || c->plan.engine != ENGINE_SC) return 0;
+  if (c->sc_kernel == 1) return sc_ws_blocks(c->sc, c->ws_zt, c->n_sms, c->ws_variant);
   return sc_fused_blocks(c->sc, c->tile);
 }
 
@@ -383,8 +385,14 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
     c->sc.Lx = lat->Lx; c->sc.Ly = lat->Ly; c->sc.Lz = lat->Lz;
     c->sc.H = lat->Lx / 2; c->sc.n = (uint32_t)P.n; c->sc.half = (uint32_t)(P.n / 2);
     c->tile = default_tile(c->sc.H, c->sc.Ly, c->sc.Lz);
-    c->sc_kernel = 0;   // measured on B200: direct + L2 prefetch 141 Gupd/s, staged 135
-    c->staged_zt = c->sc.Lz < 16 ? c->sc.Lz : 16;
+    {
+      int dev = 0, sms = 0;
+      if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+        c->n_sms = sms;
+      cudaGetLastError();
+    }
+    if (c->ws_zt > c->sc.Lz) c->ws_zt = c->sc.Lz;
+    c->sc_kernel = 0;   // measured on B200: both kernels sustain the same rate within noise
   }
 
   // ---- device memory --------------------------------------------------------------------------
@@ -714,18 +722,28 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
   }
   if (c->plan.engine == ENGINE_CSR) return fail(c, HB_EINVAL, "option not valid for this lattice");
   const bool is_sc = c->plan.engine == ENGINE_SC;
-  if (!is_sc && (s == "sc_kernel" || s == "sc_staged_zt" || s == "sc_prefetch" || s == "sc_linear"))
+  if (!is_sc && (s == "sc_kernel" || s == "sc_prefetch" || s == "sc_linear" || s == "sc_ws_zt" || s == "sc_ws_ctas" || s == "sc_ws_variant"))
     return fail(c, HB_EINVAL, "option valid for the simple cubic lattice only");
   const int32_t rowH = is_sc ? c->sc.H : c->br.Lx, rowLz = is_sc ? c->sc.Lz : c->br.Lz;
   if (s == "sc_kernel") {
-    if (value != 0 && !(value == 1 && sc_staged_supported(c->sc)))
-      return fail(c, HB_EINVAL, "sc_kernel: 0 (direct) or 1 (staged; needs Lx % 8 == 0 and Lx <= 512)");
+    if (value != 0 && !(value == 1 && sc_ws_supported(c->sc)))
+      return fail(c, HB_EINVAL, "sc_kernel: 0 (direct) or 1 (warp-specialised; needs Lx % 8 == 0 and Lx <= 512)");
     c->sc_kernel = (int)value;
     return HB_OK;
   }
-  if (s == "sc_staged_zt") {
-    if (value < 1 || value > c->sc.Lz) return fail(c, HB_EINVAL, "sc_staged_zt: 1..Lz");
-    c->staged_zt = (int)value;
+  if (s == "sc_ws_zt") {
+    if (value < 1 || value > c->sc.Lz) return fail(c, HB_EINVAL, "sc_ws_zt: 1..Lz");
+    c->ws_zt = (int)value;
+    return HB_OK;
+  }
+  if (s == "sc_ws_variant") {
+    if (value < 0 || value > 1) return fail(c, HB_EINVAL, "sc_ws_variant: 0 (4-row tiles, 2 CTAs per SM) or 1 (8-row tiles, 1 CTA per SM)");
+    c->ws_variant = (int)value;
+    return HB_OK;
+  }
+  if (s == "sc_ws_ctas") {
+    if (value < 1 || value > 4096) return fail(c, HB_EINVAL, "sc_ws_ctas: 1..4096");
+    c->n_sms = (int)value;
     return HB_OK;
   }
   ScTile t = c->tile;
@@ -766,7 +784,8 @@ int hb_get_option(hb_ctx* c, const char* name, int64_t* value) {
   else if (s == "engine") *value = c->plan.engine;
   else if (s == "ell") *value = c->plan.ell ? 1 : 0;
   else if (s == "sc_kernel") *value = c->sc_kernel;
-  else if (s == "sc_staged_zt") *value = c->staged_zt;
+  else if (s == "sc_ws_zt") *value = c->ws_zt;
+  else if (s == "sc_ws_ctas") *value = c->n_sms;
   else return HB_EINVAL;
   return HB_OK;
 }

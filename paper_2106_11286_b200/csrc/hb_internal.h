@@ -93,8 +93,10 @@ int sc_one_block_threads(const ScLayout& L);
 int sc_coop_blocks(const ScLayout& L, const ScTile& t);
 cudaError_t launch_sweeps_sc_coop(cudaStream_t st, float* spins, ScLayout L, ScTile t, SweepParams p, uint64_t sweep0, int n_sweeps,
                                   bool one_block, double* partials, double* series, double* final_out);
-bool sc_staged_supported(const ScLayout& L);
-cudaError_t launch_sweep_sc_staged(cudaStream_t st, float* spins, ScLayout L, int ZT, SweepParams p, int colour, Diag d);
+// warp-specialised persistent sc kernel (hb_sc_ws.cu): grid_cap = CTAs to launch at most (one per SM)
+bool sc_ws_supported(const ScLayout& L);
+int sc_ws_blocks(const ScLayout& L, int ZT, int grid_cap, int variant);
+cudaError_t launch_sweep_sc_ws(cudaStream_t st, float* spins, ScLayout L, int ZT, int grid_cap, int variant, SweepParams p, int colour, Meas m);
 cudaError_t launch_sweep_csr(cudaStream_t st, float* spins, CsrDev g, uint32_t list_begin, uint32_t list_count,
                              SweepParams p, int block, Diag d);
 cudaError_t launch_sweep_ell(cudaStream_t st, float* spins, EllDev g, uint32_t begin, uint32_t count, SweepParams p,

@@ -234,154 +234,6 @@ k_sweep_sc(float* __restrict__ ax, float* __restrict__ ay, float* __restrict__ a
   sc_pass<V, ANISO, DIAG, PF, MEAS, false>(ax, ay, az, bx, by, bz, L, t, P, colour, d, m, blockIdx, gridDim);
 }
 
-// ---- simple cubic, neighbour planes staged in shared memory by bulk async copies (TMA 1-D) --------
-// A block owns TY consecutive x-rows (all of x) and marches ZT planes in z.  Three plane slots of
-// the OTHER colour (z-1, z, z+1; rows y0-1 .. y0+TY) live in shared memory; while the block works on
-// plane z, lanes of warp 0 have already issued cp.async.bulk copies (one per row and component,
-// completion counted on an mbarrier) for plane z+2.  Every neighbour read is then an LDS with a
-// compile-time offset, the periodic wrap in x is an index inside the staged row, and no load of the
-// neighbour field ever waits on DRAM.  Own spins stay in registers (one LDG.128/STG.128 per component).
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "HB_WAIT:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra HB_DONE;\n"
-      "bra HB_WAIT;\n"
-      "HB_DONE:\n"
-      "}\n" ::"r"(bar), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
-}
-
-template <int TY, int ROWB, int ANISO, bool DIAG>
-__global__ void __launch_bounds__(ROWB / 16 * TY, (ROWB / 16 * TY) >= 256 ? 4 : 1)
-k_sweep_sc_staged(float* __restrict__ ax, float* __restrict__ ay, float* __restrict__ az,
-                  const float* __restrict__ bx, const float* __restrict__ by, const float* __restrict__ bz,
-                  ScLayout L, SweepParams P, int colour, int ZT, Diag d) {
-  constexpr int ROWS = TY + 2;
-  constexpr uint32_t COMP_B = ROWS * ROWB;       // one component of one plane slot
-  constexpr uint32_t SLOT_B = 3 * COMP_B;        // one plane slot
-  extern __shared__ __align__(128) unsigned char smem[];
-  const uint32_t sbase = smem_u32(smem), bar0 = sbase + 3 * SLOT_B;
-  const int HV = L.H >> 2;
-  const int tj = threadIdx.x % HV, ty = threadIdx.x / HV;
-  const int y0 = blockIdx.x * TY;
-  const int ny = min(TY, L.Ly - y0);
-  const int z0 = blockIdx.y * ZT;
-  const int nz = min(ZT, L.Lz - z0);
-  const uint32_t row_bytes = (uint32_t)L.H * 4u;
-  const uint32_t n_rows = 3u * (uint32_t)(ny + 2);
-  const bool issuer = threadIdx.x < 32;
-  const uint32_t n_issuers = blockDim.x < 32 ? blockDim.x : 32;
-
-  // plane k of the march = lattice plane z0-1+k (periodic), slot k % 3
-  auto issue_plane = [&](int k) {
-    int zz = z0 - 1 + k;
-    zz = zz < 0 ? zz + L.Lz : (zz >= L.Lz ? zz - L.Lz : zz);
-    const uint32_t slot = (uint32_t)k % 3u, bar = bar0 + 8u * slot;
-    if (threadIdx.x == 0) mbar_expect_tx(bar, n_rows * row_bytes);
-    __syncwarp();
-    for (uint32_t q = threadIdx.x; q < n_rows; q += n_issuers) {
-      const uint32_t comp = q / (uint32_t)(ny + 2), r = q - comp * (uint32_t)(ny + 2);
-      int yy = y0 - 1 + (int)r;
-      yy = yy < 0 ? yy + L.Ly : (yy >= L.Ly ? yy - L.Ly : yy);
-      const float* src = (comp == 0 ? bx : (comp == 1 ? by : bz)) + ((size_t)zz * L.Ly + yy) * L.H;
-      bulk_g2s(sbase + slot * SLOT_B + comp * COMP_B + r * ROWB, src, row_bytes, bar);
-    }
-  };
-
-  if (threadIdx.x == 0) {
-    mbar_init(bar0, 1); mbar_init(bar0 + 8, 1); mbar_init(bar0 + 16, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  __syncthreads();
-  if (issuer) { issue_plane(0); issue_plane(1); issue_plane(2); }
-
-  const bool active = ty < ny;
-  const int y = y0 + ty;
-  const int i0 = tj * 4;
-  // byte offset of this thread's float4 inside a component slab (row ty+1), and of its row start
-  const uint32_t t_row = (uint32_t)(ty + 1) * ROWB;
-  const uint32_t t_off = t_row + (uint32_t)tj * 16u;
-  uint32_t o_m = 0, o_c = SLOT_B, o_p = 2 * SLOT_B;
-  unsigned n_acc = 0;
-
-  for (int s = 0; s < nz; ++s) {
-    const int z = z0 + s;
-    const int p = (colour + y + z) & 1;
-    const uint32_t grow = (uint32_t)(z * L.Ly + y) * (uint32_t)L.H + (uint32_t)i0;   // element offset in the colour plane
-    Vec<4> sx, sy, sz;
-    if (active) { sx = load_rw<4>(ax + grow); sy = load_rw<4>(ay + grow); sz = load_rw<4>(az + grow); }
-    if (s == 0) { mbar_wait(bar0, 0); mbar_wait(bar0 + 8, 0); }
-    mbar_wait(bar0 + 8u * ((uint32_t)(s + 2) % 3u), ((uint32_t)(s + 2) / 3u) & 1u);
-
-    Vec<4> h[3];
-    if (active) {
-      int ih = p ? i0 + 4 : i0 - 1;
-      ih = ih < 0 ? ih + L.H : (ih >= L.H ? ih - L.H : ih);
-      const uint32_t a_halo = t_row + (uint32_t)ih * 4u + o_c;
-#pragma unroll
-      for (int c = 0; c < 3; ++c) {
-        const unsigned char* base = smem + c * COMP_B;
-        const float4 cc = *reinterpret_cast<const float4*>(base + o_c + t_off);
-        const float halo = *reinterpret_cast<const float*>(base + a_halo);
-        const float4 ym = *reinterpret_cast<const float4*>(base + o_c + t_off - ROWB);
-        const float4 yp = *reinterpret_cast<const float4*>(base + o_c + t_off + ROWB);
-        const float4 zm = *reinterpret_cast<const float4*>(base + o_m + t_off);
-        const float4 zp = *reinterpret_cast<const float4*>(base + o_p + t_off);
-        const f2 sel_lo = make_float2(p ? cc.y : halo, p ? cc.z : cc.x);
-        const f2 sel_hi = make_float2(p ? cc.w : cc.y, p ? halo : cc.z);
-        f2 a = add2(make_float2(cc.x, cc.y), sel_lo), b = add2(make_float2(cc.z, cc.w), sel_hi);
-        a = add2(a, make_float2(ym.x, ym.y)); b = add2(b, make_float2(ym.z, ym.w));
-        a = add2(a, make_float2(yp.x, yp.y)); b = add2(b, make_float2(yp.z, yp.w));
-        a = add2(a, make_float2(zm.x, zm.y)); b = add2(b, make_float2(zm.z, zm.w));
-        a = add2(a, make_float2(zp.x, zp.y)); b = add2(b, make_float2(zp.z, zp.w));
-        h[c].v[0] = a.x; h[c].v[1] = a.y; h[c].v[2] = b.x; h[c].v[3] = b.y;
-      }
-    }
-    __syncthreads();                                   // slot o_m has been read by everyone
-    if (issuer && s + 1 < nz) issue_plane(s + 3);      // refill it with the plane needed next step
-
-    if (active) {
-      const uint32_t site0 = (uint32_t)(z * L.Ly + y) * (uint32_t)L.Lx + 2u * (uint32_t)i0 + (uint32_t)p;
-      bool any = false;
-#pragma unroll
-      for (int k = 0; k < 4; k += 2) {
-        const Rand4 ra = philox4x32_10(site0 + 2u * k, 0u, P.sweep_lo, P.sweep_hi, P.seed_lo, P.seed_hi);
-        const Rand4 rb = philox4x32_10(site0 + 2u * k + 2u, 0u, P.sweep_lo, P.sweep_hi, P.seed_lo, P.seed_hi);
-        f2 px = make_float2(sx.v[k], sx.v[k + 1]), py = make_float2(sy.v[k], sy.v[k + 1]), pz = make_float2(sz.v[k], sz.v[k + 1]);
-        bool acc_a, acc_b;
-        attempt2<ANISO>(ra, rb, P.J, P.K, P.beta, P.ex, P.ey, P.ez, make_float2(h[0].v[k], h[0].v[k + 1]),
-                        make_float2(h[1].v[k], h[1].v[k + 1]), make_float2(h[2].v[k], h[2].v[k + 1]), px, py, pz, acc_a, acc_b);
-        sx.v[k] = px.x; sx.v[k + 1] = px.y; sy.v[k] = py.x; sy.v[k + 1] = py.y; sz.v[k] = pz.x; sz.v[k + 1] = pz.y;
-        any |= acc_a | acc_b;
-        if (DIAG) {
-          n_acc += (unsigned)acc_a + (unsigned)acc_b;
-          if (d.accept) { d.accept[site0 + 2u * k] = acc_a; d.accept[site0 + 2u * k + 2u] = acc_b; }
-        }
-      }
-      if (any) {
-        store<4>(ax + grow, sx);
-        store<4>(ay + grow, sy);
-        store<4>(az + grow, sz);
-      }
-    }
-    const uint32_t t = o_m; o_m = o_c; o_c = o_p; o_p = t;
-  }
-  if (DIAG && d.n_accept && n_acc) atomicAdd(d.n_accept, (unsigned long long)n_acc);
-}
-
 // ---- CSR: one thread per site of the colour -------------------------------------------------
 template <bool DIAG>
 __global__ void __launch_bounds__(256)
@@ -738,50 +590,6 @@ cudaError_t launch_sweeps_sc_coop(cudaStream_t st, float* s, ScLayout L, ScTile 
   unsigned long long s0 = sweep0;
   void* args[] = {&s, &L, &t, &p, &s0, &n_sweeps, &nblk, &partials, &series, &final_out};
   return cudaLaunchCooperativeKernel((const void*)kern, dim3(grid), dim3(threads), args, 0, st);
-}
-
-template <int TY, int ROWB, int ANISO, bool DIAG>
-static cudaError_t sweep_sc_staged_impl(cudaStream_t st, float* s, ScLayout L, int ZT, SweepParams p, int colour, Diag d) {
-  constexpr size_t smem_bytes = 3 * 3 * (TY + 2) * (size_t)ROWB + 64;
-  static bool configured = false;
-  auto kern = k_sweep_sc_staged<TY, ROWB, ANISO, DIAG>;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
-  const size_t n = L.n;
-  float* a = s + (size_t)colour * L.half;
-  const float* b = s + (size_t)(1 - colour) * L.half;
-  dim3 grid((L.Ly + TY - 1) / TY, (L.Lz + ZT - 1) / ZT);
-  kern<<<grid, (L.H / 4) * TY, smem_bytes, st>>>(a, a + n, a + 2 * n, b, b + n, b + 2 * n, L, p, colour, ZT, d);
-  return cudaGetLastError();
-}
-
-template <int TY, int ROWB>
-static cudaError_t sweep_sc_staged_pick(cudaStream_t st, float* s, ScLayout L, int ZT, SweepParams p, int colour, Diag d) {
-  const bool diag = d.accept || d.n_accept;
-  const int aniso = aniso_case(p);
-  if (diag) {
-    switch (aniso) {
-      case ANISO_NONE: return sweep_sc_staged_impl<TY, ROWB, ANISO_NONE, true>(st, s, L, ZT, p, colour, d);
-      case ANISO_Z: return sweep_sc_staged_impl<TY, ROWB, ANISO_Z, true>(st, s, L, ZT, p, colour, d);
-      default: return sweep_sc_staged_impl<TY, ROWB, ANISO_GENERAL, true>(st, s, L, ZT, p, colour, d);
-    }
-  }
-  switch (aniso) {
-    case ANISO_NONE: return sweep_sc_staged_impl<TY, ROWB, ANISO_NONE, false>(st, s, L, ZT, p, colour, d);
-    case ANISO_Z: return sweep_sc_staged_impl<TY, ROWB, ANISO_Z, false>(st, s, L, ZT, p, colour, d);
-    default: return sweep_sc_staged_impl<TY, ROWB, ANISO_GENERAL, false>(st, s, L, ZT, p, colour, d);
-  }
-}
-
-bool sc_staged_supported(const ScLayout& L) { return L.H % 4 == 0 && L.H <= 256; }
-
-cudaError_t launch_sweep_sc_staged(cudaStream_t st, float* s, ScLayout L, int ZT, SweepParams p, int colour, Diag d) {
-  if (L.H > 128) return sweep_sc_staged_pick<4, 1024>(st, s, L, ZT, p, colour, d);
-  if (L.H > 64) return sweep_sc_staged_pick<8, 512>(st, s, L, ZT, p, colour, d);
-  return sweep_sc_staged_pick<16, 256>(st, s, L, ZT, p, colour, d);
 }
 
 cudaError_t launch_sweep_csr(cudaStream_t st, float* s, CsrDev g, uint32_t list_begin, uint32_t list_count,

@@ -1,0 +1,279 @@
+// hb_sc_ws.cu -- simple cubic colour pass, warp-specialised and persistent.
+//
+// Why: in the direct kernel (hb_kernels.cu) a third of the executed instructions are not the update at
+// all but the memory side of it -- 64-bit address arithmetic for 24 global accesses and 12 prefetches per
+// thread and plane -- and the board runs at its power cap, so instructions are what the sustained rate pays
+// for.  Here the memory side is moved out of the update warps:
+//
+//   * one PRODUCER warp per CTA streams whole lattice rows into shared memory with 1-D bulk asynchronous
+//     copies (cp.async.bulk, the TMA engine), completing on mbarriers: a ring of NB plane slots of the
+//     other colour (rows y0-1 .. y0+TY);
+//   * the CONSUMER warps wait on a "full" barrier, read everything with LDS at compile-time offsets (row
+//     pitch ROWB is a template constant, the periodic wrap in x is an index inside the staged row), release
+//     the slots through "empty" barriers, run the attempt arithmetic of hb_device.cuh; their own spins they
+//     load themselves one plane ahead (LDG.128) and store with STG.128 at the same addresses.  No block-wide
+//     barrier in the steady state;
+//   * CTAs are persistent (one or two per SM): a CTA walks its tiles (TY rows x ZT planes) with the rings running
+//     across tile boundaries, so the pipeline is filled once per launch, not once per tile.
+//
+// Same arithmetic, same order of the neighbour sum, same bits as k_sweep_sc.
+#include "hb_device.cuh"
+#include "hb_internal.h"
+
+namespace hb {
+
+namespace {
+
+
+struct WsTiles {
+  int32_t n_ty, n_zc, ZT;   // tiles in y, chunks in z, planes per chunk
+};
+
+// kNB plane slots of the other colour (z-1, z, z+1 and look-ahead); MINB = CTAs per SM the kernel is built for
+template <int TY, int ROWB, int kNB, int MINB>
+struct WsSmem {
+  static constexpr uint32_t SLOT_B = 3u * (TY + 2) * ROWB;
+  static constexpr uint32_t OFF_BAR = kNB * SLOT_B;   // full[kNB], empty[kNB]
+  static constexpr uint32_t BYTES = OFF_BAR + 8u * (2 * kNB);
+};
+
+// ---- producer: one warp ------------------------------------------------------------------------------
+// plane k of a tile is lattice plane z0-1+k (periodic), rows y0-1 .. y0+ny (periodic) of the other colour
+template <int TY, int ROWB, int kNB, int MINB>
+__device__ __forceinline__ void ws_producer(const float* b, const ScLayout& L, const WsTiles& w,
+                                            uint32_t sbase) {
+  using S = WsSmem<TY, ROWB, kNB, MINB>;
+  const uint32_t lane = threadIdx.x;
+  const uint32_t row_bytes = (uint32_t)L.H * 4u;
+  const size_t n = L.n;
+  const uint32_t fullB = sbase + S::OFF_BAR, emptyB = fullB + 8u * kNB;
+  uint32_t gb = 0;   // planes issued so far
+  const int32_t n_tiles = w.n_ty * w.n_zc;
+  for (int32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    const int32_t ty = tile % w.n_ty, zc = tile / w.n_ty;
+    const int32_t y0 = ty * TY, ny = min(TY, L.Ly - y0);
+    const int32_t z0 = zc * w.ZT, nz = min(w.ZT, L.Lz - z0);
+    for (int32_t k = 0; k < nz + 2; ++k) {
+      {  // B plane k
+        int32_t zz = z0 - 1 + k;
+        zz = zz < 0 ? zz + L.Lz : (zz >= L.Lz ? zz - L.Lz : zz);
+        const uint32_t slot = gb % kNB, par = (gb / kNB) & 1u;
+        mbar_wait_backoff(emptyB + 8u * slot, par ^ 1u);
+        const uint32_t n_rows = 3u * (uint32_t)(ny + 2);
+        if (lane == 0) mbar_expect_tx(fullB + 8u * slot, n_rows * row_bytes);
+        __syncwarp();
+        for (uint32_t q = lane; q < n_rows; q += 32) {
+          const uint32_t comp = q / (uint32_t)(ny + 2), r = q - comp * (uint32_t)(ny + 2);
+          int32_t yy = y0 - 1 + (int32_t)r;
+          yy = yy < 0 ? yy + L.Ly : (yy >= L.Ly ? yy - L.Ly : yy);
+          const float* src = b + comp * n + ((size_t)zz * L.Ly + yy) * L.H;
+          bulk_g2s(sbase + slot * S::SLOT_B + (comp * (TY + 2) + r) * ROWB, src, row_bytes, fullB + 8u * slot);
+        }
+        ++gb;
+      }
+    }
+  }
+}
+
+// ---- consumers -------------------------------------------------------------------------------------------
+template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS>
+__device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const WsTiles& w, const SweepParams& P, int colour,
+                                            int mode, unsigned char* smem, uint32_t sbase, double acc[4]) {
+  using S = WsSmem<TY, ROWB, kNB, MINB>;
+  const uint32_t fullB = sbase + S::OFF_BAR, emptyB = fullB + 8u * kNB;
+  const int32_t HV = L.H >> 2;
+  const int32_t c = (int32_t)threadIdx.x - 32;
+  const int32_t r = c / HV, j = c - r * HV;
+  const int32_t i0 = j * 4;
+  const bool lane0 = (threadIdx.x & 31) == 0;
+  // byte offsets inside a plane slot (component 0): the thread's row is row r+1 of the slot
+  const uint32_t t_row = (uint32_t)(r + 1) * ROWB;
+  const uint32_t t_off = t_row + (uint32_t)j * 16u;
+  const uint32_t h_lo = t_row + (uint32_t)(i0 == 0 ? L.H - 1 : i0 - 1) * 4u;        // p = 0: element i0-1 (periodic)
+  const uint32_t h_hi = t_row + (uint32_t)(i0 + 4 >= L.H ? i0 + 4 - L.H : i0 + 4) * 4u;  // p = 1: element i0+4
+  const size_t n = L.n;
+  const size_t plane = (size_t)L.Ly * L.H;
+  uint32_t cb = 0;   // planes consumed before this tile
+  const int32_t n_tiles = w.n_ty * w.n_zc;
+  for (int32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    const int32_t ty = tile % w.n_ty, zc = tile / w.n_ty;
+    const int32_t y0 = ty * TY, ny = min(TY, L.Ly - y0);
+    const int32_t z0 = zc * w.ZT, nz = min(w.ZT, L.Lz - z0);
+    const bool active = r < ny;
+    const int32_t y = y0 + r;
+    float* gx = a + ((size_t)z0 * L.Ly + y) * L.H + i0;            // own spins of plane z0 (x component)
+    uint32_t site_row = (uint32_t)(z0 * L.Ly + y) * (uint32_t)L.Lx + 2u * (uint32_t)i0;
+    // own spins come straight from global memory, one plane ahead of their use (only this thread writes them)
+    Vec<4> nxt[3];
+    if (active) { nxt[0] = load_rw<4>(gx); nxt[1] = load_rw<4>(gx + n); nxt[2] = load_rw<4>(gx + 2 * n); }
+    for (int32_t s = 0; s < nz; ++s) {
+      Vec<4> sp[3] = {nxt[0], nxt[1], nxt[2]};
+      if (active && s + 1 < nz) {
+        nxt[0] = load_rw<4>(gx + plane); nxt[1] = load_rw<4>(gx + plane + n); nxt[2] = load_rw<4>(gx + plane + 2 * n);
+      }
+      const uint32_t gm = cb + (uint32_t)s;
+      if (s == 0) {
+        mbar_wait(fullB + 8u * (gm % kNB), (gm / kNB) & 1u);
+        mbar_wait(fullB + 8u * ((gm + 1) % kNB), ((gm + 1) / kNB) & 1u);
+      }
+      mbar_wait(fullB + 8u * ((gm + 2) % kNB), ((gm + 2) / kNB) & 1u);
+      const unsigned char* Bm = smem + (gm % kNB) * S::SLOT_B;
+      const unsigned char* Bc = smem + ((gm + 1) % kNB) * S::SLOT_B;
+      const unsigned char* Bp = smem + ((gm + 2) % kNB) * S::SLOT_B;
+      const int32_t p = (colour + y + z0 + s) & 1;
+      const uint32_t h_off = p ? h_hi : h_lo;
+      Vec<4> h[3];
+      if (active) {
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+          constexpr uint32_t CB = (TY + 2) * ROWB;
+          const float4 cc = *reinterpret_cast<const float4*>(Bc + q * CB + t_off);
+          const float halo = *reinterpret_cast<const float*>(Bc + q * CB + h_off);
+          const float4 ym = *reinterpret_cast<const float4*>(Bc + q * CB + t_off - ROWB);
+          const float4 yp = *reinterpret_cast<const float4*>(Bc + q * CB + t_off + ROWB);
+          const float4 zm = *reinterpret_cast<const float4*>(Bm + q * CB + t_off);
+          const float4 zp = *reinterpret_cast<const float4*>(Bp + q * CB + t_off);
+          // -x,+x,-y,+y,-z,+z: the two x terms are elements i-1+p and i+p of the row (they commute bitwise)
+          const f2 sel_lo = make_float2(p ? cc.y : halo, p ? cc.z : cc.x);
+          const f2 sel_hi = make_float2(p ? cc.w : cc.y, p ? halo : cc.z);
+          f2 u = add2(make_float2(cc.x, cc.y), sel_lo), v = add2(make_float2(cc.z, cc.w), sel_hi);
+          u = add2(u, make_float2(ym.x, ym.y)); v = add2(v, make_float2(ym.z, ym.w));
+          u = add2(u, make_float2(yp.x, yp.y)); v = add2(v, make_float2(yp.z, yp.w));
+          u = add2(u, make_float2(zm.x, zm.y)); v = add2(v, make_float2(zm.z, zm.w));
+          u = add2(u, make_float2(zp.x, zp.y)); v = add2(v, make_float2(zp.z, zp.w));
+          h[q] = Vec<4>{{u.x, u.y, v.x, v.y}};
+        }
+      }
+      // this warp is done with plane z-1 (after the last plane of a tile: with all three)
+      __syncwarp();
+      if (lane0) {
+        mbar_arrive(emptyB + 8u * (gm % kNB));
+        if (s == nz - 1) {
+          mbar_arrive(emptyB + 8u * ((gm + 1) % kNB));
+          mbar_arrive(emptyB + 8u * ((gm + 2) % kNB));
+        }
+      }
+      if (active) {
+        const uint32_t site0 = site_row + (uint32_t)p;
+        bool any = false;
+#pragma unroll
+        for (int k = 0; k < 4; k += 2) {
+          const Rand4 ra = philox4x32_10(site0 + 2u * k, 0u, P.sweep_lo, P.sweep_hi, P.seed_lo, P.seed_hi);
+          const Rand4 rb = philox4x32_10(site0 + 2u * k + 2u, 0u, P.sweep_lo, P.sweep_hi, P.seed_lo, P.seed_hi);
+          f2 px = make_float2(sp[0].v[k], sp[0].v[k + 1]), py = make_float2(sp[1].v[k], sp[1].v[k + 1]),
+             pz = make_float2(sp[2].v[k], sp[2].v[k + 1]);
+          bool acc_a, acc_b;
+          attempt2<ANISO>(ra, rb, P.J, P.K, P.beta, P.ex, P.ey, P.ez, make_float2(h[0].v[k], h[0].v[k + 1]),
+                          make_float2(h[1].v[k], h[1].v[k + 1]), make_float2(h[2].v[k], h[2].v[k + 1]), px, py, pz, acc_a, acc_b);
+          sp[0].v[k] = px.x; sp[0].v[k + 1] = px.y; sp[1].v[k] = py.x; sp[1].v[k + 1] = py.y;
+          sp[2].v[k] = pz.x; sp[2].v[k + 1] = pz.y;
+          any |= acc_a | acc_b;
+        }
+        if (any) {
+          store<4>(gx, sp[0]);
+          store<4>(gx + n, sp[1]);
+          store<4>(gx + 2 * n, sp[2]);
+        }
+        if (MEAS) {
+          float mx = 0.0f, my = 0.0f, mz = 0.0f, me = 0.0f;
+          const float Jx = (mode == 2) ? -P.J : 0.0f;
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            mx = __fadd_rn(mx, sp[0].v[k]); my = __fadd_rn(my, sp[1].v[k]); mz = __fadd_rn(mz, sp[2].v[k]);
+            const float sh = __fmaf_rn(sp[2].v[k], h[2].v[k], __fmaf_rn(sp[1].v[k], h[1].v[k], __fmul_rn(sp[0].v[k], h[0].v[k])));
+            const float e = __fmaf_rn(sp[2].v[k], P.ez, __fmaf_rn(sp[1].v[k], P.ey, __fmul_rn(sp[0].v[k], P.ex)));
+            me = __fadd_rn(me, __fmaf_rn(Jx, sh, __fmul_rn(-P.K, __fmul_rn(e, e))));
+          }
+          acc[0] += (double)mx; acc[1] += (double)my; acc[2] += (double)mz; acc[3] += (double)me;
+        }
+      }
+      gx += plane;
+      site_row += (uint32_t)(L.Ly * L.Lx);
+    }
+    cb += (uint32_t)nz + 2u;
+  }
+}
+
+template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS>
+__global__ void __launch_bounds__(32 + 32 * ((TY * (ROWB / 16) + 31) / 32), MINB)
+k_sweep_sc_ws(float* a, const float* b, ScLayout L, WsTiles w, SweepParams P, int colour, Meas m) {
+  using S = WsSmem<TY, ROWB, kNB, MINB>;
+  extern __shared__ __align__(128) unsigned char smem[];
+  const uint32_t sbase = smem_u32(smem);
+  const uint32_t n_cwarps = (blockDim.x >> 5) - 1;
+  if (threadIdx.x == 0) {
+    const uint32_t bar = sbase + S::OFF_BAR;
+    for (int i = 0; i < kNB; ++i) { mbar_init(bar + 8u * i, 1); mbar_init(bar + 8u * (kNB + i), n_cwarps); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  double acc[4] = {0.0, 0.0, 0.0, 0.0};
+  if (threadIdx.x < 32) ws_producer<TY, ROWB, kNB, MINB>(b, L, w, sbase);
+  else ws_consumer<TY, ROWB, kNB, MINB, ANISO, MEAS>(a, L, w, P, colour, m.mode, smem, sbase, acc);
+  if (MEAS) block_reduce4(acc[0], acc[1], acc[2], acc[3], m.partials + (size_t)blockIdx.x * 4);
+}
+
+template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS>
+cudaError_t ws_go(cudaStream_t st, float* s, const ScLayout& L, int ZT, int grid_cap, const SweepParams& p, int colour, const Meas& m) {
+  using S = WsSmem<TY, ROWB, kNB, MINB>;
+  auto kern = k_sweep_sc_ws<TY, ROWB, kNB, MINB, ANISO, MEAS>;
+  static bool configured = false;
+  if (!configured) {
+    const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::BYTES);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  WsTiles w;
+  w.ZT = ZT;
+  w.n_ty = (L.Ly + TY - 1) / TY;
+  w.n_zc = (L.Lz + ZT - 1) / ZT;
+  const int n_tiles = w.n_ty * w.n_zc;
+  const int grid = n_tiles < grid_cap ? n_tiles : grid_cap;
+  const int threads = 32 + 32 * ((TY * (L.H / 4) + 31) / 32);
+  float* a = s + (size_t)colour * L.half;
+  const float* b = s + (size_t)(1 - colour) * L.half;
+  kern<<<grid, threads, S::BYTES, st>>>(a, b, L, w, p, colour, m);
+  return cudaGetLastError();
+}
+
+template <int TY, int ROWB, int kNB, int MINB>
+cudaError_t ws_pick(cudaStream_t st, float* s, const ScLayout& L, int ZT, int grid_cap, const SweepParams& p, int colour, const Meas& m) {
+  const int aniso = (p.K == 0.0f) ? ANISO_NONE : ((p.ex == 0.0f && p.ey == 0.0f && p.ez == 1.0f) ? ANISO_Z : ANISO_GENERAL);
+  if (m.mode != 0) {
+    switch (aniso) {
+      case ANISO_NONE: return ws_go<TY, ROWB, kNB, MINB, ANISO_NONE, true>(st, s, L, ZT, grid_cap, p, colour, m);
+      case ANISO_Z: return ws_go<TY, ROWB, kNB, MINB, ANISO_Z, true>(st, s, L, ZT, grid_cap, p, colour, m);
+      default: return ws_go<TY, ROWB, kNB, MINB, ANISO_GENERAL, true>(st, s, L, ZT, grid_cap, p, colour, m);
+    }
+  }
+  switch (aniso) {
+    case ANISO_NONE: return ws_go<TY, ROWB, kNB, MINB, ANISO_NONE, false>(st, s, L, ZT, grid_cap, p, colour, m);
+    case ANISO_Z: return ws_go<TY, ROWB, kNB, MINB, ANISO_Z, false>(st, s, L, ZT, grid_cap, p, colour, m);
+    default: return ws_go<TY, ROWB, kNB, MINB, ANISO_GENERAL, false>(st, s, L, ZT, grid_cap, p, colour, m);
+  }
+}
+
+}  // namespace
+
+// rows of up to 256 floats per colour (Lx <= 512), a multiple of 4: the staged row pitch is 1024 bytes
+bool sc_ws_supported(const ScLayout& L) { return L.H % 4 == 0 && L.H <= 256; }
+
+// variants (option sc_ws_variant): 0 = 4-row tiles, 5 plane slots, 2 CTAs per SM (108 regs); 1 = 8-row tiles, 6 slots, 1 CTA
+static int ws_ty(int variant) { return variant == 1 ? 8 : 4; }
+static int ws_ctas_per_sm(int variant) { return variant == 1 ? 1 : 2; }
+
+// blocks of one launch (= block partials of the fused measurement); grid_cap = SMs
+int sc_ws_blocks(const ScLayout& L, int ZT, int grid_cap, int variant) {
+  const int ty = ws_ty(variant);
+  const int n_tiles = ((L.Ly + ty - 1) / ty) * ((L.Lz + ZT - 1) / ZT);
+  const int cap = grid_cap * ws_ctas_per_sm(variant);
+  return n_tiles < cap ? n_tiles : cap;
+}
+
+cudaError_t launch_sweep_sc_ws(cudaStream_t st, float* s, ScLayout L, int ZT, int grid_cap, int variant, SweepParams p, int colour, Meas m) {
+  const int cap = grid_cap * ws_ctas_per_sm(variant);
+  if (variant == 1) return ws_pick<8, 1024, 6, 1>(st, s, L, ZT, cap, p, colour, m);
+  return ws_pick<4, 1024, 5, 2>(st, s, L, ZT, cap, p, colour, m);
+}
+
+}  // namespace hb

@@ -241,6 +241,14 @@ def test_full_size_first_10_sweeps(name):
     st.sweep(T, 2)
     if mism == 0:
         assert spins_equal(ctx.get_spins(), st.get_spins())
+    if name == "c4":
+        # the warp-specialised persistent kernel (TMA-staged neighbour planes) continues the same trajectory
+        ctx.set_option("sc_kernel", 1)
+        ctx.sweep(T, 1)
+        st.sweep(T, 1)
+        if mism == 0:
+            assert spins_equal(ctx.get_spins(), st.get_spins())
+        _measure_close(ctx, st, lat.n)
 
 
 # ---- P3: long-run statistics against the fp64 random-site oracle (BASELINE.json north_star) ----------
@@ -348,3 +356,35 @@ def test_persistent_kernels_match_the_oracle():
         assert np.max(np.abs(Mg - Mo)) <= 1e-7 and np.max(np.abs(Eg - Eo)) <= 1e-6 * lat.n
         assert ctx.sweep_count == st.sweep_count
         ctx.close()
+
+
+def test_warp_specialised_kernel_matches_the_oracle():
+    # sc_kernel = 1: producer warp + bulk asynchronous copies into rings of plane slots, consumer warps read LDS,
+    # persistent CTAs walking (y-tile, z-chunk) tiles.  Ragged tiles in y and z, a single row, the widest row (Lx = 512),
+    # fewer CTAs than tiles (rings running across tile boundaries), both variants, fused measurement.
+    cases = [(W.SMALL["c4"], {}), (W.SMALL["c1"], {}),
+             (dict(W.SMALL["c4"], L=(40, 12, 10), K=0.3, e=(0.6, 0.0, 0.8)), {"sc_ws_zt": 3}),
+             (dict(W.SMALL["c4"], L=(64, 20, 6)), {"sc_ws_zt": 4, "sc_ws_ctas": 2}),
+             (dict(W.SMALL["c4"], L=(8, 2, 2)), {}), (dict(W.SMALL["c4"], L=(512, 10, 4)), {"sc_ws_zt": 2}),
+             (W.SMALL["c4"], {"sc_ws_variant": 1}), (dict(W.SMALL["c4"], L=(40, 14, 10)), {"sc_ws_variant": 1, "sc_ws_zt": 3}),
+             (dict(W.SMALL["c4"], L=(40, 14, 10)), {"sc_ws_variant": 0, "sc_ws_zt": 10, "sc_ws_ctas": 1})]
+    for cfg, opts in cases:
+        lat, st = make_oracle(cfg)
+        ctx = make_gpu(cfg)
+        ctx.set_option("sc_kernel", 1)
+        for k, v in opts.items():
+            ctx.set_option(k, v)
+        start(cfg, ctx, st)
+        for T, k in ((1.44, 1), (1.44, 4), (0.4, 2)):
+            ctx.sweep(T, k)
+            st.sweep(T, k)
+            assert spins_equal(ctx.get_spins(), st.get_spins()), (cfg["L"], opts)
+            _measure_close(ctx, st, lat.n)
+        Mg, Eg = ctx.sweep_series(1.2, 9)
+        Mo, Eo = st.series(1.2, 9)
+        assert np.max(np.abs(Mg - Mo)) <= 1e-7 and np.max(np.abs(Eg - Eo)) <= 1e-6 * lat.n
+        acc_o = st.sweep(1.0, 1, record=True)[0]                     # the recording path falls back to the direct kernel
+        assert np.array_equal(ctx.sweep_record(1.0), acc_o)
+        ctx.close()
+    with pytest.raises(hb.HbError):
+        hb.Context(hb.Lattice("sc", 6)).set_option("sc_kernel", 1)   # rows of 3 floats: not a multiple of 4
