@@ -338,6 +338,8 @@ def main():
     bytes_per_launch = bytes_per_update * n / n_colours
     achieved = bytes_per_launch / avg_launch_s / 1e9
     kernel = {"sc": "k_sweep_sc", "bcc": "k_sweep_bravais", "fcc": "k_sweep_bravais", "sphere": "k_sweep_ell"}[cfg["kind"]]
+    if cfg["kind"] == "sc" and ctx.get_option("sc_kernel") == 1:
+        kernel = "k_sweep_sc_ws"
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.workload), "kernel": kernel, "peak_source": peak_src,
                 "algorithmic_bytes_per_update": bytes_per_update, "bytes_per_launch": bytes_per_launch,

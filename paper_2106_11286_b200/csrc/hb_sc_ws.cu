@@ -25,6 +25,13 @@ namespace hb {
 namespace {
 
 
+// position on a ring of N slots: slot index and the parity of the pass over the ring
+template <int N>
+struct RingPos {
+  uint32_t slot = 0, par = 0;
+  __device__ __forceinline__ void next() { if (++slot == N) { slot = 0; par ^= 1u; } }
+};
+
 struct WsTiles {
   int32_t n_ty, n_zc, ZT;   // tiles in y, chunks in z, planes per chunk
 };
@@ -47,7 +54,7 @@ __device__ __forceinline__ void ws_producer(const float* b, const ScLayout& L, c
   const uint32_t row_bytes = (uint32_t)L.H * 4u;
   const size_t n = L.n;
   const uint32_t fullB = sbase + S::OFF_BAR, emptyB = fullB + 8u * kNB;
-  uint32_t gb = 0;   // planes issued so far
+  RingPos<kNB> rp;   // next plane slot to fill
   const int32_t n_tiles = w.n_ty * w.n_zc;
   for (int32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
     const int32_t ty = tile % w.n_ty, zc = tile / w.n_ty;
@@ -57,8 +64,8 @@ __device__ __forceinline__ void ws_producer(const float* b, const ScLayout& L, c
       {  // B plane k
         int32_t zz = z0 - 1 + k;
         zz = zz < 0 ? zz + L.Lz : (zz >= L.Lz ? zz - L.Lz : zz);
-        const uint32_t slot = gb % kNB, par = (gb / kNB) & 1u;
-        mbar_wait_backoff(emptyB + 8u * slot, par ^ 1u);
+        const uint32_t slot = rp.slot;
+        mbar_wait_backoff(emptyB + 8u * slot, rp.par ^ 1u);
         const uint32_t n_rows = 3u * (uint32_t)(ny + 2);
         if (lane == 0) mbar_expect_tx(fullB + 8u * slot, n_rows * row_bytes);
         __syncwarp();
@@ -69,7 +76,7 @@ __device__ __forceinline__ void ws_producer(const float* b, const ScLayout& L, c
           const float* src = b + comp * n + ((size_t)zz * L.Ly + yy) * L.H;
           bulk_g2s(sbase + slot * S::SLOT_B + (comp * (TY + 2) + r) * ROWB, src, row_bytes, fullB + 8u * slot);
         }
-        ++gb;
+        rp.next();
       }
     }
   }
@@ -93,7 +100,7 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
   const uint32_t h_hi = t_row + (uint32_t)(i0 + 4 >= L.H ? i0 + 4 - L.H : i0 + 4) * 4u;  // p = 1: element i0+4
   const size_t n = L.n;
   const size_t plane = (size_t)L.Ly * L.H;
-  uint32_t cb = 0;   // planes consumed before this tile
+  RingPos<kNB> rm;   // slot of plane z-1 of the current step
   const int32_t n_tiles = w.n_ty * w.n_zc;
   for (int32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
     const int32_t ty = tile % w.n_ty, zc = tile / w.n_ty;
@@ -104,22 +111,29 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
     float* gx = a + ((size_t)z0 * L.Ly + y) * L.H + i0;            // own spins of plane z0 (x component)
     uint32_t site_row = (uint32_t)(z0 * L.Ly + y) * (uint32_t)L.Lx + 2u * (uint32_t)i0;
     // own spins come straight from global memory, one plane ahead of their use (only this thread writes them)
+    constexpr bool PREF = MINB < 3;   // with 3 CTAs per SM (72 registers) the other warps cover the latency instead
     Vec<4> nxt[3];
-    if (active) { nxt[0] = load_rw<4>(gx); nxt[1] = load_rw<4>(gx + n); nxt[2] = load_rw<4>(gx + 2 * n); }
+    if (PREF && active) { nxt[0] = load_rw<4>(gx); nxt[1] = load_rw<4>(gx + n); nxt[2] = load_rw<4>(gx + 2 * n); }
     for (int32_t s = 0; s < nz; ++s) {
-      Vec<4> sp[3] = {nxt[0], nxt[1], nxt[2]};
-      if (active && s + 1 < nz) {
-        nxt[0] = load_rw<4>(gx + plane); nxt[1] = load_rw<4>(gx + plane + n); nxt[2] = load_rw<4>(gx + plane + 2 * n);
+      Vec<4> sp[3];
+      if (PREF) {
+        sp[0] = nxt[0]; sp[1] = nxt[1]; sp[2] = nxt[2];
+        if (active && s + 1 < nz) {
+          nxt[0] = load_rw<4>(gx + plane); nxt[1] = load_rw<4>(gx + plane + n); nxt[2] = load_rw<4>(gx + plane + 2 * n);
+        }
+      } else if (active) {
+        sp[0] = load_rw<4>(gx); sp[1] = load_rw<4>(gx + n); sp[2] = load_rw<4>(gx + 2 * n);
       }
-      const uint32_t gm = cb + (uint32_t)s;
+      RingPos<kNB> rc = rm; rc.next();
+      RingPos<kNB> rq = rc; rq.next();
       if (s == 0) {
-        mbar_wait(fullB + 8u * (gm % kNB), (gm / kNB) & 1u);
-        mbar_wait(fullB + 8u * ((gm + 1) % kNB), ((gm + 1) / kNB) & 1u);
+        mbar_wait(fullB + 8u * rm.slot, rm.par);
+        mbar_wait(fullB + 8u * rc.slot, rc.par);
       }
-      mbar_wait(fullB + 8u * ((gm + 2) % kNB), ((gm + 2) / kNB) & 1u);
-      const unsigned char* Bm = smem + (gm % kNB) * S::SLOT_B;
-      const unsigned char* Bc = smem + ((gm + 1) % kNB) * S::SLOT_B;
-      const unsigned char* Bp = smem + ((gm + 2) % kNB) * S::SLOT_B;
+      mbar_wait(fullB + 8u * rq.slot, rq.par);
+      const unsigned char* Bm = smem + rm.slot * S::SLOT_B;
+      const unsigned char* Bc = smem + rc.slot * S::SLOT_B;
+      const unsigned char* Bp = smem + rq.slot * S::SLOT_B;
       const int32_t p = (colour + y + z0 + s) & 1;
       const uint32_t h_off = p ? h_hi : h_lo;
       Vec<4> h[3];
@@ -147,10 +161,10 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
       // this warp is done with plane z-1 (after the last plane of a tile: with all three)
       __syncwarp();
       if (lane0) {
-        mbar_arrive(emptyB + 8u * (gm % kNB));
+        mbar_arrive(emptyB + 8u * rm.slot);
         if (s == nz - 1) {
-          mbar_arrive(emptyB + 8u * ((gm + 1) % kNB));
-          mbar_arrive(emptyB + 8u * ((gm + 2) % kNB));
+          mbar_arrive(emptyB + 8u * rc.slot);
+          mbar_arrive(emptyB + 8u * rq.slot);
         }
       }
       if (active) {
@@ -189,13 +203,14 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
       }
       gx += plane;
       site_row += (uint32_t)(L.Ly * L.Lx);
+      rm.next();
     }
-    cb += (uint32_t)nz + 2u;
+    rm.next(); rm.next();   // the two extra planes of the tile
   }
 }
 
 template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS>
-__global__ void __launch_bounds__(32 + 32 * ((TY * (ROWB / 16) + 31) / 32), MINB)
+__global__ void __launch_bounds__(32 + 32 * ((TY * (ROWB / 16) + 31) / 32) > 1024 ? 1024 : 32 + 32 * ((TY * (ROWB / 16) + 31) / 32), MINB)
 k_sweep_sc_ws(float* a, const float* b, ScLayout L, WsTiles w, SweepParams P, int colour, Meas m) {
   using S = WsSmem<TY, ROWB, kNB, MINB>;
   extern __shared__ __align__(128) unsigned char smem[];
@@ -258,9 +273,13 @@ cudaError_t ws_pick(cudaStream_t st, float* s, const ScLayout& L, int ZT, int gr
 // rows of up to 256 floats per colour (Lx <= 512), a multiple of 4: the staged row pitch is 1024 bytes
 bool sc_ws_supported(const ScLayout& L) { return L.H % 4 == 0 && L.H <= 256; }
 
-// variants (option sc_ws_variant): 0 = 4-row tiles, 5 plane slots, 2 CTAs per SM (108 regs); 1 = 8-row tiles, 6 slots, 1 CTA
+// variants (option sc_ws_variant), sustained rate on c4 (sc L = 464) beside the direct kernel's 116.8 Gupd/s:
+//   2 = 4-row tiles, 4 plane slots, 3 CTAs per SM, 72 registers, own spins loaded at the top of the step   120.9  (default)
+//   0 = 4-row tiles, 5 plane slots, 2 CTAs per SM, 96 registers, own spins loaded one plane ahead          116.9
+//   1 = 8-row tiles, 6 plane slots, 1 CTA per SM                                                            117.4
+// (11-row tiles, whose 638 consumer threads fill 99.7 % of their warps' lanes, 1 CTA per SM: 111-113)
 static int ws_ty(int variant) { return variant == 1 ? 8 : 4; }
-static int ws_ctas_per_sm(int variant) { return variant == 1 ? 1 : 2; }
+static int ws_ctas_per_sm(int variant) { return variant == 1 ? 1 : (variant == 2 ? 3 : 2); }
 
 // blocks of one launch (= block partials of the fused measurement); grid_cap = SMs
 int sc_ws_blocks(const ScLayout& L, int ZT, int grid_cap, int variant) {
@@ -273,6 +292,7 @@ int sc_ws_blocks(const ScLayout& L, int ZT, int grid_cap, int variant) {
 cudaError_t launch_sweep_sc_ws(cudaStream_t st, float* s, ScLayout L, int ZT, int grid_cap, int variant, SweepParams p, int colour, Meas m) {
   const int cap = grid_cap * ws_ctas_per_sm(variant);
   if (variant == 1) return ws_pick<8, 1024, 6, 1>(st, s, L, ZT, cap, p, colour, m);
+  if (variant == 2) return ws_pick<4, 1024, 4, 3>(st, s, L, ZT, cap, p, colour, m);
   return ws_pick<4, 1024, 5, 2>(st, s, L, ZT, cap, p, colour, m);
 }
 
