@@ -346,6 +346,8 @@ def main():
                 "avg_launch_ms": avg_launch_s * 1e3, "frac_of_8TBs_nominal": achieved / 8000.0}
 
     cpu = None if args.no_cpu_baseline else run_cpu_baseline(cfg)
+    # acceptance rate of one more sweep of the state the run ended in (reported with every timed config)
+    acceptance = float(ctx.sweep_record(T).mean())
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -355,6 +357,7 @@ def main():
                    "lattice": "%s %s" % (cfg["kind"], cfg.get("L", cfg.get("R"))), "n_spins": n, "colours": n_colours,
                    "J": cfg["J"], "K": cfg["K"], "T": T, "start": cfg["start"], "seed": cfg["seed"],
                    "sweeps_per_step": SWEEPS_PER_STEP, "measurements_per_step": 1, "options": options,
+                   "acceptance_rate": acceptance,
                    "l2": "state %.0f MB >> 126 MB L2: no flush between iterations" % (12.0 * n / 1e6)
                    if 12.0 * n > 4 * 126e6 else "state fits in L2: HBM roofline not meaningful",
                    "multi_gpu": "replicas only (seed + rank)"},

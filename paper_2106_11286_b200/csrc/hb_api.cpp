@@ -394,7 +394,7 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
     if (c->ws_zt > c->sc.Lz) c->ws_zt = c->sc.Lz;
     // the warp-specialised kernel is built for long rows (pitch 1024 B): with them, on lattices far larger than L2, it
     // sustains 3-4 % more than the direct kernel and stays below the power cap; everything else runs direct
-    c->sc_kernel = (sc_ws_supported(c->sc) && c->sc.H >= 192 && P.n >= (int64_t(1) << 24)) ? 1 : 0;
+    c->sc_kernel = (sc_ws_supported(c->sc) && c->sc.H >= 224 && P.n >= (int64_t(1) << 24)) ? 1 : 0;
     c->ws_variant = 2;
   }
 
