@@ -204,7 +204,7 @@ int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d, Meas m = Mea
     else
       HB_CUDA(c, launch_sweep_sc(c->stream, c->spins, c->sc, c->tile, p, colour, d, m));
   } else if (c->plan.engine == ENGINE_BRAVAIS) {
-    HB_CUDA(c, launch_sweep_bravais(c->stream, c->spins, c->br, c->tile, p, colour, d));
+    HB_CUDA(c, launch_sweep_bravais(c->stream, c->spins, c->br, c->tile, p, colour, d, m));
   } else {
     const uint32_t b = c->colour_begin[colour], e = c->colour_begin[colour + 1];
     if (e == b) return HB_OK;
@@ -217,7 +217,9 @@ int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d, Meas m = Mea
 
 // blocks per colour launch if this context can fuse the measurement into its colour passes, else 0
 int fused_blocks(const hb_ctx* c) {
-  if (!c->fused_measure || c->plan.engine != ENGINE_SC) return 0;
+  if (!c->fused_measure) return 0;
+  if (c->plan.engine == ENGINE_BRAVAIS) return bravais_fused_blocks(c->br, c->tile);
+  if (c->plan.engine != ENGINE_SC) return 0;
   if (c->sc_kernel == 1) return sc_ws_blocks(c->sc, c->ws_zt, c->n_sms, c->ws_variant);
   return sc_fused_blocks(c->sc, c->tile);
 }
@@ -253,7 +255,9 @@ int one_sweep(hb_ctx* c, float beta, Diag d, double* dev_out = nullptr) {
   const int fb = dev_out ? fused_blocks(c) : 0;
   for (int colour = 0; colour < c->n_colours; ++colour) {
     Meas m{nullptr, 0};
-    if (fb) m = Meas{c->partials() + (size_t)colour * fb * 4, colour == c->n_colours - 1 ? 2 : 1};
+    // sc: the last colour carries the whole exchange energy; bcc/fcc: every colour charges its bonds to lower colours
+    if (fb) m = Meas{c->partials() + (size_t)colour * fb * 4,
+                     (c->plan.engine == ENGINE_BRAVAIS || colour == c->n_colours - 1) ? 2 : 1};
     const int rc = one_colour(c, colour, p, d, m);
     if (rc != HB_OK) return rc;
   }

@@ -105,6 +105,27 @@ __device__ __forceinline__ void field(const float* __restrict__ s, uint32_t nc, 
   }
 }
 
+// the part of the field that comes from LOWER sublattices (colours already final in this sweep): with it every
+// bond is charged exactly once, at its higher-colour end, for the fused measurement
+template <int KIND, int B, int V, int K = 0>
+__device__ __forceinline__ void field_low(const float* __restrict__ s, uint32_t nc, uint32_t n, const Where& w,
+                                          Vec<V>& hx, Vec<V>& hy, Vec<V>& hz) {
+  if constexpr (K == 0) {
+#pragma unroll
+    for (int k = 0; k < V; ++k) { hx.v[k] = 0.0f; hy.v[k] = 0.0f; hz.v[k] = 0.0f; }
+  }
+  if constexpr (K < Geo<KIND>::Z) {
+    constexpr Nbr g = Geo<KIND>::nbr(B, K);
+    if constexpr (g.nb < B) {
+      const float* row = s + (size_t)g.nb * nc + (w.zo[g.dz + 1] + w.yo[g.dy + 1]);
+      hx = vadd<V>(hx, shifted<V>(row, w, g.dx));
+      hy = vadd<V>(hy, shifted<V>(row + n, w, g.dx));
+      hz = vadd<V>(hz, shifted<V>(row + 2 * (size_t)n, w, g.dx));
+    }
+    field_low<KIND, B, V, K + 1>(s, nc, n, w, hx, hy, hz);
+  }
+}
+
 __device__ __forceinline__ void where_y(Where& w, const BrLayout& L, int32_t y, int32_t i0, int V) {
   w.yo[0] = (uint32_t)((y == 0) ? L.Ly - 1 : y - 1) * (uint32_t)L.Lx;
   w.yo[1] = (uint32_t)y * (uint32_t)L.Lx;
@@ -120,18 +141,20 @@ __device__ __forceinline__ void where_z(Where& w, const BrLayout& L, int32_t z) 
   w.zo[2] = (uint32_t)((z == L.Lz - 1) ? 0 : z + 1) * plane;
 }
 
-template <int KIND, int B, int V, int ANISO, bool DIAG>
-__global__ void __launch_bounds__(256, 3)
-k_sweep_bravais(float* __restrict__ own, const float* __restrict__ all, BrLayout L, ScTile t, SweepParams P, Diag d) {
+template <int KIND, int B, int V, int ANISO, bool DIAG, bool MEAS = false>
+__global__ void __launch_bounds__(256, MEAS ? 1 : 3)
+k_sweep_bravais(float* __restrict__ own, const float* __restrict__ all, BrLayout L, ScTile t, SweepParams P, Diag d, Meas m) {
   const int32_t tj = threadIdx.x % t.JX, ty = threadIdx.x / t.JX;
   const int32_t i0 = (blockIdx.x * t.JX + tj) * V;
   const int32_t y = blockIdx.y * t.TY + ty;
-  if (i0 >= L.Lx || y >= L.Ly) return;
+  const bool outside = i0 >= L.Lx || y >= L.Ly;
+  if (!MEAS && outside) return;
   Where w;
-  where_y(w, L, y, i0, V);
-  const int32_t z0 = blockIdx.z * t.ZT, z1 = min(z0 + t.ZT, L.Lz);
+  where_y(w, L, outside ? 0 : y, outside ? 0 : i0, V);
+  const int32_t z0 = blockIdx.z * t.ZT, z1 = (MEAS && outside) ? z0 : min(z0 + t.ZT, L.Lz);
   const size_t n = L.n;
   unsigned n_acc = 0;
+  double acc_mx = 0.0, acc_my = 0.0, acc_mz = 0.0, acc_en = 0.0;
   for (int32_t z = z0; z < z1; ++z) {
     where_z(w, L, z);
     const uint32_t o = w.zo[1] + w.yo[1] + w.i0;             // offset inside the own sublattice
@@ -174,8 +197,25 @@ k_sweep_bravais(float* __restrict__ own, const float* __restrict__ all, BrLayout
       store<V>(own + n + o, sy);
       store<V>(own + 2 * n + o, sz);
     }
+    if (MEAS) {
+      Vec<V> lx, ly, lz;
+      field_low<KIND, B, V>(all, L.nc, L.n, w, lx, ly, lz);
+      float gx = 0.0f, gy = 0.0f, gz = 0.0f, ge = 0.0f;
+#pragma unroll
+      for (int k = 0; k < V; ++k) {
+        gx = __fadd_rn(gx, sx.v[k]); gy = __fadd_rn(gy, sy.v[k]); gz = __fadd_rn(gz, sz.v[k]);
+        const float sl = __fmaf_rn(sz.v[k], lz.v[k], __fmaf_rn(sy.v[k], ly.v[k], __fmul_rn(sx.v[k], lx.v[k])));
+        const float a = __fmaf_rn(sz.v[k], P.ez, __fmaf_rn(sy.v[k], P.ey, __fmul_rn(sx.v[k], P.ex)));
+        ge = __fadd_rn(ge, __fmaf_rn(-P.J, sl, __fmul_rn(-P.K, __fmul_rn(a, a))));
+      }
+      acc_mx += (double)gx; acc_my += (double)gy; acc_mz += (double)gz; acc_en += (double)ge;
+    }
   }
   if (DIAG && d.n_accept && n_acc) atomicAdd(d.n_accept, (unsigned long long)n_acc);
+  if (MEAS) {
+    const uint32_t blk = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+    block_reduce4(acc_mx, acc_my, acc_mz, acc_en, m.partials + (size_t)blk * 4);
+  }
 }
 
 // ---- measurement: M and E over all sublattices, fp64 accumulation ---------------------------------
@@ -217,19 +257,24 @@ inline int aniso_of(const SweepParams& p) {
   return (p.K == 0.0f) ? ANISO_NONE : ((p.ex == 0.0f && p.ey == 0.0f && p.ez == 1.0f) ? ANISO_Z : ANISO_GENERAL);
 }
 
-template <int KIND, int B, int V, int ANISO, bool DIAG>
-cudaError_t go(cudaStream_t st, float* s, const BrLayout& L, const ScTile& t, const SweepParams& p, const Diag& d) {
+template <int KIND, int B, int V, int ANISO, bool DIAG, bool MEAS = false>
+cudaError_t go(cudaStream_t st, float* s, const BrLayout& L, const ScTile& t, const SweepParams& p, const Diag& d,
+               const Meas& m = Meas{nullptr, 0}) {
   const int HV = L.Lx / V;
   dim3 grid((HV + t.JX - 1) / t.JX, (L.Ly + t.TY - 1) / t.TY, (L.Lz + t.ZT - 1) / t.ZT);
-  k_sweep_bravais<KIND, B, V, ANISO, DIAG><<<grid, t.JX * t.TY, 0, st>>>(s + (size_t)B * L.nc, s, L, t, p, d);
+  k_sweep_bravais<KIND, B, V, ANISO, DIAG, MEAS><<<grid, t.JX * t.TY, 0, st>>>(s + (size_t)B * L.nc, s, L, t, p, d, m);
   return cudaGetLastError();
 }
 
 // The tuned shape (V = 4, no diagnostics) carries the three anisotropy specialisations; the
 // narrow vectors and the recording variant use the general formula, which gives the same bits.
 template <int KIND, int B>
-cudaError_t pick(cudaStream_t st, float* s, const BrLayout& L, const ScTile& t, const SweepParams& p, const Diag& d) {
+cudaError_t pick(cudaStream_t st, float* s, const BrLayout& L, const ScTile& t, const SweepParams& p, const Diag& d, const Meas& m) {
   const bool diag = d.accept || d.n_accept;
+  if (m.mode != 0) {   // fused measurement: tuned vector width only, general anisotropy formula (same bits)
+    if (t.V != 4 || diag) return cudaErrorInvalidValue;
+    return go<KIND, B, 4, ANISO_GENERAL, false, true>(st, s, L, t, p, d, m);
+  }
   if (t.V == 4) {
     if (diag) return go<KIND, B, 4, ANISO_GENERAL, true>(st, s, L, t, p, d);
     switch (aniso_of(p)) {
@@ -255,18 +300,26 @@ cudaError_t measure(cudaStream_t st, const float* s, const BrLayout& L, int V, c
 
 }  // namespace
 
-cudaError_t launch_sweep_bravais(cudaStream_t st, float* s, BrLayout L, ScTile t, SweepParams p, int colour, Diag d) {
+// blocks of one colour launch if it can carry the fused measurement (4 doubles of partials per block), else 0
+int bravais_fused_blocks(const BrLayout& L, const ScTile& t) {
+  if (t.V != 4) return 0;
+  const int HV = L.Lx / 4;
+  const long long blocks = (long long)((HV + t.JX - 1) / t.JX) * ((L.Ly + t.TY - 1) / t.TY) * ((L.Lz + t.ZT - 1) / t.ZT);
+  return blocks <= kFusedBlocksMax / 2 ? (int)blocks : 0;   // four colours share the partials buffer
+}
+
+cudaError_t launch_sweep_bravais(cudaStream_t st, float* s, BrLayout L, ScTile t, SweepParams p, int colour, Diag d, Meas m) {
   if (L.kind == BR_BCC) {
     switch (colour) {
-      case 0: return pick<BR_BCC, 0>(st, s, L, t, p, d);
-      case 1: return pick<BR_BCC, 1>(st, s, L, t, p, d);
+      case 0: return pick<BR_BCC, 0>(st, s, L, t, p, d, m);
+      case 1: return pick<BR_BCC, 1>(st, s, L, t, p, d, m);
     }
   } else if (L.kind == BR_FCC) {
     switch (colour) {
-      case 0: return pick<BR_FCC, 0>(st, s, L, t, p, d);
-      case 1: return pick<BR_FCC, 1>(st, s, L, t, p, d);
-      case 2: return pick<BR_FCC, 2>(st, s, L, t, p, d);
-      case 3: return pick<BR_FCC, 3>(st, s, L, t, p, d);
+      case 0: return pick<BR_FCC, 0>(st, s, L, t, p, d, m);
+      case 1: return pick<BR_FCC, 1>(st, s, L, t, p, d, m);
+      case 2: return pick<BR_FCC, 2>(st, s, L, t, p, d, m);
+      case 3: return pick<BR_FCC, 3>(st, s, L, t, p, d, m);
     }
   }
   return cudaErrorInvalidValue;

@@ -106,7 +106,8 @@ cudaError_t launch_init_random_perm(cudaStream_t st, float* spins, const int32_t
 cudaError_t launch_fill_ell(cudaStream_t st, float* spins, uint32_t n, float x, float y, float z);
 // component comp of the internal float4 state <- plane[perm[m]] (to_internal) or plane[perm[m]] <- component
 cudaError_t launch_permute_ell(cudaStream_t st, float* spins, float* plane, const int32_t* perm, uint32_t n, int comp, bool to_internal);
-cudaError_t launch_sweep_bravais(cudaStream_t st, float* spins, BrLayout L, ScTile t, SweepParams p, int colour, Diag d);
+int bravais_fused_blocks(const BrLayout& L, const ScTile& t);
+cudaError_t launch_sweep_bravais(cudaStream_t st, float* spins, BrLayout L, ScTile t, SweepParams p, int colour, Diag d, Meas m);
 // measurement: partials must hold kMeasureBlocks*4 doubles; out receives (Mx*N, My*N, Mz*N, E)
 constexpr int kMeasureBlocks = 1184;
 cudaError_t launch_measure_sc(cudaStream_t st, const float* spins, ScLayout L, int V, SweepParams p, double* partials, double* out);

@@ -296,7 +296,10 @@ def test_fused_measurement_equals_the_separate_pass():
     # returns those.  Same P2 tolerances against the oracle, and against the separate pass on the same state.
     for cfg, opts in ((W.SMALL["c4"], {}), (W.SMALL["c1"], {}),
                       (dict(W.SMALL["c4"], L=(40, 12, 10), K=0.3, e=(0.6, 0.0, 0.8)), {"sc_jx": 3, "sc_ty": 5, "sc_zt": 3}),
-                      (dict(W.SMALL["c4"], L=(64, 8, 6)), {"sc_linear": 96})):
+                      (dict(W.SMALL["c4"], L=(64, 8, 6)), {"sc_linear": 96}),
+                      # bcc / fcc: every colour charges its bonds to the lower colours (already final in the sweep)
+                      (dict(W.SMALL["c2"], start="random"), {}), (dict(W.SMALL["c2"], L=(12, 5, 7), start="random"), {"sc_jx": 2, "sc_ty": 3, "sc_zt": 2}),
+                      (dict(W.SMALL["c3"], L=8, start="random"), {}), (dict(W.SMALL["c3"], L=(8, 3, 5), start="random"), {"sc_jx": 1, "sc_ty": 2})):
         lat, st = make_oracle(cfg)
         fused, plain = make_gpu(cfg), make_gpu(cfg)
         plain.set_option("fused_measure", 0)
