@@ -31,8 +31,9 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 # Sweeps of one step: config 4 is specified as "200 timed sweeps" (BASELINE.json), so its step is those 200 sweeps
-# followed by the measurement; the secondary workloads use 10.
-SWEEPS_BY_WORKLOAD = {"c4": 200}
+# followed by the measurement; the secondary workloads (scans of hundreds to thousands of sweeps per temperature)
+# use 50-100.
+SWEEPS_BY_WORKLOAD = {"c4": 200, "c1": 100, "c2": 100, "c3": 50, "c5": 50}
 SWEEPS_PER_STEP = 10
 METRIC = "attempted spin updates/sec (Gupd/s) and % of HBM roofline, 1 B200"
 UNIT = "Gupd/s"

@@ -110,6 +110,11 @@ struct hb_ctx {
   int csr_block = 128;
   int sc_kernel = 0;      // 0: direct loads through L1, 1: warp-specialised persistent kernel (TMA-staged neighbour planes)
   int ws_zt = 32, n_sms = 148, ws_variant = 2;   // warp-specialised kernel: planes per tile, CTAs = n_sms x CTAs/SM
+  int graph_mode = -1;         // replay hb_sweep's launches from a CUDA graph: -1 auto (lattices up to 2^23 sites), 0 off, 1 on
+  cudaStream_t cap_stream = nullptr;
+  cudaGraphExec_t gexec = nullptr;
+  float g_beta = 0.0f;
+  bool g_dirty = true;
   int sc_coop = -1;            // persistent multi-sweep kernel: -1 auto, 0 off, 1 / 2 forced (see hb_set_option)
   bool fused_measure = true;   // sc: the last sweep of hb_sweep also reduces M and E
   bool cache_valid = false;    // cached() holds the measurement of the current spins
@@ -132,6 +137,7 @@ struct hb_ctx {
   unsigned long long* counters() const { return reinterpret_cast<unsigned long long*>(ws + plan.off_counters); }
   float* staging() const { return reinterpret_cast<float*>(ws + plan.off_staging); }
   double* cached() const { return reinterpret_cast<double*>(ws + plan.off_counters + 64); }
+  unsigned long long* sweep_dev() const { return reinterpret_cast<unsigned long long*>(ws + plan.off_counters + 128); }
 };
 
 namespace {
@@ -162,6 +168,7 @@ SweepParams params(const hb_ctx* c, float beta) {
   p.J = c->J; p.K = c->K; p.ex = c->e[0]; p.ey = c->e[1]; p.ez = c->e[2]; p.beta = beta;
   p.seed_lo = (uint32_t)c->seed; p.seed_hi = (uint32_t)(c->seed >> 32);
   p.sweep_lo = (uint32_t)c->sweep; p.sweep_hi = (uint32_t)(c->sweep >> 32);
+  p.sweep_dev = nullptr;
   return p;
 }
 
@@ -267,6 +274,67 @@ int one_sweep(hb_ctx* c, float beta, Diag d, double* dev_out = nullptr) {
   }
   c->sweep += 1;
   c->attempts += (uint64_t)c->plan.n;
+  return HB_OK;
+}
+
+// ---- replayed launches ---------------------------------------------------------------------
+// Lattices whose colour pass is shorter than the gap between two kernel launches (c1, c2, most of c3 and c5) are
+// bound by the launch rate.  hb_sweep then replays a CUDA graph of kGraphSweeps sweeps; the Philox sweep counter of
+// a replayed launch is a device counter plus the sweep's index inside the graph (SweepParams::sweep_dev).
+constexpr int kGraphSweeps = 8;
+
+bool graph_wanted(const hb_ctx* c) {
+  if (c->graph_mode == 0 || coop_mode(c) != 0) return false;
+  return c->graph_mode == 1 || c->plan.n <= (int64_t(1) << 23);
+}
+
+int build_graph(hb_ctx* c, float beta) {
+  if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
+  if (!c->cap_stream) HB_CUDA(c, cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
+  cudaStream_t user = c->stream;
+  const uint64_t launches = c->launches;
+  HB_CUDA(c, cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
+  c->stream = c->cap_stream;            // the launch helpers enqueue on the context's stream
+  int rc = HB_OK;
+  SweepParams p = params(c, beta);
+  p.sweep_dev = c->sweep_dev();
+  p.sweep_hi = 0;
+  for (int u = 0; u < kGraphSweeps && rc == HB_OK; ++u) {
+    p.sweep_lo = (uint32_t)u;
+    for (int colour = 0; colour < c->n_colours && rc == HB_OK; ++colour) rc = one_colour(c, colour, p, Diag{nullptr, nullptr});
+  }
+  cudaError_t e = rc == HB_OK ? launch_set_counter(c->cap_stream, c->sweep_dev(), kGraphSweeps, true) : cudaSuccess;
+  c->stream = user;
+  c->launches = launches;
+  cudaGraph_t g = nullptr;
+  const cudaError_t e2 = cudaStreamEndCapture(c->cap_stream, &g);
+  if (rc != HB_OK) { if (g) cudaGraphDestroy(g); return rc; }
+  if (e == cudaSuccess) e = e2;
+  if (e == cudaSuccess) e = cudaGraphInstantiate(&c->gexec, g, 0);
+  if (g) cudaGraphDestroy(g);
+  if (e != cudaSuccess) { c->gexec = nullptr; return fail(c, HB_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e)); }
+  c->g_beta = beta;
+  c->g_dirty = false;
+  return HB_OK;
+}
+
+// as many whole graphs as fit in n_sweeps - 1 (the last sweep stays outside: it may carry the measurement); returns
+// the sweeps done through *done
+int graph_sweeps(hb_ctx* c, float beta, int64_t n_sweeps, int64_t* done) {
+  *done = 0;
+  const int64_t replays = (n_sweeps - 1) / kGraphSweeps;
+  if (replays < 1) return HB_OK;
+  if (!c->gexec || c->g_dirty || c->g_beta != beta) {
+    const int rc = build_graph(c, beta);
+    if (rc != HB_OK) return rc;
+  }
+  HB_CUDA(c, launch_set_counter(c->stream, c->sweep_dev(), c->sweep, false));
+  for (int64_t r = 0; r < replays; ++r) HB_CUDA(c, cudaGraphLaunch(c->gexec, c->stream));
+  const int64_t m = replays * kGraphSweeps;
+  c->launches += 1 + (uint64_t)replays * ((uint64_t)kGraphSweeps * c->n_colours + 1);
+  c->sweep += (uint64_t)m;
+  c->attempts += (uint64_t)m * (uint64_t)c->plan.n;
+  *done = m;
   return HB_OK;
 }
 
@@ -500,6 +568,8 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
 
 int hb_destroy(hb_ctx* c) {
   if (!c) return HB_OK;
+  if (c->gexec) cudaGraphExecDestroy(c->gexec);
+  if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
   if (c->own_spins && c->spins) cudaFree(c->spins);
   if (c->own_ws && c->ws) cudaFree(c->ws);
   delete c;
@@ -592,7 +662,12 @@ int hb_sweep(hb_ctx* c, float T, int64_t n_sweeps) {
     return rc;
   }
   const bool fuse = fused_blocks(c) > 0;
-  for (int64_t s = 0; s < n_sweeps; ++s) {
+  int64_t s = 0;
+  if (graph_wanted(c)) {
+    rc = graph_sweeps(c, beta, n_sweeps, &s);
+    if (rc != HB_OK) return rc;
+  }
+  for (; s < n_sweeps; ++s) {
     rc = one_sweep(c, beta, Diag{nullptr, nullptr}, (fuse && s == n_sweeps - 1) ? c->cached() : nullptr);
     if (rc != HB_OK) return rc;
   }
@@ -711,6 +786,12 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
   HB_CHECK_CTX(c);
   if (!name) return HB_EINVAL;
   const std::string s(name);
+  c->g_dirty = true;   // a cached graph was captured with the old settings
+  if (s == "graph") {
+    if (value < -1 || value > 1) return fail(c, HB_EINVAL, "graph: -1 auto, 0 off, 1 on");
+    c->graph_mode = (int)value;
+    return HB_OK;
+  }
   if (s == "sc_coop") {
     if (value < -1 || value > 2)
       return fail(c, HB_EINVAL, "sc_coop: -1 auto (one block when it fits), 0 off, 1 one block else cooperative grid, 2 cooperative grid");
@@ -781,6 +862,8 @@ int hb_get_option(hb_ctx* c, const char* name, int64_t* value) {
   if (s == "csr_block") *value = c->csr_block;
   else if (s == "fused_measure") *value = c->fused_measure ? 1 : 0;
   else if (s == "sc_coop") *value = c->sc_coop;
+  else if (s == "graph") *value = c->graph_mode;
+  else if (s == "graph_active") *value = graph_wanted(c) ? 1 : 0;
   else if (s == "coop_active") *value = coop_mode(c) != 0 ? 1 : 0;
   else if (s == "sc_v") *value = c->tile.V;
   else if (s == "sc_jx") *value = c->tile.JX;

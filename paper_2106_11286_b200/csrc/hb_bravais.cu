@@ -144,6 +144,7 @@ __device__ __forceinline__ void where_z(Where& w, const BrLayout& L, int32_t z) 
 template <int KIND, int B, int V, int ANISO, bool DIAG, bool MEAS = false>
 __global__ void __launch_bounds__(256, MEAS ? 1 : 3)
 k_sweep_bravais(float* __restrict__ own, const float* __restrict__ all, BrLayout L, ScTile t, SweepParams P, Diag d, Meas m) {
+  resolve_sweep(P);
   const int32_t tj = threadIdx.x % t.JX, ty = threadIdx.x / t.JX;
   const int32_t i0 = (blockIdx.x * t.JX + tj) * V;
   const int32_t y = blockIdx.y * t.TY + ty;

@@ -50,6 +50,7 @@ __device__ __forceinline__ void ell_field(const float4* __restrict__ S, const in
 template <int MD, bool DIAG>
 __global__ void __launch_bounds__(256)
 k_sweep_ell(float4* S, EllDev g, uint32_t begin, uint32_t count, SweepParams P, Diag d) {
+  resolve_sweep(P);
   const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= count) return;
   const uint32_t m = begin + t;

@@ -13,6 +13,9 @@ namespace hb {
 struct SweepParams {
   float J, K, ex, ey, ez, beta;
   uint32_t seed_lo, seed_hi, sweep_lo, sweep_hi;
+  // Replayed launches (CUDA graph) cannot carry the sweep counter in their parameters: with
+  // sweep_dev != nullptr the counter is *sweep_dev + sweep_lo (sweep_lo = index of the sweep inside the graph)
+  const unsigned long long* sweep_dev;
 };
 
 // simple cubic, colour-split storage
@@ -114,6 +117,8 @@ cudaError_t launch_measure_sc(cudaStream_t st, const float* spins, ScLayout L, i
 cudaError_t launch_measure_csr(cudaStream_t st, const float* spins, CsrDev g, SweepParams p, double* partials, double* out);
 cudaError_t launch_measure_bravais(cudaStream_t st, const float* spins, BrLayout L, int V, SweepParams p, double* partials, double* out);
 cudaError_t launch_reduce_final(cudaStream_t st, const double* partials, int n_blocks, double* out);
+// *counter = value (add == false) or *counter += value: the device-side sweep counter of replayed launches
+cudaError_t launch_set_counter(cudaStream_t st, unsigned long long* counter, unsigned long long value, bool add);
 
 // ---- host lattice tables (hb_lattice.cpp) -------------------------------------------------
 struct HostCsr {

@@ -231,6 +231,7 @@ __global__ void __launch_bounds__(BLK, (MEAS ? 3 : HB_SC_MINBLOCKS) * 256 / BLK)
 k_sweep_sc(float* __restrict__ ax, float* __restrict__ ay, float* __restrict__ az,
            const float* __restrict__ bx, const float* __restrict__ by, const float* __restrict__ bz,
            ScLayout L, ScTile t, SweepParams P, int colour, Diag d, Meas m) {
+  resolve_sweep(P);
   sc_pass<V, ANISO, DIAG, PF, MEAS, false>(ax, ay, az, bx, by, bz, L, t, P, colour, d, m, blockIdx, gridDim);
 }
 
@@ -239,6 +240,7 @@ template <bool DIAG>
 __global__ void __launch_bounds__(256)
 k_sweep_csr(float* sx, float* sy, float* sz, CsrDev g, uint32_t list_begin, uint32_t list_count,
             SweepParams P, Diag d) {
+  resolve_sweep(P);
   const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= list_count) return;
   const uint32_t i = (uint32_t)g.list[list_begin + t];
@@ -331,6 +333,10 @@ __device__ __forceinline__ void reduce_final_block(const double* partials, int n
     __syncthreads();
   }
   if (threadIdx.x < 4) out[threadIdx.x] = sh[threadIdx.x][0];
+}
+
+__global__ void k_set_counter(unsigned long long* counter, unsigned long long value, bool add) {
+  *counter = add ? *counter + value : value;
 }
 
 __global__ void __launch_bounds__(256) k_reduce_final(const double* partials, int n_blocks, double* out) {
@@ -601,6 +607,11 @@ cudaError_t launch_sweep_csr(cudaStream_t st, float* s, CsrDev g, uint32_t list_
     k_sweep_csr<true><<<grid, block, 0, st>>>(s, s + n, s + 2 * n, g, list_begin, list_count, p, d);
   else
     k_sweep_csr<false><<<grid, block, 0, st>>>(s, s + n, s + 2 * n, g, list_begin, list_count, p, d);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_set_counter(cudaStream_t st, unsigned long long* counter, unsigned long long value, bool add) {
+  k_set_counter<<<1, 1, 0, st>>>(counter, value, add);
   return cudaGetLastError();
 }
 

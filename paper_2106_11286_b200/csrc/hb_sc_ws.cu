@@ -212,6 +212,7 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
 template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS>
 __global__ void __launch_bounds__(32 + 32 * ((TY * (ROWB / 16) + 31) / 32) > 1024 ? 1024 : 32 + 32 * ((TY * (ROWB / 16) + 31) / 32), MINB)
 k_sweep_sc_ws(float* a, const float* b, ScLayout L, WsTiles w, SweepParams P, int colour, Meas m) {
+  resolve_sweep(P);
   using S = WsSmem<TY, ROWB, kNB, MINB>;
   extern __shared__ __align__(128) unsigned char smem[];
   const uint32_t sbase = smem_u32(smem);
