@@ -11,9 +11,9 @@
 //   * the CONSUMER warps wait on a "full" barrier, read everything with LDS at compile-time offsets (row
 //     pitch ROWB is a template constant, the periodic wrap in x is an index inside the staged row), release
 //     the slots through "empty" barriers, run the attempt arithmetic of hb_device.cuh; their own spins they
-//     load themselves one plane ahead (LDG.128) and store with STG.128 at the same addresses.  No block-wide
-//     barrier in the steady state;
-//   * CTAs are persistent (one or two per SM): a CTA walks its tiles (TY rows x ZT planes) with the rings running
+//     load themselves (LDG.128; one plane ahead in the variants that have the registers for it) and store
+//     with STG.128 at the same addresses.  No block-wide barrier in the steady state;
+//   * CTAs are persistent (one to three per SM): a CTA walks its tiles (TY rows x ZT planes) with the rings running
 //     across tile boundaries, so the pipeline is filled once per launch, not once per tile.
 //
 // Same arithmetic, same order of the neighbour sum, same bits as k_sweep_sc.
