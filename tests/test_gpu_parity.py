@@ -433,3 +433,35 @@ def test_replayed_launches_match_the_oracle():
         assert spins_equal(ctx.get_spins(), off.get_spins())
         ctx.close()
         off.close()
+
+
+def test_binder_crossing_brackets_the_critical_temperature_on_the_device():
+    # Physics of the CUDA path at sizes the oracle does not reach in seconds (paper: T_C/J = 1.445
+    # for the simple cubic lattice): the Binder cumulants U_L = 1 - <M^4> / (3 <M^2>^2) of L = 16
+    # and L = 32 (K = 0) cross at T_C up to small finite-size corrections; below it the larger lattice is the more
+    # ordered one, above it the less ordered one.
+    Ts = np.linspace(1.36, 1.52, 9)
+    U = {}
+    for L in (16, 32):
+        u = []
+        for T in Ts:
+            m2 = m4 = 0.0
+            reps = 4
+            for r in range(reps):
+                ctx = hb.Context(hb.Lattice("sc", L), 1.0, 0.0, (0.0, 0.0, 1.0), seed=500 + r)
+                ctx.init_aligned((0.0, 0.0, 1.0))
+                ctx.sweep(float(T), 1500)
+                M, _ = ctx.sweep_series(float(T), 6000)
+                q = np.sum(M * M, axis=1)
+                m2 += q.mean() / reps
+                m4 += (q * q).mean() / reps
+                ctx.close()
+            u.append(1.0 - m4 / (3.0 * m2 * m2))
+        U[L] = np.array(u)
+    d = U[32] - U[16]
+    print("T:", Ts, "U16:", U[16], "U32:", U[32])
+    assert d[0] > 0 and d[1] > 0 and d[-1] < 0 and d[-2] < 0          # ordered side / disordered side
+    k = int(np.argmax(d < 0))                                         # first temperature above the crossing
+    Tx = Ts[k - 1] + (Ts[k] - Ts[k - 1]) * d[k - 1] / (d[k - 1] - d[k])
+    print("Binder crossing of L = 16, 32 at T = %.4f" % Tx)
+    assert abs(Tx - 1.443) < 0.03
