@@ -465,3 +465,25 @@ def test_binder_crossing_brackets_the_critical_temperature_on_the_device():
     Tx = Ts[k - 1] + (Ts[k] - Ts[k - 1]) * d[k - 1] / (d[k - 1] - d[k])
     print("Binder crossing of L = 16, 32 at T = %.4f" % Tx)
     assert abs(Tx - 1.443) < 0.03
+
+
+@pytest.mark.parametrize("name", ["c2", "c3", "c5"])
+def test_full_protocol_scans(name):
+    # configs 2, 3, 5 exactly as BASELINE.json states them (full size, every temperature, every sweep), on the device:
+    # M(T) falls monotonically with T, is large on the cold side and small on the hot side, and the energy rises
+    # with T (full-size scans are sanity-checked for a monotone M(T) and the K8/K9 limits).
+    from paper_2106_11286_b200 import scan
+    cfg = W.CONFIGS[name]
+    ctx = scan.make_context(cfg)
+    res = scan.run_scan(ctx, cfg["T"], cfg["sweeps"], cfg.get("equil", 0))
+    order = np.argsort(res["T"])
+    T, m, e = res["T"][order], res["absM"][order], res["E"][order]
+    print(name, "T", T, "|M|", m, "E/N", e)
+    assert np.all(np.diff(m) < 0.01)                                  # monotone up to noise on the disordered side
+    assert np.all(np.diff(e) > 0)
+    cold, hot = {"c2": (0.85, 0.03), "c3": (0.65, 0.03), "c5": (0.30, 0.15)}[name]   # c5 starts random BELOW T_c (2.5 < 3.18): it coarsens, domains freeze in
+    assert m[0] > cold and m[-1] < hot
+    launches, attempts = ctx.counters()
+    per_T = cfg["sweeps"] + cfg.get("equil", 0)
+    assert attempts == ctx.n * per_T * len(cfg["T"])
+    ctx.close()
