@@ -93,7 +93,7 @@ def test_sc_tile_shapes_do_not_change_the_result():
     want = st.get_spins()
     for v, jx, ty, zt, coop in [(4, 5, 12, 10, 0), (4, 3, 5, 3, 0), (4, 1, 1, 1, 0), (2, 10, 7, 4, 0), (1, 20, 12, 2, 0),
                                 (4, 5, 51, 10, 0), (4, 5, 12, 10, 2), (4, 3, 5, 3, 2), (4, 2, 7, 4, 2), (4, 5, 51, 10, 2),
-                                (4, 5, 12, 10, 1)]:
+                                (4, 5, 12, 10, 1), (4, 5, 60, 10, 0), (4, 5, 200, 5, 0)]:   # the last two: 512- and 1024-thread blocks
         ctx = make_gpu(cfg)
         ctx.set_option("sc_coop", coop)
         ctx.set_option("sc_v", v)
@@ -297,6 +297,7 @@ def test_fused_measurement_equals_the_separate_pass():
     for cfg, opts in ((W.SMALL["c4"], {}), (W.SMALL["c1"], {}),
                       (dict(W.SMALL["c4"], L=(40, 12, 10), K=0.3, e=(0.6, 0.0, 0.8)), {"sc_jx": 3, "sc_ty": 5, "sc_zt": 3}),
                       (dict(W.SMALL["c4"], L=(64, 8, 6)), {"sc_linear": 96}),
+                      (dict(W.SMALL["c4"], L=(40, 12, 10)), {"sc_jx": 5, "sc_ty": 60}), (dict(W.SMALL["c4"], L=(40, 12, 10)), {"sc_jx": 5, "sc_ty": 200}),
                       # bcc / fcc: every colour charges its bonds to the lower colours (already final in the sweep)
                       (dict(W.SMALL["c2"], start="random"), {}), (dict(W.SMALL["c2"], L=(12, 5, 7), start="random"), {"sc_jx": 2, "sc_ty": 3, "sc_zt": 2}),
                       (dict(W.SMALL["c3"], L=8, start="random"), {}), (dict(W.SMALL["c3"], L=(8, 3, 5), start="random"), {"sc_jx": 1, "sc_ty": 2})):
