@@ -112,9 +112,9 @@ struct hb_ctx {
   int ws_zt = 32, n_sms = 148, ws_variant = 2;   // warp-specialised kernel: planes per tile, CTAs = n_sms x CTAs/SM
   int graph_mode = -1;         // replay hb_sweep's launches from a CUDA graph: -1 auto (lattices up to 2^23 sites), 0 off, 1 on
   cudaStream_t cap_stream = nullptr;
-  cudaGraphExec_t gexec = nullptr;
-  float g_beta = 0.0f;
-  bool g_dirty = true;
+  cudaGraphExec_t gexec[2] = {nullptr, nullptr};   // [0] plain sweeps, [1] every sweep measured into the series buffer
+  float g_beta[2] = {0.0f, 0.0f};
+  bool g_dirty[2] = {true, true};
   int sc_coop = -1;            // persistent multi-sweep kernel: -1 auto, 0 off, 1 / 2 forced (see hb_set_option)
   bool fused_measure = true;   // sc: the last sweep of hb_sweep also reduces M and E
   bool cache_valid = false;    // cached() holds the measurement of the current spins
@@ -138,6 +138,7 @@ struct hb_ctx {
   float* staging() const { return reinterpret_cast<float*>(ws + plan.off_staging); }
   double* cached() const { return reinterpret_cast<double*>(ws + plan.off_counters + 64); }
   unsigned long long* sweep_dev() const { return reinterpret_cast<unsigned long long*>(ws + plan.off_counters + 128); }
+  unsigned long long* series_idx() const { return reinterpret_cast<unsigned long long*>(ws + plan.off_counters + 136); }
 };
 
 namespace {
@@ -288,53 +289,59 @@ bool graph_wanted(const hb_ctx* c) {
   return c->graph_mode == 1 || c->plan.n <= (int64_t(1) << 23);
 }
 
-int build_graph(hb_ctx* c, float beta) {
-  if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
+int build_graph(hb_ctx* c, float beta, int meas) {
+  if (c->gexec[meas]) { cudaGraphExecDestroy(c->gexec[meas]); c->gexec[meas] = nullptr; }
   if (!c->cap_stream) HB_CUDA(c, cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
   cudaStream_t user = c->stream;
   const uint64_t launches = c->launches;
+  const int fb = meas ? fused_blocks(c) : 0;
   HB_CUDA(c, cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
   c->stream = c->cap_stream;            // the launch helpers enqueue on the context's stream
   int rc = HB_OK;
+  cudaError_t e = cudaSuccess;
   SweepParams p = params(c, beta);
   p.sweep_dev = c->sweep_dev();
   p.sweep_hi = 0;
-  for (int u = 0; u < kGraphSweeps && rc == HB_OK; ++u) {
+  for (int u = 0; u < kGraphSweeps && rc == HB_OK && e == cudaSuccess; ++u) {
     p.sweep_lo = (uint32_t)u;
-    for (int colour = 0; colour < c->n_colours && rc == HB_OK; ++colour) rc = one_colour(c, colour, p, Diag{nullptr, nullptr});
+    for (int colour = 0; colour < c->n_colours && rc == HB_OK; ++colour) {
+      Meas m{nullptr, 0};
+      if (fb) m = Meas{c->partials() + (size_t)colour * fb * 4,
+                       (c->plan.engine == ENGINE_BRAVAIS || colour == c->n_colours - 1) ? 2 : 1};
+      rc = one_colour(c, colour, p, Diag{nullptr, nullptr}, m);
+    }
+    if (fb && rc == HB_OK)
+      e = launch_reduce_final_series(c->cap_stream, c->partials(), c->n_colours * fb, c->series(), c->series_idx());
   }
-  cudaError_t e = rc == HB_OK ? launch_set_counter(c->cap_stream, c->sweep_dev(), kGraphSweeps, true) : cudaSuccess;
+  if (rc == HB_OK && e == cudaSuccess) e = launch_set_counter(c->cap_stream, c->sweep_dev(), kGraphSweeps, true);
   c->stream = user;
   c->launches = launches;
   cudaGraph_t g = nullptr;
   const cudaError_t e2 = cudaStreamEndCapture(c->cap_stream, &g);
   if (rc != HB_OK) { if (g) cudaGraphDestroy(g); return rc; }
   if (e == cudaSuccess) e = e2;
-  if (e == cudaSuccess) e = cudaGraphInstantiate(&c->gexec, g, 0);
+  if (e == cudaSuccess) e = cudaGraphInstantiate(&c->gexec[meas], g, 0);
   if (g) cudaGraphDestroy(g);
-  if (e != cudaSuccess) { c->gexec = nullptr; return fail(c, HB_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e)); }
-  c->g_beta = beta;
-  c->g_dirty = false;
+  if (e != cudaSuccess) { c->gexec[meas] = nullptr; return fail(c, HB_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e)); }
+  c->g_beta[meas] = beta;
+  c->g_dirty[meas] = false;
   return HB_OK;
 }
 
-// as many whole graphs as fit in n_sweeps - 1 (the last sweep stays outside: it may carry the measurement); returns
-// the sweeps done through *done
-int graph_sweeps(hb_ctx* c, float beta, int64_t n_sweeps, int64_t* done) {
-  *done = 0;
-  const int64_t replays = (n_sweeps - 1) / kGraphSweeps;
+// `replays` whole graphs: plain sweeps (meas = 0), or sweeps whose measurements fill the series buffer from entry 0
+int graph_sweeps(hb_ctx* c, float beta, int64_t replays, int meas) {
   if (replays < 1) return HB_OK;
-  if (!c->gexec || c->g_dirty || c->g_beta != beta) {
-    const int rc = build_graph(c, beta);
+  if (!c->gexec[meas] || c->g_dirty[meas] || c->g_beta[meas] != beta) {
+    const int rc = build_graph(c, beta, meas);
     if (rc != HB_OK) return rc;
   }
   HB_CUDA(c, launch_set_counter(c->stream, c->sweep_dev(), c->sweep, false));
-  for (int64_t r = 0; r < replays; ++r) HB_CUDA(c, cudaGraphLaunch(c->gexec, c->stream));
+  if (meas) HB_CUDA(c, launch_set_counter(c->stream, c->series_idx(), 0, false));
+  for (int64_t r = 0; r < replays; ++r) HB_CUDA(c, cudaGraphLaunch(c->gexec[meas], c->stream));
   const int64_t m = replays * kGraphSweeps;
-  c->launches += 1 + (uint64_t)replays * ((uint64_t)kGraphSweeps * c->n_colours + 1);
+  c->launches += 1 + (meas ? 1 : 0) + (uint64_t)replays * ((uint64_t)kGraphSweeps * (c->n_colours + (meas ? 1 : 0)) + 1);
   c->sweep += (uint64_t)m;
   c->attempts += (uint64_t)m * (uint64_t)c->plan.n;
-  *done = m;
   return HB_OK;
 }
 
@@ -568,7 +575,7 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
 
 int hb_destroy(hb_ctx* c) {
   if (!c) return HB_OK;
-  if (c->gexec) cudaGraphExecDestroy(c->gexec);
+  for (int k = 0; k < 2; ++k) if (c->gexec[k]) cudaGraphExecDestroy(c->gexec[k]);
   if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
   if (c->own_spins && c->spins) cudaFree(c->spins);
   if (c->own_ws && c->ws) cudaFree(c->ws);
@@ -663,9 +670,11 @@ int hb_sweep(hb_ctx* c, float T, int64_t n_sweeps) {
   }
   const bool fuse = fused_blocks(c) > 0;
   int64_t s = 0;
-  if (graph_wanted(c)) {
-    rc = graph_sweeps(c, beta, n_sweeps, &s);
+  if (graph_wanted(c)) {   // whole graphs of kGraphSweeps; the last sweep stays outside (it may carry the measurement)
+    const int64_t replays = (n_sweeps - 1) / kGraphSweeps;
+    rc = graph_sweeps(c, beta, replays, 0);
     if (rc != HB_OK) return rc;
+    s = replays * kGraphSweeps;
   }
   for (; s < n_sweeps; ++s) {
     rc = one_sweep(c, beta, Diag{nullptr, nullptr}, (fuse && s == n_sweeps - 1) ? c->cached() : nullptr);
@@ -709,14 +718,22 @@ int hb_sweep_series(hb_ctx* c, float T, int64_t n_sweeps, double* M_series, doub
     if (coop_mode(c) != 0) {
       rc = coop_sweeps(c, beta, m, c->series(), nullptr);
       if (rc != HB_OK) return rc;
-    } else
-    for (int64_t s = 0; s < m; ++s) {
+    } else {
+    int64_t s = 0;
+    if (fuse && graph_wanted(c)) {   // measured sweeps replayed: the reduction node writes entry 0, 1, 2, ... of the chunk
+      const int64_t replays = m / kGraphSweeps;
+      rc = graph_sweeps(c, beta, replays, 1);
+      if (rc != HB_OK) return rc;
+      s = replays * kGraphSweeps;
+    }
+    for (; s < m; ++s) {
       rc = one_sweep(c, beta, Diag{nullptr, nullptr}, fuse ? c->series() + 4 * s : nullptr);
       if (rc != HB_OK) return rc;
       if (!fuse) {
         rc = measure_into(c, c->series() + 4 * s);
         if (rc != HB_OK) return rc;
       }
+    }
     }
     HB_CUDA(c, cudaMemcpyAsync(h.data(), c->series(), (size_t)m * 32, cudaMemcpyDeviceToHost, c->stream));
     HB_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -786,7 +803,7 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
   HB_CHECK_CTX(c);
   if (!name) return HB_EINVAL;
   const std::string s(name);
-  c->g_dirty = true;   // a cached graph was captured with the old settings
+  c->g_dirty[0] = c->g_dirty[1] = true;   // the cached graphs were captured with the old settings
   if (s == "graph") {
     if (value < -1 || value > 1) return fail(c, HB_EINVAL, "graph: -1 auto, 0 off, 1 on");
     c->graph_mode = (int)value;

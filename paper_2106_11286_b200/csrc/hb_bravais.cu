@@ -126,6 +126,14 @@ __device__ __forceinline__ void field_low(const float* __restrict__ s, uint32_t 
   }
 }
 
+// how many of the Z neighbours of sublattice B sit on lower sublattices
+template <int KIND, int B>
+__host__ __device__ constexpr int n_low() {
+  int c = 0;
+  for (int k = 0; k < Geo<KIND>::Z; ++k) c += Geo<KIND>::nbr(B, k).nb < B ? 1 : 0;
+  return c;
+}
+
 __device__ __forceinline__ void where_y(Where& w, const BrLayout& L, int32_t y, int32_t i0, int V) {
   w.yo[0] = (uint32_t)((y == 0) ? L.Ly - 1 : y - 1) * (uint32_t)L.Lx;
   w.yo[1] = (uint32_t)y * (uint32_t)L.Lx;
@@ -142,7 +150,7 @@ __device__ __forceinline__ void where_z(Where& w, const BrLayout& L, int32_t z) 
 }
 
 template <int KIND, int B, int V, int ANISO, bool DIAG, bool MEAS = false>
-__global__ void __launch_bounds__(256, MEAS ? 1 : 3)
+__global__ void __launch_bounds__(256, (MEAS && n_low<KIND, B>() != 0 && n_low<KIND, B>() != Geo<KIND>::Z) ? 1 : (MEAS ? 2 : 3))
 k_sweep_bravais(float* __restrict__ own, const float* __restrict__ all, BrLayout L, ScTile t, SweepParams P, Diag d, Meas m) {
   resolve_sweep(P);
   const int32_t tj = threadIdx.x % t.JX, ty = threadIdx.x / t.JX;
@@ -200,7 +208,8 @@ k_sweep_bravais(float* __restrict__ own, const float* __restrict__ all, BrLayout
     }
     if (MEAS) {
       Vec<V> lx, ly, lz;
-      field_low<KIND, B, V>(all, L.nc, L.n, w, lx, ly, lz);
+      if constexpr (n_low<KIND, B>() == Geo<KIND>::Z) { lx = hx; ly = hy; lz = hz; }   // highest colour: the whole field
+      else field_low<KIND, B, V>(all, L.nc, L.n, w, lx, ly, lz);
       float gx = 0.0f, gy = 0.0f, gz = 0.0f, ge = 0.0f;
 #pragma unroll
       for (int k = 0; k < V; ++k) {

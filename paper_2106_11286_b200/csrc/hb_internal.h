@@ -117,6 +117,9 @@ cudaError_t launch_measure_sc(cudaStream_t st, const float* spins, ScLayout L, i
 cudaError_t launch_measure_csr(cudaStream_t st, const float* spins, CsrDev g, SweepParams p, double* partials, double* out);
 cudaError_t launch_measure_bravais(cudaStream_t st, const float* spins, BrLayout L, int V, SweepParams p, double* partials, double* out);
 cudaError_t launch_reduce_final(cudaStream_t st, const double* partials, int n_blocks, double* out);
+// replayed launches: (sum S, E) goes to entry *idx of series, then *idx advances by one
+cudaError_t launch_reduce_final_series(cudaStream_t st, const double* partials, int n_blocks, double* series,
+                                       unsigned long long* idx);
 // *counter = value (add == false) or *counter += value: the device-side sweep counter of replayed launches
 cudaError_t launch_set_counter(cudaStream_t st, unsigned long long* counter, unsigned long long value, bool add);
 

@@ -343,6 +343,15 @@ __global__ void __launch_bounds__(256) k_reduce_final(const double* partials, in
   reduce_final_block(partials, n_blocks, out);
 }
 
+// the same for replayed launches: entry *idx of a series (4 doubles per entry), then *idx advances
+__global__ void __launch_bounds__(256) k_reduce_final_series(const double* partials, int n_blocks, double* series,
+                                                             unsigned long long* idx) {
+  const unsigned long long i = *idx;
+  reduce_final_block(partials, n_blocks, series + 4 * i);
+  __syncthreads();
+  if (threadIdx.x == 0) *idx = i + 1;
+}
+
 // ---- persistent multi-sweep kernel for lattices whose colour pass is shorter than a kernel launch ----------
 // One cooperative launch runs n_sweeps sweeps: every block walks the virtual blocks of a colour pass, then the
 // whole grid meets at a barrier (cooperative groups) before the next colour.  Same arithmetic, same tiles, same
@@ -612,6 +621,12 @@ cudaError_t launch_sweep_csr(cudaStream_t st, float* s, CsrDev g, uint32_t list_
 
 cudaError_t launch_set_counter(cudaStream_t st, unsigned long long* counter, unsigned long long value, bool add) {
   k_set_counter<<<1, 1, 0, st>>>(counter, value, add);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_reduce_final_series(cudaStream_t st, const double* partials, int n_blocks, double* series,
+                                       unsigned long long* idx) {
+  k_reduce_final_series<<<1, 256, 0, st>>>(partials, n_blocks, series, idx);
   return cudaGetLastError();
 }
 

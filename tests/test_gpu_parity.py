@@ -424,6 +424,11 @@ def test_replayed_launches_match_the_oracle():
         st.sweep(0.7, 20)
         assert spins_equal(ctx.get_spins(), st.get_spins())
         assert ctx.sweep_count == st.sweep_count
+        # measured sweeps are replayed too where the measurement is fused (sc, bcc, fcc): 4 graphs + 5 single sweeps
+        Mg, Eg = ctx.sweep_series(1.2, 37)
+        Mo, Eo = st.series(1.2, 37)
+        assert spins_equal(ctx.get_spins(), st.get_spins())
+        assert np.max(np.abs(Mg - Mo)) <= 1e-7 and np.max(np.abs(Eg - Eo)) <= 1e-6 * lat.n
         off = make_gpu(cfg)                                          # and with the graph off: same trajectory
         off.set_option("graph", 0)
         off.set_option("sc_coop", 0)
