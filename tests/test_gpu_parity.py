@@ -493,3 +493,38 @@ def test_full_protocol_scans(name):
     per_T = cfg["sweeps"] + cfg.get("equil", 0)
     assert attempts == ctx.n * per_T * len(cfg["T"])
     ctx.close()
+
+
+def test_kernel_variants_agree_on_random_shapes():
+    # 30 seeded random simple cubic shapes (ragged tiles, single rows, wide rows): the direct kernel with a random tile,
+    # the warp-specialised kernel with random tile depth / CTA count / variant, replayed launches and the persistent
+    # kernels must all leave the same bits behind.  (The oracle pins the first of them in the tests above.)
+    rng = np.random.default_rng(20240611)
+    for it in range(30):
+        Lx = int(rng.choice([8, 16, 24, 40, 64, 120, 232, 512]))
+        Ly, Lz = int(2 * rng.integers(1, 12)), int(2 * rng.integers(1, 9))
+        K, e = (0.0, (0, 0, 1)) if it % 3 == 0 else ((0.05, (0, 0, 1)) if it % 3 == 1 else (0.2, (0.6, 0.0, 0.8)))
+        seed = int(rng.integers(1, 1 << 40))
+
+        def run(opts):
+            ctx = hb.Context(hb.Lattice("sc", Lx, Ly, Lz), 1.0, K, e, seed=seed)
+            for k, v in opts.items():
+                ctx.set_option(k, v)
+            ctx.init_random()
+            ctx.sweep(1.3, 11)
+            out = ctx.get_spins(), ctx.measure()
+            ctx.close()
+            return out
+
+        H = Lx // 2
+        ref, (Mr, Er) = run({"graph": 0, "sc_coop": 0})
+        variants = [{"graph": 0, "sc_coop": 0, "sc_jx": int(rng.integers(1, H // 4 + 1)), "sc_ty": int(rng.integers(1, 9)),
+                     "sc_zt": int(rng.integers(1, Lz + 1))},
+                    {"graph": 1, "sc_coop": 0},
+                    {"graph": 0, "sc_coop": 2},
+                    {"graph": int(rng.integers(0, 2)), "sc_kernel": 1, "sc_ws_zt": int(rng.integers(1, Lz + 1)),
+                     "sc_ws_ctas": int(rng.integers(1, 5)), "sc_ws_variant": int(rng.integers(0, 3))}]
+        for opts in variants:
+            got, (Mg, Eg) = run(opts)
+            assert spins_equal(got, ref), (Lx, Ly, Lz, opts)
+            assert np.max(np.abs(Mg - Mr)) <= 1e-7 and abs(Eg - Er) <= 1e-6 * Lx * Ly * Lz, (Lx, Ly, Lz, opts)
