@@ -107,11 +107,16 @@ int hb_get_spins(hb_ctx* ctx, float* sx, float* sy, float* sz);
 
 /* n_sweeps Metropolis sweeps at temperature T (units of J/k_B, T > 0, +inf allowed).
  * One sweep = one attempt at every site, colours in ascending order.  Asynchronous.
- * The sweep counter (the Philox counter words 2,3) advances by n_sweeps and is never reset. */
+ * The sweep counter (the Philox counter words 2,3) advances by n_sweeps and is never reset.
+ * How the launches are issued (one kernel per colour, a replayed CUDA graph of 8 sweeps on small
+ * lattices, one persistent block on tiny ones) does not change a bit of the result. */
 int hb_sweep(hb_ctx* ctx, float T, int64_t n_sweeps);
 
 /* M[3] = (1/N) sum_i S_i (eq. 2) and E = total energy of eq. 1 (each bond once), accumulated
- * in fp64 from fp32 per-site terms -0.5 J (S_i.h_i) - K_i (S_i.e_i)^2.  Synchronises. */
+ * in fp64 from fp32 per-site terms -0.5 J (S_i.h_i) - K_i (S_i.e_i)^2.  Synchronises.
+ * On the sc, bcc and fcc engines the last sweep of hb_sweep has already reduced both (each bond
+ * charged once, at its higher-colour end; same tolerances), so this call only copies 32 bytes;
+ * after hb_set_spins / hb_init_* / hb_sweep_record, and on neighbour tables, it runs one pass. */
 int hb_measure(hb_ctx* ctx, double M[3], double* E);
 
 /* n_sweeps sweeps with a measurement after each, results kept on the device until the end:
