@@ -73,6 +73,10 @@ typedef struct {
   /* any kind, optional per-site anisotropy (canonical order); NULL => the uniform (K, e) of hb_create */
   const float* K_site;     /* n entries */
   const float* e_site;     /* 3n entries, (ex,ey,ez) per site, unit vectors */
+  /* independent replicas of the lattice in one context (0 or 1: a single system).  Replica r is the system
+   * with Philox key seed + r; more than one needs a simple cubic lattice of at most 8192 sites with Lx a
+   * multiple of 8 and uniform anisotropy (each replica runs in one thread block, hb_sweep_each below). */
+  int32_t n_replicas;
 } hb_lattice;
 
 /* Caller-owned device memory (e.g. torch tensors).  Sizes from hb_sizes().  Both
@@ -126,6 +130,17 @@ int hb_sweep_series(hb_ctx* ctx, float T, int64_t n_sweeps, double* M_series, do
 /* Diagnostic: ONE sweep that also records every decision; accept[i] = 1 if the attempt at
  * canonical site i was accepted (host, n bytes).  Same arithmetic as hb_sweep.  Synchronises. */
 int hb_sweep_record(hb_ctx* ctx, float T, uint8_t* accept);
+
+/* Replicas (hb_lattice.n_replicas = R > 1): hb_init_*, hb_sweep, hb_sweep_count act on all replicas (hb_sweep at
+ * one temperature); the calls below give every replica its own temperature and return all measurements.
+ * T: R temperatures (host).  M: 3 doubles per replica; E: one per replica; series: replica-major, M_series[(r *
+ * n_sweeps + s) * 3 ..], E_series[r * n_sweeps + s].  One launch per call (per 1024 sweeps of a series): replica r
+ * runs in thread block r with everything resident in its SM.  hb_select_replica picks the replica that
+ * hb_get_spins / hb_set_spins / hb_measure address (default 0); hb_sweep_series and hb_sweep_record need R = 1. */
+int hb_sweep_each(hb_ctx* ctx, const float* T, int64_t n_sweeps);
+int hb_measure_each(hb_ctx* ctx, double* M, double* E);
+int hb_sweep_series_each(hb_ctx* ctx, const float* T, int64_t n_sweeps, double* M_series, double* E_series);
+int hb_select_replica(hb_ctx* ctx, int32_t replica);
 
 /* Checkpoint: (spins, sweep counter, seed, parameters) reproduce the trajectory bit for bit. */
 int hb_sweep_count(hb_ctx* ctx, uint64_t* out);

@@ -15,6 +15,7 @@ _KINDS = {"sc": HB_SC, "bcc": HB_BCC, "fcc": HB_FCC, "csr": HB_CSR}
 EXPORTS = [
     "hb_sizes", "hb_create", "hb_destroy", "hb_init_random", "hb_init_aligned", "hb_set_spins", "hb_get_spins",
     "hb_sweep", "hb_measure", "hb_sweep_series", "hb_sweep_record", "hb_sweep_count", "hb_set_sweep_count",
+    "hb_sweep_each", "hb_measure_each", "hb_sweep_series_each", "hb_select_replica",
     "hb_get_colouring", "hb_counters", "hb_set_option", "hb_get_option", "hb_lattice_fcc_sphere", "hb_lattice_free",
     "hb_strerror", "hb_error_detail",
 ]
@@ -23,7 +24,8 @@ EXPORTS = [
 class hb_lattice(C.Structure):
     _fields_ = [("kind", C.c_int32), ("Lx", C.c_int32), ("Ly", C.c_int32), ("Lz", C.c_int32),
                 ("n_sites", C.c_int64), ("row_ptr", C.c_void_p), ("col_idx", C.c_void_p),
-                ("n_colours", C.c_int32), ("colour", C.c_void_p), ("K_site", C.c_void_p), ("e_site", C.c_void_p)]
+                ("n_colours", C.c_int32), ("colour", C.c_void_p), ("K_site", C.c_void_p), ("e_site", C.c_void_p),
+                ("n_replicas", C.c_int32)]
 
 
 class hb_buffers(C.Structure):
@@ -67,6 +69,10 @@ def load_library():
         "hb_measure": [vp, P(C.c_double), P(C.c_double)],
         "hb_sweep_series": [vp, f32, i64, vp, vp],
         "hb_sweep_record": [vp, f32, vp],
+        "hb_sweep_each": [vp, vp, i64],
+        "hb_measure_each": [vp, vp, vp],
+        "hb_sweep_series_each": [vp, vp, i64, vp, vp],
+        "hb_select_replica": [vp, i32],
         "hb_sweep_count": [vp, P(u64)],
         "hb_set_sweep_count": [vp, u64],
         "hb_get_colouring": [vp, vp, P(i32)],
@@ -101,7 +107,7 @@ class Lattice:
     """Host description of a lattice (the hb_lattice struct plus the arrays it points to)."""
 
     def __init__(self, kind, Lx=0, Ly=0, Lz=0, row_ptr=None, col_idx=None, colour=None, n_colours=0,
-                 K_site=None, e_site=None, xyz=None):
+                 K_site=None, e_site=None, xyz=None, n_replicas=1):
         self.kind = _KINDS[kind] if isinstance(kind, str) else int(kind)
         self.Lx, self.Ly, self.Lz = int(Lx), int(Ly or Lx), int(Lz or Lx)
         self.row_ptr = _np(row_ptr, np.int64) if row_ptr is not None else None
@@ -111,6 +117,7 @@ class Lattice:
         self.K_site = _np(K_site, np.float32) if K_site is not None else None
         self.e_site = _np(e_site, np.float32) if e_site is not None else None
         self.xyz = xyz
+        self.n_replicas = int(n_replicas)
 
     @classmethod
     def fcc_sphere(cls, R, K_core=0.0, e_core=(0, 0, 1), K_surf=0.0, colouring="greedy"):
@@ -139,6 +146,7 @@ class Lattice:
     def struct(self):
         s = hb_lattice()
         s.kind, s.Lx, s.Ly, s.Lz = self.kind, self.Lx, self.Ly, self.Lz
+        s.n_replicas = self.n_replicas
         if self.row_ptr is not None:
             s.n_sites = self.row_ptr.size - 1
             s.row_ptr = _ptr(self.row_ptr)
@@ -172,7 +180,8 @@ class Context:
         self.lat = lat
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
-        self.n, spins_bytes, ws_bytes = sizes(lat)
+        self.n, spins_bytes, ws_bytes = sizes(lat)      # n: sites of ONE replica
+        self.n_replicas = max(1, lat.n_replicas)
         self._spins = torch.empty(spins_bytes, dtype=torch.uint8, device=self.device)
         self._ws = torch.empty(ws_bytes, dtype=torch.uint8, device=self.device)
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
@@ -239,6 +248,27 @@ class Context:
     def sweep_series(self, T, n_sweeps):
         M, E = np.zeros((n_sweeps, 3)), np.zeros(n_sweeps)
         self._check(self._L.hb_sweep_series(self._h, T, n_sweeps, _ptr(M), _ptr(E)), "hb_sweep_series")
+        return M, E
+
+    # ---- replicas (Lattice(..., n_replicas=R)): one launch runs all of them, each at its own temperature ----------
+    def select_replica(self, r):
+        self._check(self._L.hb_select_replica(self._h, int(r)), "hb_select_replica")
+
+    def sweep_each(self, T, n_sweeps=1):
+        t = _np(T, np.float32)
+        assert t.size == self.n_replicas
+        self._check(self._L.hb_sweep_each(self._h, _ptr(t), n_sweeps), "hb_sweep_each")
+
+    def measure_each(self):
+        M, E = np.zeros((self.n_replicas, 3)), np.zeros(self.n_replicas)
+        self._check(self._L.hb_measure_each(self._h, _ptr(M), _ptr(E)), "hb_measure_each")
+        return M, E
+
+    def sweep_series_each(self, T, n_sweeps):
+        t = _np(T, np.float32)
+        assert t.size == self.n_replicas
+        M, E = np.zeros((self.n_replicas, n_sweeps, 3)), np.zeros((self.n_replicas, n_sweeps))
+        self._check(self._L.hb_sweep_series_each(self._h, _ptr(t), n_sweeps, _ptr(M), _ptr(E)), "hb_sweep_series_each")
         return M, E
 
     def sweep_record(self, T):

@@ -25,6 +25,8 @@ struct Plan {                 // device memory plan of a lattice
   int64_t n = 0, nnz = 0;
   int engine = ENGINE_CSR;
   bool per_site = false;
+  int32_t R = 1;              // independent replicas (sc, one block per replica)
+  size_t off_each = 0, off_betas = 0;   // R > 1: per replica 16 doubles of partials + 4 of cached measurement; R betas
   bool ell = false;           // table engine: colour-major ELL layout (else plain CSR in canonical order)
   int32_t maxdeg = 0;
   size_t off_ell = 0, off_cbegin = 0;
@@ -69,12 +71,25 @@ int make_plan(const hb_lattice* lat, Plan& p, std::string& why) {
   p.per_site = lat->K_site != nullptr;
   // implicit indexing for the periodic kinds; the table engine for CSR input and per-site anisotropy
   p.engine = p.per_site || k == HB_CSR ? ENGINE_CSR : (k == HB_SC ? ENGINE_SC : ENGINE_BRAVAIS);
+  p.R = lat->n_replicas > 1 ? lat->n_replicas : 1;
+  if (p.R > 1) {
+    ScLayout sl{};
+    sl.Lx = lat->Lx; sl.Ly = lat->Ly; sl.Lz = lat->Lz; sl.H = lat->Lx / 2;
+    if (p.engine != ENGINE_SC || sc_one_block_threads(sl) == 0 || p.R > 4096) {
+      why = "replicas need a simple cubic lattice of at most 8192 sites with Lx a multiple of 8, uniform anisotropy, and at most 4096 replicas";
+      return HB_EINVAL;
+    }
+  }
   size_t o = 0;
   const size_t n_partials = kMeasureBlocks > 2 * kFusedBlocksMax ? kMeasureBlocks : 2 * kFusedBlocksMax;
   p.off_partials = o; o += align_up(n_partials * 4 * sizeof(double));
-  p.off_series = o;   o += align_up((size_t)kSeriesChunk * 4 * sizeof(double));
+  p.off_series = o;   o += align_up((size_t)p.R * kSeriesChunk * 4 * sizeof(double));
   p.off_counters = o; o += kAlign;
   p.off_staging = o;  o += align_up((size_t)p.n * sizeof(float));
+  if (p.R > 1) {
+    p.off_each = o;  o += align_up((size_t)p.R * 20 * sizeof(double));
+    p.off_betas = o; o += align_up((size_t)p.R * sizeof(float));
+  }
   if (p.engine == ENGINE_CSR) {
     // ELL when padding every row to the maximum degree costs little (regular lattices, cut-outs of them);
     // graphs with a few high-degree sites keep the plain CSR kernel
@@ -93,7 +108,7 @@ int make_plan(const hb_lattice* lat, Plan& p, std::string& why) {
     }
   }
   p.ws_bytes = o;
-  p.spins_bytes = align_up((p.ell ? 4 : 3) * (size_t)p.n * sizeof(float));   // ELL engine: AoS float4
+  p.spins_bytes = align_up((size_t)p.R * (p.ell ? 4 : 3) * (size_t)p.n * sizeof(float));   // ELL engine: AoS float4
   return HB_OK;
 }
 
@@ -125,7 +140,11 @@ struct hb_ctx {
   uint64_t seed = 0, sweep = 0;
   bool initialised = false;
   cudaStream_t stream = nullptr;
-  float* spins = nullptr;
+  float* spins = nullptr;        // state of the selected replica (the only one unless plan.R > 1)
+  float* spins_base = nullptr;   // state of replica 0
+  uint64_t seed_base = 0;
+  int32_t sel = 0;
+  bool each_valid = false;       // cached_each() holds the measurements of all replicas
   char* ws = nullptr;
   bool own_spins = false, own_ws = false;
   uint64_t launches = 0, attempts = 0;
@@ -136,6 +155,9 @@ struct hb_ctx {
   double* series() const { return reinterpret_cast<double*>(ws + plan.off_series); }
   unsigned long long* counters() const { return reinterpret_cast<unsigned long long*>(ws + plan.off_counters); }
   float* staging() const { return reinterpret_cast<float*>(ws + plan.off_staging); }
+  double* partials_each() const { return reinterpret_cast<double*>(ws + plan.off_each); }
+  double* cached_each() const { return reinterpret_cast<double*>(ws + plan.off_each) + (size_t)plan.R * 16; }
+  float* betas() const { return reinterpret_cast<float*>(ws + plan.off_betas); }
   double* cached() const { return reinterpret_cast<double*>(ws + plan.off_counters + 64); }
   unsigned long long* sweep_dev() const { return reinterpret_cast<unsigned long long*>(ws + plan.off_counters + 128); }
   unsigned long long* series_idx() const { return reinterpret_cast<unsigned long long*>(ws + plan.off_counters + 136); }
@@ -248,7 +270,7 @@ int coop_sweeps(hb_ctx* c, float beta, int64_t n_sweeps, double* series, double*
     const int m = (int)(n_sweeps - s0 < chunk ? n_sweeps - s0 : chunk);
     const bool last = s0 + m == n_sweeps;
     HB_CUDA(c, launch_sweeps_sc_coop(c->stream, c->spins, c->sc, c->tile, p, c->sweep, m, coop_mode(c) == 1, c->partials(),
-                                     series ? series + 4 * s0 : nullptr, last ? final_out : nullptr));
+                                     series ? series + 4 * s0 : nullptr, last ? final_out : nullptr, 1, nullptr, 0));
     c->launches += 1;
     c->sweep += (uint64_t)m;
     c->attempts += (uint64_t)m * (uint64_t)c->plan.n;
@@ -345,6 +367,31 @@ int graph_sweeps(hb_ctx* c, float beta, int64_t replays, int meas) {
   return HB_OK;
 }
 
+// ---- replicas (plan.R > 1): every replica in one thread block of one launch ------------------------------------
+void select_replica(hb_ctx* c, int32_t r) {
+  c->sel = r;
+  c->spins = c->spins_base + (size_t)r * 3 * (size_t)c->plan.n;
+  c->seed = c->seed_base + (uint64_t)r;
+}
+
+// n sweeps of all replicas at the temperatures beta[0..R) (host); series (device, R x kSeriesChunk x 4) or nullptr
+int replica_sweeps(hb_ctx* c, const float* beta, int64_t n_sweeps, double* series) {
+  HB_CUDA(c, cudaMemcpyAsync(c->betas(), beta, (size_t)c->plan.R * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+  SweepParams p = params(c, beta[0]);
+  p.seed_lo = (uint32_t)c->seed_base; p.seed_hi = (uint32_t)(c->seed_base >> 32);
+  const int64_t chunk = series ? kSeriesChunk : (int64_t(1) << 20);
+  for (int64_t s0 = 0; s0 < n_sweeps; s0 += chunk) {
+    const int m = (int)(n_sweeps - s0 < chunk ? n_sweeps - s0 : chunk);
+    HB_CUDA(c, launch_sweeps_sc_coop(c->stream, c->spins_base, c->sc, c->tile, p, c->sweep, m, true, c->partials_each(), series,
+                                     series ? nullptr : c->cached_each(), c->plan.R, c->betas(), (uint64_t)kSeriesChunk * 4));
+    c->launches += 1;
+    c->sweep += (uint64_t)m;
+    c->attempts += (uint64_t)m * (uint64_t)c->plan.n * (uint64_t)c->plan.R;
+    if (series) break;   // the caller copies a chunk out before the next one
+  }
+  return HB_OK;
+}
+
 int measure_into(hb_ctx* c, double* dev_out) {
   const SweepParams p = params(c, 0.0f);
   if (c->plan.engine == ENGINE_SC)
@@ -397,7 +444,7 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
   }
   c->kind = lat->kind; c->Lx = lat->Lx; c->Ly = lat->Ly; c->Lz = lat->Lz;
   c->J = J; c->K = K; c->e[0] = e[0]; c->e[1] = e[1]; c->e[2] = e[2];
-  c->seed = seed;
+  c->seed = c->seed_base = seed;
   const Plan& P = c->plan;
   if (P.per_site)
     for (int64_t i = 0; i < P.n; ++i)
@@ -484,7 +531,7 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
       c->sticky = HB_ENOMEM;
       return fail(c, HB_ENOMEM, "caller buffers are NULL, too small (see hb_sizes) or not 256-byte aligned");
     }
-    c->spins = static_cast<float*>(bufs->spins);
+    c->spins = c->spins_base = static_cast<float*>(bufs->spins);
     c->ws = static_cast<char*>(bufs->workspace);
     c->stream = static_cast<cudaStream_t>(bufs->cuda_stream);
   } else {
@@ -495,7 +542,7 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
       c->sticky = HB_ENOMEM;
       return fail(c, HB_ENOMEM, "cudaMalloc failed");
     }
-    c->spins = static_cast<float*>(a); c->ws = static_cast<char*>(b);
+    c->spins = c->spins_base = static_cast<float*>(a); c->ws = static_cast<char*>(b);
     c->own_spins = c->own_ws = true;
   }
   HB_CUDA(c, cudaMemsetAsync(c->ws + P.off_counters, 0, kAlign, c->stream));
@@ -577,7 +624,7 @@ int hb_destroy(hb_ctx* c) {
   if (!c) return HB_OK;
   for (int k = 0; k < 2; ++k) if (c->gexec[k]) cudaGraphExecDestroy(c->gexec[k]);
   if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
-  if (c->own_spins && c->spins) cudaFree(c->spins);
+  if (c->own_spins && c->spins_base) cudaFree(c->spins_base);
   if (c->own_ws && c->ws) cudaFree(c->ws);
   delete c;
   return HB_OK;
@@ -586,6 +633,16 @@ int hb_destroy(hb_ctx* c) {
 int hb_init_random(hb_ctx* c) {
   HB_CHECK_CTX(c);
   c->cache_valid = false;
+  c->each_valid = false;
+  if (c->plan.R > 1) {
+    for (int32_t r = 0; r < c->plan.R; ++r) {
+      const uint64_t sd = c->seed_base + (uint64_t)r;
+      HB_CUDA(c, launch_init_random_sc(c->stream, c->spins_base + (size_t)r * 3 * (size_t)c->plan.n, c->sc, (uint32_t)sd, (uint32_t)(sd >> 32)));
+    }
+    c->launches += (uint64_t)c->plan.R;
+    c->initialised = true;
+    return HB_OK;
+  }
   if (c->plan.engine == ENGINE_SC)
     HB_CUDA(c, launch_init_random_sc(c->stream, c->spins, c->sc, (uint32_t)c->seed, (uint32_t)(c->seed >> 32)));
   else if (c->plan.ell)
@@ -601,6 +658,14 @@ int hb_init_aligned(hb_ctx* c, const float dir[3]) {
   HB_CHECK_CTX(c);
   if (!dir || !unit_vector(dir)) return fail(c, HB_EINVAL, "dir must be a unit vector");
   c->cache_valid = false;
+  c->each_valid = false;
+  if (c->plan.R > 1) {
+    for (int32_t r = 0; r < c->plan.R; ++r)
+      HB_CUDA(c, launch_fill(c->stream, c->spins_base + (size_t)r * 3 * (size_t)c->plan.n, (uint32_t)c->plan.n, dir[0], dir[1], dir[2]));
+    c->launches += (uint64_t)c->plan.R;
+    c->initialised = true;
+    return HB_OK;
+  }
   if (c->plan.ell) HB_CUDA(c, launch_fill_ell(c->stream, c->spins, (uint32_t)c->plan.n, dir[0], dir[1], dir[2]));
   else HB_CUDA(c, launch_fill(c->stream, c->spins, (uint32_t)c->plan.n, dir[0], dir[1], dir[2]));
   c->launches += 1;
@@ -612,6 +677,7 @@ int hb_set_spins(hb_ctx* c, const float* sx, const float* sy, const float* sz) {
   HB_CHECK_CTX(c);
   c->cache_valid = false;
   if (!sx || !sy || !sz) return fail(c, HB_EINVAL, "NULL spin array");
+  c->each_valid = false;
   const size_t n = (size_t)c->plan.n;
   const float* src[3] = {sx, sy, sz};
   for (int k = 0; k < 3; ++k) {
@@ -663,6 +729,14 @@ int hb_sweep(hb_ctx* c, float T, int64_t n_sweeps) {
   int rc = check_T(c, T, &beta);
   if (rc != HB_OK) return rc;
   if (n_sweeps > 0) c->cache_valid = false;
+  if (c->plan.R > 1) {
+    if (n_sweeps == 0) return HB_OK;
+    const std::vector<float> b((size_t)c->plan.R, beta);
+    c->each_valid = false;
+    rc = replica_sweeps(c, b.data(), n_sweeps, nullptr);
+    if (rc == HB_OK) c->each_valid = true;
+    return rc;
+  }
   if (n_sweeps > 0 && coop_mode(c) != 0) {
     rc = coop_sweeps(c, beta, n_sweeps, nullptr, c->cached());
     if (rc == HB_OK) c->cache_valid = true;
@@ -688,6 +762,16 @@ int hb_measure(hb_ctx* c, double M[3], double* E) {
   HB_CHECK_CTX(c);
   if (!M || !E) return fail(c, HB_EINVAL, "NULL output");
   if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
+  if (c->plan.R > 1 && c->each_valid) {   // the replicas' last sweep left all measurements behind
+    double h[4];
+    HB_CUDA(c, cudaMemcpyAsync(h, c->cached_each() + 4 * (size_t)c->sel, sizeof h, cudaMemcpyDeviceToHost, c->stream));
+    HB_CUDA(c, cudaStreamSynchronize(c->stream));
+    const double inv = 1.0 / (double)c->plan.n;
+    M[0] = h[0] * inv; M[1] = h[1] * inv; M[2] = h[2] * inv;
+    *E = h[3];
+    return HB_OK;
+  }
+  if (c->plan.R > 1) c->cache_valid = false;   // the single slot may hold another replica's numbers
   if (!c->cache_valid) {
     const int rc = measure_into(c, c->cached());
     if (rc != HB_OK) return rc;
@@ -705,6 +789,7 @@ int hb_measure(hb_ctx* c, double M[3], double* E) {
 int hb_sweep_series(hb_ctx* c, float T, int64_t n_sweeps, double* M_series, double* E_series) {
   HB_CHECK_CTX(c);
   if (n_sweeps < 0 || !M_series || !E_series) return fail(c, HB_EINVAL, "bad series arguments");
+  if (c->plan.R > 1) return fail(c, HB_EINVAL, "a context with replicas takes hb_sweep_series_each");
   if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
   float beta;
   int rc = check_T(c, T, &beta);
@@ -750,6 +835,7 @@ int hb_sweep_series(hb_ctx* c, float T, int64_t n_sweeps, double* M_series, doub
 int hb_sweep_record(hb_ctx* c, float T, uint8_t* accept) {
   HB_CHECK_CTX(c);
   if (!accept) return fail(c, HB_EINVAL, "NULL accept array");
+  if (c->plan.R > 1) return fail(c, HB_EINVAL, "hb_sweep_record needs a context without replicas");
   if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
   float beta;
   int rc = check_T(c, T, &beta);
@@ -761,6 +847,93 @@ int hb_sweep_record(hb_ctx* c, float T, uint8_t* accept) {
   if (rc != HB_OK) return rc;
   HB_CUDA(c, cudaMemcpyAsync(accept, d_acc, (size_t)c->plan.n, cudaMemcpyDeviceToHost, c->stream));
   HB_CUDA(c, cudaStreamSynchronize(c->stream));
+  return HB_OK;
+}
+
+int hb_select_replica(hb_ctx* c, int32_t replica) {
+  HB_CHECK_CTX(c);
+  if (replica < 0 || replica >= c->plan.R) return fail(c, HB_EINVAL, "replica out of range");
+  select_replica(c, replica);
+  return HB_OK;
+}
+
+static int betas_of(hb_ctx* c, const float* T, std::vector<float>& beta) {
+  if (!T) return fail(c, HB_EINVAL, "NULL temperature array");
+  beta.resize((size_t)c->plan.R);
+  for (int32_t r = 0; r < c->plan.R; ++r) {
+    const int rc = check_T(c, T[r], &beta[r]);
+    if (rc != HB_OK) return rc;
+  }
+  return HB_OK;
+}
+
+int hb_sweep_each(hb_ctx* c, const float* T, int64_t n_sweeps) {
+  HB_CHECK_CTX(c);
+  if (n_sweeps < 0) return fail(c, HB_EINVAL, "n_sweeps < 0");
+  if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
+  std::vector<float> beta;
+  int rc = betas_of(c, T, beta);
+  if (rc != HB_OK) return rc;
+  if (c->plan.R == 1) return hb_sweep(c, T[0], n_sweeps);
+  if (n_sweeps == 0) return HB_OK;
+  c->cache_valid = c->each_valid = false;
+  rc = replica_sweeps(c, beta.data(), n_sweeps, nullptr);
+  if (rc == HB_OK) c->each_valid = true;
+  return rc;
+}
+
+int hb_measure_each(hb_ctx* c, double* M, double* E) {
+  HB_CHECK_CTX(c);
+  if (!M || !E) return fail(c, HB_EINVAL, "NULL output");
+  if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
+  if (c->plan.R == 1) return hb_measure(c, M, E);
+  if (!c->each_valid) {   // no sweep has just produced them: one pass per replica
+    const int32_t keep = c->sel;
+    for (int32_t r = 0; r < c->plan.R; ++r) {
+      select_replica(c, r);
+      const int rc = measure_into(c, c->cached_each() + 4 * (size_t)r);
+      if (rc != HB_OK) { select_replica(c, keep); return rc; }
+    }
+    select_replica(c, keep);
+    c->each_valid = true;
+  }
+  std::vector<double> h((size_t)c->plan.R * 4);
+  HB_CUDA(c, cudaMemcpyAsync(h.data(), c->cached_each(), h.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  HB_CUDA(c, cudaStreamSynchronize(c->stream));
+  const double inv = 1.0 / (double)c->plan.n;
+  for (int32_t r = 0; r < c->plan.R; ++r) {
+    M[3 * r] = h[4 * r] * inv; M[3 * r + 1] = h[4 * r + 1] * inv; M[3 * r + 2] = h[4 * r + 2] * inv;
+    E[r] = h[4 * r + 3];
+  }
+  return HB_OK;
+}
+
+int hb_sweep_series_each(hb_ctx* c, const float* T, int64_t n_sweeps, double* M_series, double* E_series) {
+  HB_CHECK_CTX(c);
+  if (n_sweeps < 0 || !M_series || !E_series) return fail(c, HB_EINVAL, "bad series arguments");
+  if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
+  std::vector<float> beta;
+  int rc = betas_of(c, T, beta);
+  if (rc != HB_OK) return rc;
+  if (c->plan.R == 1) return hb_sweep_series(c, T[0], n_sweeps, M_series, E_series);
+  if (n_sweeps > 0) c->cache_valid = c->each_valid = false;
+  const int32_t R = c->plan.R;
+  std::vector<double> h((size_t)R * kSeriesChunk * 4);
+  const double inv = 1.0 / (double)c->plan.n;
+  for (int64_t s0 = 0; s0 < n_sweeps; s0 += kSeriesChunk) {
+    const int64_t m = n_sweeps - s0 < kSeriesChunk ? n_sweeps - s0 : kSeriesChunk;
+    rc = replica_sweeps(c, beta.data(), m, c->series());
+    if (rc != HB_OK) return rc;
+    HB_CUDA(c, cudaMemcpyAsync(h.data(), c->series(), h.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    HB_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (int32_t r = 0; r < R; ++r)
+      for (int64_t s = 0; s < m; ++s) {
+        const double* q = h.data() + ((size_t)r * kSeriesChunk + (size_t)s) * 4;
+        double* Mo = M_series + ((size_t)r * (size_t)n_sweeps + (size_t)(s0 + s)) * 3;
+        Mo[0] = q[0] * inv; Mo[1] = q[1] * inv; Mo[2] = q[2] * inv;
+        E_series[(size_t)r * (size_t)n_sweeps + (size_t)(s0 + s)] = q[3];
+      }
+  }
   return HB_OK;
 }
 

@@ -94,8 +94,11 @@ int sc_fused_blocks(const ScLayout& L, const ScTile& t);
 // partials must hold 2 x 2 x blocks x 4 doubles; series (4 doubles per sweep) or final_out (4 doubles) may be null
 int sc_one_block_threads(const ScLayout& L);
 int sc_coop_blocks(const ScLayout& L, const ScTile& t);
+// one_block with n_replicas > 1: block r runs replica r (state at spins + 3 N r, key seed + r, beta betas[r] if betas,
+// partials + 16 r, series + series_stride r, final_out + 4 r)
 cudaError_t launch_sweeps_sc_coop(cudaStream_t st, float* spins, ScLayout L, ScTile t, SweepParams p, uint64_t sweep0, int n_sweeps,
-                                  bool one_block, double* partials, double* series, double* final_out);
+                                  bool one_block, double* partials, double* series, double* final_out,
+                                  int n_replicas, const float* betas, uint64_t series_stride);
 // warp-specialised persistent sc kernel (hb_sc_ws.cu): grid_cap = CTAs to launch at most (one per SM)
 bool sc_ws_supported(const ScLayout& L);
 int sc_ws_blocks(const ScLayout& L, int ZT, int grid_cap, int variant);

@@ -361,16 +361,28 @@ __global__ void __launch_bounds__(256) k_reduce_final_series(const double* parti
 // Block 0 sums the block partials of sweep s while the grid already runs colour 0 of sweep s+1, so the partials
 // are double-buffered by sweep parity (2 x 2 x total x 4 doubles).
 // ONE: the whole colour pass fits one block of up to 1024 threads (N <= 8192): a single block on a single SM, the
-// barrier is __syncthreads and the 12 N bytes of state stay in that SM's L1.
+// barrier is __syncthreads and the 12 N bytes of state stay in that SM's L1.  A grid of such blocks runs independent
+// REPLICAS of the lattice, one per block (state of replica r at s + 3 N r, Philox key seed + r, its own beta, its own
+// partials / series / final_out): many temperatures or seeds of a small lattice per launch.
 template <int ANISO, bool ONE>
 __global__ void __launch_bounds__(ONE ? 1024 : 256, ONE ? 1 : 3)
 k_sweeps_sc_coop(float* s, ScLayout L, ScTile t, SweepParams P, unsigned long long sweep0, int n_sweeps, uint3 nblk,
-                 double* partials, double* series, double* final_out) {
+                 double* partials, double* series, double* final_out, const float* betas, unsigned long long series_stride) {
   cooperative_groups::grid_group grid = cooperative_groups::this_grid();
   const size_t n = L.n;
   const uint32_t total = nblk.x * nblk.y * nblk.z;
   const Diag d{nullptr, nullptr};
-  if (ONE) t.LIN = -1;
+  if (ONE) {
+    t.LIN = -1;
+    const unsigned long long r = blockIdx.x;
+    const unsigned long long seed = (((unsigned long long)P.seed_hi << 32) | P.seed_lo) + r;
+    P.seed_lo = (uint32_t)seed; P.seed_hi = (uint32_t)(seed >> 32);
+    if (betas) P.beta = betas[r];
+    s += 3 * n * r;
+    partials += 16 * r;
+    if (series) series += series_stride * r;
+    if (final_out) final_out += 4 * r;
+  }
   for (int sw = 0; sw < n_sweeps; ++sw) {
     const unsigned long long sc = sweep0 + (unsigned long long)sw;
     P.sweep_lo = (uint32_t)sc; P.sweep_hi = (uint32_t)(sc >> 32);
@@ -379,7 +391,7 @@ k_sweeps_sc_coop(float* s, ScLayout L, ScTile t, SweepParams P, unsigned long lo
     for (int colour = 0; colour < 2; ++colour) {
       float* a = s + (size_t)colour * L.half;
       const float* b = s + (size_t)(1 - colour) * L.half;
-      for (uint32_t v = blockIdx.x; v < total; v += gridDim.x) {
+      for (uint32_t v = ONE ? 0u : blockIdx.x; v < total; v += ONE ? 1u : gridDim.x) {
         const uint3 bid = make_uint3(v % nblk.x, (v / nblk.x) % nblk.y, v / (nblk.x * nblk.y));
         if (meas) {
           const Meas mc{part + (size_t)colour * total * 4, colour == 1 ? 2 : 1};
@@ -390,8 +402,11 @@ k_sweeps_sc_coop(float* s, ScLayout L, ScTile t, SweepParams P, unsigned long lo
       }
       if (ONE) __syncthreads(); else grid.sync();
     }
-    if (meas && blockIdx.x == 0)
+    if (ONE) {   // two partials (one per colour), already behind the colour step's barrier: same sum, no tree
+      if (meas && threadIdx.x < 4) (series ? series + 4 * (size_t)sw : final_out)[threadIdx.x] = part[threadIdx.x] + part[4 + threadIdx.x];
+    } else if (meas && blockIdx.x == 0) {
       reduce_final_block(part, 2 * (int)total, series ? series + 4 * (size_t)sw : final_out);
+    }
   }
 }
 
@@ -571,22 +586,24 @@ int sc_coop_blocks(const ScLayout& L, const ScTile& t) {
 }
 
 cudaError_t launch_sweeps_sc_coop(cudaStream_t st, float* s, ScLayout L, ScTile t, SweepParams p, uint64_t sweep0, int n_sweeps,
-                                  bool one_block, double* partials, double* series, double* final_out) {
+                                  bool one_block, double* partials, double* series, double* final_out,
+                                  int n_replicas, const float* betas, uint64_t series_stride) {
   const int aniso = aniso_case(p);
   if (one_block) {
     const int threads = sc_one_block_threads(L);
-    if (!threads) return cudaErrorInvalidValue;
+    if (!threads || n_replicas < 1) return cudaErrorInvalidValue;
     const uint3 nblk = make_uint3(1, 1, 1);
+    const unsigned long long stride = series_stride;
     switch (aniso) {
-      case ANISO_NONE: k_sweeps_sc_coop<ANISO_NONE, true><<<1, threads, 0, st>>>(s, L, t, p, sweep0, n_sweeps, nblk, partials, series, final_out); break;
-      case ANISO_Z: k_sweeps_sc_coop<ANISO_Z, true><<<1, threads, 0, st>>>(s, L, t, p, sweep0, n_sweeps, nblk, partials, series, final_out); break;
-      default: k_sweeps_sc_coop<ANISO_GENERAL, true><<<1, threads, 0, st>>>(s, L, t, p, sweep0, n_sweeps, nblk, partials, series, final_out); break;
+      case ANISO_NONE: k_sweeps_sc_coop<ANISO_NONE, true><<<n_replicas, threads, 0, st>>>(s, L, t, p, sweep0, n_sweeps, nblk, partials, series, final_out, betas, stride); break;
+      case ANISO_Z: k_sweeps_sc_coop<ANISO_Z, true><<<n_replicas, threads, 0, st>>>(s, L, t, p, sweep0, n_sweeps, nblk, partials, series, final_out, betas, stride); break;
+      default: k_sweeps_sc_coop<ANISO_GENERAL, true><<<n_replicas, threads, 0, st>>>(s, L, t, p, sweep0, n_sweeps, nblk, partials, series, final_out, betas, stride); break;
     }
     return cudaGetLastError();
   }
   dim3 vgrid; int threads;
   sc_launch_shape(L, t, 4, vgrid, threads);
-  void (*kern)(float*, ScLayout, ScTile, SweepParams, unsigned long long, int, uint3, double*, double*, double*);
+  void (*kern)(float*, ScLayout, ScTile, SweepParams, unsigned long long, int, uint3, double*, double*, double*, const float*, unsigned long long);
   switch (aniso) {
     case ANISO_NONE: kern = k_sweeps_sc_coop<ANISO_NONE, false>; break;
     case ANISO_Z: kern = k_sweeps_sc_coop<ANISO_Z, false>; break;
@@ -603,7 +620,9 @@ cudaError_t launch_sweeps_sc_coop(cudaStream_t st, float* s, ScLayout L, ScTile 
   const unsigned grid = (unsigned)(total < resident ? total : resident);
   uint3 nblk = make_uint3(vgrid.x, vgrid.y, vgrid.z);
   unsigned long long s0 = sweep0;
-  void* args[] = {&s, &L, &t, &p, &s0, &n_sweeps, &nblk, &partials, &series, &final_out};
+  const float* no_betas = nullptr;
+  unsigned long long no_stride = 0;
+  void* args[] = {&s, &L, &t, &p, &s0, &n_sweeps, &nblk, &partials, &series, &final_out, &no_betas, &no_stride};
   return cudaLaunchCooperativeKernel((const void*)kern, dim3(grid), dim3(threads), args, 0, st);
 }
 

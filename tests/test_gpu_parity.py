@@ -528,3 +528,59 @@ def test_kernel_variants_agree_on_random_shapes():
             got, (Mg, Eg) = run(opts)
             assert spins_equal(got, ref), (Lx, Ly, Lz, opts)
             assert np.max(np.abs(Mg - Mr)) <= 1e-7 and abs(Eg - Er) <= 1e-6 * Lx * Ly * Lz, (Lx, Ly, Lz, opts)
+
+
+def test_replicas_match_independent_oracle_runs():
+    # hb_lattice.n_replicas = R: replica r is the system with seed + r; one launch sweeps all of them, each in its own
+    # thread block at its own temperature.  Every replica must walk the trajectory the oracle walks
+    # for (seed + r, T_r), and its measurements and series must be the oracle's.
+    for cfg, R in ((W.SMALL["c1"], 5), (dict(W.SMALL["c4"], L=(8, 6, 4), K=0.3, e=(0.6, 0.0, 0.8)), 37),
+                   (dict(W.SMALL["c4"], L=(16, 16, 32)), 3)):
+        L = cfg["L"]
+        Lx, Ly, Lz = (L, L, L) if isinstance(L, int) else L
+        ctx = hb.Context(hb.Lattice("sc", Lx, Ly, Lz, n_replicas=R), cfg["J"], cfg["K"], cfg["e"], cfg["seed"])
+        Ts = np.linspace(0.6, 2.4, R).astype(np.float32)
+        states = []
+        for r in range(R):
+            lat, st = make_oracle(dict(cfg, seed=cfg["seed"] + r))
+            st.init_random()
+            states.append(st)
+        ctx.init_random()
+        l0, _ = ctx.counters()
+        ctx.sweep_each(Ts, 7)
+        l1, a1 = ctx.counters()
+        assert l1 - l0 == 1 and a1 == 7 * lat.n * R                   # one launch for all replicas
+        for r, st in enumerate(states):
+            st.sweep(float(Ts[r]), 7)
+        M, E = ctx.measure_each()                                     # reduced inside that launch
+        for r, st in enumerate(states):
+            Mo, Eo32, Eo64 = st.measure()
+            assert np.max(np.abs(M[r] - Mo)) <= 1e-7 and abs(E[r] - Eo32) <= 1e-6 * lat.n
+            ctx.select_replica(r)
+            assert spins_equal(ctx.get_spins(), st.get_spins()), (cfg["L"], r)
+            Ms, Es = ctx.measure()
+            assert np.max(np.abs(Ms - Mo)) <= 1e-7 and abs(Es - Eo32) <= 1e-6 * lat.n
+        Mser, Eser = ctx.sweep_series_each(Ts, 9)
+        ctx.sweep(1.1, 2)                                             # one temperature for all
+        for r, st in enumerate(states):
+            Mo, Eo = st.series(float(Ts[r]), 9)
+            assert np.max(np.abs(Mser[r] - Mo)) <= 1e-7 and np.max(np.abs(Eser[r] - Eo)) <= 1e-6 * lat.n
+            st.sweep(1.1, 2)
+            ctx.select_replica(r)
+            assert spins_equal(ctx.get_spins(), st.get_spins())
+        # a replica's state can be replaced; measuring then takes the separate pass
+        S = W.random_unit_vectors(lat.n, 5)
+        ctx.select_replica(1)
+        ctx.set_spins(S[:, 0], S[:, 1], S[:, 2])
+        states[1].set_spins(S[:, 0], S[:, 1], S[:, 2])
+        M, E = ctx.measure_each()
+        for r in (0, 1, R - 1):
+            Mo, Eo32, _ = states[r].measure()
+            assert np.max(np.abs(M[r] - Mo)) <= 1e-7 and abs(E[r] - Eo32) <= 1e-6 * lat.n
+        with pytest.raises(hb.HbError):
+            ctx.sweep_record(1.0)
+        ctx.close()
+    with pytest.raises(hb.HbError):
+        hb.Context(hb.Lattice("sc", 32, n_replicas=2))                # 32768 sites: a colour pass does not fit one block
+    with pytest.raises(hb.HbError):
+        hb.Context(hb.Lattice("bcc", 4, n_replicas=2))
