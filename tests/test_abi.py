@@ -87,6 +87,27 @@ def test_sizes_rejects_bad_lattices():
         hb.sizes(hb.Lattice("fcc", 1100))
 
 
+def test_memory_plan_of_table_engines_and_replicas():
+    # host logic of hb_sizes: neighbour tables of near-uniform degree take the colour-major ELL layout with AoS float4
+    # spins (16 B per site), irregular graphs the plain CSR layout (12 B per site); replicas multiply the state
+    from paper_2106_11286_b200 import workloads as W
+    sph = hb.Lattice.fcc_sphere(5, 0.05, (0, 0, 1), 0.5)
+    n, spins_bytes, _ = hb.sizes(sph)
+    assert n == 2123 and spins_bytes == -(-16 * n // 256) * 256
+    rp, ci = W.random_csr_graph(5000, 7.0, seed=3)
+    n, spins_bytes, _ = hb.sizes(hb.Lattice("csr", row_ptr=rp, col_idx=ci))
+    assert n == 5000 and spins_bytes == -(-12 * n // 256) * 256
+    per_site = hb.Lattice("bcc", 4, K_site=np.zeros(128, np.float32), e_site=np.tile(np.float32([0, 0, 1]), (128, 1)))
+    assert hb.sizes(per_site)[1] == -(-16 * 128 // 256) * 256           # regular degree 8: ELL
+    n, one, ws1 = hb.sizes(hb.Lattice("sc", 16))
+    n_r, many, ws37 = hb.sizes(hb.Lattice("sc", 16, n_replicas=37))
+    assert n_r == n == 4096 and many == 37 * one and ws37 > ws1         # n_sites is per replica
+    for bad in (hb.Lattice("sc", 32, n_replicas=2), hb.Lattice("bcc", 4, n_replicas=2), hb.Lattice("sc", 12, n_replicas=2),
+                hb.Lattice("sc", 8, n_replicas=5000)):
+        with pytest.raises(hb.HbError):
+            hb.sizes(bad)
+
+
 def test_sphere_builder_matches_the_oracles_independent_builder():
     """Host logic of rows a1/a2: the library's fcc-sphere table, anisotropy classes and greedy
     colouring against the oracle's own construction (the two share no code)."""
