@@ -124,7 +124,7 @@ struct hb_ctx {
   EllDev ell{};
   int csr_block = 128;
   int sc_kernel = 0;      // 0: direct loads through L1, 1: warp-specialised persistent kernel (TMA-staged neighbour planes)
-  int ws_zt = 32, n_sms = 148, ws_variant = 2;   // warp-specialised kernel: planes per tile, CTAs = n_sms x CTAs/SM
+  int ws_zt = 0, n_sms = 148, ws_variant = 2;   // warp-specialised kernel: planes per tile (0: balanced automatically), CTAs = n_sms x CTAs/SM
   int graph_mode = -1;         // replay hb_sweep's launches from a CUDA graph: -1 auto (lattices up to 2^23 sites), 0 off, 1 on
   cudaStream_t cap_stream = nullptr;
   cudaGraphExec_t gexec[2] = {nullptr, nullptr};   // [0] plain sweeps, [1] every sweep measured into the series buffer
@@ -1010,12 +1010,14 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
     return HB_OK;
   }
   if (s == "sc_ws_zt") {
-    if (value < 1 || value > c->sc.Lz) return fail(c, HB_EINVAL, "sc_ws_zt: 1..Lz");
+    if (value < 0 || value > c->sc.Lz) return fail(c, HB_EINVAL, "sc_ws_zt: 1..Lz, or 0 = balanced over the persistent CTAs");
     c->ws_zt = (int)value;
     return HB_OK;
   }
   if (s == "sc_ws_variant") {
-    if (value < 0 || value > 2) return fail(c, HB_EINVAL, "sc_ws_variant: 0 (4-row tiles, 2 CTAs per SM), 1 (8-row tiles, 1 CTA per SM), 2 (4-row tiles, 3 CTAs per SM)");
+    if (!sc_ws_variant_supported(c->sc, (int)value))
+      return fail(c, HB_EINVAL, "sc_ws_variant: 0 (4-row tiles, 2 CTAs per SM), 1 (8-row tiles, 1 CTA per SM), 2 (4-row tiles, 3 CTAs per SM), "
+                                "3 (16-row tiles, 1 CTA per SM; rows of up to 248 floats)");
     c->ws_variant = (int)value;
     return HB_OK;
   }

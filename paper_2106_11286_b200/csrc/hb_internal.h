@@ -101,6 +101,7 @@ cudaError_t launch_sweeps_sc_coop(cudaStream_t st, float* spins, ScLayout L, ScT
                                   int n_replicas, const float* betas, uint64_t series_stride);
 // warp-specialised persistent sc kernel (hb_sc_ws.cu): grid_cap = CTAs to launch at most (one per SM)
 bool sc_ws_supported(const ScLayout& L);
+bool sc_ws_variant_supported(const ScLayout& L, int variant);
 int sc_ws_blocks(const ScLayout& L, int ZT, int grid_cap, int variant);
 cudaError_t launch_sweep_sc_ws(cudaStream_t st, float* spins, ScLayout L, int ZT, int grid_cap, int variant, SweepParams p, int colour, Meas m);
 cudaError_t launch_sweep_csr(cudaStream_t st, float* spins, CsrDev g, uint32_t list_begin, uint32_t list_count,

@@ -33,7 +33,7 @@ struct RingPos {
 };
 
 struct WsTiles {
-  int32_t n_ty, n_zc, ZT;   // tiles in y, chunks in z, planes per chunk
+  int32_t n_ty, n_zc;   // tiles in y, chunks in z: chunk zc = planes [zc Lz / n_zc, (zc+1) Lz / n_zc), sizes differ by at most one
 };
 
 // kNB plane slots of the other colour (z-1, z, z+1 and look-ahead); MINB = CTAs per SM the kernel is built for
@@ -59,7 +59,7 @@ __device__ __forceinline__ void ws_producer(const float* b, const ScLayout& L, c
   for (int32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
     const int32_t ty = tile % w.n_ty, zc = tile / w.n_ty;
     const int32_t y0 = ty * TY, ny = min(TY, L.Ly - y0);
-    const int32_t z0 = zc * w.ZT, nz = min(w.ZT, L.Lz - z0);
+    const int32_t z0 = (int32_t)(((int64_t)zc * L.Lz) / w.n_zc), nz = (int32_t)(((int64_t)(zc + 1) * L.Lz) / w.n_zc) - z0;
     for (int32_t k = 0; k < nz + 2; ++k) {
       {  // B plane k
         int32_t zz = z0 - 1 + k;
@@ -105,7 +105,7 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
   for (int32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
     const int32_t ty = tile % w.n_ty, zc = tile / w.n_ty;
     const int32_t y0 = ty * TY, ny = min(TY, L.Ly - y0);
-    const int32_t z0 = zc * w.ZT, nz = min(w.ZT, L.Lz - z0);
+    const int32_t z0 = (int32_t)(((int64_t)zc * L.Lz) / w.n_zc), nz = (int32_t)(((int64_t)(zc + 1) * L.Lz) / w.n_zc) - z0;
     const bool active = r < ny;
     const int32_t y = y0 + r;
     float* gx = a + ((size_t)z0 * L.Ly + y) * L.H + i0;            // own spins of plane z0 (x component)
@@ -230,7 +230,7 @@ k_sweep_sc_ws(float* a, const float* b, ScLayout L, WsTiles w, SweepParams P, in
 }
 
 template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS>
-cudaError_t ws_go(cudaStream_t st, float* s, const ScLayout& L, int ZT, int grid_cap, const SweepParams& p, int colour, const Meas& m) {
+cudaError_t ws_go(cudaStream_t st, float* s, const ScLayout& L, int n_zc, int grid_cap, const SweepParams& p, int colour, const Meas& m) {
   using S = WsSmem<TY, ROWB, kNB, MINB>;
   auto kern = k_sweep_sc_ws<TY, ROWB, kNB, MINB, ANISO, MEAS>;
   static bool configured = false;
@@ -240,9 +240,8 @@ cudaError_t ws_go(cudaStream_t st, float* s, const ScLayout& L, int ZT, int grid
     configured = true;
   }
   WsTiles w;
-  w.ZT = ZT;
   w.n_ty = (L.Ly + TY - 1) / TY;
-  w.n_zc = (L.Lz + ZT - 1) / ZT;
+  w.n_zc = n_zc;
   const int n_tiles = w.n_ty * w.n_zc;
   const int grid = n_tiles < grid_cap ? n_tiles : grid_cap;
   const int threads = 32 + 32 * ((TY * (L.H / 4) + 31) / 32);
@@ -253,19 +252,19 @@ cudaError_t ws_go(cudaStream_t st, float* s, const ScLayout& L, int ZT, int grid
 }
 
 template <int TY, int ROWB, int kNB, int MINB>
-cudaError_t ws_pick(cudaStream_t st, float* s, const ScLayout& L, int ZT, int grid_cap, const SweepParams& p, int colour, const Meas& m) {
+cudaError_t ws_pick(cudaStream_t st, float* s, const ScLayout& L, int n_zc, int grid_cap, const SweepParams& p, int colour, const Meas& m) {
   const int aniso = (p.K == 0.0f) ? ANISO_NONE : ((p.ex == 0.0f && p.ey == 0.0f && p.ez == 1.0f) ? ANISO_Z : ANISO_GENERAL);
   if (m.mode != 0) {
     switch (aniso) {
-      case ANISO_NONE: return ws_go<TY, ROWB, kNB, MINB, ANISO_NONE, true>(st, s, L, ZT, grid_cap, p, colour, m);
-      case ANISO_Z: return ws_go<TY, ROWB, kNB, MINB, ANISO_Z, true>(st, s, L, ZT, grid_cap, p, colour, m);
-      default: return ws_go<TY, ROWB, kNB, MINB, ANISO_GENERAL, true>(st, s, L, ZT, grid_cap, p, colour, m);
+      case ANISO_NONE: return ws_go<TY, ROWB, kNB, MINB, ANISO_NONE, true>(st, s, L, n_zc, grid_cap, p, colour, m);
+      case ANISO_Z: return ws_go<TY, ROWB, kNB, MINB, ANISO_Z, true>(st, s, L, n_zc, grid_cap, p, colour, m);
+      default: return ws_go<TY, ROWB, kNB, MINB, ANISO_GENERAL, true>(st, s, L, n_zc, grid_cap, p, colour, m);
     }
   }
   switch (aniso) {
-    case ANISO_NONE: return ws_go<TY, ROWB, kNB, MINB, ANISO_NONE, false>(st, s, L, ZT, grid_cap, p, colour, m);
-    case ANISO_Z: return ws_go<TY, ROWB, kNB, MINB, ANISO_Z, false>(st, s, L, ZT, grid_cap, p, colour, m);
-    default: return ws_go<TY, ROWB, kNB, MINB, ANISO_GENERAL, false>(st, s, L, ZT, grid_cap, p, colour, m);
+    case ANISO_NONE: return ws_go<TY, ROWB, kNB, MINB, ANISO_NONE, false>(st, s, L, n_zc, grid_cap, p, colour, m);
+    case ANISO_Z: return ws_go<TY, ROWB, kNB, MINB, ANISO_Z, false>(st, s, L, n_zc, grid_cap, p, colour, m);
+    default: return ws_go<TY, ROWB, kNB, MINB, ANISO_GENERAL, false>(st, s, L, n_zc, grid_cap, p, colour, m);
   }
 }
 
@@ -275,26 +274,51 @@ cudaError_t ws_pick(cudaStream_t st, float* s, const ScLayout& L, int ZT, int gr
 bool sc_ws_supported(const ScLayout& L) { return L.H % 4 == 0 && L.H <= 256; }
 
 // variants (option sc_ws_variant), sustained rate on c4 (sc L = 464) beside the direct kernel's 116.8 Gupd/s:
-//   2 = 4-row tiles, 4 plane slots, 3 CTAs per SM, 72 registers, own spins loaded at the top of the step   120.9  (default)
+//   2 = 4-row tiles, 4 plane slots, 3 CTAs per SM, 72 registers, own spins loaded at the top of the step   120.9
 //   0 = 4-row tiles, 5 plane slots, 2 CTAs per SM, 96 registers, own spins loaded one plane ahead          116.9
 //   1 = 8-row tiles, 6 plane slots, 1 CTA per SM                                                            117.4
+//   3 = 16-row tiles, 4 plane slots (216 KB), 1 CTA per SM of up to 31 consumer warps, 64 registers: for rows of up to
+//       248 floats; with 232-float rows (c4) the 928 consumer threads are exactly 29 full warps
 // (11-row tiles, whose 638 consumer threads fill 99.7 % of their warps' lanes, 1 CTA per SM: 111-113)
-static int ws_ty(int variant) { return variant == 1 ? 8 : 4; }
-static int ws_ctas_per_sm(int variant) { return variant == 1 ? 1 : (variant == 2 ? 3 : 2); }
+static int ws_ty(int variant) { return variant == 1 ? 8 : (variant == 3 ? 16 : 4); }
+static int ws_ctas_per_sm(int variant) { return (variant == 1 || variant == 3) ? 1 : (variant == 2 ? 3 : 2); }
+
+bool sc_ws_variant_supported(const ScLayout& L, int variant) {
+  if (variant < 0 || variant > 3 || !sc_ws_supported(L)) return false;
+  return variant != 3 || 16 * (L.H / 4) <= 992;   // 1024 threads less the producer warp
+}
+
+// Chunks in z of one launch.  ZT > 0: chunks of at most ZT planes.  ZT = 0: the count that minimises the longest
+// walk of a CTA, rounds x (planes per chunk + 2): tiles are dealt round-robin to the persistent CTAs, a tile costs its
+// planes plus the two extra planes the producer stages for it.
+int sc_ws_chunks(const ScLayout& L, int ZT, int grid_cap, int variant) {
+  if (ZT > 0) return (L.Lz + ZT - 1) / ZT;
+  const int ty = ws_ty(variant);
+  const long long n_ty = (L.Ly + ty - 1) / ty, cap = (long long)grid_cap * ws_ctas_per_sm(variant);
+  long long best = -1; int best_n = 1;
+  const int n_max = L.Lz < 4096 ? L.Lz : 4096;
+  for (int n = 1; n <= n_max; ++n) {
+    const long long tiles = n_ty * n, rounds = (tiles + cap - 1) / cap, cost = rounds * ((L.Lz + n - 1) / n + 2);
+    if (best < 0 || cost < best) { best = cost; best_n = n; }
+  }
+  return best_n;
+}
 
 // blocks of one launch (= block partials of the fused measurement); grid_cap = SMs
 int sc_ws_blocks(const ScLayout& L, int ZT, int grid_cap, int variant) {
   const int ty = ws_ty(variant);
-  const int n_tiles = ((L.Ly + ty - 1) / ty) * ((L.Lz + ZT - 1) / ZT);
+  const int n_tiles = ((L.Ly + ty - 1) / ty) * sc_ws_chunks(L, ZT, grid_cap, variant);
   const int cap = grid_cap * ws_ctas_per_sm(variant);
   return n_tiles < cap ? n_tiles : cap;
 }
 
 cudaError_t launch_sweep_sc_ws(cudaStream_t st, float* s, ScLayout L, int ZT, int grid_cap, int variant, SweepParams p, int colour, Meas m) {
   const int cap = grid_cap * ws_ctas_per_sm(variant);
-  if (variant == 1) return ws_pick<8, 1024, 6, 1>(st, s, L, ZT, cap, p, colour, m);
-  if (variant == 2) return ws_pick<4, 1024, 4, 3>(st, s, L, ZT, cap, p, colour, m);
-  return ws_pick<4, 1024, 5, 2>(st, s, L, ZT, cap, p, colour, m);
+  const int n_zc = sc_ws_chunks(L, ZT, grid_cap, variant);
+  if (variant == 3) return ws_pick<16, 1024, 4, 1>(st, s, L, n_zc, cap, p, colour, m);
+  if (variant == 1) return ws_pick<8, 1024, 6, 1>(st, s, L, n_zc, cap, p, colour, m);
+  if (variant == 2) return ws_pick<4, 1024, 4, 3>(st, s, L, n_zc, cap, p, colour, m);
+  return ws_pick<4, 1024, 5, 2>(st, s, L, n_zc, cap, p, colour, m);
 }
 
 }  // namespace hb

@@ -44,7 +44,51 @@ def run_scan(ctx, temperatures, sweeps, equil=0):
     return {k: np.array(v) for k, v in out.items()}
 
 
+def fit_order_parameter(T, m, t_lo, t_hi):
+    """Least squares of log m = log A + beta log(1 - T/Tc) over the points with t_lo <= 1 - T/Tc <= t_hi, scanning Tc
+    (the form the paper fits in its Fig. 3).  Returns (Tc, beta, A, rms of the log residual)."""
+    best = None
+    for Tc in np.arange(max(T) * 0.9, max(T) * 1.2, 0.0005):
+        t = 1.0 - T / Tc
+        sel = (t >= t_lo) & (t <= t_hi)
+        if sel.sum() < 4:
+            continue
+        x, y = np.log(t[sel]), np.log(m[sel])
+        beta, logA = np.polyfit(x, y, 1)
+        rms = float(np.sqrt(np.mean((y - (beta * x + logA)) ** 2)))
+        if best is None or rms < best[3]:
+            best = (float(Tc), float(beta), float(np.exp(logA)), rms)
+    return best
+
+
 def main(argv):
+    """python -m paper_2106_11286_b200.scan c2 | --sc L [--K k] [--T a:b:n] [--equil e] [--sweeps s] [--fit t_lo:t_hi]"""
+    if len(argv) > 1 and argv[1] == "--sc":
+        import argparse
+        ap = argparse.ArgumentParser()
+        ap.add_argument("--sc", type=int, required=True)
+        ap.add_argument("--K", type=float, default=0.01)
+        ap.add_argument("--T", default="1.00:1.50:26")
+        ap.add_argument("--equil", type=int, default=10000)
+        ap.add_argument("--sweeps", type=int, default=10000)
+        ap.add_argument("--fit", default="0.02:0.2")
+        a = ap.parse_args(argv[1:])
+        lo, hi, k = a.T.split(":")
+        Ts = [float(x) for x in np.linspace(float(lo), float(hi), int(k))]
+        cfg = dict(kind="sc", L=a.sc, J=1.0, K=a.K, e=(0.0, 0.0, 1.0), seed=1, start="aligned")
+        ctx = make_context(cfg)
+        res = run_scan(ctx, Ts, a.sweeps, a.equil)
+        print("# sc %d^3, K = %g, aligned start, heating, %d + %d sweeps per temperature" % (a.sc, a.K, a.equil, a.sweeps))
+        print("# T  <|M|>  <E>/N  chi  C")
+        for i in range(len(Ts)):
+            print("%.4f  %.6f  %.6f  %.4f  %.4f" % tuple(res[k][i] for k in ("T", "absM", "E", "chi", "C")))
+        t_lo, t_hi = (float(x) for x in a.fit.split(":"))
+        fit = fit_order_parameter(res["T"], res["absM"], t_lo, t_hi)
+        if fit:
+            print("# fit M = A (1 - T/Tc)^beta over %g <= 1 - T/Tc <= %g: Tc = %.4f, beta = %.4f, A = %.4f, rms(log) = %.2e" %
+                  ((t_lo, t_hi) + fit))
+        ctx.close()
+        return
     name = argv[1] if len(argv) > 1 else "c2"
     cfg = workloads.CONFIGS[name]
     ctx = make_context(cfg)
