@@ -521,7 +521,7 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
     // the warp-specialised kernel is built for long rows (pitch 1024 B): with them, on lattices far larger than L2, it
     // sustains 3-4 % more than the direct kernel and stays below the power cap; everything else runs direct
     c->sc_kernel = (sc_ws_supported(c->sc) && c->sc.H >= 224 && P.n >= (int64_t(1) << 24)) ? 1 : 0;
-    c->ws_variant = 2;
+    c->ws_variant = sc_ws_variant_supported(c->sc, 4) ? 4 : 2;   // 7-row tiles where the rows fit them (c4: +2 %), else 4-row tiles
   }
 
   // ---- device memory --------------------------------------------------------------------------
@@ -1017,7 +1017,7 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
   if (s == "sc_ws_variant") {
     if (!sc_ws_variant_supported(c->sc, (int)value))
       return fail(c, HB_EINVAL, "sc_ws_variant: 0 (4-row tiles, 2 CTAs per SM), 1 (8-row tiles, 1 CTA per SM), 2 (4-row tiles, 3 CTAs per SM), "
-                                "3 (16-row tiles, 1 CTA per SM; rows of up to 248 floats)");
+                                "3 (16-row tiles, 1 CTA per SM; rows of up to 248 floats), 4 (7-row tiles, 2 CTAs per SM; rows of up to 236 floats)");
     c->ws_variant = (int)value;
     return HB_OK;
   }

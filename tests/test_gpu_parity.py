@@ -370,13 +370,17 @@ def test_warp_specialised_kernel_matches_the_oracle():
              (dict(W.SMALL["c4"], L=(40, 12, 10), K=0.3, e=(0.6, 0.0, 0.8)), {"sc_ws_zt": 3}),
              (dict(W.SMALL["c4"], L=(64, 20, 6)), {"sc_ws_zt": 4, "sc_ws_ctas": 2}),
              (dict(W.SMALL["c4"], L=(8, 2, 2)), {}), (dict(W.SMALL["c4"], L=(512, 10, 4)), {"sc_ws_zt": 2}),
-             (W.SMALL["c4"], {"sc_ws_variant": 1}), (dict(W.SMALL["c4"], L=(40, 14, 10)), {"sc_ws_variant": 1, "sc_ws_zt": 3}),
+             (W.SMALL["c4"], {"sc_ws_variant": 2}), (W.SMALL["c4"], {"sc_ws_variant": 1}), (dict(W.SMALL["c4"], L=(40, 14, 10)), {"sc_ws_variant": 1, "sc_ws_zt": 3}),
              (dict(W.SMALL["c4"], L=(40, 14, 10)), {"sc_ws_variant": 0, "sc_ws_zt": 10, "sc_ws_ctas": 1}),
              # 16-row tiles (one CTA of up to 31 consumer warps per SM): a ragged single tile, three tiles with a ragged
              # last one and balanced z-chunks (sc_ws_zt = 0), the widest row this variant takes (Lx = 496)
              (dict(W.SMALL["c4"], L=(40, 14, 10)), {"sc_ws_variant": 3, "sc_ws_zt": 3}),
              (dict(W.SMALL["c4"], L=(64, 36, 10)), {"sc_ws_variant": 3, "sc_ws_zt": 0, "sc_ws_ctas": 2}),
-             (dict(W.SMALL["c4"], L=(496, 34, 6), K=0.3, e=(0.6, 0.0, 0.8)), {"sc_ws_variant": 3})]
+             (dict(W.SMALL["c4"], L=(496, 34, 6), K=0.3, e=(0.6, 0.0, 0.8)), {"sc_ws_variant": 3}),
+             # 7-row tiles, two CTAs per SM (the default for config 4's rows of 232 floats): ragged tiles, full-width rows
+             (dict(W.SMALL["c4"], L=(40, 14, 10)), {"sc_ws_variant": 4, "sc_ws_zt": 3}),
+             (dict(W.SMALL["c4"], L=(464, 16, 6), K=0.3, e=(0.6, 0.0, 0.8)), {"sc_ws_variant": 4}),
+             (dict(W.SMALL["c4"], L=(472, 30, 4)), {"sc_ws_variant": 4, "sc_ws_ctas": 3})]
     for cfg, opts in cases:
         lat, st = make_oracle(cfg)
         ctx = make_gpu(cfg)
@@ -399,6 +403,8 @@ def test_warp_specialised_kernel_matches_the_oracle():
         hb.Context(hb.Lattice("sc", 6)).set_option("sc_kernel", 1)   # rows of 3 floats: not a multiple of 4
     with pytest.raises(hb.HbError):
         hb.Context(hb.Lattice("sc", 512, 4, 4)).set_option("sc_ws_variant", 3)   # 16 rows of 64 vectors: more than 1024 threads
+    with pytest.raises(hb.HbError):
+        hb.Context(hb.Lattice("sc", 480, 4, 4)).set_option("sc_ws_variant", 4)   # 7 rows of 60 vectors: more than 13 warps
 
 
 def test_replayed_launches_match_the_oracle():
@@ -530,7 +536,7 @@ def test_kernel_variants_agree_on_random_shapes():
                     {"graph": 1, "sc_coop": 0},
                     {"graph": 0, "sc_coop": 2},
                     {"graph": int(rng.integers(0, 2)), "sc_kernel": 1, "sc_ws_zt": int(rng.integers(0, Lz + 1)),
-                     "sc_ws_ctas": int(rng.integers(1, 5)), "sc_ws_variant": int(rng.integers(0, 4 if H <= 248 else 3))}]
+                     "sc_ws_ctas": int(rng.integers(1, 5)), "sc_ws_variant": int(rng.integers(0, 5 if H <= 236 else 3))}]
         for opts in variants:
             got, (Mg, Eg) = run(opts)
             assert spins_equal(got, ref), (Lx, Ly, Lz, opts)
