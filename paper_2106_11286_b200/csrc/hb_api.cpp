@@ -161,6 +161,7 @@ struct hb_ctx {
   double* cached() const { return reinterpret_cast<double*>(ws + plan.off_counters + 64); }
   unsigned long long* sweep_dev() const { return reinterpret_cast<unsigned long long*>(ws + plan.off_counters + 128); }
   unsigned long long* series_idx() const { return reinterpret_cast<unsigned long long*>(ws + plan.off_counters + 136); }
+  uint32_t* ws_sched() const { return reinterpret_cast<uint32_t*>(ws + plan.off_counters + 144); }   // tile scheduler of k_sweep_sc_ws
 };
 
 namespace {
@@ -230,7 +231,7 @@ int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d, Meas m = Mea
   if (c->plan.engine == ENGINE_SC) {
     const bool diag = d.accept || d.n_accept;
     if (c->sc_kernel == 1 && !diag)
-      HB_CUDA(c, launch_sweep_sc_ws(c->stream, c->spins, c->sc, c->ws_zt, c->n_sms, c->ws_variant, p, colour, m));
+      HB_CUDA(c, launch_sweep_sc_ws(c->stream, c->spins, c->sc, c->ws_zt, c->n_sms, c->ws_variant, c->ws_sched(), p, colour, m));
     else
       HB_CUDA(c, launch_sweep_sc(c->stream, c->spins, c->sc, c->tile, p, colour, d, m));
   } else if (c->plan.engine == ENGINE_BRAVAIS) {

@@ -103,7 +103,8 @@ cudaError_t launch_sweeps_sc_coop(cudaStream_t st, float* spins, ScLayout L, ScT
 bool sc_ws_supported(const ScLayout& L);
 bool sc_ws_variant_supported(const ScLayout& L, int variant);
 int sc_ws_blocks(const ScLayout& L, int ZT, int grid_cap, int variant);
-cudaError_t launch_sweep_sc_ws(cudaStream_t st, float* spins, ScLayout L, int ZT, int grid_cap, int variant, SweepParams p, int colour, Meas m);
+cudaError_t launch_sweep_sc_ws(cudaStream_t st, float* spins, ScLayout L, int ZT, int grid_cap, int variant, uint32_t* sched /* 2 device words, zero */,
+                               SweepParams p, int colour, Meas m);
 cudaError_t launch_sweep_csr(cudaStream_t st, float* spins, CsrDev g, uint32_t list_begin, uint32_t list_count,
                              SweepParams p, int block, Diag d);
 cudaError_t launch_sweep_ell(cudaStream_t st, float* spins, EllDev g, uint32_t begin, uint32_t count, SweepParams p,

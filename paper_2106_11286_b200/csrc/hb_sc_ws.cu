@@ -13,8 +13,9 @@
 //     the slots through "empty" barriers, run the attempt arithmetic of hb_device.cuh; their own spins they
 //     load themselves (LDG.128; one plane ahead in the variants that have the registers for it) and store
 //     with STG.128 at the same addresses.  No block-wide barrier in the steady state;
-//   * CTAs are persistent (one to three per SM): a CTA walks its tiles (TY rows x ZT planes) with the rings running
-//     across tile boundaries, so the pipeline is filled once per launch, not once per tile.
+//   * CTAs are persistent (one to three per SM): a CTA takes tiles (TY rows x a chunk of planes) from a device counter,
+//     one after the other, with the rings running across tile boundaries, so the pipeline is filled once per launch,
+//     not once per tile, and no CTA is left with a fixed share when its SM runs slower than the others.
 //
 // Same arithmetic, same order of the neighbour sum, same bits as k_sweep_sc.
 #include "hb_device.cuh"
@@ -46,6 +47,7 @@ __host__ __device__ constexpr bool ws_pref() { return MINB < 3 && TY != 7; }
 
 struct WsTiles {
   int32_t n_ty, n_zc;   // tiles in y, chunks in z: chunk zc = planes [zc Lz / n_zc, (zc+1) Lz / n_zc), sizes differ by at most one
+  uint32_t* sched;      // device, two words, zero between launches: next tile to hand out, CTAs that have finished
 };
 
 // kNB plane slots of the other colour (z-1, z, z+1 and look-ahead); MINB = CTAs per SM the kernel is built for
@@ -53,14 +55,16 @@ template <int TY, int ROWB, int kNB, int MINB>
 struct WsSmem {
   static constexpr uint32_t SLOT_B = 3u * (TY + 2) * ROWB;
   static constexpr uint32_t OFF_BAR = kNB * SLOT_B;   // full[kNB], empty[kNB]
-  static constexpr uint32_t BYTES = OFF_BAR + 8u * (2 * kNB);
+  static constexpr uint32_t OFF_TILE = OFF_BAR + 8u * (2 * kNB);   // tile[kNB]: the tile a staged plane belongs to, -1 = no more tiles
+  static constexpr uint32_t BYTES = OFF_TILE + 4u * 8u;
+  static_assert(kNB <= 8, "tile words");
 };
 
 // ---- producer: one warp ------------------------------------------------------------------------------
 // plane k of a tile is lattice plane z0-1+k (periodic), rows y0-1 .. y0+ny (periodic) of the other colour
 template <int TY, int ROWB, int kNB, int MINB>
 __device__ __forceinline__ void ws_producer(const float* b, const ScLayout& L, const WsTiles& w,
-                                            uint32_t sbase) {
+                                            unsigned char* smem, uint32_t sbase) {
   using S = WsSmem<TY, ROWB, kNB, MINB>;
   const uint32_t lane = threadIdx.x;
   const uint32_t row_bytes = (uint32_t)L.H * 4u;
@@ -68,7 +72,19 @@ __device__ __forceinline__ void ws_producer(const float* b, const ScLayout& L, c
   const uint32_t fullB = sbase + S::OFF_BAR, emptyB = fullB + 8u * kNB;
   RingPos<kNB> rp;   // next plane slot to fill
   const int32_t n_tiles = w.n_ty * w.n_zc;
-  for (int32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+  volatile int32_t* tile_of = reinterpret_cast<volatile int32_t*>(smem + S::OFF_TILE);
+  // Tiles are handed out dynamically (one atomic per tile): the CTAs of a launch do not run at the same speed, and with a
+  // fixed share per CTA the fast SMs idled at the end of every launch (ncu: SMs active 70-99 % of the launch).  The
+  // consumers learn the tile from a word written beside the plane slot before the slot's "full" barrier is armed.
+  for (;;) {
+    int32_t tile = 0;
+    if (lane == 0) tile = (int32_t)atomicAdd(w.sched, 1u);
+    tile = __shfl_sync(0xffffffffu, tile, 0);
+    if (tile >= n_tiles) {   // tell the consumers: the slot they will wait on next carries no plane
+      mbar_wait_backoff(emptyB + 8u * rp.slot, rp.par ^ 1u);
+      if (lane == 0) { tile_of[rp.slot] = -1; mbar_arrive(fullB + 8u * rp.slot); }
+      break;
+    }
     const int32_t ty = tile % w.n_ty, zc = tile / w.n_ty;
     const int32_t y0 = ty * TY, ny = min(TY, L.Ly - y0);
     const int32_t z0 = (int32_t)(((int64_t)zc * L.Lz) / w.n_zc), nz = (int32_t)(((int64_t)(zc + 1) * L.Lz) / w.n_zc) - z0;
@@ -79,7 +95,7 @@ __device__ __forceinline__ void ws_producer(const float* b, const ScLayout& L, c
         const uint32_t slot = rp.slot;
         mbar_wait_backoff(emptyB + 8u * slot, rp.par ^ 1u);
         const uint32_t n_rows = 3u * (uint32_t)(ny + 2);
-        if (lane == 0) mbar_expect_tx(fullB + 8u * slot, n_rows * row_bytes);
+        if (lane == 0) { tile_of[slot] = tile; mbar_expect_tx(fullB + 8u * slot, n_rows * row_bytes); }
         __syncwarp();
         for (uint32_t q = lane; q < n_rows; q += 32) {
           const uint32_t comp = q / (uint32_t)(ny + 2), r = q - comp * (uint32_t)(ny + 2);
@@ -113,8 +129,11 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
   const size_t n = L.n;
   const size_t plane = (size_t)L.Ly * L.H;
   RingPos<kNB> rm;   // slot of plane z-1 of the current step
-  const int32_t n_tiles = w.n_ty * w.n_zc;
-  for (int32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+  const volatile int32_t* tile_of = reinterpret_cast<const volatile int32_t*>(smem + S::OFF_TILE);
+  for (;;) {
+    mbar_wait(fullB + 8u * rm.slot, rm.par);   // first plane of the next tile, or the producer's "no more tiles"
+    const int32_t tile = tile_of[rm.slot];
+    if (tile < 0) break;
     const int32_t ty = tile % w.n_ty, zc = tile / w.n_ty;
     const int32_t y0 = ty * TY, ny = min(TY, L.Ly - y0);
     const int32_t z0 = (int32_t)(((int64_t)zc * L.Lz) / w.n_zc), nz = (int32_t)(((int64_t)(zc + 1) * L.Lz) / w.n_zc) - z0;
@@ -138,10 +157,7 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
       }
       RingPos<kNB> rc = rm; rc.next();
       RingPos<kNB> rq = rc; rq.next();
-      if (s == 0) {
-        mbar_wait(fullB + 8u * rm.slot, rm.par);
-        mbar_wait(fullB + 8u * rc.slot, rc.par);
-      }
+      if (s == 0) mbar_wait(fullB + 8u * rc.slot, rc.par);
       mbar_wait(fullB + 8u * rq.slot, rq.par);
       const unsigned char* Bm = smem + rm.slot * S::SLOT_B;
       const unsigned char* Bc = smem + rc.slot * S::SLOT_B;
@@ -236,13 +252,17 @@ k_sweep_sc_ws(float* a, const float* b, ScLayout L, WsTiles w, SweepParams P, in
   }
   __syncthreads();
   double acc[4] = {0.0, 0.0, 0.0, 0.0};
-  if (threadIdx.x < 32) ws_producer<TY, ROWB, kNB, MINB>(b, L, w, sbase);
+  if (threadIdx.x < 32) ws_producer<TY, ROWB, kNB, MINB>(b, L, w, smem, sbase);
   else ws_consumer<TY, ROWB, kNB, MINB, ANISO, MEAS>(a, L, w, P, colour, m.mode, smem, sbase, acc);
+  if (threadIdx.x == 0) {   // this thread took the CTA's last tile number above; the last CTA to finish re-arms the scheduler
+    __threadfence();
+    if (atomicAdd(w.sched + 1, 1u) == gridDim.x - 1) { w.sched[0] = 0u; w.sched[1] = 0u; }
+  }
   if (MEAS) block_reduce4(acc[0], acc[1], acc[2], acc[3], m.partials + (size_t)blockIdx.x * 4);
 }
 
 template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS>
-cudaError_t ws_go(cudaStream_t st, float* s, const ScLayout& L, int n_zc, int grid_cap, const SweepParams& p, int colour, const Meas& m) {
+cudaError_t ws_go(cudaStream_t st, float* s, const ScLayout& L, int n_zc, int grid_cap, uint32_t* sched, const SweepParams& p, int colour, const Meas& m) {
   using S = WsSmem<TY, ROWB, kNB, MINB>;
   auto kern = k_sweep_sc_ws<TY, ROWB, kNB, MINB, ANISO, MEAS>;
   static bool configured = false;
@@ -254,6 +274,7 @@ cudaError_t ws_go(cudaStream_t st, float* s, const ScLayout& L, int n_zc, int gr
   WsTiles w;
   w.n_ty = (L.Ly + TY - 1) / TY;
   w.n_zc = n_zc;
+  w.sched = sched;
   const int n_tiles = w.n_ty * w.n_zc;
   const int grid = n_tiles < grid_cap ? n_tiles : grid_cap;
   const int threads = 32 + 32 * ((TY * (L.H / 4) + 31) / 32);
@@ -264,19 +285,19 @@ cudaError_t ws_go(cudaStream_t st, float* s, const ScLayout& L, int n_zc, int gr
 }
 
 template <int TY, int ROWB, int kNB, int MINB>
-cudaError_t ws_pick(cudaStream_t st, float* s, const ScLayout& L, int n_zc, int grid_cap, const SweepParams& p, int colour, const Meas& m) {
+cudaError_t ws_pick(cudaStream_t st, float* s, const ScLayout& L, int n_zc, int grid_cap, uint32_t* sched, const SweepParams& p, int colour, const Meas& m) {
   const int aniso = (p.K == 0.0f) ? ANISO_NONE : ((p.ex == 0.0f && p.ey == 0.0f && p.ez == 1.0f) ? ANISO_Z : ANISO_GENERAL);
   if (m.mode != 0) {
     switch (aniso) {
-      case ANISO_NONE: return ws_go<TY, ROWB, kNB, MINB, ANISO_NONE, true>(st, s, L, n_zc, grid_cap, p, colour, m);
-      case ANISO_Z: return ws_go<TY, ROWB, kNB, MINB, ANISO_Z, true>(st, s, L, n_zc, grid_cap, p, colour, m);
-      default: return ws_go<TY, ROWB, kNB, MINB, ANISO_GENERAL, true>(st, s, L, n_zc, grid_cap, p, colour, m);
+      case ANISO_NONE: return ws_go<TY, ROWB, kNB, MINB, ANISO_NONE, true>(st, s, L, n_zc, grid_cap, sched, p, colour, m);
+      case ANISO_Z: return ws_go<TY, ROWB, kNB, MINB, ANISO_Z, true>(st, s, L, n_zc, grid_cap, sched, p, colour, m);
+      default: return ws_go<TY, ROWB, kNB, MINB, ANISO_GENERAL, true>(st, s, L, n_zc, grid_cap, sched, p, colour, m);
     }
   }
   switch (aniso) {
-    case ANISO_NONE: return ws_go<TY, ROWB, kNB, MINB, ANISO_NONE, false>(st, s, L, n_zc, grid_cap, p, colour, m);
-    case ANISO_Z: return ws_go<TY, ROWB, kNB, MINB, ANISO_Z, false>(st, s, L, n_zc, grid_cap, p, colour, m);
-    default: return ws_go<TY, ROWB, kNB, MINB, ANISO_GENERAL, false>(st, s, L, n_zc, grid_cap, p, colour, m);
+    case ANISO_NONE: return ws_go<TY, ROWB, kNB, MINB, ANISO_NONE, false>(st, s, L, n_zc, grid_cap, sched, p, colour, m);
+    case ANISO_Z: return ws_go<TY, ROWB, kNB, MINB, ANISO_Z, false>(st, s, L, n_zc, grid_cap, sched, p, colour, m);
+    default: return ws_go<TY, ROWB, kNB, MINB, ANISO_GENERAL, false>(st, s, L, n_zc, grid_cap, sched, p, colour, m);
   }
 }
 
@@ -305,8 +326,9 @@ bool sc_ws_variant_supported(const ScLayout& L, int variant) {
 }
 
 // Chunks in z of one launch.  ZT > 0: chunks of at most ZT planes.  ZT = 0: the count that minimises the longest
-// walk of a CTA, rounds x (planes per chunk + 2): tiles are dealt round-robin to the persistent CTAs, a tile costs its
-// planes plus the two extra planes the producer stages for it.
+// walk of a CTA, rounds x (planes per chunk + 2): the persistent CTAs take the tiles in order, a tile costs its planes
+// plus the two extra planes the producer stages for it (measured on c4, 7-row tiles: 13 chunks 130.7 Gupd/s, chunks of
+// 24 / 16 / 12 / 8 planes 128.7 / 127 / 128 / 128).
 int sc_ws_chunks(const ScLayout& L, int ZT, int grid_cap, int variant) {
   if (ZT > 0) return (L.Lz + ZT - 1) / ZT;
   const int ty = ws_ty(variant);
@@ -328,14 +350,14 @@ int sc_ws_blocks(const ScLayout& L, int ZT, int grid_cap, int variant) {
   return n_tiles < cap ? n_tiles : cap;
 }
 
-cudaError_t launch_sweep_sc_ws(cudaStream_t st, float* s, ScLayout L, int ZT, int grid_cap, int variant, SweepParams p, int colour, Meas m) {
+cudaError_t launch_sweep_sc_ws(cudaStream_t st, float* s, ScLayout L, int ZT, int grid_cap, int variant, uint32_t* sched, SweepParams p, int colour, Meas m) {
   const int cap = grid_cap * ws_ctas_per_sm(variant);
   const int n_zc = sc_ws_chunks(L, ZT, grid_cap, variant);
-  if (variant == 4) return ws_pick<7, 1024, 4, 2>(st, s, L, n_zc, cap, p, colour, m);
-  if (variant == 3) return ws_pick<16, 1024, 4, 1>(st, s, L, n_zc, cap, p, colour, m);
-  if (variant == 1) return ws_pick<8, 1024, 6, 1>(st, s, L, n_zc, cap, p, colour, m);
-  if (variant == 2) return ws_pick<4, 1024, 4, 3>(st, s, L, n_zc, cap, p, colour, m);
-  return ws_pick<4, 1024, 5, 2>(st, s, L, n_zc, cap, p, colour, m);
+  if (variant == 4) return ws_pick<7, 1024, 4, 2>(st, s, L, n_zc, cap, sched, p, colour, m);
+  if (variant == 3) return ws_pick<16, 1024, 4, 1>(st, s, L, n_zc, cap, sched, p, colour, m);
+  if (variant == 1) return ws_pick<8, 1024, 6, 1>(st, s, L, n_zc, cap, sched, p, colour, m);
+  if (variant == 2) return ws_pick<4, 1024, 4, 3>(st, s, L, n_zc, cap, sched, p, colour, m);
+  return ws_pick<4, 1024, 5, 2>(st, s, L, n_zc, cap, sched, p, colour, m);
 }
 
 }  // namespace hb
