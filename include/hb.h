@@ -77,6 +77,12 @@ typedef struct {
    * with Philox key seed + r; more than one needs a simple cubic lattice of at most 8192 sites with Lx a
    * multiple of 8 and uniform anisotropy (each replica runs in one thread block, hb_sweep_each below). */
   int32_t n_replicas;
+  /* Slab of a larger periodic simple cubic lattice (multi-GPU decomposition along z).
+   * slab_Lz = 0: none.  slab_Lz > 0 (HB_SC only): the context holds planes z = slab_z0 .. slab_z0 + Lz - 1 of a lattice
+   * of Lx x Ly x slab_Lz sites (Lz, slab_z0, slab_Lz even), plus one ghost plane on each side that the caller keeps
+   * current (hb_slab_face).  Philox is keyed by the GLOBAL site id, so the slabs together walk the trajectory of the
+   * whole lattice bit for bit.  Such a context is driven with hb_slab_pass / hb_slab_next_sweep instead of hb_sweep. */
+  int32_t slab_Lz, slab_z0;
 } hb_lattice;
 
 /* Caller-owned device memory (e.g. torch tensors).  Sizes from hb_sizes().  Both
@@ -151,6 +157,23 @@ int hb_get_colouring(hb_ctx* ctx, int32_t* colour, int32_t* n_colours);
 
 /* Counters since hb_create: kernels launched by this context, sites attempted. */
 int hb_counters(hb_ctx* ctx, uint64_t* kernel_launches, uint64_t* attempts);
+
+/* ---- slab contexts (hb_lattice.slab_Lz > 0): one sweep of the whole lattice is, on every slab,
+ *        for colour in (0, 1):  hb_slab_pass(colour);  exchange the faces of that colour with both z-neighbours;
+ *        hb_slab_next_sweep()
+ * Colour = (x + y + z) mod 2 in GLOBAL coordinates.  hb_slab_pass launches the colour kernel on the slab (asynchronous, on
+ * the context's stream).  hb_slab_face gives, as offsets in floats into the spins buffer (hb_buffers.spins, or the
+ * library's own allocation) and a length in floats, the three contiguous component runs of one face of one colour:
+ * side 0 = low z, 1 = high z; ghost 0 = the slab's own boundary plane (to send), 1 = the ghost plane beyond it (to
+ * receive into: the neighbour's boundary plane of the same colour).  The copy itself (cudaMemcpyPeer, NCCL send/recv,
+ * peer stores) is the caller's, in stream order with the passes.  After hb_init_* / hb_set_spins the ghost planes of
+ * BOTH colours must be exchanged once.  hb_measure on a slab returns its share: M = (sum over the slab's own sites) / (Lx Ly
+ * slab_Lz) and the energy of its own sites with every bond counted half at each end, so that the sum over the slabs is M
+ * and E of the whole lattice.  hb_get_spins / hb_set_spins move the slab's own Lx Ly Lz sites in canonical order
+ * (z slowest).  hb_sweep, hb_sweep_series, hb_sweep_record and replicas return HB_ESTATE / HB_EINVAL on a slab. */
+int hb_slab_pass(hb_ctx* ctx, float T, int32_t colour);
+int hb_slab_next_sweep(hb_ctx* ctx);
+int hb_slab_face(hb_ctx* ctx, int32_t colour, int32_t side, int32_t ghost, size_t offset_floats[3], size_t* count_floats);
 
 /* Tuning knobs, by name (DESIGN.md section 6 lists them); unknown names give HB_EINVAL. */
 int hb_set_option(hb_ctx* ctx, const char* name, int64_t value);

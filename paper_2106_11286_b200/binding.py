@@ -25,7 +25,7 @@ class hb_lattice(C.Structure):
     _fields_ = [("kind", C.c_int32), ("Lx", C.c_int32), ("Ly", C.c_int32), ("Lz", C.c_int32),
                 ("n_sites", C.c_int64), ("row_ptr", C.c_void_p), ("col_idx", C.c_void_p),
                 ("n_colours", C.c_int32), ("colour", C.c_void_p), ("K_site", C.c_void_p), ("e_site", C.c_void_p),
-                ("n_replicas", C.c_int32)]
+                ("n_replicas", C.c_int32), ("slab_Lz", C.c_int32), ("slab_z0", C.c_int32)]
 
 
 class hb_buffers(C.Structure):
@@ -73,6 +73,9 @@ def load_library():
         "hb_measure_each": [vp, vp, vp],
         "hb_sweep_series_each": [vp, vp, i64, vp, vp],
         "hb_select_replica": [vp, i32],
+        "hb_slab_pass": [vp, f32, i32],
+        "hb_slab_next_sweep": [vp],
+        "hb_slab_face": [vp, i32, i32, i32, P(C.c_size_t), P(C.c_size_t)],
         "hb_sweep_count": [vp, P(u64)],
         "hb_set_sweep_count": [vp, u64],
         "hb_get_colouring": [vp, vp, P(i32)],
@@ -107,7 +110,7 @@ class Lattice:
     """Host description of a lattice (the hb_lattice struct plus the arrays it points to)."""
 
     def __init__(self, kind, Lx=0, Ly=0, Lz=0, row_ptr=None, col_idx=None, colour=None, n_colours=0,
-                 K_site=None, e_site=None, xyz=None, n_replicas=1):
+                 K_site=None, e_site=None, xyz=None, n_replicas=1, slab=None):
         self.kind = _KINDS[kind] if isinstance(kind, str) else int(kind)
         self.Lx, self.Ly, self.Lz = int(Lx), int(Ly or Lx), int(Lz or Lx)
         self.row_ptr = _np(row_ptr, np.int64) if row_ptr is not None else None
@@ -118,6 +121,8 @@ class Lattice:
         self.e_site = _np(e_site, np.float32) if e_site is not None else None
         self.xyz = xyz
         self.n_replicas = int(n_replicas)
+        # slab = (z0, Lz_global): this lattice is planes z0 .. z0 + Lz - 1 of a periodic sc lattice Lx x Ly x Lz_global
+        self.slab = (int(slab[0]), int(slab[1])) if slab is not None else None
 
     @classmethod
     def fcc_sphere(cls, R, K_core=0.0, e_core=(0, 0, 1), K_surf=0.0, colouring="greedy"):
@@ -147,6 +152,8 @@ class Lattice:
         s = hb_lattice()
         s.kind, s.Lx, s.Ly, s.Lz = self.kind, self.Lx, self.Ly, self.Lz
         s.n_replicas = self.n_replicas
+        if self.slab is not None:
+            s.slab_z0, s.slab_Lz = self.slab
         if self.row_ptr is not None:
             s.n_sites = self.row_ptr.size - 1
             s.row_ptr = _ptr(self.row_ptr)
@@ -270,6 +277,22 @@ class Context:
         M, E = np.zeros((self.n_replicas, n_sweeps, 3)), np.zeros((self.n_replicas, n_sweeps))
         self._check(self._L.hb_sweep_series_each(self._h, _ptr(t), n_sweeps, _ptr(M), _ptr(E)), "hb_sweep_series_each")
         return M, E
+
+    # ---- slabs (Lattice("sc", Lx, Ly, Lz, slab=(z0, Lz_global))); paper_2106_11286_b200.slabs drives them --------
+    def slab_pass(self, T, colour):
+        self._check(self._L.hb_slab_pass(self._h, T, int(colour)), "hb_slab_pass")
+
+    def slab_next_sweep(self):
+        self._check(self._L.hb_slab_next_sweep(self._h), "hb_slab_next_sweep")
+
+    def slab_face(self, colour, side, ghost):
+        """The three component runs (torch float32 views of the spins buffer) of one face of one colour: side 0 = low z,
+        1 = high z; ghost False = the slab's own boundary plane, True = the ghost plane beyond it."""
+        import torch
+        off, cnt = (C.c_size_t * 3)(), C.c_size_t()
+        self._check(self._L.hb_slab_face(self._h, int(colour), int(side), int(bool(ghost)), off, C.byref(cnt)), "hb_slab_face")
+        f = self._spins.view(torch.float32)
+        return [f[off[k]:off[k] + cnt.value] for k in range(3)]
 
     def sweep_record(self, T):
         acc = np.zeros(self.n, np.uint8)

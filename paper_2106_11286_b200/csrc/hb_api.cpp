@@ -35,6 +35,24 @@ struct Plan {                 // device memory plan of a lattice
   size_t off_row_ptr = 0, off_col = 0, off_list = 0, off_K = 0, off_e = 0;
 };
 
+// A slab (hb_lattice.slab_Lz > 0) is run as a periodic lattice of Lz + 2 planes whose first and last planes are the
+// ghost planes: the kernels need no special case, the two ghost planes are updated with meaningless neighbours and
+// overwritten by the caller's face exchange before anything reads them.  Returns the padded description.
+int pad_slab(const hb_lattice* lat, hb_lattice& padded, std::string& why) {
+  padded = *lat;
+  if (lat->slab_Lz <= 0) return HB_OK;
+  if (lat->kind != HB_SC || lat->n_replicas > 1 || lat->K_site || lat->e_site) {
+    why = "a slab needs a simple cubic lattice with uniform anisotropy and no replicas"; return HB_EINVAL;
+  }
+  if (lat->Lz < 2 || ((lat->Lz | lat->slab_Lz | lat->slab_z0) & 1) || lat->slab_z0 < 0 || lat->slab_z0 + lat->Lz > lat->slab_Lz) {
+    why = "slab: Lz, slab_Lz, slab_z0 even, Lz >= 2, 0 <= slab_z0, slab_z0 + Lz <= slab_Lz"; return HB_EINVAL;
+  }
+  if ((int64_t)lat->Lx * lat->Ly * lat->slab_Lz > 0xFFFFFFFFll) { why = "more than 2^32-1 sites in the whole lattice"; return HB_EINVAL; }
+  padded.Lz = lat->Lz + 2;
+  padded.slab_Lz = 0;
+  return HB_OK;
+}
+
 int make_plan(const hb_lattice* lat, Plan& p, std::string& why) {
   if (!lat) { why = "lattice is NULL"; return HB_EINVAL; }
   const int k = lat->kind;
@@ -130,6 +148,7 @@ struct hb_ctx {
   cudaGraphExec_t gexec[2] = {nullptr, nullptr};   // [0] plain sweeps, [1] every sweep measured into the series buffer
   float g_beta[2] = {0.0f, 0.0f};
   bool g_dirty[2] = {true, true};
+  int32_t slab_Lz = 0, slab_z0 = 0;   // > 0: this context is a slab of a larger lattice (planes 0 and Lz-1 of sc are ghosts)
   int sc_coop = -1;            // persistent multi-sweep kernel: -1 auto, 0 off, 1 / 2 forced (see hb_set_option)
   bool fused_measure = true;   // sc: the last sweep of hb_sweep also reduces M and E
   bool cache_valid = false;    // cached() holds the measurement of the current spins
@@ -420,9 +439,13 @@ extern "C" {
 int hb_sizes(const hb_lattice* lat, int64_t* n_sites, size_t* spins_bytes, size_t* workspace_bytes) {
   Plan p;
   std::string why;
-  const int rc = make_plan(lat, p, why);
+  if (!lat) return HB_EINVAL;
+  hb_lattice padded;
+  int rc = pad_slab(lat, padded, why);
   if (rc != HB_OK) return rc;
-  if (n_sites) *n_sites = p.n;
+  rc = make_plan(&padded, p, why);
+  if (rc != HB_OK) return rc;
+  if (n_sites) *n_sites = lat->slab_Lz > 0 ? (int64_t)lat->Lx * lat->Ly * lat->Lz : p.n;   // a slab's own sites
   if (spins_bytes) *spins_bytes = p.spins_bytes;
   if (workspace_bytes) *workspace_bytes = p.ws_bytes;
   return HB_OK;
@@ -437,7 +460,13 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
   // the context is handed back even on failure so that hb_error_detail can say why
   *out = c;
   std::string why;
-  int rc = make_plan(lat, c->plan, why);
+  if (!lat) { c->sticky = HB_EINVAL; return fail(c, HB_EINVAL, "lattice is NULL"); }
+  hb_lattice padded;
+  int rc = pad_slab(lat, padded, why);
+  if (rc != HB_OK) { c->sticky = rc; return fail(c, rc, why); }
+  if (lat->slab_Lz > 0) { c->slab_Lz = lat->slab_Lz; c->slab_z0 = lat->slab_z0; }
+  lat = &padded;
+  rc = make_plan(lat, c->plan, why);
   if (rc != HB_OK) { c->sticky = rc; return fail(c, rc, why); }
   if (!e || !unit_vector(e) || !std::isfinite(J) || !std::isfinite(K)) {
     c->sticky = HB_EINVAL;
@@ -522,6 +551,11 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
     // the warp-specialised kernel is built for long rows (pitch 1024 B): with them, on lattices far larger than L2, it
     // sustains 3-4 % more than the direct kernel and stays below the power cap; everything else runs direct
     c->sc_kernel = (sc_ws_supported(c->sc) && c->sc.H >= 224 && P.n >= (int64_t(1) << 24)) ? 1 : 0;
+    if (c->slab_Lz > 0) {   // local plane 1 is global plane slab_z0; graphs, persistent kernels and the fused measurement are for whole lattices
+      c->sc.ghost = 1;
+      c->sc.site_base = (uint32_t)(((int64_t)c->slab_z0 - 1) * lat->Ly * lat->Lx);
+      c->graph_mode = 0; c->sc_coop = 0; c->fused_measure = false;
+    }
     c->ws_variant = sc_ws_variant_supported(c->sc, 4) ? 4 : 2;   // 7-row tiles where the rows fit them (c4: +2 %), else 4-row tiles
   }
 
@@ -680,6 +714,14 @@ int hb_set_spins(hb_ctx* c, const float* sx, const float* sy, const float* sz) {
   if (!sx || !sy || !sz) return fail(c, HB_EINVAL, "NULL spin array");
   c->each_valid = false;
   const size_t n = (size_t)c->plan.n;
+  std::vector<float> padded;   // slab: the caller's Lx Ly Lz sites sit between two ghost planes (zero until exchanged)
+  if (c->slab_Lz > 0) {
+    const size_t plane = (size_t)c->sc.Lx * c->sc.Ly, own = n - 2 * plane;
+    padded.assign(3 * n, 0.0f);
+    const float* in[3] = {sx, sy, sz};
+    for (int k = 0; k < 3; ++k) std::memcpy(padded.data() + k * n + plane, in[k], own * sizeof(float));
+    sx = padded.data(); sy = sx + n; sz = sy + n;
+  }
   const float* src[3] = {sx, sy, sz};
   for (int k = 0; k < 3; ++k) {
     if (c->plan.engine == ENGINE_SC) {
@@ -709,7 +751,9 @@ int hb_get_spins(hb_ctx* c, float* sx, float* sy, float* sz) {
     if (c->plan.engine == ENGINE_SC) {
       HB_CUDA(c, launch_sc_permute(c->stream, c->staging(), c->spins + k * n, c->sc, false));
       c->launches += 1;
-      HB_CUDA(c, cudaMemcpyAsync(dst[k], c->staging(), n * 4, cudaMemcpyDeviceToHost, c->stream));
+      // a slab hands out its own planes only: they are contiguous in canonical order, between the two ghost planes
+      const size_t skip = c->slab_Lz > 0 ? (size_t)c->sc.Lx * c->sc.Ly : 0;
+      HB_CUDA(c, cudaMemcpyAsync(dst[k], c->staging() + skip, (n - 2 * skip) * 4, cudaMemcpyDeviceToHost, c->stream));
     } else if (c->plan.ell) {
       HB_CUDA(c, launch_permute_ell(c->stream, c->spins, c->staging(), c->ell.perm, (uint32_t)n, k, false));
       c->launches += 1;
@@ -724,6 +768,7 @@ int hb_get_spins(hb_ctx* c, float* sx, float* sy, float* sz) {
 
 int hb_sweep(hb_ctx* c, float T, int64_t n_sweeps) {
   HB_CHECK_CTX(c);
+  if (c->slab_Lz > 0) return fail(c, HB_ESTATE, "slab context: drive it with hb_slab_pass / hb_slab_next_sweep and exchange the faces (include/hb.h)");
   if (n_sweeps < 0) return fail(c, HB_EINVAL, "n_sweeps < 0");
   if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
   float beta;
@@ -781,7 +826,8 @@ int hb_measure(hb_ctx* c, double M[3], double* E) {
   double h[4];
   HB_CUDA(c, cudaMemcpyAsync(h, c->cached(), sizeof h, cudaMemcpyDeviceToHost, c->stream));
   HB_CUDA(c, cudaStreamSynchronize(c->stream));
-  const double inv = 1.0 / (double)c->plan.n;
+  // a slab returns its share of M of the whole lattice (the kernel skipped the ghost planes)
+  const double inv = 1.0 / (c->slab_Lz > 0 ? (double)c->sc.Lx * c->sc.Ly * c->slab_Lz : (double)c->plan.n);
   M[0] = h[0] * inv; M[1] = h[1] * inv; M[2] = h[2] * inv;
   *E = h[3];
   return HB_OK;
@@ -789,6 +835,7 @@ int hb_measure(hb_ctx* c, double M[3], double* E) {
 
 int hb_sweep_series(hb_ctx* c, float T, int64_t n_sweeps, double* M_series, double* E_series) {
   HB_CHECK_CTX(c);
+  if (c->slab_Lz > 0) return fail(c, HB_ESTATE, "slab context: drive it with hb_slab_pass / hb_slab_next_sweep and exchange the faces (include/hb.h)");
   if (n_sweeps < 0 || !M_series || !E_series) return fail(c, HB_EINVAL, "bad series arguments");
   if (c->plan.R > 1) return fail(c, HB_EINVAL, "a context with replicas takes hb_sweep_series_each");
   if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
@@ -835,6 +882,7 @@ int hb_sweep_series(hb_ctx* c, float T, int64_t n_sweeps, double* M_series, doub
 
 int hb_sweep_record(hb_ctx* c, float T, uint8_t* accept) {
   HB_CHECK_CTX(c);
+  if (c->slab_Lz > 0) return fail(c, HB_ESTATE, "slab context: drive it with hb_slab_pass / hb_slab_next_sweep and exchange the faces (include/hb.h)");
   if (!accept) return fail(c, HB_EINVAL, "NULL accept array");
   if (c->plan.R > 1) return fail(c, HB_EINVAL, "hb_sweep_record needs a context without replicas");
   if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
@@ -938,6 +986,44 @@ int hb_sweep_series_each(hb_ctx* c, const float* T, int64_t n_sweeps, double* M_
   return HB_OK;
 }
 
+// ---- slabs (include/hb.h) -------------------------------------------------------------------
+// Local plane z_l holds global plane slab_z0 + z_l - 1 and slab_z0 is even, so the parity of a local plane is the
+// opposite of its global one: the sites of GLOBAL colour g are the local colour plane 1 - g.
+int hb_slab_pass(hb_ctx* c, float T, int32_t colour) {
+  HB_CHECK_CTX(c);
+  if (c->slab_Lz <= 0) return fail(c, HB_ESTATE, "not a slab context");
+  if (colour != 0 && colour != 1) return fail(c, HB_EINVAL, "colour: 0 or 1");
+  if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
+  float beta;
+  int rc = check_T(c, T, &beta);
+  if (rc != HB_OK) return rc;
+  c->cache_valid = false;
+  rc = one_colour(c, 1 - colour, params(c, beta), Diag{nullptr, nullptr});
+  if (rc != HB_OK) return rc;
+  c->attempts += (uint64_t)c->sc.Lx * c->sc.Ly * (uint64_t)(c->sc.Lz - 2) / 2;
+  return HB_OK;
+}
+
+int hb_slab_next_sweep(hb_ctx* c) {
+  HB_CHECK_CTX(c);
+  if (c->slab_Lz <= 0) return fail(c, HB_ESTATE, "not a slab context");
+  c->sweep += 1;
+  return HB_OK;
+}
+
+int hb_slab_face(hb_ctx* c, int32_t colour, int32_t side, int32_t ghost, size_t offset_floats[3], size_t* count_floats) {
+  HB_CHECK_CTX(c);
+  if (c->slab_Lz <= 0) return fail(c, HB_ESTATE, "not a slab context");
+  if ((colour | side | ghost) & ~1) return fail(c, HB_EINVAL, "colour, side, ghost: 0 or 1");
+  if (!offset_floats || !count_floats) return fail(c, HB_EINVAL, "NULL output");
+  const size_t plane = (size_t)c->sc.Ly * c->sc.H;   // sites of one colour in a z-plane: one contiguous run per component
+  const int32_t z = side == 0 ? (ghost ? 0 : 1) : (ghost ? c->sc.Lz - 1 : c->sc.Lz - 2);
+  for (int k = 0; k < 3; ++k)
+    offset_floats[k] = (size_t)k * c->sc.n + (size_t)(1 - colour) * c->sc.half + (size_t)z * plane;
+  *count_floats = plane;
+  return HB_OK;
+}
+
 int hb_sweep_count(hb_ctx* c, uint64_t* out) {
   if (!c || !out) return HB_EINVAL;
   *out = c->sweep;
@@ -952,6 +1038,7 @@ int hb_set_sweep_count(hb_ctx* c, uint64_t value) {
 
 int hb_get_colouring(hb_ctx* c, int32_t* colour, int32_t* n_colours) {
   HB_CHECK_CTX(c);
+  if (c->slab_Lz > 0) return fail(c, HB_ESTATE, "slab context: the colour of a site is (x + y + z) mod 2 in global coordinates");
   if (n_colours) *n_colours = c->n_colours;
   if (!colour) return HB_OK;
   if (c->plan.engine == ENGINE_SC) {

@@ -24,6 +24,10 @@ struct ScLayout {
   int32_t H;        // Lx/2: sites of one colour per x-row
   uint32_t half;    // N/2: sites per colour
   uint32_t n;       // N
+  // slab of a larger lattice (include/hb.h, hb_lattice.slab_Lz): planes 0 and Lz-1 are ghost planes, the Philox site id
+  // of local site s is s + site_base (mod 2^32); both 0 for a whole lattice
+  uint32_t site_base;
+  int32_t ghost;
 };
 
 // launch shape of the sc kernels: a block is JX x TY threads, each thread owns V

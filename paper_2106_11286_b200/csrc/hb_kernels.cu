@@ -174,7 +174,7 @@ __device__ __forceinline__ void sc_pass(float* ax, float* ay, float* az, const f
       prefetch_line<PF>(bx + pzp + yp); prefetch_line<PF>(by + pzp + yp); prefetch_line<PF>(bz + pzp + yp);
       prefetch_line<PF>(bx + zpp); prefetch_line<PF>(by + zpp); prefetch_line<PF>(bz + zpp);
     }
-    const uint32_t site0 = (uint32_t)(z * L.Ly + y) * (uint32_t)L.Lx + 2u * (uint32_t)i0 + (uint32_t)p;
+    const uint32_t site0 = (uint32_t)(z * L.Ly + y) * (uint32_t)L.Lx + 2u * (uint32_t)i0 + (uint32_t)p + L.site_base;
     bool any = false;
     if (V >= 2) {
 #pragma unroll
@@ -280,7 +280,7 @@ __device__ __forceinline__ uint32_t sc_canonical(const ScLayout& L, uint32_t m) 
 
 __global__ void k_init_random_sc(float* sx, float* sy, float* sz, ScLayout L, uint32_t seed_lo, uint32_t seed_hi) {
   for (uint32_t m = blockIdx.x * blockDim.x + threadIdx.x; m < L.n; m += gridDim.x * blockDim.x) {
-    const Rand4 r = philox4x32_10(sc_canonical(L, m), 1u, 0u, 0u, seed_lo, seed_hi);
+    const Rand4 r = philox4x32_10(sc_canonical(L, m) + L.site_base, 1u, 0u, 0u, seed_lo, seed_hi);
     float x, y, z;
     sphere(r.r0, r.r1, x, y, z);
     sx[m] = x; sy[m] = y; sz[m] = z;
@@ -422,6 +422,7 @@ k_measure_sc(const float* __restrict__ sx, const float* __restrict__ sy, const f
     const uint32_t r = q - c * per_colour;
     const uint32_t row = r / HV, j = r - row * HV;
     const int32_t z = (int32_t)(row / (uint32_t)L.Ly), y = (int32_t)(row - (uint32_t)z * (uint32_t)L.Ly);
+    if (L.ghost && (z == 0 || z == L.Lz - 1)) continue;   // a slab sums its own planes only
     const int32_t ym = (y == 0) ? L.Ly - 1 : y - 1, yp = (y == L.Ly - 1) ? 0 : y + 1;
     const int32_t zm = (z == 0) ? L.Lz - 1 : z - 1, zp = (z == L.Lz - 1) ? 0 : z + 1;
     const int32_t p = (int32_t)((c + (uint32_t)y + (uint32_t)z) & 1u), i0 = (int32_t)(j * V);

@@ -140,7 +140,7 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
     const bool active = r < ny;
     const int32_t y = y0 + r;
     float* gx = a + ((size_t)z0 * L.Ly + y) * L.H + i0;            // own spins of plane z0 (x component)
-    uint32_t site_row = (uint32_t)(z0 * L.Ly + y) * (uint32_t)L.Lx + 2u * (uint32_t)i0;
+    uint32_t site_row = (uint32_t)(z0 * L.Ly + y) * (uint32_t)L.Lx + 2u * (uint32_t)i0 + L.site_base;
     // own spins come straight from global memory, one plane ahead of their use (only this thread writes them)
     constexpr bool PREF = ws_pref<TY, MINB>();   // otherwise (72 registers) the other warps cover the latency instead
     Vec<4> nxt[3];

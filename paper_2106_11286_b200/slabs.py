@@ -1,0 +1,198 @@
+"""Slab decomposition of the periodic simple cubic lattice along z.
+
+Every slab is an hb context over planes z0 .. z0 + nz - 1 of the whole lattice plus one ghost plane on each side
+(include/hb.h, hb_lattice.slab_Lz).  One sweep of the whole lattice is, on every slab,
+
+    for colour in (0, 1):  hb_slab_pass(colour);  send the two boundary planes of that colour to the z-neighbours
+    hb_slab_next_sweep()
+
+i.e. ONE exchange step per colour: 2 faces x 3 components x (Lx Ly / 2) floats per slab.  Philox is keyed by the global
+site id, so the slabs together walk the single-context trajectory bit for bit (tests/test_slabs.py).
+
+* `LocalSlabs`: all slabs in this process (one GPU, or several devices of one process); faces move with
+  `Tensor.copy_` on the contexts' stream (a device-to-device / peer copy).
+* `DistSlab`: one slab per rank of a `torch.distributed` group (one process per GPU); faces move with
+  `batch_isend_irecv` (NCCL send/recv over NVLink between GPUs), M and E with one all_reduce of 4 doubles.
+
+Host-side orchestration only: every pass and reduction runs in the CUDA library, the copies are library copies.
+"""
+import numpy as np
+
+
+def partition(Lz, n_slabs):
+    """[(z0, nz)] with every nz even and >= 2, as equal as possible, summing to Lz (Lz even)."""
+    if Lz % 2 or n_slabs < 1 or Lz < 2 * n_slabs:
+        raise ValueError("partition: Lz must be even and hold at least two planes per slab")
+    pairs, extra = divmod(Lz // 2, n_slabs)
+    out, z0 = [], 0
+    for r in range(n_slabs):
+        nz = 2 * (pairs + (1 if r < extra else 0))
+        out.append((z0, nz))
+        z0 += nz
+    return out
+
+
+def neighbours(rank, world):
+    """(rank owning the planes below this slab, rank owning the planes above), periodic."""
+    return (rank - 1) % world, (rank + 1) % world
+
+
+def exchange_local(ctxs, colour):
+    """Faces of one colour between slabs that live in this process: slab r's low boundary plane becomes the high ghost
+    plane of slab r-1, its high boundary plane the low ghost plane of slab r+1 (periodic; a single slab feeds itself)."""
+    G = len(ctxs)
+    for r, c in enumerate(ctxs):
+        down, up = neighbours(r, G)
+        for src, dst in zip(c.slab_face(colour, 0, False), ctxs[down].slab_face(colour, 1, True)):
+            dst.copy_(src, non_blocking=True)
+        for src, dst in zip(c.slab_face(colour, 1, False), ctxs[up].slab_face(colour, 0, True)):
+            dst.copy_(src, non_blocking=True)
+
+
+def exchange_dist(ctx, colour, rank, world, group=None):
+    """The same between ranks.  Sends go out low face first, then high face; a rank's receives are posted in the order
+    its neighbours send (the upper neighbour's low face fills the high ghost plane, the lower neighbour's high face the
+    low ghost plane), so that with two ranks, where both neighbours are the same peer, messages still pair up."""
+    import torch.distributed as dist
+    down, up = neighbours(rank, world)
+    if world == 1:
+        exchange_local([ctx], colour)
+        return
+    ops = []
+    for t in ctx.slab_face(colour, 0, False):
+        ops.append(dist.P2POp(dist.isend, t, down, group))
+    for t in ctx.slab_face(colour, 1, False):
+        ops.append(dist.P2POp(dist.isend, t, up, group))
+    for t in ctx.slab_face(colour, 1, True):
+        ops.append(dist.P2POp(dist.irecv, t, up, group))
+    for t in ctx.slab_face(colour, 0, True):
+        ops.append(dist.P2POp(dist.irecv, t, down, group))
+    for req in dist.batch_isend_irecv(ops):
+        req.wait()
+
+
+class LocalSlabs:
+    """n_slabs slab contexts of one periodic sc lattice in this process."""
+
+    def __init__(self, Lx, Ly, Lz, n_slabs, J=1.0, K=0.0, e=(0.0, 0.0, 1.0), seed=1, devices=None, options=None):
+        from .binding import Context, Lattice
+        self.shape = (Lx, Ly, Lz)
+        self.parts = partition(Lz, n_slabs)
+        devices = devices or ["cuda:0"] * n_slabs
+        self.ctxs = [Context(Lattice("sc", Lx, Ly, nz, slab=(z0, Lz)), J, K, e, seed, device=devices[r])
+                     for r, (z0, nz) in enumerate(self.parts)]
+        for c in self.ctxs:
+            for k, v in (options or {}).items():
+                c.set_option(k, v)
+        self.n = Lx * Ly * Lz
+
+    def _sync(self):
+        import torch
+        for c in self.ctxs:
+            torch.cuda.synchronize(c.device)
+
+    def _fill_ghosts(self):
+        self._sync()
+        for colour in (0, 1):
+            exchange_local(self.ctxs, colour)
+        self._sync()
+
+    def init_random(self):
+        for c in self.ctxs:
+            c.init_random()
+        self._fill_ghosts()
+
+    def init_aligned(self, direction):
+        for c in self.ctxs:
+            c.init_aligned(direction)
+        self._fill_ghosts()
+
+    def set_spins(self, sx, sy, sz):
+        plane = self.shape[0] * self.shape[1]
+        for c, (z0, nz) in zip(self.ctxs, self.parts):
+            c.set_spins(*[np.asarray(a, np.float32)[z0 * plane:(z0 + nz) * plane] for a in (sx, sy, sz)])
+        self._fill_ghosts()
+
+    def get_spins(self):
+        parts = [c.get_spins() for c in self.ctxs]
+        return [np.concatenate([p[k] for p in parts]) for k in range(3)]
+
+    def sweep(self, T, n_sweeps=1):
+        several = len({str(c.device) for c in self.ctxs}) > 1 or len({c.stream.cuda_stream for c in self.ctxs}) > 1
+        for _ in range(n_sweeps):
+            for colour in (0, 1):
+                for c in self.ctxs:
+                    c.slab_pass(T, colour)
+                if several:          # contexts on one stream are ordered by it; otherwise passes and copies meet here
+                    self._sync()
+                exchange_local(self.ctxs, colour)
+                if several:
+                    self._sync()
+            for c in self.ctxs:
+                c.slab_next_sweep()
+
+    def measure(self):
+        M, E = np.zeros(3), 0.0
+        for c in self.ctxs:
+            m, e = c.measure()
+            M += m
+            E += e
+        return M, E
+
+    def close(self):
+        for c in self.ctxs:
+            c.close()
+
+
+class DistSlab:
+    """This rank's slab of a periodic sc lattice split over the ranks of a torch.distributed group."""
+
+    def __init__(self, Lx, Ly, Lz, J=1.0, K=0.0, e=(0.0, 0.0, 1.0), seed=1, device=None, group=None, options=None):
+        import torch.distributed as dist
+        from .binding import Context, Lattice
+        self.group = group
+        self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
+        self.shape = (Lx, Ly, Lz)
+        self.z0, self.nz = partition(Lz, self.world)[self.rank]
+        self.ctx = Context(Lattice("sc", Lx, Ly, self.nz, slab=(self.z0, Lz)), J, K, e, seed,
+                           device=device or "cuda:0")
+        for k, v in (options or {}).items():
+            self.ctx.set_option(k, v)
+        self.n = Lx * Ly * Lz
+
+    def _fill_ghosts(self):
+        for colour in (0, 1):
+            exchange_dist(self.ctx, colour, self.rank, self.world, self.group)
+
+    def init_random(self):
+        self.ctx.init_random()
+        self._fill_ghosts()
+
+    def init_aligned(self, direction):
+        self.ctx.init_aligned(direction)
+        self._fill_ghosts()
+
+    def sweep(self, T, n_sweeps=1):
+        for _ in range(n_sweeps):
+            for colour in (0, 1):
+                self.ctx.slab_pass(T, colour)
+                exchange_dist(self.ctx, colour, self.rank, self.world, self.group)
+            self.ctx.slab_next_sweep()
+
+    def measure(self):
+        """M and E of the WHOLE lattice on every rank (one all_reduce of 4 doubles)."""
+        import torch
+        import torch.distributed as dist
+        m, e = self.ctx.measure()
+        t = torch.tensor([m[0], m[1], m[2], e], dtype=torch.float64, device=self.ctx.device)
+        if self.world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.SUM, group=self.group)
+        t = t.cpu().numpy()
+        return t[:3].copy(), float(t[3])
+
+    def get_spins(self):
+        """This rank's own planes (canonical order, z slowest)."""
+        return self.ctx.get_spins()
+
+    def close(self):
+        self.ctx.close()

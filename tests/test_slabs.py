@@ -1,0 +1,133 @@
+"""Slab decomposition along z: host logic on CPU (partition, neighbour ranks, the face exchange
+between ranks under gloo), and on the GPU the sharded trajectory against the oracle's single-lattice trajectory."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2106_11286_b200 import slabs
+from test_multiproc import json_lines, torchrun
+
+
+def test_partition_even_planes_cover_the_lattice():
+    assert slabs.partition(464, 1) == [(0, 464)]
+    assert slabs.partition(464, 8) == [(58 * r, 58) for r in range(8)]
+    assert slabs.partition(20, 4) == [(0, 6), (6, 6), (12, 4), (16, 4)]
+    for Lz in (2, 4, 10, 16, 30, 464):
+        for G in range(1, Lz // 2 + 1):
+            p = slabs.partition(Lz, G)
+            assert p[0][0] == 0 and all(nz >= 2 and nz % 2 == 0 and z0 % 2 == 0 for z0, nz in p)
+            assert all(p[r][0] + p[r][1] == p[r + 1][0] for r in range(G - 1)) and p[-1][0] + p[-1][1] == Lz
+            assert max(nz for _, nz in p) - min(nz for _, nz in p) <= 2
+    with pytest.raises(ValueError):
+        slabs.partition(6, 4)
+    with pytest.raises(ValueError):
+        slabs.partition(7, 1)
+    assert slabs.neighbours(0, 4) == (3, 1) and slabs.neighbours(3, 4) == (2, 0) and slabs.neighbours(0, 1) == (0, 0)
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_face_exchange_between_ranks_gloo(world):
+    res = torchrun([os.path.join("tests", "gloo_slab_worker.py")], nproc=world)
+    assert res.returncode == 0, res.stderr[-2000:]
+    (r,) = json_lines(res.stdout)
+    assert r["world"] == world and r["sum"] == [sum(range(1, world + 1)), 0.0, 0.0, -2.0 * sum(range(1, world + 1))]
+    for rank, ghosts in enumerate(r["ghosts"]):
+        down, up = (rank - 1) % world, (rank + 1) % world
+        for colour in (0, 1):
+            for k in range(3):
+                # low ghost plane <- the lower neighbour's high boundary plane; high ghost <- the upper neighbour's low one
+                assert set(ghosts["%d0%d" % (colour, k)]) == {1000.0 * down + 100 * colour + 10 * 1 + k}
+                assert set(ghosts["%d1%d" % (colour, k)]) == {1000.0 * up + 100 * colour + 10 * 0 + k}
+
+
+# ---- GPU: the slabs together walk the oracle's trajectory of the whole lattice -----------------------------------------
+def _oracle(shape, K, e, seed):
+    import oracle
+    lat = oracle.Lattice.sc(*shape)
+    lat.set_uniform_anisotropy(K, e)
+    return lat, oracle.State32(lat, 1.0, seed)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("shape,n_slabs,K,e,options", [
+    ((16, 12, 16), 2, 0.0, (0.0, 0.0, 1.0), {}),
+    ((16, 12, 20), 4, 0.05, (0.0, 0.0, 1.0), {}),                 # unequal slabs 6, 6, 4, 4
+    ((8, 4, 4), 2, 0.3, (0.6, 0.0, 0.8), {}),                     # two-plane slabs: every plane is a boundary plane
+    ((16, 12, 12), 1, 0.05, (0.0, 0.0, 1.0), {}),                 # one slab feeding its own ghost planes
+    ((40, 14, 24), 3, 0.01, (0.0, 0.0, 1.0), {"sc_kernel": 1}),   # warp-specialised kernel, ragged tiles
+    ((464, 8, 8), 2, 0.01, (0.0, 0.0, 1.0), {"sc_kernel": 1}),    # config 4's rows (7-row tiles)
+])
+def test_slabs_walk_the_single_lattice_trajectory(shape, n_slabs, K, e, options):
+    from hbtest import spins_equal
+    seed = 12345
+    lat, st = _oracle(shape, K, e, seed)
+    sl = slabs.LocalSlabs(*shape, n_slabs, J=1.0, K=K, e=e, seed=seed, options=options)
+    st.init_random()
+    sl.init_random()                       # Philox draw 1 keyed by the global site id
+    assert spins_equal(sl.get_spins(), st.get_spins())
+    for T, k in ((1.44, 1), (1.44, 3), (0.5, 2)):
+        sl.sweep(T, k)
+        st.sweep(T, k)
+        assert spins_equal(sl.get_spins(), st.get_spins()), (shape, n_slabs, T)
+        Mg, Eg = sl.measure()
+        Mo, Eo = st.measure()[:2]
+        assert np.max(np.abs(Mg - np.asarray(Mo))) <= 1e-7 and abs(Eg - Eo) <= 1e-6 * lat.n
+    # a state handed in from the host, and the checkpointed sweep counter, continue the same trajectory
+    sx, sy, sz = st.get_spins()
+    sl2 = slabs.LocalSlabs(*shape, n_slabs, J=1.0, K=K, e=e, seed=seed, options=options)
+    sl2.set_spins(sx, sy, sz)
+    for c in sl2.ctxs:
+        c.sweep_count = st.sweep_count
+    sl2.sweep(1.2, 2)
+    st.sweep(1.2, 2)
+    assert spins_equal(sl2.get_spins(), st.get_spins())
+    sl.close()
+    sl2.close()
+
+
+@pytest.mark.gpu
+def test_slab_contexts_refuse_whole_lattice_calls():
+    import paper_2106_11286_b200 as hb
+    ctx = hb.Context(hb.Lattice("sc", 8, 4, 4, slab=(4, 12)), 1.0, 0.0, (0, 0, 1), 1)
+    ctx.init_random()
+    assert ctx.n == 8 * 4 * 4
+    with pytest.raises(hb.HbError):
+        ctx.sweep(1.0, 1)
+    with pytest.raises(hb.HbError):
+        ctx.sweep_series(1.0, 2)
+    with pytest.raises(hb.HbError):
+        ctx.slab_pass(1.0, 2)
+    ctx.close()
+    for bad in [dict(slab=(3, 12)), dict(slab=(4, 6)), dict(slab=(0, 11))]:
+        with pytest.raises(hb.HbError):
+            hb.Context(hb.Lattice("sc", 8, 4, 4, **bad), 1.0, 0.0, (0, 0, 1), 1)
+    with pytest.raises(hb.HbError):
+        hb.Context(hb.Lattice("bcc", 4, 4, 4, slab=(0, 8)), 1.0, 0.0, (0, 0, 1), 1)
+    whole = hb.Context(hb.Lattice("sc", 8, 4, 4), 1.0, 0.0, (0, 0, 1), 1)
+    with pytest.raises(hb.HbError):
+        whole.slab_pass(1.0, 0)
+    whole.close()
+
+
+@pytest.mark.gpu
+def test_dist_slab_single_rank():
+    # world_size 1: the rank's slab is the whole lattice and feeds its own ghost planes; all_reduce is skipped
+    import torch.distributed as dist
+    from hbtest import spins_equal
+    from test_multiproc import free_port
+    dist.init_process_group("gloo", init_method="tcp://127.0.0.1:%d" % free_port(), rank=0, world_size=1)
+    try:
+        lat, st = _oracle((16, 8, 8), 0.05, (0.0, 0.0, 1.0), 7)
+        d = slabs.DistSlab(16, 8, 8, 1.0, 0.05, (0.0, 0.0, 1.0), 7)
+        d.init_random()
+        st.init_random()
+        d.sweep(1.3, 4)
+        st.sweep(1.3, 4)
+        assert spins_equal(d.get_spins(), st.get_spins())
+        M, E = d.measure()
+        Mo, Eo = st.measure()[:2]
+        assert np.max(np.abs(M - np.asarray(Mo))) <= 1e-7 and abs(E - Eo) <= 1e-6 * lat.n
+        d.close()
+    finally:
+        dist.destroy_process_group()
