@@ -221,6 +221,69 @@ def run_reference(args, cfg, name):
     }))
 
 
+def run_slabs(args, cfg, rank, world, device, barrier):
+    """--multi slabs: ONE lattice of the workload's size cut into `world` z-slabs (paper_2106_11286_b200.slabs.DistSlab):
+    a step is the same SWEEPS_PER_STEP sweeps + one measurement of the WHOLE lattice; every colour pass is followed by the
+    exchange of its two faces with the z-neighbours (NCCL send/recv; a single rank feeds its own ghost planes) and the
+    measurement by one all_reduce of 4 doubles.  Timed on the device, MAX over ranks; total work is fixed: strong scaling."""
+    import torch
+    import torch.distributed as dist
+    from paper_2106_11286_b200 import slabs
+    if cfg["kind"] != "sc":
+        raise SystemExit("--multi slabs: simple cubic workloads (c1, c4)")
+    L = cfg["L"]
+    Lx, Ly, Lz = (L, L, L) if isinstance(L, int) else L
+    options = dict((kv.split("=", 1)[0], int(kv.split("=", 1)[1])) for kv in args.option)
+    sl = slabs.DistSlab(Lx, Ly, Lz, cfg["J"], cfg["K"], cfg["e"], cfg["seed"], device=device, options=options)
+    sl.init_random() if cfg["start"] == "random" else sl.init_aligned(cfg["e"])
+    T = cfg["T"][0]
+    for _ in range(args.warmup):
+        sl.sweep(T, SWEEPS_PER_STEP)
+        sl.measure()
+    sampler = ClockSampler(int(device.split(":")[1])) if rank == 0 else None
+    if sampler:
+        time.sleep(0.5)
+        sl.sweep(T, min(SWEEPS_PER_STEP, 20))
+    l0, _ = sl.ctx.counters()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        sl.sweep(T, SWEEPS_PER_STEP)
+        M, E = sl.measure()
+    e1.record()
+    barrier()
+    l1, _ = sl.ctx.counters()
+    clocks = sampler.stop() if sampler else None
+    (ms,), (launches,) = reduce_over_ranks([e0.elapsed_time(e1)], [l1 - l0], device)
+    if rank == 0:
+        n = sl.n
+        value = float(n) * SWEEPS_PER_STEP * args.steps / (ms * 1e-3) / 1e9
+        peak, peak_src = measured_peaks()
+        achieved = 36.0 * value     # GB/s: algorithmic 36 B per attempted update, copies and exchanges inside the time
+        face_bytes = 2 * 2 * 3 * (Lx * Ly // 2) * 4   # per sweep and slab: 2 colours x 2 faces x 3 components, sent (and received)
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": args.workload, "lattice": "sc %s" % L, "n_spins": n, "colours": 2, "J": cfg["J"], "K": cfg["K"],
+                       "T": T, "start": cfg["start"], "seed": cfg["seed"], "sweeps_per_step": SWEEPS_PER_STEP,
+                       "measurements_per_step": 1, "options": options,
+                       "multi_gpu": "slabs along z: %s planes per rank, %d bytes of faces sent per rank and sweep, "
+                                    "one all_reduce of 32 bytes per measurement" % ([nz for _, nz in slabs.partition(Lz, world)], face_bytes),
+                       "l2": "state %.0f MB per rank" % (12.0 * n / world / 1e6)},
+            "ns_per_update": 1.0 / value, "clocks": clocks, "e2e": None, "gpu_launches": launches,
+            "M": [float(x) for x in M], "E_per_spin": E / n,
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak * world, "unit": "GB/s", "frac": achieved / (peak * world),
+                         "traffic": None, "kernel": "k_sweep_sc_ws" if sl.ctx.get_option("sc_kernel") == 1 else "k_sweep_sc",
+                         "peak_source": peak_src + " x n_gpus", "algorithmic_bytes_per_update": 36.0,
+                         "note": "whole step (colour passes + face exchanges + measurement) against the aggregate peak"},
+            "cpu_baseline": None}))
+    sl.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -230,6 +293,9 @@ def main():
     ap.add_argument("--workload", default="c4", help="c1..c5 (BASELINE.json configs); the headline is c4")
     ap.add_argument("--option", action="append", default=[], metavar="NAME=VALUE",
                     help="hb_set_option on the context (tuning knobs of DESIGN.md section 6), repeatable")
+    ap.add_argument("--multi", default="replicas", choices=["replicas", "slabs"],
+                    help="N > 1: independent replicas (default, weak scaling) or ONE lattice cut into z-slabs with a face "
+                         "exchange per colour (strong scaling; simple cubic workloads; DESIGN.md section 9)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -258,6 +324,9 @@ def main():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
+
+    if args.multi == "slabs":
+        return run_slabs(args, cfg, rank, world, device, barrier)
 
     ctx = make_context(cfg, rank, device)
     options = {}

@@ -151,7 +151,10 @@ class DistSlab:
         import torch.distributed as dist
         from .binding import Context, Lattice
         self.group = group
-        self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
+        if dist.is_available() and dist.is_initialized():
+            self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
+        else:                                   # no process group: the whole lattice as one slab
+            self.rank, self.world = 0, 1
         self.shape = (Lx, Ly, Lz)
         self.z0, self.nz = partition(Lz, self.world)[self.rank]
         self.ctx = Context(Lattice("sc", Lx, Ly, self.nz, slab=(self.z0, Lz)), J, K, e, seed,
