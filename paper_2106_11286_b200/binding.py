@@ -16,6 +16,7 @@ EXPORTS = [
     "hb_sizes", "hb_create", "hb_destroy", "hb_init_random", "hb_init_aligned", "hb_set_spins", "hb_get_spins",
     "hb_sweep", "hb_measure", "hb_sweep_series", "hb_sweep_record", "hb_sweep_count", "hb_set_sweep_count",
     "hb_sweep_each", "hb_measure_each", "hb_sweep_series_each", "hb_select_replica",
+    "hb_slab_pass", "hb_slab_next_sweep", "hb_slab_face",
     "hb_get_colouring", "hb_counters", "hb_set_option", "hb_get_option", "hb_lattice_fcc_sphere", "hb_lattice_free",
     "hb_strerror", "hb_error_detail",
 ]
