@@ -84,9 +84,10 @@ int make_plan(const hb_lattice* lat, Plan& p, std::string& why) {
   }
   if (p.n < 1) { why = "lattice has no sites"; return HB_EINVAL; }
   if (p.n > 0xFFFFFFFFll) { why = "more than 2^32-1 sites (site ids are 32-bit Philox counter words)"; return HB_EINVAL; }
-  if (p.nnz >= 0x7FFFFFFFll) { why = "more than 2^31-2 neighbour entries"; return HB_EINVAL; }
   if ((lat->K_site == nullptr) != (lat->e_site == nullptr)) { why = "K_site and e_site go together"; return HB_EINVAL; }
   p.per_site = lat->K_site != nullptr;
+  // only the table engine materialises the neighbour entries (32-bit offsets); the implicit kinds go up to 2^32-1 sites
+  if ((p.per_site || k == HB_CSR) && p.nnz >= 0x7FFFFFFFll) { why = "more than 2^31-2 neighbour entries"; return HB_EINVAL; }
   // implicit indexing for the periodic kinds; the table engine for CSR input and per-site anisotropy
   p.engine = p.per_site || k == HB_CSR ? ENGINE_CSR : (k == HB_SC ? ENGINE_SC : ENGINE_BRAVAIS);
   p.R = lat->n_replicas > 1 ? lat->n_replicas : 1;

@@ -131,3 +131,34 @@ def test_dist_slab_single_rank():
         d.close()
     finally:
         dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+def test_more_than_2_31_sites_whole_lattice_equals_its_slabs():
+    # 1600 x 1600 x 840 = 2,150,400,000 sites (> 2^31; 25.8 GB of spins): a property that holds at any size -- the whole
+    # lattice in one context and the same lattice as two slabs (1.08e9 sites each, other index ranges in every kernel)
+    # walk the same trajectory, so M and E agree to the rounding of the final fp64 sums.  The paper stops at 512^3
+    # ("1024^3 ... each array would occupy 4.3 GB"); site ids are 32-bit Philox counter words, so the
+    # limit here is 2^32 - 1 sites.
+    import torch
+    import paper_2106_11286_b200 as hb
+    if torch.cuda.mem_get_info()[1] < 100e9:
+        pytest.skip("needs ~70 GB of device memory")
+    shape, T = (1600, 1600, 840), 1.44
+    ctx = hb.Context(hb.Lattice("sc", *shape), 1.0, 0.01, (0.0, 0.0, 1.0), 1)
+    ctx.init_random()
+    ctx.sweep(T, 2)
+    M, E = ctx.measure()
+    n = ctx.n
+    ctx.close()
+    del ctx
+    torch.cuda.empty_cache()
+    assert n == 2150400000 and np.linalg.norm(M) < 1e-3 and -1.0 < E / n < -0.3   # two sweeps after a random start
+    sl = slabs.LocalSlabs(*shape, 2, J=1.0, K=0.01, e=(0.0, 0.0, 1.0), seed=1)
+    sl.init_random()
+    sl.sweep(T, 2)
+    Ms, Es = sl.measure()
+    sl.close()
+    del sl
+    torch.cuda.empty_cache()
+    assert np.max(np.abs(Ms - M)) <= 1e-12 and abs(Es - E) <= 1e-12 * abs(E)
