@@ -415,6 +415,14 @@ def main():
                 "algorithmic_bytes_per_update": bytes_per_update, "bytes_per_launch": bytes_per_launch,
                 "avg_launch_ms": avg_launch_s * 1e3, "frac_of_8TBs_nominal": achieved / 8000.0}
 
+    # the second ceiling: the attempt arithmetic alone, no memory traffic, measured now on this device
+    # in a 1 s run (so at the clock a long run holds); per GPU, like `achieved`
+    from paper_2106_11286_b200 import probe_alu
+    alu_peak = probe_alu(1.0, device) / 1e9
+    roofline["alu"] = {"bound": "alu", "achieved": value / world, "peak": alu_peak, "unit": UNIT, "frac": value / world / alu_peak,
+                       "peak_source": "hb_probe_alu: Philox + proposal + neighbour sum on registers + delta-H + acceptance, "
+                                      "4 attempts per thread as two packed pairs, 256-thread blocks, 4 per SM, measured in this run"}
+
     cpu = None if args.no_cpu_baseline else run_cpu_baseline(cfg)
     # acceptance rate of one more sweep of the state the run ended in (reported with every timed config)
     acceptance = float(ctx.sweep_record(T).mean())

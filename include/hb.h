@@ -175,6 +175,12 @@ int hb_slab_pass(hb_ctx* ctx, float T, int32_t colour);
 int hb_slab_next_sweep(hb_ctx* ctx);
 int hb_slab_face(hb_ctx* ctx, int32_t colour, int32_t side, int32_t ghost, size_t offset_floats[3], size_t* count_floats);
 
+/* Diagnostic: the rate (attempted updates per second) at which this device executes the attempt arithmetic alone --
+ * Philox, proposal, neighbour sum on registers, delta-H, acceptance; no memory traffic -- in launches issued back to back on
+ * `cuda_stream` for about `seconds` (0 < seconds <= 10; the second half is timed, so the clock is the one a long run
+ * holds).  It is the arithmetic ceiling of the colour kernels on this chip.  Synchronises. */
+int hb_probe_alu(void* cuda_stream, double seconds, double* updates_per_second);
+
 /* Tuning knobs, by name (DESIGN.md section 6 lists them); unknown names give HB_EINVAL. */
 int hb_set_option(hb_ctx* ctx, const char* name, int64_t value);
 int hb_get_option(hb_ctx* ctx, const char* name, int64_t* value);

@@ -16,7 +16,7 @@ EXPORTS = [
     "hb_sizes", "hb_create", "hb_destroy", "hb_init_random", "hb_init_aligned", "hb_set_spins", "hb_get_spins",
     "hb_sweep", "hb_measure", "hb_sweep_series", "hb_sweep_record", "hb_sweep_count", "hb_set_sweep_count",
     "hb_sweep_each", "hb_measure_each", "hb_sweep_series_each", "hb_select_replica",
-    "hb_slab_pass", "hb_slab_next_sweep", "hb_slab_face",
+    "hb_slab_pass", "hb_slab_next_sweep", "hb_slab_face", "hb_probe_alu",
     "hb_get_colouring", "hb_counters", "hb_set_option", "hb_get_option", "hb_lattice_fcc_sphere", "hb_lattice_free",
     "hb_strerror", "hb_error_detail",
 ]
@@ -77,6 +77,7 @@ def load_library():
         "hb_slab_pass": [vp, f32, i32],
         "hb_slab_next_sweep": [vp],
         "hb_slab_face": [vp, i32, i32, i32, P(C.c_size_t), P(C.c_size_t)],
+        "hb_probe_alu": [vp, C.c_double, P(C.c_double)],
         "hb_sweep_count": [vp, P(u64)],
         "hb_set_sweep_count": [vp, u64],
         "hb_get_colouring": [vp, vp, P(i32)],
@@ -164,6 +165,18 @@ class Lattice:
         if self.K_site is not None:
             s.K_site, s.e_site = _ptr(self.K_site), _ptr(self.e_site)
         return s
+
+
+def probe_alu(seconds=0.5, device="cuda:0"):
+    """hb_probe_alu: attempted updates per second of the attempt arithmetic alone (no memory traffic) on `device`."""
+    import torch
+    L = load_library()
+    torch.cuda.set_device(torch.device(device))
+    v = C.c_double()
+    rc = L.hb_probe_alu(torch.cuda.current_stream(torch.device(device)).cuda_stream, float(seconds), C.byref(v))
+    if rc != 0:
+        raise HbError(rc, "hb_probe_alu", L.hb_strerror(rc).decode())
+    return v.value
 
 
 def sizes(lat):

@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libhb.so")
-SOURCES = ["hb_api.cpp", "hb_lattice.cpp", "hb_kernels.cu", "hb_bravais.cu", "hb_ell.cu", "hb_sc_ws.cu"]
+SOURCES = ["hb_api.cpp", "hb_lattice.cpp", "hb_kernels.cu", "hb_bravais.cu", "hb_ell.cu", "hb_sc_ws.cu", "hb_probe.cu"]
 HEADERS = ["hb_internal.h", "hb_device.cuh", os.path.join("..", "..", "include", "hb.h")]
 
 NVCC_FLAGS = [

@@ -597,3 +597,12 @@ def test_replicas_match_independent_oracle_runs():
         hb.Context(hb.Lattice("sc", 32, n_replicas=2))                # 32768 sites: a colour pass does not fit one block
     with pytest.raises(hb.HbError):
         hb.Context(hb.Lattice("bcc", 4, n_replicas=2))
+
+
+def test_alu_probe_reports_a_plausible_ceiling():
+    # hb_probe_alu: the attempt arithmetic alone; any colour kernel must stay below it, and it cannot exceed the issue
+    # bound of 20 IMAD.WIDE per attempt (one per 4 clocks per SM sub-partition: 592 x 32 lanes x 1.965 GHz / 80)
+    rate = hb.probe_alu(0.2)
+    assert 2e10 < rate < 592 * 32 * 1.965e9 / 80
+    with pytest.raises(hb.HbError):
+        hb.probe_alu(0.0)
