@@ -149,6 +149,7 @@ struct hb_ctx {
   cudaGraphExec_t gexec[2] = {nullptr, nullptr};   // [0] plain sweeps, [1] every sweep measured into the series buffer
   float g_beta[2] = {0.0f, 0.0f};
   bool g_dirty[2] = {true, true};
+  int pdl = 1;                 // colour kernels are launched with programmatic stream serialisation (option pdl)
   int32_t slab_Lz = 0, slab_z0 = 0;   // > 0: this context is a slab of a larger lattice (planes 0 and Lz-1 of sc are ghosts)
   int sc_coop = -1;            // persistent multi-sweep kernel: -1 auto, 0 off, 1 / 2 forced (see hb_set_option)
   bool fused_measure = true;   // sc: the last sweep of hb_sweep also reduces M and E
@@ -213,6 +214,7 @@ SweepParams params(const hb_ctx* c, float beta) {
   p.seed_lo = (uint32_t)c->seed; p.seed_hi = (uint32_t)(c->seed >> 32);
   p.sweep_lo = (uint32_t)c->sweep; p.sweep_hi = (uint32_t)(c->sweep >> 32);
   p.sweep_dev = nullptr;
+  p.pdl = c->pdl;
   return p;
 }
 
@@ -559,6 +561,11 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
     }
     c->ws_variant = sc_ws_variant_supported(c->sc, 4) ? 4 : 2;   // 7-row tiles where the rows fit them (c4: +2 %), else 4-row tiles
   }
+
+  // programmatic stream serialisation of the colour launches, where it was measured to pay: the sc
+  // kernels at every size (+1.5 to +5 % below L = 256), bcc / fcc on large lattices only (fcc 128^3 +1.5 %, bcc 64^3 -18 %:
+  // the early blocks of the next colour crowd the single wave of a small launch), not the table kernels (-1 %)
+  c->pdl = (P.engine == ENGINE_SC || (P.engine == ENGINE_BRAVAIS && P.n >= (int64_t(1) << 22))) ? 1 : 0;
 
   // ---- device memory --------------------------------------------------------------------------
   if (bufs) {
@@ -1082,6 +1089,12 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
     c->fused_measure = value != 0;
     return HB_OK;
   }
+  if (s == "pdl") {
+    if (value != 0 && value != 1) return fail(c, HB_EINVAL, "pdl: 0 or 1");
+    c->pdl = (int)value;
+    c->g_dirty[0] = c->g_dirty[1] = true;   // captured launches carry the attribute
+    return HB_OK;
+  }
   if (s == "csr_block") {
     if (value < 32 || value > 256 || value % 32) return fail(c, HB_EINVAL, "csr_block: multiple of 32 in [32,256]");
     c->csr_block = (int)value;
@@ -1141,6 +1154,7 @@ int hb_get_option(hb_ctx* c, const char* name, int64_t* value) {
   if (!c || !name || !value) return HB_EINVAL;
   const std::string s(name);
   if (s == "csr_block") *value = c->csr_block;
+  else if (s == "pdl") *value = c->pdl;
   else if (s == "fused_measure") *value = c->fused_measure ? 1 : 0;
   else if (s == "sc_coop") *value = c->sc_coop;
   else if (s == "graph") *value = c->graph_mode;

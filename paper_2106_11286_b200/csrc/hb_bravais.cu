@@ -272,8 +272,8 @@ cudaError_t go(cudaStream_t st, float* s, const BrLayout& L, const ScTile& t, co
                const Meas& m = Meas{nullptr, 0}) {
   const int HV = L.Lx / V;
   dim3 grid((HV + t.JX - 1) / t.JX, (L.Ly + t.TY - 1) / t.TY, (L.Lz + t.ZT - 1) / t.ZT);
-  k_sweep_bravais<KIND, B, V, ANISO, DIAG, MEAS><<<grid, t.JX * t.TY, 0, st>>>(s + (size_t)B * L.nc, s, L, t, p, d, m);
-  return cudaGetLastError();
+  return launch_colour_kernel(k_sweep_bravais<KIND, B, V, ANISO, DIAG, MEAS>, grid, dim3(t.JX * t.TY), 0, st, p.pdl != 0,
+                              s + (size_t)B * L.nc, s, L, t, p, d, m);
 }
 
 // The tuned shape (V = 4, no diagnostics) carries the three anisotropy specialisations; the

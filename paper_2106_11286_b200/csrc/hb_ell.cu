@@ -123,9 +123,8 @@ cudaError_t sweep_go(cudaStream_t st, float* s, const EllDev& g, uint32_t begin,
                      int block, const Diag& d) {
   float4* S = reinterpret_cast<float4*>(s);
   const int grid = (int)((count + block - 1) / block);
-  if (d.accept || d.n_accept) k_sweep_ell<MD, true><<<grid, block, 0, st>>>(S, g, begin, count, p, d);
-  else k_sweep_ell<MD, false><<<grid, block, 0, st>>>(S, g, begin, count, p, d);
-  return cudaGetLastError();
+  if (d.accept || d.n_accept) return launch_colour_kernel(k_sweep_ell<MD, true>, dim3(grid), dim3(block), 0, st, p.pdl != 0, S, g, begin, count, p, d);
+  return launch_colour_kernel(k_sweep_ell<MD, false>, dim3(grid), dim3(block), 0, st, p.pdl != 0, S, g, begin, count, p, d);
 }
 
 }  // namespace

@@ -16,7 +16,24 @@ struct SweepParams {
   // Replayed launches (CUDA graph) cannot carry the sweep counter in their parameters: with
   // sweep_dev != nullptr the counter is *sweep_dev + sweep_lo (sweep_lo = index of the sweep inside the graph)
   const unsigned long long* sweep_dev;
+  // launch the colour kernel with programmatic stream serialisation: its blocks may become resident
+  // while the previous kernel of the stream drains; every colour kernel waits (griddepcontrol.wait, in resolve_sweep)
+  // for that kernel to complete before it touches memory
+  int32_t pdl;
 };
+
+// kern<<<grid, block, smem, st>>>(args...), with the programmatic-serialisation attribute when pdl is set
+template <class... KArgs, class... Args>
+inline cudaError_t launch_colour_kernel(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl,
+                                        Args&&... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
 
 // simple cubic, colour-split storage
 struct ScLayout {

@@ -548,8 +548,7 @@ static cudaError_t sweep_sc_impl(cudaStream_t st, float* s, ScLayout L, ScTile t
   const float* b = s + (size_t)(1 - colour) * L.half;
   dim3 grid;
   sc_launch_shape(L, t, V, grid, threads);
-  kern<<<grid, threads, 0, st>>>(a, a + n, a + 2 * n, b, b + n, b + 2 * n, L, t, p, colour, d, m);
-  return cudaGetLastError();
+  return launch_colour_kernel(kern, grid, dim3(threads), 0, st, p.pdl != 0, a, a + n, a + 2 * n, b, b + n, b + 2 * n, L, t, p, colour, d, m);
 }
 
 template <int V, bool DIAG>
@@ -633,10 +632,8 @@ cudaError_t launch_sweep_csr(cudaStream_t st, float* s, CsrDev g, uint32_t list_
   const size_t n = g.n;
   const int grid = (int)((list_count + block - 1) / block);
   if (d.accept || d.n_accept)
-    k_sweep_csr<true><<<grid, block, 0, st>>>(s, s + n, s + 2 * n, g, list_begin, list_count, p, d);
-  else
-    k_sweep_csr<false><<<grid, block, 0, st>>>(s, s + n, s + 2 * n, g, list_begin, list_count, p, d);
-  return cudaGetLastError();
+    return launch_colour_kernel(k_sweep_csr<true>, dim3(grid), dim3(block), 0, st, p.pdl != 0, s, s + n, s + 2 * n, g, list_begin, list_count, p, d);
+  return launch_colour_kernel(k_sweep_csr<false>, dim3(grid), dim3(block), 0, st, p.pdl != 0, s, s + n, s + 2 * n, g, list_begin, list_count, p, d);
 }
 
 cudaError_t launch_set_counter(cudaStream_t st, unsigned long long* counter, unsigned long long value, bool add) {

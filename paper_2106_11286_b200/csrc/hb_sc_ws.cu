@@ -280,8 +280,7 @@ cudaError_t ws_go(cudaStream_t st, float* s, const ScLayout& L, int n_zc, int gr
   const int threads = 32 + 32 * ((TY * (L.H / 4) + 31) / 32);
   float* a = s + (size_t)colour * L.half;
   const float* b = s + (size_t)(1 - colour) * L.half;
-  kern<<<grid, threads, S::BYTES, st>>>(a, b, L, w, p, colour, m);
-  return cudaGetLastError();
+  return launch_colour_kernel(kern, dim3(grid), dim3(threads), S::BYTES, st, p.pdl != 0, a, b, L, w, p, colour, m);
 }
 
 template <int TY, int ROWB, int kNB, int MINB>

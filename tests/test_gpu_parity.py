@@ -532,8 +532,8 @@ def test_kernel_variants_agree_on_random_shapes():
         H = Lx // 2
         ref, (Mr, Er) = run({"graph": 0, "sc_coop": 0})
         variants = [{"graph": 0, "sc_coop": 0, "sc_jx": int(rng.integers(1, H // 4 + 1)), "sc_ty": int(rng.integers(1, 9)),
-                     "sc_zt": int(rng.integers(1, Lz + 1))},
-                    {"graph": 1, "sc_coop": 0},
+                     "sc_zt": int(rng.integers(1, Lz + 1)), "pdl": it % 2},
+                    {"graph": 1, "sc_coop": 0, "pdl": (it + 1) % 2},
                     {"graph": 0, "sc_coop": 2},
                     {"graph": int(rng.integers(0, 2)), "sc_kernel": 1, "sc_ws_zt": int(rng.integers(0, Lz + 1)),
                      "sc_ws_ctas": int(rng.integers(1, 5)), "sc_ws_variant": int(rng.integers(0, 5 if H <= 236 else 3))}]
@@ -606,3 +606,26 @@ def test_alu_probe_reports_a_plausible_ceiling():
     assert 2e10 < rate < 592 * 32 * 1.965e9 / 80
     with pytest.raises(hb.HbError):
         hb.probe_alu(0.0)
+
+
+def test_programmatic_launches_match_the_oracle():
+    # option pdl = 1: colour kernels launched with programmatic stream serialisation (their blocks become resident while the
+    # previous colour drains and wait in griddepcontrol.wait before they read anything).  Every engine, with plain
+    # launches and with replayed graphs, many short launches back to back: the trajectory must be the oracle's.
+    for name in ("c1", "c2", "c3", "c5"):
+        cfg = W.SMALL[name]
+        for graph in (0, 1):
+            lat, st = make_oracle(cfg)
+            ctx = make_gpu(cfg)
+            ctx.set_option("pdl", 1)
+            ctx.set_option("graph", graph)
+            if cfg["kind"] == "sc":
+                ctx.set_option("sc_coop", 0)
+            assert ctx.get_option("pdl") == 1
+            start(cfg, ctx, st)
+            for T, k in ((1.5, 20), (0.7, 13)):
+                ctx.sweep(T, k)
+                st.sweep(T, k)
+                assert spins_equal(ctx.get_spins(), st.get_spins()), (name, graph)
+                _measure_close(ctx, st, lat.n)
+            ctx.close()
