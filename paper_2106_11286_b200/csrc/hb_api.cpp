@@ -562,10 +562,9 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
     c->ws_variant = sc_ws_variant_supported(c->sc, 4) ? 4 : 2;   // 7-row tiles where the rows fit them (c4: +2 %), else 4-row tiles
   }
 
-  // programmatic stream serialisation of the colour launches, where it was measured to pay: the sc
-  // kernels at every size (+1.5 to +5 % below L = 256), bcc / fcc on large lattices only (fcc 128^3 +1.5 %, bcc 64^3 -18 %:
-  // the early blocks of the next colour crowd the single wave of a small launch), not the table kernels (-1 %)
-  c->pdl = (P.engine == ENGINE_SC || (P.engine == ENGINE_BRAVAIS && P.n >= (int64_t(1) << 22))) ? 1 : 0;
+  // programmatic stream serialisation of the colour launches: mode 1 (the next launch comes in as blocks
+  // exit) was measured to pay on every engine and size; mode 2 crowds the single wave of small launches
+  c->pdl = 1;
 
   // ---- device memory --------------------------------------------------------------------------
   if (bufs) {
@@ -1090,7 +1089,7 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
     return HB_OK;
   }
   if (s == "pdl") {
-    if (value != 0 && value != 1) return fail(c, HB_EINVAL, "pdl: 0 or 1");
+    if (value < 0 || value > 2) return fail(c, HB_EINVAL, "pdl: 0 (off), 1 (the next launch comes in as blocks exit), 2 (as soon as every block has started)");
     c->pdl = (int)value;
     c->g_dirty[0] = c->g_dirty[1] = true;   // captured launches carry the attribute
     return HB_OK;
