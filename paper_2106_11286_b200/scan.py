@@ -61,8 +61,40 @@ def fit_order_parameter(T, m, t_lo, t_hi):
     return best
 
 
+def throughput_vs_size(sizes, T=1.30, K=0.01, seconds=0.5):
+    """The paper's Fig. 2 [PAPER.md lines 44-50]: time per attempted spin update against the system size, simple cubic,
+    J = 1, K = 0.01 [P:40], at T = 0.9 T_C [P:42], random start.  Each size runs sweeps for about `seconds` after as many
+    warm-up sweeps, timed with CUDA events around one hb_sweep call.  Returns rows (L, N, sweeps, Gupd/s, ns per update)."""
+    import torch
+    rows = []
+    for L in sizes:
+        ctx = make_context(dict(kind="sc", L=L, J=1.0, K=K, e=(0.0, 0.0, 1.0), seed=1, start="random"))
+        n = ctx.n
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ctx.sweep(T, 8)
+        a.record(); ctx.sweep(T, 8); b.record(); torch.cuda.synchronize()
+        sweeps = max(8, int(seconds / (a.elapsed_time(b) * 1e-3 / 8)))
+        ctx.sweep(T, sweeps)
+        a.record(); ctx.sweep(T, sweeps); b.record(); torch.cuda.synchronize()
+        dt = a.elapsed_time(b) * 1e-3
+        rows.append((L, n, sweeps, n * sweeps / dt / 1e9, dt / (n * sweeps) * 1e9))
+        ctx.close()
+        del ctx
+        torch.cuda.empty_cache()
+    return rows
+
+
 def main(argv):
-    """python -m paper_2106_11286_b200.scan c2 | --sc L [--K k] [--T a:b:n] [--equil e] [--sweeps s] [--fit t_lo:t_hi]"""
+    """python -m paper_2106_11286_b200.scan c2 | --sc L [--K k] [--T a:b:n] [--equil e] [--sweeps s] [--fit t_lo:t_hi]
+    | --fig2 [L ...]"""
+    if len(argv) > 1 and argv[1] == "--fig2":
+        sizes = [int(x) for x in argv[2:]] or [16, 32, 64, 128, 256, 464, 512, 1024]
+        print("# sc L^3, J = 1, K = 0.01, T = 1.30 (0.9 T_C), random start: attempted updates per second, time per update")
+        print("# the paper (V100, its own scheme): 1.59 ns per update for N >= 2^18 [P:50], ~100 ns on a CPU [P:42]")
+        print("# L  N  sweeps  Gupd/s  ns/update")
+        for r in throughput_vs_size(sizes):
+            print("%d  %d  %d  %.2f  %.5f" % r)
+        return
     if len(argv) > 1 and argv[1] == "--sc":
         import argparse
         ap = argparse.ArgumentParser()
