@@ -55,6 +55,8 @@ def fit_order_parameter(T, m, t_lo, t_hi):
             continue
         x, y = np.log(t[sel]), np.log(m[sel])
         beta, logA = np.polyfit(x, y, 1)
+        if not 0.05 < beta < 1.0:      # a window that fell into the disordered tail, not a power law in 1 - T/Tc
+            continue
         rms = float(np.sqrt(np.mean((y - (beta * x + logA)) ** 2)))
         if best is None or rms < best[3]:
             best = (float(Tc), float(beta), float(np.exp(logA)), rms)

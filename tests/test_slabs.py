@@ -162,3 +162,13 @@ def test_more_than_2_31_sites_whole_lattice_equals_its_slabs():
     del sl
     torch.cuda.empty_cache()
     assert np.max(np.abs(Ms - M)) <= 1e-12 and abs(Es - E) <= 1e-12 * abs(E)
+
+
+def test_order_parameter_fit_recovers_a_power_law():
+    # host logic of `scan --sc L --fit`: log-log least squares with T_C scanned (the form fitted in the paper's Fig. 3 inset)
+    from paper_2106_11286_b200.scan import fit_order_parameter
+    T = np.linspace(1.2, 1.5, 61)
+    Tc, beta, A = 1.443, 0.3645, 1.05
+    m = np.where(T < Tc, A * np.clip(1.0 - T / Tc, 1e-12, None) ** beta, 1e-3)
+    got = fit_order_parameter(T, m, 0.01, 0.1)
+    assert abs(got[0] - Tc) <= 6e-4 and abs(got[1] - beta) <= 5e-3 and abs(got[2] - A) <= 2e-2 and got[3] < 2e-3
