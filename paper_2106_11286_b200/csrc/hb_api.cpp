@@ -565,6 +565,7 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
   // programmatic stream serialisation of the colour launches: mode 1 (the next launch comes in as blocks
   // exit) was measured to pay on every engine and size; mode 2 crowds the single wave of small launches
   c->pdl = 1;
+  if (P.ell) c->csr_block = 64;   // ELL kernel: blocks of 64 threads (c5 greedy colouring 29.2 against 28.5 Gupd/s with 128)
 
   // ---- device memory --------------------------------------------------------------------------
   if (bufs) {
