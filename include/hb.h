@@ -174,6 +174,15 @@ int hb_counters(hb_ctx* ctx, uint64_t* kernel_launches, uint64_t* attempts);
 int hb_slab_pass(hb_ctx* ctx, float T, int32_t colour);
 int hb_slab_next_sweep(hb_ctx* ctx);
 int hb_slab_face(hb_ctx* ctx, int32_t colour, int32_t side, int32_t ghost, size_t offset_floats[3], size_t* count_floats);
+/* Peer stores instead of the exchange step: after hb_slab_set_peer(ctx, side, peer_spins, peer_Lz) every colour pass of
+ * this slab stores the spins it updates on its low (side 0) / high (side 1) boundary plane also into the ghost plane of
+ * the z-neighbour on that side -- peer_spins is the DEVICE address, valid on this context's device, of that neighbour's
+ * spins buffer (the same device, a peer device with access enabled, or an address opened from a CUDA IPC handle) and
+ * peer_Lz its number of own planes (same Lx, Ly).  The transfer then overlaps the pass, store by store; what remains
+ * between two passes is a barrier: no slab may start the next colour before its neighbours have finished this one
+ * (stream order on one device; a collective or an event between devices).  The ghost planes must still be filled once
+ * with hb_slab_face copies after hb_init_* / hb_set_spins.  peer_spins = NULL switches the side back to copies. */
+int hb_slab_set_peer(hb_ctx* ctx, int32_t side, void* peer_spins, int32_t peer_Lz);
 
 /* Diagnostic: the rate (attempted updates per second) at which this device executes the attempt arithmetic alone --
  * Philox, proposal, neighbour sum on registers, delta-H, acceptance; no memory traffic -- in launches issued back to back on

@@ -16,7 +16,7 @@ EXPORTS = [
     "hb_sizes", "hb_create", "hb_destroy", "hb_init_random", "hb_init_aligned", "hb_set_spins", "hb_get_spins",
     "hb_sweep", "hb_measure", "hb_sweep_series", "hb_sweep_record", "hb_sweep_count", "hb_set_sweep_count",
     "hb_sweep_each", "hb_measure_each", "hb_sweep_series_each", "hb_select_replica",
-    "hb_slab_pass", "hb_slab_next_sweep", "hb_slab_face", "hb_probe_alu",
+    "hb_slab_pass", "hb_slab_next_sweep", "hb_slab_face", "hb_slab_set_peer", "hb_probe_alu",
     "hb_get_colouring", "hb_counters", "hb_set_option", "hb_get_option", "hb_lattice_fcc_sphere", "hb_lattice_free",
     "hb_strerror", "hb_error_detail",
 ]
@@ -77,6 +77,7 @@ def load_library():
         "hb_slab_pass": [vp, f32, i32],
         "hb_slab_next_sweep": [vp],
         "hb_slab_face": [vp, i32, i32, i32, P(C.c_size_t), P(C.c_size_t)],
+        "hb_slab_set_peer": [vp, i32, vp, i32],
         "hb_probe_alu": [vp, C.c_double, P(C.c_double)],
         "hb_sweep_count": [vp, P(u64)],
         "hb_set_sweep_count": [vp, u64],
@@ -307,6 +308,14 @@ class Context:
         self._check(self._L.hb_slab_face(self._h, int(colour), int(side), int(bool(ghost)), off, C.byref(cnt)), "hb_slab_face")
         f = self._spins.view(torch.float32)
         return [f[off[k]:off[k] + cnt.value] for k in range(3)]
+
+    def slab_set_peer(self, side, peer_spins_ptr, peer_Lz):
+        """Peer stores for one side (include/hb.h): peer_spins_ptr = device address of the z-neighbour's spins buffer."""
+        self._check(self._L.hb_slab_set_peer(self._h, int(side), C.c_void_p(peer_spins_ptr), int(peer_Lz)), "hb_slab_set_peer")
+
+    @property
+    def spins_ptr(self):
+        return self._spins.data_ptr()
 
     def sweep_record(self, T):
         acc = np.zeros(self.n, np.uint8)

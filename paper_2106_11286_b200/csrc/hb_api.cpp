@@ -1032,6 +1032,21 @@ int hb_slab_face(hb_ctx* c, int32_t colour, int32_t side, int32_t ghost, size_t 
   return HB_OK;
 }
 
+int hb_slab_set_peer(hb_ctx* c, int32_t side, void* peer_spins, int32_t peer_Lz) {
+  HB_CHECK_CTX(c);
+  if (c->slab_Lz <= 0) return fail(c, HB_ESTATE, "not a slab context");
+  if (side != 0 && side != 1) return fail(c, HB_EINVAL, "side: 0 or 1");
+  if (peer_spins && (peer_Lz < 2 || (peer_Lz & 1) || (int64_t)c->sc.Lx * c->sc.Ly * ((int64_t)peer_Lz + 2) > 0xFFFFFFFFll))
+    return fail(c, HB_EINVAL, "peer_Lz: the neighbour's number of own planes (even, >= 2)");
+  const uint32_t plane = (uint32_t)c->sc.Ly * (uint32_t)c->sc.H;   // one colour of one z-plane
+  c->sc.peer[side] = static_cast<float*>(peer_spins);
+  c->sc.peer_n[side] = peer_spins ? (uint32_t)((int64_t)c->sc.Lx * c->sc.Ly * (peer_Lz + 2)) : 0u;
+  c->sc.peer_half[side] = c->sc.peer_n[side] / 2;
+  // my low face is the lower neighbour's high ghost plane (its local plane peer_Lz + 1); my high face the upper one's plane 0
+  c->sc.peer_zoff[side] = (peer_spins && side == 0) ? (uint32_t)(peer_Lz + 1) * plane : 0u;
+  return HB_OK;
+}
+
 int hb_sweep_count(hb_ctx* c, uint64_t* out) {
   if (!c || !out) return HB_EINVAL;
   *out = c->sweep;

@@ -45,6 +45,12 @@ struct ScLayout {
   // of local site s is s + site_base (mod 2^32); both 0 for a whole lattice
   uint32_t site_base;
   int32_t ghost;
+  // slab with peer stores (hb_slab_set_peer): a thread that stores an updated spin of its first / last own plane also
+  // stores it into the ghost plane of the z-neighbour's spins buffer (peer memory over NVLink, or the same device):
+  // peer[side] = that buffer (x component), peer_n / peer_half its component and colour strides, peer_zoff the offset
+  // of its ghost plane; side 0 = my low face -> the lower neighbour's high ghost plane, 1 = the other way
+  float* peer[2];
+  uint32_t peer_n[2], peer_half[2], peer_zoff[2];
 };
 
 // launch shape of the sc kernels: a block is JX x TY threads, each thread owns V

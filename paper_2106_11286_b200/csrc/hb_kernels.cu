@@ -156,6 +156,7 @@ __device__ __forceinline__ void sc_pass(float* ax, float* ay, float* az, const f
   unsigned n_acc = 0;
   double acc_mx = 0.0, acc_my = 0.0, acc_mz = 0.0, acc_en = 0.0;
   for (int32_t z = z0; z < z1; ++z) {
+    if (L.ghost && (z == 0 || z == L.Lz - 1)) continue;   // ghost planes of a slab: the z-neighbour owns them
     const uint32_t pz = (uint32_t)z * plane;
     const uint32_t pzm = (uint32_t)((z == 0) ? L.Lz - 1 : z - 1) * plane;
     const uint32_t pzp = (uint32_t)((z == L.Lz - 1) ? 0 : z + 1) * plane;
@@ -204,6 +205,17 @@ __device__ __forceinline__ void sc_pass(float* ax, float* ay, float* az, const f
       store<V>(ax + oc, sx);
       store<V>(ay + oc, sy);
       store<V>(az + oc, sz);
+      if (L.ghost) {   // slab with peer stores: the boundary planes go straight into the neighbours' ghost planes
+        const bool lo = z == 1, hi = z == L.Lz - 2;   // (distinct planes: a slab has at least two of its own)
+        float* pb = lo ? L.peer[0] : (hi ? L.peer[1] : nullptr);
+        if (pb) {
+          const uint32_t pn = lo ? L.peer_n[0] : L.peer_n[1], ph = lo ? L.peer_half[0] : L.peer_half[1];
+          float* q = pb + (size_t)colour * ph + (lo ? L.peer_zoff[0] : L.peer_zoff[1]) + yc;
+          store<V>(q, sx);
+          store<V>(q + pn, sy);
+          store<V>(q + 2 * (size_t)pn, sz);
+        }
+      }
     }
     if (MEAS) {
       // fp32 per-site terms, summed over the thread's V sites in fp32, accumulated in fp64

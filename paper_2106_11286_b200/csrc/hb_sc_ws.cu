@@ -146,13 +146,16 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
     Vec<4> nxt[3];
     if (PREF && active) { nxt[0] = load_rw<4>(gx); nxt[1] = load_rw<4>(gx + n); nxt[2] = load_rw<4>(gx + 2 * n); }
     for (int32_t s = 0; s < nz; ++s) {
+      // ghost planes of a slab are staged as neighbours but not updated: the z-neighbour owns them
+      const int32_t zs = z0 + s;
+      const bool act = active && !(L.ghost && (zs == 0 || zs == L.Lz - 1));
       Vec<4> sp[3];
       if (PREF) {
         sp[0] = nxt[0]; sp[1] = nxt[1]; sp[2] = nxt[2];
         if (active && s + 1 < nz) {
           nxt[0] = load_rw<4>(gx + plane); nxt[1] = load_rw<4>(gx + plane + n); nxt[2] = load_rw<4>(gx + plane + 2 * n);
         }
-      } else if (active) {
+      } else if (act) {
         sp[0] = load_rw<4>(gx); sp[1] = load_rw<4>(gx + n); sp[2] = load_rw<4>(gx + 2 * n);
       }
       RingPos<kNB> rc = rm; rc.next();
@@ -165,7 +168,7 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
       const int32_t p = (colour + y + z0 + s) & 1;
       const uint32_t h_off = p ? h_hi : h_lo;
       Vec<4> h[3];
-      if (active) {
+      if (act) {
 #pragma unroll
         for (int q = 0; q < 3; ++q) {
           constexpr uint32_t CB = (TY + 2) * ROWB;
@@ -195,7 +198,7 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
           mbar_arrive(emptyB + 8u * rq.slot);
         }
       }
-      if (active) {
+      if (act) {
         const uint32_t site0 = site_row + (uint32_t)p;
         bool any = false;
 #pragma unroll
@@ -215,6 +218,17 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
           store<4>(gx, sp[0]);
           store<4>(gx + n, sp[1]);
           store<4>(gx + 2 * n, sp[2]);
+          if (L.ghost) {   // slab with peer stores: the boundary planes go straight into the neighbours' ghost planes
+            const bool lo = zs == 1, hi = zs == L.Lz - 2;
+            float* pb = lo ? L.peer[0] : (hi ? L.peer[1] : nullptr);
+            if (pb) {
+              const uint32_t pn = lo ? L.peer_n[0] : L.peer_n[1], ph = lo ? L.peer_half[0] : L.peer_half[1];
+              float* q = pb + (size_t)colour * ph + (lo ? L.peer_zoff[0] : L.peer_zoff[1]) + (size_t)y * L.H + i0;
+              store<4>(q, sp[0]);
+              store<4>(q + pn, sp[1]);
+              store<4>(q + 2 * (size_t)pn, sp[2]);
+            }
+          }
         }
         if (MEAS) {
           float mx = 0.0f, my = 0.0f, mz = 0.0f, me = 0.0f;

@@ -10,7 +10,9 @@ i.e. ONE exchange step per colour: 2 faces x 3 components x (Lx Ly / 2) floats p
 site id, so the slabs together walk the single-context trajectory bit for bit (tests/test_slabs.py).
 
 * `LocalSlabs`: all slabs in this process (one GPU, or several devices of one process); faces move with
-  `Tensor.copy_` on the contexts' stream (a device-to-device / peer copy).
+  `Tensor.copy_` on the contexts' stream (a device-to-device / peer copy), or, with `peer_stores=True`, inside the colour
+  kernels themselves: a thread that stores an updated spin of a boundary plane stores it into the neighbour's ghost plane
+  too (`hb_slab_set_peer`), so the transfer overlaps the pass and only a barrier remains between two passes.
 * `DistSlab`: one slab per rank of a `torch.distributed` group (one process per GPU); faces move with
   `batch_isend_irecv` (NCCL send/recv over NVLink between GPUs), M and E with one all_reduce of 4 doubles.
 
@@ -74,7 +76,8 @@ def exchange_dist(ctx, colour, rank, world, group=None):
 class LocalSlabs:
     """n_slabs slab contexts of one periodic sc lattice in this process."""
 
-    def __init__(self, Lx, Ly, Lz, n_slabs, J=1.0, K=0.0, e=(0.0, 0.0, 1.0), seed=1, devices=None, options=None):
+    def __init__(self, Lx, Ly, Lz, n_slabs, J=1.0, K=0.0, e=(0.0, 0.0, 1.0), seed=1, devices=None, options=None,
+                 peer_stores=False):
         from .binding import Context, Lattice
         self.shape = (Lx, Ly, Lz)
         self.parts = partition(Lz, n_slabs)
@@ -85,6 +88,14 @@ class LocalSlabs:
             for k, v in (options or {}).items():
                 c.set_option(k, v)
         self.n = Lx * Ly * Lz
+        # peer stores (hb_slab_set_peer): the colour kernels write their boundary planes straight into the neighbours'
+        # ghost planes, the exchange step disappears; contexts on different devices need peer access enabled
+        self.peer_stores = bool(peer_stores)
+        if self.peer_stores:
+            for r, c in enumerate(self.ctxs):
+                down, up = neighbours(r, n_slabs)
+                c.slab_set_peer(0, self.ctxs[down].spins_ptr, self.parts[down][1])
+                c.slab_set_peer(1, self.ctxs[up].spins_ptr, self.parts[up][1])
 
     def _sync(self):
         import torch
@@ -125,9 +136,10 @@ class LocalSlabs:
                     c.slab_pass(T, colour)
                 if several:          # contexts on one stream are ordered by it; otherwise passes and copies meet here
                     self._sync()
-                exchange_local(self.ctxs, colour)
-                if several:
-                    self._sync()
+                if not self.peer_stores:
+                    exchange_local(self.ctxs, colour)
+                    if several:
+                        self._sync()
             for c in self.ctxs:
                 c.slab_next_sweep()
 

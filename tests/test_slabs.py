@@ -87,6 +87,38 @@ def test_slabs_walk_the_single_lattice_trajectory(shape, n_slabs, K, e, options)
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("shape,n_slabs,options", [
+    ((16, 12, 16), 2, {}), ((16, 12, 20), 4, {}), ((8, 4, 4), 2, {}), ((16, 12, 12), 1, {}),
+    ((40, 14, 24), 3, {"sc_kernel": 1}), ((464, 8, 8), 2, {"sc_kernel": 1}), ((64, 20, 12), 2, {"sc_kernel": 1, "sc_ws_variant": 2}),
+])
+def test_peer_stores_replace_the_exchange_step(shape, n_slabs, options):
+    # hb_slab_set_peer: the colour kernels store their boundary planes into the neighbours' ghost planes themselves; after
+    # the initial fill no face is ever copied, and the slabs still walk the oracle's trajectory of the whole lattice
+    from hbtest import spins_equal
+    K, e, seed = 0.05, (0.0, 0.6, 0.8), 99
+    lat, st = _oracle(shape, K, e, seed)
+    sl = slabs.LocalSlabs(*shape, n_slabs, J=1.0, K=K, e=e, seed=seed, options=options, peer_stores=True)
+    st.init_random()
+    sl.init_random()
+    for T, k in ((1.44, 1), (1.44, 5), (0.3, 3), (50.0, 2)):     # low and high acceptance: few / all boundary stores
+        sl.sweep(T, k)
+        st.sweep(T, k)
+        assert spins_equal(sl.get_spins(), st.get_spins()), (shape, n_slabs, T)
+        Mg, Eg = sl.measure()
+        Mo, Eo = st.measure()[:2]
+        assert np.max(np.abs(Mg - np.asarray(Mo))) <= 1e-7 and abs(Eg - Eo) <= 1e-6 * lat.n
+    # the ghost planes hold exactly the neighbours' boundary planes (what a face exchange would have written)
+    for colour in (0, 1):
+        for r, c in enumerate(sl.ctxs):
+            down, up = slabs.neighbours(r, n_slabs)
+            for mine, theirs in zip(c.slab_face(colour, 0, True), sl.ctxs[down].slab_face(colour, 1, False)):
+                assert bool((mine == theirs).all())
+            for mine, theirs in zip(c.slab_face(colour, 1, True), sl.ctxs[up].slab_face(colour, 0, False)):
+                assert bool((mine == theirs).all())
+    sl.close()
+
+
+@pytest.mark.gpu
 def test_slab_contexts_refuse_whole_lattice_calls():
     import paper_2106_11286_b200 as hb
     ctx = hb.Context(hb.Lattice("sc", 8, 4, 4, slab=(4, 12)), 1.0, 0.0, (0, 0, 1), 1)
