@@ -184,6 +184,17 @@ int hb_slab_face(hb_ctx* ctx, int32_t colour, int32_t side, int32_t ghost, size_
  * with hb_slab_face copies after hb_init_* / hb_set_spins.  peer_spins = NULL switches the side back to copies. */
 int hb_slab_set_peer(hb_ctx* ctx, int32_t side, void* peer_spins, int32_t peer_Lz);
 
+/* Device memory that another process can map (one process per GPU, peer stores between slabs): hb_device_alloc is a
+ * plain cudaMalloc on the current device (the result can be handed to hb_create in hb_buffers.spins), hb_ipc_export fills
+ * a 64-byte CUDA IPC handle for it, hb_ipc_open maps such a handle from another process into this one and returns the
+ * address to pass to hb_slab_set_peer (peer access between the two devices is enabled by the mapping), hb_ipc_close
+ * unmaps.  Memory of a caching allocator (torch) cannot be exported reliably, hence the allocator here. */
+int hb_device_alloc(size_t bytes, void** ptr);
+int hb_device_free(void* ptr);
+int hb_ipc_export(void* ptr, unsigned char handle[64]);
+int hb_ipc_open(const unsigned char handle[64], void** ptr);
+int hb_ipc_close(void* ptr);
+
 /* Diagnostic: the rate (attempted updates per second) at which this device executes the attempt arithmetic alone --
  * Philox, proposal, neighbour sum on registers, delta-H, acceptance; no memory traffic -- in launches issued back to back on
  * `cuda_stream` for about `seconds` (0 < seconds <= 10; the second half is timed, so the clock is the one a long run

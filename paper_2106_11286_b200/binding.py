@@ -17,6 +17,7 @@ EXPORTS = [
     "hb_sweep", "hb_measure", "hb_sweep_series", "hb_sweep_record", "hb_sweep_count", "hb_set_sweep_count",
     "hb_sweep_each", "hb_measure_each", "hb_sweep_series_each", "hb_select_replica",
     "hb_slab_pass", "hb_slab_next_sweep", "hb_slab_face", "hb_slab_set_peer", "hb_probe_alu",
+    "hb_device_alloc", "hb_device_free", "hb_ipc_export", "hb_ipc_open", "hb_ipc_close",
     "hb_get_colouring", "hb_counters", "hb_set_option", "hb_get_option", "hb_lattice_fcc_sphere", "hb_lattice_free",
     "hb_strerror", "hb_error_detail",
 ]
@@ -79,6 +80,11 @@ def load_library():
         "hb_slab_face": [vp, i32, i32, i32, P(C.c_size_t), P(C.c_size_t)],
         "hb_slab_set_peer": [vp, i32, vp, i32],
         "hb_probe_alu": [vp, C.c_double, P(C.c_double)],
+        "hb_device_alloc": [C.c_size_t, P(vp)],
+        "hb_device_free": [vp],
+        "hb_ipc_export": [vp, vp],
+        "hb_ipc_open": [vp, P(vp)],
+        "hb_ipc_close": [vp],
         "hb_sweep_count": [vp, P(u64)],
         "hb_set_sweep_count": [vp, u64],
         "hb_get_colouring": [vp, vp, P(i32)],
@@ -194,7 +200,9 @@ def sizes(lat):
 class Context:
     """hb_ctx with torch-owned device memory.  Method names follow include/hb.h."""
 
-    def __init__(self, lat, J=1.0, K=0.0, e=(0.0, 0.0, 1.0), seed=1, device="cuda:0", stream=None):
+    def __init__(self, lat, J=1.0, K=0.0, e=(0.0, 0.0, 1.0), seed=1, device="cuda:0", stream=None, ipc=False):
+        """ipc=True: the spins buffer comes from hb_device_alloc (a plain cudaMalloc) instead of torch's caching allocator, so
+        that another process can map it (ipc_handle / open_ipc; peer stores between slabs of different processes)."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2106_11286_b200 needs a CUDA device; there is no CPU path")
@@ -204,7 +212,19 @@ class Context:
         torch.cuda.set_device(self.device)
         self.n, spins_bytes, ws_bytes = sizes(lat)      # n: sites of ONE replica
         self.n_replicas = max(1, lat.n_replicas)
-        self._spins = torch.empty(spins_bytes, dtype=torch.uint8, device=self.device)
+        self._raw = None
+        if ipc:
+            raw = C.c_void_p()
+            rc = self._L.hb_device_alloc(spins_bytes, C.byref(raw))
+            if rc != 0:
+                raise HbError(rc, "hb_device_alloc", self._L.hb_strerror(rc).decode())
+            self._raw = raw
+
+            class _View:      # torch maps foreign device memory through the CUDA array interface, without a copy
+                __cuda_array_interface__ = {"shape": (spins_bytes,), "typestr": "|u1", "data": (raw.value, False), "version": 2}
+            self._spins = torch.as_tensor(_View(), device=self.device)
+        else:
+            self._spins = torch.empty(spins_bytes, dtype=torch.uint8, device=self.device)
         self._ws = torch.empty(ws_bytes, dtype=torch.uint8, device=self.device)
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         bufs = hb_buffers(self._spins.data_ptr(), spins_bytes, self._ws.data_ptr(), ws_bytes, self.stream.cuda_stream)
@@ -226,6 +246,30 @@ class Context:
         if getattr(self, "_h", None):
             self._L.hb_destroy(self._h)
             self._h = None
+        if getattr(self, "_raw", None):
+            import torch
+            torch.cuda.synchronize(self.device)
+            self._spins = None
+            self._L.hb_device_free(self._raw)
+            self._raw = None
+
+    def ipc_handle(self):
+        """64-byte CUDA IPC handle of the spins buffer (Context(..., ipc=True))."""
+        if not self._raw:
+            raise RuntimeError("ipc_handle needs Context(..., ipc=True)")
+        h = (C.c_ubyte * 64)()
+        self._check(self._L.hb_ipc_export(self._raw, h), "hb_ipc_export")
+        return bytes(h)
+
+    def open_ipc(self, handle):
+        """Map another process's spins buffer; returns its device address here (for slab_set_peer)."""
+        h = (C.c_ubyte * 64).from_buffer_copy(handle)
+        p = C.c_void_p()
+        self._check(self._L.hb_ipc_open(h, C.byref(p)), "hb_ipc_open")
+        return p.value
+
+    def close_ipc(self, ptr):
+        self._L.hb_ipc_close(C.c_void_p(ptr))
 
     def __del__(self):
         try:

@@ -6,6 +6,8 @@
 // blocks, 4 blocks per SM.  The rate it returns is what the instruction mix of the arithmetic contract (DESIGN.md
 // section 4) allows on this chip at the clock it holds: the "alu" roofline bench.py reports beside the HBM one
 // (DESIGN.md section 7).
+#include <cstring>
+
 #include "../../include/hb.h"
 #include "hb_device.cuh"
 #include "hb_internal.h"
@@ -76,4 +78,42 @@ extern "C" int hb_probe_alu(void* cuda_stream, double seconds, double* updates_p
   if (e1) cudaEventDestroy(e1);
   cudaFree(out);
   return rc;
+}
+
+// ---- device memory another process can map (include/hb.h) ----------------------------------------------------------------
+static_assert(sizeof(cudaIpcMemHandle_t) == 64, "CUDA IPC handle size");
+
+extern "C" int hb_device_alloc(size_t bytes, void** ptr) {
+  if (!ptr || bytes == 0) return HB_EINVAL;
+  *ptr = nullptr;
+  const cudaError_t e = cudaMalloc(ptr, bytes);
+  if (e != cudaSuccess) { cudaGetLastError(); return e == cudaErrorMemoryAllocation ? HB_ENOMEM : HB_ECUDA; }
+  return HB_OK;
+}
+
+extern "C" int hb_device_free(void* ptr) {
+  if (!ptr) return HB_OK;
+  return cudaFree(ptr) == cudaSuccess ? HB_OK : HB_ECUDA;
+}
+
+extern "C" int hb_ipc_export(void* ptr, unsigned char handle[64]) {
+  if (!ptr || !handle) return HB_EINVAL;
+  cudaIpcMemHandle_t h;
+  if (cudaIpcGetMemHandle(&h, ptr) != cudaSuccess) { cudaGetLastError(); return HB_ECUDA; }
+  memcpy(handle, &h, sizeof h);
+  return HB_OK;
+}
+
+extern "C" int hb_ipc_open(const unsigned char handle[64], void** ptr) {
+  if (!handle || !ptr) return HB_EINVAL;
+  cudaIpcMemHandle_t h;
+  memcpy(&h, handle, sizeof h);
+  *ptr = nullptr;
+  if (cudaIpcOpenMemHandle(ptr, h, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) { cudaGetLastError(); return HB_ECUDA; }
+  return HB_OK;
+}
+
+extern "C" int hb_ipc_close(void* ptr) {
+  if (!ptr) return HB_OK;
+  return cudaIpcCloseMemHandle(ptr) == cudaSuccess ? HB_OK : HB_ECUDA;
 }

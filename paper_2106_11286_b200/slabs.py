@@ -60,17 +60,23 @@ def exchange_dist(ctx, colour, rank, world, group=None):
     if world == 1:
         exchange_local([ctx], colour)
         return
-    ops = []
-    for t in ctx.slab_face(colour, 0, False):
-        ops.append(dist.P2POp(dist.isend, t, down, group))
-    for t in ctx.slab_face(colour, 1, False):
-        ops.append(dist.P2POp(dist.isend, t, up, group))
-    for t in ctx.slab_face(colour, 1, True):
-        ops.append(dist.P2POp(dist.irecv, t, up, group))
-    for t in ctx.slab_face(colour, 0, True):
-        ops.append(dist.P2POp(dist.irecv, t, down, group))
+    send = ctx.slab_face(colour, 0, False) + ctx.slab_face(colour, 1, False)      # low face down, high face up
+    recv = ctx.slab_face(colour, 1, True) + ctx.slab_face(colour, 0, True)        # from up into the high ghost, from down
+    peers_s, peers_r = [down] * 3 + [up] * 3, [up] * 3 + [down] * 3
+    # NCCL moves device memory directly (NVLink between GPUs); any other backend (gloo in the tests) gets host copies
+    staged = send[0].is_cuda and dist.get_backend(group) != "nccl"
+    if staged:
+        send_b = [t.cpu() for t in send]            # synchronises with the stream the pass ran on
+        recv_b = [t.new_empty(t.shape, device="cpu") for t in recv]
+    else:
+        send_b, recv_b = send, recv
+    ops = [dist.P2POp(dist.isend, t, p, group) for t, p in zip(send_b, peers_s)]
+    ops += [dist.P2POp(dist.irecv, t, p, group) for t, p in zip(recv_b, peers_r)]
     for req in dist.batch_isend_irecv(ops):
         req.wait()
+    if staged:
+        for dst, src in zip(recv, recv_b):
+            dst.copy_(src)
 
 
 class LocalSlabs:
@@ -157,9 +163,16 @@ class LocalSlabs:
 
 
 class DistSlab:
-    """This rank's slab of a periodic sc lattice split over the ranks of a torch.distributed group."""
+    """This rank's slab of a periodic sc lattice split over the ranks of a torch.distributed group.
 
-    def __init__(self, Lx, Ly, Lz, J=1.0, K=0.0, e=(0.0, 0.0, 1.0), seed=1, device=None, group=None, options=None):
+    peer_stores=True: every rank maps its two z-neighbours' spins buffers (CUDA IPC; on a multi-GPU node this is peer
+    memory over NVLink) and the colour kernels store their boundary planes straight into the neighbours' ghost planes
+    (hb_slab_set_peer).  No face is sent after the initial fill; between two colour passes there is only a barrier
+    (an all_reduce of one word on the stream under NCCL; a host barrier under gloo)."""
+
+    def __init__(self, Lx, Ly, Lz, J=1.0, K=0.0, e=(0.0, 0.0, 1.0), seed=1, device=None, group=None, options=None,
+                 peer_stores=False):
+        import torch
         import torch.distributed as dist
         from .binding import Context, Lattice
         self.group = group
@@ -168,16 +181,47 @@ class DistSlab:
         else:                                   # no process group: the whole lattice as one slab
             self.rank, self.world = 0, 1
         self.shape = (Lx, Ly, Lz)
-        self.z0, self.nz = partition(Lz, self.world)[self.rank]
+        parts = partition(Lz, self.world)
+        self.z0, self.nz = parts[self.rank]
+        self.peer_stores = bool(peer_stores)
         self.ctx = Context(Lattice("sc", Lx, Ly, self.nz, slab=(self.z0, Lz)), J, K, e, seed,
-                           device=device or "cuda:0")
+                           device=device or "cuda:0", ipc=self.peer_stores and self.world > 1)
         for k, v in (options or {}).items():
             self.ctx.set_option(k, v)
         self.n = Lx * Ly * Lz
+        self._mapped = {}
+        if self.peer_stores:
+            down, up = neighbours(self.rank, self.world)
+            if self.world == 1:
+                ptrs = {0: self.ctx.spins_ptr}
+            else:
+                handles = [None] * self.world
+                dist.all_gather_object(handles, self.ctx.ipc_handle(), group=group)
+                for r in {down, up}:
+                    self._mapped[r] = self.ctx.open_ipc(handles[r])
+                ptrs = self._mapped
+            self.ctx.slab_set_peer(0, ptrs[down], parts[down][1])
+            self.ctx.slab_set_peer(1, ptrs[up], parts[up][1])
+            self._nccl = self.world > 1 and dist.get_backend(group) == "nccl"
+            self._flag = torch.zeros(1, dtype=torch.int32, device=self.ctx.device) if self._nccl else None
+
+    def _pass_barrier(self):
+        """No rank starts the next colour before every rank has finished this one."""
+        if self.world == 1:
+            return                                   # one stream orders the passes
+        import torch
+        import torch.distributed as dist
+        if self._nccl:
+            dist.all_reduce(self._flag, group=self.group)    # stream-ordered: the next pass queues behind it
+        else:
+            torch.cuda.synchronize(self.ctx.device)
+            dist.barrier(group=self.group)
 
     def _fill_ghosts(self):
         for colour in (0, 1):
             exchange_dist(self.ctx, colour, self.rank, self.world, self.group)
+        if self.peer_stores:
+            self._pass_barrier()
 
     def init_random(self):
         self.ctx.init_random()
@@ -191,7 +235,10 @@ class DistSlab:
         for _ in range(n_sweeps):
             for colour in (0, 1):
                 self.ctx.slab_pass(T, colour)
-                exchange_dist(self.ctx, colour, self.rank, self.world, self.group)
+                if self.peer_stores:
+                    self._pass_barrier()
+                else:
+                    exchange_dist(self.ctx, colour, self.rank, self.world, self.group)
             self.ctx.slab_next_sweep()
 
     def measure(self):
@@ -210,4 +257,13 @@ class DistSlab:
         return self.ctx.get_spins()
 
     def close(self):
+        if self.peer_stores and self.world > 1:
+            import torch
+            import torch.distributed as dist
+            torch.cuda.synchronize(self.ctx.device)
+            dist.barrier(group=self.group)           # nobody unmaps or frees while a neighbour may still store
+            for ptr in self._mapped.values():
+                self.ctx.close_ipc(ptr)
+            self._mapped = {}
+            dist.barrier(group=self.group)
         self.ctx.close()

@@ -204,3 +204,24 @@ def test_order_parameter_fit_recovers_a_power_law():
     m = np.where(T < Tc, A * np.clip(1.0 - T / Tc, 1e-12, None) ** beta, 1e-3)
     got = fit_order_parameter(T, m, 0.01, 0.1)
     assert abs(got[0] - Tc) <= 6e-4 and abs(got[1] - beta) <= 5e-3 and abs(got[2] - A) <= 2e-2 and got[3] < 2e-3
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("mode", ["copies", "peer"])
+def test_two_processes_one_slab_each(mode):
+    # one process per slab (torchrun, gloo, both ranks on cuda:0): faces by send/recv, or -- "peer" -- no faces at all:
+    # each rank maps the other's spins buffer through CUDA IPC and the colour kernels store into its ghost planes
+    import base64
+    from hbtest import spins_equal
+    shape = (16, 12, 16)
+    res = torchrun([os.path.join("tests", "gloo_slab_gpu_worker.py"), mode] + [str(x) for x in shape], nproc=2, timeout=600)
+    assert res.returncode == 0, res.stderr[-3000:]
+    (r,) = json_lines(res.stdout)
+    lat, st = _oracle(shape, 0.05, (0.0, 0.6, 0.8), 4242)
+    st.init_random()
+    st.sweep(1.44, 3)
+    st.sweep(0.4, 2)
+    got = [np.concatenate([np.frombuffer(base64.b64decode(part[k]), np.float32) for part in r["spins"]]) for k in range(3)]
+    assert spins_equal(got, st.get_spins())
+    Mo, Eo = st.measure()[:2]
+    assert np.max(np.abs(np.asarray(r["M"]) - np.asarray(Mo))) <= 1e-7 and abs(r["E"] - Eo) <= 1e-6 * lat.n
