@@ -234,7 +234,8 @@ def run_slabs(args, cfg, rank, world, device, barrier):
     L = cfg["L"]
     Lx, Ly, Lz = (L, L, L) if isinstance(L, int) else L
     options = dict((kv.split("=", 1)[0], int(kv.split("=", 1)[1])) for kv in args.option)
-    sl = slabs.DistSlab(Lx, Ly, Lz, cfg["J"], cfg["K"], cfg["e"], cfg["seed"], device=device, options=options)
+    sl = slabs.DistSlab(Lx, Ly, Lz, cfg["J"], cfg["K"], cfg["e"], cfg["seed"], device=device, options=options,
+                        peer_stores=args.slab_exchange == "peer")
     sl.init_random() if cfg["start"] == "random" else sl.init_aligned(cfg["e"])
     T = cfg["T"][0]
     for _ in range(args.warmup):
@@ -269,8 +270,11 @@ def run_slabs(args, cfg, rank, world, device, barrier):
             "config": {"workload": args.workload, "lattice": "sc %s" % L, "n_spins": n, "colours": 2, "J": cfg["J"], "K": cfg["K"],
                        "T": T, "start": cfg["start"], "seed": cfg["seed"], "sweeps_per_step": SWEEPS_PER_STEP,
                        "measurements_per_step": 1, "options": options,
-                       "multi_gpu": "slabs along z: %s planes per rank, %d bytes of faces sent per rank and sweep, "
-                                    "one all_reduce of 32 bytes per measurement" % ([nz for _, nz in slabs.partition(Lz, world)], face_bytes),
+                       "multi_gpu": "slabs along z: %s planes per rank, %d bytes of boundary planes per rank and sweep (%s), "
+                                    "one all_reduce of 32 bytes per measurement" % (
+                                        [nz for _, nz in slabs.partition(Lz, world)], face_bytes,
+                                        "stored by the colour kernels into the neighbours' ghost planes, a barrier per pass"
+                                        if args.slab_exchange == "peer" else "sent as faces after every pass"),
                        "l2": "state %.0f MB per rank" % (12.0 * n / world / 1e6)},
             "ns_per_update": 1.0 / value, "clocks": clocks, "e2e": None, "gpu_launches": launches,
             "M": [float(x) for x in M], "E_per_spin": E / n,
@@ -296,6 +300,9 @@ def main():
     ap.add_argument("--multi", default="replicas", choices=["replicas", "slabs"],
                     help="N > 1: independent replicas (default, weak scaling) or ONE lattice cut into z-slabs with a face "
                          "exchange per colour (strong scaling; simple cubic workloads; DESIGN.md section 9)")
+    ap.add_argument("--slab-exchange", default="peer", choices=["peer", "copies"],
+                    help="--multi slabs: boundary planes stored by the colour kernels straight into the neighbours' ghost planes "
+                         "(peer memory, CUDA IPC between the ranks; default) or sent as faces after every pass (NCCL send/recv)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
