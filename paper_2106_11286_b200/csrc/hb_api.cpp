@@ -36,8 +36,8 @@ struct Plan {                 // device memory plan of a lattice
 };
 
 // A slab (hb_lattice.slab_Lz > 0) is run as a periodic lattice of Lz + 2 planes whose first and last planes are the
-// ghost planes: the kernels need no special case, the two ghost planes are updated with meaningless neighbours and
-// overwritten by the caller's face exchange before anything reads them.  Returns the padded description.
+// ghost planes: the kernels index it like any other lattice and only skip the updates of those two planes
+// (ScLayout::ghost), which the z-neighbours own and fill (face copies or peer stores).  Returns the padded description.
 int pad_slab(const hb_lattice* lat, hb_lattice& padded, std::string& why) {
   padded = *lat;
   if (lat->slab_Lz <= 0) return HB_OK;
