@@ -120,7 +120,9 @@ __device__ __forceinline__ Vec<V> sc_field_off(const float* b, uint32_t oc, uint
 // has exactly one end in it, -J sum_{i in last colour} S_i.h_i is the whole exchange energy.
 // The pass of one block (bid of nblk): the body of k_sweep_sc, and of the persistent multi-sweep kernel below,
 // which walks virtual blocks and needs coherent loads (CO) because other blocks of the same launch wrote b.
-template <int V, int ANISO, bool DIAG, int PF, bool MEAS, bool CO>
+// SLAB: first and last planes are ghost planes of a slab (not updated), boundary-plane stores are repeated into the
+// z-neighbours' buffers (hb_slab_set_peer); a separate instantiation, so that whole lattices carry none of it
+template <int V, int ANISO, bool DIAG, int PF, bool MEAS, bool CO, bool SLAB = false>
 __device__ __forceinline__ void sc_pass(float* ax, float* ay, float* az, const float* bx, const float* by, const float* bz,
                                         const ScLayout& L, const ScTile& t, const SweepParams& P, int colour, const Diag& d,
                                         const Meas& m, const uint3 bid, const uint3 nblk) {
@@ -156,7 +158,7 @@ __device__ __forceinline__ void sc_pass(float* ax, float* ay, float* az, const f
   unsigned n_acc = 0;
   double acc_mx = 0.0, acc_my = 0.0, acc_mz = 0.0, acc_en = 0.0;
   for (int32_t z = z0; z < z1; ++z) {
-    if (L.ghost && (z == 0 || z == L.Lz - 1)) continue;   // ghost planes of a slab: the z-neighbour owns them
+    if (SLAB && (z == 0 || z == L.Lz - 1)) continue;   // ghost planes of a slab: the z-neighbour owns them
     const uint32_t pz = (uint32_t)z * plane;
     const uint32_t pzm = (uint32_t)((z == 0) ? L.Lz - 1 : z - 1) * plane;
     const uint32_t pzp = (uint32_t)((z == L.Lz - 1) ? 0 : z + 1) * plane;
@@ -205,7 +207,7 @@ __device__ __forceinline__ void sc_pass(float* ax, float* ay, float* az, const f
       store<V>(ax + oc, sx);
       store<V>(ay + oc, sy);
       store<V>(az + oc, sz);
-      if (L.ghost) {   // slab with peer stores: the boundary planes go straight into the neighbours' ghost planes
+      if (SLAB) {   // slab with peer stores: the boundary planes go straight into the neighbours' ghost planes
         const bool lo = z == 1, hi = z == L.Lz - 2;   // (distinct planes: a slab has at least two of its own)
         float* pb = lo ? L.peer[0] : (hi ? L.peer[1] : nullptr);
         if (pb) {
@@ -238,13 +240,13 @@ __device__ __forceinline__ void sc_pass(float* ax, float* ay, float* az, const f
   }
 }
 
-template <int V, int ANISO, bool DIAG, int PF, int BLK = 256, bool MEAS = false>
+template <int V, int ANISO, bool DIAG, int PF, int BLK = 256, bool MEAS = false, bool SLAB = false>
 __global__ void __launch_bounds__(BLK, (MEAS ? 3 : HB_SC_MINBLOCKS) * 256 / BLK)   // MEAS needs ~80 registers
 k_sweep_sc(float* __restrict__ ax, float* __restrict__ ay, float* __restrict__ az,
            const float* __restrict__ bx, const float* __restrict__ by, const float* __restrict__ bz,
            ScLayout L, ScTile t, SweepParams P, int colour, Diag d, Meas m) {
   resolve_sweep(P);
-  sc_pass<V, ANISO, DIAG, PF, MEAS, false>(ax, ay, az, bx, by, bz, L, t, P, colour, d, m, blockIdx, gridDim);
+  sc_pass<V, ANISO, DIAG, PF, MEAS, false, SLAB>(ax, ay, az, bx, by, bz, L, t, P, colour, d, m, blockIdx, gridDim);
 }
 
 // ---- CSR: one thread per site of the colour -------------------------------------------------
@@ -538,7 +540,15 @@ static cudaError_t sweep_sc_impl(cudaStream_t st, float* s, ScLayout L, ScTile t
   constexpr bool TUNED = !DIAG && V == 4;   // the tuned configuration carries the prefetch, big-block and fused-measurement variants
   constexpr int P1 = TUNED ? 1 : 0, B512 = TUNED ? 512 : 256, B1024 = TUNED ? 1024 : 256;
   if (m.mode != 0 && !TUNED) return cudaErrorInvalidValue;
-  if (TUNED) {
+  if (L.ghost) {   // slab contexts: one variant (blocks of up to 256 threads, no fused measurement, no recording)
+    if (m.mode != 0 || DIAG) return cudaErrorInvalidValue;
+    kern = k_sweep_sc<V, ANISO, DIAG, P1, 256, false, true>;
+    if (threads > 256) {
+      if (t.JX > 256) t.JX = 256;
+      t.TY = 256 / t.JX;
+      if (t.LIN > 256) t.LIN = 256;
+    }
+  } else if (TUNED) {
     if (m.mode != 0) {
       if (threads > 512) kern = k_sweep_sc<V, ANISO, DIAG, P1, B1024, TUNED>;
       else if (threads > 256) kern = k_sweep_sc<V, ANISO, DIAG, P1, B512, TUNED>;

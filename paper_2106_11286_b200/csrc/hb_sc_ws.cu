@@ -111,7 +111,7 @@ __device__ __forceinline__ void ws_producer(const float* b, const ScLayout& L, c
 }
 
 // ---- consumers -------------------------------------------------------------------------------------------
-template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS>
+template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS, bool SLAB>
 __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const WsTiles& w, const SweepParams& P, int colour,
                                             int mode, unsigned char* smem, uint32_t sbase, double acc[4]) {
   using S = WsSmem<TY, ROWB, kNB, MINB>;
@@ -148,7 +148,7 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
     for (int32_t s = 0; s < nz; ++s) {
       // ghost planes of a slab are staged as neighbours but not updated: the z-neighbour owns them
       const int32_t zs = z0 + s;
-      const bool act = active && !(L.ghost && (zs == 0 || zs == L.Lz - 1));
+      const bool act = active && !(SLAB && (zs == 0 || zs == L.Lz - 1));
       Vec<4> sp[3];
       if (PREF) {
         sp[0] = nxt[0]; sp[1] = nxt[1]; sp[2] = nxt[2];
@@ -218,7 +218,7 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
           store<4>(gx, sp[0]);
           store<4>(gx + n, sp[1]);
           store<4>(gx + 2 * n, sp[2]);
-          if (L.ghost) {   // slab with peer stores: the boundary planes go straight into the neighbours' ghost planes
+          if (SLAB) {   // slab with peer stores: the boundary planes go straight into the neighbours' ghost planes
             const bool lo = zs == 1, hi = zs == L.Lz - 2;
             float* pb = lo ? L.peer[0] : (hi ? L.peer[1] : nullptr);
             if (pb) {
@@ -251,7 +251,10 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
   }
 }
 
-template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS>
+// SLAB: the lattice is a slab of a larger one (ScLayout::ghost): its first and last planes are ghost planes, staged as
+// neighbours but not updated, and boundary-plane stores are repeated into the z-neighbours' buffers (hb_slab_set_peer).
+// A separate instantiation: the whole-lattice kernel carries none of it.
+template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS, bool SLAB>
 __global__ void __launch_bounds__((ws_max_threads<TY, ROWB>()), MINB)
 k_sweep_sc_ws(float* a, const float* b, ScLayout L, WsTiles w, SweepParams P, int colour, Meas m) {
   resolve_sweep(P);
@@ -267,7 +270,7 @@ k_sweep_sc_ws(float* a, const float* b, ScLayout L, WsTiles w, SweepParams P, in
   __syncthreads();
   double acc[4] = {0.0, 0.0, 0.0, 0.0};
   if (threadIdx.x < 32) ws_producer<TY, ROWB, kNB, MINB>(b, L, w, smem, sbase);
-  else ws_consumer<TY, ROWB, kNB, MINB, ANISO, MEAS>(a, L, w, P, colour, m.mode, smem, sbase, acc);
+  else ws_consumer<TY, ROWB, kNB, MINB, ANISO, MEAS, SLAB>(a, L, w, P, colour, m.mode, smem, sbase, acc);
   if (threadIdx.x == 0) {   // this thread took the CTA's last tile number above; the last CTA to finish re-arms the scheduler
     __threadfence();
     if (atomicAdd(w.sched + 1, 1u) == gridDim.x - 1) { w.sched[0] = 0u; w.sched[1] = 0u; }
@@ -275,10 +278,10 @@ k_sweep_sc_ws(float* a, const float* b, ScLayout L, WsTiles w, SweepParams P, in
   if (MEAS) block_reduce4(acc[0], acc[1], acc[2], acc[3], m.partials + (size_t)blockIdx.x * 4);
 }
 
-template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS>
+template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS, bool SLAB = false>
 cudaError_t ws_go(cudaStream_t st, float* s, const ScLayout& L, int n_zc, int grid_cap, uint32_t* sched, const SweepParams& p, int colour, const Meas& m) {
   using S = WsSmem<TY, ROWB, kNB, MINB>;
-  auto kern = k_sweep_sc_ws<TY, ROWB, kNB, MINB, ANISO, MEAS>;
+  auto kern = k_sweep_sc_ws<TY, ROWB, kNB, MINB, ANISO, MEAS, SLAB>;
   static bool configured = false;
   if (!configured) {
     const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::BYTES);
@@ -300,6 +303,14 @@ cudaError_t ws_go(cudaStream_t st, float* s, const ScLayout& L, int n_zc, int gr
 template <int TY, int ROWB, int kNB, int MINB>
 cudaError_t ws_pick(cudaStream_t st, float* s, const ScLayout& L, int n_zc, int grid_cap, uint32_t* sched, const SweepParams& p, int colour, const Meas& m) {
   const int aniso = (p.K == 0.0f) ? ANISO_NONE : ((p.ex == 0.0f && p.ey == 0.0f && p.ez == 1.0f) ? ANISO_Z : ANISO_GENERAL);
+  if (L.ghost) {   // slab contexts measure with the separate pass
+    if (m.mode != 0) return cudaErrorInvalidValue;
+    switch (aniso) {
+      case ANISO_NONE: return ws_go<TY, ROWB, kNB, MINB, ANISO_NONE, false, true>(st, s, L, n_zc, grid_cap, sched, p, colour, m);
+      case ANISO_Z: return ws_go<TY, ROWB, kNB, MINB, ANISO_Z, false, true>(st, s, L, n_zc, grid_cap, sched, p, colour, m);
+      default: return ws_go<TY, ROWB, kNB, MINB, ANISO_GENERAL, false, true>(st, s, L, n_zc, grid_cap, sched, p, colour, m);
+    }
+  }
   if (m.mode != 0) {
     switch (aniso) {
       case ANISO_NONE: return ws_go<TY, ROWB, kNB, MINB, ANISO_NONE, true>(st, s, L, n_zc, grid_cap, sched, p, colour, m);
