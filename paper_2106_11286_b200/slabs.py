@@ -192,18 +192,33 @@ class DistSlab:
         self._mapped = {}
         if self.peer_stores:
             down, up = neighbours(self.rank, self.world)
+            self._nccl = self.world > 1 and dist.get_backend(group) == "nccl"
+            self._flag = torch.zeros(1, dtype=torch.int32, device=self.ctx.device) if self._nccl else None
             if self.world == 1:
-                ptrs = {0: self.ctx.spins_ptr}
+                ptrs, ok = {0: self.ctx.spins_ptr}, True
             else:
                 handles = [None] * self.world
                 dist.all_gather_object(handles, self.ctx.ipc_handle(), group=group)
-                for r in {down, up}:
-                    self._mapped[r] = self.ctx.open_ipc(handles[r])
+                ok = True
+                try:
+                    for r in {down, up}:
+                        self._mapped[r] = self.ctx.open_ipc(handles[r])
+                except Exception:               # no peer access between the two devices: every rank falls back together
+                    ok = False
                 ptrs = self._mapped
-            self.ctx.slab_set_peer(0, ptrs[down], parts[down][1])
-            self.ctx.slab_set_peer(1, ptrs[up], parts[up][1])
-            self._nccl = self.world > 1 and dist.get_backend(group) == "nccl"
-            self._flag = torch.zeros(1, dtype=torch.int32, device=self.ctx.device) if self._nccl else None
+                agree = torch.tensor([1 if ok else 0], dtype=torch.int32, device=self.ctx.device if self._nccl else "cpu")
+                dist.all_reduce(agree, op=dist.ReduceOp.MIN, group=group)
+                ok = bool(agree.item())
+            if ok:
+                self.ctx.slab_set_peer(0, ptrs[down], parts[down][1])
+                self.ctx.slab_set_peer(1, ptrs[up], parts[up][1])
+            else:
+                import warnings
+                warnings.warn("DistSlab: a neighbour's spins buffer could not be mapped; faces are sent after every pass instead")
+                for ptr in self._mapped.values():
+                    self.ctx.close_ipc(ptr)
+                self._mapped = {}
+                self.peer_stores = False
 
     def _pass_barrier(self):
         """No rank starts the next colour before every rank has finished this one."""
