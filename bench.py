@@ -274,7 +274,7 @@ def run_slabs(args, cfg, rank, world, device, barrier):
                                     "one all_reduce of 32 bytes per measurement" % (
                                         [nz for _, nz in slabs.partition(Lz, world)], face_bytes,
                                         "stored by the colour kernels into the neighbours' ghost planes, a barrier per pass"
-                                        if args.slab_exchange == "peer" else "sent as faces after every pass"),
+                                        if sl.peer_stores else "sent as faces after every pass"),
                        "l2": "state %.0f MB per rank" % (12.0 * n / world / 1e6)},
             "ns_per_update": 1.0 / value, "clocks": clocks, "e2e": None, "gpu_launches": launches,
             "M": [float(x) for x in M], "E_per_spin": E / n,
