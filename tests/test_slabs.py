@@ -225,3 +225,20 @@ def test_two_processes_one_slab_each(mode):
     assert spins_equal(got, st.get_spins())
     Mo, Eo = st.measure()[:2]
     assert np.max(np.abs(np.asarray(r["M"]) - np.asarray(Mo))) <= 1e-7 and abs(r["E"] - Eo) <= 1e-6 * lat.n
+
+
+def test_slab_lattice_sizes_host_logic():
+    # hb_sizes runs no device code: a slab reports its own sites and a buffer that also holds the two ghost planes
+    import paper_2106_11286_b200 as hb
+    n, spins, ws = hb.sizes(hb.Lattice("sc", 8, 4, 4, slab=(4, 12)))
+    n_whole, spins_whole, _ = hb.sizes(hb.Lattice("sc", 8, 4, 6))
+    assert n == 8 * 4 * 4 and spins == spins_whole >= 3 * 4 * 8 * 4 * 6
+    for bad in [dict(slab=(3, 12)), dict(slab=(4, 6)), dict(slab=(0, 11)), dict(slab=(-2, 12))]:
+        with pytest.raises(hb.HbError):
+            hb.sizes(hb.Lattice("sc", 8, 4, 4, **bad))
+    with pytest.raises(hb.HbError):
+        hb.sizes(hb.Lattice("fcc", 4, 4, 4, slab=(0, 8)))
+    # implicit lattices go up to 2^32 - 1 sites; the table engine is bounded by its 32-bit neighbour offsets
+    assert hb.sizes(hb.Lattice("sc", 1600, 1600, 1600))[0] == 4096000000
+    with pytest.raises(hb.HbError):
+        hb.sizes(hb.Lattice("sc", 1626, 1626, 1626))
