@@ -553,13 +553,14 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
     if (c->ws_zt > c->sc.Lz) c->ws_zt = c->sc.Lz;
     // the warp-specialised kernel is built for long rows (pitch 1024 B): with them, on lattices far larger than L2, it
     // sustains 3-4 % more than the direct kernel and stays below the power cap; everything else runs direct
-    c->sc_kernel = (sc_ws_supported(c->sc) && c->sc.H >= 224 && P.n >= (int64_t(1) << 24)) ? 1 : 0;
+    c->sc_kernel = (sc_ws_supported(c->sc) && (c->sc.H >= 224 || (c->sc.H >= 112 && c->sc.H <= 128)) && P.n >= (int64_t(1) << 24)) ? 1 : 0;
     if (c->slab_Lz > 0) {   // local plane 1 is global plane slab_z0; graphs, persistent kernels and the fused measurement are for whole lattices
       c->sc.ghost = 1;
       c->sc.site_base = (uint32_t)(((int64_t)c->slab_z0 - 1) * lat->Ly * lat->Lx);
       c->graph_mode = 0; c->sc_coop = 0; c->fused_measure = false;
     }
-    c->ws_variant = sc_ws_variant_supported(c->sc, 4) ? 4 : 2;   // 7-row tiles where the rows fit them (c4: +2 %), else 4-row tiles
+    if (c->sc.H <= 128) c->ws_variant = 5;   // rows of 112-128 floats (256^3): 8-row tiles at a 512-byte pitch, +2.5 % over the direct kernel
+    else c->ws_variant = sc_ws_variant_supported(c->sc, 4) ? 4 : 2;   // 7-row tiles where the rows fit them (c4: +2 %), else 4-row tiles
   }
 
   // programmatic stream serialisation of the colour launches: mode 1 (the next launch comes in as blocks
@@ -1134,7 +1135,8 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
   if (s == "sc_ws_variant") {
     if (!sc_ws_variant_supported(c->sc, (int)value))
       return fail(c, HB_EINVAL, "sc_ws_variant: 0 (4-row tiles, 2 CTAs per SM), 1 (8-row tiles, 1 CTA per SM), 2 (4-row tiles, 3 CTAs per SM), "
-                                "3 (16-row tiles, 1 CTA per SM; rows of up to 248 floats), 4 (7-row tiles, 2 CTAs per SM; rows of up to 236 floats)");
+                                "3 (16-row tiles, 1 CTA per SM; rows of up to 248 floats), 4 (7-row tiles, 2 CTAs per SM; rows of up to 236 floats), "
+                                "5 (8-row tiles at a 512-byte pitch, 3 CTAs per SM; rows of up to 128 floats)");
     c->ws_variant = (int)value;
     return HB_OK;
   }

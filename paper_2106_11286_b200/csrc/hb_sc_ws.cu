@@ -339,11 +339,14 @@ bool sc_ws_supported(const ScLayout& L) { return L.H % 4 == 0 && L.H <= 256; }
 // (11-row tiles, whose 638 consumer threads fill 99.7 % of their warps' lanes, 1 CTA per SM: 111-113)
 //   4 = 7-row tiles, 4 plane slots (108 KB), 2 CTAs per SM of 13 consumer warps, 72 registers: for rows of up to 236
 //       floats; with 232-float rows (c4) 406 of the 416 consumer lanes work (97.6 %, against 90.6 % of the 4-row tile)
-static int ws_ty(int variant) { return variant == 1 ? 8 : (variant == 3 ? 16 : (variant == 4 ? 7 : 4)); }
-static int ws_ctas_per_sm(int variant) { return (variant == 1 || variant == 3) ? 1 : (variant == 2 ? 3 : 2); }
+//   5 = 8-row tiles at a row pitch of 512 bytes, 4 plane slots (61 KB), 3 CTAs per SM of 8 consumer warps: for rows of up to
+//       128 floats (Lx <= 256); with 128-float rows every consumer lane works
+static int ws_ty(int variant) { return (variant == 1 || variant == 5) ? 8 : (variant == 3 ? 16 : (variant == 4 ? 7 : 4)); }
+static int ws_ctas_per_sm(int variant) { return (variant == 1 || variant == 3) ? 1 : ((variant == 2 || variant == 5) ? 3 : 2); }
 
 bool sc_ws_variant_supported(const ScLayout& L, int variant) {
-  if (variant < 0 || variant > 4 || !sc_ws_supported(L)) return false;
+  if (variant < 0 || variant > 5 || !sc_ws_supported(L)) return false;
+  if (variant == 5) return L.H <= 128;              // row pitch of 512 bytes
   if (variant == 3) return 16 * (L.H / 4) <= 992;   // 1024 threads less the producer warp
   if (variant == 4) return 7 * (L.H / 4) <= 416;    // 13 consumer warps
   return true;
@@ -377,6 +380,7 @@ int sc_ws_blocks(const ScLayout& L, int ZT, int grid_cap, int variant) {
 cudaError_t launch_sweep_sc_ws(cudaStream_t st, float* s, ScLayout L, int ZT, int grid_cap, int variant, uint32_t* sched, SweepParams p, int colour, Meas m) {
   const int cap = grid_cap * ws_ctas_per_sm(variant);
   const int n_zc = sc_ws_chunks(L, ZT, grid_cap, variant);
+  if (variant == 5) return ws_pick<8, 512, 4, 3>(st, s, L, n_zc, cap, sched, p, colour, m);
   if (variant == 4) return ws_pick<7, 1024, 4, 2>(st, s, L, n_zc, cap, sched, p, colour, m);
   if (variant == 3) return ws_pick<16, 1024, 4, 1>(st, s, L, n_zc, cap, sched, p, colour, m);
   if (variant == 1) return ws_pick<8, 1024, 6, 1>(st, s, L, n_zc, cap, sched, p, colour, m);

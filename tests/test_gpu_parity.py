@@ -380,7 +380,10 @@ def test_warp_specialised_kernel_matches_the_oracle():
              # 7-row tiles, two CTAs per SM (the default for config 4's rows of 232 floats): ragged tiles, full-width rows
              (dict(W.SMALL["c4"], L=(40, 14, 10)), {"sc_ws_variant": 4, "sc_ws_zt": 3}),
              (dict(W.SMALL["c4"], L=(464, 16, 6), K=0.3, e=(0.6, 0.0, 0.8)), {"sc_ws_variant": 4}),
-             (dict(W.SMALL["c4"], L=(472, 30, 4)), {"sc_ws_variant": 4, "sc_ws_ctas": 3})]
+             (dict(W.SMALL["c4"], L=(472, 30, 4)), {"sc_ws_variant": 4, "sc_ws_ctas": 3}),
+             # 8-row tiles at a 512-byte row pitch, three CTAs per SM (rows of up to 128 floats): full-width and short rows
+             (dict(W.SMALL["c4"], L=(256, 20, 6)), {"sc_ws_variant": 5}),
+             (dict(W.SMALL["c4"], L=(40, 14, 10), K=0.3, e=(0.6, 0.0, 0.8)), {"sc_ws_variant": 5, "sc_ws_zt": 3, "sc_ws_ctas": 1})]
     for cfg, opts in cases:
         lat, st = make_oracle(cfg)
         ctx = make_gpu(cfg)
@@ -405,6 +408,8 @@ def test_warp_specialised_kernel_matches_the_oracle():
         hb.Context(hb.Lattice("sc", 512, 4, 4)).set_option("sc_ws_variant", 3)   # 16 rows of 64 vectors: more than 1024 threads
     with pytest.raises(hb.HbError):
         hb.Context(hb.Lattice("sc", 480, 4, 4)).set_option("sc_ws_variant", 4)   # 7 rows of 60 vectors: more than 13 warps
+    with pytest.raises(hb.HbError):
+        hb.Context(hb.Lattice("sc", 264, 4, 4)).set_option("sc_ws_variant", 5)   # rows of 132 floats: longer than the 512-byte pitch
 
 
 def test_replayed_launches_match_the_oracle():
@@ -536,7 +541,8 @@ def test_kernel_variants_agree_on_random_shapes():
                     {"graph": 1, "sc_coop": 0, "pdl": (it + 1) % 2},
                     {"graph": 0, "sc_coop": 2},
                     {"graph": int(rng.integers(0, 2)), "sc_kernel": 1, "sc_ws_zt": int(rng.integers(0, Lz + 1)),
-                     "sc_ws_ctas": int(rng.integers(1, 5)), "sc_ws_variant": int(rng.integers(0, 5 if H <= 236 else 3))}]
+                     "sc_ws_ctas": int(rng.integers(1, 5)),
+                     "sc_ws_variant": int(rng.choice([0, 1, 2] + ([3] if H <= 248 else []) + ([4] if H <= 236 else []) + ([5] if H <= 128 else [])))}]
         for opts in variants:
             got, (Mg, Eg) = run(opts)
             assert spins_equal(got, ref), (Lx, Ly, Lz, opts)
