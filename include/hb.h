@@ -158,6 +158,13 @@ int hb_get_colouring(hb_ctx* ctx, int32_t* colour, int32_t* n_colours);
 /* Counters since hb_create: kernels launched by this context, sites attempted. */
 int hb_counters(hb_ctx* ctx, uint64_t* kernel_launches, uint64_t* attempts);
 
+/* Acceptance statistics of rule (iii) (a move is accepted if dH <= 0 or P <= exp(-beta dH)):
+ * `accepts` of `attempts` moves were accepted, summed since hb_create over the COUNTED sweeps.  Counting is part of the
+ * measuring colour passes (a warp vote and one atomic per warp), so the plain passes carry none of it: counted are the
+ * last sweep of every hb_sweep / hb_sweep_each call, every sweep of hb_sweep_series(_each) and every hb_sweep_record
+ * sweep (all replicas together).  Slab passes are not counted.  Synchronises. */
+int hb_stats(hb_ctx* ctx, uint64_t* attempts, uint64_t* accepts);
+
 /* ---- slab contexts (hb_lattice.slab_Lz > 0): one sweep of the whole lattice is, on every slab,
  *        for colour in (0, 1):  hb_slab_pass(colour);  exchange the faces of that colour with both z-neighbours;
  *        hb_slab_next_sweep()
@@ -200,6 +207,21 @@ int hb_ipc_close(void* ptr);
  * `cuda_stream` for about `seconds` (0 < seconds <= 10; the second half is timed, so the clock is the one a long run
  * holds).  It is the arithmetic ceiling of the colour kernels on this chip.  Synchronises. */
 int hb_probe_alu(void* cuda_stream, double seconds, double* updates_per_second);
+
+/* Diagnostic (self-test of the arithmetic contract): evaluates on the current device, element by
+ * element, the building blocks of one attempt exactly as the colour kernels evaluate them -- the scalar functions AND the
+ * packed fp32x2 copies the tuned kernels use -- so that tests can compare them bit for bit with the CPU oracle over every
+ * argument that can occur.  Host pointers; `count` elements (at most 2^26); synchronises; uses the legacy default stream.
+ *   HB_MATH_U01     out[2i] = u(in0[i]) scalar, out[2i+1] = packed                        (u(r) = (2 (r >> 9) + 1) 2^-24)
+ *   HB_MATH_SINCOS  out[2i] = sin, out[2i+1] = cos of 2 pi k / 2^24, k = (in0[i] >> 8) | 1
+ *   HB_MATH_SPHERE  out[6i..6i+2] = proposal (x, y, z) from random words (in0[i], in1[i]), scalar; out[6i+3..6i+5] packed
+ *   HB_MATH_EXP     out[2i] = exp_spec(x) scalar, out[2i+1] packed; x = the float whose bits are in0[i], in [-17, 0]
+ *   HB_MATH_SQRT    out[2i] = the library's square root of w = 1 - (1 - 2 u(in0[i]))^2, out[2i+1] = IEEE sqrt of the same w
+ *   HB_MATH_ATTEMPT one whole packed attempt per element: in0[i] = site id, in1[16i..] = (sweep_lo, sweep_hi, seed_lo,
+ *                   seed_hi) as integers and (J, K, beta, ex, ey, ez, hx, hy, hz, sx, sy, sz) as float bits; elements 2t and
+ *                   2t+1 form a pair and use (J, K, beta, e) of element 2t; out[4i..] = the spin after the attempt, accepted */
+enum { HB_MATH_U01 = 0, HB_MATH_SINCOS = 1, HB_MATH_SPHERE = 2, HB_MATH_EXP = 3, HB_MATH_SQRT = 4, HB_MATH_ATTEMPT = 5 };
+int hb_device_math(int32_t op, int64_t count, const uint32_t* in0, const uint32_t* in1, float* out);
 
 /* Tuning knobs, by name (DESIGN.md section 6 lists them); unknown names give HB_EINVAL. */
 int hb_set_option(hb_ctx* ctx, const char* name, int64_t value);

@@ -18,7 +18,7 @@ EXPORTS = [
     "hb_sweep_each", "hb_measure_each", "hb_sweep_series_each", "hb_select_replica",
     "hb_slab_pass", "hb_slab_next_sweep", "hb_slab_face", "hb_slab_set_peer", "hb_probe_alu",
     "hb_device_alloc", "hb_device_free", "hb_ipc_export", "hb_ipc_open", "hb_ipc_close",
-    "hb_get_colouring", "hb_counters", "hb_set_option", "hb_get_option", "hb_lattice_fcc_sphere", "hb_lattice_free",
+    "hb_get_colouring", "hb_counters", "hb_stats", "hb_device_math", "hb_set_option", "hb_get_option", "hb_lattice_fcc_sphere", "hb_lattice_free",
     "hb_strerror", "hb_error_detail",
 ]
 
@@ -89,6 +89,8 @@ def load_library():
         "hb_set_sweep_count": [vp, u64],
         "hb_get_colouring": [vp, vp, P(i32)],
         "hb_counters": [vp, P(u64), P(u64)],
+        "hb_stats": [vp, P(u64), P(u64)],
+        "hb_device_math": [i32, i64, vp, vp, vp],
         "hb_set_option": [vp, C.c_char_p, i64],
         "hb_get_option": [vp, C.c_char_p, P(i64)],
         "hb_lattice_fcc_sphere": [i32, f32, P(f32), f32, i32, P(hb_lattice), P(vp)],
@@ -184,6 +186,26 @@ def probe_alu(seconds=0.5, device="cuda:0"):
     if rc != 0:
         raise HbError(rc, "hb_probe_alu", L.hb_strerror(rc).decode())
     return v.value
+
+
+MATH_OPS = {"u01": (0, 2, 0), "sincos": (1, 2, 0), "sphere": (2, 6, 1), "exp": (3, 2, 0), "sqrt": (4, 2, 0), "attempt": (5, 4, 16)}
+
+
+def device_math(op, in0, in1=None, device="cuda:0"):
+    """hb_device_math: the device's building blocks of an attempt, element by element (include/hb.h).
+    Returns a float32 array of shape (count, floats per element)."""
+    import torch
+    L = load_library()
+    torch.cuda.set_device(torch.device(device))
+    code, per_out, per_in1 = MATH_OPS[op]
+    a = _np(in0, np.uint32).ravel()
+    b = _np(in1, np.uint32).ravel() if in1 is not None else None
+    assert (b is None) == (per_in1 == 0) and (b is None or b.size == per_in1 * a.size)
+    out = np.zeros((a.size, per_out), np.float32)
+    rc = L.hb_device_math(code, a.size, _ptr(a), _ptr(b) if b is not None else None, _ptr(out))
+    if rc != 0:
+        raise HbError(rc, "hb_device_math", L.hb_strerror(rc).decode())
+    return out
 
 
 def sizes(lat):
@@ -384,6 +406,12 @@ class Context:
     def counters(self):
         a, b = C.c_uint64(), C.c_uint64()
         self._check(self._L.hb_counters(self._h, C.byref(a), C.byref(b)), "hb_counters")
+        return a.value, b.value
+
+    def stats(self):
+        """hb_stats -> (attempts, accepts) of the counted sweeps (include/hb.h)."""
+        a, b = C.c_uint64(), C.c_uint64()
+        self._check(self._L.hb_stats(self._h, C.byref(a), C.byref(b)), "hb_stats")
         return a.value, b.value
 
     def set_option(self, name, value):

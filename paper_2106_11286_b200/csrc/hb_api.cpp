@@ -169,6 +169,7 @@ struct hb_ctx {
   char* ws = nullptr;
   bool own_spins = false, own_ws = false;
   uint64_t launches = 0, attempts = 0;
+  uint64_t stat_attempts = 0;   // attempts of the sweeps whose accepted moves were counted on the device (hb_stats)
   int sticky = HB_OK;
   std::string detail;
 
@@ -249,7 +250,7 @@ ScTile default_tile(int32_t H, int32_t Ly, int32_t Lz) {
   return t;
 }
 
-int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d, Meas m = Meas{nullptr, 0}) {
+int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d, Meas m = Meas{nullptr, 0, nullptr}) {
   if (c->plan.engine == ENGINE_SC) {
     const bool diag = d.accept || d.n_accept;
     if (c->sc_kernel == 1 && !diag)
@@ -293,7 +294,8 @@ int coop_sweeps(hb_ctx* c, float beta, int64_t n_sweeps, double* series, double*
     const int m = (int)(n_sweeps - s0 < chunk ? n_sweeps - s0 : chunk);
     const bool last = s0 + m == n_sweeps;
     HB_CUDA(c, launch_sweeps_sc_coop(c->stream, c->spins, c->sc, c->tile, p, c->sweep, m, coop_mode(c) == 1, c->partials(),
-                                     series ? series + 4 * s0 : nullptr, last ? final_out : nullptr, 1, nullptr, 0));
+                                     series ? series + 4 * s0 : nullptr, last ? final_out : nullptr, 1, nullptr, 0, c->counters()));
+    c->stat_attempts += (uint64_t)(series ? m : ((last && final_out) ? 1 : 0)) * (uint64_t)c->plan.n;   // the measured sweeps count their accepts
     c->launches += 1;
     c->sweep += (uint64_t)m;
     c->attempts += (uint64_t)m * (uint64_t)c->plan.n;
@@ -302,15 +304,18 @@ int coop_sweeps(hb_ctx* c, float beta, int64_t n_sweeps, double* series, double*
 }
 
 // one sweep; with dev_out != nullptr (and fused_blocks() > 0) the colour passes also reduce M and E of
-// the state they leave behind, and dev_out receives (sum Sx, sum Sy, sum Sz, E)
-int one_sweep(hb_ctx* c, float beta, Diag d, double* dev_out = nullptr) {
+// the state they leave behind, and dev_out receives (sum Sx, sum Sy, sum Sz, E).  counted: the accepted moves of the
+// sweep are added to the device counter behind hb_stats (in the measuring passes, else through the diagnostic variant)
+int one_sweep(hb_ctx* c, float beta, Diag d, double* dev_out = nullptr, bool counted = false) {
   const SweepParams p = params(c, beta);
   const int fb = dev_out ? fused_blocks(c) : 0;
+  if (counted && !fb) d.n_accept = c->counters();
+  if (counted || d.n_accept) c->stat_attempts += (uint64_t)c->plan.n;
   for (int colour = 0; colour < c->n_colours; ++colour) {
-    Meas m{nullptr, 0};
+    Meas m{nullptr, 0, nullptr};
     // sc: the last colour carries the whole exchange energy; bcc/fcc: every colour charges its bonds to lower colours
     if (fb) m = Meas{c->partials() + (size_t)colour * fb * 4,
-                     (c->plan.engine == ENGINE_BRAVAIS || colour == c->n_colours - 1) ? 2 : 1};
+                     (c->plan.engine == ENGINE_BRAVAIS || colour == c->n_colours - 1) ? 2 : 1, (counted && !d.n_accept) ? c->counters() : nullptr};
     const int rc = one_colour(c, colour, p, d, m);
     if (rc != HB_OK) return rc;
   }
@@ -350,9 +355,9 @@ int build_graph(hb_ctx* c, float beta, int meas) {
   for (int u = 0; u < kGraphSweeps && rc == HB_OK && e == cudaSuccess; ++u) {
     p.sweep_lo = (uint32_t)u;
     for (int colour = 0; colour < c->n_colours && rc == HB_OK; ++colour) {
-      Meas m{nullptr, 0};
+      Meas m{nullptr, 0, nullptr};
       if (fb) m = Meas{c->partials() + (size_t)colour * fb * 4,
-                       (c->plan.engine == ENGINE_BRAVAIS || colour == c->n_colours - 1) ? 2 : 1};
+                       (c->plan.engine == ENGINE_BRAVAIS || colour == c->n_colours - 1) ? 2 : 1, c->counters()};
       rc = one_colour(c, colour, p, Diag{nullptr, nullptr}, m);
     }
     if (fb && rc == HB_OK)
@@ -387,6 +392,7 @@ int graph_sweeps(hb_ctx* c, float beta, int64_t replays, int meas) {
   c->launches += 1 + (meas ? 1 : 0) + (uint64_t)replays * ((uint64_t)kGraphSweeps * (c->n_colours + (meas ? 1 : 0)) + 1);
   c->sweep += (uint64_t)m;
   c->attempts += (uint64_t)m * (uint64_t)c->plan.n;
+  if (meas) c->stat_attempts += (uint64_t)m * (uint64_t)c->plan.n;
   return HB_OK;
 }
 
@@ -406,7 +412,8 @@ int replica_sweeps(hb_ctx* c, const float* beta, int64_t n_sweeps, double* serie
   for (int64_t s0 = 0; s0 < n_sweeps; s0 += chunk) {
     const int m = (int)(n_sweeps - s0 < chunk ? n_sweeps - s0 : chunk);
     HB_CUDA(c, launch_sweeps_sc_coop(c->stream, c->spins_base, c->sc, c->tile, p, c->sweep, m, true, c->partials_each(), series,
-                                     series ? nullptr : c->cached_each(), c->plan.R, c->betas(), (uint64_t)kSeriesChunk * 4));
+                                     series ? nullptr : c->cached_each(), c->plan.R, c->betas(), (uint64_t)kSeriesChunk * 4, c->counters()));
+    c->stat_attempts += (uint64_t)(series ? m : 1) * (uint64_t)c->plan.n * (uint64_t)c->plan.R;
     c->launches += 1;
     c->sweep += (uint64_t)m;
     c->attempts += (uint64_t)m * (uint64_t)c->plan.n * (uint64_t)c->plan.R;
@@ -806,7 +813,8 @@ int hb_sweep(hb_ctx* c, float T, int64_t n_sweeps) {
     s = replays * kGraphSweeps;
   }
   for (; s < n_sweeps; ++s) {
-    rc = one_sweep(c, beta, Diag{nullptr, nullptr}, (fuse && s == n_sweeps - 1) ? c->cached() : nullptr);
+    const bool last = s == n_sweeps - 1;   // carries the fused measurement and counts its accepted moves (hb_stats)
+    rc = one_sweep(c, beta, Diag{nullptr, nullptr}, (fuse && last) ? c->cached() : nullptr, last);
     if (rc != HB_OK) return rc;
   }
   if (fuse && n_sweeps > 0) c->cache_valid = true;
@@ -869,7 +877,7 @@ int hb_sweep_series(hb_ctx* c, float T, int64_t n_sweeps, double* M_series, doub
       s = replays * kGraphSweeps;
     }
     for (; s < m; ++s) {
-      rc = one_sweep(c, beta, Diag{nullptr, nullptr}, fuse ? c->series() + 4 * s : nullptr);
+      rc = one_sweep(c, beta, Diag{nullptr, nullptr}, fuse ? c->series() + 4 * s : nullptr, true);
       if (rc != HB_OK) return rc;
       if (!fuse) {
         rc = measure_into(c, c->series() + 4 * s);
@@ -1084,6 +1092,17 @@ int hb_counters(hb_ctx* c, uint64_t* kernel_launches, uint64_t* attempts) {
   return HB_OK;
 }
 
+int hb_stats(hb_ctx* c, uint64_t* attempts, uint64_t* accepts) {
+  HB_CHECK_CTX(c);
+  if (!attempts || !accepts) return fail(c, HB_EINVAL, "NULL output");
+  unsigned long long acc = 0;
+  HB_CUDA(c, cudaMemcpyAsync(&acc, c->counters(), sizeof acc, cudaMemcpyDeviceToHost, c->stream));
+  HB_CUDA(c, cudaStreamSynchronize(c->stream));
+  *attempts = c->stat_attempts;
+  *accepts = (uint64_t)acc;
+  return HB_OK;
+}
+
 int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
   HB_CHECK_CTX(c);
   if (!name) return HB_EINVAL;
@@ -1188,6 +1207,7 @@ int hb_get_option(hb_ctx* c, const char* name, int64_t* value) {
   else if (s == "sc_kernel") *value = c->sc_kernel;
   else if (s == "sc_ws_zt") *value = c->ws_zt;
   else if (s == "sc_ws_ctas") *value = c->n_sms;
+  else if (s == "sc_ws_variant") *value = c->ws_variant;
   else return HB_EINVAL;
   return HB_OK;
 }

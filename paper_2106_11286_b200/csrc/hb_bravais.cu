@@ -183,8 +183,8 @@ k_sweep_bravais(float* __restrict__ own, const float* __restrict__ all, BrLayout
                         make_float2(hy.v[k], hy.v[k + 1]), make_float2(hz.v[k], hz.v[k + 1]), px, py, pz, acc_a, acc_b);
         sx.v[k] = px.x; sx.v[k + 1] = px.y; sy.v[k] = py.x; sy.v[k + 1] = py.y; sz.v[k] = pz.x; sz.v[k + 1] = pz.y;
         any |= acc_a | acc_b;
+        if (DIAG || MEAS) n_acc += (unsigned)acc_a + (unsigned)acc_b;
         if (DIAG) {
-          n_acc += (unsigned)acc_a + (unsigned)acc_b;
           if (d.accept) { d.accept[site0 + k] = acc_a; d.accept[site0 + k + 1] = acc_b; }
         }
       }
@@ -196,8 +196,8 @@ k_sweep_bravais(float* __restrict__ own, const float* __restrict__ all, BrLayout
       const bool acc = metropolis_accept(dH, P.beta, r.r2);
       if (acc) { sx.v[0] = nx; sy.v[0] = ny; sz.v[0] = nz; }
       any = acc;
+      if (DIAG || MEAS) n_acc += acc;
       if (DIAG) {
-        n_acc += acc;
         if (d.accept) d.accept[site0] = acc;
       }
     }
@@ -225,6 +225,7 @@ k_sweep_bravais(float* __restrict__ own, const float* __restrict__ all, BrLayout
   if (MEAS) {
     const uint32_t blk = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
     block_reduce4(acc_mx, acc_my, acc_mz, acc_en, m.partials + (size_t)blk * 4);
+    if (!DIAG) count_accepts(m.n_accept, n_acc);
   }
 }
 
@@ -269,7 +270,7 @@ inline int aniso_of(const SweepParams& p) {
 
 template <int KIND, int B, int V, int ANISO, bool DIAG, bool MEAS = false>
 cudaError_t go(cudaStream_t st, float* s, const BrLayout& L, const ScTile& t, const SweepParams& p, const Diag& d,
-               const Meas& m = Meas{nullptr, 0}) {
+               const Meas& m = Meas{nullptr, 0, nullptr}) {
   const int HV = L.Lx / V;
   dim3 grid((HV + t.JX - 1) / t.JX, (L.Ly + t.TY - 1) / t.TY, (L.Lz + t.ZT - 1) / t.ZT);
   return launch_colour_kernel(k_sweep_bravais<KIND, B, V, ANISO, DIAG, MEAS>, grid, dim3(t.JX * t.TY), 0, st, p.pdl != 0,

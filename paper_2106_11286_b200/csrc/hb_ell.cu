@@ -90,7 +90,10 @@ k_sweep_ell(float4* S, EllDev g, uint32_t begin, uint32_t count, SweepParams P, 
   if (acc) S[m] = make_float4(nx, ny, nz, 0.0f);
   if (DIAG) {
     if (d.accept) d.accept[site] = acc;
-    if (d.n_accept && acc) atomicAdd(d.n_accept, 1ull);
+    if (d.n_accept) {   // one atomic per warp (some lanes of the last warp have left)
+      const unsigned live = __activemask(), votes = __ballot_sync(live, acc);
+      if (votes && (threadIdx.x & 31) == (unsigned)(__ffs(live) - 1)) atomicAdd(d.n_accept, (unsigned long long)__popc(votes));
+    }
   }
 }
 

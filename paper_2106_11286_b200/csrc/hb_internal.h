@@ -105,7 +105,9 @@ struct Diag {
 struct Meas {
   double* partials;   // 4 doubles per block of the launch, or nullptr
   int mode;           // 0 off, 1 own spins + anisotropy energy, 2 also the exchange energy (last colour)
+  unsigned long long* n_accept = nullptr;   // accepted moves of the pass are added here (hb_stats), one atomic per warp; or nullptr
 };
+
 constexpr int kFusedBlocksMax = 16384;   // per colour: larger grids use the separate measurement pass
 
 // ---- kernels (hb_kernels.cu); every launcher returns the launch status -----------------
@@ -125,7 +127,7 @@ int sc_coop_blocks(const ScLayout& L, const ScTile& t);
 // partials + 16 r, series + series_stride r, final_out + 4 r)
 cudaError_t launch_sweeps_sc_coop(cudaStream_t st, float* spins, ScLayout L, ScTile t, SweepParams p, uint64_t sweep0, int n_sweeps,
                                   bool one_block, double* partials, double* series, double* final_out,
-                                  int n_replicas, const float* betas, uint64_t series_stride);
+                                  int n_replicas, const float* betas, uint64_t series_stride, unsigned long long* n_accept);
 // warp-specialised persistent sc kernel (hb_sc_ws.cu): grid_cap = CTAs to launch at most (one per SM)
 bool sc_ws_supported(const ScLayout& L);
 bool sc_ws_variant_supported(const ScLayout& L, int variant);

@@ -190,16 +190,16 @@ __device__ __forceinline__ void sc_pass(float* ax, float* ay, float* az, const f
                         make_float2(hy.v[k], hy.v[k + 1]), make_float2(hz.v[k], hz.v[k + 1]), px, py, pz, acc_a, acc_b);
         sx.v[k] = px.x; sx.v[k + 1] = px.y; sy.v[k] = py.x; sy.v[k + 1] = py.y; sz.v[k] = pz.x; sz.v[k + 1] = pz.y;
         any |= acc_a | acc_b;
+        if (DIAG || MEAS) n_acc += (unsigned)acc_a + (unsigned)acc_b;
         if (DIAG) {
-          n_acc += (unsigned)acc_a + (unsigned)acc_b;
           if (d.accept) { d.accept[site0 + 2u * k] = acc_a; d.accept[site0 + 2u * k + 2u] = acc_b; }
         }
       }
     } else {
       const bool acc = attempt<ANISO>(site0, P, P.K, P.ex, P.ey, P.ez, hx.v[0], hy.v[0], hz.v[0], sx.v[0], sy.v[0], sz.v[0]);
       any |= acc;
+      if (DIAG || MEAS) n_acc += acc;
       if (DIAG) {
-        n_acc += acc;
         if (d.accept) d.accept[site0] = acc;
       }
     }
@@ -237,6 +237,7 @@ __device__ __forceinline__ void sc_pass(float* ax, float* ay, float* az, const f
   if (MEAS) {
     const uint32_t blk = (bid.z * nblk.y + bid.y) * nblk.x + bid.x;
     block_reduce4(acc_mx, acc_my, acc_mz, acc_en, m.partials + (size_t)blk * 4);
+    if (!DIAG) count_accepts(m.n_accept, n_acc);
   }
 }
 
@@ -278,7 +279,10 @@ k_sweep_csr(float* sx, float* sy, float* sz, CsrDev g, uint32_t list_begin, uint
   if (acc) { sx[i] = ox; sy[i] = oy; sz[i] = oz; }
   if (DIAG) {
     if (d.accept) d.accept[i] = acc;
-    if (d.n_accept && acc) atomicAdd(d.n_accept, 1ull);
+    if (d.n_accept) {   // one atomic per warp (some lanes of the last warp have left)
+      const unsigned live = __activemask(), votes = __ballot_sync(live, acc);
+      if (votes && (threadIdx.x & 31) == (unsigned)(__ffs(live) - 1)) atomicAdd(d.n_accept, (unsigned long long)__popc(votes));
+    }
   }
 }
 
@@ -381,7 +385,8 @@ __global__ void __launch_bounds__(256) k_reduce_final_series(const double* parti
 template <int ANISO, bool ONE>
 __global__ void __launch_bounds__(ONE ? 1024 : 256, ONE ? 1 : 3)
 k_sweeps_sc_coop(float* s, ScLayout L, ScTile t, SweepParams P, unsigned long long sweep0, int n_sweeps, uint3 nblk,
-                 double* partials, double* series, double* final_out, const float* betas, unsigned long long series_stride) {
+                 double* partials, double* series, double* final_out, const float* betas, unsigned long long series_stride,
+                 unsigned long long* n_accept) {
   cooperative_groups::grid_group grid = cooperative_groups::this_grid();
   const size_t n = L.n;
   const uint32_t total = nblk.x * nblk.y * nblk.z;
@@ -408,10 +413,10 @@ k_sweeps_sc_coop(float* s, ScLayout L, ScTile t, SweepParams P, unsigned long lo
       for (uint32_t v = ONE ? 0u : blockIdx.x; v < total; v += ONE ? 1u : gridDim.x) {
         const uint3 bid = make_uint3(v % nblk.x, (v / nblk.x) % nblk.y, v / (nblk.x * nblk.y));
         if (meas) {
-          const Meas mc{part + (size_t)colour * total * 4, colour == 1 ? 2 : 1};
+          const Meas mc{part + (size_t)colour * total * 4, colour == 1 ? 2 : 1, n_accept};
           sc_pass<4, ANISO, false, 0, true, true>(a, a + n, a + 2 * n, b, b + n, b + 2 * n, L, t, P, colour, d, mc, bid, nblk);
         } else {
-          sc_pass<4, ANISO, false, 0, false, true>(a, a + n, a + 2 * n, b, b + n, b + 2 * n, L, t, P, colour, d, Meas{nullptr, 0}, bid, nblk);
+          sc_pass<4, ANISO, false, 0, false, true>(a, a + n, a + 2 * n, b, b + n, b + 2 * n, L, t, P, colour, d, Meas{nullptr, 0, nullptr}, bid, nblk);
         }
       }
       if (ONE) __syncthreads(); else grid.sync();
@@ -609,7 +614,7 @@ int sc_coop_blocks(const ScLayout& L, const ScTile& t) {
 
 cudaError_t launch_sweeps_sc_coop(cudaStream_t st, float* s, ScLayout L, ScTile t, SweepParams p, uint64_t sweep0, int n_sweeps,
                                   bool one_block, double* partials, double* series, double* final_out,
-                                  int n_replicas, const float* betas, uint64_t series_stride) {
+                                  int n_replicas, const float* betas, uint64_t series_stride, unsigned long long* n_accept) {
   const int aniso = aniso_case(p);
   if (one_block) {
     const int threads = sc_one_block_threads(L);
@@ -617,15 +622,15 @@ cudaError_t launch_sweeps_sc_coop(cudaStream_t st, float* s, ScLayout L, ScTile 
     const uint3 nblk = make_uint3(1, 1, 1);
     const unsigned long long stride = series_stride;
     switch (aniso) {
-      case ANISO_NONE: k_sweeps_sc_coop<ANISO_NONE, true><<<n_replicas, threads, 0, st>>>(s, L, t, p, sweep0, n_sweeps, nblk, partials, series, final_out, betas, stride); break;
-      case ANISO_Z: k_sweeps_sc_coop<ANISO_Z, true><<<n_replicas, threads, 0, st>>>(s, L, t, p, sweep0, n_sweeps, nblk, partials, series, final_out, betas, stride); break;
-      default: k_sweeps_sc_coop<ANISO_GENERAL, true><<<n_replicas, threads, 0, st>>>(s, L, t, p, sweep0, n_sweeps, nblk, partials, series, final_out, betas, stride); break;
+      case ANISO_NONE: k_sweeps_sc_coop<ANISO_NONE, true><<<n_replicas, threads, 0, st>>>(s, L, t, p, sweep0, n_sweeps, nblk, partials, series, final_out, betas, stride, n_accept); break;
+      case ANISO_Z: k_sweeps_sc_coop<ANISO_Z, true><<<n_replicas, threads, 0, st>>>(s, L, t, p, sweep0, n_sweeps, nblk, partials, series, final_out, betas, stride, n_accept); break;
+      default: k_sweeps_sc_coop<ANISO_GENERAL, true><<<n_replicas, threads, 0, st>>>(s, L, t, p, sweep0, n_sweeps, nblk, partials, series, final_out, betas, stride, n_accept); break;
     }
     return cudaGetLastError();
   }
   dim3 vgrid; int threads;
   sc_launch_shape(L, t, 4, vgrid, threads);
-  void (*kern)(float*, ScLayout, ScTile, SweepParams, unsigned long long, int, uint3, double*, double*, double*, const float*, unsigned long long);
+  void (*kern)(float*, ScLayout, ScTile, SweepParams, unsigned long long, int, uint3, double*, double*, double*, const float*, unsigned long long, unsigned long long*);
   switch (aniso) {
     case ANISO_NONE: kern = k_sweeps_sc_coop<ANISO_NONE, false>; break;
     case ANISO_Z: kern = k_sweeps_sc_coop<ANISO_Z, false>; break;
@@ -644,7 +649,7 @@ cudaError_t launch_sweeps_sc_coop(cudaStream_t st, float* s, ScLayout L, ScTile 
   unsigned long long s0 = sweep0;
   const float* no_betas = nullptr;
   unsigned long long no_stride = 0;
-  void* args[] = {&s, &L, &t, &p, &s0, &n_sweeps, &nblk, &partials, &series, &final_out, &no_betas, &no_stride};
+  void* args[] = {&s, &L, &t, &p, &s0, &n_sweeps, &nblk, &partials, &series, &final_out, &no_betas, &no_stride, &n_accept};
   return cudaLaunchCooperativeKernel((const void*)kern, dim3(grid), dim3(threads), args, 0, st);
 }
 

@@ -80,6 +80,103 @@ extern "C" int hb_probe_alu(void* cuda_stream, double seconds, double* updates_p
   return rc;
 }
 
+// ---- hb_device_math: the building blocks of an attempt, element by element (include/hb.h) ----------------------------------
+namespace hb {
+namespace {
+
+// one thread per PAIR of elements (2t, 2t+1): the scalar path on each, and the packed fp32x2 path on the pair
+__global__ void __launch_bounds__(256) k_device_math(int op, long long count, const uint32_t* in0, const uint32_t* in1, float* out) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long i = 2 * t, j = (i + 1 < count) ? i + 1 : i;
+  if (i >= count) return;
+  const uint32_t a0 = in0[i], b0 = in0[j];
+  const uint32_t a1 = in1 ? in1[i] : 0u, b1 = in1 ? in1[j] : 0u;
+  switch (op) {
+    case HB_MATH_U01: {
+      const f2 p = u01_2(a0, b0);
+      out[2 * i] = u01(a0); out[2 * i + 1] = p.x;
+      if (j != i) { out[2 * j] = u01(b0); out[2 * j + 1] = p.y; }
+      break;
+    }
+    case HB_MATH_SINCOS: {   // scalar only: the packed evaluation is part of HB_MATH_SPHERE
+      float s, c;
+      sincos_spec((a0 >> 8) | 1u, s, c); out[2 * i] = s; out[2 * i + 1] = c;
+      if (j != i) { sincos_spec((b0 >> 8) | 1u, s, c); out[2 * j] = s; out[2 * j + 1] = c; }
+      break;
+    }
+    case HB_MATH_SPHERE: {
+      float x, y, z;
+      f2 nx, ny, nz;
+      proposal2(Rand4{a0, a1, 0u, 0u}, Rand4{b0, b1, 0u, 0u}, nx, ny, nz);
+      sphere(a0, a1, x, y, z);
+      out[6 * i] = x; out[6 * i + 1] = y; out[6 * i + 2] = z; out[6 * i + 3] = nx.x; out[6 * i + 4] = ny.x; out[6 * i + 5] = nz.x;
+      if (j != i) {
+        sphere(b0, b1, x, y, z);
+        out[6 * j] = x; out[6 * j + 1] = y; out[6 * j + 2] = z; out[6 * j + 3] = nx.y; out[6 * j + 4] = ny.y; out[6 * j + 5] = nz.y;
+      }
+      break;
+    }
+    case HB_MATH_EXP: {
+      const f2 p = exp_spec2(make_float2(__uint_as_float(a0), __uint_as_float(b0)));
+      out[2 * i] = exp_spec(__uint_as_float(a0)); out[2 * i + 1] = p.x;
+      if (j != i) { out[2 * j] = exp_spec(__uint_as_float(b0)); out[2 * j + 1] = p.y; }
+      break;
+    }
+    case HB_MATH_SQRT: {   // w = 1 - z^2 of the proposal from random word r0: sqrt_rn_unit(w) beside the IEEE square root
+      const float za = __fmaf_rn(-2.0f, u01(a0), 1.0f), zb = __fmaf_rn(-2.0f, u01(b0), 1.0f);
+      const float wa = __fmaf_rn(-za, za, 1.0f), wb = __fmaf_rn(-zb, zb, 1.0f);
+      out[2 * i] = sqrt_rn_unit(wa); out[2 * i + 1] = __fsqrt_rn(wa);
+      if (j != i) { out[2 * j] = sqrt_rn_unit(wb); out[2 * j + 1] = __fsqrt_rn(wb); }
+      break;
+    }
+    case HB_MATH_ATTEMPT: {  // whole packed attempts against given old spins and fields: in0 = site ids, in1 = 16 words per
+      // element (sweep_lo, sweep_hi, seed_lo, seed_hi, J, K, beta, ex, ey, ez, hx, hy, hz, sx, sy, sz as float bits)
+      const uint32_t* pa = in1 + 16 * i; const uint32_t* pb = in1 + 16 * j;
+      auto F = [](uint32_t w) { return __uint_as_float(w); };
+      const Rand4 ra = philox4x32_10(a0, 0u, pa[0], pa[1], pa[2], pa[3]);
+      const Rand4 rb = philox4x32_10(b0, 0u, pb[0], pb[1], pb[2], pb[3]);
+      // the pair shares (J, K, beta, e) of element i, as the lanes of a kernel do
+      f2 sx = make_float2(F(pa[13]), F(pb[13])), sy = make_float2(F(pa[14]), F(pb[14])), sz = make_float2(F(pa[15]), F(pb[15]));
+      bool aa, ab;
+      attempt2<ANISO_GENERAL>(ra, rb, F(pa[4]), F(pa[5]), F(pa[6]), F(pa[7]), F(pa[8]), F(pa[9]), make_float2(F(pa[10]), F(pb[10])),
+                              make_float2(F(pa[11]), F(pb[11])), make_float2(F(pa[12]), F(pb[12])), sx, sy, sz, aa, ab);
+      out[4 * i] = sx.x; out[4 * i + 1] = sy.x; out[4 * i + 2] = sz.x; out[4 * i + 3] = aa ? 1.0f : 0.0f;
+      if (j != i) { out[4 * j] = sx.y; out[4 * j + 1] = sy.y; out[4 * j + 2] = sz.y; out[4 * j + 3] = ab ? 1.0f : 0.0f; }
+      break;
+    }
+    default: break;
+  }
+}
+
+}  // namespace
+}  // namespace hb
+
+extern "C" int hb_device_math(int32_t op, int64_t count, const uint32_t* in0, const uint32_t* in1, float* out) {
+  static const int per_out[] = {2, 2, 6, 2, 2, 4};
+  static const int per_in1[] = {0, 0, 1, 0, 0, 16};
+  if (op < 0 || op > HB_MATH_ATTEMPT || count < 0 || count > (int64_t(1) << 26) || !in0 || !out || (per_in1[op] && !in1)) return HB_EINVAL;
+  if (count == 0) return HB_OK;
+  const size_t nb0 = (size_t)count * 4, nb1 = (size_t)count * 4 * per_in1[op], nbo = (size_t)count * 4 * per_out[op];
+  uint32_t *d0 = nullptr, *d1 = nullptr;
+  float* dout = nullptr;
+  int rc = HB_OK;
+  if (cudaMalloc(&d0, nb0) != cudaSuccess || (nb1 && cudaMalloc(&d1, nb1) != cudaSuccess) || cudaMalloc(&dout, nbo) != cudaSuccess) rc = HB_ENOMEM;
+  if (rc == HB_OK) {
+    cudaError_t e = cudaMemcpy(d0, in0, nb0, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && nb1) e = cudaMemcpy(d1, in1, nb1, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+      const long long pairs = (count + 1) / 2;
+      hb::k_device_math<<<(unsigned)((pairs + 255) / 256), 256>>>(op, (long long)count, d0, d1, dout);
+      e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(out, dout, nbo, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) rc = HB_ECUDA;
+  }
+  cudaFree(d0); cudaFree(d1); cudaFree(dout);
+  cudaGetLastError();
+  return rc;
+}
+
 // ---- device memory another process can map (include/hb.h) ----------------------------------------------------------------
 static_assert(sizeof(cudaIpcMemHandle_t) == 64, "CUDA IPC handle size");
 

@@ -113,7 +113,7 @@ __device__ __forceinline__ void ws_producer(const float* b, const ScLayout& L, c
 // ---- consumers -------------------------------------------------------------------------------------------
 template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS, bool SLAB>
 __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const WsTiles& w, const SweepParams& P, int colour,
-                                            int mode, unsigned char* smem, uint32_t sbase, double acc[4]) {
+                                            int mode, unsigned char* smem, uint32_t sbase, double acc[4], unsigned& n_acc) {
   using S = WsSmem<TY, ROWB, kNB, MINB>;
   const uint32_t fullB = sbase + S::OFF_BAR, emptyB = fullB + 8u * kNB;
   const int32_t HV = L.H >> 2;
@@ -213,6 +213,7 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
           sp[0].v[k] = px.x; sp[0].v[k + 1] = px.y; sp[1].v[k] = py.x; sp[1].v[k + 1] = py.y;
           sp[2].v[k] = pz.x; sp[2].v[k + 1] = pz.y;
           any |= acc_a | acc_b;
+          if (MEAS) n_acc += (unsigned)acc_a + (unsigned)acc_b;
         }
         if (any) {
           store<4>(gx, sp[0]);
@@ -269,13 +270,17 @@ k_sweep_sc_ws(float* a, const float* b, ScLayout L, WsTiles w, SweepParams P, in
   }
   __syncthreads();
   double acc[4] = {0.0, 0.0, 0.0, 0.0};
+  unsigned n_acc = 0;
   if (threadIdx.x < 32) ws_producer<TY, ROWB, kNB, MINB>(b, L, w, smem, sbase);
-  else ws_consumer<TY, ROWB, kNB, MINB, ANISO, MEAS, SLAB>(a, L, w, P, colour, m.mode, smem, sbase, acc);
+  else ws_consumer<TY, ROWB, kNB, MINB, ANISO, MEAS, SLAB>(a, L, w, P, colour, m.mode, smem, sbase, acc, n_acc);
   if (threadIdx.x == 0) {   // this thread took the CTA's last tile number above; the last CTA to finish re-arms the scheduler
     __threadfence();
     if (atomicAdd(w.sched + 1, 1u) == gridDim.x - 1) { w.sched[0] = 0u; w.sched[1] = 0u; }
   }
-  if (MEAS) block_reduce4(acc[0], acc[1], acc[2], acc[3], m.partials + (size_t)blockIdx.x * 4);
+  if (MEAS) {
+    block_reduce4(acc[0], acc[1], acc[2], acc[3], m.partials + (size_t)blockIdx.x * 4);
+    count_accepts(m.n_accept, n_acc);
+  }
 }
 
 template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS, bool SLAB = false>

@@ -56,6 +56,36 @@ def test_library_has_sm100a_code_only():
     assert archs == {"100a"}, archs
 
 
+def test_packed_multiplies_are_not_contracted_into_fused_multiply_adds():
+    """The arithmetic contract spells out every fused multiply-add.  ptxas 12.9 contracts
+    mul.rn.f32x2 + add.rn.f32x2 into one FFMA2 although both carry .rn (hb_device.cuh, add2_prod): one rounding where
+    the oracle has two.  Guard: the arithmetic probe holds exactly two packed ANISO_Z attempts per iteration, each with
+    13 packed multiplications that must survive as FMUL2, and 24 written fused multiply-adds plus the one fma(prod, 1, c)
+    of exp_spec2 that stands for an addition; the warp-specialised and direct sc kernels hold the same two attempts."""
+    import shutil
+    import subprocess
+    exe = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(exe):
+        pytest.skip("cuobjdump not available")
+    sass = subprocess.run([exe, "-sass", binding.library_path()], capture_output=True, text=True).stdout
+    funcs = {}
+    name = None
+    for line in sass.splitlines():
+        m = re.search(r"Function : (\S+)", line)
+        if m:
+            name = m.group(1)
+            funcs[name] = []
+        elif name is not None:
+            funcs[name].append(line)
+    def mix(substr):
+        hit = [k for k in funcs if substr in k]
+        assert len(hit) == 1, (substr, hit)
+        text = "\n".join(funcs[hit[0]])
+        return len(re.findall(r"\bFMUL2\b", text)), len(re.findall(r"\bFFMA2\b", text))
+    for kernel in ("k_probe_alu", "k_sweep_sc_wsILi7ELi1024ELi4ELi2ELi1ELb0ELb0E", "k_sweep_scILi4ELi1ELb0ELi1ELi256ELb0ELb0E"):
+        assert mix(kernel) == (26, 50), (kernel, mix(kernel))
+
+
 def test_strerror_and_null_arguments():
     lib = hb.load_library()
     assert lib.hb_strerror(0) == b"ok"

@@ -635,3 +635,67 @@ def test_programmatic_launches_match_the_oracle():
                 assert spins_equal(ctx.get_spins(), st.get_spins()), (name, graph)
                 _measure_close(ctx, st, lat.n)
             ctx.close()
+
+
+@pytest.mark.parametrize("name", ["sc16_c1", "sc24_K", "sc_wide", "sc_v2_ragged", "bcc8", "fcc6", "sphere5", "sc_persite"])
+def test_stats_count_the_accepted_moves_like_the_oracle(name):
+    # hb_stats (rule (iii) [P:20] defines an accepted move): the device counts, inside the measuring passes,
+    # exactly the moves the oracle accepts
+    cfg = SMALL_CASES[name]
+    ctx = make_gpu(cfg)
+    lat, st = make_oracle(cfg)
+    start(cfg, ctx, st)
+    n = lat.n
+    assert ctx.stats() == (0, 0)
+    for T in (cfg["T"][0], 0.4):
+        for _ in range(3):                      # one-sweep calls: every sweep is the last of its call, so every sweep counts
+            ctx.sweep(T, 1)
+            st.sweep(T, 1)
+    assert ctx.stats() == st.stats() == (6 * n, st.stats()[1])
+    ctx.sweep_series(1.1, 5)                    # every sweep of a series counts
+    st.sweep(1.1, 5)
+    assert ctx.stats() == st.stats()
+    before = ctx.stats()
+    ctx.sweep(0.9, 19)                          # a longer call counts its last sweep only (graph replay + a measured tail)
+    acc = st.sweep(0.9, 19, record=True)
+    after = ctx.stats()
+    assert after[0] - before[0] == n and after[1] - before[1] == int(acc[-1].sum())
+    got = ctx.sweep_record(0.9)                 # a recorded sweep counts what it records
+    assert ctx.stats()[1] - after[1] == int(got.sum()) and ctx.stats()[0] - after[0] == n
+    assert spins_equal(ctx.get_spins(), (st.sweep(0.9, 1), st.get_spins())[1])
+    ctx.close()
+
+
+def test_stats_on_the_warp_specialised_kernel_and_on_replicas():
+    cfg = dict(W.SMALL["c4"], L=(64, 12, 10))
+    ctx = make_gpu(cfg)
+    ctx.set_option("sc_coop", 0)
+    ctx.set_option("sc_kernel", 1)
+    lat, st = make_oracle(cfg)
+    start(cfg, ctx, st)
+    for _ in range(4):
+        ctx.sweep(1.44, 1)
+        st.sweep(1.44, 1)
+    assert ctx.stats() == st.stats()
+    ctx.close()
+    # replicas: the counter sums over all of them
+    R, T = 5, [0.8, 1.2, 1.44, 2.0, 3.0]
+    lat_g = hb.Lattice("sc", 8, 8, 8, n_replicas=R)
+    ctx = hb.Context(lat_g, 1.0, 0.01, (0, 0, 1), seed=7)
+    ctx.init_random()
+    want_att = want_acc = 0
+    olat = oracle.Lattice.sc(8)
+    olat.set_uniform_anisotropy(0.01, (0, 0, 1))
+    sts = [oracle.State32(olat, 1.0, 7 + r) for r in range(R)]
+    for s in sts:
+        s.init_random()
+    for _ in range(3):
+        ctx.sweep_each(T, 1)
+        for r, s in enumerate(sts):
+            s.sweep(T[r], 1)
+    for s in sts:
+        a, b = s.stats()
+        want_att += a
+        want_acc += b
+    assert ctx.stats() == (want_att, want_acc)
+    ctx.close()

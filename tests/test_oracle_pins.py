@@ -336,10 +336,35 @@ def test_delta_h_equals_bruteforce_energy_difference(make):
         T2[i] = new32
         assert abs(float(st32.delta_h(i, new32)) - (_total_energy_numpy(lat, J, T2) - E0_32)) <= 1e-5
     # the measured energy is the same total
-    _, e32, e64 = st32.measure()
+    m32, e32, e64 = st32.measure()
     assert abs(e64 - E0_32) <= 1e-9 and abs(e32 - E0_32) <= 2e-6 * n
+    # eq. (2) [P:22] by component, sign included: a permuted or negated component of O32's M fails here
+    want_m = S32.astype(np.float64).mean(0)
+    assert np.max(np.abs(np.asarray(m32, np.float64) - want_m)) <= 1e-7
+    assert np.max(np.abs(want_m)) > 1e-3 and len({round(abs(float(v)), 6) for v in want_m}) == 3   # the pin can tell components apart
     M, E = st64.measure()
     assert abs(E - E0) <= 1e-10 and np.allclose(M, S.mean(0), atol=1e-14)
+
+
+@pytest.mark.parametrize("make", [lambda: oracle.Lattice.sc(4), lambda: oracle.Lattice.bcc(3), lambda: oracle.Lattice.fcc(2),
+                                  lambda: oracle.Lattice.fcc_sphere(2)])
+def test_o32_magnetisation_by_component(make):
+    # eq. (2) [P:22]: M = (1/N) sum_i S_i as a VECTOR.  A state whose three component sums are distinct, of mixed sign and
+    # known in closed form: S_i = (0.6, 0, -0.8) on even sites, (0, 1, 0) on odd ones.
+    lat = make()
+    lat.set_uniform_anisotropy(0.0, (0, 0, 1))
+    n = lat.n
+    even = (np.arange(n) % 2 == 0)
+    sx = np.where(even, np.float32(0.6), np.float32(0.0)).astype(np.float32)
+    sy = np.where(even, np.float32(0.0), np.float32(1.0)).astype(np.float32)
+    sz = np.where(even, np.float32(-0.8), np.float32(0.0)).astype(np.float32)
+    st = oracle.State32(lat, 1.0, 1)
+    st.set_spins(sx, sy, sz)
+    M = np.asarray(st.measure()[0], np.float64)
+    ne = int(even.sum())
+    want = np.array([float(np.float32(0.6)) * ne / n, (n - ne) / n, float(np.float32(-0.8)) * ne / n])
+    assert np.max(np.abs(M - want)) <= 1e-12
+    assert M[0] > 0 > M[2] and M[1] > M[0]
 
 
 # ---- K12/K13: invariants of the counter-based stream ----------------------------------
