@@ -150,6 +150,24 @@ def make_context(cfg, seed_offset, device):
     return ctx
 
 
+def host_cpu():
+    """Model string and core count of the box the oracle is timed on ("oracle timing beside it")."""
+    model = "unknown"
+    try:
+        with open("/proc/cpuinfo") as f:
+            for ln in f:
+                if ln.lower().startswith("model name"):
+                    model = ln.split(":", 1)[1].strip()
+                    break
+    except OSError:
+        pass
+    return model, os.cpu_count() or 0
+
+
+def sample_lattice_label(scfg):
+    return "%s %s" % (scfg["kind"], scfg.get("L", scfg.get("R")))
+
+
 def cpu_sample_cfg(cfg):
     """A bounded sample of the workload for the single-threaded oracle (about 10-30 s of CPU work)."""
     if cfg["kind"] == "sc" and cfg["L"] > 232:
@@ -187,8 +205,10 @@ def run_cpu_baseline(cfg, budget_attempts=2.5e8):   # ~14 s at the oracle's 55 n
     st.sweep(T, sweeps)
     st.measure()
     dt = time.perf_counter() - t0
+    model, nproc = host_cpu()
     return {"value": n * sweeps / dt / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
             "sample": "%s; %d sweeps + 1 measurement (%d attempts), O32 single thread" % (what, sweeps, n * sweeps),
+            "sample_lattice": sample_lattice_label(scfg), "cpu_model": model, "nproc": nproc,
             "ns_per_update": dt / (n * sweeps) * 1e9}
 
 
@@ -209,13 +229,18 @@ def run_reference(args, cfg, name):
     dt = time.perf_counter() - t0
     value = lat.n * args.steps / dt / 1e9
     sample = "%s; each step = 1 sweep + 1 measurement of the sample, O32 single thread" % what
+    model, nproc = host_cpu()
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": name, "lattice": "%s %s" % (cfg["kind"], cfg.get("L", cfg.get("R"))),
-                   "T": T, "J": cfg["J"], "K": cfg["K"]},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        # the lattice that RAN: the bounded sample of the workload, not the workload's full size
+        "config": {"workload": name,
+                   "lattice": sample_lattice_label(scfg) if scfg == cfg else
+                   "%s (bounded sample of the workload's %s)" % (sample_lattice_label(scfg), sample_lattice_label(cfg)),
+                   "n_spins": lat.n, "T": T, "J": cfg["J"], "K": cfg["K"]},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                         "sample_lattice": sample_lattice_label(scfg), "cpu_model": model, "nproc": nproc},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
@@ -374,7 +399,9 @@ def main():
         if sampler:
             time.sleep(0.5)          # nvidia-smi needs a moment before its first sample
             ctx.sweep(T, min(SWEEPS_PER_STEP, 20))   # keep the device under load while it starts
+        stats0 = ctx.stats()
         ms, ms_sweeps, launches = timed_run(args.steps)
+        stats1 = ctx.stats()
         clocks = sampler.stop() if sampler else None
         bad = clocks and any(r in clocks["reasons"] for r in ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"))
         if not bad:
@@ -431,8 +458,9 @@ def main():
                                       "4 attempts per thread as two packed pairs, 256-thread blocks, 4 per SM, measured in this run"}
 
     cpu = None if args.no_cpu_baseline else run_cpu_baseline(cfg)
-    # acceptance rate of one more sweep of the state the run ended in (reported with every timed config)
-    acceptance = float(ctx.sweep_record(T).mean())
+    # acceptance rate of the timed sweeps themselves (reported with every timed config): hb_stats counts the
+    # accepted moves inside the measuring passes, i.e. in the last sweep of every timed step
+    acceptance = (stats1[1] - stats0[1]) / max(1, stats1[0] - stats0[0])
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -442,7 +470,7 @@ def main():
                    "lattice": "%s %s" % (cfg["kind"], cfg.get("L", cfg.get("R"))), "n_spins": n, "colours": n_colours,
                    "J": cfg["J"], "K": cfg["K"], "T": T, "start": cfg["start"], "seed": cfg["seed"],
                    "sweeps_per_step": SWEEPS_PER_STEP, "measurements_per_step": 1, "options": options,
-                   "acceptance_rate": acceptance,
+                   "acceptance_rate": acceptance, "acceptance_counted_attempts": stats1[0] - stats0[0],
                    "l2": "state %.0f MB >> 126 MB L2: no flush between iterations" % (12.0 * n / 1e6)
                    if 12.0 * n > 4 * 126e6 else "state fits in L2: HBM roofline not meaningful",
                    "multi_gpu": "replicas only (seed + rank)"},

@@ -223,6 +223,15 @@ int hb_probe_alu(void* cuda_stream, double seconds, double* updates_per_second);
 enum { HB_MATH_U01 = 0, HB_MATH_SINCOS = 1, HB_MATH_SPHERE = 2, HB_MATH_EXP = 3, HB_MATH_SQRT = 4, HB_MATH_ATTEMPT = 5 };
 int hb_device_math(int32_t op, int64_t count, const uint32_t* in0, const uint32_t* in1, float* out);
 
+/* Diagnostic: the rate (attempted updates per second) of the warp-specialised simple cubic colour kernel when its HBM
+ * traffic is taken away: n_sweeps sweeps (two launches each, timed with CUDA events after two untimed ones) in which plane z
+ * is read and written at the address of plane z mod `planes` (a power of two, e.g. 16), so that the whole launch lives in
+ * a few L2-resident planes while every attempt is still computed.  It is the ceiling of any scheme that keeps the kernel's
+ * arithmetic and only removes DRAM traffic (fused colours, temporal blocking: DESIGN.md 6.9).  The result is NOT a
+ * trajectory: the call leaves the spins undefined (HB_ESTATE until hb_init_* / hb_set_spins).  Simple cubic, whole lattice,
+ * rows that fit the kernel's 7-row variant.  Synchronises. */
+int hb_probe_sc_l2(hb_ctx* ctx, float T, int64_t n_sweeps, int32_t planes, double* updates_per_second);
+
 /* Tuning knobs, by name (DESIGN.md section 6 lists them); unknown names give HB_EINVAL. */
 int hb_set_option(hb_ctx* ctx, const char* name, int64_t value);
 int hb_get_option(hb_ctx* ctx, const char* name, int64_t* value);

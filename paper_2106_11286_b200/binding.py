@@ -18,7 +18,7 @@ EXPORTS = [
     "hb_sweep_each", "hb_measure_each", "hb_sweep_series_each", "hb_select_replica",
     "hb_slab_pass", "hb_slab_next_sweep", "hb_slab_face", "hb_slab_set_peer", "hb_probe_alu",
     "hb_device_alloc", "hb_device_free", "hb_ipc_export", "hb_ipc_open", "hb_ipc_close",
-    "hb_get_colouring", "hb_counters", "hb_stats", "hb_device_math", "hb_set_option", "hb_get_option", "hb_lattice_fcc_sphere", "hb_lattice_free",
+    "hb_get_colouring", "hb_counters", "hb_stats", "hb_device_math", "hb_probe_sc_l2", "hb_set_option", "hb_get_option", "hb_lattice_fcc_sphere", "hb_lattice_free",
     "hb_strerror", "hb_error_detail",
 ]
 
@@ -91,6 +91,7 @@ def load_library():
         "hb_counters": [vp, P(u64), P(u64)],
         "hb_stats": [vp, P(u64), P(u64)],
         "hb_device_math": [i32, i64, vp, vp, vp],
+        "hb_probe_sc_l2": [vp, f32, i64, i32, P(C.c_double)],
         "hb_set_option": [vp, C.c_char_p, i64],
         "hb_get_option": [vp, C.c_char_p, P(i64)],
         "hb_lattice_fcc_sphere": [i32, f32, P(f32), f32, i32, P(hb_lattice), P(vp)],
@@ -413,6 +414,12 @@ class Context:
         a, b = C.c_uint64(), C.c_uint64()
         self._check(self._L.hb_stats(self._h, C.byref(a), C.byref(b)), "hb_stats")
         return a.value, b.value
+
+    def probe_sc_l2(self, T, n_sweeps=50, planes=16):
+        """hb_probe_sc_l2: updates per second of the sc colour kernel with its HBM traffic folded into L2 (destroys the state)."""
+        v = C.c_double()
+        self._check(self._L.hb_probe_sc_l2(self._h, T, int(n_sweeps), int(planes), C.byref(v)), "hb_probe_sc_l2")
+        return v.value
 
     def set_option(self, name, value):
         self._check(self._L.hb_set_option(self._h, name.encode(), int(value)), "hb_set_option(%s)" % name)

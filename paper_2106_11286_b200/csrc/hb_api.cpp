@@ -31,7 +31,7 @@ struct Plan {                 // device memory plan of a lattice
   int32_t maxdeg = 0;
   size_t off_ell = 0, off_cbegin = 0;
   size_t spins_bytes = 0, ws_bytes = 0;
-  size_t off_partials = 0, off_series = 0, off_counters = 0, off_staging = 0;
+  size_t off_partials = 0, off_series = 0, off_counters = 0, off_staging = 0, off_wsdone = 0;
   size_t off_row_ptr = 0, off_col = 0, off_list = 0, off_K = 0, off_e = 0;
 };
 
@@ -105,6 +105,7 @@ int make_plan(const hb_lattice* lat, Plan& p, std::string& why) {
   p.off_series = o;   o += align_up((size_t)p.R * kSeriesChunk * 4 * sizeof(double));
   p.off_counters = o; o += kAlign;
   p.off_staging = o;  o += align_up((size_t)p.n * sizeof(float));
+  if (p.engine == ENGINE_SC) { p.off_wsdone = o; o += align_up((size_t)kWsDoneWords * sizeof(uint32_t)); }   // progress words of fused launches
   if (p.R > 1) {
     p.off_each = o;  o += align_up((size_t)p.R * 20 * sizeof(double));
     p.off_betas = o; o += align_up((size_t)p.R * sizeof(float));
@@ -142,7 +143,9 @@ struct hb_ctx {
   CsrDev csr{};
   EllDev ell{};
   int csr_block = 128;
-  int sc_kernel = 0;      // 0: direct loads through L1, 1: warp-specialised persistent kernel (TMA-staged neighbour planes)
+  int sc_kernel = 0;      // 0: direct loads through L1, 1: warp-specialised persistent kernel (TMA-staged neighbour planes),
+                          // 2: the same kernel with all colour passes of up to fused_sweeps sweeps in ONE launch
+  int fused_sweeps = 8, fused_lag = 6, fused_zt = 24;   // the fastest setting measured on c4
   int ws_zt = 0, n_sms = 148, ws_variant = 2;   // warp-specialised kernel: planes per tile (0: balanced automatically), CTAs = n_sms x CTAs/SM
   int graph_mode = -1;         // replay hb_sweep's launches from a CUDA graph: -1 auto (lattices up to 2^23 sites), 0 off, 1 on
   cudaStream_t cap_stream = nullptr;
@@ -184,6 +187,7 @@ struct hb_ctx {
   unsigned long long* sweep_dev() const { return reinterpret_cast<unsigned long long*>(ws + plan.off_counters + 128); }
   unsigned long long* series_idx() const { return reinterpret_cast<unsigned long long*>(ws + plan.off_counters + 136); }
   uint32_t* ws_sched() const { return reinterpret_cast<uint32_t*>(ws + plan.off_counters + 144); }   // tile scheduler of k_sweep_sc_ws
+  uint32_t* ws_done() const { return reinterpret_cast<uint32_t*>(ws + plan.off_wsdone); }            // progress words of its fused launches
 };
 
 namespace {
@@ -253,7 +257,7 @@ ScTile default_tile(int32_t H, int32_t Ly, int32_t Lz) {
 int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d, Meas m = Meas{nullptr, 0, nullptr}) {
   if (c->plan.engine == ENGINE_SC) {
     const bool diag = d.accept || d.n_accept;
-    if (c->sc_kernel == 1 && !diag)
+    if (c->sc_kernel >= 1 && !diag)
       HB_CUDA(c, launch_sweep_sc_ws(c->stream, c->spins, c->sc, c->ws_zt, c->n_sms, c->ws_variant, c->ws_sched(), p, colour, m));
     else
       HB_CUDA(c, launch_sweep_sc(c->stream, c->spins, c->sc, c->tile, p, colour, d, m));
@@ -274,6 +278,7 @@ int fused_blocks(const hb_ctx* c) {
   if (!c->fused_measure) return 0;
   if (c->plan.engine == ENGINE_BRAVAIS) return bravais_fused_blocks(c->br, c->tile);
   if (c->plan.engine != ENGINE_SC) return 0;
+  if (c->sc_kernel == 2) return sc_ws_fused_blocks(c->sc, c->fused_zt, c->n_sms, c->ws_variant, 1);
   if (c->sc_kernel == 1) return sc_ws_blocks(c->sc, c->ws_zt, c->n_sms, c->ws_variant);
   return sc_fused_blocks(c->sc, c->tile);
 }
@@ -303,12 +308,35 @@ int coop_sweeps(hb_ctx* c, float beta, int64_t n_sweeps, double* series, double*
   return HB_OK;
 }
 
+// sc_kernel = 2: n_sweeps whole sweeps in ONE launch (both colours of every sweep, tiles with dependencies instead of a launch
+// boundary per colour); with dev_out the launch is one sweep whose passes also reduce M and E, as in one_sweep below
+int fused_sweeps_launch(hb_ctx* c, float beta, int n_sweeps, double* dev_out, bool counted) {
+  const SweepParams p = params(c, beta);
+  Meas m{nullptr, 0, nullptr};
+  const int fb = dev_out ? fused_blocks(c) : 0;
+  if (fb) m = Meas{c->partials(), 2, counted ? c->counters() : nullptr};
+  HB_CUDA(c, launch_sweep_sc_ws_fused(c->stream, c->spins, c->sc, c->fused_zt, c->fused_lag, c->n_sms, c->ws_variant, c->ws_sched(), c->ws_done(),
+                                      p, n_sweeps, m));
+  c->launches += 1;
+  if (fb) {
+    HB_CUDA(c, launch_reduce_final(c->stream, c->partials(), fb, dev_out));
+    c->launches += 1;
+    if (counted) c->stat_attempts += (uint64_t)c->plan.n;
+  }
+  c->sweep += (uint64_t)n_sweeps;
+  c->attempts += (uint64_t)n_sweeps * (uint64_t)c->plan.n;
+  return HB_OK;
+}
+
+bool fused_kernel(const hb_ctx* c) { return c->plan.engine == ENGINE_SC && c->sc_kernel == 2; }
+
 // one sweep; with dev_out != nullptr (and fused_blocks() > 0) the colour passes also reduce M and E of
 // the state they leave behind, and dev_out receives (sum Sx, sum Sy, sum Sz, E).  counted: the accepted moves of the
 // sweep are added to the device counter behind hb_stats (in the measuring passes, else through the diagnostic variant)
 int one_sweep(hb_ctx* c, float beta, Diag d, double* dev_out = nullptr, bool counted = false) {
   const SweepParams p = params(c, beta);
   const int fb = dev_out ? fused_blocks(c) : 0;
+  if (fused_kernel(c) && !d.accept && !d.n_accept && (fb || !counted)) return fused_sweeps_launch(c, beta, 1, fb ? dev_out : nullptr, counted);
   if (counted && !fb) d.n_accept = c->counters();
   if (counted || d.n_accept) c->stat_attempts += (uint64_t)c->plan.n;
   for (int colour = 0; colour < c->n_colours; ++colour) {
@@ -597,6 +625,7 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
     c->own_spins = c->own_ws = true;
   }
   HB_CUDA(c, cudaMemsetAsync(c->ws + P.off_counters, 0, kAlign, c->stream));
+  if (P.engine == ENGINE_SC) HB_CUDA(c, cudaMemsetAsync(c->ws + P.off_wsdone, 0, (size_t)kWsDoneWords * sizeof(uint32_t), c->stream));
 
   if (P.engine == ENGINE_CSR) {
     // sites sorted by (colour, id): one contiguous list segment per colour
@@ -811,6 +840,14 @@ int hb_sweep(hb_ctx* c, float T, int64_t n_sweeps) {
     rc = graph_sweeps(c, beta, replays, 0);
     if (rc != HB_OK) return rc;
     s = replays * kGraphSweeps;
+  }
+  if (fused_kernel(c)) {   // all but the last sweep: up to fused_sweeps sweeps per launch
+    while (s < n_sweeps - 1) {
+      const int g = (int)(n_sweeps - 1 - s < c->fused_sweeps ? n_sweeps - 1 - s : c->fused_sweeps);
+      rc = fused_sweeps_launch(c, beta, g, nullptr, false);
+      if (rc != HB_OK) return rc;
+      s += g;
+    }
   }
   for (; s < n_sweeps; ++s) {
     const bool last = s == n_sweeps - 1;   // carries the fused measurement and counts its accepted moves (hb_stats)
@@ -1092,6 +1129,40 @@ int hb_counters(hb_ctx* c, uint64_t* kernel_launches, uint64_t* attempts) {
   return HB_OK;
 }
 
+int hb_probe_sc_l2(hb_ctx* c, float T, int64_t n_sweeps, int32_t planes, double* updates_per_second) {
+  HB_CHECK_CTX(c);
+  if (!updates_per_second || n_sweeps < 1 || n_sweeps > 100000) return fail(c, HB_EINVAL, "hb_probe_sc_l2: 1 <= n_sweeps <= 100000, non-NULL output");
+  if (c->plan.engine != ENGINE_SC || c->slab_Lz > 0 || c->plan.R > 1 || !sc_ws_variant_supported(c->sc, 4) || planes < 2 ||
+      (planes & (planes - 1)) || planes > c->sc.Lz)
+    return fail(c, HB_EINVAL, "hb_probe_sc_l2: a whole simple cubic lattice with rows of 8..472 sites (Lx % 8 == 0), planes a power of two in [2, Lz]");
+  if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
+  float beta;
+  int rc = check_T(c, T, &beta);
+  if (rc != HB_OK) return rc;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  HB_CUDA(c, cudaEventCreate(&e0));
+  if (cudaEventCreate(&e1) != cudaSuccess) { cudaEventDestroy(e0); return fail(c, HB_ECUDA, "cudaEventCreate"); }
+  c->cache_valid = c->each_valid = false;
+  c->initialised = false;   // the folded addresses leave the lattice in no meaningful state
+  SweepParams p = params(c, beta);
+  cudaError_t e = cudaSuccess;
+  for (int64_t s = -2; s < n_sweeps && e == cudaSuccess; ++s) {   // two untimed sweeps first
+    if (s == 0) e = cudaEventRecord(e0, c->stream);
+    for (int colour = 0; colour < 2 && e == cudaSuccess; ++colour)
+      e = launch_sweep_sc_ws_alias(c->stream, c->spins, c->sc, c->n_sms, c->ws_sched(), p, colour, planes);
+    p.sweep_lo += 1;
+    c->launches += 2;
+  }
+  if (e == cudaSuccess) e = cudaEventRecord(e1, c->stream);
+  if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+  float ms = 0.0f;
+  if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  if (e != cudaSuccess) return fail(c, HB_ECUDA, std::string("hb_probe_sc_l2: ") + cudaGetErrorString(e));
+  *updates_per_second = (double)c->plan.n * (double)n_sweeps / ((double)ms * 1e-3);
+  return HB_OK;
+}
+
 int hb_stats(hb_ctx* c, uint64_t* attempts, uint64_t* accepts) {
   HB_CHECK_CTX(c);
   if (!attempts || !accepts) return fail(c, HB_EINVAL, "NULL output");
@@ -1137,13 +1208,27 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
   }
   if (c->plan.engine == ENGINE_CSR) return fail(c, HB_EINVAL, "option not valid for this lattice");
   const bool is_sc = c->plan.engine == ENGINE_SC;
-  if (!is_sc && (s == "sc_kernel" || s == "sc_prefetch" || s == "sc_linear" || s == "sc_ws_zt" || s == "sc_ws_ctas" || s == "sc_ws_variant"))
+  if (!is_sc && (s == "sc_kernel" || s == "sc_prefetch" || s == "sc_linear" || s == "sc_ws_zt" || s == "sc_ws_ctas" || s == "sc_ws_variant" ||
+                 s == "sc_fused_sweeps" || s == "sc_fused_lag" || s == "sc_fused_zt"))
     return fail(c, HB_EINVAL, "option valid for the simple cubic lattice only");
   const int32_t rowH = is_sc ? c->sc.H : c->br.Lx, rowLz = is_sc ? c->sc.Lz : c->br.Lz;
   if (s == "sc_kernel") {
-    if (value != 0 && !(value == 1 && sc_ws_supported(c->sc)))
-      return fail(c, HB_EINVAL, "sc_kernel: 0 (direct) or 1 (warp-specialised; needs Lx % 8 == 0 and Lx <= 512)");
+    if (value == 2 && 2 * c->fused_sweeps * sc_ws_fused_chunks(c->sc, c->fused_zt) > kWsDoneWords) c->fused_sweeps = 1;
+    if (value != 0 && !(value == 1 && sc_ws_supported(c->sc)) &&
+        !(value == 2 && sc_ws_fused_supported(c->sc, c->ws_variant) && 2 * c->fused_sweeps * sc_ws_fused_chunks(c->sc, c->fused_zt) <= kWsDoneWords))
+      return fail(c, HB_EINVAL, "sc_kernel: 0 (direct), 1 (warp-specialised; needs Lx % 8 == 0 and Lx <= 512) or 2 (the same with all colour "
+                                "passes of several sweeps in one launch; whole lattices, sc_ws_variant 2, 4 or 5)");
     c->sc_kernel = (int)value;
+    return HB_OK;
+  }
+  if (s == "sc_fused_sweeps" || s == "sc_fused_lag" || s == "sc_fused_zt") {
+    if (s == "sc_fused_sweeps") { if (value < 1 || value > 16) return fail(c, HB_EINVAL, "sc_fused_sweeps: 1..16 sweeps per launch"); c->fused_sweeps = (int)value; }
+    else if (s == "sc_fused_lag") { if (value < 3 || value > 64) return fail(c, HB_EINVAL, "sc_fused_lag: 3..64 rounds between two colour passes"); c->fused_lag = (int)value; }
+    else { if (value < 1 || value > c->sc.Lz) return fail(c, HB_EINVAL, "sc_fused_zt: 1..Lz planes per chunk"); c->fused_zt = (int)value; }
+    if (2 * c->fused_sweeps * sc_ws_fused_chunks(c->sc, c->fused_zt) > kWsDoneWords) {
+      c->fused_sweeps = 1; c->fused_zt = 8;
+      return fail(c, HB_EINVAL, "sc_fused_*: passes x chunks exceeds the progress words of the workspace");
+    }
     return HB_OK;
   }
   if (s == "sc_ws_zt") {
@@ -1157,6 +1242,7 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
                                 "3 (16-row tiles, 1 CTA per SM; rows of up to 248 floats), 4 (7-row tiles, 2 CTAs per SM; rows of up to 236 floats), "
                                 "5 (8-row tiles at a 512-byte pitch, 3 CTAs per SM; rows of up to 128 floats)");
     c->ws_variant = (int)value;
+    if (c->sc_kernel == 2 && !sc_ws_fused_supported(c->sc, c->ws_variant)) c->sc_kernel = 1;
     return HB_OK;
   }
   if (s == "sc_ws_ctas") {
@@ -1208,6 +1294,9 @@ int hb_get_option(hb_ctx* c, const char* name, int64_t* value) {
   else if (s == "sc_ws_zt") *value = c->ws_zt;
   else if (s == "sc_ws_ctas") *value = c->n_sms;
   else if (s == "sc_ws_variant") *value = c->ws_variant;
+  else if (s == "sc_fused_sweeps") *value = c->fused_sweeps;
+  else if (s == "sc_fused_lag") *value = c->fused_lag;
+  else if (s == "sc_fused_zt") *value = c->fused_zt;
   else return HB_EINVAL;
   return HB_OK;
 }

@@ -134,6 +134,17 @@ bool sc_ws_variant_supported(const ScLayout& L, int variant);
 int sc_ws_blocks(const ScLayout& L, int ZT, int grid_cap, int variant);
 cudaError_t launch_sweep_sc_ws(cudaStream_t st, float* spins, ScLayout L, int ZT, int grid_cap, int variant, uint32_t* sched /* 2 device words, zero */,
                                SweepParams p, int colour, Meas m);
+// diagnostic (hb_probe_sc_l2): one colour pass of the 7-row variant with the address of plane z folded onto plane z mod planes
+cudaError_t launch_sweep_sc_ws_alias(cudaStream_t st, float* spins, ScLayout L, int grid_cap, uint32_t* sched, SweepParams p, int colour, int planes);
+// fused launches of the same kernel: n_sweeps whole sweeps = 2 n_sweeps colour passes in ONE launch, tiles
+// ordered in rounds with `lag` (>= 3) rounds between two passes; done = kWsDoneWords device words, zero between launches;
+// m.mode != 0: the LAST sweep of the launch carries the fused measurement (block partials: one per CTA)
+constexpr int kWsDoneWords = 16384;
+bool sc_ws_fused_supported(const ScLayout& L, int variant);
+int sc_ws_fused_chunks(const ScLayout& L, int ZT);
+int sc_ws_fused_blocks(const ScLayout& L, int ZT, int grid_cap, int variant, int n_sweeps);
+cudaError_t launch_sweep_sc_ws_fused(cudaStream_t st, float* spins, ScLayout L, int ZT, int lag, int grid_cap, int variant, uint32_t* sched,
+                                     uint32_t* done, SweepParams p, int n_sweeps, Meas m);
 cudaError_t launch_sweep_csr(cudaStream_t st, float* spins, CsrDev g, uint32_t list_begin, uint32_t list_count,
                              SweepParams p, int block, Diag d);
 cudaError_t launch_sweep_ell(cudaStream_t st, float* spins, EllDev g, uint32_t begin, uint32_t count, SweepParams p,

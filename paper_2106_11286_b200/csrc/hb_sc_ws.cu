@@ -18,6 +18,16 @@
 //     not once per tile, and no CTA is left with a fixed share when its SM runs slower than the others.
 //
 // Same arithmetic, same order of the neighbour sum, same bits as k_sweep_sc.
+//
+// FUSED (sc_kernel = 2): ONE launch runs several colour passes -- both colours of a sweep, or of several
+// sweeps -- as one stream of tiles with dependencies between them instead of a launch boundary after every colour
+// (the multi-colour tile kernel; the on-chip memory that carries the freshly written colour from one
+// pass to the next is the 126 MB L2 rather than shared memory, so no halo is recomputed and the update stays in place).
+// Pass p = (sweep p/2, colour p%2) walks the z-chunks in the order p, p+1, ... (mod n: the rotation makes the
+// periodic wrap in z a dependency on an EARLIER chunk), `lag` rounds behind pass p-1; its k-th chunk may start when pass
+// p-1 has finished its chunks k, k+1, k+2 (the planes it reads as neighbours, and the readers of what it overwrites).
+// Tiles are handed out in round order from the same device counter, so every dependency of a tile was handed out
+// before it: the oldest unfinished tile can always run, whatever the CTAs hold.
 #include "hb_device.cuh"
 #include "hb_internal.h"
 
@@ -48,21 +58,57 @@ __host__ __device__ constexpr bool ws_pref() { return MINB < 3 && TY != 7; }
 struct WsTiles {
   int32_t n_ty, n_zc;   // tiles in y, chunks in z: chunk zc = planes [zc Lz / n_zc, (zc+1) Lz / n_zc), sizes differ by at most one
   uint32_t* sched;      // device, two words, zero between launches: next tile to hand out, CTAs that have finished
+  // fused launches only: colour passes of the launch (pass p: sweep p / 2, colour p % 2), rounds between two passes (>= 3),
+  // and passes x n_zc progress words, zero between launches: consumer warps that have finished a tile of (pass, k-th chunk)
+  int32_t passes, lag;
+  uint32_t* done;
+  // diagnostic launches only (ALIAS, hb_probe_sc_l2): plane z is read and written at the address of plane z & zmask, so the
+  // whole launch lives in a few L2-resident planes -- the kernel's rate with its HBM traffic taken away
+  uint32_t zmask;
 };
+
+// a tile of a fused launch: pass, position k of its chunk in the pass's order, the chunk itself, the tile in y
+struct FusedTile { int32_t p, k, zc, ty; };
+
+// Round r holds the k-th chunk of pass p for r = lag p + k; within a round passes ascend.  S(r) = (pass, chunk) pairs in
+// rounds before r = sum_p clamp(r - lag p, 0, n).
+__device__ __forceinline__ FusedTile fused_decode(int32_t tile, const WsTiles& w) {
+  const int32_t q = tile / w.n_ty, n = w.n_zc, P = w.passes, lag = w.lag;
+  // passes 0 .. sat-1 have all n chunks behind them at round r, passes sat .. j-1 have r - lag p of them, the rest none
+  auto before = [&](int32_t r) {
+    const int32_t j = min(P, (r + lag - 1) / lag), sat = r >= n ? min(P, (r - n) / lag + 1) : 0;
+    return sat * n + (j - sat) * r - lag * (((sat + j - 1) * (j - sat)) / 2);
+  };
+  int32_t lo = 0, hi = n + lag * (P - 1);   // before(lo) <= q < before(hi)
+  while (hi - lo > 1) { const int32_t mid = (lo + hi) >> 1; if (before(mid) <= q) lo = mid; else hi = mid; }
+  FusedTile t;
+  t.p = (lo < n ? 0 : (lo - n) / lag + 1) + (q - before(lo));
+  t.k = lo - lag * t.p;
+  t.zc = (t.k + t.p) % n;
+  t.ty = tile - q * w.n_ty;
+  return t;
+}
+
+__device__ __forceinline__ uint32_t ld_acquire_gpu(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
 
 // kNB plane slots of the other colour (z-1, z, z+1 and look-ahead); MINB = CTAs per SM the kernel is built for
 template <int TY, int ROWB, int kNB, int MINB>
 struct WsSmem {
   static constexpr uint32_t SLOT_B = 3u * (TY + 2) * ROWB;
   static constexpr uint32_t OFF_BAR = kNB * SLOT_B;   // full[kNB], empty[kNB]
-  static constexpr uint32_t OFF_TILE = OFF_BAR + 8u * (2 * kNB);   // tile[kNB]: the tile a staged plane belongs to, -1 = no more tiles
-  static constexpr uint32_t BYTES = OFF_TILE + 4u * 8u;
-  static_assert(kNB <= 8, "tile words");
+  static constexpr uint32_t OFF_TILE = OFF_BAR + 8u * (2 * kNB);   // info[kNB]: the tile a staged plane belongs to (x = tile, -1 = no more
+                                                                    // tiles; fused launches: y = pass, z = chunk, w = tile in y)
+  static constexpr uint32_t BYTES = OFF_TILE + 16u * kNB;
+  static_assert((OFF_TILE % 16u) == 0, "tile info alignment");
 };
 
 // ---- producer: one warp ------------------------------------------------------------------------------
 // plane k of a tile is lattice plane z0-1+k (periodic), rows y0-1 .. y0+ny (periodic) of the other colour
-template <int TY, int ROWB, int kNB, int MINB>
+template <int TY, int ROWB, int kNB, int MINB, bool FUSED, bool ALIAS>
 __device__ __forceinline__ void ws_producer(const float* b, const ScLayout& L, const WsTiles& w,
                                             unsigned char* smem, uint32_t sbase) {
   using S = WsSmem<TY, ROWB, kNB, MINB>;
@@ -71,8 +117,9 @@ __device__ __forceinline__ void ws_producer(const float* b, const ScLayout& L, c
   const size_t n = L.n;
   const uint32_t fullB = sbase + S::OFF_BAR, emptyB = fullB + 8u * kNB;
   RingPos<kNB> rp;   // next plane slot to fill
-  const int32_t n_tiles = w.n_ty * w.n_zc;
-  volatile int32_t* tile_of = reinterpret_cast<volatile int32_t*>(smem + S::OFF_TILE);
+  const int32_t n_tiles = w.n_ty * w.n_zc * (FUSED ? w.passes : 1);
+  volatile int4* info = reinterpret_cast<volatile int4*>(smem + S::OFF_TILE);
+  const float* const spins = b;   // FUSED: b is the base of the spins; the colour a tile reads depends on its pass
   // Tiles are handed out dynamically (one atomic per tile): the CTAs of a launch do not run at the same speed, and with a
   // fixed share per CTA the fast SMs idled at the end of every launch (ncu: SMs active 70-99 % of the launch).  The
   // consumers learn the tile from a word written beside the plane slot before the slot's "full" barrier is armed.
@@ -82,10 +129,24 @@ __device__ __forceinline__ void ws_producer(const float* b, const ScLayout& L, c
     tile = __shfl_sync(0xffffffffu, tile, 0);
     if (tile >= n_tiles) {   // tell the consumers: the slot they will wait on next carries no plane
       mbar_wait_backoff(emptyB + 8u * rp.slot, rp.par ^ 1u);
-      if (lane == 0) { tile_of[rp.slot] = -1; mbar_arrive(fullB + 8u * rp.slot); }
+      if (lane == 0) { info[rp.slot].x = -1; mbar_arrive(fullB + 8u * rp.slot); }
       break;
     }
-    const int32_t ty = tile % w.n_ty, zc = tile / w.n_ty;
+    int32_t ty = tile % w.n_ty, zc = tile / w.n_ty, pass = 0;
+    if (FUSED) {
+      const FusedTile t = fused_decode(tile, w);
+      ty = t.ty; zc = t.zc; pass = t.p;
+      if (t.p > 0) {   // the chunks of the previous pass this tile reads, and whose readers must be done before it writes
+        if (lane < 3) {
+          const uint32_t* d = w.done + (size_t)(t.p - 1) * w.n_zc + (t.k + (int32_t)lane) % w.n_zc;
+          const uint32_t all = (uint32_t)w.n_ty * ((blockDim.x >> 5) - 1u);
+          while (ld_acquire_gpu(d) < all) __nanosleep(256);
+        }
+        __syncwarp();
+        asm volatile("fence.proxy.async;" ::: "memory");   // the bulk copies below read what other CTAs stored (generic proxy)
+      }
+      b = spins + (size_t)(1 - (t.p & 1)) * L.half;          // pass p updates colour p % 2 and reads the other one
+    }
     const int32_t y0 = ty * TY, ny = min(TY, L.Ly - y0);
     const int32_t z0 = (int32_t)(((int64_t)zc * L.Lz) / w.n_zc), nz = (int32_t)(((int64_t)(zc + 1) * L.Lz) / w.n_zc) - z0;
     for (int32_t k = 0; k < nz + 2; ++k) {
@@ -95,13 +156,16 @@ __device__ __forceinline__ void ws_producer(const float* b, const ScLayout& L, c
         const uint32_t slot = rp.slot;
         mbar_wait_backoff(emptyB + 8u * slot, rp.par ^ 1u);
         const uint32_t n_rows = 3u * (uint32_t)(ny + 2);
-        if (lane == 0) { tile_of[slot] = tile; mbar_expect_tx(fullB + 8u * slot, n_rows * row_bytes); }
+        if (lane == 0) {
+          info[slot].x = tile; info[slot].y = pass; info[slot].z = zc; info[slot].w = ty;
+          mbar_expect_tx(fullB + 8u * slot, n_rows * row_bytes);
+        }
         __syncwarp();
         for (uint32_t q = lane; q < n_rows; q += 32) {
           const uint32_t comp = q / (uint32_t)(ny + 2), r = q - comp * (uint32_t)(ny + 2);
           int32_t yy = y0 - 1 + (int32_t)r;
           yy = yy < 0 ? yy + L.Ly : (yy >= L.Ly ? yy - L.Ly : yy);
-          const float* src = b + comp * n + ((size_t)zz * L.Ly + yy) * L.H;
+          const float* src = b + comp * n + ((size_t)(ALIAS ? (int32_t)((uint32_t)zz & w.zmask) : zz) * L.Ly + yy) * L.H;
           bulk_g2s(sbase + slot * S::SLOT_B + (comp * (TY + 2) + r) * ROWB, src, row_bytes, fullB + 8u * slot);
         }
         rp.next();
@@ -111,7 +175,7 @@ __device__ __forceinline__ void ws_producer(const float* b, const ScLayout& L, c
 }
 
 // ---- consumers -------------------------------------------------------------------------------------------
-template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS, bool SLAB>
+template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS, bool SLAB, bool FUSED, bool ALIAS>
 __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const WsTiles& w, const SweepParams& P, int colour,
                                             int mode, unsigned char* smem, uint32_t sbase, double acc[4], unsigned& n_acc) {
   using S = WsSmem<TY, ROWB, kNB, MINB>;
@@ -129,17 +193,49 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
   const size_t n = L.n;
   const size_t plane = (size_t)L.Ly * L.H;
   RingPos<kNB> rm;   // slot of plane z-1 of the current step
-  const volatile int32_t* tile_of = reinterpret_cast<const volatile int32_t*>(smem + S::OFF_TILE);
+  const volatile int4* info = reinterpret_cast<const volatile int4*>(smem + S::OFF_TILE);
+  float* const spins = a;   // FUSED: a is the base of the spins; the colour a tile updates depends on its pass
+  uint32_t sweep_lo = P.sweep_lo, sweep_hi = P.sweep_hi;
+  int32_t pass = 0;
+  // FUSED: the progress word this warp still has to bump for the tile it finished last.  The bump needs a device-wide
+  // fence behind the tile's stores; issued right after them the fence waits ~1 us for their acknowledgement (ncu: 7 % of
+  // the warps' time in membar).  So it is deferred to just before the first stores of the NEXT tile, one plane of
+  // arithmetic later, when the earlier stores have long been acknowledged.
+  uint32_t* pending = nullptr;
+  auto publish = [&]() {
+    __syncwarp();
+    if (lane0) {
+      asm volatile("fence.proxy.async;" ::: "memory");   // the waiting CTAs read these stores with bulk copies (async proxy)
+      __threadfence();
+      atomicAdd(pending, 1u);
+    }
+    pending = nullptr;
+  };
   for (;;) {
+    if (FUSED && pending) {
+      // Deferring is only safe once the producer is past the dependencies of the next tile (they may include the very
+      // tile this warp has not published yet): that is the case when the tile's first plane has been staged.
+      uint32_t staged = 0;
+      if (lane0) staged = mbar_test(fullB + 8u * rm.slot, rm.par) ? 1u : 0u;
+      if (!__shfl_sync(0xffffffffu, staged, 0)) publish();
+    }
     mbar_wait(fullB + 8u * rm.slot, rm.par);   // first plane of the next tile, or the producer's "no more tiles"
-    const int32_t tile = tile_of[rm.slot];
-    if (tile < 0) break;
-    const int32_t ty = tile % w.n_ty, zc = tile / w.n_ty;
+    const int32_t tile = info[rm.slot].x;
+    if (tile < 0) { if (FUSED && pending) publish(); break; }
+    int32_t ty = tile % w.n_ty, zc = tile / w.n_ty;
+    if (FUSED) {
+      pass = info[rm.slot].y; zc = info[rm.slot].z; ty = info[rm.slot].w;
+      colour = pass & 1;
+      a = spins + (size_t)colour * L.half;
+      const unsigned long long sw = (((unsigned long long)P.sweep_hi << 32) | P.sweep_lo) + (unsigned long long)(pass >> 1);
+      sweep_lo = (uint32_t)sw; sweep_hi = (uint32_t)(sw >> 32);
+      if (MEAS) mode = pass == w.passes - 1 ? 2 : (pass == w.passes - 2 ? 1 : 0);   // the last sweep of the launch is the measured one
+    }
     const int32_t y0 = ty * TY, ny = min(TY, L.Ly - y0);
     const int32_t z0 = (int32_t)(((int64_t)zc * L.Lz) / w.n_zc), nz = (int32_t)(((int64_t)(zc + 1) * L.Lz) / w.n_zc) - z0;
     const bool active = r < ny;
     const int32_t y = y0 + r;
-    float* gx = a + ((size_t)z0 * L.Ly + y) * L.H + i0;            // own spins of plane z0 (x component)
+    float* gx = a + ((size_t)(ALIAS ? (int32_t)((uint32_t)z0 & w.zmask) : z0) * L.Ly + y) * L.H + i0;   // own spins of plane z0 (x component)
     uint32_t site_row = (uint32_t)(z0 * L.Ly + y) * (uint32_t)L.Lx + 2u * (uint32_t)i0 + L.site_base;
     // own spins come straight from global memory, one plane ahead of their use (only this thread writes them)
     constexpr bool PREF = ws_pref<TY, MINB>();   // otherwise (72 registers) the other warps cover the latency instead
@@ -156,7 +252,11 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
           nxt[0] = load_rw<4>(gx + plane); nxt[1] = load_rw<4>(gx + plane + n); nxt[2] = load_rw<4>(gx + plane + 2 * n);
         }
       } else if (act) {
-        sp[0] = load_rw<4>(gx); sp[1] = load_rw<4>(gx + n); sp[2] = load_rw<4>(gx + 2 * n);
+        if (FUSED) {   // an earlier pass of this launch, on any SM, wrote them: read at the L2, never a line kept in this SM's L1
+          sp[0] = load_cg<4>(gx); sp[1] = load_cg<4>(gx + n); sp[2] = load_cg<4>(gx + 2 * n);
+        } else {
+          sp[0] = load_rw<4>(gx); sp[1] = load_rw<4>(gx + n); sp[2] = load_rw<4>(gx + 2 * n);
+        }
       }
       RingPos<kNB> rc = rm; rc.next();
       RingPos<kNB> rq = rc; rq.next();
@@ -198,13 +298,13 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
           mbar_arrive(emptyB + 8u * rq.slot);
         }
       }
+      bool any_acc = false;
       if (act) {
         const uint32_t site0 = site_row + (uint32_t)p;
-        bool any = false;
 #pragma unroll
         for (int k = 0; k < 4; k += 2) {
-          const Rand4 ra = philox4x32_10(site0 + 2u * k, 0u, P.sweep_lo, P.sweep_hi, P.seed_lo, P.seed_hi);
-          const Rand4 rb = philox4x32_10(site0 + 2u * k + 2u, 0u, P.sweep_lo, P.sweep_hi, P.seed_lo, P.seed_hi);
+          const Rand4 ra = philox4x32_10(site0 + 2u * k, 0u, sweep_lo, sweep_hi, P.seed_lo, P.seed_hi);
+          const Rand4 rb = philox4x32_10(site0 + 2u * k + 2u, 0u, sweep_lo, sweep_hi, P.seed_lo, P.seed_hi);
           f2 px = make_float2(sp[0].v[k], sp[0].v[k + 1]), py = make_float2(sp[1].v[k], sp[1].v[k + 1]),
              pz = make_float2(sp[2].v[k], sp[2].v[k + 1]);
           bool acc_a, acc_b;
@@ -212,10 +312,13 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
                           make_float2(h[1].v[k], h[1].v[k + 1]), make_float2(h[2].v[k], h[2].v[k + 1]), px, py, pz, acc_a, acc_b);
           sp[0].v[k] = px.x; sp[0].v[k + 1] = px.y; sp[1].v[k] = py.x; sp[1].v[k + 1] = py.y;
           sp[2].v[k] = pz.x; sp[2].v[k + 1] = pz.y;
-          any |= acc_a | acc_b;
-          if (MEAS) n_acc += (unsigned)acc_a + (unsigned)acc_b;
+          any_acc |= acc_a | acc_b;
+          if (MEAS && (!FUSED || mode != 0)) n_acc += (unsigned)acc_a + (unsigned)acc_b;
         }
-        if (any) {
+      }
+      if (FUSED && pending) publish();   // (outside the divergent part: the whole warp)
+      if (act) {
+        if (any_acc) {
           store<4>(gx, sp[0]);
           store<4>(gx + n, sp[1]);
           store<4>(gx + 2 * n, sp[2]);
@@ -231,7 +334,7 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
             }
           }
         }
-        if (MEAS) {
+        if (MEAS && (!FUSED || mode != 0)) {
           float mx = 0.0f, my = 0.0f, mz = 0.0f, me = 0.0f;
           const float Jx = (mode == 2) ? -P.J : 0.0f;
 #pragma unroll
@@ -244,18 +347,24 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
           acc[0] += (double)mx; acc[1] += (double)my; acc[2] += (double)mz; acc[3] += (double)me;
         }
       }
-      gx += plane;
+      if (ALIAS) gx = a + ((size_t)((uint32_t)(z0 + s + 1) & w.zmask) * L.Ly + y) * L.H + i0; else gx += plane;
       site_row += (uint32_t)(L.Ly * L.Lx);
       rm.next();
     }
     rm.next(); rm.next();   // the two extra planes of the tile
+    if (FUSED && pass + 1 < w.passes) {
+      // this warp's stores of the tile are done: the next pass waits for the chunk's progress word (see publish above)
+      int32_t k = zc - pass % w.n_zc;   // position of the chunk in the pass's order (chunk = (k + pass) mod n)
+      k = k < 0 ? k + w.n_zc : k;
+      pending = w.done + (size_t)pass * w.n_zc + k;
+    }
   }
 }
 
 // SLAB: the lattice is a slab of a larger one (ScLayout::ghost): its first and last planes are ghost planes, staged as
 // neighbours but not updated, and boundary-plane stores are repeated into the z-neighbours' buffers (hb_slab_set_peer).
 // A separate instantiation: the whole-lattice kernel carries none of it.
-template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS, bool SLAB>
+template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS, bool SLAB, bool FUSED, bool ALIAS>
 __global__ void __launch_bounds__((ws_max_threads<TY, ROWB>()), MINB)
 k_sweep_sc_ws(float* a, const float* b, ScLayout L, WsTiles w, SweepParams P, int colour, Meas m) {
   resolve_sweep(P);
@@ -271,9 +380,20 @@ k_sweep_sc_ws(float* a, const float* b, ScLayout L, WsTiles w, SweepParams P, in
   __syncthreads();
   double acc[4] = {0.0, 0.0, 0.0, 0.0};
   unsigned n_acc = 0;
-  if (threadIdx.x < 32) ws_producer<TY, ROWB, kNB, MINB>(b, L, w, smem, sbase);
-  else ws_consumer<TY, ROWB, kNB, MINB, ANISO, MEAS, SLAB>(a, L, w, P, colour, m.mode, smem, sbase, acc, n_acc);
-  if (threadIdx.x == 0) {   // this thread took the CTA's last tile number above; the last CTA to finish re-arms the scheduler
+  if (threadIdx.x < 32) ws_producer<TY, ROWB, kNB, MINB, FUSED, ALIAS>(b, L, w, smem, sbase);
+  else ws_consumer<TY, ROWB, kNB, MINB, ANISO, MEAS, SLAB, FUSED, ALIAS>(a, L, w, P, colour, m.mode, smem, sbase, acc, n_acc);
+  if (FUSED) {
+    // the last CTA to finish re-arms the scheduler and clears the progress words; all of its warps must be through first
+    __shared__ uint32_t s_last;
+    __syncthreads();
+    if (threadIdx.x == 0) { __threadfence(); s_last = atomicAdd(w.sched + 1, 1u) == gridDim.x - 1 ? 1u : 0u; }
+    __syncthreads();
+    if (s_last) {
+      __threadfence();
+      for (int32_t i = threadIdx.x; i < w.passes * w.n_zc; i += blockDim.x) w.done[i] = 0u;
+      if (threadIdx.x == 0) { w.sched[0] = 0u; w.sched[1] = 0u; }
+    }
+  } else if (threadIdx.x == 0) {   // this thread took the CTA's last tile number above; the last CTA to finish re-arms the scheduler
     __threadfence();
     if (atomicAdd(w.sched + 1, 1u) == gridDim.x - 1) { w.sched[0] = 0u; w.sched[1] = 0u; }
   }
@@ -283,31 +403,61 @@ k_sweep_sc_ws(float* a, const float* b, ScLayout L, WsTiles w, SweepParams P, in
   }
 }
 
-template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS, bool SLAB = false>
-cudaError_t ws_go(cudaStream_t st, float* s, const ScLayout& L, int n_zc, int grid_cap, uint32_t* sched, const SweepParams& p, int colour, const Meas& m) {
+// the dynamic shared memory limit is an attribute of (function, device): set once per device
+inline cudaError_t ws_configure(const void* kern, int bytes, unsigned long long& configured_mask) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 64 && ((configured_mask >> dev) & 1ull)) return cudaSuccess;
+  e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess && dev < 64) configured_mask |= 1ull << dev;
+  return e;
+}
+
+struct FusedArgs { int passes, lag; uint32_t* done; uint32_t zmask = 0xffffffffu; };   // passes = 0: a plain launch of one colour
+
+template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS, bool SLAB = false, bool FUSED = false, bool ALIAS = false>
+cudaError_t ws_go(cudaStream_t st, float* s, const ScLayout& L, int n_zc, int grid_cap, uint32_t* sched, const SweepParams& p, int colour, const Meas& m,
+                  const FusedArgs& f = FusedArgs{0, 0, nullptr}) {
   using S = WsSmem<TY, ROWB, kNB, MINB>;
-  auto kern = k_sweep_sc_ws<TY, ROWB, kNB, MINB, ANISO, MEAS, SLAB>;
-  static bool configured = false;
-  if (!configured) {
-    const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::BYTES);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  auto kern = k_sweep_sc_ws<TY, ROWB, kNB, MINB, ANISO, MEAS, SLAB, FUSED, ALIAS>;
+  static unsigned long long configured = 0;
+  const cudaError_t e = ws_configure((const void*)kern, (int)S::BYTES, configured);
+  if (e != cudaSuccess) return e;
   WsTiles w;
   w.n_ty = (L.Ly + TY - 1) / TY;
   w.n_zc = n_zc;
   w.sched = sched;
-  const int n_tiles = w.n_ty * w.n_zc;
-  const int grid = n_tiles < grid_cap ? n_tiles : grid_cap;
+  w.passes = f.passes; w.lag = f.lag; w.done = f.done; w.zmask = f.zmask;
+  const long long n_tiles = (long long)w.n_ty * w.n_zc * (FUSED ? f.passes : 1);
+  const int grid = n_tiles < grid_cap ? (int)n_tiles : grid_cap;
   const int threads = 32 + 32 * ((TY * (L.H / 4) + 31) / 32);
+  if (FUSED)   // the kernel picks the colour planes per tile from the base of the spins
+    return launch_colour_kernel(kern, dim3(grid), dim3(threads), S::BYTES, st, p.pdl != 0, s, s, L, w, p, 0, m);
   float* a = s + (size_t)colour * L.half;
   const float* b = s + (size_t)(1 - colour) * L.half;
   return launch_colour_kernel(kern, dim3(grid), dim3(threads), S::BYTES, st, p.pdl != 0, a, b, L, w, p, colour, m);
 }
 
 template <int TY, int ROWB, int kNB, int MINB>
-cudaError_t ws_pick(cudaStream_t st, float* s, const ScLayout& L, int n_zc, int grid_cap, uint32_t* sched, const SweepParams& p, int colour, const Meas& m) {
+cudaError_t ws_pick(cudaStream_t st, float* s, const ScLayout& L, int n_zc, int grid_cap, uint32_t* sched, const SweepParams& p, int colour, const Meas& m,
+                    const FusedArgs& f = FusedArgs{0, 0, nullptr}) {
   const int aniso = (p.K == 0.0f) ? ANISO_NONE : ((p.ex == 0.0f && p.ey == 0.0f && p.ez == 1.0f) ? ANISO_Z : ANISO_GENERAL);
+  if (f.passes > 0) {   // several colour passes in one launch (whole lattices only)
+    if (L.ghost) return cudaErrorInvalidValue;
+    if (m.mode != 0) {
+      switch (aniso) {
+        case ANISO_NONE: return ws_go<TY, ROWB, kNB, MINB, ANISO_NONE, true, false, true>(st, s, L, n_zc, grid_cap, sched, p, colour, m, f);
+        case ANISO_Z: return ws_go<TY, ROWB, kNB, MINB, ANISO_Z, true, false, true>(st, s, L, n_zc, grid_cap, sched, p, colour, m, f);
+        default: return ws_go<TY, ROWB, kNB, MINB, ANISO_GENERAL, true, false, true>(st, s, L, n_zc, grid_cap, sched, p, colour, m, f);
+      }
+    }
+    switch (aniso) {
+      case ANISO_NONE: return ws_go<TY, ROWB, kNB, MINB, ANISO_NONE, false, false, true>(st, s, L, n_zc, grid_cap, sched, p, colour, m, f);
+      case ANISO_Z: return ws_go<TY, ROWB, kNB, MINB, ANISO_Z, false, false, true>(st, s, L, n_zc, grid_cap, sched, p, colour, m, f);
+      default: return ws_go<TY, ROWB, kNB, MINB, ANISO_GENERAL, false, false, true>(st, s, L, n_zc, grid_cap, sched, p, colour, m, f);
+    }
+  }
   if (L.ghost) {   // slab contexts measure with the separate pass
     if (m.mode != 0) return cudaErrorInvalidValue;
     switch (aniso) {
@@ -391,6 +541,47 @@ cudaError_t launch_sweep_sc_ws(cudaStream_t st, float* s, ScLayout L, int ZT, in
   if (variant == 1) return ws_pick<8, 1024, 6, 1>(st, s, L, n_zc, cap, sched, p, colour, m);
   if (variant == 2) return ws_pick<4, 1024, 4, 3>(st, s, L, n_zc, cap, sched, p, colour, m);
   return ws_pick<4, 1024, 5, 2>(st, s, L, n_zc, cap, sched, p, colour, m);
+}
+
+// ---- diagnostic: one colour pass of the 7-row kernel with every plane folded onto the first `planes` (a power of two) ----------
+cudaError_t launch_sweep_sc_ws_alias(cudaStream_t st, float* s, ScLayout L, int grid_cap, uint32_t* sched, SweepParams p, int colour, int planes) {
+  if (!sc_ws_variant_supported(L, 4) || L.ghost || planes < 2 || (planes & (planes - 1)) || planes > L.Lz) return cudaErrorInvalidValue;
+  const int cap = grid_cap * ws_ctas_per_sm(4);
+  const int n_zc = sc_ws_chunks(L, 0, grid_cap, 4);
+  FusedArgs f{0, 0, nullptr};
+  f.zmask = (uint32_t)planes - 1u;
+  const int aniso = (p.K == 0.0f) ? ANISO_NONE : ((p.ex == 0.0f && p.ey == 0.0f && p.ez == 1.0f) ? ANISO_Z : ANISO_GENERAL);
+  const Meas m{nullptr, 0, nullptr};
+  switch (aniso) {
+    case ANISO_NONE: return ws_go<7, 1024, 4, 2, ANISO_NONE, false, false, false, true>(st, s, L, n_zc, cap, sched, p, colour, m, f);
+    case ANISO_Z: return ws_go<7, 1024, 4, 2, ANISO_Z, false, false, false, true>(st, s, L, n_zc, cap, sched, p, colour, m, f);
+    default: return ws_go<7, 1024, 4, 2, ANISO_GENERAL, false, false, false, true>(st, s, L, n_zc, cap, sched, p, colour, m, f);
+  }
+}
+
+// ---- fused launches: n_sweeps whole sweeps (2 n_sweeps colour passes) in ONE launch (variants 2, 4, 5) --------------------
+bool sc_ws_fused_supported(const ScLayout& L, int variant) {
+  return !L.ghost && (variant == 2 || variant == 4 || variant == 5) && sc_ws_variant_supported(L, variant);
+}
+// chunks in z of a fused launch: ZT planes each (ZT = 0: 24)
+int sc_ws_fused_chunks(const ScLayout& L, int ZT) {
+  const int zt = ZT > 0 ? ZT : 24;
+  return (L.Lz + zt - 1) / zt;
+}
+int sc_ws_fused_blocks(const ScLayout& L, int ZT, int grid_cap, int variant, int n_sweeps) {
+  const long long n_tiles = (long long)((L.Ly + ws_ty(variant) - 1) / ws_ty(variant)) * sc_ws_fused_chunks(L, ZT) * 2 * n_sweeps;
+  const long long cap = (long long)grid_cap * ws_ctas_per_sm(variant);
+  return (int)(n_tiles < cap ? n_tiles : cap);
+}
+cudaError_t launch_sweep_sc_ws_fused(cudaStream_t st, float* s, ScLayout L, int ZT, int lag, int grid_cap, int variant, uint32_t* sched,
+                                     uint32_t* done, SweepParams p, int n_sweeps, Meas m) {
+  const int n_zc = sc_ws_fused_chunks(L, ZT);
+  if (!sc_ws_fused_supported(L, variant) || n_sweeps < 1 || lag < 3 || 2 * n_sweeps * n_zc > kWsDoneWords) return cudaErrorInvalidValue;
+  const int cap = grid_cap * ws_ctas_per_sm(variant);
+  const FusedArgs f{2 * n_sweeps, lag, done};
+  if (variant == 5) return ws_pick<8, 512, 4, 3>(st, s, L, n_zc, cap, sched, p, 0, m, f);
+  if (variant == 4) return ws_pick<7, 1024, 4, 2>(st, s, L, n_zc, cap, sched, p, 0, m, f);
+  return ws_pick<4, 1024, 4, 3>(st, s, L, n_zc, cap, sched, p, 0, m, f);
 }
 
 }  // namespace hb

@@ -82,7 +82,7 @@ def test_packed_multiplies_are_not_contracted_into_fused_multiply_adds():
         assert len(hit) == 1, (substr, hit)
         text = "\n".join(funcs[hit[0]])
         return len(re.findall(r"\bFMUL2\b", text)), len(re.findall(r"\bFFMA2\b", text))
-    for kernel in ("k_probe_alu", "k_sweep_sc_wsILi7ELi1024ELi4ELi2ELi1ELb0ELb0E", "k_sweep_scILi4ELi1ELb0ELi1ELi256ELb0ELb0E"):
+    for kernel in ("k_probe_alu", "k_sweep_sc_wsILi7ELi1024ELi4ELi2ELi1ELb0ELb0ELb0ELb0EE", "k_sweep_sc_wsILi7ELi1024ELi4ELi2ELi1ELb0ELb0ELb1ELb0EE", "k_sweep_scILi4ELi1ELb0ELi1ELi256ELb0ELb0E"):
         assert mix(kernel) == (26, 50), (kernel, mix(kernel))
 
 

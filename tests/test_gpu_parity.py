@@ -699,3 +699,80 @@ def test_stats_on_the_warp_specialised_kernel_and_on_replicas():
         want_acc += b
     assert ctx.stats() == (want_att, want_acc)
     ctx.close()
+
+
+def test_fused_launches_match_the_oracle():
+    # sc_kernel = 2 (DESIGN 6.9): all colour passes of several sweeps in ONE launch, tiles ordered in rounds with
+    # dependencies between the passes instead of a launch boundary per colour.  Same trajectory, bit for bit, for every
+    # chunk size / lag / sweeps per launch, ragged tiles in y and z, fewer chunks than the dependency window, general anisotropy,
+    # the fused measurement, the series, hb_stats and a sweep counter that crosses 2^32 inside a launch.
+    cases = [(dict(W.SMALL["c4"], L=(64, 30, 22)), [dict(sc_ws_variant=2), dict(sc_ws_variant=4, sc_fused_zt=3, sc_fused_lag=3, sc_fused_sweeps=3),
+                                                     dict(sc_ws_variant=5, sc_fused_zt=1, sc_fused_lag=5, sc_fused_sweeps=16),
+                                                     dict(sc_ws_variant=4, sc_fused_zt=22, sc_fused_sweeps=2),          # one chunk
+                                                     dict(sc_ws_variant=2, sc_fused_zt=11, sc_fused_lag=7, sc_fused_sweeps=5)]),   # two chunks
+             (dict(W.SMALL["c4"], L=(464, 16, 12), K=0.3, e=(0.6, 0.0, 0.8)), [dict(sc_ws_variant=4, sc_fused_zt=2, sc_fused_sweeps=4),
+                                                                             dict(sc_ws_variant=2, sc_fused_zt=5, sc_fused_lag=3)]),
+             (dict(W.SMALL["c4"], L=(240, 44, 40), K=0.0), [dict(sc_ws_variant=5, sc_fused_zt=4, sc_fused_sweeps=6, sc_ws_ctas=3),   # few CTAs: deep queues
+                                                            dict(sc_ws_variant=4, sc_fused_zt=8, sc_fused_sweeps=2)])]
+    for cfg, variants in cases:
+        lat, st0 = make_oracle(cfg)
+        for opts in variants:
+            lat, st = make_oracle(cfg)
+            ctx = make_gpu(cfg)
+            ctx.set_option("sc_coop", 0)
+            ctx.set_option("graph", 0)
+            for k, v in opts.items():
+                if k == "sc_ws_variant":
+                    ctx.set_option(k, v)
+            ctx.set_option("sc_kernel", 2)
+            for k, v in opts.items():
+                ctx.set_option(k, v)
+            assert ctx.get_option("sc_kernel") == 2
+            start(cfg, ctx, st)
+            ctx.sweep_count = st.sweep_count = (1 << 32) - 3
+            for T, k in ((1.44, 1), (1.44, 2), (1.44, 11), (0.4, 7)):
+                l0, a0 = ctx.counters()
+                ctx.sweep(T, k)
+                l1, a1 = ctx.counters()
+                assert a1 - a0 == k * lat.n
+                S = opts.get("sc_fused_sweeps", 8)
+                assert l1 - l0 == -(-(k - 1) // S) + 2                  # ceil((k-1)/S) launches + the measured sweep + its reduction
+                st.sweep(T, k)
+                assert spins_equal(ctx.get_spins(), st.get_spins()), (cfg["L"], opts, T, k)
+                _measure_close(ctx, st, lat.n)
+            Mg, Eg = ctx.sweep_series(1.2, 5)
+            Mo, Eo = st.series(1.2, 5)
+            assert np.max(np.abs(Mg - Mo)) <= 1e-7 and np.max(np.abs(Eg - Eo)) <= 1e-6 * lat.n
+            assert ctx.sweep_count == st.sweep_count
+            ctx.close()
+        # hb_stats through the fused measuring launch
+        lat, st = make_oracle(cfg)
+        ctx = make_gpu(cfg)
+        ctx.set_option("sc_coop", 0)
+        ctx.set_option("graph", 0)
+        ctx.set_option("sc_ws_variant", 2)
+        ctx.set_option("sc_kernel", 2)
+        start(cfg, ctx, st)
+        for _ in range(3):
+            ctx.sweep(1.0, 1)
+            st.sweep(1.0, 1)
+        assert ctx.stats() == st.stats()
+        ctx.close()
+    with pytest.raises(hb.HbError):
+        hb.Context(hb.Lattice("sc", 6)).set_option("sc_kernel", 2)
+
+
+def test_l2_fold_probe_reports_a_rate_and_invalidates_the_state():
+    # hb_probe_sc_l2: the sc colour kernel with plane addresses folded onto 16 L2-resident planes (DESIGN 6.9): a rate, not a
+    # trajectory; the spins are undefined afterwards
+    ctx = hb.Context(hb.Lattice("sc", 232, 64, 64), 1.0, 0.01, (0, 0, 1), seed=1)
+    ctx.init_random()
+    rate = ctx.probe_sc_l2(1.44, 10, 16)
+    assert 1e9 < rate < 400e9
+    with pytest.raises(hb.HbError):
+        ctx.sweep(1.44, 1)                      # HB_ESTATE until the spins are initialised again
+    ctx.init_random()
+    ctx.sweep(1.44, 1)
+    with pytest.raises(hb.HbError):
+        ctx.probe_sc_l2(1.44, 10, 12)           # planes must be a power of two
+    ctx.close()
