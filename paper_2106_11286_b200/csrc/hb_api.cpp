@@ -105,7 +105,7 @@ int make_plan(const hb_lattice* lat, Plan& p, std::string& why) {
   p.off_series = o;   o += align_up((size_t)p.R * kSeriesChunk * 4 * sizeof(double));
   p.off_counters = o; o += kAlign;
   p.off_staging = o;  o += align_up((size_t)p.n * sizeof(float));
-  if (p.engine == ENGINE_SC) { p.off_wsdone = o; o += align_up((size_t)kWsDoneWords * sizeof(uint32_t)); }   // progress words of fused launches
+  if (p.engine == ENGINE_SC || p.engine == ENGINE_BRAVAIS) { p.off_wsdone = o; o += align_up((size_t)kWsDoneWords * sizeof(uint32_t)); }   // progress words of fused launches
   if (p.R > 1) {
     p.off_each = o;  o += align_up((size_t)p.R * 20 * sizeof(double));
     p.off_betas = o; o += align_up((size_t)p.R * sizeof(float));
@@ -146,6 +146,8 @@ struct hb_ctx {
   int sc_kernel = 0;      // 0: direct loads through L1, 1: warp-specialised persistent kernel (TMA-staged neighbour planes),
                           // 2: the same kernel with all colour passes of up to fused_sweeps sweeps in ONE launch
   int fused_sweeps = 8, fused_lag = 6, fused_zt = 24;   // the fastest setting measured on c4
+  int br_kernel = 0, br_zt = 0;   // bcc / fcc: 0 direct loads through L1, 1 warp-specialised persistent kernel (one launch per colour),
+                                  // 2 the same with all colour passes of up to fused_sweeps sweeps in one launch
   int ws_zt = 0, n_sms = 148, ws_variant = 2;   // warp-specialised kernel: planes per tile (0: balanced automatically), CTAs = n_sms x CTAs/SM
   int graph_mode = -1;         // replay hb_sweep's launches from a CUDA graph: -1 auto (lattices up to 2^23 sites), 0 off, 1 on
   cudaStream_t cap_stream = nullptr;
@@ -262,7 +264,10 @@ int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d, Meas m = Mea
     else
       HB_CUDA(c, launch_sweep_sc(c->stream, c->spins, c->sc, c->tile, p, colour, d, m));
   } else if (c->plan.engine == ENGINE_BRAVAIS) {
-    HB_CUDA(c, launch_sweep_bravais(c->stream, c->spins, c->br, c->tile, p, colour, d, m));
+    if (c->br_kernel >= 1 && !(d.accept || d.n_accept))
+      HB_CUDA(c, launch_sweep_bravais_ws(c->stream, c->spins, c->br, c->br_zt, c->fused_lag, c->n_sms, c->ws_sched(), c->ws_done(), p, colour, 1, m));
+    else
+      HB_CUDA(c, launch_sweep_bravais(c->stream, c->spins, c->br, c->tile, p, colour, d, m));
   } else {
     const uint32_t b = c->colour_begin[colour], e = c->colour_begin[colour + 1];
     if (e == b) return HB_OK;
@@ -276,6 +281,7 @@ int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d, Meas m = Mea
 // blocks per colour launch if this context can fuse the measurement into its colour passes, else 0
 int fused_blocks(const hb_ctx* c) {
   if (!c->fused_measure) return 0;
+  if (c->plan.engine == ENGINE_BRAVAIS && c->br_kernel >= 1) return bravais_ws_blocks(c->br, c->br_zt, c->n_sms, c->br_kernel == 2 ? c->n_colours : 1);
   if (c->plan.engine == ENGINE_BRAVAIS) return bravais_fused_blocks(c->br, c->tile);
   if (c->plan.engine != ENGINE_SC) return 0;
   if (c->sc_kernel == 2) return sc_ws_fused_blocks(c->sc, c->fused_zt, c->n_sms, c->ws_variant, 1);
@@ -315,6 +321,10 @@ int fused_sweeps_launch(hb_ctx* c, float beta, int n_sweeps, double* dev_out, bo
   Meas m{nullptr, 0, nullptr};
   const int fb = dev_out ? fused_blocks(c) : 0;
   if (fb) m = Meas{c->partials(), 2, counted ? c->counters() : nullptr};
+  if (c->plan.engine == ENGINE_BRAVAIS)
+    HB_CUDA(c, launch_sweep_bravais_ws(c->stream, c->spins, c->br, c->br_zt, c->fused_lag, c->n_sms, c->ws_sched(), c->ws_done(), p, 0,
+                                       c->n_colours * n_sweeps, m));
+  else
   HB_CUDA(c, launch_sweep_sc_ws_fused(c->stream, c->spins, c->sc, c->fused_zt, c->fused_lag, c->n_sms, c->ws_variant, c->ws_sched(), c->ws_done(),
                                       p, n_sweeps, m));
   c->launches += 1;
@@ -328,7 +338,9 @@ int fused_sweeps_launch(hb_ctx* c, float beta, int n_sweeps, double* dev_out, bo
   return HB_OK;
 }
 
-bool fused_kernel(const hb_ctx* c) { return c->plan.engine == ENGINE_SC && c->sc_kernel == 2; }
+bool fused_kernel(const hb_ctx* c) {
+  return (c->plan.engine == ENGINE_SC && c->sc_kernel == 2) || (c->plan.engine == ENGINE_BRAVAIS && c->br_kernel == 2);
+}
 
 // one sweep; with dev_out != nullptr (and fused_blocks() > 0) the colour passes also reduce M and E of
 // the state they leave behind, and dev_out receives (sum Sx, sum Sy, sum Sz, E).  counted: the accepted moves of the
@@ -363,7 +375,7 @@ int one_sweep(hb_ctx* c, float beta, Diag d, double* dev_out = nullptr, bool cou
 constexpr int kGraphSweeps = 8;
 
 bool graph_wanted(const hb_ctx* c) {
-  if (c->graph_mode == 0 || coop_mode(c) != 0) return false;
+  if (c->graph_mode == 0 || coop_mode(c) != 0 || fused_kernel(c)) return false;   // fused launches carry whole sweeps already
   return c->graph_mode == 1 || c->plan.n <= (int64_t(1) << 23);
 }
 
@@ -574,6 +586,21 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
     c->br.kind = lat->kind; c->br.Lx = lat->Lx; c->br.Ly = lat->Ly; c->br.Lz = lat->Lz;
     c->br.n = (uint32_t)P.n; c->br.nc = (uint32_t)(P.n / c->n_colours);
     c->tile = default_tile(lat->Lx, lat->Ly, lat->Lz);
+    // The warp-specialised kernel pays on lattices far larger than L2: bcc +2 ... +10 % over the direct kernel
+    // (33.5 M sites, rows of 64 / 128 / 256 cells: 112 / 117 / 125 against 109 / 108 / 114 Gupd/s); fcc only with all passes in one
+    // launch and long rows (89.9 against 85.1), its staged groups being three sublattices wide.  c2 and c3 (0.5 M and 8.4 M
+    // sites, L2-resident, a handful of plane steps per CTA and pass) stay on the direct kernel: 27 against 70, 59 against 80.
+    if (bravais_ws_supported(c->br) && P.n >= (int64_t(1) << 24)) {
+      if (lat->kind == HB_BCC) { c->br_kernel = 1; c->br_zt = (lat->Lx > 64 && lat->Lx <= 128) ? 8 : 16; }
+      else if (lat->Lx > 128) { c->br_kernel = 2; c->br_zt = 16; }
+      if (c->br_zt > lat->Lz) c->br_zt = lat->Lz;
+    }
+    {
+      int dev = 0, sms = 0;
+      if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+        c->n_sms = sms;
+      cudaGetLastError();
+    }
   } else {
     c->n_colours = 2;
     c->sc.Lx = lat->Lx; c->sc.Ly = lat->Ly; c->sc.Lz = lat->Lz;
@@ -625,7 +652,7 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
     c->own_spins = c->own_ws = true;
   }
   HB_CUDA(c, cudaMemsetAsync(c->ws + P.off_counters, 0, kAlign, c->stream));
-  if (P.engine == ENGINE_SC) HB_CUDA(c, cudaMemsetAsync(c->ws + P.off_wsdone, 0, (size_t)kWsDoneWords * sizeof(uint32_t), c->stream));
+  if (P.engine == ENGINE_SC || P.engine == ENGINE_BRAVAIS) HB_CUDA(c, cudaMemsetAsync(c->ws + P.off_wsdone, 0, (size_t)kWsDoneWords * sizeof(uint32_t), c->stream));
 
   if (P.engine == ENGINE_CSR) {
     // sites sorted by (colour, id): one contiguous list segment per colour
@@ -1201,6 +1228,19 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
     c->g_dirty[0] = c->g_dirty[1] = true;   // captured launches carry the attribute
     return HB_OK;
   }
+  if (s == "br_kernel" || s == "br_zt") {
+    if (c->plan.engine != ENGINE_BRAVAIS) return fail(c, HB_EINVAL, "option valid for bcc / fcc lattices only");
+    if (s == "br_kernel") {
+      if (value < 0 || value > 2 || (value >= 1 && !bravais_ws_supported(c->br)))
+        return fail(c, HB_EINVAL, "br_kernel: 0 (direct), 1 (warp-specialised; needs Lx % 4 == 0 and Lx <= 256), 2 (the same, all colour passes of several sweeps in one launch)");
+      c->br_kernel = (int)value;
+    } else {
+      if (value < 0 || value > c->br.Lz) return fail(c, HB_EINVAL, "br_zt: 1..Lz planes per chunk, 0 = automatic");
+      c->br_zt = (int)value;
+    }
+    if ((long long)(c->n_colours * c->fused_sweeps - 1) * bravais_ws_chunks(c->br, c->br_zt, c->n_sms) > kWsDoneWords) c->fused_sweeps = 1;
+    return HB_OK;
+  }
   if (s == "csr_block") {
     if (value < 32 || value > 256 || value % 32) return fail(c, HB_EINVAL, "csr_block: multiple of 32 in [32,256]");
     c->csr_block = (int)value;
@@ -1208,8 +1248,14 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
   }
   if (c->plan.engine == ENGINE_CSR) return fail(c, HB_EINVAL, "option not valid for this lattice");
   const bool is_sc = c->plan.engine == ENGINE_SC;
-  if (!is_sc && (s == "sc_kernel" || s == "sc_prefetch" || s == "sc_linear" || s == "sc_ws_zt" || s == "sc_ws_ctas" || s == "sc_ws_variant" ||
-                 s == "sc_fused_sweeps" || s == "sc_fused_lag" || s == "sc_fused_zt"))
+  if (!is_sc && (s == "sc_fused_sweeps" || s == "sc_fused_lag" || s == "sc_ws_ctas")) {   // shared with the bcc / fcc warp-specialised kernel
+    if (s == "sc_fused_sweeps") { if (value < 1 || value > 16) return fail(c, HB_EINVAL, "sc_fused_sweeps: 1..16 sweeps per launch"); c->fused_sweeps = (int)value; }
+    else if (s == "sc_fused_lag") { if (value < 3 || value > 64) return fail(c, HB_EINVAL, "sc_fused_lag: 3..64 rounds between two colour passes"); c->fused_lag = (int)value; }
+    else { if (value < 1 || value > 4096) return fail(c, HB_EINVAL, "sc_ws_ctas: 1..4096"); c->n_sms = (int)value; }
+    if ((long long)(c->n_colours * c->fused_sweeps - 1) * bravais_ws_chunks(c->br, c->br_zt, c->n_sms) > kWsDoneWords) c->fused_sweeps = 1;
+    return HB_OK;
+  }
+  if (!is_sc && (s == "sc_kernel" || s == "sc_prefetch" || s == "sc_linear" || s == "sc_ws_zt" || s == "sc_ws_variant" || s == "sc_fused_zt"))
     return fail(c, HB_EINVAL, "option valid for the simple cubic lattice only");
   const int32_t rowH = is_sc ? c->sc.H : c->br.Lx, rowLz = is_sc ? c->sc.Lz : c->br.Lz;
   if (s == "sc_kernel") {
@@ -1297,6 +1343,8 @@ int hb_get_option(hb_ctx* c, const char* name, int64_t* value) {
   else if (s == "sc_fused_sweeps") *value = c->fused_sweeps;
   else if (s == "sc_fused_lag") *value = c->fused_lag;
   else if (s == "sc_fused_zt") *value = c->fused_zt;
+  else if (s == "br_kernel") *value = c->br_kernel;
+  else if (s == "br_zt") *value = c->br_zt;
   else return HB_EINVAL;
   return HB_OK;
 }

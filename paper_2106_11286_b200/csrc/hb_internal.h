@@ -154,6 +154,13 @@ cudaError_t launch_init_random_perm(cudaStream_t st, float* spins, const int32_t
 cudaError_t launch_fill_ell(cudaStream_t st, float* spins, uint32_t n, float x, float y, float z);
 // component comp of the internal float4 state <- plane[perm[m]] (to_internal) or plane[perm[m]] <- component
 cudaError_t launch_permute_ell(cudaStream_t st, float* spins, float* plane, const int32_t* perm, uint32_t n, int comp, bool to_internal);
+// warp-specialised persistent bcc / fcc kernel (hb_bravais_ws.cu): `passes` colour passes in one launch, starting with colour
+// `first` of the sweep in p (one pass = a plain colour launch); rows of up to 256 cells, Lx a multiple of 4
+bool bravais_ws_supported(const BrLayout& L);
+int bravais_ws_chunks(const BrLayout& L, int ZT, int grid_cap);
+int bravais_ws_blocks(const BrLayout& L, int ZT, int grid_cap, int passes);
+cudaError_t launch_sweep_bravais_ws(cudaStream_t st, float* spins, BrLayout L, int ZT, int lag, int grid_cap, uint32_t* sched, uint32_t* done,
+                                    SweepParams p, int first, int passes, Meas m);
 int bravais_fused_blocks(const BrLayout& L, const ScTile& t);
 cudaError_t launch_sweep_bravais(cudaStream_t st, float* spins, BrLayout L, ScTile t, SweepParams p, int colour, Diag d, Meas m);
 // measurement: partials must hold kMeasureBlocks*4 doubles; out receives (Mx*N, My*N, Mz*N, E)

@@ -30,18 +30,12 @@
 // before it: the oldest unfinished tile can always run, whatever the CTAs hold.
 #include "hb_device.cuh"
 #include "hb_internal.h"
+#include "hb_ws.cuh"
 
 namespace hb {
 
 namespace {
 
-
-// position on a ring of N slots: slot index and the parity of the pass over the ring
-template <int N>
-struct RingPos {
-  uint32_t slot = 0, par = 0;
-  __device__ __forceinline__ void next() { if (++slot == N) { slot = 0; par ^= 1u; } }
-};
 
 // threads of a CTA the kernel is compiled for: the producer warp plus TY rows of ROWB/16 vectors; the 7-row shape is built
 // for rows of at most 59 vectors (13 consumer warps: 448 threads, two CTAs per SM at 72 registers)
@@ -54,46 +48,6 @@ __host__ __device__ constexpr int ws_max_threads() {
 // own spins one plane ahead in registers: only where the register budget allows (4-row tiles, 2 CTAs per SM)
 template <int TY, int MINB>
 __host__ __device__ constexpr bool ws_pref() { return MINB < 3 && TY != 7; }
-
-struct WsTiles {
-  int32_t n_ty, n_zc;   // tiles in y, chunks in z: chunk zc = planes [zc Lz / n_zc, (zc+1) Lz / n_zc), sizes differ by at most one
-  uint32_t* sched;      // device, two words, zero between launches: next tile to hand out, CTAs that have finished
-  // fused launches only: colour passes of the launch (pass p: sweep p / 2, colour p % 2), rounds between two passes (>= 3),
-  // and passes x n_zc progress words, zero between launches: consumer warps that have finished a tile of (pass, k-th chunk)
-  int32_t passes, lag;
-  uint32_t* done;
-  // diagnostic launches only (ALIAS, hb_probe_sc_l2): plane z is read and written at the address of plane z & zmask, so the
-  // whole launch lives in a few L2-resident planes -- the kernel's rate with its HBM traffic taken away
-  uint32_t zmask;
-};
-
-// a tile of a fused launch: pass, position k of its chunk in the pass's order, the chunk itself, the tile in y
-struct FusedTile { int32_t p, k, zc, ty; };
-
-// Round r holds the k-th chunk of pass p for r = lag p + k; within a round passes ascend.  S(r) = (pass, chunk) pairs in
-// rounds before r = sum_p clamp(r - lag p, 0, n).
-__device__ __forceinline__ FusedTile fused_decode(int32_t tile, const WsTiles& w) {
-  const int32_t q = tile / w.n_ty, n = w.n_zc, P = w.passes, lag = w.lag;
-  // passes 0 .. sat-1 have all n chunks behind them at round r, passes sat .. j-1 have r - lag p of them, the rest none
-  auto before = [&](int32_t r) {
-    const int32_t j = min(P, (r + lag - 1) / lag), sat = r >= n ? min(P, (r - n) / lag + 1) : 0;
-    return sat * n + (j - sat) * r - lag * (((sat + j - 1) * (j - sat)) / 2);
-  };
-  int32_t lo = 0, hi = n + lag * (P - 1);   // before(lo) <= q < before(hi)
-  while (hi - lo > 1) { const int32_t mid = (lo + hi) >> 1; if (before(mid) <= q) lo = mid; else hi = mid; }
-  FusedTile t;
-  t.p = (lo < n ? 0 : (lo - n) / lag + 1) + (q - before(lo));
-  t.k = lo - lag * t.p;
-  t.zc = (t.k + t.p) % n;
-  t.ty = tile - q * w.n_ty;
-  return t;
-}
-
-__device__ __forceinline__ uint32_t ld_acquire_gpu(const uint32_t* p) {
-  uint32_t v;
-  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
 
 // kNB plane slots of the other colour (z-1, z, z+1 and look-ahead); MINB = CTAs per SM the kernel is built for
 template <int TY, int ROWB, int kNB, int MINB>
@@ -403,17 +357,6 @@ k_sweep_sc_ws(float* a, const float* b, ScLayout L, WsTiles w, SweepParams P, in
   }
 }
 
-// the dynamic shared memory limit is an attribute of (function, device): set once per device
-inline cudaError_t ws_configure(const void* kern, int bytes, unsigned long long& configured_mask) {
-  int dev = 0;
-  cudaError_t e = cudaGetDevice(&dev);
-  if (e != cudaSuccess) return e;
-  if (dev < 64 && ((configured_mask >> dev) & 1ull)) return cudaSuccess;
-  e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-  if (e == cudaSuccess && dev < 64) configured_mask |= 1ull << dev;
-  return e;
-}
-
 struct FusedArgs { int passes, lag; uint32_t* done; uint32_t zmask = 0xffffffffu; };   // passes = 0: a plain launch of one colour
 
 template <int TY, int ROWB, int kNB, int MINB, int ANISO, bool MEAS, bool SLAB = false, bool FUSED = false, bool ALIAS = false>
@@ -428,7 +371,7 @@ cudaError_t ws_go(cudaStream_t st, float* s, const ScLayout& L, int n_zc, int gr
   w.n_ty = (L.Ly + TY - 1) / TY;
   w.n_zc = n_zc;
   w.sched = sched;
-  w.passes = f.passes; w.lag = f.lag; w.done = f.done; w.zmask = f.zmask;
+  w.passes = f.passes; w.lag = f.lag; w.done = f.done; w.zmask = f.zmask; w.first = 0;
   const long long n_tiles = (long long)w.n_ty * w.n_zc * (FUSED ? f.passes : 1);
   const int grid = n_tiles < grid_cap ? (int)n_tiles : grid_cap;
   const int threads = 32 + 32 * ((TY * (L.H / 4) + 31) / 32);

@@ -776,3 +776,59 @@ def test_l2_fold_probe_reports_a_rate_and_invalidates_the_state():
     with pytest.raises(hb.HbError):
         ctx.probe_sc_l2(1.44, 10, 12)           # planes must be a power of two
     ctx.close()
+
+
+def test_bravais_warp_specialised_kernel_matches_the_oracle():
+    # br_kernel = 1 / 2 (DESIGN 6.10): bcc and fcc colour passes with TMA-staged neighbour groups; 2 = all colour passes of
+    # several sweeps in one launch.  Every launch shape (rows of up to 64 / 128 / 256 cells), ragged tiles in y and z, every
+    # anisotropy case, the fused measurement, series, stats, a sweep counter crossing 2^32.
+    cases = [dict(W.SMALL["c2"]), dict(W.SMALL["c2"], L=(12, 5, 7), K=0.0), dict(W.SMALL["c2"], L=(68, 11, 6), K=0.3, e=(0.6, 0.0, 0.8)),
+             dict(W.SMALL["c2"], L=(132, 6, 5)), dict(W.SMALL["c3"], L=(8, 6, 6), start="random"),
+             dict(W.SMALL["c3"], L=(4, 3, 5), start="random", K=0.0), dict(W.SMALL["c3"], L=(72, 9, 4), start="random", K=0.2, e=(0.0, 0.0, 1.0)),
+             dict(W.SMALL["c3"], L=(132, 5, 3), start="random"), dict(W.SMALL["c3"], L=(64, 16, 24), start="aligned")]
+    for cfg in cases:
+        for opts in (dict(br_kernel=1), dict(br_kernel=2), dict(br_kernel=2, br_zt=1, sc_fused_lag=3, sc_fused_sweeps=3),
+                     dict(br_kernel=2, br_zt=2, sc_fused_lag=5, sc_fused_sweeps=16, sc_ws_ctas=2), dict(br_kernel=1, br_zt=3, graph=0)):
+            lat, st = make_oracle(cfg)
+            ctx = make_gpu(cfg)
+            for k, v in opts.items():
+                ctx.set_option(k, v)
+            start(cfg, ctx, st)
+            ctx.sweep_count = st.sweep_count = (1 << 32) - 4
+            for T, k in ((cfg["T"][0], 1), (cfg["T"][0], 2), (1.5, 13), (0.4, 6)):
+                ctx.sweep(T, k)
+                st.sweep(T, k)
+                assert spins_equal(ctx.get_spins(), st.get_spins()), (cfg["kind"], cfg["L"], opts, T, k)
+                _measure_close(ctx, st, lat.n)
+            Mg, Eg = ctx.sweep_series(1.2, 5)
+            Mo, Eo = st.series(1.2, 5)
+            assert np.max(np.abs(Mg - Mo)) <= 1e-7 and np.max(np.abs(Eg - Eo)) <= 1e-6 * lat.n
+            acc_o = st.sweep(1.0, 1, record=True)[0]                 # the recording path stays on the direct kernel
+            assert np.array_equal(ctx.sweep_record(1.0), acc_o)
+            assert ctx.sweep_count == st.sweep_count
+            ctx.close()
+        lat, st = make_oracle(cfg)
+        ctx = make_gpu(cfg)
+        ctx.set_option("br_kernel", 2)
+        start(cfg, ctx, st)
+        for _ in range(3):
+            ctx.sweep(1.0, 1)
+            st.sweep(1.0, 1)
+        assert ctx.stats() == st.stats()
+        ctx.close()
+    with pytest.raises(hb.HbError):
+        hb.Context(hb.Lattice("bcc", 6)).set_option("br_kernel", 1)      # rows of 6 cells: not a multiple of 4
+
+
+def test_large_bcc_runs_the_warp_specialised_kernel_by_default():
+    # lattices of 2^24 sites and more: bcc defaults to br_kernel = 1 (DESIGN 6.10); first sweeps against the oracle, bit for bit
+    cfg = dict(W.SMALL["c2"], L=(256, 128, 256))
+    ctx = make_gpu(cfg)
+    assert ctx.get_option("br_kernel") == 1 and ctx.get_option("graph_active") == 0
+    lat, st = make_oracle(cfg)
+    start(cfg, ctx, st)
+    ctx.sweep(1.8, 2)
+    st.sweep(1.8, 2)
+    assert spins_equal(ctx.get_spins(), st.get_spins())
+    _measure_close(ctx, st, lat.n)
+    ctx.close()
