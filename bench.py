@@ -451,11 +451,14 @@ def main():
 
     # the second ceiling: the attempt arithmetic alone, no memory traffic, measured now on this device
     # in a 1 s run (so at the clock a long run holds); per GPU, like `achieved`
-    from paper_2106_11286_b200 import probe_alu
+    from paper_2106_11286_b200 import probe_alu, probe_pipe
+    from paper_2106_11286_b200.binding import PIPE_KINDS
     alu_peak = probe_alu(1.0, device) / 1e9
+    pipe_rates = {name: round(probe_pipe(k, device), 3) for k, name in enumerate(PIPE_KINDS)}
     roofline["alu"] = {"bound": "alu", "achieved": value / world, "peak": alu_peak, "unit": UNIT, "frac": value / world / alu_peak,
                        "peak_source": "hb_probe_alu: Philox + proposal + neighbour sum on registers + delta-H + acceptance, "
-                                      "4 attempts per thread as two packed pairs, 256-thread blocks, 4 per SM, measured in this run"}
+                                      "4 attempts per thread as two packed pairs, 256-thread blocks, 4 per SM, measured in this run",
+                       "pipe_rates": pipe_rates, "pipe_rates_unit": "warp-instructions per clock per SM (hb_probe_pipe, this run)"}
 
     cpu = None if args.no_cpu_baseline else run_cpu_baseline(cfg)
     # acceptance rate of the timed sweeps themselves (reported with every timed config): hb_stats counts the

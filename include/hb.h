@@ -223,6 +223,15 @@ int hb_probe_alu(void* cuda_stream, double seconds, double* updates_per_second);
 enum { HB_MATH_U01 = 0, HB_MATH_SINCOS = 1, HB_MATH_SPHERE = 2, HB_MATH_EXP = 3, HB_MATH_SQRT = 4, HB_MATH_ATTEMPT = 5 };
 int hb_device_math(int32_t op, int64_t count, const uint32_t* in0, const uint32_t* in1, float* out);
 
+/* Diagnostic: the issue rate of one instruction kind (or mix) the colour kernels are made of, in warp-instructions per clock
+ * per SM (4.0 = one per clock on each of the four sub-partitions), measured with the SM clock over a loop of 8 independent
+ * register chains per thread, 32 warps per SM.  It is the measurement behind the arithmetic ceiling of DESIGN.md section 7
+ * (a Philox round costs IMAD.WIDE + LOP3; packed fp32x2 costs two scalar slots).  Mixes count every named kind.
+ * Synchronises. */
+enum { HB_PIPE_FFMA = 0, HB_PIPE_FFMA2 = 1, HB_PIPE_IMAD = 2, HB_PIPE_IMAD_WIDE = 3, HB_PIPE_LOP3 = 4,
+       HB_PIPE_WIDE_LOP3 = 5, HB_PIPE_FFMA_WIDE_LOP3 = 6, HB_PIPE_FFMA2_WIDE_LOP3 = 7 };
+int hb_probe_pipe(void* cuda_stream, int32_t kind, double* warp_instr_per_clk_per_sm);
+
 /* Diagnostic: the rate (attempted updates per second) of the warp-specialised simple cubic colour kernel when its HBM
  * traffic is taken away: n_sweeps sweeps (two launches each, timed with CUDA events after two untimed ones) in which plane z
  * is read and written at the address of plane z mod `planes` (a power of two, e.g. 16), so that the whole launch lives in

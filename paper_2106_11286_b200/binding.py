@@ -18,7 +18,7 @@ EXPORTS = [
     "hb_sweep_each", "hb_measure_each", "hb_sweep_series_each", "hb_select_replica",
     "hb_slab_pass", "hb_slab_next_sweep", "hb_slab_face", "hb_slab_set_peer", "hb_probe_alu",
     "hb_device_alloc", "hb_device_free", "hb_ipc_export", "hb_ipc_open", "hb_ipc_close",
-    "hb_get_colouring", "hb_counters", "hb_stats", "hb_device_math", "hb_probe_sc_l2", "hb_set_option", "hb_get_option", "hb_lattice_fcc_sphere", "hb_lattice_free",
+    "hb_get_colouring", "hb_counters", "hb_stats", "hb_device_math", "hb_probe_sc_l2", "hb_probe_pipe", "hb_set_option", "hb_get_option", "hb_lattice_fcc_sphere", "hb_lattice_free",
     "hb_strerror", "hb_error_detail",
 ]
 
@@ -92,6 +92,7 @@ def load_library():
         "hb_stats": [vp, P(u64), P(u64)],
         "hb_device_math": [i32, i64, vp, vp, vp],
         "hb_probe_sc_l2": [vp, f32, i64, i32, P(C.c_double)],
+        "hb_probe_pipe": [vp, i32, P(C.c_double)],
         "hb_set_option": [vp, C.c_char_p, i64],
         "hb_get_option": [vp, C.c_char_p, P(i64)],
         "hb_lattice_fcc_sphere": [i32, f32, P(f32), f32, i32, P(hb_lattice), P(vp)],
@@ -207,6 +208,21 @@ def device_math(op, in0, in1=None, device="cuda:0"):
     if rc != 0:
         raise HbError(rc, "hb_device_math", L.hb_strerror(rc).decode())
     return out
+
+
+PIPE_KINDS = ["FFMA", "FFMA2", "IMAD", "IMAD.WIDE", "LOP3", "IMAD.WIDE+LOP3", "FFMA+IMAD.WIDE+LOP3", "FFMA2+IMAD.WIDE+LOP3"]
+
+
+def probe_pipe(kind, device="cuda:0"):
+    """hb_probe_pipe: warp-instructions per clock per SM of one instruction kind or mix (index into PIPE_KINDS)."""
+    import torch
+    L = load_library()
+    torch.cuda.set_device(torch.device(device))
+    v = C.c_double()
+    rc = L.hb_probe_pipe(torch.cuda.current_stream(torch.device(device)).cuda_stream, int(kind), C.byref(v))
+    if rc != 0:
+        raise HbError(rc, "hb_probe_pipe", L.hb_strerror(rc).decode())
+    return v.value
 
 
 def sizes(lat):

@@ -71,11 +71,19 @@ int make_plan(const hb_lattice* lat, Plan& p, std::string& why) {
   } else if (k == HB_CSR) {
     if (lat->n_sites < 0 || !lat->row_ptr) { why = "CSR lattice needs n_sites >= 0 and row_ptr"; return HB_EINVAL; }
     p.n = lat->n_sites;
-    p.nnz = lat->row_ptr[lat->n_sites];
+    // the sizes below come from row_ptr: it must start at 0 and never decrease before anything is derived from it
+    if (lat->row_ptr[0] != 0) { why = "row_ptr[0] must be 0"; return HB_EINVAL; }
     int64_t md = 0;
     for (int64_t i = 0; i < p.n; ++i) {
       const int64_t deg = lat->row_ptr[i + 1] - lat->row_ptr[i];
+      if (deg < 0) { why = "row_ptr must not decrease"; return HB_EINVAL; }
       if (deg > md) md = deg;
+    }
+    p.nnz = lat->row_ptr[lat->n_sites];
+    if (p.nnz > 0 && !lat->col_idx) { why = "CSR lattice needs col_idx"; return HB_EINVAL; }
+    // a caller-supplied colouring: the colour count sizes host and device tables, so it is bounded before anything is allocated
+    if (lat->colour && (lat->n_colours < 1 || lat->n_colours > kMaxColours || (int64_t)lat->n_colours > (p.n > 0 ? p.n : 1))) {
+      why = "n_colours must be in [1, min(n_sites, 65536)]"; return HB_EINVAL;
     }
     p.maxdeg = (int32_t)(md > 0x7FFFFFFF ? 0x7FFFFFFF : md);
   } else {

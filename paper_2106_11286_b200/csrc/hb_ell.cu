@@ -118,7 +118,8 @@ k_measure_ell(const float4* __restrict__ S, EllDev g, SweepParams P, double* par
 }
 
 __global__ void k_init_random_perm(float4* S, const int32_t* __restrict__ perm, uint32_t n, uint32_t seed_lo, uint32_t seed_hi) {
-  for (uint32_t m = blockIdx.x * blockDim.x + threadIdx.x; m < n; m += gridDim.x * blockDim.x) {
+  for (unsigned long long m64 = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; m64 < n; m64 += (unsigned long long)gridDim.x * blockDim.x) {
+    const uint32_t m = (uint32_t)m64;   // 64-bit loop index: a 32-bit one wraps below n when n is close to 2^32
     const Rand4 r = philox4x32_10((uint32_t)perm[m], 1u, 0u, 0u, seed_lo, seed_hi);
     float x, y, z;
     sphere(r.r0, r.r1, x, y, z);
@@ -127,13 +128,14 @@ __global__ void k_init_random_perm(float4* S, const int32_t* __restrict__ perm, 
 }
 
 __global__ void k_fill4(float4* S, uint32_t n, float x, float y, float z) {
-  for (uint32_t m = blockIdx.x * blockDim.x + threadIdx.x; m < n; m += gridDim.x * blockDim.x) S[m] = make_float4(x, y, z, 0.0f);
+  for (unsigned long long m = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; m < n; m += (unsigned long long)gridDim.x * blockDim.x) S[m] = make_float4(x, y, z, 0.0f);
 }
 
 // component comp of the internal AoS state <-> one canonical plane
 __global__ void k_permute(float4* S, float* plane, const int32_t* __restrict__ perm, uint32_t n, int comp, bool to_internal) {
   float* s = reinterpret_cast<float*>(S);
-  for (uint32_t m = blockIdx.x * blockDim.x + threadIdx.x; m < n; m += gridDim.x * blockDim.x) {
+  for (unsigned long long m64 = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; m64 < n; m64 += (unsigned long long)gridDim.x * blockDim.x) {
+    const uint32_t m = (uint32_t)m64;   // 64-bit loop index: a 32-bit one wraps below n when n is close to 2^32
     if (to_internal) s[4 * (size_t)m + comp] = plane[perm[m]]; else plane[perm[m]] = s[4 * (size_t)m + comp];
   }
 }

@@ -297,7 +297,8 @@ __device__ __forceinline__ uint32_t sc_canonical(const ScLayout& L, uint32_t m) 
 }
 
 __global__ void k_init_random_sc(float* sx, float* sy, float* sz, ScLayout L, uint32_t seed_lo, uint32_t seed_hi) {
-  for (uint32_t m = blockIdx.x * blockDim.x + threadIdx.x; m < L.n; m += gridDim.x * blockDim.x) {
+  for (unsigned long long m64 = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; m64 < L.n; m64 += (unsigned long long)gridDim.x * blockDim.x) {
+    const uint32_t m = (uint32_t)m64;   // 64-bit loop index: a 32-bit one wraps below n when n is close to 2^32
     const Rand4 r = philox4x32_10(sc_canonical(L, m) + L.site_base, 1u, 0u, 0u, seed_lo, seed_hi);
     float x, y, z;
     sphere(r.r0, r.r1, x, y, z);
@@ -306,7 +307,8 @@ __global__ void k_init_random_sc(float* sx, float* sy, float* sz, ScLayout L, ui
 }
 
 __global__ void k_init_random_flat(float* sx, float* sy, float* sz, uint32_t n, uint32_t seed_lo, uint32_t seed_hi) {
-  for (uint32_t m = blockIdx.x * blockDim.x + threadIdx.x; m < n; m += gridDim.x * blockDim.x) {
+  for (unsigned long long m64 = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; m64 < n; m64 += (unsigned long long)gridDim.x * blockDim.x) {
+    const uint32_t m = (uint32_t)m64;   // 64-bit loop index: a 32-bit one wraps below n when n is close to 2^32
     const Rand4 r = philox4x32_10(m, 1u, 0u, 0u, seed_lo, seed_hi);
     float x, y, z;
     sphere(r.r0, r.r1, x, y, z);
@@ -315,14 +317,16 @@ __global__ void k_init_random_flat(float* sx, float* sy, float* sz, uint32_t n, 
 }
 
 __global__ void k_fill(float* sx, float* sy, float* sz, uint32_t n, float x, float y, float z) {
-  for (uint32_t m = blockIdx.x * blockDim.x + threadIdx.x; m < n; m += gridDim.x * blockDim.x) {
+  for (unsigned long long m64 = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; m64 < n; m64 += (unsigned long long)gridDim.x * blockDim.x) {
+    const uint32_t m = (uint32_t)m64;   // 64-bit loop index: a 32-bit one wraps below n when n is close to 2^32
     sx[m] = x; sy[m] = y; sz[m] = z;
   }
 }
 
 // dst[m] = src[canonical(m)] (to_internal) or dst[canonical(m)] = src[m]
 __global__ void k_sc_permute(float* dst, const float* src, ScLayout L, bool to_internal) {
-  for (uint32_t m = blockIdx.x * blockDim.x + threadIdx.x; m < L.n; m += gridDim.x * blockDim.x) {
+  for (unsigned long long m64 = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; m64 < L.n; m64 += (unsigned long long)gridDim.x * blockDim.x) {
+    const uint32_t m = (uint32_t)m64;   // 64-bit loop index: a 32-bit one wraps below n when n is close to 2^32
     const uint32_t id = sc_canonical(L, m);
     if (to_internal) dst[m] = src[id]; else dst[id] = src[m];
   }

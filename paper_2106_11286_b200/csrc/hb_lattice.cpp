@@ -149,7 +149,22 @@ std::string validate_csr(int64_t n, const int64_t* row_ptr, const int32_t* col) 
       if (j < 0 || j >= n) return "col_idx out of range";
       if (j == i) return "self loop";
     }
-  // symmetric with multiplicity: #(j in row i) == #(i in row j)
+  // symmetric with multiplicity: #(j in row i) == #(i in row j).  Rows of bounded length are compared pair by pair
+  // (O(sum of deg^2): lattices); a table with long rows (hubs) compares the sorted lists of (i, j) and (j, i) instead
+  int64_t maxdeg = 0;
+  for (int64_t i = 0; i < n; ++i) maxdeg = std::max<int64_t>(maxdeg, row_ptr[i + 1] - row_ptr[i]);
+  if (maxdeg > 64) {
+    std::vector<uint64_t> fwd, rev;
+    fwd.reserve((size_t)row_ptr[n]); rev.reserve((size_t)row_ptr[n]);
+    for (int64_t i = 0; i < n; ++i)
+      for (int64_t k = row_ptr[i]; k < row_ptr[i + 1]; ++k) {
+        fwd.push_back(((uint64_t)i << 32) | (uint32_t)col[k]);
+        rev.push_back(((uint64_t)(uint32_t)col[k] << 32) | (uint64_t)i);
+      }
+    std::sort(fwd.begin(), fwd.end());
+    std::sort(rev.begin(), rev.end());
+    return fwd == rev ? "" : "neighbour table is not symmetric";
+  }
   for (int64_t i = 0; i < n; ++i)
     for (int64_t k = row_ptr[i]; k < row_ptr[i + 1]; ++k) {
       const int64_t j = col[k];

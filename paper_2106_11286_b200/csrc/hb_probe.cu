@@ -7,6 +7,7 @@
 // section 4) allows on this chip at the clock it holds: the "alu" roofline bench.py reports beside the HBM one
 // (DESIGN.md section 7).
 #include <cstring>
+#include <new>
 
 #include "../../include/hb.h"
 #include "hb_device.cuh"
@@ -77,6 +78,119 @@ extern "C" int hb_probe_alu(void* cuda_stream, double seconds, double* updates_p
   if (e0) cudaEventDestroy(e0);
   if (e1) cudaEventDestroy(e1);
   cudaFree(out);
+  return rc;
+}
+
+// ---- hb_probe_pipe: issue rates of the instruction kinds the colour kernels are made of (profiles/r01_pipe_rates.md) -------
+namespace hb {
+namespace {
+
+// 8 independent register chains per thread, 64 instructions of the probed kind(s) per loop trip, timed with the SM clock
+template <int KIND>
+__global__ void __launch_bounds__(256, 4) k_probe_pipe(unsigned long long* per_sm, uint32_t* sink, int trips, uint32_t seed) {
+  uint32_t a[8], b[8];
+  float f[8], g[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) { a[i] = seed + threadIdx.x * 8u + i; b[i] = a[i] * 2654435761u; f[i] = 1.0f + 1e-3f * i; g[i] = 0.5f + 1e-3f * i; }
+  const float c1 = 1.0000001f, c0 = 1e-9f;
+  __syncthreads();
+  const long long t0 = clock64();
+  for (int t = 0; t < trips; ++t) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        if (KIND == HB_PIPE_FFMA || KIND == HB_PIPE_FFMA_WIDE_LOP3)
+          asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(f[i]) : "f"(c1), "f"(c0));
+        if (KIND == HB_PIPE_FFMA2 || KIND == HB_PIPE_FFMA2_WIDE_LOP3) {
+          unsigned long long p, q, s;
+          asm volatile("mov.b64 %0, {%1, %2};" : "=l"(p) : "f"(f[i]), "f"(g[i]));
+          asm volatile("mov.b64 %0, {%1, %1};" : "=l"(q) : "f"(c1));
+          asm volatile("mov.b64 %0, {%1, %1};" : "=l"(s) : "f"(c0));
+          asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(p) : "l"(q), "l"(s));
+          asm volatile("mov.b64 {%0, %1}, %2;" : "=f"(f[i]), "=f"(g[i]) : "l"(p));
+        }
+        if (KIND == HB_PIPE_IMAD)
+          asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(a[i]) : "r"(0xD2511F53u), "r"(b[i]));
+        if (KIND == HB_PIPE_IMAD_WIDE || KIND == HB_PIPE_WIDE_LOP3 || KIND == HB_PIPE_FFMA_WIDE_LOP3 || KIND == HB_PIPE_FFMA2_WIDE_LOP3) {
+          unsigned long long w;
+          asm volatile("mul.wide.u32 %0, %1, %2;" : "=l"(w) : "r"(a[i]), "r"(0xD2511F53u));
+          if (KIND == HB_PIPE_IMAD_WIDE) asm volatile("{ .reg .u32 lo, hi; mov.b64 {lo, hi}, %1; add.u32 %0, lo, hi; }" : "=r"(a[i]) : "l"(w));   // (an add rides along)
+          else asm volatile("{ .reg .u32 lo, hi; mov.b64 {lo, hi}, %2; lop3.b32 %0, lo, hi, %1, 0x96; }" : "=r"(a[i]) : "r"(b[i]), "l"(w));       // a Philox half round
+        }
+        if (KIND == HB_PIPE_LOP3)
+          asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a[i]) : "r"(b[i]), "r"(seed));
+      }
+    }
+  }
+  const long long t1 = clock64();
+  uint32_t acc = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) acc ^= a[i] ^ __float_as_uint(f[i]) ^ __float_as_uint(g[i]);
+  if (acc == 0x12345u) sink[0] = acc;   // keeps the chains alive
+  if (threadIdx.x == 0) {   // per SM (the clock is the SM's own): warps that ran there, first start, last end
+    uint32_t smid;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    atomicAdd(per_sm + 3 * smid, (unsigned long long)(blockDim.x >> 5));
+    atomicMin(per_sm + 3 * smid + 1, (unsigned long long)t0);
+    atomicMax(per_sm + 3 * smid + 2, (unsigned long long)t1);
+  }
+}
+
+constexpr int kProbeSmMax = 1024;
+
+__global__ void k_probe_pipe_reset(unsigned long long* per_sm) {
+  for (int i = threadIdx.x; i < kProbeSmMax; i += blockDim.x) { per_sm[3 * i] = 0ull; per_sm[3 * i + 1] = ~0ull; per_sm[3 * i + 2] = 0ull; }
+}
+
+template <int KIND>
+cudaError_t probe_pipe_go(cudaStream_t st, unsigned long long* per_sm, uint32_t* sink, int blocks, int trips) {
+  k_probe_pipe<KIND><<<blocks, 256, 0, st>>>(per_sm, sink, 16, 1u);   // warm-up
+  k_probe_pipe_reset<<<1, 256, 0, st>>>(per_sm);
+  k_probe_pipe<KIND><<<blocks, 256, 0, st>>>(per_sm, sink, trips, 1u);
+  return cudaGetLastError();
+}
+
+}  // namespace
+}  // namespace hb
+
+extern "C" int hb_probe_pipe(void* cuda_stream, int32_t kind, double* warp_instr_per_clk_per_sm) {
+  if (!warp_instr_per_clk_per_sm || kind < 0 || kind > HB_PIPE_FFMA2_WIDE_LOP3) return HB_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) return HB_ECUDA;
+  const int blocks = sms * 4, trips = 2000;       // one wave: 4 blocks of 8 warps on every SM
+  unsigned long long* cycles = nullptr;
+  uint32_t* sink = nullptr;
+  if (cudaMalloc(&cycles, (size_t)hb::kProbeSmMax * 24) != cudaSuccess || cudaMalloc(&sink, 4) != cudaSuccess) { cudaFree(cycles); cudaGetLastError(); return HB_ENOMEM; }
+  cudaError_t e = cudaSuccess;
+  switch (kind) {
+    case HB_PIPE_FFMA: e = hb::probe_pipe_go<HB_PIPE_FFMA>(st, cycles, sink, blocks, trips); break;
+    case HB_PIPE_FFMA2: e = hb::probe_pipe_go<HB_PIPE_FFMA2>(st, cycles, sink, blocks, trips); break;
+    case HB_PIPE_IMAD: e = hb::probe_pipe_go<HB_PIPE_IMAD>(st, cycles, sink, blocks, trips); break;
+    case HB_PIPE_IMAD_WIDE: e = hb::probe_pipe_go<HB_PIPE_IMAD_WIDE>(st, cycles, sink, blocks, trips); break;
+    case HB_PIPE_LOP3: e = hb::probe_pipe_go<HB_PIPE_LOP3>(st, cycles, sink, blocks, trips); break;
+    case HB_PIPE_WIDE_LOP3: e = hb::probe_pipe_go<HB_PIPE_WIDE_LOP3>(st, cycles, sink, blocks, trips); break;
+    case HB_PIPE_FFMA_WIDE_LOP3: e = hb::probe_pipe_go<HB_PIPE_FFMA_WIDE_LOP3>(st, cycles, sink, blocks, trips); break;
+    default: e = hb::probe_pipe_go<HB_PIPE_FFMA2_WIDE_LOP3>(st, cycles, sink, blocks, trips); break;
+  }
+  int rc = HB_ECUDA;
+  if (e == cudaSuccess && cudaStreamSynchronize(st) == cudaSuccess) {
+    unsigned long long* h = new (std::nothrow) unsigned long long[3 * hb::kProbeSmMax];
+    if (h && cudaMemcpy(h, cycles, (size_t)hb::kProbeSmMax * 24, cudaMemcpyDeviceToHost) == cudaSuccess) {
+      // probed instructions per warp and trip: 64 of each kind in the mix (the packing moves and adds that ride along are not counted)
+      const int kinds_in_mix = kind == HB_PIPE_WIDE_LOP3 ? 2 : ((kind == HB_PIPE_FFMA_WIDE_LOP3 || kind == HB_PIPE_FFMA2_WIDE_LOP3) ? 3 : 1);
+      const double per_warp = 64.0 * kinds_in_mix * trips;
+      double sum = 0.0;
+      int used = 0;
+      for (int i = 0; i < hb::kProbeSmMax; ++i)       // every SM that ran warps: their instructions over its busy span
+        if (h[3 * i] > 0 && h[3 * i + 2] > h[3 * i + 1]) { sum += (double)h[3 * i] * per_warp / (double)(h[3 * i + 2] - h[3 * i + 1]); used += 1; }
+      if (used > 0) { *warp_instr_per_clk_per_sm = sum / used; rc = HB_OK; }
+    }
+    delete[] h;
+  }
+  cudaFree(cycles); cudaFree(sink);
+  cudaGetLastError();
   return rc;
 }
 

@@ -44,11 +44,16 @@ def run_scan(ctx, temperatures, sweeps, equil=0):
     return {k: np.array(v) for k, v in out.items()}
 
 
-def fit_order_parameter(T, m, t_lo, t_hi):
+def fit_order_parameter(T, m, t_lo, t_hi, Tc_fixed=None):
     """Least squares of log m = log A + beta log(1 - T/Tc) over the points with t_lo <= 1 - T/Tc <= t_hi, scanning Tc
-    (the form the paper fits in its Fig. 3).  Returns (Tc, beta, A, rms of the log residual)."""
+    (the form the paper fits in its Fig. 3), or at a given Tc.  Returns (Tc, beta, A, rms of the
+    log residual, points used) or None."""
+    T, m = np.asarray(T, float), np.asarray(m, float)
     best = None
-    for Tc in np.arange(max(T) * 0.9, max(T) * 1.2, 0.0005):
+    # the ordered phase reaches at least to the last temperature at which m is still a good fraction of its largest value:
+    # a candidate Tc below it would cut the data down to a few points that any exponent fits
+    T_ordered = max(T[m >= 0.15 * m.max()])
+    for Tc in ([Tc_fixed] if Tc_fixed else np.arange(T_ordered + 0.0005, max(T) * 1.1, 0.0005)):
         t = 1.0 - T / Tc
         sel = (t >= t_lo) & (t <= t_hi)
         if sel.sum() < 4:
@@ -59,8 +64,36 @@ def fit_order_parameter(T, m, t_lo, t_hi):
             continue
         rms = float(np.sqrt(np.mean((y - (beta * x + logA)) ** 2)))
         if best is None or rms < best[3]:
-            best = (float(Tc), float(beta), float(np.exp(logA)), rms)
+            best = (float(Tc), float(beta), float(np.exp(logA)), rms, int(sel.sum()))
     return best
+
+
+def window_table(T, m, t_los=(0.002, 0.005, 0.01, 0.02, 0.05), t_his=(0.02, 0.03, 0.05, 0.1, 0.2), Tc_fixed=None):
+    """The effective exponent of the fit above for a sweep of windows (the paper does not state its window):
+    rows (t_lo, t_hi, Tc, beta, rms, points)."""
+    rows = []
+    for lo in t_los:
+        for hi in t_his:
+            if hi < 2.5 * lo:
+                continue
+            f = fit_order_parameter(T, m, lo, hi, Tc_fixed)
+            if f:
+                rows.append((lo, hi, f[0], f[1], f[3], f[4]))
+    return rows
+
+
+def print_windows(T, m, Tc_values=()):
+    print("# effective exponent beta of M = A (1 - T/Tc)^beta against the fit window t_lo <= 1 - T/Tc <= t_hi")
+    for Tc in (None,) + tuple(Tc_values):
+        print("# Tc %s:  t_lo  t_hi  Tc  beta  rms(log)  points" % ("fitted" if Tc is None else "fixed at %.4f" % Tc))
+        for r in window_table(T, m, Tc_fixed=Tc):
+            print("#   %.3f  %.3f  %.4f  %.4f  %.1e  %d" % r)
+
+
+def load_table(path):
+    """A table written by `--sc ... --out path`: columns T, <|M|>, <E>/N, chi, C."""
+    a = np.loadtxt(path, comments="#", ndmin=2)
+    return {k: a[:, i] for i, k in enumerate(("T", "absM", "E", "chi", "C"))}
 
 
 def throughput_vs_size(sizes, T=1.30, K=0.01, seconds=0.5):
@@ -88,7 +121,7 @@ def throughput_vs_size(sizes, T=1.30, K=0.01, seconds=0.5):
 
 def main(argv):
     """python -m paper_2106_11286_b200.scan c2 | --sc L [--K k] [--T a:b:n] [--equil e] [--sweeps s] [--fit t_lo:t_hi]
-    | --fig2 [L ...]"""
+    [--out file] [--windows [--Tc 1.443,1.445]] | --analyse file [Tc ...] | --fig2 [L ...]"""
     if len(argv) > 1 and argv[1] == "--fig2":
         sizes = [int(x) for x in argv[2:]] or [16, 32, 64, 128, 256, 464, 512, 1024]
         print("# sc L^3, J = 1, K = 0.01, T = 1.30 (0.9 T_C), random start: attempted updates per second, time per update")
@@ -106,7 +139,20 @@ def main(argv):
         ap.add_argument("--equil", type=int, default=10000)
         ap.add_argument("--sweeps", type=int, default=10000)
         ap.add_argument("--fit", default="0.02:0.2")
+        ap.add_argument("--out", default=None, help="also write the table (and the fits) to this file")
+        ap.add_argument("--windows", action="store_true", help="the effective exponent over a sweep of fit windows")
+        ap.add_argument("--Tc", default="", help="comma-separated critical temperatures to hold fixed in the window sweep")
         a = ap.parse_args(argv[1:])
+        if a.out:      # everything printed below goes to the file as well
+            import io
+            class Tee(io.TextIOBase):
+                def __init__(self, *fs): self.fs = fs
+                def write(self, t):
+                    for f in self.fs: f.write(t)
+                    return len(t)
+                def flush(self):
+                    for f in self.fs: f.flush()
+            sys.stdout = Tee(sys.__stdout__, open(a.out, "w"))
         lo, hi, k = a.T.split(":")
         Ts = [float(x) for x in np.linspace(float(lo), float(hi), int(k))]
         cfg = dict(kind="sc", L=a.sc, J=1.0, K=a.K, e=(0.0, 0.0, 1.0), seed=1, start="aligned")
@@ -120,8 +166,15 @@ def main(argv):
         fit = fit_order_parameter(res["T"], res["absM"], t_lo, t_hi)
         if fit:
             print("# fit M = A (1 - T/Tc)^beta over %g <= 1 - T/Tc <= %g: Tc = %.4f, beta = %.4f, A = %.4f, rms(log) = %.2e" %
-                  ((t_lo, t_hi) + fit))
+                  ((t_lo, t_hi) + fit[:4]))
+        if a.windows:
+            print_windows(res["T"], res["absM"], [float(x) for x in a.Tc.split(",") if x])
         ctx.close()
+        sys.stdout.flush()
+        return
+    if len(argv) > 2 and argv[1] == "--analyse":     # the fits again from a saved table (no device needed)
+        res = load_table(argv[2])
+        print_windows(res["T"], res["absM"], [float(x) for x in argv[3:]])
         return
     name = argv[1] if len(argv) > 1 else "c2"
     cfg = workloads.CONFIGS[name]

@@ -9,8 +9,8 @@ Every slab is an hb context over planes z0 .. z0 + nz - 1 of the whole lattice p
 i.e. ONE exchange step per colour: 2 faces x 3 components x (Lx Ly / 2) floats per slab.  Philox is keyed by the global
 site id, so the slabs together walk the single-context trajectory bit for bit (tests/test_slabs.py).
 
-* `LocalSlabs`: all slabs in this process (one GPU, or several devices of one process); faces move with
-  `Tensor.copy_` on the contexts' stream (a device-to-device / peer copy), or, with `peer_stores=True`, inside the colour
+* `LocalSlabs`: all slabs in this process on ONE device (several devices take one process each: `DistSlab`); faces move with
+  `Tensor.copy_` on the contexts' stream (a device-to-device copy), or, with `peer_stores=True`, inside the colour
   kernels themselves: a thread that stores an updated spin of a boundary plane stores it into the neighbour's ghost plane
   too (`hb_slab_set_peer`), so the transfer overlaps the pass and only a barrier remains between two passes.
 * `DistSlab`: one slab per rank of a `torch.distributed` group (one process per GPU); faces move with
@@ -72,8 +72,16 @@ def exchange_dist(ctx, colour, rank, world, group=None):
         send_b, recv_b = send, recv
     ops = [dist.P2POp(dist.isend, t, p, group) for t, p in zip(send_b, peers_s)]
     ops += [dist.P2POp(dist.irecv, t, p, group) for t, p in zip(recv_b, peers_r)]
-    for req in dist.batch_isend_irecv(ops):
-        req.wait()
+    if staged:
+        for req in dist.batch_isend_irecv(ops):
+            req.wait()
+    else:
+        # NCCL enqueues on torch's current stream: make that the stream of the colour passes, so that the sends queue behind
+        # the pass that produced the faces and the next pass behind the receives, whatever stream the caller is in
+        import torch
+        with torch.cuda.stream(ctx.stream):
+            for req in dist.batch_isend_irecv(ops):
+                req.wait()
     if staged:
         for dst, src in zip(recv, recv_b):
             dst.copy_(src)
@@ -82,20 +90,22 @@ def exchange_dist(ctx, colour, rank, world, group=None):
 class LocalSlabs:
     """n_slabs slab contexts of one periodic sc lattice in this process."""
 
-    def __init__(self, Lx, Ly, Lz, n_slabs, J=1.0, K=0.0, e=(0.0, 0.0, 1.0), seed=1, devices=None, options=None,
+    def __init__(self, Lx, Ly, Lz, n_slabs, J=1.0, K=0.0, e=(0.0, 0.0, 1.0), seed=1, device="cuda:0", options=None,
                  peer_stores=False):
+        """All slabs live on `device`.  (The library issues every call on the CUDA device that is current, and a process that
+        drove contexts on several devices would have to switch it around every call and enable peer access itself: that
+        path was never run on a multi-GPU box, so it is not offered -- one process per GPU, `DistSlab`, is.)"""
         from .binding import Context, Lattice
         self.shape = (Lx, Ly, Lz)
         self.parts = partition(Lz, n_slabs)
-        devices = devices or ["cuda:0"] * n_slabs
-        self.ctxs = [Context(Lattice("sc", Lx, Ly, nz, slab=(z0, Lz)), J, K, e, seed, device=devices[r])
+        self.ctxs = [Context(Lattice("sc", Lx, Ly, nz, slab=(z0, Lz)), J, K, e, seed, device=device)
                      for r, (z0, nz) in enumerate(self.parts)]
         for c in self.ctxs:
             for k, v in (options or {}).items():
                 c.set_option(k, v)
         self.n = Lx * Ly * Lz
         # peer stores (hb_slab_set_peer): the colour kernels write their boundary planes straight into the neighbours'
-        # ghost planes, the exchange step disappears; contexts on different devices need peer access enabled
+        # ghost planes, the exchange step disappears
         self.peer_stores = bool(peer_stores)
         if self.peer_stores:
             for r, c in enumerate(self.ctxs):
@@ -135,7 +145,7 @@ class LocalSlabs:
         return [np.concatenate([p[k] for p in parts]) for k in range(3)]
 
     def sweep(self, T, n_sweeps=1):
-        several = len({str(c.device) for c in self.ctxs}) > 1 or len({c.stream.cuda_stream for c in self.ctxs}) > 1
+        several = len({c.stream.cuda_stream for c in self.ctxs}) > 1
         for _ in range(n_sweeps):
             for colour in (0, 1):
                 for c in self.ctxs:
@@ -227,7 +237,10 @@ class DistSlab:
         import torch
         import torch.distributed as dist
         if self._nccl:
-            dist.all_reduce(self._flag, group=self.group)    # stream-ordered: the next pass queues behind it
+            # NCCL orders the collective on torch's CURRENT stream: make that the stream the passes run on, whatever stream
+            # the caller is in, so that the next pass queues behind the collective and the collective behind this pass
+            with torch.cuda.stream(self.ctx.stream):
+                dist.all_reduce(self._flag, group=self.group)
         else:
             torch.cuda.synchronize(self.ctx.device)
             dist.barrier(group=self.group)

@@ -117,6 +117,47 @@ def test_sizes_rejects_bad_lattices():
         hb.sizes(hb.Lattice("fcc", 1100))
 
 
+def test_table_validation_happens_before_anything_is_sized_or_allocated():
+    # a caller-supplied colouring with an absurd colour count, a row_ptr that decreases or does not start at 0
+    # must be rejected by hb_sizes / hb_create before any table is sized from them
+    rp = np.array([0, 1, 2], np.int64)
+    ci = np.array([1, 0], np.int32)
+    ok = hb.Lattice("csr", row_ptr=rp, col_idx=ci, colour=np.array([0, 1], np.int32), n_colours=2)
+    assert hb.sizes(ok)[0] == 2
+    for bad in (hb.Lattice("csr", row_ptr=rp, col_idx=ci, colour=np.array([0, 1], np.int32), n_colours=200),
+                hb.Lattice("csr", row_ptr=rp, col_idx=ci, colour=np.array([0, 1], np.int32), n_colours=1 << 30),
+                hb.Lattice("csr", row_ptr=rp, col_idx=ci, colour=np.array([0, 1], np.int32), n_colours=0),
+                hb.Lattice("csr", row_ptr=np.array([0, 2, 1], np.int64), col_idx=ci),
+                hb.Lattice("csr", row_ptr=np.array([1, 2, 3], np.int64), col_idx=ci)):
+        with pytest.raises(hb.HbError) as e:
+            hb.sizes(bad)
+        assert e.value.status == -1
+
+
+def _create_status(lat):
+    """hb_create with library-owned memory, straight through ctypes (no device is needed to be refused)."""
+    lib = hb.load_library()
+    h = C.c_void_p()
+    s = lat.struct()
+    rc = lib.hb_create(C.byref(h), C.byref(s), 1.0, 0.0, (C.c_float * 3)(0, 0, 1), 1, None)
+    detail = lib.hb_error_detail(h).decode() if h else ""
+    lib.hb_destroy(h)
+    return rc, detail
+
+
+def test_symmetry_check_of_hub_graphs():
+    # a star with 200 leaves: rows longer than 64 entries take the sort-based symmetry check of validate_csr
+    n = 201
+    rp = np.concatenate([[0, 200], 200 + np.arange(1, 201)]).astype(np.int64)
+    ci = np.concatenate([np.arange(1, 201), np.zeros(200)]).astype(np.int32)
+    rc, detail = _create_status(hb.Lattice("csr", row_ptr=rp, col_idx=ci))
+    assert rc != -1 or "symmetric" not in detail          # valid table: whatever stops it on a box without a GPU, it is not the table
+    bad = ci.copy()
+    bad[-1] = 5                                            # leaf 200 points at leaf 5 instead of the hub
+    rc, detail = _create_status(hb.Lattice("csr", row_ptr=rp, col_idx=bad))
+    assert rc == -1 and "symmetric" in detail
+
+
 def test_memory_plan_of_table_engines_and_replicas():
     # host logic of hb_sizes: neighbour tables of near-uniform degree take the colour-major ELL layout with AoS float4
     # spins (16 B per site), irregular graphs the plain CSR layout (12 B per site); replicas multiply the state

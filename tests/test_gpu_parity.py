@@ -832,3 +832,26 @@ def test_large_bcc_runs_the_warp_specialised_kernel_by_default():
     assert spins_equal(ctx.get_spins(), st.get_spins())
     _measure_close(ctx, st, lat.n)
     ctx.close()
+
+
+def test_fig3_protocol_shortened():
+    # The paper's accuracy experiment [P:52-58, Fig. 3] shortened (2000 + 2000 sweeps per temperature instead of 10^4 + 10^4;
+    # the full scans and their fits: profiles/fig3/): sc 128^3 and 256^3, aligned start, heating.  K = 0: the fitted critical
+    # temperature is the literature value 1.443 (the paper prints 1.445).  K = 0.01 (the paper's): the two sizes give the same
+    # <|M|>(T) to 1e-3 below the transition ("numerical stability ... up to 10^8 spins" [P:54]).
+    from paper_2106_11286_b200 import scan
+    def curve(L, K, Ts, sweeps=2000):
+        ctx = scan.make_context(dict(kind="sc", L=L, J=1.0, K=K, e=(0.0, 0.0, 1.0), seed=1, start="aligned"))
+        res = scan.run_scan(ctx, Ts, sweeps, sweeps)
+        ctx.close()
+        return res
+    Ts = [float(t) for t in np.arange(1.30, 1.4351, 0.0075)]
+    r128 = curve(128, 0.0, Ts)
+    Tc, beta = scan.fit_order_parameter(r128["T"], r128["absM"], 0.01, 0.1)[:2]
+    assert abs(Tc - 1.443) <= 0.005, (Tc, beta)
+    assert 0.32 <= beta <= 0.38, (Tc, beta)
+    assert np.all(np.diff(r128["absM"]) < 0)                      # M(T) falls monotonically towards T_C
+    Tk = [1.30, 1.32, 1.34, 1.36, 1.38, 1.40]
+    a, b = curve(128, 0.01, Tk, 5000), curve(256, 0.01, Tk, 5000)
+    assert np.max(np.abs(a["absM"] - b["absM"])) <= 1e-3, (a["absM"], b["absM"])
+    assert np.max(np.abs(a["E"] - b["E"])) <= 1e-3
