@@ -260,7 +260,7 @@ def run_slabs(args, cfg, rank, world, device, barrier):
     Lx, Ly, Lz = (L, L, L) if isinstance(L, int) else L
     options = dict((kv.split("=", 1)[0], int(kv.split("=", 1)[1])) for kv in args.option)
     sl = slabs.DistSlab(Lx, Ly, Lz, cfg["J"], cfg["K"], cfg["e"], cfg["seed"], device=device, options=options,
-                        peer_stores=args.slab_exchange == "peer")
+                        peer_stores=args.slab_exchange in ("peer", "flags"), flags=args.slab_exchange == "flags")
     sl.init_random() if cfg["start"] == "random" else sl.init_aligned(cfg["e"])
     T = cfg["T"][0]
     for _ in range(args.warmup):
@@ -298,8 +298,9 @@ def run_slabs(args, cfg, rank, world, device, barrier):
                        "multi_gpu": "slabs along z: %s planes per rank, %d bytes of boundary planes per rank and sweep (%s), "
                                     "one all_reduce of 32 bytes per measurement" % (
                                         [nz for _, nz in slabs.partition(Lz, world)], face_bytes,
-                                        "stored by the colour kernels into the neighbours' ghost planes, a barrier per pass"
-                                        if sl.peer_stores else "sent as faces after every pass"),
+                                        "stored by the colour kernels into the neighbours' ghost planes, neighbour flags inside the kernels"
+                                        if sl.flags else ("stored by the colour kernels into the neighbours' ghost planes, a barrier per pass"
+                                                          if sl.peer_stores else "sent as faces after every pass")),
                        "l2": "state %.0f MB per rank" % (12.0 * n / world / 1e6)},
             "ns_per_update": 1.0 / value, "clocks": clocks, "e2e": None, "gpu_launches": launches,
             "M": [float(x) for x in M], "E_per_spin": E / n,
@@ -325,9 +326,11 @@ def main():
     ap.add_argument("--multi", default="replicas", choices=["replicas", "slabs"],
                     help="N > 1: independent replicas (default, weak scaling) or ONE lattice cut into z-slabs with a face "
                          "exchange per colour (strong scaling; simple cubic workloads; DESIGN.md section 9)")
-    ap.add_argument("--slab-exchange", default="peer", choices=["peer", "copies"],
+    ap.add_argument("--slab-exchange", default="peer", choices=["peer", "flags", "copies"],
                     help="--multi slabs: boundary planes stored by the colour kernels straight into the neighbours' ghost planes "
-                         "(peer memory, CUDA IPC between the ranks; default) or sent as faces after every pass (NCCL send/recv)")
+                         "(peer memory, CUDA IPC between the ranks) with a one-word all_reduce as barrier between passes (peer, default) "
+                         "or with neighbour flags set and awaited inside the kernels, boundary tiles first (flags; one GPU per rank), "
+                         "or faces sent after every pass (copies: NCCL send/recv)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()

@@ -190,6 +190,14 @@ int hb_slab_face(hb_ctx* ctx, int32_t colour, int32_t side, int32_t ghost, size_
  * (stream order on one device; a collective or an event between devices).  The ghost planes must still be filled once
  * with hb_slab_face copies after hb_init_* / hb_set_spins.  peer_spins = NULL switches the side back to copies. */
 int hb_slab_set_peer(hb_ctx* ctx, int32_t side, void* peer_spins, int32_t peer_Lz);
+/* hb_set_option(ctx, "slab_flags", 1) (after hb_slab_set_peer on both sides; warp-specialised kernel) replaces that barrier by
+ * flags between neighbours, kept in the two words behind each slab's spins (so that a peer mapping of the spins buffer
+ * reaches them; hb_sizes counts them): colour pass number s of a slab takes its two boundary chunks first; a boundary tile
+ * waits (acquire at system scope) until the neighbour on its side has finished the boundary chunk of ITS pass s - 1, and the
+ * last warp of a boundary chunk writes s into that neighbour's flag (release at system scope) after the chunk's stores,
+ * the ones into the neighbour's ghost plane included.  Interior tiles never wait.  All slabs must issue the same sequence
+ * of hb_slab_pass calls, and the kernels of neighbouring slabs must be able to run at the same time (one GPU each) or in
+ * the order of the passes (one stream): two processes that share one GPU must not use it. */
 
 /* Device memory that another process can map (one process per GPU, peer stores between slabs): hb_device_alloc is a
  * plain cudaMalloc on the current device (the result can be handed to hb_create in hb_buffers.spins), hb_ipc_export fills

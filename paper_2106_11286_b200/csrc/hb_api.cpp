@@ -164,6 +164,8 @@ struct hb_ctx {
   bool g_dirty[2] = {true, true};
   int pdl = 1;                 // colour kernels are launched with programmatic stream serialisation (option pdl)
   int32_t slab_Lz = 0, slab_z0 = 0;   // > 0: this context is a slab of a larger lattice (planes 0 and Lz-1 of sc are ghosts)
+  uint32_t slab_stamp = 0;            // colour passes of this slab so far (neighbour flags, option slab_flags)
+  uint32_t* slab_flags() const { return reinterpret_cast<uint32_t*>(spins_base + 3 * (size_t)plan.n); }   // two words behind the spins
   int sc_coop = -1;            // persistent multi-sweep kernel: -1 auto, 0 off, 1 / 2 forced (see hb_set_option)
   bool fused_measure = true;   // sc: the last sweep of hb_sweep also reduces M and E
   bool cache_valid = false;    // cached() holds the measurement of the current spins
@@ -197,6 +199,7 @@ struct hb_ctx {
   unsigned long long* sweep_dev() const { return reinterpret_cast<unsigned long long*>(ws + plan.off_counters + 128); }
   unsigned long long* series_idx() const { return reinterpret_cast<unsigned long long*>(ws + plan.off_counters + 136); }
   uint32_t* ws_sched() const { return reinterpret_cast<uint32_t*>(ws + plan.off_counters + 144); }   // tile scheduler of k_sweep_sc_ws
+  uint32_t* slab_bnd_count() const { return reinterpret_cast<uint32_t*>(ws + plan.off_counters + 160); }   // two words
   uint32_t* ws_done() const { return reinterpret_cast<uint32_t*>(ws + plan.off_wsdone); }            // progress words of its fused launches
 };
 
@@ -504,6 +507,7 @@ int hb_sizes(const hb_lattice* lat, int64_t* n_sites, size_t* spins_bytes, size_
   rc = make_plan(&padded, p, why);
   if (rc != HB_OK) return rc;
   if (n_sites) *n_sites = lat->slab_Lz > 0 ? (int64_t)lat->Lx * lat->Ly * lat->Lz : p.n;   // a slab's own sites
+  if (lat->slab_Lz > 0) p.spins_bytes += kAlign;   // the neighbour flags live behind the spins, where a peer mapping of the buffer reaches them
   if (spins_bytes) *spins_bytes = p.spins_bytes;
   if (workspace_bytes) *workspace_bytes = p.ws_bytes;
   return HB_OK;
@@ -526,6 +530,7 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
   lat = &padded;
   rc = make_plan(lat, c->plan, why);
   if (rc != HB_OK) { c->sticky = rc; return fail(c, rc, why); }
+  if (c->slab_Lz > 0) c->plan.spins_bytes += kAlign;   // neighbour flags behind the spins (hb_sizes)
   if (!e || !unit_vector(e) || !std::isfinite(J) || !std::isfinite(K)) {
     c->sticky = HB_EINVAL;
     return fail(c, HB_EINVAL, "J, K must be finite and e a unit vector");
@@ -660,6 +665,7 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
     c->own_spins = c->own_ws = true;
   }
   HB_CUDA(c, cudaMemsetAsync(c->ws + P.off_counters, 0, kAlign, c->stream));
+  if (c->slab_Lz > 0) HB_CUDA(c, cudaMemsetAsync(c->slab_flags(), 0, kAlign, c->stream));
   if (P.engine == ENGINE_SC || P.engine == ENGINE_BRAVAIS) HB_CUDA(c, cudaMemsetAsync(c->ws + P.off_wsdone, 0, (size_t)kWsDoneWords * sizeof(uint32_t), c->stream));
 
   if (P.engine == ENGINE_CSR) {
@@ -1087,6 +1093,7 @@ int hb_slab_pass(hb_ctx* c, float T, int32_t colour) {
   int rc = check_T(c, T, &beta);
   if (rc != HB_OK) return rc;
   c->cache_valid = false;
+  if (c->sc.flag_in) c->sc.stamp = ++c->slab_stamp;   // neighbour flags: this is the slab's pass number `stamp`
   rc = one_colour(c, 1 - colour, params(c, beta), Diag{nullptr, nullptr});
   if (rc != HB_OK) return rc;
   c->attempts += (uint64_t)c->sc.Lx * c->sc.Ly * (uint64_t)(c->sc.Lz - 2) / 2;
@@ -1125,6 +1132,10 @@ int hb_slab_set_peer(hb_ctx* c, int32_t side, void* peer_spins, int32_t peer_Lz)
   c->sc.peer_half[side] = c->sc.peer_n[side] / 2;
   // my low face is the lower neighbour's high ghost plane (its local plane peer_Lz + 1); my high face the upper one's plane 0
   c->sc.peer_zoff[side] = (peer_spins && side == 0) ? (uint32_t)(peer_Lz + 1) * plane : 0u;
+  // the neighbour's flag words sit behind its spins: my low side is its upper neighbour (its word 1), my high side its lower (word 0)
+  c->sc.flag_out[side] = peer_spins ? reinterpret_cast<uint32_t*>(static_cast<float*>(peer_spins) + 3 * (size_t)c->sc.peer_n[side]) + (side == 0 ? 1 : 0)
+                                    : nullptr;
+  if (!peer_spins) c->sc.flag_in = nullptr;   // flags need peer stores on both sides
   return HB_OK;
 }
 
@@ -1236,6 +1247,15 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
     c->g_dirty[0] = c->g_dirty[1] = true;   // captured launches carry the attribute
     return HB_OK;
   }
+  if (s == "slab_flags") {
+    if (value != 0 && value != 1) return fail(c, HB_EINVAL, "slab_flags: 0 or 1");
+    if (value == 1 && (c->slab_Lz <= 0 || !c->sc.peer[0] || !c->sc.peer[1] || !sc_ws_supported(c->sc)))
+      return fail(c, HB_EINVAL, "slab_flags: a slab context with hb_slab_set_peer on both sides and rows the warp-specialised kernel takes (Lx % 8 == 0, Lx <= 512)");
+    c->sc.flag_in = value ? c->slab_flags() : nullptr;
+    c->sc.bnd_count = value ? c->slab_bnd_count() : nullptr;
+    if (value && c->sc_kernel == 0) c->sc_kernel = 1;   // the flag protocol is part of the warp-specialised kernel
+    return HB_OK;
+  }
   if (s == "br_kernel" || s == "br_zt") {
     if (c->plan.engine != ENGINE_BRAVAIS) return fail(c, HB_EINVAL, "option valid for bcc / fcc lattices only");
     if (s == "br_kernel") {
@@ -1272,6 +1292,7 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
         !(value == 2 && sc_ws_fused_supported(c->sc, c->ws_variant) && 2 * c->fused_sweeps * sc_ws_fused_chunks(c->sc, c->fused_zt) <= kWsDoneWords))
       return fail(c, HB_EINVAL, "sc_kernel: 0 (direct), 1 (warp-specialised; needs Lx % 8 == 0 and Lx <= 512) or 2 (the same with all colour "
                                 "passes of several sweeps in one launch; whole lattices, sc_ws_variant 2, 4 or 5)");
+    if (value == 0 && c->sc.flag_in) return fail(c, HB_EINVAL, "sc_kernel: the neighbour flags of this slab (slab_flags) need the warp-specialised kernel");
     c->sc_kernel = (int)value;
     return HB_OK;
   }
@@ -1351,6 +1372,7 @@ int hb_get_option(hb_ctx* c, const char* name, int64_t* value) {
   else if (s == "sc_fused_sweeps") *value = c->fused_sweeps;
   else if (s == "sc_fused_lag") *value = c->fused_lag;
   else if (s == "sc_fused_zt") *value = c->fused_zt;
+  else if (s == "slab_flags") *value = c->sc.flag_in ? 1 : 0;
   else if (s == "br_kernel") *value = c->br_kernel;
   else if (s == "br_zt") *value = c->br_zt;
   else return HB_EINVAL;

@@ -51,6 +51,17 @@ struct ScLayout {
   // of its ghost plane; side 0 = my low face -> the lower neighbour's high ghost plane, 1 = the other way
   float* peer[2];
   uint32_t peer_n[2], peer_half[2], peer_zoff[2];
+  // Neighbour flags instead of a barrier between two colour passes (hb_set_option "slab_flags", warp-specialised kernel, peer
+  // stores on both sides).  Pass number `stamp` (1, 2, ...) of a slab takes its two boundary chunks
+  // first; a boundary tile waits until the neighbour on that side has finished ITS boundary chunk of pass stamp - 1
+  // (flag_in[side] >= stamp - 1: the ghost plane it reads is complete, and the neighbour no longer reads the ghost plane
+  // this pass stores into); the warp that finishes the last tile of a boundary chunk writes `stamp` into the neighbour's
+  // flag (flag_out[side], peer memory, release at system scope).  flag_in: two words behind this slab's spins;
+  // bnd_count: two words of its workspace; nullptr = off.
+  uint32_t* flag_in;
+  uint32_t* flag_out[2];
+  uint32_t* bnd_count;
+  uint32_t stamp;
 };
 
 // launch shape of the sc kernels: a block is JX x TY threads, each thread owns V

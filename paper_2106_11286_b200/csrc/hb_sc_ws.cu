@@ -49,6 +49,20 @@ __host__ __device__ constexpr int ws_max_threads() {
 template <int TY, int MINB>
 __host__ __device__ constexpr bool ws_pref() { return MINB < 3 && TY != 7; }
 
+// slab with neighbour flags: the two boundary chunks (the first and the last in z) are handed out first
+__device__ __forceinline__ int32_t ws_chunk_in_order(int32_t q, int32_t n_zc, bool boundary_first) {
+  if (!boundary_first || n_zc < 3) return q;
+  return q == 0 ? 0 : (q == 1 ? n_zc - 1 : q - 1);
+}
+__device__ __forceinline__ uint32_t ld_acquire_sys(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release_sys(uint32_t* p, uint32_t v) {
+  asm volatile("st.release.sys.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
 // kNB plane slots of the other colour (z-1, z, z+1 and look-ahead); MINB = CTAs per SM the kernel is built for
 template <int TY, int ROWB, int kNB, int MINB>
 struct WsSmem {
@@ -86,7 +100,16 @@ __device__ __forceinline__ void ws_producer(const float* b, const ScLayout& L, c
       if (lane == 0) { info[rp.slot].x = -1; mbar_arrive(fullB + 8u * rp.slot); }
       break;
     }
-    int32_t ty = tile % w.n_ty, zc = tile / w.n_ty, pass = 0;
+    int32_t ty = tile % w.n_ty, zc = ws_chunk_in_order(tile / w.n_ty, w.n_zc, L.flag_in != nullptr), pass = 0;
+    if (!FUSED && L.flag_in) {   // a boundary tile of a slab: the neighbour on that side must be through its boundary chunk of the pass before
+      const bool lo = zc == 0, hi = zc == w.n_zc - 1;
+      if (lo || hi) {
+        if (lane == 0 && lo) while ((int32_t)(ld_acquire_sys(L.flag_in) - (L.stamp - 1u)) < 0) __nanosleep(200);
+        if (lane == 1 && hi) while ((int32_t)(ld_acquire_sys(L.flag_in + 1) - (L.stamp - 1u)) < 0) __nanosleep(200);
+        __syncwarp();
+        asm volatile("fence.proxy.async;" ::: "memory");   // the bulk copies below read the ghost plane the neighbour stored
+      }
+    }
     if (FUSED) {
       const FusedTile t = fused_decode(tile, w);
       ty = t.ty; zc = t.zc; pass = t.p;
@@ -176,7 +199,7 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
     mbar_wait(fullB + 8u * rm.slot, rm.par);   // first plane of the next tile, or the producer's "no more tiles"
     const int32_t tile = info[rm.slot].x;
     if (tile < 0) { if (FUSED && pending) publish(); break; }
-    int32_t ty = tile % w.n_ty, zc = tile / w.n_ty;
+    int32_t ty = tile % w.n_ty, zc = ws_chunk_in_order(tile / w.n_ty, w.n_zc, SLAB && L.flag_in != nullptr);
     if (FUSED) {
       pass = info[rm.slot].y; zc = info[rm.slot].z; ty = info[rm.slot].w;
       colour = pass & 1;
@@ -306,6 +329,25 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
       rm.next();
     }
     rm.next(); rm.next();   // the two extra planes of the tile
+    if (SLAB && L.flag_in) {
+      // a boundary tile is done: the last warp of the last tile of a boundary chunk tells the neighbour on that side
+      const bool lo = zc == 0, hi = zc == w.n_zc - 1;
+      if (lo || hi) {
+        __syncwarp();
+        if (lane0) {
+          __threadfence_system();   // this warp's stores, the ones into the neighbour's ghost plane included
+          const uint32_t all = (uint32_t)w.n_ty * ((blockDim.x >> 5) - 1u);
+#pragma unroll
+          for (int side = 0; side < 2; ++side)
+            if (side == 0 ? lo : hi)
+              if (atomicAdd(L.bnd_count + side, 1u) == all - 1u) {
+                L.bnd_count[side] = 0u;
+                __threadfence_system();
+                st_release_sys(L.flag_out[side], L.stamp);
+              }
+        }
+      }
+    }
     if (FUSED && pass + 1 < w.passes) {
       // this warp's stores of the tile are done: the next pass waits for the chunk's progress word (see publish above)
       int32_t k = zc - pass % w.n_zc;   // position of the chunk in the pass's order (chunk = (k + pass) mod n)
@@ -477,7 +519,8 @@ int sc_ws_blocks(const ScLayout& L, int ZT, int grid_cap, int variant) {
 
 cudaError_t launch_sweep_sc_ws(cudaStream_t st, float* s, ScLayout L, int ZT, int grid_cap, int variant, uint32_t* sched, SweepParams p, int colour, Meas m) {
   const int cap = grid_cap * ws_ctas_per_sm(variant);
-  const int n_zc = sc_ws_chunks(L, ZT, grid_cap, variant);
+  int n_zc = sc_ws_chunks(L, ZT, grid_cap, variant);
+  if (L.flag_in && n_zc > L.Lz / 2) n_zc = L.Lz / 2 > 0 ? L.Lz / 2 : 1;   // neighbour flags: the boundary chunks hold the planes next to the ghosts
   if (variant == 5) return ws_pick<8, 512, 4, 3>(st, s, L, n_zc, cap, sched, p, colour, m);
   if (variant == 4) return ws_pick<7, 1024, 4, 2>(st, s, L, n_zc, cap, sched, p, colour, m);
   if (variant == 3) return ws_pick<16, 1024, 4, 1>(st, s, L, n_zc, cap, sched, p, colour, m);

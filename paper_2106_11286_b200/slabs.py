@@ -72,7 +72,7 @@ def exchange_dist(ctx, colour, rank, world, group=None):
         send_b, recv_b = send, recv
     ops = [dist.P2POp(dist.isend, t, p, group) for t, p in zip(send_b, peers_s)]
     ops += [dist.P2POp(dist.irecv, t, p, group) for t, p in zip(recv_b, peers_r)]
-    if staged:
+    if staged or not send[0].is_cuda:
         for req in dist.batch_isend_irecv(ops):
             req.wait()
     else:
@@ -91,7 +91,7 @@ class LocalSlabs:
     """n_slabs slab contexts of one periodic sc lattice in this process."""
 
     def __init__(self, Lx, Ly, Lz, n_slabs, J=1.0, K=0.0, e=(0.0, 0.0, 1.0), seed=1, device="cuda:0", options=None,
-                 peer_stores=False):
+                 peer_stores=False, flags=False):
         """All slabs live on `device`.  (The library issues every call on the CUDA device that is current, and a process that
         drove contexts on several devices would have to switch it around every call and enable peer access itself: that
         path was never run on a multi-GPU box, so it is not offered -- one process per GPU, `DistSlab`, is.)"""
@@ -112,6 +112,13 @@ class LocalSlabs:
                 down, up = neighbours(r, n_slabs)
                 c.slab_set_peer(0, self.ctxs[down].spins_ptr, self.parts[down][1])
                 c.slab_set_peer(1, self.ctxs[up].spins_ptr, self.parts[up][1])
+        # neighbour flags (include/hb.h, "slab_flags"): the kernels themselves wait for and signal their z-neighbours.  The
+        # contexts of this class share one stream, so a pass finds the flags of the pass before already set: this exercises
+        # the protocol's bookkeeping (stamps, boundary counters, flag addresses), not its concurrency.
+        self.flags = bool(flags) and self.peer_stores
+        if self.flags:
+            for c in self.ctxs:
+                c.set_option("slab_flags", 1)
 
     def _sync(self):
         import torch
@@ -181,7 +188,10 @@ class DistSlab:
     (an all_reduce of one word on the stream under NCCL; a host barrier under gloo)."""
 
     def __init__(self, Lx, Ly, Lz, J=1.0, K=0.0, e=(0.0, 0.0, 1.0), seed=1, device=None, group=None, options=None,
-                 peer_stores=False):
+                 peer_stores=False, flags=False):
+        """flags=True (with peer_stores, one GPU per rank): no barrier between two colour passes; the kernels wait for and
+        signal their two z-neighbours through flag words in peer memory (include/hb.h, "slab_flags"), boundary tiles first,
+        so that interior tiles hide the wait.  Never with several ranks on ONE GPU: their kernels would wait on one another."""
         import torch
         import torch.distributed as dist
         from .binding import Context, Lattice
@@ -200,6 +210,7 @@ class DistSlab:
             self.ctx.set_option(k, v)
         self.n = Lx * Ly * Lz
         self._mapped = {}
+        self.flags = False
         if self.peer_stores:
             down, up = neighbours(self.rank, self.world)
             self._nccl = self.world > 1 and dist.get_backend(group) == "nccl"
@@ -222,6 +233,9 @@ class DistSlab:
             if ok:
                 self.ctx.slab_set_peer(0, ptrs[down], parts[down][1])
                 self.ctx.slab_set_peer(1, ptrs[up], parts[up][1])
+                if flags:
+                    self.ctx.set_option("slab_flags", 1)
+                    self.flags = True
             else:
                 import warnings
                 warnings.warn("DistSlab: a neighbour's spins buffer could not be mapped; faces are sent after every pass instead")
@@ -263,7 +277,9 @@ class DistSlab:
         for _ in range(n_sweeps):
             for colour in (0, 1):
                 self.ctx.slab_pass(T, colour)
-                if self.peer_stores:
+                if self.peer_stores and self.flags:
+                    pass                         # the next pass's boundary tiles wait for the neighbours' flags on the device
+                elif self.peer_stores:
                     self._pass_barrier()
                 else:
                     exchange_dist(self.ctx, colour, self.rank, self.world, self.group)

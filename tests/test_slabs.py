@@ -119,6 +119,40 @@ def test_peer_stores_replace_the_exchange_step(shape, n_slabs, options):
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("shape,n_slabs,options", [
+    ((40, 14, 24), 3, {"sc_kernel": 1}), ((464, 8, 8), 2, {}), ((64, 20, 12), 2, {"sc_kernel": 1, "sc_ws_variant": 2}),
+    ((64, 16, 40), 1, {"sc_ws_variant": 4}), ((64, 16, 44), 4, {"sc_ws_variant": 5, "sc_ws_zt": 3}),
+])
+def test_neighbour_flags_replace_the_barrier(shape, n_slabs, options):
+    # hb_set_option("slab_flags", 1): boundary chunks first, a boundary tile waits for its neighbour's flag of the pass before,
+    # the last warp of a boundary chunk sets the neighbour's flag.  On one stream every flag is already set when it is waited
+    # for: the test covers the bookkeeping (stamps, counters, flag words behind the spins, chunk order), bit for bit against
+    # the oracle, and that every slab has published every pass.
+    import torch
+    from hbtest import spins_equal
+    K, e, seed = 0.05, (0.0, 0.6, 0.8), 99
+    lat, st = _oracle(shape, K, e, seed)
+    sl = slabs.LocalSlabs(*shape, n_slabs, J=1.0, K=K, e=e, seed=seed, options=options, peer_stores=True, flags=True)
+    assert all(c.get_option("slab_flags") == 1 and c.get_option("sc_kernel") == 1 for c in sl.ctxs)
+    st.init_random()
+    sl.init_random()
+    passes = 0
+    for T, k in ((1.44, 1), (1.44, 4), (0.3, 2)):
+        sl.sweep(T, k)
+        st.sweep(T, k)
+        passes += 2 * k
+        assert spins_equal(sl.get_spins(), st.get_spins()), (shape, n_slabs, T)
+        for c, (z0, nz) in zip(sl.ctxs, sl.parts):      # both flag words of every slab (behind its spins) carry the number of the last pass
+            at = 12 * shape[0] * shape[1] * (nz + 2)
+            words = c._spins[at:at + 8].view(torch.int32).cpu().numpy()
+            assert list(words) == [passes, passes], (words, passes)
+    Mg, Eg = sl.measure()
+    Mo, Eo = st.measure()[:2]
+    assert np.max(np.abs(Mg - np.asarray(Mo))) <= 1e-7 and abs(Eg - Eo) <= 1e-6 * lat.n
+    sl.close()
+
+
+@pytest.mark.gpu
 def test_slab_contexts_refuse_whole_lattice_calls():
     import paper_2106_11286_b200 as hb
     ctx = hb.Context(hb.Lattice("sc", 8, 4, 4, slab=(4, 12)), 1.0, 0.0, (0, 0, 1), 1)
