@@ -463,6 +463,28 @@ def main():
                                       "4 attempts per thread as two packed pairs, 256-thread blocks, 4 per SM, measured in this run",
                        "pipe_rates": pipe_rates, "pipe_rates_unit": "warp-instructions per clock per SM (hb_probe_pipe, this run)"}
 
+    # NEXT-1 beside the default: the same workload through the one-launch-per-colour kernel and through the fused
+    # launches (all colour passes of 8 sweeps per launch), interleaved short runs after the timed region, and the rate of the
+    # colour kernel with its HBM traffic folded into L2 (hb_probe_sc_l2: the ceiling of any scheme that only removes traffic)
+    kernels = None
+    if cfg["kind"] == "sc" and ctx.get_option("sc_kernel") >= 1 and "sc_kernel" not in options:
+        def rate(kernel, sweeps=40):
+            ctx.set_option("sc_kernel", kernel)
+            ctx.sweep(T, 8)
+            a, b = ev(), ev()
+            a.record(); ctx.sweep(T, sweeps); b.record(); torch.cuda.synchronize()
+            return float(n) * sweeps / (a.elapsed_time(b) * 1e-3) / 1e9
+        try:
+            default_kernel = ctx.get_option("sc_kernel")
+            pairs = [(rate(1), rate(2)) for _ in range(3)]
+            ctx.set_option("sc_kernel", default_kernel)
+            kernels = {"unit": UNIT, "one_launch_per_colour (sc_kernel=1)": max(p[0] for p in pairs),
+                       "fused_launches (sc_kernel=2, 8 sweeps per launch)": max(p[1] for p in pairs),
+                       "note": "3 interleaved runs of 40 sweeps each, best of each; profiles/r02_c4_fused_full.md has the ncu comparison"}
+            kernels["hbm_traffic_folded_into_l2 (hb_probe_sc_l2)"] = ctx.probe_sc_l2(T, 40, 16) / 1e9   # leaves the state undefined: last
+        except Exception as exc:          # the fused launches need a row length the kernel takes
+            kernels = {"unavailable": str(exc)}
+
     cpu = None if args.no_cpu_baseline else run_cpu_baseline(cfg)
     # acceptance rate of the timed sweeps themselves (reported with every timed config): hb_stats counts the
     # accepted moves inside the measuring passes, i.e. in the last sweep of every timed step
@@ -483,6 +505,8 @@ def main():
         "ns_per_update": 1.0 / value, "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
         "roofline": roofline, "cpu_baseline": cpu,
     }
+    if kernels is not None:
+        line["sc_kernels"] = kernels
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
