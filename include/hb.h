@@ -231,6 +231,15 @@ int hb_probe_alu(void* cuda_stream, double seconds, double* updates_per_second);
 enum { HB_MATH_U01 = 0, HB_MATH_SINCOS = 1, HB_MATH_SPHERE = 2, HB_MATH_EXP = 3, HB_MATH_SQRT = 4, HB_MATH_ATTEMPT = 5 };
 int hb_device_math(int32_t op, int64_t count, const uint32_t* in0, const uint32_t* in1, float* out);
 
+/* Context, not the product path: n_mcs Monte Carlo steps per spin of the PAPER'S OWN update scheme (PAPER.md
+ * lines 30-32), emulated: the linearised array is cut into N / n_per_block "blocks" of n_per_block consecutive sites, at
+ * every step every block updates ONE randomly chosen spin of its own against whatever its neighbours hold in global memory
+ * at that moment (other blocks update theirs concurrently: racy by construction, "loss of continuity" for small n), one
+ * launch per step, n_per_block steps per MCS.  The paper's choice is n_per_block = 8.  Not reproducible bit for bit and
+ * never compared with the trajectory oracle: only its statistics (against the fp64 random-site oracle) and its rate mean
+ * anything.  Simple cubic, whole lattice.  The sweep counter advances by n_mcs; hb_stats counts every attempt.  Asynchronous. */
+int hb_sweep_paper_scheme(hb_ctx* ctx, float T, int64_t n_mcs, int32_t n_per_block);
+
 /* Diagnostic: the issue rate of one instruction kind (or mix) the colour kernels are made of, in warp-instructions per clock
  * per SM (4.0 = one per clock on each of the four sub-partitions), measured with the SM clock over a loop of 8 independent
  * register chains per thread, 32 warps per SM.  It is the measurement behind the arithmetic ceiling of DESIGN.md section 7

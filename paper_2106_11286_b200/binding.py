@@ -18,7 +18,7 @@ EXPORTS = [
     "hb_sweep_each", "hb_measure_each", "hb_sweep_series_each", "hb_select_replica",
     "hb_slab_pass", "hb_slab_next_sweep", "hb_slab_face", "hb_slab_set_peer", "hb_probe_alu",
     "hb_device_alloc", "hb_device_free", "hb_ipc_export", "hb_ipc_open", "hb_ipc_close",
-    "hb_get_colouring", "hb_counters", "hb_stats", "hb_device_math", "hb_probe_sc_l2", "hb_probe_pipe", "hb_set_option", "hb_get_option", "hb_lattice_fcc_sphere", "hb_lattice_free",
+    "hb_get_colouring", "hb_counters", "hb_stats", "hb_device_math", "hb_probe_sc_l2", "hb_probe_pipe", "hb_sweep_paper_scheme", "hb_set_option", "hb_get_option", "hb_lattice_fcc_sphere", "hb_lattice_free",
     "hb_strerror", "hb_error_detail",
 ]
 
@@ -93,6 +93,7 @@ def load_library():
         "hb_device_math": [i32, i64, vp, vp, vp],
         "hb_probe_sc_l2": [vp, f32, i64, i32, P(C.c_double)],
         "hb_probe_pipe": [vp, i32, P(C.c_double)],
+        "hb_sweep_paper_scheme": [vp, f32, i64, i32],
         "hb_set_option": [vp, C.c_char_p, i64],
         "hb_get_option": [vp, C.c_char_p, P(i64)],
         "hb_lattice_fcc_sphere": [i32, f32, P(f32), f32, i32, P(hb_lattice), P(vp)],
@@ -430,6 +431,10 @@ class Context:
         a, b = C.c_uint64(), C.c_uint64()
         self._check(self._L.hb_stats(self._h, C.byref(a), C.byref(b)), "hb_stats")
         return a.value, b.value
+
+    def sweep_paper_scheme(self, T, n_mcs=1, n_per_block=8):
+        """hb_sweep_paper_scheme: the paper's own racy block scheme, emulated (context only; include/hb.h)."""
+        self._check(self._L.hb_sweep_paper_scheme(self._h, T, int(n_mcs), int(n_per_block)), "hb_sweep_paper_scheme")
 
     def probe_sc_l2(self, T, n_sweeps=50, planes=16):
         """hb_probe_sc_l2: updates per second of the sc colour kernel with its HBM traffic folded into L2 (destroys the state)."""

@@ -1175,6 +1175,30 @@ int hb_counters(hb_ctx* c, uint64_t* kernel_launches, uint64_t* attempts) {
   return HB_OK;
 }
 
+int hb_sweep_paper_scheme(hb_ctx* c, float T, int64_t n_mcs, int32_t n_per_block) {
+  HB_CHECK_CTX(c);
+  if (c->plan.engine != ENGINE_SC || c->slab_Lz > 0 || c->plan.R > 1) return fail(c, HB_EINVAL, "hb_sweep_paper_scheme: a whole simple cubic lattice without replicas");
+  if (n_mcs < 0 || n_per_block < 1 || n_per_block > 65536 || c->plan.n % n_per_block) return fail(c, HB_EINVAL, "hb_sweep_paper_scheme: n_mcs >= 0, 1 <= n_per_block <= 65536 dividing the number of sites");
+  if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
+  float beta;
+  const int rc = check_T(c, T, &beta);
+  if (rc != HB_OK) return rc;
+  if (n_mcs > 0) c->cache_valid = false;
+  SweepParams p = params(c, beta);
+  for (int64_t s = 0; s < n_mcs; ++s) {
+    for (int32_t k = 0; k < n_per_block; ++k) {   // one MCS = N attempts = n_per_block steps of N / n_per_block attempts
+      const uint64_t step = c->sweep * 65536ull + (uint64_t)k;
+      p.sweep_lo = (uint32_t)step; p.sweep_hi = (uint32_t)(step >> 32);
+      HB_CUDA(c, launch_paper_step(c->stream, c->spins, c->sc, p, (uint32_t)n_per_block, c->counters()));
+    }
+    c->launches += (uint64_t)n_per_block;
+    c->sweep += 1;
+    c->attempts += (uint64_t)c->plan.n;
+    c->stat_attempts += (uint64_t)c->plan.n;
+  }
+  return HB_OK;
+}
+
 int hb_probe_sc_l2(hb_ctx* c, float T, int64_t n_sweeps, int32_t planes, double* updates_per_second) {
   HB_CHECK_CTX(c);
   if (!updates_per_second || n_sweeps < 1 || n_sweeps > 100000) return fail(c, HB_EINVAL, "hb_probe_sc_l2: 1 <= n_sweeps <= 100000, non-NULL output");

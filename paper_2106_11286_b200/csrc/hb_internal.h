@@ -126,6 +126,8 @@ cudaError_t launch_init_random_sc(cudaStream_t st, float* spins, ScLayout L, uin
 cudaError_t launch_init_random_flat(cudaStream_t st, float* spins, uint32_t n, uint32_t seed_lo, uint32_t seed_hi);
 cudaError_t launch_fill(cudaStream_t st, float* spins, uint32_t n, float x, float y, float z);
 cudaError_t launch_sc_permute(cudaStream_t st, float* dst, const float* src, ScLayout L, bool to_internal);
+// one step of the paper's own scheme, emulated (hb_sweep_paper_scheme): p.sweep_lo/hi = the step number
+cudaError_t launch_paper_step(cudaStream_t st, float* spins, ScLayout L, SweepParams p, uint32_t n_per_block, unsigned long long* n_accept);
 cudaError_t launch_sweep_sc(cudaStream_t st, float* spins, ScLayout L, ScTile t, SweepParams p, int colour, Diag d, Meas m);
 // blocks one launch_sweep_sc launch uses with this tile if it can carry the fused measurement, else 0
 int sc_fused_blocks(const ScLayout& L, const ScTile& t);

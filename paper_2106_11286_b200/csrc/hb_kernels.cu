@@ -286,6 +286,49 @@ k_sweep_csr(float* sx, float* sy, float* sz, CsrDev g, uint32_t list_begin, uint
   }
 }
 
+// ---- the paper's own update scheme, emulated (context for BASELINE.md, not the product path) -----------------
+// [P:30-32]: "each GPU block handles a part of that array ... N_b blocks are called to perform a spin update in parallel.
+// Each block handles n spins, and within each block one of those spins is selected at random to be updated at every step",
+// the spins being read from and written to global memory while other blocks update theirs: with small n a spin's
+// neighbours change under the energy calculation ("loss of continuity").  Here one THREAD plays one of the paper's
+// blocks: it owns the n consecutive sites [t n, (t+1) n) of the linearised (canonical) array, draws one of them, runs rule
+// (ii)-(iii) on it against whatever its neighbours hold at that moment, and stores the result.  One launch = one step =
+// N / n attempts; one MCS = n steps.  Racy by construction and not reproducible bit for bit: only its statistics and its
+// rate are meaningful.  Random numbers: Philox(counter = (t, 2, step), key = seed) picks the site, (site, 3, step) feeds the attempt.
+template <int ANISO>
+__global__ void __launch_bounds__(256)
+k_paper_step(float* s, ScLayout L, SweepParams P, uint32_t n_per_block, uint32_t n_blocks, unsigned long long* n_accept) {
+  const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
+  bool acc = false;
+  if (t < n_blocks) {
+    const Rand4 pick = philox4x32_10(t, 2u, P.sweep_lo, P.sweep_hi, P.seed_lo, P.seed_hi);
+    const uint32_t id = t * n_per_block + pick.r0 % n_per_block;
+    const uint32_t Lx = (uint32_t)L.Lx, Ly = (uint32_t)L.Ly, Lz = (uint32_t)L.Lz, H = (uint32_t)L.H;
+    const uint32_t x = id % Lx, yz = id / Lx, y = yz % Ly, z = yz / Ly;
+    const uint32_t c = (x + y + z) & 1u;
+    auto at = [&](uint32_t xx, uint32_t yy, uint32_t zz, uint32_t cc) { return cc * L.half + (zz * Ly + yy) * H + (xx >> 1); };
+    const uint32_t m = at(x, y, z, c), o = 1u - c;
+    const uint32_t nb[6] = {at(x ? x - 1 : Lx - 1, y, z, o), at(x + 1 < Lx ? x + 1 : 0, y, z, o), at(x, y ? y - 1 : Ly - 1, z, o),
+                            at(x, y + 1 < Ly ? y + 1 : 0, z, o), at(x, y, z ? z - 1 : Lz - 1, o), at(x, y, z + 1 < Lz ? z + 1 : 0, o)};
+    const size_t n = L.n;
+    const volatile float* v = s;       // whatever the other "blocks" have stored by now
+    float hx = 0.0f, hy = 0.0f, hz = 0.0f;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) { hx = __fadd_rn(hx, v[nb[k]]); hy = __fadd_rn(hy, v[n + nb[k]]); hz = __fadd_rn(hz, v[2 * n + nb[k]]); }
+    float sx = v[m], sy = v[n + m], sz = v[2 * n + m];
+    const Rand4 r = philox4x32_10(id, 3u, P.sweep_lo, P.sweep_hi, P.seed_lo, P.seed_hi);
+    float nx, ny, nz;
+    sphere(r.r0, r.r1, nx, ny, nz);
+    const float dH = delta_h_t<ANISO>(sx, sy, sz, nx, ny, nz, hx, hy, hz, P.J, P.K, P.ex, P.ey, P.ez);
+    acc = metropolis_accept(dH, P.beta, r.r2);
+    if (acc) { s[m] = nx; s[n + m] = ny; s[2 * n + m] = nz; }
+  }
+  if (n_accept) {
+    const unsigned votes = __ballot_sync(0xffffffffu, acc);
+    if (votes && (threadIdx.x & 31) == 0) atomicAdd(n_accept, (unsigned long long)__popc(votes));
+  }
+}
+
 // ---- initial states -----------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t sc_canonical(const ScLayout& L, uint32_t m) {
   // internal index m = c*half + (z*Ly + y)*H + i  ->  canonical id (z*Ly + y)*Lx + 2i + ((c+y+z)&1)
@@ -514,6 +557,19 @@ cudaError_t launch_init_random_flat(cudaStream_t st, float* s, uint32_t n, uint3
 
 cudaError_t launch_fill(cudaStream_t st, float* s, uint32_t n, float x, float y, float z) {
   k_fill<<<grid_for(n, 256, 148 * 16), 256, 0, st>>>(s, s + n, s + 2 * (size_t)n, n, x, y, z);
+  return cudaGetLastError();
+}
+
+inline int aniso_case(const SweepParams& p);
+
+cudaError_t launch_paper_step(cudaStream_t st, float* s, ScLayout L, SweepParams p, uint32_t n_per_block, unsigned long long* n_accept) {
+  const uint32_t n_blocks = L.n / n_per_block;
+  const unsigned grid = (n_blocks + 255u) / 256u;
+  switch (aniso_case(p)) {
+    case ANISO_NONE: k_paper_step<ANISO_NONE><<<grid, 256, 0, st>>>(s, L, p, n_per_block, n_blocks, n_accept); break;
+    case ANISO_Z: k_paper_step<ANISO_Z><<<grid, 256, 0, st>>>(s, L, p, n_per_block, n_blocks, n_accept); break;
+    default: k_paper_step<ANISO_GENERAL><<<grid, 256, 0, st>>>(s, L, p, n_per_block, n_blocks, n_accept); break;
+  }
   return cudaGetLastError();
 }
 

@@ -121,7 +121,7 @@ def throughput_vs_size(sizes, T=1.30, K=0.01, seconds=0.5):
 
 def main(argv):
     """python -m paper_2106_11286_b200.scan c2 | --sc L [--K k] [--T a:b:n] [--equil e] [--sweeps s] [--fit t_lo:t_hi]
-    [--out file] [--windows [--Tc 1.443,1.445]] | --analyse file [Tc ...] | --fig2 [L ...]"""
+    [--out file] [--windows [--Tc 1.443,1.445]] | --analyse file [Tc ...] | --fig2 [L ...] | --paper-scheme [L ...]"""
     if len(argv) > 1 and argv[1] == "--fig2":
         sizes = [int(x) for x in argv[2:]] or [16, 32, 64, 128, 256, 464, 512, 1024]
         print("# sc L^3, J = 1, K = 0.01, T = 1.30 (0.9 T_C), random start: attempted updates per second, time per update")
@@ -129,6 +129,23 @@ def main(argv):
         print("# L  N  sweeps  Gupd/s  ns/update")
         for r in throughput_vs_size(sizes):
             print("%d  %d  %d  %.2f  %.5f" % r)
+        return
+    if len(argv) > 1 and argv[1] == "--paper-scheme":
+        # the paper's own block scheme, emulated (hb_sweep_paper_scheme), at the parameters of its Figs. 1-2: rate against L and n
+        import torch
+        sizes = [int(x) for x in argv[2:]] or [128, 256, 464]
+        print("# the paper's scheme (N/n blocks of n spins, one random spin per block and step [P:30-32]) emulated on this device;")
+        print("# sc L^3, J = 1, K = 0.01, T = 1.30; the paper: 0.61-0.63 Gupd/s on a V100 with n = 8 [P:42-44]")
+        print("# L  n  Gupd/s")
+        for L in sizes:
+            ctx = make_context(dict(kind="sc", L=L, J=1.0, K=0.01, e=(0.0, 0.0, 1.0), seed=1, start="random"))
+            ctx.sweep(1.30, 20)
+            for n in (4, 8, 16, 64):
+                ctx.sweep_paper_scheme(1.30, 2, n)
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(); ctx.sweep_paper_scheme(1.30, 10, n); b.record(); torch.cuda.synchronize()
+                print("%d  %d  %.2f" % (L, n, ctx.n * 10 / (a.elapsed_time(b) * 1e-3) / 1e9))
+            ctx.close()
         return
     if len(argv) > 1 and argv[1] == "--sc":
         import argparse

@@ -895,3 +895,51 @@ def test_scan_statistics_over_the_full_temperature_lists(name):
     assert int(np.sum(np.abs(z) > 3.0)) <= 2, z
     m = g[:, :, 0].mean(axis=0)                                # the transition lies inside the window: ordered at one end, not at the other
     assert max(m[0], m[-1]) > 1.5 * min(m[0], m[-1])
+
+
+def test_paper_scheme_emulation_statistics():
+    # the paper's own block scheme [P:30-32] (N / n blocks of n spins, one random spin per block and step, racy),
+    # emulated by hb_sweep_paper_scheme.  It has no trajectory to compare; its statistics are compared with the fp64 random-site
+    # oracle (the same steps (i)-(iii) of [P:20], sequentially).  With the paper's n = 8 the two agree to a few 1e-3 on a 16^3
+    # lattice below T_C; n = 1 (every spin updated at once against its neighbours' old values) is the limit in which the
+    # "loss of continuity" [P:32] is complete.  Counters: N attempts per MCS, all of them counted by hb_stats.
+    cfg = W.CONFIGS["c1"]
+    lat, _ = make_oracle(cfg)
+    T, equil, meas, reps = 1.2, 300, 400, 12
+    def gpu(n_per_block):
+        m_all, e_all = [], []
+        for r in range(reps):
+            ctx = make_gpu(dict(cfg, seed=500 + r))
+            ctx.init_random()
+            ctx.sweep_paper_scheme(T, equil, n_per_block)
+            ms, es = [], []
+            for _ in range(meas):
+                ctx.sweep_paper_scheme(T, 1, n_per_block)
+                M, E = ctx.measure()
+                ms.append(np.linalg.norm(M)); es.append(E / lat.n)
+            m_all.append(np.mean(ms)); e_all.append(np.mean(es))
+            if r == 0:
+                att, acc = ctx.stats()
+                assert att == (equil + meas) * lat.n and 0 < acc < att
+                assert ctx.sweep_count == equil + meas
+            ctx.close()
+        return np.array(m_all), np.array(e_all)
+    o_m, o_e = [], []
+    for r in range(reps):
+        st = oracle.State64(lat, cfg["J"], 700 + r)
+        st.init_random()
+        st.sweep(T, equil)
+        m, e, _ = st.series(T, meas)
+        o_m.append(m.mean()); o_e.append(e.mean() / lat.n)
+    o_m, o_e = np.array(o_m), np.array(o_e)
+    for n_per_block in (8, 64, 1):
+        g_m, g_e = gpu(n_per_block)
+        dm, de = g_m.mean() - o_m.mean(), g_e.mean() - o_e.mean()
+        se_m = math.sqrt(g_m.var(ddof=1) / reps + o_m.var(ddof=1) / reps)
+        se_e = math.sqrt(g_e.var(ddof=1) / reps + o_e.var(ddof=1) / reps)
+        print("paper scheme n = %d: |M| %.5f (o64 %.5f, diff %+.1e, se %.1e)  E/N %.5f (o64 %.5f, diff %+.1e, se %.1e)" %
+              (n_per_block, g_m.mean(), o_m.mean(), dm, se_m, g_e.mean(), o_e.mean(), de, se_e))
+        if n_per_block >= 8:
+            assert abs(dm) <= 0.01 and abs(de) <= 0.01, (n_per_block, dm, de)
+    with pytest.raises(hb.HbError):
+        hb.Context(hb.Lattice("sc", 6)).sweep_paper_scheme(1.0, 1, 8)     # before init; and 216 sites are not a multiple of 8
