@@ -114,6 +114,14 @@ int hb_init_random(hb_ctx* ctx);
 int hb_init_aligned(hb_ctx* ctx, const float dir[3]);
 int hb_set_spins(hb_ctx* ctx, const float* sx, const float* sy, const float* sz);
 int hb_get_spins(hb_ctx* ctx, float* sx, float* sy, float* sz);
+/* The same upload in two halves, so that the copy of the NEXT state overlaps the sweeps of the current one (a run that
+ * feeds a fresh state every step): hb_stage_spins starts the host->device copy of three canonical arrays (pinned host
+ * memory, or the copy is not asynchronous) into a library-owned upload area of 3 n floats on a stream of its own and returns
+ * at once; hb_commit_spins waits for that copy, then makes the staged state the context's state, in stream order with the
+ * sweeps before and after it.  The host arrays must stay untouched until hb_commit_spins has returned.  Whole lattices
+ * without replicas. */
+int hb_stage_spins(hb_ctx* ctx, const float* sx, const float* sy, const float* sz);
+int hb_commit_spins(hb_ctx* ctx);
 
 /* n_sweeps Metropolis sweeps at temperature T (units of J/k_B, T > 0, +inf allowed).
  * One sweep = one attempt at every site, colours in ascending order.  Asynchronous.

@@ -14,6 +14,7 @@ _KINDS = {"sc": HB_SC, "bcc": HB_BCC, "fcc": HB_FCC, "csr": HB_CSR}
 
 EXPORTS = [
     "hb_sizes", "hb_create", "hb_destroy", "hb_init_random", "hb_init_aligned", "hb_set_spins", "hb_get_spins",
+    "hb_stage_spins", "hb_commit_spins",
     "hb_sweep", "hb_measure", "hb_sweep_series", "hb_sweep_record", "hb_sweep_count", "hb_set_sweep_count",
     "hb_sweep_each", "hb_measure_each", "hb_sweep_series_each", "hb_select_replica",
     "hb_slab_pass", "hb_slab_next_sweep", "hb_slab_face", "hb_slab_set_peer", "hb_probe_alu",
@@ -67,6 +68,8 @@ def load_library():
         "hb_init_aligned": [vp, P(f32)],
         "hb_set_spins": [vp, vp, vp, vp],
         "hb_get_spins": [vp, vp, vp, vp],
+        "hb_stage_spins": [vp, vp, vp, vp],
+        "hb_commit_spins": [vp],
         "hb_sweep": [vp, f32, i64],
         "hb_measure": [vp, P(C.c_double), P(C.c_double)],
         "hb_sweep_series": [vp, f32, i64, vp, vp],
@@ -327,6 +330,16 @@ class Context:
         """Host arrays (numpy, or pinned torch CPU tensors) of n floats, canonical order."""
         p = [self._host_ptr(a) for a in (sx, sy, sz)]
         self._check(self._L.hb_set_spins(self._h, p[0][0], p[1][0], p[2][0]), "hb_set_spins")
+
+    def stage_spins(self, sx, sy, sz):
+        """hb_stage_spins: start the upload of the next state (pinned torch CPU tensors) while the stream computes."""
+        p = [self._host_ptr(a) for a in (sx, sy, sz)]
+        self._staged = [q[1] for q in p]          # keep the host arrays alive until the commit
+        self._check(self._L.hb_stage_spins(self._h, p[0][0], p[1][0], p[2][0]), "hb_stage_spins")
+
+    def commit_spins(self):
+        self._check(self._L.hb_commit_spins(self._h), "hb_commit_spins")
+        self._staged = None
 
     def _host_ptr(self, a):
         if isinstance(a, np.ndarray):

@@ -165,6 +165,12 @@ struct hb_ctx {
   int pdl = 1;                 // colour kernels are launched with programmatic stream serialisation (option pdl)
   int32_t slab_Lz = 0, slab_z0 = 0;   // > 0: this context is a slab of a larger lattice (planes 0 and Lz-1 of sc are ghosts)
   uint32_t slab_stamp = 0;            // colour passes of this slab so far (neighbour flags, option slab_flags)
+  // hb_stage_spins / hb_commit_spins: a library-owned upload area of 3 n floats, filled on its own stream while the context's
+  // stream computes (allocated at the first hb_stage_spins, freed by hb_destroy)
+  float* stage = nullptr;
+  cudaStream_t stage_stream = nullptr;
+  cudaEvent_t stage_filled = nullptr, stage_free = nullptr;
+  bool stage_pending = false;
   uint32_t* slab_flags() const { return reinterpret_cast<uint32_t*>(spins_base + 3 * (size_t)plan.n); }   // two words behind the spins
   int sc_coop = -1;            // persistent multi-sweep kernel: -1 auto, 0 off, 1 / 2 forced (see hb_set_option)
   bool fused_measure = true;   // sc: the last sweep of hb_sweep also reduces M and E
@@ -745,6 +751,10 @@ int hb_destroy(hb_ctx* c) {
   if (!c) return HB_OK;
   for (int k = 0; k < 2; ++k) if (c->gexec[k]) cudaGraphExecDestroy(c->gexec[k]);
   if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+  if (c->stage_stream) { cudaStreamSynchronize(c->stage_stream); cudaStreamDestroy(c->stage_stream); }
+  if (c->stage_filled) cudaEventDestroy(c->stage_filled);
+  if (c->stage_free) cudaEventDestroy(c->stage_free);
+  if (c->stage) cudaFree(c->stage);
   if (c->own_spins && c->spins_base) cudaFree(c->spins_base);
   if (c->own_ws && c->ws) cudaFree(c->ws);
   delete c;
@@ -823,6 +833,51 @@ int hb_set_spins(hb_ctx* c, const float* sx, const float* sy, const float* sz) {
     }
   }
   HB_CUDA(c, cudaStreamSynchronize(c->stream));   // the caller may reuse its arrays
+  c->initialised = true;
+  return HB_OK;
+}
+
+// ---- staged upload: the host->device copy of the NEXT state overlaps the sweeps of the current one ---------------------------
+int hb_stage_spins(hb_ctx* c, const float* sx, const float* sy, const float* sz) {
+  HB_CHECK_CTX(c);
+  if (!sx || !sy || !sz) return fail(c, HB_EINVAL, "NULL spin array");
+  if (c->slab_Lz > 0 || c->plan.R > 1) return fail(c, HB_EINVAL, "hb_stage_spins: whole lattices without replicas");
+  const size_t n = (size_t)c->plan.n;
+  if (!c->stage) {
+    if (cudaMalloc(reinterpret_cast<void**>(&c->stage), 3 * n * sizeof(float)) != cudaSuccess) { cudaGetLastError(); return fail(c, HB_ENOMEM, "hb_stage_spins: cudaMalloc of the upload area failed"); }
+    HB_CUDA(c, cudaStreamCreateWithFlags(&c->stage_stream, cudaStreamNonBlocking));
+    HB_CUDA(c, cudaEventCreateWithFlags(&c->stage_filled, cudaEventDisableTiming));
+    HB_CUDA(c, cudaEventCreateWithFlags(&c->stage_free, cudaEventDisableTiming));
+    HB_CUDA(c, cudaEventRecord(c->stage_free, c->stream));
+  }
+  HB_CUDA(c, cudaStreamWaitEvent(c->stage_stream, c->stage_free, 0));   // the last commit has read the area
+  const float* src[3] = {sx, sy, sz};
+  for (int k = 0; k < 3; ++k)
+    HB_CUDA(c, cudaMemcpyAsync(c->stage + k * n, src[k], n * sizeof(float), cudaMemcpyHostToDevice, c->stage_stream));
+  HB_CUDA(c, cudaEventRecord(c->stage_filled, c->stage_stream));
+  c->stage_pending = true;
+  return HB_OK;
+}
+
+int hb_commit_spins(hb_ctx* c) {
+  HB_CHECK_CTX(c);
+  if (!c->stage_pending) return fail(c, HB_ESTATE, "hb_commit_spins without a staged state (hb_stage_spins)");
+  HB_CUDA(c, cudaEventSynchronize(c->stage_filled));                     // the caller may reuse its host arrays after this call
+  c->cache_valid = c->each_valid = false;
+  const size_t n = (size_t)c->plan.n;
+  for (int k = 0; k < 3; ++k) {
+    if (c->plan.engine == ENGINE_SC) {
+      HB_CUDA(c, launch_sc_permute(c->stream, c->spins + k * n, c->stage + k * n, c->sc, true));
+      c->launches += 1;
+    } else if (c->plan.ell) {
+      HB_CUDA(c, launch_permute_ell(c->stream, c->spins, c->stage + k * n, c->ell.perm, (uint32_t)n, k, true));
+      c->launches += 1;
+    } else {
+      HB_CUDA(c, cudaMemcpyAsync(c->spins + k * n, c->stage + k * n, n * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+    }
+  }
+  HB_CUDA(c, cudaEventRecord(c->stage_free, c->stream));
+  c->stage_pending = false;
   c->initialised = true;
   return HB_OK;
 }

@@ -943,3 +943,35 @@ def test_paper_scheme_emulation_statistics():
             assert abs(dm) <= 0.01 and abs(de) <= 0.01, (n_per_block, dm, de)
     with pytest.raises(hb.HbError):
         hb.Context(hb.Lattice("sc", 6)).sweep_paper_scheme(1.0, 1, 8)     # before init; and 216 sites are not a multiple of 8
+
+
+@pytest.mark.parametrize("name", ["sc24_K", "sc16_c1", "bcc8", "sphere5"])
+def test_staged_upload_equals_set_spins(name):
+    # hb_stage_spins / hb_commit_spins: the upload in two halves (the copy overlaps earlier sweeps); the committed state is the
+    # one hb_set_spins would have set, in stream order with the sweeps around it
+    import torch
+    cfg = SMALL_CASES[name]
+    ctx = make_gpu(cfg)
+    lat, st = make_oracle(cfg)
+    start(cfg, ctx, st)
+    st.sweep(1.3, 2)
+    target = st.get_spins()
+    host = [torch.from_numpy(a.copy()).pin_memory() for a in target]
+    with pytest.raises(hb.HbError):
+        ctx.commit_spins()                         # nothing staged
+    ctx.sweep(1.3, 5)                              # work in flight while the copy runs
+    ctx.stage_spins(*host)
+    ctx.sweep(1.3, 3)
+    ctx.commit_spins()
+    assert spins_equal(ctx.get_spins(), target)
+    ctx.sweep_count = st.sweep_count
+    for k in (1, 4):                               # and twice in a row: the second upload waits for the first commit's reads
+        ctx.sweep(1.3, k)
+        st.sweep(1.3, k)
+        assert spins_equal(ctx.get_spins(), st.get_spins())
+        _measure_close(ctx, st, lat.n)
+        host2 = [torch.from_numpy(a.copy()).pin_memory() for a in st.get_spins()]
+        ctx.stage_spins(*host2)
+        ctx.commit_spins()
+        assert spins_equal(ctx.get_spins(), st.get_spins())
+    ctx.close()
