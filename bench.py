@@ -33,7 +33,7 @@ sys.path.insert(0, ROOT)
 # Sweeps of one step: config 4 is specified as "200 timed sweeps" (BASELINE.json), so its step is those 200 sweeps
 # followed by the measurement; the secondary workloads (scans of hundreds to thousands of sweeps per temperature)
 # use 50-100.
-SWEEPS_BY_WORKLOAD = {"c4": 200, "c1": 100, "c2": 100, "c3": 50, "c5": 50}
+SWEEPS_BY_WORKLOAD = {"c4": 200, "c1": 100, "c2": 100, "c3": 50, "c5": 50, "x_bcc256": 50, "x_fcc256": 20}
 SWEEPS_PER_STEP = 10
 METRIC = "attempted spin updates/sec (Gupd/s) and % of HBM roofline, 1 B200"
 UNIT = "Gupd/s"
@@ -452,8 +452,10 @@ def main():
     bytes_per_launch = bytes_per_update * n / n_colours
     achieved = bytes_per_launch / avg_launch_s / 1e9
     kernel = {"sc": "k_sweep_sc", "bcc": "k_sweep_bravais", "fcc": "k_sweep_bravais", "sphere": "k_sweep_ell"}[cfg["kind"]]
-    if cfg["kind"] == "sc" and ctx.get_option("sc_kernel") == 1:
+    if cfg["kind"] == "sc" and ctx.get_option("sc_kernel") >= 1:
         kernel = "k_sweep_sc_ws"
+    if cfg["kind"] in ("bcc", "fcc") and ctx.get_option("br_kernel") >= 1:
+        kernel = "k_sweep_bravais_ws"
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.workload), "kernel": kernel, "peak_source": peak_src,
                 "algorithmic_bytes_per_update": bytes_per_update, "bytes_per_launch": bytes_per_launch,

@@ -20,6 +20,12 @@ namespace hb {
 namespace {
 
 // what a thread knows about its V cells in row (y,z): element offsets inside one sublattice array
+// resident 256-thread blocks per SM the plain pass is compiled for: fcc runs 5 % faster with four (64 registers, 16-24 bytes of
+// spills: its 36 neighbour loads per thread and plane want warps more than registers: c3 80.0 -> 84.3 Gupd/s), bcc 3 % slower
+#ifndef HB_FCC_MINBLOCKS
+#define HB_FCC_MINBLOCKS 4
+#endif
+template <int KIND> __host__ __device__ constexpr int br_min_blocks() { return KIND == BR_FCC ? HB_FCC_MINBLOCKS : 3; }
 struct Where {
   uint32_t yo[3];   // (y-1, y, y+1 periodic) * Lx
   uint32_t zo[3];   // (z-1, z, z+1 periodic) * Ly * Lx
@@ -111,7 +117,7 @@ __device__ __forceinline__ void where_z(Where& w, const BrLayout& L, int32_t z) 
 }
 
 template <int KIND, int B, int V, int ANISO, bool DIAG, bool MEAS = false>
-__global__ void __launch_bounds__(256, (MEAS && n_low<KIND, B>() != 0 && n_low<KIND, B>() != Geo<KIND>::Z) ? 1 : (MEAS ? 2 : 3))
+__global__ void __launch_bounds__(256, (MEAS && n_low<KIND, B>() != 0 && n_low<KIND, B>() != Geo<KIND>::Z) ? 1 : (MEAS ? 2 : br_min_blocks<KIND>()))
 k_sweep_bravais(float* __restrict__ own, const float* __restrict__ all, BrLayout L, ScTile t, SweepParams P, Diag d, Meas m) {
   resolve_sweep(P);
   const int32_t tj = threadIdx.x % t.JX, ty = threadIdx.x / t.JX;
