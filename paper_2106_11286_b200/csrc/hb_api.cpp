@@ -810,18 +810,14 @@ int hb_set_spins(hb_ctx* c, const float* sx, const float* sy, const float* sz) {
   if (!sx || !sy || !sz) return fail(c, HB_EINVAL, "NULL spin array");
   c->each_valid = false;
   const size_t n = (size_t)c->plan.n;
-  std::vector<float> padded;   // slab: the caller's Lx Ly Lz sites sit between two ghost planes (zero until exchanged)
-  if (c->slab_Lz > 0) {
-    const size_t plane = (size_t)c->sc.Lx * c->sc.Ly, own = n - 2 * plane;
-    padded.assign(3 * n, 0.0f);
-    const float* in[3] = {sx, sy, sz};
-    for (int k = 0; k < 3; ++k) std::memcpy(padded.data() + k * n + plane, in[k], own * sizeof(float));
-    sx = padded.data(); sy = sx + n; sz = sy + n;
-  }
+  // slab: the caller's Lx Ly Lz sites sit between two ghost planes (zero until exchanged): they are copied into the middle
+  // of the zeroed staging plane, no padded host copy is made
+  const size_t skip = c->slab_Lz > 0 ? (size_t)c->sc.Lx * c->sc.Ly : 0;
   const float* src[3] = {sx, sy, sz};
   for (int k = 0; k < 3; ++k) {
     if (c->plan.engine == ENGINE_SC) {
-      HB_CUDA(c, cudaMemcpyAsync(c->staging(), src[k], n * 4, cudaMemcpyHostToDevice, c->stream));
+      if (skip) HB_CUDA(c, cudaMemsetAsync(c->staging(), 0, n * 4, c->stream));
+      HB_CUDA(c, cudaMemcpyAsync(c->staging() + skip, src[k], (n - 2 * skip) * 4, cudaMemcpyHostToDevice, c->stream));
       HB_CUDA(c, launch_sc_permute(c->stream, c->spins + k * n, c->staging(), c->sc, true));
       c->launches += 1;
     } else if (c->plan.ell) {
