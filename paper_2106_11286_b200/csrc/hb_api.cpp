@@ -605,6 +605,15 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
     c->br.kind = lat->kind; c->br.Lx = lat->Lx; c->br.Ly = lat->Ly; c->br.Lz = lat->Lz;
     c->br.n = (uint32_t)P.n; c->br.nc = (uint32_t)(P.n / c->n_colours);
     c->tile = default_tile(lat->Lx, lat->Ly, lat->Lz);
+    if (c->tile.V == 4 && c->tile.ZT == 1 && c->tile.JX * c->tile.TY > 128 && c->tile.JX <= 128) {
+      // bcc / fcc launches of few blocks (the default above ended at one plane per block): blocks of 128 threads spread them
+      // more evenly over the SMs, and two planes per block where that still leaves eight blocks per SM
+      // (c2: 70.3 -> 72.8, c3: 84.2 -> 91.0 Gupd/s); lattices whose default marches several planes keep it
+      c->tile.TY = 128 / c->tile.JX > 0 ? 128 / c->tile.JX : 1;
+      if (c->tile.TY > lat->Ly) c->tile.TY = lat->Ly;
+      const int64_t cols = (int64_t)((lat->Lx / 4 + c->tile.JX - 1) / c->tile.JX) * ((lat->Ly + c->tile.TY - 1) / c->tile.TY);
+      c->tile.ZT = (lat->Lz >= 2 && cols * (lat->Lz / 2) >= 148 * 8) ? 2 : 1;
+    }
     // The warp-specialised kernel pays on lattices far larger than L2: bcc +2 ... +10 % over the direct kernel
     // (33.5 M sites, rows of 64 / 128 / 256 cells: 112 / 117 / 125 against 109 / 108 / 114 Gupd/s); fcc only with all passes in one
     // launch and long rows (89.9 against 85.1), its staged groups being three sublattices wide.  c2 and c3 (0.5 M and 8.4 M
