@@ -543,6 +543,10 @@ def test_kernel_variants_agree_on_random_shapes():
                     {"graph": int(rng.integers(0, 2)), "sc_kernel": 1, "sc_ws_zt": int(rng.integers(0, Lz + 1)),
                      "sc_ws_ctas": int(rng.integers(1, 5)),
                      "sc_ws_variant": int(rng.choice([0, 1, 2] + ([3] if H <= 248 else []) + ([4] if H <= 236 else []) + ([5] if H <= 128 else [])))}]
+        # fused launches (sc_kernel = 2): random chunk size, lag, sweeps per launch and CTA count; the variant first, then the kernel
+        fv = int(rng.choice([2] + ([4] if H <= 236 else []) + ([5] if H <= 128 else [])))
+        variants.append({"graph": 0, "sc_coop": 0, "sc_ws_variant": fv, "sc_kernel": 2, "sc_fused_zt": int(rng.integers(1, Lz + 1)),
+                         "sc_fused_lag": int(rng.integers(3, 9)), "sc_fused_sweeps": int(rng.integers(1, 17)), "sc_ws_ctas": int(rng.integers(1, 5))})
         for opts in variants:
             got, (Mg, Eg) = run(opts)
             assert spins_equal(got, ref), (Lx, Ly, Lz, opts)
