@@ -270,6 +270,16 @@ ScTile default_tile(int32_t H, int32_t Ly, int32_t Lz) {
   const int64_t cols = (int64_t)((HV + t.JX - 1) / t.JX) * ((L.Ly + t.TY - 1) / t.TY);
   t.ZT = 8;
   while (t.ZT > 1 && cols * ((L.Lz + t.ZT - 1) / t.ZT) < 148 * 16) t.ZT /= 2;
+  if (t.ZT == 1 && t.V == 4 && t.JX * t.TY > 128) {
+    // A launch of few blocks (the loop above ended at one plane per block): blocks of 128 threads spread it more evenly
+    // over the SMs, and march as many planes as still leave eight blocks per SM.  Measured (Gupd/s, replayed launches):
+    // sc 96^3 73 -> 80, sc 160^3 113 -> 118, sc 192^3 113 -> 116-119, c2 (bcc 64^3) 70.3 -> 72.8, c3 (fcc 128^3) 84.2 -> 91.0.
+    t.TY = 128 / t.JX > 0 ? 128 / t.JX : 1;
+    if (t.TY > L.Ly) t.TY = L.Ly;
+    const int64_t cols2 = (int64_t)((HV + t.JX - 1) / t.JX) * ((L.Ly + t.TY - 1) / t.TY);
+    t.ZT = 8;
+    while (t.ZT > 1 && cols2 * ((L.Lz + t.ZT - 1) / t.ZT) < 148 * 8) t.ZT /= 2;
+  }
   return t;
 }
 
@@ -605,15 +615,6 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
     c->br.kind = lat->kind; c->br.Lx = lat->Lx; c->br.Ly = lat->Ly; c->br.Lz = lat->Lz;
     c->br.n = (uint32_t)P.n; c->br.nc = (uint32_t)(P.n / c->n_colours);
     c->tile = default_tile(lat->Lx, lat->Ly, lat->Lz);
-    if (c->tile.V == 4 && c->tile.ZT == 1 && c->tile.JX * c->tile.TY > 128 && c->tile.JX <= 128) {
-      // bcc / fcc launches of few blocks (the default above ended at one plane per block): blocks of 128 threads spread them
-      // more evenly over the SMs, and two planes per block where that still leaves eight blocks per SM
-      // (c2: 70.3 -> 72.8, c3: 84.2 -> 91.0 Gupd/s); lattices whose default marches several planes keep it
-      c->tile.TY = 128 / c->tile.JX > 0 ? 128 / c->tile.JX : 1;
-      if (c->tile.TY > lat->Ly) c->tile.TY = lat->Ly;
-      const int64_t cols = (int64_t)((lat->Lx / 4 + c->tile.JX - 1) / c->tile.JX) * ((lat->Ly + c->tile.TY - 1) / c->tile.TY);
-      c->tile.ZT = (lat->Lz >= 2 && cols * (lat->Lz / 2) >= 148 * 8) ? 2 : 1;
-    }
     // The warp-specialised kernel pays on lattices far larger than L2: bcc +2 ... +10 % over the direct kernel
     // (33.5 M sites, rows of 64 / 128 / 256 cells: 112 / 117 / 125 against 109 / 108 / 114 Gupd/s); fcc only with all passes in one
     // launch and long rows (89.9 against 85.1), its staged groups being three sublattices wide.  c2 and c3 (0.5 M and 8.4 M
