@@ -169,7 +169,9 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
   const uint32_t h_hi = t_row + (uint32_t)(i0 + 4 >= L.H ? i0 + 4 - L.H : i0 + 4) * 4u;  // p = 1: element i0+4
   const size_t n = L.n;
   const size_t plane = (size_t)L.Ly * L.H;
-  RingPos<kNB> rm;   // slot of plane z-1 of the current step
+  RingPos<kNB> rm;   // slot of plane z-1 of the current step; rc, rq (planes z, z+1) are carried beside it: one next() per step
+  RingPos<kNB> rc = rm; rc.next();
+  RingPos<kNB> rq = rc; rq.next();
   const volatile int4* info = reinterpret_cast<const volatile int4*>(smem + S::OFF_TILE);
   float* const spins = a;   // FUSED: a is the base of the spins; the colour a tile updates depends on its pass
   uint32_t sweep_lo = P.sweep_lo, sweep_hi = P.sweep_hi;
@@ -235,8 +237,6 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
           sp[0] = load_rw<4>(gx); sp[1] = load_rw<4>(gx + n); sp[2] = load_rw<4>(gx + 2 * n);
         }
       }
-      RingPos<kNB> rc = rm; rc.next();
-      RingPos<kNB> rq = rc; rq.next();
       if (s == 0) mbar_wait(fullB + 8u * rc.slot, rc.par);
       mbar_wait(fullB + 8u * rq.slot, rq.par);
       const unsigned char* Bm = smem + rm.slot * S::SLOT_B;
@@ -326,9 +326,9 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
       }
       if (ALIAS) gx = a + ((size_t)((uint32_t)(z0 + s + 1) & w.zmask) * L.Ly + y) * L.H + i0; else gx += plane;
       site_row += (uint32_t)(L.Ly * L.Lx);
-      rm.next();
+      rm = rc; rc = rq; rq.next();
     }
-    rm.next(); rm.next();   // the two extra planes of the tile
+    rm = rq; rc = rm; rc.next(); rq = rc; rq.next();   // past the two extra planes of the tile
     if (SLAB && L.flag_in) {
       // a boundary tile is done: the last warp of the last tile of a boundary chunk tells the neighbour on that side
       const bool lo = zc == 0, hi = zc == w.n_zc - 1;
