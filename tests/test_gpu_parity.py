@@ -249,6 +249,31 @@ def test_full_size_first_10_sweeps(name):
         if mism == 0:
             assert spins_equal(ctx.get_spins(), st.get_spins())
         _measure_close(ctx, st, lat.n)
+        # and so do its fused launches (sc_kernel = 2, NEXT-1): three sweeps = one launch of two sweeps (four colour passes
+        # chained by progress words over 296 CTAs) + the measured sweep; then the traffic-minimal setting of
+        # profiles/r02_c4_fused_full.md (4-plane chunks, lag 3, one sweep per launch)
+        ctx.set_option("sc_kernel", 2)
+        ctx.sweep(T, 3)
+        st.sweep(T, 3)
+        if mism == 0:
+            assert spins_equal(ctx.get_spins(), st.get_spins())
+        _measure_close(ctx, st, lat.n)
+        for k, v in (("sc_fused_zt", 4), ("sc_fused_lag", 3), ("sc_fused_sweeps", 1)):
+            ctx.set_option(k, v)
+        ctx.sweep(T, 2)
+        st.sweep(T, 2)
+        if mism == 0:
+            assert spins_equal(ctx.get_spins(), st.get_spins())
+        _measure_close(ctx, st, lat.n)
+    if name in ("c2", "c3"):
+        # the warp-specialised bcc / fcc kernel (not the default at these sizes) continues the same trajectory, plain and fused
+        for kern in (1, 2):
+            ctx.set_option("br_kernel", kern)
+            ctx.sweep(T, 3)
+            st.sweep(T, 3)
+            if mism == 0:
+                assert spins_equal(ctx.get_spins(), st.get_spins())
+            _measure_close(ctx, st, lat.n)
 
 
 # ---- P3: long-run statistics against the fp64 random-site oracle (BASELINE.json north_star) ----------
