@@ -77,10 +77,10 @@ typedef struct {
    * with Philox key seed + r; more than one needs a simple cubic lattice of at most 8192 sites with Lx a
    * multiple of 8 and uniform anisotropy (each replica runs in one thread block, hb_sweep_each below). */
   int32_t n_replicas;
-  /* Slab of a larger periodic simple cubic lattice (multi-GPU decomposition along z).
-   * slab_Lz = 0: none.  slab_Lz > 0 (HB_SC only): the context holds planes z = slab_z0 .. slab_z0 + Lz - 1 of a lattice
-   * of Lx x Ly x slab_Lz sites (Lz, slab_z0, slab_Lz even), plus one ghost plane on each side that the caller keeps
-   * current (hb_slab_face).  Philox is keyed by the GLOBAL site id, so the slabs together walk the trajectory of the
+  /* Slab of a larger periodic sc, bcc or fcc lattice (multi-GPU decomposition along z).
+   * slab_Lz = 0: none.  slab_Lz > 0: the context holds planes (of conventional cells) z = slab_z0 .. slab_z0 + Lz - 1 of a
+   * lattice of Lx x Ly x slab_Lz cells (sc: Lz, slab_z0, slab_Lz even), plus, for every sublattice, one ghost plane on each
+   * side that the caller keeps current (hb_slab_face).  Philox is keyed by the GLOBAL site id, so the slabs together walk the trajectory of the
    * whole lattice bit for bit.  Such a context is driven with hb_slab_pass / hb_slab_next_sweep instead of hb_sweep. */
   int32_t slab_Lz, slab_z0;
 } hb_lattice;
@@ -174,9 +174,10 @@ int hb_counters(hb_ctx* ctx, uint64_t* kernel_launches, uint64_t* attempts);
 int hb_stats(hb_ctx* ctx, uint64_t* attempts, uint64_t* accepts);
 
 /* ---- slab contexts (hb_lattice.slab_Lz > 0): one sweep of the whole lattice is, on every slab,
- *        for colour in (0, 1):  hb_slab_pass(colour);  exchange the faces of that colour with both z-neighbours;
+ *        for colour in 0 .. colours-1:  hb_slab_pass(colour);  exchange the faces of that colour with both z-neighbours;
  *        hb_slab_next_sweep()
- * Colour = (x + y + z) mod 2 in GLOBAL coordinates.  hb_slab_pass launches the colour kernel on the slab (asynchronous, on
+ * Colour = (x + y + z) mod 2 in GLOBAL coordinates (sc), the basis index (bcc: 2, fcc: 4 colours; a face is then one cell
+ * plane of that sublattice).  hb_slab_pass launches the colour kernel on the slab (asynchronous, on
  * the context's stream).  hb_slab_face gives, as offsets in floats into the spins buffer (hb_buffers.spins, or the
  * library's own allocation) and a length in floats, the three contiguous component runs of one face of one colour:
  * side 0 = low z, 1 = high z; ghost 0 = the slab's own boundary plane (to send), 1 = the ghost plane beyond it (to

@@ -41,13 +41,16 @@ struct Plan {                 // device memory plan of a lattice
 int pad_slab(const hb_lattice* lat, hb_lattice& padded, std::string& why) {
   padded = *lat;
   if (lat->slab_Lz <= 0) return HB_OK;
-  if (lat->kind != HB_SC || lat->n_replicas > 1 || lat->K_site || lat->e_site) {
-    why = "a slab needs a simple cubic lattice with uniform anisotropy and no replicas"; return HB_EINVAL;
+  if ((lat->kind != HB_SC && lat->kind != HB_BCC && lat->kind != HB_FCC) || lat->n_replicas > 1 || lat->K_site || lat->e_site) {
+    why = "a slab needs a periodic sc, bcc or fcc lattice with uniform anisotropy and no replicas"; return HB_EINVAL;
   }
-  if (lat->Lz < 2 || ((lat->Lz | lat->slab_Lz | lat->slab_z0) & 1) || lat->slab_z0 < 0 || lat->slab_z0 + lat->Lz > lat->slab_Lz) {
-    why = "slab: Lz, slab_Lz, slab_z0 even, Lz >= 2, 0 <= slab_z0, slab_z0 + Lz <= slab_Lz"; return HB_EINVAL;
+  // sc: the checkerboard colour of a local plane must be known from its index, hence even offsets; bcc / fcc colour by basis index
+  const int odd = lat->kind == HB_SC ? ((lat->Lz | lat->slab_Lz | lat->slab_z0) & 1) : 0;
+  if (lat->Lz < (lat->kind == HB_SC ? 2 : 1) || odd || lat->slab_z0 < 0 || lat->slab_z0 + lat->Lz > lat->slab_Lz) {
+    why = "slab: 0 <= slab_z0, slab_z0 + Lz <= slab_Lz; simple cubic: Lz, slab_Lz, slab_z0 even and Lz >= 2"; return HB_EINVAL;
   }
-  if ((int64_t)lat->Lx * lat->Ly * lat->slab_Lz > 0xFFFFFFFFll) { why = "more than 2^32-1 sites in the whole lattice"; return HB_EINVAL; }
+  const int basis = lat->kind == HB_SC ? 1 : (lat->kind == HB_BCC ? 2 : 4);
+  if ((int64_t)lat->Lx * lat->Ly * lat->slab_Lz * basis > 0xFFFFFFFFll) { why = "more than 2^32-1 sites in the whole lattice"; return HB_EINVAL; }
   padded.Lz = lat->Lz + 2;
   padded.slab_Lz = 0;
   return HB_OK;
@@ -522,7 +525,7 @@ int hb_sizes(const hb_lattice* lat, int64_t* n_sites, size_t* spins_bytes, size_
   if (rc != HB_OK) return rc;
   rc = make_plan(&padded, p, why);
   if (rc != HB_OK) return rc;
-  if (n_sites) *n_sites = lat->slab_Lz > 0 ? (int64_t)lat->Lx * lat->Ly * lat->Lz : p.n;   // a slab's own sites
+  if (n_sites) *n_sites = lat->slab_Lz > 0 ? (int64_t)lat->Lx * lat->Ly * lat->Lz * (lat->kind == HB_SC ? 1 : (lat->kind == HB_BCC ? 2 : 4)) : p.n;   // a slab's own sites
   if (lat->slab_Lz > 0) p.spins_bytes += kAlign;   // the neighbour flags live behind the spins, where a peer mapping of the buffer reaches them
   if (spins_bytes) *spins_bytes = p.spins_bytes;
   if (workspace_bytes) *workspace_bytes = p.ws_bytes;
@@ -614,12 +617,19 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
     c->n_colours = lat->kind == HB_BCC ? 2 : 4;       // colour = basis index
     c->br.kind = lat->kind; c->br.Lx = lat->Lx; c->br.Ly = lat->Ly; c->br.Lz = lat->Lz;
     c->br.n = (uint32_t)P.n; c->br.nc = (uint32_t)(P.n / c->n_colours);
+    c->br.ghost = 0; c->br.nc_id = c->br.nc; c->br.cell_base = 0;
+    if (c->slab_Lz > 0) {   // local cell plane 1 is global plane slab_z0 (lat is the padded description here: Lz + 2 planes)
+      c->br.ghost = 1;
+      c->br.nc_id = (uint32_t)((int64_t)lat->Lx * lat->Ly * c->slab_Lz);
+      c->br.cell_base = (uint32_t)(((int64_t)c->slab_z0 - 1) * lat->Ly * lat->Lx);
+      c->graph_mode = 0; c->fused_measure = false;
+    }
     c->tile = default_tile(lat->Lx, lat->Ly, lat->Lz);
     // The warp-specialised kernel pays on lattices far larger than L2: bcc +2 ... +10 % over the direct kernel
     // (33.5 M sites, rows of 64 / 128 / 256 cells: 112 / 117 / 125 against 109 / 108 / 114 Gupd/s); fcc only with all passes in one
     // launch and long rows (89.9 against 85.1), its staged groups being three sublattices wide.  c2 and c3 (0.5 M and 8.4 M
     // sites, L2-resident, a handful of plane steps per CTA and pass) stay on the direct kernel: 27 against 70, 59 against 80.
-    if (bravais_ws_supported(c->br) && P.n >= (int64_t(1) << 24)) {
+    if (bravais_ws_supported(c->br) && P.n >= (int64_t(1) << 24)) {   // (never a slab: bravais_ws_supported)
       if (lat->kind == HB_BCC) { c->br_kernel = 1; c->br_zt = (lat->Lx > 64 && lat->Lx <= 128) ? 8 : 16; }
       else if (lat->Lx > 128) { c->br_kernel = 2; c->br_zt = 16; }
       if (c->br_zt > lat->Lz) c->br_zt = lat->Lz;
@@ -788,6 +798,8 @@ int hb_init_random(hb_ctx* c) {
     HB_CUDA(c, launch_init_random_sc(c->stream, c->spins, c->sc, (uint32_t)c->seed, (uint32_t)(c->seed >> 32)));
   else if (c->plan.ell)
     HB_CUDA(c, launch_init_random_perm(c->stream, c->spins, c->ell.perm, (uint32_t)c->plan.n, (uint32_t)c->seed, (uint32_t)(c->seed >> 32)));
+  else if (c->plan.engine == ENGINE_BRAVAIS)
+    HB_CUDA(c, launch_init_random_bravais(c->stream, c->spins, c->br, (uint32_t)c->seed, (uint32_t)(c->seed >> 32)));
   else
     HB_CUDA(c, launch_init_random_flat(c->stream, c->spins, (uint32_t)c->plan.n, (uint32_t)c->seed, (uint32_t)(c->seed >> 32)));
   c->launches += 1;
@@ -822,10 +834,16 @@ int hb_set_spins(hb_ctx* c, const float* sx, const float* sy, const float* sz) {
   const size_t n = (size_t)c->plan.n;
   // slab: the caller's Lx Ly Lz sites sit between two ghost planes (zero until exchanged): they are copied into the middle
   // of the zeroed staging plane, no padded host copy is made
-  const size_t skip = c->slab_Lz > 0 ? (size_t)c->sc.Lx * c->sc.Ly : 0;
+  const size_t skip = (c->slab_Lz > 0 && c->plan.engine == ENGINE_SC) ? (size_t)c->sc.Lx * c->sc.Ly : 0;
   const float* src[3] = {sx, sy, sz};
   for (int k = 0; k < 3; ++k) {
-    if (c->plan.engine == ENGINE_SC) {
+    if (c->plan.engine == ENGINE_BRAVAIS && c->slab_Lz > 0) {
+      // a bcc / fcc slab: the own cell planes of every sublattice are one contiguous run between its two ghost planes
+      const size_t plane = (size_t)c->br.Lx * c->br.Ly, own = (size_t)c->br.nc - 2 * plane;
+      HB_CUDA(c, cudaMemsetAsync(c->spins + k * n, 0, n * 4, c->stream));
+      for (int b = 0; b < c->n_colours; ++b)
+        HB_CUDA(c, cudaMemcpyAsync(c->spins + k * n + (size_t)b * c->br.nc + plane, src[k] + (size_t)b * own, own * 4, cudaMemcpyHostToDevice, c->stream));
+    } else if (c->plan.engine == ENGINE_SC) {
       if (skip) HB_CUDA(c, cudaMemsetAsync(c->staging(), 0, n * 4, c->stream));
       HB_CUDA(c, cudaMemcpyAsync(c->staging() + skip, src[k], (n - 2 * skip) * 4, cudaMemcpyHostToDevice, c->stream));
       HB_CUDA(c, launch_sc_permute(c->stream, c->spins + k * n, c->staging(), c->sc, true));
@@ -895,7 +913,11 @@ int hb_get_spins(hb_ctx* c, float* sx, float* sy, float* sz) {
   const size_t n = (size_t)c->plan.n;
   float* dst[3] = {sx, sy, sz};
   for (int k = 0; k < 3; ++k) {
-    if (c->plan.engine == ENGINE_SC) {
+    if (c->plan.engine == ENGINE_BRAVAIS && c->slab_Lz > 0) {
+      const size_t plane = (size_t)c->br.Lx * c->br.Ly, own = (size_t)c->br.nc - 2 * plane;
+      for (int b = 0; b < c->n_colours; ++b)
+        HB_CUDA(c, cudaMemcpyAsync(dst[k] + (size_t)b * own, c->spins + k * n + (size_t)b * c->br.nc + plane, own * 4, cudaMemcpyDeviceToHost, c->stream));
+    } else if (c->plan.engine == ENGINE_SC) {
       HB_CUDA(c, launch_sc_permute(c->stream, c->staging(), c->spins + k * n, c->sc, false));
       c->launches += 1;
       // a slab hands out its own planes only: they are contiguous in canonical order, between the two ghost planes
@@ -983,7 +1005,7 @@ int hb_measure(hb_ctx* c, double M[3], double* E) {
   HB_CUDA(c, cudaMemcpyAsync(h, c->cached(), sizeof h, cudaMemcpyDeviceToHost, c->stream));
   HB_CUDA(c, cudaStreamSynchronize(c->stream));
   // a slab returns its share of M of the whole lattice (the kernel skipped the ghost planes)
-  const double inv = 1.0 / (c->slab_Lz > 0 ? (double)c->sc.Lx * c->sc.Ly * c->slab_Lz : (double)c->plan.n);
+  const double inv = 1.0 / (c->slab_Lz > 0 ? (double)c->Lx * c->Ly * c->slab_Lz * (c->plan.engine == ENGINE_SC ? 1 : c->n_colours) : (double)c->plan.n);
   M[0] = h[0] * inv; M[1] = h[1] * inv; M[2] = h[2] * inv;
   *E = h[3];
   return HB_OK;
@@ -1148,12 +1170,18 @@ int hb_sweep_series_each(hb_ctx* c, const float* T, int64_t n_sweeps, double* M_
 int hb_slab_pass(hb_ctx* c, float T, int32_t colour) {
   HB_CHECK_CTX(c);
   if (c->slab_Lz <= 0) return fail(c, HB_ESTATE, "not a slab context");
-  if (colour != 0 && colour != 1) return fail(c, HB_EINVAL, "colour: 0 or 1");
+  if (colour < 0 || colour >= c->n_colours) return fail(c, HB_EINVAL, "colour: 0 .. colours - 1 (sc: 0 or 1)");
   if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
   float beta;
   int rc = check_T(c, T, &beta);
   if (rc != HB_OK) return rc;
   c->cache_valid = false;
+  if (c->plan.engine == ENGINE_BRAVAIS) {   // colour = basis index, whatever the slab's offset
+    rc = one_colour(c, colour, params(c, beta), Diag{nullptr, nullptr});
+    if (rc != HB_OK) return rc;
+    c->attempts += (uint64_t)c->br.nc - 2ull * (uint64_t)c->br.Lx * c->br.Ly;
+    return HB_OK;
+  }
   if (c->sc.flag_in) c->sc.stamp = ++c->slab_stamp;   // neighbour flags: this is the slab's pass number `stamp`
   rc = one_colour(c, 1 - colour, params(c, beta), Diag{nullptr, nullptr});
   if (rc != HB_OK) return rc;
@@ -1171,8 +1199,15 @@ int hb_slab_next_sweep(hb_ctx* c) {
 int hb_slab_face(hb_ctx* c, int32_t colour, int32_t side, int32_t ghost, size_t offset_floats[3], size_t* count_floats) {
   HB_CHECK_CTX(c);
   if (c->slab_Lz <= 0) return fail(c, HB_ESTATE, "not a slab context");
-  if ((colour | side | ghost) & ~1) return fail(c, HB_EINVAL, "colour, side, ghost: 0 or 1");
+  if (colour < 0 || colour >= c->n_colours || ((side | ghost) & ~1)) return fail(c, HB_EINVAL, "colour: 0 .. colours - 1; side, ghost: 0 or 1");
   if (!offset_floats || !count_floats) return fail(c, HB_EINVAL, "NULL output");
+  if (c->plan.engine == ENGINE_BRAVAIS) {   // one cell plane of sublattice `colour`: a contiguous run per component
+    const size_t plane = (size_t)c->br.Lx * c->br.Ly;
+    const int32_t z = side == 0 ? (ghost ? 0 : 1) : (ghost ? c->br.Lz - 1 : c->br.Lz - 2);
+    for (int k = 0; k < 3; ++k) offset_floats[k] = (size_t)k * c->br.n + (size_t)colour * c->br.nc + (size_t)z * plane;
+    *count_floats = plane;
+    return HB_OK;
+  }
   const size_t plane = (size_t)c->sc.Ly * c->sc.H;   // sites of one colour in a z-plane: one contiguous run per component
   const int32_t z = side == 0 ? (ghost ? 0 : 1) : (ghost ? c->sc.Lz - 1 : c->sc.Lz - 2);
   for (int k = 0; k < 3; ++k)
@@ -1184,6 +1219,7 @@ int hb_slab_face(hb_ctx* c, int32_t colour, int32_t side, int32_t ghost, size_t 
 int hb_slab_set_peer(hb_ctx* c, int32_t side, void* peer_spins, int32_t peer_Lz) {
   HB_CHECK_CTX(c);
   if (c->slab_Lz <= 0) return fail(c, HB_ESTATE, "not a slab context");
+  if (c->plan.engine != ENGINE_SC) return fail(c, HB_EINVAL, "peer stores exist for simple cubic slabs; bcc / fcc slabs exchange faces (hb_slab_face)");
   if (side != 0 && side != 1) return fail(c, HB_EINVAL, "side: 0 or 1");
   if (peer_spins && (peer_Lz < 2 || (peer_Lz & 1) || (int64_t)c->sc.Lx * c->sc.Ly * ((int64_t)peer_Lz + 2) > 0xFFFFFFFFll))
     return fail(c, HB_EINVAL, "peer_Lz: the neighbour's number of own planes (even, >= 2)");

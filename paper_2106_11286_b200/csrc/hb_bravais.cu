@@ -132,12 +132,13 @@ k_sweep_bravais(float* __restrict__ own, const float* __restrict__ all, BrLayout
   unsigned n_acc = 0;
   double acc_mx = 0.0, acc_my = 0.0, acc_mz = 0.0, acc_en = 0.0;
   for (int32_t z = z0; z < z1; ++z) {
+    if (L.ghost && (z == 0 || z == L.Lz - 1)) continue;      // ghost planes of a slab: the z-neighbour owns them
     where_z(w, L, z);
     const uint32_t o = w.zo[1] + w.yo[1] + w.i0;             // offset inside the own sublattice
     Vec<V> sx = load_rw<V>(own + o), sy = load_rw<V>(own + n + o), sz = load_rw<V>(own + 2 * n + o);
     Vec<V> hx, hy, hz;
     field<KIND, B, V>(all, L.nc, L.n, w, hx, hy, hz);
-    const uint32_t site0 = (uint32_t)B * L.nc + o;          // canonical id = b*Nc + cell
+    const uint32_t site0 = (uint32_t)B * L.nc_id + o + L.cell_base;   // canonical id = b*Nc + cell (of the whole lattice)
     bool any = false;
     if constexpr (V >= 2) {
 #pragma unroll
@@ -206,6 +207,7 @@ __device__ __forceinline__ void measure_sub(const float* __restrict__ s, const B
     for (uint32_t q = blockIdx.x * blockDim.x + threadIdx.x; q < chunks; q += gridDim.x * blockDim.x) {
       const uint32_t row = q / HV, j = q - row * HV;
       const int32_t z = (int32_t)(row / (uint32_t)L.Ly), y = (int32_t)(row - (uint32_t)z * (uint32_t)L.Ly);
+      if (L.ghost && (z == 0 || z == L.Lz - 1)) continue;    // a slab sums its own planes only
       Where w;
       where_y(w, L, y, (int32_t)(j * V), V);
       where_z(w, L, z);
@@ -229,6 +231,16 @@ k_measure_bravais(const float* __restrict__ s, BrLayout L, SweepParams P, double
   double mx = 0, my = 0, mz = 0, en = 0;
   measure_sub<KIND, 0, V>(s, L, P, mx, my, mz, en);
   block_reduce4(mx, my, mz, en, partials + (size_t)blockIdx.x * 4);
+}
+
+__global__ void k_init_random_bravais(float* sx, float* sy, float* sz, BrLayout L, uint32_t seed_lo, uint32_t seed_hi) {
+  for (unsigned long long m64 = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; m64 < L.n; m64 += (unsigned long long)gridDim.x * blockDim.x) {
+    const uint32_t m = (uint32_t)m64, b = m / L.nc, q = m - b * L.nc;
+    const Rand4 r = philox4x32_10(b * L.nc_id + q + L.cell_base, 1u, 0u, 0u, seed_lo, seed_hi);
+    float x, y, z;
+    sphere(r.r0, r.r1, x, y, z);
+    sx[m] = x; sy[m] = y; sz[m] = z;
+  }
 }
 
 inline int aniso_of(const SweepParams& p) {
@@ -301,6 +313,12 @@ cudaError_t launch_sweep_bravais(cudaStream_t st, float* s, BrLayout L, ScTile t
     }
   }
   return cudaErrorInvalidValue;
+}
+
+cudaError_t launch_init_random_bravais(cudaStream_t st, float* s, BrLayout L, uint32_t seed_lo, uint32_t seed_hi) {
+  const long long g = ((long long)L.n + 255) / 256;
+  k_init_random_bravais<<<(unsigned)(g < 1 ? 1 : (g > 148 * 16 ? 148 * 16 : g)), 256, 0, st>>>(s, s + L.n, s + 2 * (size_t)L.n, L, seed_lo, seed_hi);
+  return cudaGetLastError();
 }
 
 cudaError_t launch_measure_bravais(cudaStream_t st, const float* s, BrLayout L, int V, SweepParams p, double* partials, double* out) {

@@ -406,7 +406,7 @@ cudaError_t bw_pick(cudaStream_t st, float* s, const BrLayout& L, const SweepPar
 }  // namespace
 
 // rows of up to 256 cells, a multiple of 4 (16-byte bulk copies)
-bool bravais_ws_supported(const BrLayout& L) { return (L.kind == BR_BCC || L.kind == BR_FCC) && L.Lx % 4 == 0 && L.Lx <= 256; }
+bool bravais_ws_supported(const BrLayout& L) { return !L.ghost && (L.kind == BR_BCC || L.kind == BR_FCC) && L.Lx % 4 == 0 && L.Lx <= 256; }
 
 // chunks in z: ZT planes each (0: chosen so that one pass holds a few tiles per resident CTA)
 int bravais_ws_chunks(const BrLayout& L, int ZT, int grid_cap) {

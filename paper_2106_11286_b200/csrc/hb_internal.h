@@ -80,6 +80,11 @@ struct BrLayout {
   int32_t Lx, Ly, Lz;
   uint32_t nc;      // cells = sites per sublattice
   uint32_t n;       // N
+  // slab of a larger lattice along z (include/hb.h, hb_lattice.slab_Lz): cell planes 0 and Lz-1 of every sublattice are
+  // ghost planes (staged as neighbours, not updated, not measured); the Philox id of local cell q of sublattice b is
+  // b * nc_id + q + cell_base (mod 2^32) with nc_id the cells of the WHOLE lattice.  ghost = 0: nc_id = nc, cell_base = 0.
+  int32_t ghost;
+  uint32_t nc_id, cell_base;
 };
 
 // CSR tables on the device
@@ -124,6 +129,7 @@ constexpr int kFusedBlocksMax = 16384;   // per colour: larger grids use the sep
 // ---- kernels (hb_kernels.cu); every launcher returns the launch status -----------------
 cudaError_t launch_init_random_sc(cudaStream_t st, float* spins, ScLayout L, uint32_t seed_lo, uint32_t seed_hi);
 cudaError_t launch_init_random_flat(cudaStream_t st, float* spins, uint32_t n, uint32_t seed_lo, uint32_t seed_hi);
+cudaError_t launch_init_random_bravais(cudaStream_t st, float* spins, BrLayout L, uint32_t seed_lo, uint32_t seed_hi);
 cudaError_t launch_fill(cudaStream_t st, float* spins, uint32_t n, float x, float y, float z);
 cudaError_t launch_sc_permute(cudaStream_t st, float* dst, const float* src, ScLayout L, bool to_internal);
 // one step of the paper's own scheme, emulated (hb_sweep_paper_scheme): p.sweep_lo/hi = the step number

@@ -91,19 +91,25 @@ class LocalSlabs:
     """n_slabs slab contexts of one periodic sc lattice in this process."""
 
     def __init__(self, Lx, Ly, Lz, n_slabs, J=1.0, K=0.0, e=(0.0, 0.0, 1.0), seed=1, device="cuda:0", options=None,
-                 peer_stores=False, flags=False):
+                 peer_stores=False, flags=False, kind="sc"):
         """All slabs live on `device`.  (The library issues every call on the CUDA device that is current, and a process that
         drove contexts on several devices would have to switch it around every call and enable peer access itself: that
         path was never run on a multi-GPU box, so it is not offered -- one process per GPU, `DistSlab`, is.)"""
         from .binding import Context, Lattice
         self.shape = (Lx, Ly, Lz)
         self.parts = partition(Lz, n_slabs)
-        self.ctxs = [Context(Lattice("sc", Lx, Ly, nz, slab=(z0, Lz)), J, K, e, seed, device=device)
+        # kind "bcc" / "fcc": slabs of conventional cells; the colours are the basis indices, one face exchange per sublattice
+        # pass; peer stores and flags exist for the simple cubic kernels only
+        self.kind = kind
+        self.n_colours = {"sc": 2, "bcc": 2, "fcc": 4}[kind]
+        if kind != "sc" and (peer_stores or flags):
+            raise ValueError("peer stores and neighbour flags exist for simple cubic slabs")
+        self.ctxs = [Context(Lattice(kind, Lx, Ly, nz, slab=(z0, Lz)), J, K, e, seed, device=device)
                      for r, (z0, nz) in enumerate(self.parts)]
         for c in self.ctxs:
             for k, v in (options or {}).items():
                 c.set_option(k, v)
-        self.n = Lx * Ly * Lz
+        self.n = Lx * Ly * Lz * {"sc": 1, "bcc": 2, "fcc": 4}[kind]
         # peer stores (hb_slab_set_peer): the colour kernels write their boundary planes straight into the neighbours'
         # ghost planes, the exchange step disappears
         self.peer_stores = bool(peer_stores)
@@ -127,7 +133,7 @@ class LocalSlabs:
 
     def _fill_ghosts(self):
         self._sync()
-        for colour in (0, 1):
+        for colour in range(self.n_colours):
             exchange_local(self.ctxs, colour)
         self._sync()
 
@@ -142,19 +148,26 @@ class LocalSlabs:
         self._fill_ghosts()
 
     def set_spins(self, sx, sy, sz):
-        plane = self.shape[0] * self.shape[1]
+        # canonical order of the whole lattice: basis-major, z slowest inside a sublattice; a slab takes, per sublattice, its planes
+        plane, nb = self.shape[0] * self.shape[1], self.n // (self.shape[0] * self.shape[1] * self.shape[2])
+        nc = plane * self.shape[2]
         for c, (z0, nz) in zip(self.ctxs, self.parts):
-            c.set_spins(*[np.asarray(a, np.float32)[z0 * plane:(z0 + nz) * plane] for a in (sx, sy, sz)])
+            c.set_spins(*[np.concatenate([np.asarray(a, np.float32)[b * nc + z0 * plane:b * nc + (z0 + nz) * plane] for b in range(nb)])
+                          for a in (sx, sy, sz)])
         self._fill_ghosts()
 
     def get_spins(self):
+        plane, nb = self.shape[0] * self.shape[1], self.n // (self.shape[0] * self.shape[1] * self.shape[2])
         parts = [c.get_spins() for c in self.ctxs]
-        return [np.concatenate([p[k] for p in parts]) for k in range(3)]
+        out = []
+        for k in range(3):
+            out.append(np.concatenate([p[k][b * nz * plane:(b + 1) * nz * plane] for b in range(nb) for p, (z0, nz) in zip(parts, self.parts)]))
+        return out
 
     def sweep(self, T, n_sweeps=1):
         several = len({c.stream.cuda_stream for c in self.ctxs}) > 1
         for _ in range(n_sweeps):
-            for colour in (0, 1):
+            for colour in range(self.n_colours):
                 for c in self.ctxs:
                     c.slab_pass(T, colour)
                 if several:          # contexts on one stream are ordered by it; otherwise passes and copies meet here
@@ -188,7 +201,7 @@ class DistSlab:
     (an all_reduce of one word on the stream under NCCL; a host barrier under gloo)."""
 
     def __init__(self, Lx, Ly, Lz, J=1.0, K=0.0, e=(0.0, 0.0, 1.0), seed=1, device=None, group=None, options=None,
-                 peer_stores=False, flags=False):
+                 peer_stores=False, flags=False, kind="sc"):
         """flags=True (with peer_stores, one GPU per rank): no barrier between two colour passes; the kernels wait for and
         signal their two z-neighbours through flag words in peer memory (include/hb.h, "slab_flags"), boundary tiles first,
         so that interior tiles hide the wait.  Never with several ranks on ONE GPU: their kernels would wait on one another."""
@@ -203,12 +216,15 @@ class DistSlab:
         self.shape = (Lx, Ly, Lz)
         parts = partition(Lz, self.world)
         self.z0, self.nz = parts[self.rank]
-        self.peer_stores = bool(peer_stores)
-        self.ctx = Context(Lattice("sc", Lx, Ly, self.nz, slab=(self.z0, Lz)), J, K, e, seed,
+        self.kind = kind
+        self.n_colours = {"sc": 2, "bcc": 2, "fcc": 4}[kind]      # bcc / fcc: slabs of conventional cells, one face exchange per sublattice pass
+        self.peer_stores = bool(peer_stores) and kind == "sc"      # peer stores and flags: simple cubic kernels only
+        flags = bool(flags) and kind == "sc"
+        self.ctx = Context(Lattice(kind, Lx, Ly, self.nz, slab=(self.z0, Lz)), J, K, e, seed,
                            device=device or "cuda:0", ipc=self.peer_stores and self.world > 1)
         for k, v in (options or {}).items():
             self.ctx.set_option(k, v)
-        self.n = Lx * Ly * Lz
+        self.n = Lx * Ly * Lz * {"sc": 1, "bcc": 2, "fcc": 4}[kind]
         self._mapped = {}
         self.flags = False
         if self.peer_stores:
@@ -260,7 +276,7 @@ class DistSlab:
             dist.barrier(group=self.group)
 
     def _fill_ghosts(self):
-        for colour in (0, 1):
+        for colour in range(self.n_colours):
             exchange_dist(self.ctx, colour, self.rank, self.world, self.group)
         if self.peer_stores:
             self._pass_barrier()
@@ -275,7 +291,7 @@ class DistSlab:
 
     def sweep(self, T, n_sweeps=1):
         for _ in range(n_sweeps):
-            for colour in (0, 1):
+            for colour in range(self.n_colours):
                 self.ctx.slab_pass(T, colour)
                 if self.peer_stores and self.flags:
                     pass                         # the next pass's boundary tiles wait for the neighbours' flags on the device

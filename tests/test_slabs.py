@@ -169,7 +169,9 @@ def test_slab_contexts_refuse_whole_lattice_calls():
         with pytest.raises(hb.HbError):
             hb.Context(hb.Lattice("sc", 8, 4, 4, **bad), 1.0, 0.0, (0, 0, 1), 1)
     with pytest.raises(hb.HbError):
-        hb.Context(hb.Lattice("bcc", 4, 4, 4, slab=(0, 8)), 1.0, 0.0, (0, 0, 1), 1)
+        hb.Context(hb.Lattice("bcc", 4, 4, 4, slab=(6, 8)), 1.0, 0.0, (0, 0, 1), 1)     # 6 + 4 planes do not fit into 8
+    with pytest.raises(hb.HbError):
+        hb.Context(hb.Lattice("sc", 8, 4, 4, slab=(4, 12), n_replicas=2), 1.0, 0.0, (0, 0, 1), 1)
     whole = hb.Context(hb.Lattice("sc", 8, 4, 4), 1.0, 0.0, (0, 0, 1), 1)
     with pytest.raises(hb.HbError):
         whole.slab_pass(1.0, 0)
@@ -271,9 +273,47 @@ def test_slab_lattice_sizes_host_logic():
     for bad in [dict(slab=(3, 12)), dict(slab=(4, 6)), dict(slab=(0, 11)), dict(slab=(-2, 12))]:
         with pytest.raises(hb.HbError):
             hb.sizes(hb.Lattice("sc", 8, 4, 4, **bad))
+    assert hb.sizes(hb.Lattice("fcc", 4, 4, 3, slab=(1, 8)))[0] == 4 * 4 * 4 * 3       # bcc / fcc slabs: any offset, own sites of all sublattices
     with pytest.raises(hb.HbError):
-        hb.sizes(hb.Lattice("fcc", 4, 4, 4, slab=(0, 8)))
+        hb.sizes(hb.Lattice("fcc", 4, 4, 4, slab=(6, 8)))
     # implicit lattices go up to 2^32 - 1 sites; the table engine is bounded by its 32-bit neighbour offsets
     assert hb.sizes(hb.Lattice("sc", 1600, 1600, 1600))[0] == 4096000000
     with pytest.raises(hb.HbError):
         hb.sizes(hb.Lattice("sc", 1626, 1626, 1626))
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("kind,shape,n_slabs,K,e", [
+    ("bcc", (8, 6, 8), 2, 0.1, (0.0, 0.0, 1.0)), ("bcc", (12, 5, 12), 3, 0.3, (0.6, 0.0, 0.8)), ("bcc", (4, 4, 4), 1, 0.0, (0.0, 0.0, 1.0)),
+    ("fcc", (8, 6, 8), 2, 0.05, (0.0, 0.6, 0.8)), ("fcc", (4, 3, 12), 4, 0.0, (0.0, 0.0, 1.0)), ("fcc", (16, 4, 6), 3, 0.2, (0.0, 0.0, 1.0)),
+])
+def test_bcc_and_fcc_slabs_walk_the_single_lattice_trajectory(kind, shape, n_slabs, K, e):
+    # SURVEY 8(e) for the lattices with a basis: slabs of conventional cells, one ghost cell plane per side and sublattice, one
+    # face exchange per sublattice pass; Philox keyed by the global site id b * Ncell + cell, so the slabs together walk the
+    # oracle's trajectory of the whole lattice bit for bit, from init_random, from a state handed in, and in M and E
+    import oracle
+    from hbtest import spins_equal
+    lat = getattr(oracle.Lattice, kind)(*shape)
+    lat.set_uniform_anisotropy(K, e)
+    st = oracle.State32(lat, 1.0, 31)
+    sl = slabs.LocalSlabs(*shape, n_slabs, J=1.0, K=K, e=e, seed=31, kind=kind)
+    assert sl.n == lat.n
+    st.init_random()
+    sl.init_random()
+    assert spins_equal(sl.get_spins(), st.get_spins())
+    for T, k in ((2.0, 1), (2.0, 4), (0.4, 3)):
+        sl.sweep(T, k)
+        st.sweep(T, k)
+        assert spins_equal(sl.get_spins(), st.get_spins()), (kind, shape, n_slabs, T)
+        Mg, Eg = sl.measure()
+        Mo, Eo = st.measure()[:2]
+        assert np.max(np.abs(Mg - np.asarray(Mo))) <= 1e-7 and abs(Eg - Eo) <= 1e-6 * lat.n
+    sl2 = slabs.LocalSlabs(*shape, n_slabs, J=1.0, K=K, e=e, seed=31, kind=kind)      # checkpoint: state + counter handed in
+    sl2.set_spins(*st.get_spins())
+    for c in sl2.ctxs:
+        c.sweep_count = st.sweep_count
+    sl2.sweep(1.5, 2)
+    st.sweep(1.5, 2)
+    assert spins_equal(sl2.get_spins(), st.get_spins())
+    sl.close()
+    sl2.close()
