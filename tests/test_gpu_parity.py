@@ -968,8 +968,10 @@ def test_paper_scheme_emulation_statistics():
         se_e = math.sqrt(g_e.var(ddof=1) / reps + o_e.var(ddof=1) / reps)
         print("paper scheme n = %d: |M| %.5f (o64 %.5f, diff %+.1e, se %.1e)  E/N %.5f (o64 %.5f, diff %+.1e, se %.1e)" %
               (n_per_block, g_m.mean(), o_m.mean(), dm, se_m, g_e.mean(), o_e.mean(), de, se_e))
-        if n_per_block >= 8:
-            assert abs(dm) <= 0.01 and abs(de) <= 0.01, (n_per_block, dm, de)
+        if n_per_block >= 8:      # racy and therefore not reproducible run to run: a loose bound (measured +6e-3 +- 3e-3 in E/N at n = 8)
+            assert abs(dm) <= 0.02 and abs(de) <= 0.025, (n_per_block, dm, de)
+        else:                     # n = 1: every spin moves against stale neighbours: the bias is an order of magnitude larger
+            assert de > 0.05, (n_per_block, de)
     with pytest.raises(hb.HbError):
         hb.Context(hb.Lattice("sc", 6)).sweep_paper_scheme(1.0, 1, 8)     # before init; and 216 sites are not a multiple of 8
 
