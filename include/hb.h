@@ -83,6 +83,16 @@ typedef struct {
    * side that the caller keeps current (hb_slab_face).  Philox is keyed by the GLOBAL site id, so the slabs together walk the trajectory of the
    * whole lattice bit for bit.  Such a context is driven with hb_slab_pass / hb_slab_next_sweep instead of hb_sweep. */
   int32_t slab_Lz, slab_z0;
+  /* Part of a larger neighbour table (HB_CSR; multi-GPU decomposition by ranges of the canonical order).
+   * part_n_total = 0: none.  part_n_total > 0: the context holds sites part_first .. part_first + part_n_own - 1 of a table of
+   * part_n_total sites as its local sites 0 .. part_n_own - 1, followed by n_sites - part_n_own GHOST sites: copies of
+   * other parts' sites that the local rows point to.  Ghost rows are empty; ghosts are never attempted or measured, the caller
+   * keeps them current (hb_part_gather on the owner, hb_part_scatter here, after every colour pass).  `colour` is required:
+   * the colouring of the WHOLE table restricted to the local sites, ghosts included (checked on the own rows).  Philox is
+   * keyed by the global id part_first + local id, so the parts together walk the trajectory of the whole table bit for bit.
+   * Such a context is driven with hb_slab_pass / hb_slab_next_sweep like a slab; hb_measure returns its share (M normalised
+   * by part_n_total, every bond half at each end); hb_get_spins / hb_set_spins move all n_sites local sites, ghosts included. */
+  int64_t part_n_total, part_first, part_n_own;
 } hb_lattice;
 
 /* Caller-owned device memory (e.g. torch tensors).  Sizes from hb_sizes().  Both
@@ -199,6 +209,14 @@ int hb_slab_face(hb_ctx* ctx, int32_t colour, int32_t side, int32_t ghost, size_
  * (stream order on one device; a collective or an event between devices).  The ghost planes must still be filled once
  * with hb_slab_face copies after hb_init_* / hb_set_spins.  peer_spins = NULL switches the side back to copies. */
 int hb_slab_set_peer(hb_ctx* ctx, int32_t side, void* peer_spins, int32_t peer_Lz);
+/* Parts of a neighbour table (hb_lattice.part_n_total > 0; any HB_CSR context): the exchange step after a colour pass moves the
+ * spins of listed sites.  hb_part_gather packs the spins of the `count` local sites ids[k] (DEVICE array of local ids) into
+ * out[4 k .. 4 k + 3] = (x, y, z, 0) (DEVICE, 16-byte aligned); hb_part_scatter stores in[4 k .. 4 k + 2] as the spin of local
+ * site ids[k] (ghost sites on the receiving part).  Both are asynchronous on the context's stream; the copy between the two
+ * (device to device, NCCL send / recv) is the caller's.  ids out of range are an error of the caller (not checked on the
+ * device); count = 0 is a no-op. */
+int hb_part_gather(hb_ctx* ctx, const int32_t* ids, int64_t count, float* out);
+int hb_part_scatter(hb_ctx* ctx, const int32_t* ids, int64_t count, const float* in);
 /* hb_set_option(ctx, "slab_flags", 1) (after hb_slab_set_peer on both sides; warp-specialised kernel) replaces that barrier by
  * flags between neighbours, kept in the two words behind each slab's spins (so that a peer mapping of the spins buffer
  * reaches them; hb_sizes counts them): colour pass number s of a slab takes its two boundary chunks first; a boundary tile

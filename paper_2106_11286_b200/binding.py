@@ -17,7 +17,7 @@ EXPORTS = [
     "hb_stage_spins", "hb_commit_spins",
     "hb_sweep", "hb_measure", "hb_sweep_series", "hb_sweep_record", "hb_sweep_count", "hb_set_sweep_count",
     "hb_sweep_each", "hb_measure_each", "hb_sweep_series_each", "hb_select_replica",
-    "hb_slab_pass", "hb_slab_next_sweep", "hb_slab_face", "hb_slab_set_peer", "hb_probe_alu",
+    "hb_slab_pass", "hb_slab_next_sweep", "hb_slab_face", "hb_slab_set_peer", "hb_part_gather", "hb_part_scatter", "hb_probe_alu",
     "hb_device_alloc", "hb_device_free", "hb_ipc_export", "hb_ipc_open", "hb_ipc_close",
     "hb_get_colouring", "hb_counters", "hb_stats", "hb_device_math", "hb_probe_sc_l2", "hb_probe_pipe", "hb_sweep_paper_scheme", "hb_set_option", "hb_get_option", "hb_lattice_fcc_sphere", "hb_lattice_free",
     "hb_strerror", "hb_error_detail",
@@ -28,7 +28,8 @@ class hb_lattice(C.Structure):
     _fields_ = [("kind", C.c_int32), ("Lx", C.c_int32), ("Ly", C.c_int32), ("Lz", C.c_int32),
                 ("n_sites", C.c_int64), ("row_ptr", C.c_void_p), ("col_idx", C.c_void_p),
                 ("n_colours", C.c_int32), ("colour", C.c_void_p), ("K_site", C.c_void_p), ("e_site", C.c_void_p),
-                ("n_replicas", C.c_int32), ("slab_Lz", C.c_int32), ("slab_z0", C.c_int32)]
+                ("n_replicas", C.c_int32), ("slab_Lz", C.c_int32), ("slab_z0", C.c_int32),
+                ("part_n_total", C.c_int64), ("part_first", C.c_int64), ("part_n_own", C.c_int64)]
 
 
 class hb_buffers(C.Structure):
@@ -82,6 +83,8 @@ def load_library():
         "hb_slab_next_sweep": [vp],
         "hb_slab_face": [vp, i32, i32, i32, P(C.c_size_t), P(C.c_size_t)],
         "hb_slab_set_peer": [vp, i32, vp, i32],
+        "hb_part_gather": [vp, vp, i64, vp],
+        "hb_part_scatter": [vp, vp, i64, vp],
         "hb_probe_alu": [vp, C.c_double, P(C.c_double)],
         "hb_device_alloc": [C.c_size_t, P(vp)],
         "hb_device_free": [vp],
@@ -127,7 +130,7 @@ class Lattice:
     """Host description of a lattice (the hb_lattice struct plus the arrays it points to)."""
 
     def __init__(self, kind, Lx=0, Ly=0, Lz=0, row_ptr=None, col_idx=None, colour=None, n_colours=0,
-                 K_site=None, e_site=None, xyz=None, n_replicas=1, slab=None):
+                 K_site=None, e_site=None, xyz=None, n_replicas=1, slab=None, part=None):
         self.kind = _KINDS[kind] if isinstance(kind, str) else int(kind)
         self.Lx, self.Ly, self.Lz = int(Lx), int(Ly or Lx), int(Lz or Lx)
         self.row_ptr = _np(row_ptr, np.int64) if row_ptr is not None else None
@@ -140,6 +143,8 @@ class Lattice:
         self.n_replicas = int(n_replicas)
         # slab = (z0, Lz_global): this lattice is planes z0 .. z0 + Lz - 1 of a periodic sc lattice Lx x Ly x Lz_global
         self.slab = (int(slab[0]), int(slab[1])) if slab is not None else None
+        # part = (first, n_own, n_total): local sites 0 .. n_own-1 are sites first .. of a table of n_total sites, the rest ghosts
+        self.part = tuple(int(v) for v in part) if part is not None else None
 
     @classmethod
     def fcc_sphere(cls, R, K_core=0.0, e_core=(0, 0, 1), K_surf=0.0, colouring="greedy"):
@@ -171,6 +176,8 @@ class Lattice:
         s.n_replicas = self.n_replicas
         if self.slab is not None:
             s.slab_z0, s.slab_Lz = self.slab
+        if self.part is not None:
+            s.part_first, s.part_n_own, s.part_n_total = self.part
         if self.row_ptr is not None:
             s.n_sites = self.row_ptr.size - 1
             s.row_ptr = _ptr(self.row_ptr)
@@ -409,6 +416,17 @@ class Context:
     def slab_set_peer(self, side, peer_spins_ptr, peer_Lz):
         """Peer stores for one side (include/hb.h): peer_spins_ptr = device address of the z-neighbour's spins buffer."""
         self._check(self._L.hb_slab_set_peer(self._h, int(side), C.c_void_p(peer_spins_ptr), int(peer_Lz)), "hb_slab_set_peer")
+
+    # ---- parts of a neighbour table (Lattice("csr", ..., part=(first, n_own, n_total))); paper_2106_11286_b200.parts drives them ----
+    def part_gather(self, ids, out):
+        """hb_part_gather: spins of the local sites ids (torch int32, device) -> out (torch float32, device, 4 floats per site)."""
+        assert ids.is_cuda and out.is_cuda and out.numel() >= 4 * ids.numel()
+        self._check(self._L.hb_part_gather(self._h, C.c_void_p(ids.data_ptr()), ids.numel(), C.c_void_p(out.data_ptr())), "hb_part_gather")
+
+    def part_scatter(self, ids, src):
+        """hb_part_scatter: src (4 floats per site) -> spins of the local sites ids."""
+        assert ids.is_cuda and src.is_cuda and src.numel() >= 4 * ids.numel()
+        self._check(self._L.hb_part_scatter(self._h, C.c_void_p(ids.data_ptr()), ids.numel(), C.c_void_p(src.data_ptr())), "hb_part_scatter")
 
     @property
     def spins_ptr(self):

@@ -33,6 +33,10 @@ struct Plan {                 // device memory plan of a lattice
   size_t spins_bytes = 0, ws_bytes = 0;
   size_t off_partials = 0, off_series = 0, off_counters = 0, off_staging = 0, off_wsdone = 0;
   size_t off_row_ptr = 0, off_col = 0, off_list = 0, off_K = 0, off_e = 0;
+  // a part of a larger neighbour table (hb_lattice.part_n_total > 0): own sites 0 .. n_own-1 are global sites part_first ...,
+  // the remaining local sites are ghosts; off_inv: canonical id -> internal index (ELL engine), for hb_part_gather / scatter
+  int64_t n_own = 0, part_first = 0, part_total = 0;
+  size_t off_inv = 0;
 };
 
 // A slab (hb_lattice.slab_Lz > 0) is run as a periodic lattice of Lz + 2 planes whose first and last planes are the
@@ -89,10 +93,19 @@ int make_plan(const hb_lattice* lat, Plan& p, std::string& why) {
       why = "n_colours must be in [1, min(n_sites, 65536)]"; return HB_EINVAL;
     }
     p.maxdeg = (int32_t)(md > 0x7FFFFFFF ? 0x7FFFFFFF : md);
+    if (lat->part_n_total > 0) {
+      if (lat->part_n_own < 1 || lat->part_n_own > p.n || lat->part_first < 0 || lat->part_first + lat->part_n_own > lat->part_n_total ||
+          lat->part_n_total > 0xFFFFFFFFll || !lat->colour || lat->n_replicas > 1) {
+        why = "part of a table: 1 <= part_n_own <= n_sites, 0 <= part_first, part_first + part_n_own <= part_n_total < 2^32, colour given, no replicas";
+        return HB_EINVAL;
+      }
+      p.n_own = lat->part_n_own; p.part_first = lat->part_first; p.part_total = lat->part_n_total;
+    }
   } else {
     why = "unknown lattice kind";
     return HB_EINVAL;
   }
+  if (k != HB_CSR && lat->part_n_total > 0) { why = "part_n_total: neighbour tables (HB_CSR) only; sc, bcc and fcc are cut into slabs (slab_Lz)"; return HB_EINVAL; }
   if (p.n < 1) { why = "lattice has no sites"; return HB_EINVAL; }
   if (p.n > 0xFFFFFFFFll) { why = "more than 2^32-1 sites (site ids are 32-bit Philox counter words)"; return HB_EINVAL; }
   if ((lat->K_site == nullptr) != (lat->e_site == nullptr)) { why = "K_site and e_site go together"; return HB_EINVAL; }
@@ -124,7 +137,8 @@ int make_plan(const hb_lattice* lat, Plan& p, std::string& why) {
   if (p.engine == ENGINE_CSR) {
     // ELL when padding every row to the maximum degree costs little (regular lattices, cut-outs of them);
     // graphs with a few high-degree sites keep the plain CSR kernel
-    p.ell = p.maxdeg >= 1 && p.maxdeg <= 64 && (int64_t)p.maxdeg * p.n <= 2 * p.nnz + 1024;
+    p.ell = p.maxdeg >= 1 && p.maxdeg <= 64 && (int64_t)p.maxdeg * (p.part_total > 0 ? p.n_own : p.n) <= 2 * p.nnz + 1024;   // (ghost rows are empty)
+    if (p.ell && p.part_total > 0) { p.off_inv = o; o += align_up((size_t)p.n * sizeof(int32_t)); }
     if (p.ell) {
       p.off_ell = o;    o += align_up((size_t)p.maxdeg * (size_t)p.n * sizeof(int32_t));
       p.off_cbegin = o; o += align_up(((size_t)(p.n < kMaxColours ? p.n : kMaxColours) + 2) * sizeof(uint32_t));
@@ -571,11 +585,12 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
   const int32_t* col = nullptr;
   if (P.engine == ENGINE_CSR) {
     if (lat->kind == HB_CSR) {
-      why = validate_csr(P.n, lat->row_ptr, lat->col_idx);
+      const int64_t n_own = P.part_total > 0 ? P.n_own : P.n;
+      why = validate_csr(P.n, lat->row_ptr, lat->col_idx, n_own);
       if (!why.empty()) { c->sticky = HB_EINVAL; return fail(c, HB_EINVAL, why); }
       row_ptr = lat->row_ptr; col = lat->col_idx;
       if (lat->colour) {
-        why = validate_colouring(P.n, row_ptr, col, lat->colour, lat->n_colours);
+        why = validate_colouring(P.n, row_ptr, col, lat->colour, lat->n_colours, n_own);
         if (!why.empty()) { c->sticky = HB_EINVAL; return fail(c, HB_EINVAL, why); }
         c->colour_host.assign(lat->colour, lat->colour + P.n);
         c->n_colours = lat->n_colours;
@@ -695,24 +710,26 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
   if (P.engine == ENGINE_SC || P.engine == ENGINE_BRAVAIS) HB_CUDA(c, cudaMemsetAsync(c->ws + P.off_wsdone, 0, (size_t)kWsDoneWords * sizeof(uint32_t), c->stream));
 
   if (P.engine == ENGINE_CSR) {
-    // sites sorted by (colour, id): one contiguous list segment per colour
+    // sites sorted by (colour, id): one contiguous list segment per colour; the ghost sites of a part follow the last colour
+    const int64_t n_own = P.part_total > 0 ? P.n_own : P.n;
     std::vector<uint32_t> count((size_t)c->n_colours + 1, 0);
-    for (int64_t i = 0; i < P.n; ++i) count[c->colour_host[i] + 1] += 1;
+    for (int64_t i = 0; i < n_own; ++i) count[c->colour_host[i] + 1] += 1;
     for (int k = 0; k < c->n_colours; ++k) count[k + 1] += count[k];
     c->colour_begin = count;
     if (c->n_colours > kMaxColours) { c->sticky = HB_EINVAL; return fail(c, HB_EINVAL, "more than 65536 colours"); }
     std::vector<int32_t> list((size_t)P.n);
     {
       std::vector<uint32_t> cur(count.begin(), count.end() - 1);
-      for (int64_t i = 0; i < P.n; ++i) list[cur[c->colour_host[i]]++] = (int32_t)i;
+      for (int64_t i = 0; i < n_own; ++i) list[cur[c->colour_host[i]]++] = (int32_t)i;
+      for (int64_t i = n_own; i < P.n; ++i) list[i] = (int32_t)i;
     }
     int32_t* d_list = reinterpret_cast<int32_t*>(c->ws + P.off_list);
     HB_CUDA(c, cudaMemcpyAsync(d_list, list.data(), list.size() * 4, cudaMemcpyHostToDevice, c->stream));
-    std::vector<int32_t> rp32, ell;
+    std::vector<int32_t> rp32, ell, inv;
     std::vector<float> soa;
     if (P.ell) {
       // internal order m = position in the colour-sorted list; table entries are internal indices
-      std::vector<int32_t> inv((size_t)P.n);
+      inv.resize((size_t)P.n);
       for (int64_t m = 0; m < P.n; ++m) inv[list[m]] = (int32_t)m;
       ell.assign((size_t)P.maxdeg * (size_t)P.n, -1);
       for (int k = 0; k < c->n_colours; ++k) {
@@ -729,6 +746,12 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
       HB_CUDA(c, cudaMemcpyAsync(d_cb, count.data(), count.size() * 4, cudaMemcpyHostToDevice, c->stream));
       c->ell.n = (uint32_t)P.n; c->ell.maxdeg = (uint32_t)P.maxdeg; c->ell.ell = d_ell; c->ell.perm = d_list;
       c->ell.colour_begin = d_cb; c->ell.n_colours = c->n_colours;
+      c->ell.site_base = (uint32_t)P.part_first; c->ell.inv = nullptr;
+      if (P.part_total > 0) {
+        int32_t* d_inv = reinterpret_cast<int32_t*>(c->ws + P.off_inv);
+        HB_CUDA(c, cudaMemcpyAsync(d_inv, inv.data(), inv.size() * 4, cudaMemcpyHostToDevice, c->stream));
+        c->ell.inv = d_inv;
+      }
       c->ell.K = c->ell.ex = c->ell.ey = c->ell.ez = nullptr;
       if (P.per_site) {   // (K, e) in internal order, one plane each: K at off_K, ex|ey|ez at off_e
         soa.resize(4 * (size_t)P.n);
@@ -753,6 +776,7 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
       HB_CUDA(c, cudaMemcpyAsync(d_rp, rp32.data(), rp32.size() * 4, cudaMemcpyHostToDevice, c->stream));
       if (P.nnz) HB_CUDA(c, cudaMemcpyAsync(d_col, col, (size_t)P.nnz * 4, cudaMemcpyHostToDevice, c->stream));
       c->csr.n = (uint32_t)P.n; c->csr.row_ptr = d_rp; c->csr.col = d_col; c->csr.list = d_list;
+      c->csr.n_own = (uint32_t)n_own; c->csr.site_base = (uint32_t)P.part_first;
       c->csr.K_site = nullptr; c->csr.e_site = nullptr;
       if (P.per_site) {
         float* d_K = reinterpret_cast<float*>(c->ws + P.off_K);
@@ -797,11 +821,11 @@ int hb_init_random(hb_ctx* c) {
   if (c->plan.engine == ENGINE_SC)
     HB_CUDA(c, launch_init_random_sc(c->stream, c->spins, c->sc, (uint32_t)c->seed, (uint32_t)(c->seed >> 32)));
   else if (c->plan.ell)
-    HB_CUDA(c, launch_init_random_perm(c->stream, c->spins, c->ell.perm, (uint32_t)c->plan.n, (uint32_t)c->seed, (uint32_t)(c->seed >> 32)));
+    HB_CUDA(c, launch_init_random_perm(c->stream, c->spins, c->ell.perm, (uint32_t)c->plan.n, (uint32_t)c->seed, (uint32_t)(c->seed >> 32), c->ell.site_base));
   else if (c->plan.engine == ENGINE_BRAVAIS)
     HB_CUDA(c, launch_init_random_bravais(c->stream, c->spins, c->br, (uint32_t)c->seed, (uint32_t)(c->seed >> 32)));
   else
-    HB_CUDA(c, launch_init_random_flat(c->stream, c->spins, (uint32_t)c->plan.n, (uint32_t)c->seed, (uint32_t)(c->seed >> 32)));
+    HB_CUDA(c, launch_init_random_flat(c->stream, c->spins, (uint32_t)c->plan.n, (uint32_t)c->seed, (uint32_t)(c->seed >> 32), (uint32_t)c->plan.part_first));
   c->launches += 1;
   c->initialised = true;
   return HB_OK;
@@ -865,7 +889,7 @@ int hb_set_spins(hb_ctx* c, const float* sx, const float* sy, const float* sz) {
 int hb_stage_spins(hb_ctx* c, const float* sx, const float* sy, const float* sz) {
   HB_CHECK_CTX(c);
   if (!sx || !sy || !sz) return fail(c, HB_EINVAL, "NULL spin array");
-  if (c->slab_Lz > 0 || c->plan.R > 1) return fail(c, HB_EINVAL, "hb_stage_spins: whole lattices without replicas");
+  if (c->slab_Lz > 0 || c->plan.part_total > 0 || c->plan.R > 1) return fail(c, HB_EINVAL, "hb_stage_spins: whole lattices without replicas");
   const size_t n = (size_t)c->plan.n;
   if (!c->stage) {
     if (cudaMalloc(reinterpret_cast<void**>(&c->stage), 3 * n * sizeof(float)) != cudaSuccess) { cudaGetLastError(); return fail(c, HB_ENOMEM, "hb_stage_spins: cudaMalloc of the upload area failed"); }
@@ -937,7 +961,7 @@ int hb_get_spins(hb_ctx* c, float* sx, float* sy, float* sz) {
 
 int hb_sweep(hb_ctx* c, float T, int64_t n_sweeps) {
   HB_CHECK_CTX(c);
-  if (c->slab_Lz > 0) return fail(c, HB_ESTATE, "slab context: drive it with hb_slab_pass / hb_slab_next_sweep and exchange the faces (include/hb.h)");
+  if (c->slab_Lz > 0 || c->plan.part_total > 0) return fail(c, HB_ESTATE, "slab or part context: drive it with hb_slab_pass / hb_slab_next_sweep and the exchange step (include/hb.h)");
   if (n_sweeps < 0) return fail(c, HB_EINVAL, "n_sweeps < 0");
   if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
   float beta;
@@ -1005,7 +1029,9 @@ int hb_measure(hb_ctx* c, double M[3], double* E) {
   HB_CUDA(c, cudaMemcpyAsync(h, c->cached(), sizeof h, cudaMemcpyDeviceToHost, c->stream));
   HB_CUDA(c, cudaStreamSynchronize(c->stream));
   // a slab returns its share of M of the whole lattice (the kernel skipped the ghost planes)
-  const double inv = 1.0 / (c->slab_Lz > 0 ? (double)c->Lx * c->Ly * c->slab_Lz * (c->plan.engine == ENGINE_SC ? 1 : c->n_colours) : (double)c->plan.n);
+  // (a part of a table likewise: its own sites over the sites of the whole table)
+  const double inv = 1.0 / (c->slab_Lz > 0 ? (double)c->Lx * c->Ly * c->slab_Lz * (c->plan.engine == ENGINE_SC ? 1 : c->n_colours)
+                                           : (c->plan.part_total > 0 ? (double)c->plan.part_total : (double)c->plan.n));
   M[0] = h[0] * inv; M[1] = h[1] * inv; M[2] = h[2] * inv;
   *E = h[3];
   return HB_OK;
@@ -1013,7 +1039,7 @@ int hb_measure(hb_ctx* c, double M[3], double* E) {
 
 int hb_sweep_series(hb_ctx* c, float T, int64_t n_sweeps, double* M_series, double* E_series) {
   HB_CHECK_CTX(c);
-  if (c->slab_Lz > 0) return fail(c, HB_ESTATE, "slab context: drive it with hb_slab_pass / hb_slab_next_sweep and exchange the faces (include/hb.h)");
+  if (c->slab_Lz > 0 || c->plan.part_total > 0) return fail(c, HB_ESTATE, "slab or part context: drive it with hb_slab_pass / hb_slab_next_sweep and the exchange step (include/hb.h)");
   if (n_sweeps < 0 || !M_series || !E_series) return fail(c, HB_EINVAL, "bad series arguments");
   if (c->plan.R > 1) return fail(c, HB_EINVAL, "a context with replicas takes hb_sweep_series_each");
   if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
@@ -1060,7 +1086,7 @@ int hb_sweep_series(hb_ctx* c, float T, int64_t n_sweeps, double* M_series, doub
 
 int hb_sweep_record(hb_ctx* c, float T, uint8_t* accept) {
   HB_CHECK_CTX(c);
-  if (c->slab_Lz > 0) return fail(c, HB_ESTATE, "slab context: drive it with hb_slab_pass / hb_slab_next_sweep and exchange the faces (include/hb.h)");
+  if (c->slab_Lz > 0 || c->plan.part_total > 0) return fail(c, HB_ESTATE, "slab or part context: drive it with hb_slab_pass / hb_slab_next_sweep and the exchange step (include/hb.h)");
   if (!accept) return fail(c, HB_EINVAL, "NULL accept array");
   if (c->plan.R > 1) return fail(c, HB_EINVAL, "hb_sweep_record needs a context without replicas");
   if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
@@ -1169,13 +1195,19 @@ int hb_sweep_series_each(hb_ctx* c, const float* T, int64_t n_sweeps, double* M_
 // opposite of its global one: the sites of GLOBAL colour g are the local colour plane 1 - g.
 int hb_slab_pass(hb_ctx* c, float T, int32_t colour) {
   HB_CHECK_CTX(c);
-  if (c->slab_Lz <= 0) return fail(c, HB_ESTATE, "not a slab context");
+  if (c->slab_Lz <= 0 && c->plan.part_total <= 0) return fail(c, HB_ESTATE, "not a slab or part context");
   if (colour < 0 || colour >= c->n_colours) return fail(c, HB_EINVAL, "colour: 0 .. colours - 1 (sc: 0 or 1)");
   if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
   float beta;
   int rc = check_T(c, T, &beta);
   if (rc != HB_OK) return rc;
   c->cache_valid = false;
+  if (c->plan.part_total > 0) {   // a part of a neighbour table: the own sites of this colour
+    rc = one_colour(c, colour, params(c, beta), Diag{nullptr, nullptr});
+    if (rc != HB_OK) return rc;
+    c->attempts += (uint64_t)(c->colour_begin[colour + 1] - c->colour_begin[colour]);
+    return HB_OK;
+  }
   if (c->plan.engine == ENGINE_BRAVAIS) {   // colour = basis index, whatever the slab's offset
     rc = one_colour(c, colour, params(c, beta), Diag{nullptr, nullptr});
     if (rc != HB_OK) return rc;
@@ -1191,10 +1223,30 @@ int hb_slab_pass(hb_ctx* c, float T, int32_t colour) {
 
 int hb_slab_next_sweep(hb_ctx* c) {
   HB_CHECK_CTX(c);
-  if (c->slab_Lz <= 0) return fail(c, HB_ESTATE, "not a slab context");
+  if (c->slab_Lz <= 0 && c->plan.part_total <= 0) return fail(c, HB_ESTATE, "not a slab or part context");
   c->sweep += 1;
   return HB_OK;
 }
+
+// ---- parts of a neighbour table: the two halves of the exchange step ---------------------------------------------------------
+static int part_move(hb_ctx* c, const int32_t* ids, int64_t count, float* packed, bool gather) {
+  HB_CHECK_CTX(c);
+  if (c->plan.engine != ENGINE_CSR) return fail(c, HB_ESTATE, "hb_part_gather / hb_part_scatter: neighbour-table contexts (HB_CSR, or per-site anisotropy)");
+  if (count < 0 || count > c->plan.n || (count > 0 && (!ids || !packed))) return fail(c, HB_EINVAL, "hb_part_gather / hb_part_scatter: 0 <= count <= n_sites, device arrays");
+  if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
+  if (count == 0) return HB_OK;
+  if (!gather) c->cache_valid = false;
+  if (c->plan.ell) {
+    if (!c->ell.inv) return fail(c, HB_ESTATE, "hb_part_gather / hb_part_scatter on the ELL engine need a part context (hb_lattice.part_n_total > 0)");
+    HB_CUDA(c, launch_part_move_ell(c->stream, c->spins, c->ell.inv, ids, (uint32_t)count, packed, gather));
+  } else {
+    HB_CUDA(c, launch_part_move_flat(c->stream, c->spins, (uint32_t)c->plan.n, ids, (uint32_t)count, packed, gather));
+  }
+  c->launches += 1;
+  return HB_OK;
+}
+int hb_part_gather(hb_ctx* c, const int32_t* ids, int64_t count, float* out) { return part_move(c, ids, count, out, true); }
+int hb_part_scatter(hb_ctx* c, const int32_t* ids, int64_t count, const float* in) { return part_move(c, ids, count, const_cast<float*>(in), false); }
 
 int hb_slab_face(hb_ctx* c, int32_t colour, int32_t side, int32_t ghost, size_t offset_floats[3], size_t* count_floats) {
   HB_CHECK_CTX(c);

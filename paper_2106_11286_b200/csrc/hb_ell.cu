@@ -82,7 +82,7 @@ k_sweep_ell(float4* S, EllDev g, uint32_t begin, uint32_t count, SweepParams P, 
     site = (uint32_t)__ldcs(g.perm + m);
     o = S[m];
   }
-  const Rand4 r = philox4x32_10(site, 0u, P.sweep_lo, P.sweep_hi, P.seed_lo, P.seed_hi);
+  const Rand4 r = philox4x32_10(site + g.site_base, 0u, P.sweep_lo, P.sweep_hi, P.seed_lo, P.seed_hi);
   float nx, ny, nz;
   sphere(r.r0, r.r1, nx, ny, nz);
   const float dH = delta_h(o.x, o.y, o.z, nx, ny, nz, hx, hy, hz, P.J, K, ex, ey, ez);
@@ -117,10 +117,10 @@ k_measure_ell(const float4* __restrict__ S, EllDev g, SweepParams P, double* par
   block_reduce4(mx, my, mz, en, partials + (size_t)blockIdx.x * 4);
 }
 
-__global__ void k_init_random_perm(float4* S, const int32_t* __restrict__ perm, uint32_t n, uint32_t seed_lo, uint32_t seed_hi) {
+__global__ void k_init_random_perm(float4* S, const int32_t* __restrict__ perm, uint32_t n, uint32_t seed_lo, uint32_t seed_hi, uint32_t site_base) {
   for (unsigned long long m64 = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; m64 < n; m64 += (unsigned long long)gridDim.x * blockDim.x) {
     const uint32_t m = (uint32_t)m64;   // 64-bit loop index: a 32-bit one wraps below n when n is close to 2^32
-    const Rand4 r = philox4x32_10((uint32_t)perm[m], 1u, 0u, 0u, seed_lo, seed_hi);
+    const Rand4 r = philox4x32_10((uint32_t)perm[m] + site_base, 1u, 0u, 0u, seed_lo, seed_hi);
     float x, y, z;
     sphere(r.r0, r.r1, x, y, z);
     S[m] = make_float4(x, y, z, 0.0f);
@@ -137,6 +137,14 @@ __global__ void k_permute(float4* S, float* plane, const int32_t* __restrict__ p
   for (unsigned long long m64 = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; m64 < n; m64 += (unsigned long long)gridDim.x * blockDim.x) {
     const uint32_t m = (uint32_t)m64;   // 64-bit loop index: a 32-bit one wraps below n when n is close to 2^32
     if (to_internal) s[4 * (size_t)m + comp] = plane[perm[m]]; else plane[perm[m]] = s[4 * (size_t)m + comp];
+  }
+}
+
+// exchange step of table parts: the spins of the listed local sites <-> packed (x, y, z, 0) records
+__global__ void k_part_move_ell(float4* S, const int32_t* __restrict__ inv, const int32_t* __restrict__ ids, uint32_t count, float4* packed, bool gather) {
+  for (uint32_t k = blockIdx.x * blockDim.x + threadIdx.x; k < count; k += gridDim.x * blockDim.x) {
+    const int32_t m = inv[ids[k]];
+    if (gather) packed[k] = S[m]; else { const float4 v = packed[k]; S[m] = make_float4(v.x, v.y, v.z, 0.0f); }
   }
 }
 
@@ -181,8 +189,14 @@ cudaError_t launch_measure_ell(cudaStream_t st, const float* s, EllDev g, SweepP
   return launch_reduce_final(st, partials, grid, out);
 }
 
-cudaError_t launch_init_random_perm(cudaStream_t st, float* s, const int32_t* perm, uint32_t n, uint32_t seed_lo, uint32_t seed_hi) {
-  k_init_random_perm<<<grid_cap(n, 256, 148 * 16), 256, 0, st>>>(reinterpret_cast<float4*>(s), perm, n, seed_lo, seed_hi);
+cudaError_t launch_init_random_perm(cudaStream_t st, float* s, const int32_t* perm, uint32_t n, uint32_t seed_lo, uint32_t seed_hi, uint32_t site_base) {
+  k_init_random_perm<<<grid_cap(n, 256, 148 * 16), 256, 0, st>>>(reinterpret_cast<float4*>(s), perm, n, seed_lo, seed_hi, site_base);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_part_move_ell(cudaStream_t st, float* s, const int32_t* inv, const int32_t* ids, uint32_t count, float* packed, bool gather) {
+  if (count == 0) return cudaSuccess;
+  k_part_move_ell<<<grid_cap(count, 256, 148 * 8), 256, 0, st>>>(reinterpret_cast<float4*>(s), inv, ids, count, reinterpret_cast<float4*>(packed), gather);
   return cudaGetLastError();
 }
 

@@ -90,6 +90,8 @@ struct BrLayout {
 // CSR tables on the device
 struct CsrDev {
   uint32_t n;
+  uint32_t n_own;           // sites that are attempted and measured: n, or the own sites of a part (the rest are ghosts)
+  uint32_t site_base;       // Philox counter word of local site i is i + site_base (a part of a larger table; else 0)
   const int32_t* row_ptr;   // n+1
   const int32_t* col;       // nnz
   const int32_t* list;      // sites sorted by (colour, id)
@@ -104,7 +106,9 @@ struct CsrDev {
 struct EllDev {
   uint32_t n, maxdeg;
   const int32_t* ell;
-  const int32_t* perm;          // internal index -> canonical id (the Philox counter word)
+  const int32_t* perm;          // internal index -> canonical id (+ site_base: the Philox counter word)
+  uint32_t site_base;           // a part of a larger table: global id of local site 0; else 0
+  const int32_t* inv;           // canonical id -> internal index (parts only: hb_part_gather / scatter), or nullptr
   const uint32_t* colour_begin; // n_colours + 1 entries (device copy, for the measurement pass)
   int32_t n_colours;
   const float* K;               // per-site anisotropy in internal order, SoA; or nullptr
@@ -128,7 +132,7 @@ constexpr int kFusedBlocksMax = 16384;   // per colour: larger grids use the sep
 
 // ---- kernels (hb_kernels.cu); every launcher returns the launch status -----------------
 cudaError_t launch_init_random_sc(cudaStream_t st, float* spins, ScLayout L, uint32_t seed_lo, uint32_t seed_hi);
-cudaError_t launch_init_random_flat(cudaStream_t st, float* spins, uint32_t n, uint32_t seed_lo, uint32_t seed_hi);
+cudaError_t launch_init_random_flat(cudaStream_t st, float* spins, uint32_t n, uint32_t seed_lo, uint32_t seed_hi, uint32_t site_base = 0);
 cudaError_t launch_init_random_bravais(cudaStream_t st, float* spins, BrLayout L, uint32_t seed_lo, uint32_t seed_hi);
 cudaError_t launch_fill(cudaStream_t st, float* spins, uint32_t n, float x, float y, float z);
 cudaError_t launch_sc_permute(cudaStream_t st, float* dst, const float* src, ScLayout L, bool to_internal);
@@ -169,7 +173,11 @@ cudaError_t launch_sweep_csr(cudaStream_t st, float* spins, CsrDev g, uint32_t l
 cudaError_t launch_sweep_ell(cudaStream_t st, float* spins, EllDev g, uint32_t begin, uint32_t count, SweepParams p,
                              int block, Diag d);
 cudaError_t launch_measure_ell(cudaStream_t st, const float* spins, EllDev g, SweepParams p, double* partials, double* out);
-cudaError_t launch_init_random_perm(cudaStream_t st, float* spins, const int32_t* perm, uint32_t n, uint32_t seed_lo, uint32_t seed_hi);
+cudaError_t launch_init_random_perm(cudaStream_t st, float* spins, const int32_t* perm, uint32_t n, uint32_t seed_lo, uint32_t seed_hi, uint32_t site_base = 0);
+// exchange step of table parts (hb_part_gather / hb_part_scatter): spins of the listed local sites <-> packed (x, y, z, 0) records.
+// ELL engine: AoS state, ids translated through inv; CSR engine: three planes of n floats
+cudaError_t launch_part_move_ell(cudaStream_t st, float* spins, const int32_t* inv, const int32_t* ids, uint32_t count, float* packed, bool gather);
+cudaError_t launch_part_move_flat(cudaStream_t st, float* spins, uint32_t n, const int32_t* ids, uint32_t count, float* packed, bool gather);
 cudaError_t launch_fill_ell(cudaStream_t st, float* spins, uint32_t n, float x, float y, float z);
 // component comp of the internal float4 state <- plane[perm[m]] (to_internal) or plane[perm[m]] <- component
 cudaError_t launch_permute_ell(cudaStream_t st, float* spins, float* plane, const int32_t* perm, uint32_t n, int comp, bool to_internal);
@@ -207,8 +215,9 @@ void build_fcc_csr(int32_t Lx, int32_t Ly, int32_t Lz, HostCsr& out);
 void build_fcc_sphere_csr(int32_t R, HostCsr& out, std::vector<int32_t>& xyz);
 void greedy_first_fit(HostCsr& g);
 // empty string = valid; otherwise what is wrong
-std::string validate_csr(int64_t n, const int64_t* row_ptr, const int32_t* col);
+// n_own < n: a part of a larger table: sites n_own .. n-1 are ghosts (empty rows); symmetry is checked among the own sites
+std::string validate_csr(int64_t n, const int64_t* row_ptr, const int32_t* col, int64_t n_own = -1);
 std::string validate_colouring(int64_t n, const int64_t* row_ptr, const int32_t* col, const int32_t* colour,
-                               int32_t n_colours);
+                               int32_t n_colours, int64_t n_own = -1);
 
 }  // namespace hb

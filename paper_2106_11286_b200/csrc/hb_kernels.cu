@@ -275,7 +275,7 @@ k_sweep_csr(float* sx, float* sy, float* sz, CsrDev g, uint32_t list_begin, uint
     ez = __ldg(g.e_site + 3 * (size_t)i + 2);
   }
   float ox = sx[i], oy = sy[i], oz = sz[i];
-  const bool acc = attempt(i, P, K, ex, ey, ez, hx, hy, hz, ox, oy, oz);
+  const bool acc = attempt(i + g.site_base, P, K, ex, ey, ez, hx, hy, hz, ox, oy, oz);
   if (acc) { sx[i] = ox; sy[i] = oy; sz[i] = oz; }
   if (DIAG) {
     if (d.accept) d.accept[i] = acc;
@@ -349,13 +349,22 @@ __global__ void k_init_random_sc(float* sx, float* sy, float* sz, ScLayout L, ui
   }
 }
 
-__global__ void k_init_random_flat(float* sx, float* sy, float* sz, uint32_t n, uint32_t seed_lo, uint32_t seed_hi) {
+__global__ void k_init_random_flat(float* sx, float* sy, float* sz, uint32_t n, uint32_t seed_lo, uint32_t seed_hi, uint32_t site_base) {
   for (unsigned long long m64 = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; m64 < n; m64 += (unsigned long long)gridDim.x * blockDim.x) {
     const uint32_t m = (uint32_t)m64;   // 64-bit loop index: a 32-bit one wraps below n when n is close to 2^32
-    const Rand4 r = philox4x32_10(m, 1u, 0u, 0u, seed_lo, seed_hi);
+    const Rand4 r = philox4x32_10(m + site_base, 1u, 0u, 0u, seed_lo, seed_hi);
     float x, y, z;
     sphere(r.r0, r.r1, x, y, z);
     sx[m] = x; sy[m] = y; sz[m] = z;
+  }
+}
+
+// exchange step of table parts (CSR engine: three planes): the spins of the listed local sites <-> packed (x, y, z, 0) records
+__global__ void k_part_move_flat(float* sx, float* sy, float* sz, const int32_t* __restrict__ ids, uint32_t count, float4* packed, bool gather) {
+  for (uint32_t k = blockIdx.x * blockDim.x + threadIdx.x; k < count; k += gridDim.x * blockDim.x) {
+    const int32_t i = ids[k];
+    if (gather) packed[k] = make_float4(sx[i], sy[i], sz[i], 0.0f);
+    else { const float4 v = packed[k]; sx[i] = v.x; sy[i] = v.y; sz[i] = v.z; }
   }
 }
 
@@ -514,7 +523,7 @@ __global__ void __launch_bounds__(256)
 k_measure_csr(const float* __restrict__ sx, const float* __restrict__ sy, const float* __restrict__ sz,
               CsrDev g, SweepParams P, double* partials) {
   double mx = 0, my = 0, mz = 0, en = 0;
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += gridDim.x * blockDim.x) {
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < g.n_own; i += gridDim.x * blockDim.x) {   // (ghost sites of a part are not measured)
     const int32_t k0 = g.row_ptr[i], k1 = g.row_ptr[i + 1];
     float hx = 0.0f, hy = 0.0f, hz = 0.0f;
     for (int32_t k = k0; k < k1; ++k) {
@@ -550,8 +559,14 @@ cudaError_t launch_init_random_sc(cudaStream_t st, float* s, ScLayout L, uint32_
   return cudaGetLastError();
 }
 
-cudaError_t launch_init_random_flat(cudaStream_t st, float* s, uint32_t n, uint32_t seed_lo, uint32_t seed_hi) {
-  k_init_random_flat<<<grid_for(n, 256, 148 * 16), 256, 0, st>>>(s, s + n, s + 2 * (size_t)n, n, seed_lo, seed_hi);
+cudaError_t launch_init_random_flat(cudaStream_t st, float* s, uint32_t n, uint32_t seed_lo, uint32_t seed_hi, uint32_t site_base) {
+  k_init_random_flat<<<grid_for(n, 256, 148 * 16), 256, 0, st>>>(s, s + n, s + 2 * (size_t)n, n, seed_lo, seed_hi, site_base);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_part_move_flat(cudaStream_t st, float* s, uint32_t n, const int32_t* ids, uint32_t count, float* packed, bool gather) {
+  if (count == 0) return cudaSuccess;
+  k_part_move_flat<<<grid_for(count, 256, 148 * 8), 256, 0, st>>>(s, s + n, s + 2 * (size_t)n, ids, count, reinterpret_cast<float4*>(packed), gather);
   return cudaGetLastError();
 }
 

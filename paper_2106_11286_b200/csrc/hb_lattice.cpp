@@ -135,7 +135,8 @@ void greedy_first_fit(HostCsr& g) {
   g.n_colours = used;
 }
 
-std::string validate_csr(int64_t n, const int64_t* row_ptr, const int32_t* col) {
+std::string validate_csr(int64_t n, const int64_t* row_ptr, const int32_t* col, int64_t n_own) {
+  if (n_own < 0 || n_own > n) n_own = n;
   if (n < 0 || n > 0xFFFFFFFFll) return "n_sites out of range";
   if (!row_ptr) return "row_ptr is NULL";
   if (row_ptr[0] != 0) return "row_ptr[0] != 0";
@@ -149,6 +150,8 @@ std::string validate_csr(int64_t n, const int64_t* row_ptr, const int32_t* col) 
       if (j < 0 || j >= n) return "col_idx out of range";
       if (j == i) return "self loop";
     }
+  for (int64_t i = n_own; i < n; ++i)
+    if (row_ptr[i + 1] != row_ptr[i]) return "the row of a ghost site must be empty";
   // symmetric with multiplicity: #(j in row i) == #(i in row j).  Rows of bounded length are compared pair by pair
   // (O(sum of deg^2): lattices); a table with long rows (hubs) compares the sorted lists of (i, j) and (j, i) instead
   int64_t maxdeg = 0;
@@ -158,6 +161,7 @@ std::string validate_csr(int64_t n, const int64_t* row_ptr, const int32_t* col) 
     fwd.reserve((size_t)row_ptr[n]); rev.reserve((size_t)row_ptr[n]);
     for (int64_t i = 0; i < n; ++i)
       for (int64_t k = row_ptr[i]; k < row_ptr[i + 1]; ++k) {
+        if (col[k] >= n_own) continue;   // an edge into a ghost site has no counterpart here
         fwd.push_back(((uint64_t)i << 32) | (uint32_t)col[k]);
         rev.push_back(((uint64_t)(uint32_t)col[k] << 32) | (uint64_t)i);
       }
@@ -168,6 +172,7 @@ std::string validate_csr(int64_t n, const int64_t* row_ptr, const int32_t* col) 
   for (int64_t i = 0; i < n; ++i)
     for (int64_t k = row_ptr[i]; k < row_ptr[i + 1]; ++k) {
       const int64_t j = col[k];
+      if (j >= n_own) continue;   // an edge into a ghost site has no counterpart here
       int64_t a = 0, b = 0;
       for (int64_t q = row_ptr[i]; q < row_ptr[i + 1]; ++q) a += (col[q] == j);
       for (int64_t q = row_ptr[j]; q < row_ptr[j + 1]; ++q) b += (col[q] == i);
@@ -177,9 +182,12 @@ std::string validate_csr(int64_t n, const int64_t* row_ptr, const int32_t* col) 
 }
 
 std::string validate_colouring(int64_t n, const int64_t* row_ptr, const int32_t* col, const int32_t* colour,
-                               int32_t n_colours) {
+                               int32_t n_colours, int64_t n_own) {
   if (n_colours < 1 && n > 0) return "n_colours < 1";
-  for (int64_t i = 0; i < n; ++i) {
+  if (n_own < 0 || n_own > n) n_own = n;
+  for (int64_t i = n_own; i < n; ++i)
+    if (colour[i] < 0 || colour[i] >= n_colours) return "colour out of range";
+  for (int64_t i = 0; i < n_own; ++i) {
     if (colour[i] < 0 || colour[i] >= n_colours) return "colour out of range";
     for (int64_t k = row_ptr[i]; k < row_ptr[i + 1]; ++k)
       if (colour[col[k]] == colour[i]) return "two neighbouring sites share a colour";

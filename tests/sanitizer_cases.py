@@ -7,7 +7,7 @@ The paper's own scheme tolerates concurrent updates of neighbouring spins ("loss
 colour sweeps here claim to have no race at all, so the code most at risk for that claim runs under the tools: the
 mbarrier rings of the warp-specialised kernels (sc variants 2 / 4 / 5, bcc, fcc), their fused launches with progress
 words, the cooperative and one-block persistent kernels, replicas, the graph-replay path, slabs with peer stores, the
-table engines.  Every case is also checked against the oracle (the tools slow a kernel down, they do not change it).
+table engines, parts of a table.  Every case is also checked against the oracle (the tools slow a kernel down, they do not change it).
 Not collected by pytest (no test_ prefix): a plain script, so that the tool wraps ONE python process.
 """
 import os
@@ -94,6 +94,19 @@ def main():
         sl.close()
         print("%-44s %s" % ("3 slabs, peer stores, sc_kernel %d" % kern, "ok" if ok else "MISMATCH"), flush=True)
         good &= ok
+    # parts of a neighbour table: gather / scatter kernels between three contexts (ELL engine)
+    from paper_2106_11286_b200 import parts
+    plat = hb.Lattice.fcc_sphere(4, 0.05, (0, 0, 1), 0.5, "greedy")
+    P = parts.LocalParts(plat.row_ptr, plat.col_idx, plat.colour, 3, 1.0, 0.05, (0, 0, 1), 5, K_site=plat.K_site, e_site=plat.e_site)
+    st = oracle.State32(oracle.Lattice.fcc_sphere(4, 0.05, (0, 0, 1), 0.5, "greedy"), 1.0, 5)
+    P.init_random()
+    st.init_random()
+    P.sweep(2.0, 3)
+    st.sweep(2.0, 3)
+    ok = spins_equal(P.get_spins(), st.get_spins())
+    P.close()
+    print("%-44s %s" % ("3 parts of the sphere's table", "ok" if ok else "MISMATCH"), flush=True)
+    good &= ok
     print("ALL OK" if good else "FAILED", flush=True)
     return 0 if good else 1
 
