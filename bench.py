@@ -498,6 +498,8 @@ def main():
                 ctx.sweep(T, 8)
             kernels["hbm_traffic_folded_into_l2 (hb_probe_sc_l2)"] = max(f[1] for f in fold)
             kernels["default kernel beside the fold"] = max(f[0] for f in fold)
+            kernels["fold_note"] = ("short runs (40 sweeps) after the probes, near boost clock: there the HBM traffic costs nothing and the fold's "
+                                    "per-step address arithmetic shows; sustained at the power cap the fold gains 5-14 % (DESIGN.md section 7)")
         except Exception as exc:          # the fused launches need a row length the kernel takes
             kernels = {"unavailable": str(exc)}
 

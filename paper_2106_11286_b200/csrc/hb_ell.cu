@@ -142,7 +142,7 @@ __global__ void k_permute(float4* S, float* plane, const int32_t* __restrict__ p
 
 // exchange step of table parts: the spins of the listed local sites <-> packed (x, y, z, 0) records
 __global__ void k_part_move_ell(float4* S, const int32_t* __restrict__ inv, const int32_t* __restrict__ ids, uint32_t count, float4* packed, bool gather) {
-  for (uint32_t k = blockIdx.x * blockDim.x + threadIdx.x; k < count; k += gridDim.x * blockDim.x) {
+  for (unsigned long long k = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; k < count; k += (unsigned long long)gridDim.x * blockDim.x) {
     const int32_t m = inv[ids[k]];
     if (gather) packed[k] = S[m]; else { const float4 v = packed[k]; S[m] = make_float4(v.x, v.y, v.z, 0.0f); }
   }

@@ -361,7 +361,7 @@ __global__ void k_init_random_flat(float* sx, float* sy, float* sz, uint32_t n, 
 
 // exchange step of table parts (CSR engine: three planes): the spins of the listed local sites <-> packed (x, y, z, 0) records
 __global__ void k_part_move_flat(float* sx, float* sy, float* sz, const int32_t* __restrict__ ids, uint32_t count, float4* packed, bool gather) {
-  for (uint32_t k = blockIdx.x * blockDim.x + threadIdx.x; k < count; k += gridDim.x * blockDim.x) {
+  for (unsigned long long k = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; k < count; k += (unsigned long long)gridDim.x * blockDim.x) {
     const int32_t i = ids[k];
     if (gather) packed[k] = make_float4(sx[i], sy[i], sz[i], 0.0f);
     else { const float4 v = packed[k]; sx[i] = v.x; sy[i] = v.y; sz[i] = v.z; }
