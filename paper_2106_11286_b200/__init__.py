@@ -9,5 +9,5 @@ The work happens in libhb.so (C ABI: include/hb.h; CUDA kernels: csrc/).  Import
 package does not load the library; constructing a Context does, and raises if the
 library is not built or no CUDA device is present -- there is no CPU path.
 """
-from .binding import Context, HbError, Lattice, device_math, load_library, probe_alu, probe_pipe, sizes  # noqa: F401
+from .binding import Context, HbError, Lattice, device_math, load_library, measure_sc_noalloc, probe_alu, probe_pipe, sizes  # noqa: F401
 from . import workloads  # noqa: F401

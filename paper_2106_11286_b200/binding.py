@@ -21,6 +21,7 @@ EXPORTS = [
     "hb_device_alloc", "hb_device_free", "hb_ipc_export", "hb_ipc_open", "hb_ipc_close",
     "hb_get_colouring", "hb_counters", "hb_stats", "hb_device_math", "hb_probe_sc_l2", "hb_probe_pipe", "hb_sweep_paper_scheme", "hb_set_option", "hb_get_option", "hb_lattice_fcc_sphere", "hb_lattice_free",
     "hb_strerror", "hb_error_detail",
+    "hb_measure_sc_noalloc",     # include/hb_noalloc.h
 ]
 
 
@@ -104,6 +105,7 @@ def load_library():
         "hb_get_option": [vp, C.c_char_p, P(i64)],
         "hb_lattice_fcc_sphere": [i32, f32, P(f32), f32, i32, P(hb_lattice), P(vp)],
         "hb_lattice_free": [P(hb_lattice)],
+        "hb_measure_sc_noalloc": [vp, vp, vp, i32, i32, i32, f32, f32, P(f32), vp, vp, C.c_char_p, C.c_size_t],
     }
     for name, args in protos.items():
         fn = getattr(L, name)
@@ -234,6 +236,36 @@ def probe_pipe(kind, device="cuda:0"):
     if rc != 0:
         raise HbError(rc, "hb_probe_pipe", L.hb_strerror(rc).decode())
     return v.value
+
+
+NOALLOC_MAX_SITES = 4096 * 8192     # HB_NOALLOC_MAX_SITES of include/hb_noalloc.h
+
+
+def measure_sc_noalloc(sx, sy, sz, Lx, Ly, Lz, J, K, e, out, stream=None):
+    """hb_measure_sc_noalloc (include/hb_noalloc.h): M and E of a periodic simple cubic lattice from three CUDA float32
+    tensors in canonical site order, written into `out`, a CUDA float64 tensor of 4 elements (Mx, My, Mz, E), on `stream`
+    (default: torch's current stream of that device), without synchronising.
+
+    This is the call for code that must not allocate device memory where it runs: the library side neither calls
+    cudaMalloc nor needs a Context or a workspace, because its partial sums live in a 256 KiB array built into
+    libhb.so.  The wrapper keeps to that too: it allocates no tensor, the caller brings `out`.  The first call on
+    a device looks up that array's address, so make it during start-up.  All calls on one GPU share the array: keep
+    them on one stream.  Lattices of more than NOALLOC_MAX_SITES sites raise HbError with the limit in the message."""
+    import torch
+    L = load_library()
+    n = int(Lx) * int(Ly) * int(Lz)
+    for t in (sx, sy, sz):
+        assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.numel() == n and t.device == out.device
+    assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == 4
+    if stream is None:
+        stream = torch.cuda.current_stream(out.device)
+    err = C.create_string_buffer(512)
+    with torch.cuda.device(out.device):
+        rc = L.hb_measure_sc_noalloc(sx.data_ptr(), sy.data_ptr(), sz.data_ptr(), int(Lx), int(Ly), int(Lz), float(J), float(K),
+                                     _vec3(e), out.data_ptr(), stream.cuda_stream, err, len(err))
+    if rc != 0:
+        raise HbError(rc, "hb_measure_sc_noalloc", err.value.decode() or L.hb_strerror(rc).decode())
+    return out
 
 
 def sizes(lat):
