@@ -300,6 +300,11 @@ class DistSlab:
                 else:
                     exchange_dist(self.ctx, colour, self.rank, self.world, self.group)
             self.ctx.slab_next_sweep()
+        if self.peer_stores and self.flags and n_sweeps > 0:
+            # Flags order a pass only against the neighbours' NEXT pass.  Nothing on this rank's stream waits for the stores
+            # the neighbours' LAST pass makes into this slab's ghost planes, and measure() (boundary bonds) and the next
+            # ghost fill read those planes: one barrier per call closes the gap (include/hb.h, hb_slab_set_peer).
+            self._pass_barrier()
 
     def measure(self):
         """M and E of the WHOLE lattice on every rank (one all_reduce of 4 doubles)."""

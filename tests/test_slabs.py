@@ -317,3 +317,29 @@ def test_bcc_and_fcc_slabs_walk_the_single_lattice_trajectory(kind, shape, n_sla
     assert spins_equal(sl2.get_spins(), st.get_spins())
     sl.close()
     sl2.close()
+
+
+def test_flagged_sweeps_end_with_one_barrier_before_anything_reads_the_ghost_planes():
+    """Host logic only: with neighbour flags a pass is ordered against the neighbours' NEXT pass, so the stores
+    their LAST pass makes into this slab's ghost planes are ordered by nothing unless sweep() ends with a barrier.  A stub
+    context records the call order; no device, no process group."""
+    calls = []
+
+    class Ctx:
+        def slab_pass(self, T, colour):
+            calls.append(("pass", colour))
+
+        def slab_next_sweep(self):
+            calls.append(("next",))
+
+    for flags, want in ((True, [("pass", 0), ("pass", 1), ("next",)] * 3 + [("barrier",)]),
+                        (False, [("pass", 0), ("barrier",), ("pass", 1), ("barrier",), ("next",)] * 3)):
+        d = slabs.DistSlab.__new__(slabs.DistSlab)
+        d.ctx, d.n_colours, d.peer_stores, d.flags, d.world = Ctx(), 2, True, flags, 2
+        d._pass_barrier = lambda: calls.append(("barrier",))
+        del calls[:]
+        d.sweep(1.0, 3)
+        assert calls == want
+        del calls[:]
+        d.sweep(1.0, 0)
+        assert calls == []
