@@ -128,8 +128,8 @@ int hb_get_spins(hb_ctx* ctx, float* sx, float* sy, float* sz);
  * feeds a fresh state every step): hb_stage_spins starts the host->device copy of three canonical arrays (pinned host
  * memory, or the copy is not asynchronous) into a library-owned upload area of 3 n floats on a stream of its own and returns
  * at once; hb_commit_spins waits for that copy, then makes the staged state the context's state, in stream order with the
- * sweeps before and after it.  The host arrays must stay untouched until hb_commit_spins has returned.  Whole lattices
- * without replicas. */
+ * sweeps before and after it.  The host arrays must stay untouched until hb_commit_spins has returned.  One staged state
+ * at a time: a second hb_stage_spins before the commit returns HB_ESTATE.  Whole lattices without replicas. */
 int hb_stage_spins(hb_ctx* ctx, const float* sx, const float* sy, const float* sz);
 int hb_commit_spins(hb_ctx* ctx);
 
@@ -209,6 +209,18 @@ int hb_slab_face(hb_ctx* ctx, int32_t colour, int32_t side, int32_t ghost, size_
  * (stream order on one device; a collective or an event between devices).  The ghost planes must still be filled once
  * with hb_slab_face copies after hb_init_* / hb_set_spins.  peer_spins = NULL switches the side back to copies. */
 int hb_slab_set_peer(hb_ctx* ctx, int32_t side, void* peer_spins, int32_t peer_Lz);
+/* hb_set_option(ctx, "slab_flags", 1) (after hb_slab_set_peer on both sides; warp-specialised kernel) replaces that barrier by
+ * flags between neighbours, kept in the two words behind each slab's spins (so that a peer mapping of the spins buffer
+ * reaches them; hb_sizes counts them): colour pass number s of a slab takes its two boundary chunks first; a boundary tile
+ * waits (acquire at system scope) until the neighbour on its side has finished the boundary chunk of ITS pass s - 1, and the
+ * last warp of a boundary chunk writes s into that neighbour's flag (release at system scope) after the chunk's stores,
+ * the ones into the neighbour's ghost plane included.  Interior tiles never wait.  All slabs must issue the same sequence
+ * of hb_slab_pass calls, and the kernels of neighbouring slabs must be able to run at the same time (one GPU each) or in
+ * the order of the passes (one stream): two processes that share one GPU must not use it.
+ * With flags on, a pass is ordered only against the neighbours' NEXT pass: after the LAST pass of a run nothing on this
+ * slab's stream waits for the stores the neighbours' last pass makes into its ghost planes.  Before hb_measure (boundary
+ * bonds read the ghost planes), hb_get_spins on the ghost planes or hb_slab_face copies, the caller must synchronise with
+ * both neighbours once (a barrier across the slabs, as without flags); DistSlab.sweep does so at the end of every call. */
 /* Parts of a neighbour table (hb_lattice.part_n_total > 0; any HB_CSR context): the exchange step after a colour pass moves the
  * spins of listed sites.  hb_part_gather packs the spins of the `count` local sites ids[k] (DEVICE array of local ids) into
  * out[4 k .. 4 k + 3] = (x, y, z, 0) (DEVICE, 16-byte aligned); hb_part_scatter stores in[4 k .. 4 k + 2] as the spin of local
@@ -217,14 +229,6 @@ int hb_slab_set_peer(hb_ctx* ctx, int32_t side, void* peer_spins, int32_t peer_L
  * device); count = 0 is a no-op. */
 int hb_part_gather(hb_ctx* ctx, const int32_t* ids, int64_t count, float* out);
 int hb_part_scatter(hb_ctx* ctx, const int32_t* ids, int64_t count, const float* in);
-/* hb_set_option(ctx, "slab_flags", 1) (after hb_slab_set_peer on both sides; warp-specialised kernel) replaces that barrier by
- * flags between neighbours, kept in the two words behind each slab's spins (so that a peer mapping of the spins buffer
- * reaches them; hb_sizes counts them): colour pass number s of a slab takes its two boundary chunks first; a boundary tile
- * waits (acquire at system scope) until the neighbour on its side has finished the boundary chunk of ITS pass s - 1, and the
- * last warp of a boundary chunk writes s into that neighbour's flag (release at system scope) after the chunk's stores,
- * the ones into the neighbour's ghost plane included.  Interior tiles never wait.  All slabs must issue the same sequence
- * of hb_slab_pass calls, and the kernels of neighbouring slabs must be able to run at the same time (one GPU each) or in
- * the order of the passes (one stream): two processes that share one GPU must not use it. */
 
 /* Device memory that another process can map (one process per GPU, peer stores between slabs): hb_device_alloc is a
  * plain cudaMalloc on the current device (the result can be handed to hb_create in hb_buffers.spins), hb_ipc_export fills

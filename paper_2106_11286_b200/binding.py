@@ -373,8 +373,8 @@ class Context:
     def stage_spins(self, sx, sy, sz):
         """hb_stage_spins: start the upload of the next state (pinned torch CPU tensors) while the stream computes."""
         p = [self._host_ptr(a) for a in (sx, sy, sz)]
+        self._check(self._L.hb_stage_spins(self._h, p[0][0], p[1][0], p[2][0]), "hb_stage_spins")   # HB_ESTATE if one is pending
         self._staged = [q[1] for q in p]          # keep the host arrays alive until the commit
-        self._check(self._L.hb_stage_spins(self._h, p[0][0], p[1][0], p[2][0]), "hb_stage_spins")
 
     def commit_spins(self):
         self._check(self._L.hb_commit_spins(self._h), "hb_commit_spins")

@@ -322,10 +322,25 @@ int one_colour(hb_ctx* c, int colour, const SweepParams& p, Diag d, Meas m = Mea
   return HB_OK;
 }
 
+// The all-passes launch of the bcc / fcc warp-specialised kernel (br_kernel 2) marks progress in kWsDoneWords words, one per
+// (pass, chunk): a lattice with too many chunks along z runs one sweep per launch, and if that still does not fit, one
+// pass per launch (br_kernel 1), instead of failing in launch_sweep_bravais_ws.
+void clamp_bravais_ws(hb_ctx* c) {
+  if (c->plan.engine != ENGINE_BRAVAIS || c->br_kernel < 1) return;
+  const long long chunks = bravais_ws_chunks(c->br, c->br_zt, c->n_sms);
+  if ((long long)(c->n_colours * c->fused_sweeps - 1) * chunks > kWsDoneWords) c->fused_sweeps = 1;
+  if (c->br_kernel == 2 && (long long)(c->n_colours - 1) * chunks > kWsDoneWords) c->br_kernel = 1;
+}
+
 // blocks per colour launch if this context can fuse the measurement into its colour passes, else 0
 int fused_blocks(const hb_ctx* c) {
   if (!c->fused_measure) return 0;
-  if (c->plan.engine == ENGINE_BRAVAIS && c->br_kernel >= 1) return bravais_ws_blocks(c->br, c->br_zt, c->n_sms, c->br_kernel == 2 ? c->n_colours : 1);
+  if (c->plan.engine == ENGINE_BRAVAIS && c->br_kernel >= 1) {
+    const int fb = bravais_ws_blocks(c->br, c->br_zt, c->n_sms, c->br_kernel == 2 ? c->n_colours : 1);
+    // one launch per colour keeps n_colours sets of block partials side by side in a buffer of 2 kFusedBlocksMax blocks
+    // (sc_ws_ctas up to 4096 x 3 resident blocks x 4 colours would overrun it): such grids use the separate measurement pass
+    return (long long)c->n_colours * fb <= 2 * kFusedBlocksMax ? fb : 0;
+  }
   if (c->plan.engine == ENGINE_BRAVAIS) return bravais_fused_blocks(c->br, c->tile);
   if (c->plan.engine != ENGINE_SC) return 0;
   if (c->sc_kernel == 2) return sc_ws_fused_blocks(c->sc, c->fused_zt, c->n_sms, c->ws_variant, 1);
@@ -655,6 +670,7 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
         c->n_sms = sms;
       cudaGetLastError();
     }
+    clamp_bravais_ws(c);   // (needs n_sms: the chunk count depends on the grid)
   } else {
     c->n_colours = 2;
     c->sc.Lx = lat->Lx; c->sc.Ly = lat->Ly; c->sc.Lz = lat->Lz;
@@ -890,6 +906,8 @@ int hb_stage_spins(hb_ctx* c, const float* sx, const float* sy, const float* sz)
   HB_CHECK_CTX(c);
   if (!sx || !sy || !sz) return fail(c, HB_EINVAL, "NULL spin array");
   if (c->slab_Lz > 0 || c->plan.part_total > 0 || c->plan.R > 1) return fail(c, HB_EINVAL, "hb_stage_spins: whole lattices without replicas");
+  // a second upload would overwrite the area while the first may still be in flight from host arrays the caller no longer holds
+  if (c->stage_pending) return fail(c, HB_ESTATE, "hb_stage_spins: a staged state is waiting for hb_commit_spins");
   const size_t n = (size_t)c->plan.n;
   if (!c->stage) {
     if (cudaMalloc(reinterpret_cast<void**>(&c->stage), 3 * n * sizeof(float)) != cudaSuccess) { cudaGetLastError(); return fail(c, HB_ENOMEM, "hb_stage_spins: cudaMalloc of the upload area failed"); }
@@ -1439,7 +1457,7 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
       if (value < 0 || value > c->br.Lz) return fail(c, HB_EINVAL, "br_zt: 1..Lz planes per chunk, 0 = automatic");
       c->br_zt = (int)value;
     }
-    if ((long long)(c->n_colours * c->fused_sweeps - 1) * bravais_ws_chunks(c->br, c->br_zt, c->n_sms) > kWsDoneWords) c->fused_sweeps = 1;
+    clamp_bravais_ws(c);
     return HB_OK;
   }
   if (s == "csr_block") {
@@ -1453,7 +1471,7 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
     if (s == "sc_fused_sweeps") { if (value < 1 || value > 16) return fail(c, HB_EINVAL, "sc_fused_sweeps: 1..16 sweeps per launch"); c->fused_sweeps = (int)value; }
     else if (s == "sc_fused_lag") { if (value < 3 || value > 64) return fail(c, HB_EINVAL, "sc_fused_lag: 3..64 rounds between two colour passes"); c->fused_lag = (int)value; }
     else { if (value < 1 || value > 4096) return fail(c, HB_EINVAL, "sc_ws_ctas: 1..4096"); c->n_sms = (int)value; }
-    if ((long long)(c->n_colours * c->fused_sweeps - 1) * bravais_ws_chunks(c->br, c->br_zt, c->n_sms) > kWsDoneWords) c->fused_sweeps = 1;
+    clamp_bravais_ws(c);
     return HB_OK;
   }
   if (!is_sc && (s == "sc_kernel" || s == "sc_prefetch" || s == "sc_linear" || s == "sc_ws_zt" || s == "sc_ws_variant" || s == "sc_fused_zt"))

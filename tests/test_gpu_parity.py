@@ -992,6 +992,9 @@ def test_staged_upload_equals_set_spins(name):
         ctx.commit_spins()                         # nothing staged
     ctx.sweep(1.3, 5)                              # work in flight while the copy runs
     ctx.stage_spins(*host)
+    with pytest.raises(hb.HbError) as second:      # one staged state at a time: the area and the first host arrays are still in use
+        ctx.stage_spins(*host)
+    assert second.value.status == -4               # HB_ESTATE
     ctx.sweep(1.3, 3)
     ctx.commit_spins()
     assert spins_equal(ctx.get_spins(), target)
@@ -1006,3 +1009,45 @@ def test_staged_upload_equals_set_spins(name):
         ctx.commit_spins()
         assert spins_equal(ctx.get_spins(), st.get_spins())
     ctx.close()
+
+
+def test_long_fcc_lattice_runs_on_its_default_kernel_choice():
+    # hb_create picks the all-passes launch (br_kernel 2, 8 sweeps per launch) for fcc with Lx > 128 and
+    # >= 2^24 sites without checking its progress-word bound; a long thin lattice (31 * ceil(Lz / 16) > 16384 words) then
+    # failed in hb_sweep with HB_ECUDA.  The choice is clamped at create time now (one sweep per launch): the default
+    # context sweeps, and walks the trajectory of the direct kernel bit for bit.
+    cfg = dict(W.SMALL["c3"], L=(132, 4, 8452), start="random")
+    a, b = make_gpu(cfg), make_gpu(cfg)
+    assert a.get_option("br_kernel") == 2 and a.get_option("sc_fused_sweeps") == 1
+    b.set_option("br_kernel", 0)
+    for c in (a, b):
+        c.init_random()
+        c.sweep(1.1, 3)
+    assert spins_equal(a.get_spins(), b.get_spins())
+    Ma, Ea = a.measure()
+    Mb, Eb = b.measure()
+    assert np.max(np.abs(Ma - Mb)) <= 1e-7 and abs(Ea - Eb) <= 1e-6 * a.n
+    a.close()
+    b.close()
+
+
+def test_many_ctas_of_the_bcc_fcc_ws_kernel_do_not_overrun_the_block_partials():
+    # with sc_ws_ctas = 4096 a colour launch of the warp-specialised fcc kernel can have 12288 blocks; four
+    # colours of block partials side by side would overrun the buffer (32768 blocks) into the series / counter area.  Such
+    # grids now measure in the separate pass: M, E and the acceptance counters stay those of the default grid.
+    cfg = dict(W.SMALL["c3"], L=(64, 256, 260), start="random")    # 32 row groups x 260 one-plane chunks = 8320 blocks per colour
+    a, b = make_gpu(cfg), make_gpu(cfg)
+    for c, ctas in ((a, 4096), (b, 0)):
+        c.set_option("br_kernel", 1)
+        c.set_option("br_zt", 1)
+        if ctas:
+            c.set_option("sc_ws_ctas", ctas)
+        c.init_random()
+        c.sweep(1.1, 3)
+    Ma, Ea = a.measure()
+    Mb, Eb = b.measure()
+    assert spins_equal(a.get_spins(), b.get_spins())
+    assert np.max(np.abs(Ma - Mb)) <= 1e-7 and abs(Ea - Eb) <= 1e-6 * a.n
+    assert a.stats() == b.stats()
+    a.close()
+    b.close()
