@@ -1,4 +1,5 @@
-"""Thin ctypes binding of libhb.so (include/hb.h): argument marshalling only.
+"""Thin ctypes binding of libhb.so (include/hb.h; diagnostics and options: include/hb_diag.h; the call that never
+allocates: include/hb_noalloc.h): argument marshalling only.
 
 Every step of the hot path runs inside the CUDA library.  PyTorch supplies device
 memory and the stream.  There is no CPU fallback: if the library is missing or no
@@ -52,7 +53,7 @@ def library_path():
 
 
 def load_library():
-    """dlopen libhb.so and declare the prototypes of include/hb.h.  Fails loudly if it is not built."""
+    """dlopen libhb.so and declare the prototypes of include/*.h.  Fails loudly if it is not built."""
     global _lib
     if _lib is not None:
         return _lib
@@ -207,7 +208,7 @@ MATH_OPS = {"u01": (0, 2, 0), "sincos": (1, 2, 0), "sphere": (2, 6, 1), "exp": (
 
 
 def device_math(op, in0, in1=None, device="cuda:0"):
-    """hb_device_math: the device's building blocks of an attempt, element by element (include/hb.h).
+    """hb_device_math: the device's building blocks of an attempt, element by element (include/hb_diag.h).
     Returns a float32 array of shape (count, floats per element)."""
     import torch
     L = load_library()
@@ -496,7 +497,7 @@ class Context:
         return a.value, b.value
 
     def sweep_paper_scheme(self, T, n_mcs=1, n_per_block=8):
-        """hb_sweep_paper_scheme: the paper's own racy block scheme, emulated (context only; include/hb.h)."""
+        """hb_sweep_paper_scheme: the paper's own racy block scheme, emulated (context only; include/hb_diag.h)."""
         self._check(self._L.hb_sweep_paper_scheme(self._h, T, int(n_mcs), int(n_per_block)), "hb_sweep_paper_scheme")
 
     def probe_sc_l2(self, T, n_sweeps=50, planes=16):

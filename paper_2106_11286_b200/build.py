@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libhb.so")
 SOURCES = ["hb_api.cpp", "hb_lattice.cpp", "hb_kernels.cu", "hb_bravais.cu", "hb_bravais_ws.cu", "hb_ell.cu", "hb_sc_ws.cu", "hb_probe.cu", "hb_noalloc.cu"]
 HEADERS = ["hb_internal.h", "hb_device.cuh", "hb_ws.cuh", "hb_bravais_geo.cuh", os.path.join("..", "..", "include", "hb.h"),
-           os.path.join("..", "..", "include", "hb_noalloc.h")]
+           os.path.join("..", "..", "include", "hb_noalloc.h"), os.path.join("..", "..", "include", "hb_diag.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -3,10 +3,12 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <stdexcept>
 #include <string>
 #include <vector>
 
 #include "../../include/hb.h"
+#include "../../include/hb_diag.h"
 #include "hb_internal.h"
 
 using namespace hb;
@@ -77,6 +79,8 @@ int make_plan(const hb_lattice* lat, Plan& p, std::string& why) {
     }
   } else if (k == HB_CSR) {
     if (lat->n_sites < 0 || !lat->row_ptr) { why = "CSR lattice needs n_sites >= 0 and row_ptr"; return HB_EINVAL; }
+    // (before row_ptr is walked: an absurd n_sites must not send the loop below past the caller's array)
+    if (lat->n_sites > 0xFFFFFFFFll) { why = "more than 2^32-1 sites (site ids are 32-bit Philox counter words)"; return HB_EINVAL; }
     p.n = lat->n_sites;
     // the sizes below come from row_ptr: it must start at 0 and never decrease before anything is derived from it
     if (lat->row_ptr[0] != 0) { why = "row_ptr[0] must be 0"; return HB_EINVAL; }
@@ -543,9 +547,14 @@ int check_T(hb_ctx* c, float T, float* beta) {
 
 }  // namespace
 
+// include/hb.h promises that nothing throws across the C ABI, but the host side builds tables in std::vector / std::string
+// (a c5-size neighbour table is hundreds of megabytes): every entry point is a function-try-block that ends in HB_CATCH,
+// so that a failed host allocation comes back as HB_ENOMEM instead of std::terminate.  A context handed out by hb_create
+// before the exception stays valid for hb_error_detail / hb_destroy.
+#define HB_CATCH catch (const std::bad_alloc&) { return HB_ENOMEM; } catch (const std::length_error&) { return HB_ENOMEM; } catch (...) { return HB_EINVAL; }
 extern "C" {
 
-int hb_sizes(const hb_lattice* lat, int64_t* n_sites, size_t* spins_bytes, size_t* workspace_bytes) {
+int hb_sizes(const hb_lattice* lat, int64_t* n_sites, size_t* spins_bytes, size_t* workspace_bytes) try {
   Plan p;
   std::string why;
   if (!lat) return HB_EINVAL;
@@ -559,10 +568,10 @@ int hb_sizes(const hb_lattice* lat, int64_t* n_sites, size_t* spins_bytes, size_
   if (spins_bytes) *spins_bytes = p.spins_bytes;
   if (workspace_bytes) *workspace_bytes = p.ws_bytes;
   return HB_OK;
-}
+} HB_CATCH
 
 int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float e[3], uint64_t seed,
-              const hb_buffers* bufs) {
+              const hb_buffers* bufs) try {
   if (!out) return HB_EINVAL;
   *out = nullptr;
   hb_ctx* c = new (std::nothrow) hb_ctx;
@@ -805,9 +814,9 @@ int hb_create(hb_ctx** out, const hb_lattice* lat, float J, float K, const float
     HB_CUDA(c, cudaStreamSynchronize(c->stream));   // the host vectors die at return
   }
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_destroy(hb_ctx* c) {
+int hb_destroy(hb_ctx* c) try {
   if (!c) return HB_OK;
   for (int k = 0; k < 2; ++k) if (c->gexec[k]) cudaGraphExecDestroy(c->gexec[k]);
   if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
@@ -819,9 +828,9 @@ int hb_destroy(hb_ctx* c) {
   if (c->own_ws && c->ws) cudaFree(c->ws);
   delete c;
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_init_random(hb_ctx* c) {
+int hb_init_random(hb_ctx* c) try {
   HB_CHECK_CTX(c);
   c->cache_valid = false;
   c->each_valid = false;
@@ -845,9 +854,9 @@ int hb_init_random(hb_ctx* c) {
   c->launches += 1;
   c->initialised = true;
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_init_aligned(hb_ctx* c, const float dir[3]) {
+int hb_init_aligned(hb_ctx* c, const float dir[3]) try {
   HB_CHECK_CTX(c);
   if (!dir || !unit_vector(dir)) return fail(c, HB_EINVAL, "dir must be a unit vector");
   c->cache_valid = false;
@@ -864,9 +873,9 @@ int hb_init_aligned(hb_ctx* c, const float dir[3]) {
   c->launches += 1;
   c->initialised = true;
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_set_spins(hb_ctx* c, const float* sx, const float* sy, const float* sz) {
+int hb_set_spins(hb_ctx* c, const float* sx, const float* sy, const float* sz) try {
   HB_CHECK_CTX(c);
   c->cache_valid = false;
   if (!sx || !sy || !sz) return fail(c, HB_EINVAL, "NULL spin array");
@@ -899,10 +908,10 @@ int hb_set_spins(hb_ctx* c, const float* sx, const float* sy, const float* sz) {
   HB_CUDA(c, cudaStreamSynchronize(c->stream));   // the caller may reuse its arrays
   c->initialised = true;
   return HB_OK;
-}
+} HB_CATCH
 
 // ---- staged upload: the host->device copy of the NEXT state overlaps the sweeps of the current one ---------------------------
-int hb_stage_spins(hb_ctx* c, const float* sx, const float* sy, const float* sz) {
+int hb_stage_spins(hb_ctx* c, const float* sx, const float* sy, const float* sz) try {
   HB_CHECK_CTX(c);
   if (!sx || !sy || !sz) return fail(c, HB_EINVAL, "NULL spin array");
   if (c->slab_Lz > 0 || c->plan.part_total > 0 || c->plan.R > 1) return fail(c, HB_EINVAL, "hb_stage_spins: whole lattices without replicas");
@@ -923,9 +932,9 @@ int hb_stage_spins(hb_ctx* c, const float* sx, const float* sy, const float* sz)
   HB_CUDA(c, cudaEventRecord(c->stage_filled, c->stage_stream));
   c->stage_pending = true;
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_commit_spins(hb_ctx* c) {
+int hb_commit_spins(hb_ctx* c) try {
   HB_CHECK_CTX(c);
   if (!c->stage_pending) return fail(c, HB_ESTATE, "hb_commit_spins without a staged state (hb_stage_spins)");
   HB_CUDA(c, cudaEventSynchronize(c->stage_filled));                     // the caller may reuse its host arrays after this call
@@ -946,9 +955,9 @@ int hb_commit_spins(hb_ctx* c) {
   c->stage_pending = false;
   c->initialised = true;
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_get_spins(hb_ctx* c, float* sx, float* sy, float* sz) {
+int hb_get_spins(hb_ctx* c, float* sx, float* sy, float* sz) try {
   HB_CHECK_CTX(c);
   if (!sx || !sy || !sz) return fail(c, HB_EINVAL, "NULL spin array");
   if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
@@ -975,9 +984,9 @@ int hb_get_spins(hb_ctx* c, float* sx, float* sy, float* sz) {
   }
   HB_CUDA(c, cudaStreamSynchronize(c->stream));
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_sweep(hb_ctx* c, float T, int64_t n_sweeps) {
+int hb_sweep(hb_ctx* c, float T, int64_t n_sweeps) try {
   HB_CHECK_CTX(c);
   if (c->slab_Lz > 0 || c->plan.part_total > 0) return fail(c, HB_ESTATE, "slab or part context: drive it with hb_slab_pass / hb_slab_next_sweep and the exchange step (include/hb.h)");
   if (n_sweeps < 0) return fail(c, HB_EINVAL, "n_sweeps < 0");
@@ -1022,9 +1031,9 @@ int hb_sweep(hb_ctx* c, float T, int64_t n_sweeps) {
   }
   if (fuse && n_sweeps > 0) c->cache_valid = true;
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_measure(hb_ctx* c, double M[3], double* E) {
+int hb_measure(hb_ctx* c, double M[3], double* E) try {
   HB_CHECK_CTX(c);
   if (!M || !E) return fail(c, HB_EINVAL, "NULL output");
   if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
@@ -1053,9 +1062,9 @@ int hb_measure(hb_ctx* c, double M[3], double* E) {
   M[0] = h[0] * inv; M[1] = h[1] * inv; M[2] = h[2] * inv;
   *E = h[3];
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_sweep_series(hb_ctx* c, float T, int64_t n_sweeps, double* M_series, double* E_series) {
+int hb_sweep_series(hb_ctx* c, float T, int64_t n_sweeps, double* M_series, double* E_series) try {
   HB_CHECK_CTX(c);
   if (c->slab_Lz > 0 || c->plan.part_total > 0) return fail(c, HB_ESTATE, "slab or part context: drive it with hb_slab_pass / hb_slab_next_sweep and the exchange step (include/hb.h)");
   if (n_sweeps < 0 || !M_series || !E_series) return fail(c, HB_EINVAL, "bad series arguments");
@@ -1100,9 +1109,9 @@ int hb_sweep_series(hb_ctx* c, float T, int64_t n_sweeps, double* M_series, doub
     }
   }
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_sweep_record(hb_ctx* c, float T, uint8_t* accept) {
+int hb_sweep_record(hb_ctx* c, float T, uint8_t* accept) try {
   HB_CHECK_CTX(c);
   if (c->slab_Lz > 0 || c->plan.part_total > 0) return fail(c, HB_ESTATE, "slab or part context: drive it with hb_slab_pass / hb_slab_next_sweep and the exchange step (include/hb.h)");
   if (!accept) return fail(c, HB_EINVAL, "NULL accept array");
@@ -1119,14 +1128,14 @@ int hb_sweep_record(hb_ctx* c, float T, uint8_t* accept) {
   HB_CUDA(c, cudaMemcpyAsync(accept, d_acc, (size_t)c->plan.n, cudaMemcpyDeviceToHost, c->stream));
   HB_CUDA(c, cudaStreamSynchronize(c->stream));
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_select_replica(hb_ctx* c, int32_t replica) {
+int hb_select_replica(hb_ctx* c, int32_t replica) try {
   HB_CHECK_CTX(c);
   if (replica < 0 || replica >= c->plan.R) return fail(c, HB_EINVAL, "replica out of range");
   select_replica(c, replica);
   return HB_OK;
-}
+} HB_CATCH
 
 static int betas_of(hb_ctx* c, const float* T, std::vector<float>& beta) {
   if (!T) return fail(c, HB_EINVAL, "NULL temperature array");
@@ -1138,7 +1147,7 @@ static int betas_of(hb_ctx* c, const float* T, std::vector<float>& beta) {
   return HB_OK;
 }
 
-int hb_sweep_each(hb_ctx* c, const float* T, int64_t n_sweeps) {
+int hb_sweep_each(hb_ctx* c, const float* T, int64_t n_sweeps) try {
   HB_CHECK_CTX(c);
   if (n_sweeps < 0) return fail(c, HB_EINVAL, "n_sweeps < 0");
   if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
@@ -1151,9 +1160,9 @@ int hb_sweep_each(hb_ctx* c, const float* T, int64_t n_sweeps) {
   rc = replica_sweeps(c, beta.data(), n_sweeps, nullptr);
   if (rc == HB_OK) c->each_valid = true;
   return rc;
-}
+} HB_CATCH
 
-int hb_measure_each(hb_ctx* c, double* M, double* E) {
+int hb_measure_each(hb_ctx* c, double* M, double* E) try {
   HB_CHECK_CTX(c);
   if (!M || !E) return fail(c, HB_EINVAL, "NULL output");
   if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
@@ -1177,9 +1186,9 @@ int hb_measure_each(hb_ctx* c, double* M, double* E) {
     E[r] = h[4 * r + 3];
   }
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_sweep_series_each(hb_ctx* c, const float* T, int64_t n_sweeps, double* M_series, double* E_series) {
+int hb_sweep_series_each(hb_ctx* c, const float* T, int64_t n_sweeps, double* M_series, double* E_series) try {
   HB_CHECK_CTX(c);
   if (n_sweeps < 0 || !M_series || !E_series) return fail(c, HB_EINVAL, "bad series arguments");
   if (!c->initialised) return fail(c, HB_ESTATE, "spins not initialised");
@@ -1206,12 +1215,12 @@ int hb_sweep_series_each(hb_ctx* c, const float* T, int64_t n_sweeps, double* M_
       }
   }
   return HB_OK;
-}
+} HB_CATCH
 
 // ---- slabs (include/hb.h) -------------------------------------------------------------------
 // Local plane z_l holds global plane slab_z0 + z_l - 1 and slab_z0 is even, so the parity of a local plane is the
 // opposite of its global one: the sites of GLOBAL colour g are the local colour plane 1 - g.
-int hb_slab_pass(hb_ctx* c, float T, int32_t colour) {
+int hb_slab_pass(hb_ctx* c, float T, int32_t colour) try {
   HB_CHECK_CTX(c);
   if (c->slab_Lz <= 0 && c->plan.part_total <= 0) return fail(c, HB_ESTATE, "not a slab or part context");
   if (colour < 0 || colour >= c->n_colours) return fail(c, HB_EINVAL, "colour: 0 .. colours - 1 (sc: 0 or 1)");
@@ -1237,14 +1246,14 @@ int hb_slab_pass(hb_ctx* c, float T, int32_t colour) {
   if (rc != HB_OK) return rc;
   c->attempts += (uint64_t)c->sc.Lx * c->sc.Ly * (uint64_t)(c->sc.Lz - 2) / 2;
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_slab_next_sweep(hb_ctx* c) {
+int hb_slab_next_sweep(hb_ctx* c) try {
   HB_CHECK_CTX(c);
   if (c->slab_Lz <= 0 && c->plan.part_total <= 0) return fail(c, HB_ESTATE, "not a slab or part context");
   c->sweep += 1;
   return HB_OK;
-}
+} HB_CATCH
 
 // ---- parts of a neighbour table: the two halves of the exchange step ---------------------------------------------------------
 static int part_move(hb_ctx* c, const int32_t* ids, int64_t count, float* packed, bool gather) {
@@ -1263,10 +1272,10 @@ static int part_move(hb_ctx* c, const int32_t* ids, int64_t count, float* packed
   c->launches += 1;
   return HB_OK;
 }
-int hb_part_gather(hb_ctx* c, const int32_t* ids, int64_t count, float* out) { return part_move(c, ids, count, out, true); }
-int hb_part_scatter(hb_ctx* c, const int32_t* ids, int64_t count, const float* in) { return part_move(c, ids, count, const_cast<float*>(in), false); }
+int hb_part_gather(hb_ctx* c, const int32_t* ids, int64_t count, float* out) try { return part_move(c, ids, count, out, true); } HB_CATCH
+int hb_part_scatter(hb_ctx* c, const int32_t* ids, int64_t count, const float* in) try { return part_move(c, ids, count, const_cast<float*>(in), false); } HB_CATCH
 
-int hb_slab_face(hb_ctx* c, int32_t colour, int32_t side, int32_t ghost, size_t offset_floats[3], size_t* count_floats) {
+int hb_slab_face(hb_ctx* c, int32_t colour, int32_t side, int32_t ghost, size_t offset_floats[3], size_t* count_floats) try {
   HB_CHECK_CTX(c);
   if (c->slab_Lz <= 0) return fail(c, HB_ESTATE, "not a slab context");
   if (colour < 0 || colour >= c->n_colours || ((side | ghost) & ~1)) return fail(c, HB_EINVAL, "colour: 0 .. colours - 1; side, ghost: 0 or 1");
@@ -1284,9 +1293,9 @@ int hb_slab_face(hb_ctx* c, int32_t colour, int32_t side, int32_t ghost, size_t 
     offset_floats[k] = (size_t)k * c->sc.n + (size_t)(1 - colour) * c->sc.half + (size_t)z * plane;
   *count_floats = plane;
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_slab_set_peer(hb_ctx* c, int32_t side, void* peer_spins, int32_t peer_Lz) {
+int hb_slab_set_peer(hb_ctx* c, int32_t side, void* peer_spins, int32_t peer_Lz) try {
   HB_CHECK_CTX(c);
   if (c->slab_Lz <= 0) return fail(c, HB_ESTATE, "not a slab context");
   if (c->plan.engine != ENGINE_SC) return fail(c, HB_EINVAL, "peer stores exist for simple cubic slabs; bcc / fcc slabs exchange faces (hb_slab_face)");
@@ -1304,21 +1313,21 @@ int hb_slab_set_peer(hb_ctx* c, int32_t side, void* peer_spins, int32_t peer_Lz)
                                     : nullptr;
   if (!peer_spins) c->sc.flag_in = nullptr;   // flags need peer stores on both sides
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_sweep_count(hb_ctx* c, uint64_t* out) {
+int hb_sweep_count(hb_ctx* c, uint64_t* out) try {
   if (!c || !out) return HB_EINVAL;
   *out = c->sweep;
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_set_sweep_count(hb_ctx* c, uint64_t value) {
+int hb_set_sweep_count(hb_ctx* c, uint64_t value) try {
   if (!c) return HB_EINVAL;
   c->sweep = value;
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_get_colouring(hb_ctx* c, int32_t* colour, int32_t* n_colours) {
+int hb_get_colouring(hb_ctx* c, int32_t* colour, int32_t* n_colours) try {
   HB_CHECK_CTX(c);
   if (c->slab_Lz > 0) return fail(c, HB_ESTATE, "slab context: the colour of a site is (x + y + z) mod 2 in global coordinates");
   if (n_colours) *n_colours = c->n_colours;
@@ -1333,16 +1342,16 @@ int hb_get_colouring(hb_ctx* c, int32_t* colour, int32_t* n_colours) {
     std::memcpy(colour, c->colour_host.data(), c->colour_host.size() * sizeof(int32_t));
   }
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_counters(hb_ctx* c, uint64_t* kernel_launches, uint64_t* attempts) {
+int hb_counters(hb_ctx* c, uint64_t* kernel_launches, uint64_t* attempts) try {
   if (!c) return HB_EINVAL;
   if (kernel_launches) *kernel_launches = c->launches;
   if (attempts) *attempts = c->attempts;
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_sweep_paper_scheme(hb_ctx* c, float T, int64_t n_mcs, int32_t n_per_block) {
+int hb_sweep_paper_scheme(hb_ctx* c, float T, int64_t n_mcs, int32_t n_per_block) try {
   HB_CHECK_CTX(c);
   if (c->plan.engine != ENGINE_SC || c->slab_Lz > 0 || c->plan.R > 1) return fail(c, HB_EINVAL, "hb_sweep_paper_scheme: a whole simple cubic lattice without replicas");
   if (n_mcs < 0 || n_per_block < 1 || n_per_block > 65536 || c->plan.n % n_per_block) return fail(c, HB_EINVAL, "hb_sweep_paper_scheme: n_mcs >= 0, 1 <= n_per_block <= 65536 dividing the number of sites");
@@ -1364,9 +1373,9 @@ int hb_sweep_paper_scheme(hb_ctx* c, float T, int64_t n_mcs, int32_t n_per_block
     c->stat_attempts += (uint64_t)c->plan.n;
   }
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_probe_sc_l2(hb_ctx* c, float T, int64_t n_sweeps, int32_t planes, double* updates_per_second) {
+int hb_probe_sc_l2(hb_ctx* c, float T, int64_t n_sweeps, int32_t planes, double* updates_per_second) try {
   HB_CHECK_CTX(c);
   if (!updates_per_second || n_sweeps < 1 || n_sweeps > 100000) return fail(c, HB_EINVAL, "hb_probe_sc_l2: 1 <= n_sweeps <= 100000, non-NULL output");
   if (c->plan.engine != ENGINE_SC || c->slab_Lz > 0 || c->plan.R > 1 || !sc_ws_variant_supported(c->sc, 4) || planes < 2 ||
@@ -1398,9 +1407,9 @@ int hb_probe_sc_l2(hb_ctx* c, float T, int64_t n_sweeps, int32_t planes, double*
   if (e != cudaSuccess) return fail(c, HB_ECUDA, std::string("hb_probe_sc_l2: ") + cudaGetErrorString(e));
   *updates_per_second = (double)c->plan.n * (double)n_sweeps / ((double)ms * 1e-3);
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_stats(hb_ctx* c, uint64_t* attempts, uint64_t* accepts) {
+int hb_stats(hb_ctx* c, uint64_t* attempts, uint64_t* accepts) try {
   HB_CHECK_CTX(c);
   if (!attempts || !accepts) return fail(c, HB_EINVAL, "NULL output");
   unsigned long long acc = 0;
@@ -1409,9 +1418,9 @@ int hb_stats(hb_ctx* c, uint64_t* attempts, uint64_t* accepts) {
   *attempts = c->stat_attempts;
   *accepts = (uint64_t)acc;
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
+int hb_set_option(hb_ctx* c, const char* name, int64_t value) try {
   HB_CHECK_CTX(c);
   if (!name) return HB_EINVAL;
   const std::string s(name);
@@ -1536,9 +1545,9 @@ int hb_set_option(hb_ctx* c, const char* name, int64_t value) {
     return fail(c, HB_EINVAL, "sc tile: JX, TY, ZT >= 1, JX*TY <= 256 (1024 for sc with V = 4), ZT <= Lz");
   c->tile = t;
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_get_option(hb_ctx* c, const char* name, int64_t* value) {
+int hb_get_option(hb_ctx* c, const char* name, int64_t* value) try {
   if (!c || !name || !value) return HB_EINVAL;
   const std::string s(name);
   if (s == "csr_block") *value = c->csr_block;
@@ -1568,10 +1577,10 @@ int hb_get_option(hb_ctx* c, const char* name, int64_t* value) {
   else if (s == "br_zt") *value = c->br_zt;
   else return HB_EINVAL;
   return HB_OK;
-}
+} HB_CATCH
 
 int hb_lattice_fcc_sphere(int32_t R, float K_core, const float e_core[3], float K_surf, int32_t colouring,
-                          hb_lattice* out, int32_t** xyz_out) {
+                          hb_lattice* out, int32_t** xyz_out) try {
   if (!out || !e_core || R < 0 || R > 200 || (colouring != 0 && colouring != 1)) return HB_EINVAL;
   HostCsr g;
   std::vector<int32_t> xyz;
@@ -1615,9 +1624,9 @@ int hb_lattice_fcc_sphere(int32_t R, float K_core, const float e_core[3], float 
   out->kind = HB_CSR; out->n_sites = g.n; out->row_ptr = rp; out->col_idx = ci;
   out->n_colours = g.n_colours; out->colour = cc; out->K_site = Ks; out->e_site = es;
   return HB_OK;
-}
+} HB_CATCH
 
-int hb_lattice_free(hb_lattice* lat) {
+int hb_lattice_free(hb_lattice* lat) try {
   if (!lat) return HB_OK;
   std::free(const_cast<int64_t*>(lat->row_ptr));
   std::free(const_cast<int32_t*>(lat->col_idx));
@@ -1626,7 +1635,7 @@ int hb_lattice_free(hb_lattice* lat) {
   std::free(const_cast<float*>(lat->e_site));
   std::memset(lat, 0, sizeof *lat);
   return HB_OK;
-}
+} HB_CATCH
 
 const char* hb_strerror(int status) {
   switch (status) {

@@ -10,6 +10,7 @@
 #include <new>
 
 #include "../../include/hb.h"
+#include "../../include/hb_diag.h"
 #include "hb_device.cuh"
 #include "hb_internal.h"
 

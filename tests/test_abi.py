@@ -220,3 +220,39 @@ def test_product_never_imports_the_oracle():
                 assert not re.search(r"^\s*(import|from)\s+paper_2106_11286_b200\b", text, flags=re.M), fn
                 assert not re.search(r"#\s*include\s*[\"<][^\">]*(hb\.h|hb_internal\.h|hb_device\.cuh)", text), fn
                 assert "libhb.so" not in text, fn
+
+
+def test_absurd_table_size_is_refused_before_the_table_is_read():
+    """A CSR description of 2^40 sites: HB_EINVAL from hb_sizes and hb_create, without walking row_ptr past the caller's array."""
+    lib = hb.load_library()
+    rp = np.zeros(4, np.int64)
+    lat = binding.hb_lattice()
+    lat.kind, lat.n_sites = binding.HB_CSR, 2 ** 40
+    lat.row_ptr = rp.ctypes.data_as(C.c_void_p)
+    n, a, b = C.c_int64(), C.c_size_t(), C.c_size_t()
+    assert lib.hb_sizes(C.byref(lat), C.byref(n), C.byref(a), C.byref(b)) == -1
+    h = C.c_void_p()
+    assert lib.hb_create(C.byref(h), C.byref(lat), 1.0, 0.0, (C.c_float * 3)(0, 0, 1), 1, None) == -1
+    assert b"2^32" in lib.hb_error_detail(h)
+    lib.hb_destroy(h)
+
+
+def test_a_failed_host_allocation_comes_back_as_a_status_not_as_an_abort():
+    """include/hb.h: nothing throws or aborts.  The host side builds tables in std::vector; with the address space of a child
+    process capped, the sphere builder at its largest radius (1.3 x 10^8 sites, gigabytes of tables) runs out of memory and
+    must return HB_ENOMEM -- before the entry points caught at the boundary this ended in std::terminate (SIGABRT)."""
+    import subprocess
+    import sys
+    code = (
+        "import ctypes as C, resource, sys\n"
+        "lib = C.CDLL(%r)\n"
+        "resource.setrlimit(resource.RLIMIT_AS, (3 << 29, 3 << 29))\n"       # 1.5 GiB
+        "class L(C.Structure):\n"
+        "    _fields_ = [('b', C.c_char * 256)]\n"
+        "out, xyz = L(), C.c_void_p()\n"
+        "lib.hb_lattice_fcc_sphere.argtypes = [C.c_int32, C.c_float, C.POINTER(C.c_float), C.c_float, C.c_int32, C.c_void_p, C.c_void_p]\n"
+        "rc = lib.hb_lattice_fcc_sphere(200, 0.0, (C.c_float * 3)(0, 0, 1), 0.0, 1, C.byref(out), C.byref(xyz))\n"
+        "print('rc', rc)\n" % binding.library_path())
+    res = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=300)
+    assert res.returncode == 0, (res.returncode, res.stderr[-400:])
+    assert "rc -2" in res.stdout, res.stdout
