@@ -968,8 +968,14 @@ def test_paper_scheme_emulation_statistics():
         se_e = math.sqrt(g_e.var(ddof=1) / reps + o_e.var(ddof=1) / reps)
         print("paper scheme n = %d: |M| %.5f (o64 %.5f, diff %+.1e, se %.1e)  E/N %.5f (o64 %.5f, diff %+.1e, se %.1e)" %
               (n_per_block, g_m.mean(), o_m.mean(), dm, se_m, g_e.mean(), o_e.mean(), de, se_e))
-        if n_per_block >= 8:      # racy and therefore not reproducible run to run: a loose bound (measured +6e-3 +- 3e-3 in E/N at n = 8)
-            assert abs(dm) <= 0.02 and abs(de) <= 0.025, (n_per_block, dm, de)
+        if n_per_block >= 8:
+            # The emulation is racy by the paper's own account [P:32], so its bias is a property of the scheme, not a parity
+            # figure; the bound is the bias measured on B200s (n = 8: +6.4e-3 in E/N, +2e-3 in |M|; n = 64: +3e-3 +- 3e-3, taken as 1e-3;
+            # DESIGN.md 4b) plus 4 standard errors of THIS run's two replica sets (se ~ 2.5e-3 each): ~0.016, where the
+            # n = 1 limit sits at +0.17.  A materially worse emulation (a scheme that lets more neighbours move at once)
+            # lands between the two and fails.
+            bias_e, bias_m = (6e-3, 2e-3) if n_per_block == 8 else (1e-3, 1e-3)
+            assert abs(de) <= bias_e + 4.0 * se_e and abs(dm) <= bias_m + 4.0 * se_m, (n_per_block, dm, se_m, de, se_e)
         else:                     # n = 1: every spin moves against stale neighbours: the bias is an order of magnitude larger
             assert de > 0.05, (n_per_block, de)
     with pytest.raises(hb.HbError):
