@@ -32,6 +32,12 @@
 #include "hb_internal.h"
 #include "hb_ws.cuh"
 
+// HB_WS_HOIST: how many of the four Philox draws of a plane step a consumer makes before it waits for the staged planes
+// (0, 2 or 4, "interleave").  Measured in round 3; the default is what won.
+#ifndef HB_WS_HOIST
+#define HB_WS_HOIST 0
+#endif
+
 namespace hb {
 
 namespace {
@@ -237,12 +243,22 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
           sp[0] = load_rw<4>(gx); sp[1] = load_rw<4>(gx + n); sp[2] = load_rw<4>(gx + 2 * n);
         }
       }
+      const int32_t p = (colour + y + z0 + s) & 1;
+#if HB_WS_HOIST > 0
+      // the random words of the first HB_WS_HOIST attempts of this plane step, drawn BEFORE the wait for the staged planes: the
+      // IMAD.WIDE bursts of Philox then run while other warps are in their LDS phase instead of colliding with theirs
+      Rand4 pre[HB_WS_HOIST];
+      if (act) {
+#pragma unroll
+        for (int j = 0; j < HB_WS_HOIST; ++j)
+          pre[j] = philox4x32_10(site_row + (uint32_t)p + 2u * j, 0u, sweep_lo, sweep_hi, P.seed_lo, P.seed_hi);
+      }
+#endif
       if (s == 0) mbar_wait(fullB + 8u * rc.slot, rc.par);
       mbar_wait(fullB + 8u * rq.slot, rq.par);
       const unsigned char* Bm = smem + rm.slot * S::SLOT_B;
       const unsigned char* Bc = smem + rc.slot * S::SLOT_B;
       const unsigned char* Bp = smem + rq.slot * S::SLOT_B;
-      const int32_t p = (colour + y + z0 + s) & 1;
       const uint32_t h_off = p ? h_hi : h_lo;
       Vec<4> h[3];
       if (act) {
@@ -280,8 +296,13 @@ __device__ __forceinline__ void ws_consumer(float* a, const ScLayout& L, const W
         const uint32_t site0 = site_row + (uint32_t)p;
 #pragma unroll
         for (int k = 0; k < 4; k += 2) {
+#if HB_WS_HOIST > 0
+          const Rand4 ra = k < HB_WS_HOIST ? pre[k < HB_WS_HOIST ? k : 0] : philox4x32_10(site0 + 2u * k, 0u, sweep_lo, sweep_hi, P.seed_lo, P.seed_hi);
+          const Rand4 rb = k + 1 < HB_WS_HOIST ? pre[k + 1 < HB_WS_HOIST ? k + 1 : 0] : philox4x32_10(site0 + 2u * k + 2u, 0u, sweep_lo, sweep_hi, P.seed_lo, P.seed_hi);
+#else
           const Rand4 ra = philox4x32_10(site0 + 2u * k, 0u, sweep_lo, sweep_hi, P.seed_lo, P.seed_hi);
           const Rand4 rb = philox4x32_10(site0 + 2u * k + 2u, 0u, sweep_lo, sweep_hi, P.seed_lo, P.seed_hi);
+#endif
           f2 px = make_float2(sp[0].v[k], sp[0].v[k + 1]), py = make_float2(sp[1].v[k], sp[1].v[k + 1]),
              pz = make_float2(sp[2].v[k], sp[2].v[k + 1]);
           bool acc_a, acc_b;
