@@ -15,6 +15,11 @@ independent replica of that workload (seed + rank): the path has no multi-GPU ex
 scope ("replicas only"), so scaling is weak and there is no collective
 on the data path.
 
+After the headline's timed region the default run (c4, N = 1) also times the other configs and the size sweep of the paper's
+Fig. 2 for about a second each (`workloads`), repeats the timed region twice more (`repeats`) and times the same sweeps with a
+measurement after every one (`with_per_sweep_measurement`); `roofline.cycles_per_launch` / `updates_per_clock` are the
+clock-independent figures ("report for every timed config").
+
 Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle instead (the tier's
 reference arm): single-threaded, on a bounded sample of the same workload.
 """
